@@ -1,0 +1,534 @@
+/*
+ * top_oracle.c -- plain, slow, obviously-correct CPU oracle of the CADMM sweep of
+ * TOP (arXiv 2507.10290).  TEST INFRASTRUCTURE ONLY: nothing in the product path
+ * (paper_2507_10290_b200/, the C ABI in include/top.h) includes, links or calls
+ * this file; only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may.  It shares no code, header, table or constant
+ * generator with the CUDA path.
+ *
+ * What it computes: Algorithm 1 of the paper, closed-form
+ * branch, one sweep k -> k+1 written in the paper's order and notation, raw
+ * monomial basis in physical time, global frame (Eq. 18):
+ *
+ *   c_i   <- [2Q + rho(M'M + Ao'Ao + sum Av'Av)]^-1 rho[M'(z~-u) + Ao'(b-s-v) + sum Av'(phi-w)]
+ *                                                   (Eq. 20a; rho on the RHS: reading A3)
+ *   phi,w <- projection onto the ball and its dual   (Eq. 14/20f/20g)
+ *   z_j   <- average of the two adjacent boundary-derivative vectors (Eq. 6b/20b)
+ *   r_p, r_d                                         (Eq. 21-22; readings A7, A8)
+ *   s     <- max(0, -(Ao c - b + v))                 (Eq. 10/20d)
+ *   u,v   <- scaled dual updates                     (Eq. 6c/20c/20e)
+ *
+ * Readings of the paper taken here:
+ *   A1  consensus carries derivative orders 0..s-1 (n_c = s), so M is 2s x 2s.
+ *   A2  waypoint mode: HARD (default; sigma_i(0)=p_{i-1}, sigma_i(T_i)=p_i imposed as
+ *       equalities inside each segment QP: Pm = H^-1 - K Ew H^-1, c0 = K [p_{i-1};p_i],
+ *       K = H^-1 Ew'(Ew H^-1 Ew')^-1), PINNED_Z (Eq. 20a verbatim, position row of z_j held
+ *       at p_j), FREE (paper's Alg. 1 verbatim, positions averaged too).
+ *   A3  H c = rho * rhs.      A5  u is the scaled dual (never multiplied by rho).
+ *   A7  r_p = || stack_i (M c_i - z~_i) ||_2 over ALL rows; Eq. 21 verbatim (junction gaps) is
+ *       reported beside it.
+ *   A8  r_d = rho || stack_i M(T_i)'(z~_i^{k+1} - z~_i^k) ||_2 in monomial physical-time
+ *       coefficient space; the normalised variant divides component j by T_i^j.
+ *   A9  Init: chord at constant speed; z0_j = (p_j, mean of adjacent chord velocities, 0..);
+ *       duals 0; S = max(0,.) of the chord samples; Phi = projection of the chord velocity.
+ *   A10 sample times t_ij = T_i * j/(Ms+1), j = 1..Ms.
+ *   A11 box corridor: Ao = [E0; -E0] per axis, b = [hi; -lo].
+ *   A15 ball projection scale = min(1, bound/||y||), ||y|| = 0 -> scale 1.
+ *   A18 a single rho for every penalty.   A19 cost c'Qc without 1/2  =>  2Q in H.
+ *
+ * Precision: the sweep is fp64 (real_t = double).  The one-off per-segment operator
+ * (H, its inverse, K, Pm, c0) is formed and inverted in long double with Jacobi
+ * equilibration and then rounded to real_t, so that the oracle's own conditioning
+ * error (cond(H) up to 1e13 in the raw basis) does not consume the
+ * 1e-9 parity budget.  Building with -DORACLE_LONG_DOUBLE makes the sweep long double
+ * too (used by a test that bounds the fp64 oracle's own rounding error).
+ *
+ * Parity pins: tests/test_oracle_pins.py (closed forms, dense KKT, banded solve, SLSQP,
+ * KKT certificate, per-iterate invariants).  Finite-iteration iterates themselves depend on
+ * readings A2/A9: PARITY UNPINNED for those (GPU-vs-oracle only), as DESIGN.md states.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#ifdef ORACLE_LONG_DOUBLE
+typedef long double real_t;
+#define R_SQRT sqrtl
+#else
+typedef double real_t;
+#define R_SQRT sqrt
+#endif
+typedef long double pre_t; /* precision of the one-off operator precompute */
+
+#define NMAX 8   /* n = 2s <= 8 */
+#define MODE_HARD 0
+#define MODE_PINNED_Z 1
+#define MODE_FREE 2
+
+typedef struct {
+    int N, s, n, m, Ms, mode;
+    int has_box, has_vel, has_acc;
+    real_t rho, vmax, amax;
+    real_t *T;      /* [N] */
+    real_t *p;      /* [N+1][m] waypoints */
+    real_t *lo, *hi;/* [N][m] */
+    /* per-segment matrices (Eq. 19 / L231) */
+    real_t *Q;      /* [N][n][n]   */
+    real_t *M;      /* [N][2s][n]  */
+    real_t *E0, *E1, *E2; /* [N][Ms][n] : rows beta_k(t_ij) */
+    real_t *Pm;     /* [N][n][n]   */
+    real_t *c0;     /* [N][n][m]   */
+    /* state */
+    real_t *C;      /* [N][n][m]   */
+    real_t *z, *zprev; /* [N+1][s][m] */
+    real_t *u;      /* [N][2s][m]  */
+    real_t *Sp, *Sn, *Vp, *Vn;   /* [N][Ms][m] slack / dual of the box, + and - side */
+    real_t *PhiV, *WV, *PhiA, *WA; /* [N][Ms][m] */
+    real_t *part;   /* [N][4] residual partial sums */
+    double rp, rd, rd_norm, rp_gap;
+    int64_t iter;
+} oracle_t;
+
+/* [beta_k(t)]_j = j!/(j-k)! t^(j-k) for j >= k, else 0          (Eq. 18 differentiated) */
+static void beta_row(int n, int k, pre_t t, pre_t *row) {
+    for (int j = 0; j < n; ++j) {
+        if (j < k) { row[j] = 0; continue; }
+        pre_t f = 1;
+        for (int q = 0; q < k; ++q) f *= (pre_t)(j - q);
+        pre_t pw = 1;
+        for (int q = 0; q < j - k; ++q) pw *= t;
+        row[j] = f * pw;
+    }
+}
+
+/* Q(T) = int_0^T beta^(s) beta^(s)' dt
+ * Q_jl = j!/(j-s)! l!/(l-s)! T^(j+l-2s+1)/(j+l-2s+1), j,l >= s */
+static void build_Q(int n, int s, pre_t T, pre_t *Q) {
+    for (int j = 0; j < n; ++j)
+        for (int l = 0; l < n; ++l) {
+            if (j < s || l < s) { Q[j * n + l] = 0; continue; }
+            pre_t fj = 1, fl = 1;
+            for (int q = 0; q < s; ++q) { fj *= (pre_t)(j - q); fl *= (pre_t)(l - q); }
+            int e = j + l - 2 * s + 1;
+            pre_t pw = 1;
+            for (int q = 0; q < e; ++q) pw *= T;
+            Q[j * n + l] = fj * fl * pw / (pre_t)e;
+        }
+}
+
+/* inverse of an SPD n x n matrix: Jacobi equilibration + Cholesky, all in pre_t. returns 0 on success */
+static int spd_inverse(int n, const pre_t *A, pre_t *Ainv) {
+    pre_t d[NMAX], L[NMAX * NMAX], X[NMAX * NMAX];
+    for (int i = 0; i < n; ++i) {
+        if (!(A[i * n + i] > 0)) return -1;
+        d[i] = 1 / sqrtl(A[i * n + i]);
+    }
+    memset(L, 0, sizeof L);
+    for (int i = 0; i < n; ++i)
+        for (int j = 0; j <= i; ++j) {
+            pre_t acc = A[i * n + j] * d[i] * d[j];
+            for (int k = 0; k < j; ++k) acc -= L[i * n + k] * L[j * n + k];
+            if (i == j) { if (!(acc > 0)) return -1; L[i * n + i] = sqrtl(acc); }
+            else L[i * n + j] = acc / L[j * n + j];
+        }
+    /* solve (L L') X = I column by column */
+    for (int c = 0; c < n; ++c) {
+        pre_t y[NMAX];
+        for (int i = 0; i < n; ++i) {
+            pre_t acc = (i == c) ? 1 : 0;
+            for (int k = 0; k < i; ++k) acc -= L[i * n + k] * y[k];
+            y[i] = acc / L[i * n + i];
+        }
+        for (int i = n - 1; i >= 0; --i) {
+            pre_t acc = y[i];
+            for (int k = i + 1; k < n; ++k) acc -= L[k * n + i] * X[k * n + c];
+            X[i * n + c] = acc / L[i * n + i];
+        }
+    }
+    for (int i = 0; i < n; ++i)
+        for (int j = 0; j < n; ++j) Ainv[i * n + j] = X[i * n + j] * d[i] * d[j];
+    return 0;
+}
+
+/* ------------------------------------------------------------------ create */
+
+#define ALLOC(ptr, count) do { (ptr) = (real_t *)calloc((size_t)(count) > 0 ? (size_t)(count) : 1, sizeof(real_t)); \
+                               if (!(ptr)) { oracle_destroy(o); return NULL; } } while (0)
+
+void oracle_destroy(oracle_t *o) {
+    if (!o) return;
+    free(o->T); free(o->p); free(o->lo); free(o->hi);
+    free(o->Q); free(o->M); free(o->E0); free(o->E1); free(o->E2); free(o->Pm); free(o->c0);
+    free(o->C); free(o->z); free(o->zprev); free(o->u);
+    free(o->Sp); free(o->Sn); free(o->Vp); free(o->Vn);
+    free(o->PhiV); free(o->WV); free(o->PhiA); free(o->WA); free(o->part);
+    free(o);
+}
+
+/* project the m-vector y onto ||.|| <= bound (Eq. 14 / 20f; reading A15) */
+static void proj_ball(int m, const real_t *y, real_t bound, real_t *phi) {
+    real_t n2 = 0;
+    for (int d = 0; d < m; ++d) n2 += y[d] * y[d];
+    real_t scale = 1;
+    if (n2 > bound * bound) scale = bound / R_SQRT(n2);
+    for (int d = 0; d < m; ++d) phi[d] = scale * y[d];
+}
+
+/* per-segment operator Pm, c0 (reading A2) in long double, rounded to real_t */
+static int build_operator(oracle_t *o, int i) {
+    const int n = o->n, s = o->s, Ms = o->Ms, m = o->m;
+    const pre_t T = (pre_t)o->T[i], rho = (pre_t)o->rho;
+    pre_t Q[NMAX * NMAX], H[NMAX * NMAX], Hinv[NMAX * NMAX], row[NMAX];
+    build_Q(n, s, T, Q);
+    for (int a = 0; a < n * n; ++a) { o->Q[(size_t)i * n * n + a] = (real_t)Q[a]; H[a] = 2 * Q[a]; }
+    /* M(T): rows beta_0(0)..beta_{s-1}(0), beta_0(T)..beta_{s-1}(T) */
+    for (int r = 0; r < 2 * s; ++r) {
+        beta_row(n, r % s, r < s ? (pre_t)0 : T, row);
+        for (int j = 0; j < n; ++j) o->M[((size_t)i * 2 * s + r) * n + j] = (real_t)row[j];
+        for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) H[a * n + b] += rho * row[a] * row[b];
+    }
+    /* sample rows (A10) and their Gram terms: 2 E0'E0 (two box sides, A11), E1'E1, E2'E2 */
+    for (int j = 0; j < Ms; ++j) {
+        pre_t t = T * (pre_t)(j + 1) / (pre_t)(Ms + 1);
+        for (int k = 0; k < 3; ++k) {
+            real_t *E = k == 0 ? o->E0 : (k == 1 ? o->E1 : o->E2);
+            int on = k == 0 ? o->has_box : (k == 1 ? o->has_vel : o->has_acc);
+            pre_t w = k == 0 ? 2 : 1;
+            beta_row(n, k, t, row);
+            for (int a = 0; a < n; ++a) E[((size_t)i * Ms + j) * n + a] = (real_t)row[a];
+            if (!on) continue;
+            for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) H[a * n + b] += rho * w * row[a] * row[b];
+        }
+    }
+    if (spd_inverse(n, H, Hinv)) return -1;
+    pre_t Pm[NMAX * NMAX], c0[NMAX * 3];
+    memset(c0, 0, sizeof c0);
+    if (o->mode == MODE_HARD) {
+        /* Ew = [beta_0(0); beta_0(T)],  K = Hinv Ew'(Ew Hinv Ew')^-1,  Pm = Hinv - K Ew Hinv,  c0 = K [p_{i-1}; p_i] */
+        pre_t Ew[2 * NMAX], HE[NMAX * 2], S[4], Si[4], K[NMAX * 2];
+        beta_row(n, 0, 0, Ew); beta_row(n, 0, T, Ew + n);
+        for (int a = 0; a < n; ++a) for (int c = 0; c < 2; ++c) {
+            pre_t acc = 0; for (int b = 0; b < n; ++b) acc += Hinv[a * n + b] * Ew[c * n + b];
+            HE[a * 2 + c] = acc;
+        }
+        for (int r = 0; r < 2; ++r) for (int c = 0; c < 2; ++c) {
+            pre_t acc = 0; for (int b = 0; b < n; ++b) acc += Ew[r * n + b] * HE[b * 2 + c];
+            S[r * 2 + c] = acc;
+        }
+        pre_t det = S[0] * S[3] - S[1] * S[2];
+        if (!(det > 0)) return -1;
+        Si[0] = S[3] / det; Si[1] = -S[1] / det; Si[2] = -S[2] / det; Si[3] = S[0] / det;
+        for (int a = 0; a < n; ++a) for (int c = 0; c < 2; ++c)
+            K[a * 2 + c] = HE[a * 2 + 0] * Si[0 * 2 + c] + HE[a * 2 + 1] * Si[1 * 2 + c];
+        for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b)
+            Pm[a * n + b] = Hinv[a * n + b] - (K[a * 2 + 0] * HE[b * 2 + 0] + K[a * 2 + 1] * HE[b * 2 + 1]);
+        for (int a = 0; a < n; ++a) for (int d = 0; d < m; ++d)
+            c0[a * 3 + d] = K[a * 2 + 0] * (pre_t)o->p[(size_t)i * m + d] + K[a * 2 + 1] * (pre_t)o->p[(size_t)(i + 1) * m + d];
+    } else {
+        memcpy(Pm, Hinv, sizeof(pre_t) * n * n);
+    }
+    for (int a = 0; a < n * n; ++a) o->Pm[(size_t)i * n * n + a] = (real_t)Pm[a];
+    for (int a = 0; a < n; ++a) for (int d = 0; d < m; ++d) o->c0[((size_t)i * n + a) * m + d] = (real_t)c0[a * 3 + d];
+    return 0;
+}
+
+/*
+ * All inputs are host fp64.  waypoints [N+1][m]; durations [N]; start/end_derivs [s-1][m] (orders
+ * 1..s-1) or NULL = rest; box_lo/hi [N][m] or NULL; vmax/amax <= 0 => off; Ms = samples per segment.
+ */
+oracle_t *oracle_create(int N, int s, int m, const double *waypoints, const double *durations,
+                        const double *start_derivs, const double *end_derivs, int Ms,
+                        const double *box_lo, const double *box_hi, double vmax, double amax,
+                        double rho, int mode) {
+    if (N < 1 || (s != 3 && s != 4) || m < 1 || m > 3 || Ms < 0 || !(rho > 0) || mode < 0 || mode > 2) return NULL;
+    oracle_t *o = (oracle_t *)calloc(1, sizeof(oracle_t));
+    if (!o) return NULL;
+    const int n = 2 * s;
+    o->N = N; o->s = s; o->n = n; o->m = m; o->Ms = Ms; o->mode = mode;
+    o->rho = (real_t)rho; o->vmax = (real_t)vmax; o->amax = (real_t)amax;
+    o->has_box = (Ms > 0 && box_lo && box_hi);
+    o->has_vel = (Ms > 0 && vmax > 0);
+    o->has_acc = (Ms > 0 && amax > 0);
+    ALLOC(o->T, N); ALLOC(o->p, (N + 1) * m); ALLOC(o->lo, N * m); ALLOC(o->hi, N * m);
+    ALLOC(o->Q, (size_t)N * n * n); ALLOC(o->M, (size_t)N * 2 * s * n);
+    ALLOC(o->E0, (size_t)N * Ms * n); ALLOC(o->E1, (size_t)N * Ms * n); ALLOC(o->E2, (size_t)N * Ms * n);
+    ALLOC(o->Pm, (size_t)N * n * n); ALLOC(o->c0, (size_t)N * n * m);
+    ALLOC(o->C, (size_t)N * n * m); ALLOC(o->z, (size_t)(N + 1) * s * m); ALLOC(o->zprev, (size_t)(N + 1) * s * m);
+    ALLOC(o->u, (size_t)N * 2 * s * m);
+    ALLOC(o->Sp, (size_t)N * Ms * m); ALLOC(o->Sn, (size_t)N * Ms * m);
+    ALLOC(o->Vp, (size_t)N * Ms * m); ALLOC(o->Vn, (size_t)N * Ms * m);
+    ALLOC(o->PhiV, (size_t)N * Ms * m); ALLOC(o->WV, (size_t)N * Ms * m);
+    ALLOC(o->PhiA, (size_t)N * Ms * m); ALLOC(o->WA, (size_t)N * Ms * m);
+    ALLOC(o->part, (size_t)N * 4);
+    for (int i = 0; i < N; ++i) { if (!(durations[i] > 0)) { oracle_destroy(o); return NULL; } o->T[i] = (real_t)durations[i]; }
+    for (int a = 0; a < (N + 1) * m; ++a) o->p[a] = (real_t)waypoints[a];
+    if (o->has_box) for (int a = 0; a < N * m; ++a) { o->lo[a] = (real_t)box_lo[a]; o->hi[a] = (real_t)box_hi[a]; }
+    for (int i = 0; i < N; ++i) if (build_operator(o, i)) { oracle_destroy(o); return NULL; }
+
+    /* ---- Init (Alg. 1 line 1; reading A9) ---- */
+    for (int i = 0; i < N; ++i) {          /* C0 = chord at constant speed */
+        for (int d = 0; d < m; ++d) {
+            o->C[((size_t)i * n + 0) * m + d] = o->p[(size_t)i * m + d];
+            o->C[((size_t)i * n + 1) * m + d] = (o->p[(size_t)(i + 1) * m + d] - o->p[(size_t)i * m + d]) / o->T[i];
+        }
+    }
+    for (int j = 0; j <= N; ++j)           /* z0_j: position p_j, mean chord velocity, higher orders 0 */
+        for (int d = 0; d < m; ++d) {
+            o->z[((size_t)j * s + 0) * m + d] = o->p[(size_t)j * m + d];
+            if (j >= 1 && j <= N - 1)
+                o->z[((size_t)j * s + 1) * m + d] = (real_t)0.5 * (o->C[((size_t)(j - 1) * n + 1) * m + d] + o->C[((size_t)j * n + 1) * m + d]);
+        }
+    for (int k = 1; k < s; ++k)            /* z_0, z_N = given end states (Eq. 2c); rest if NULL */
+        for (int d = 0; d < m; ++d) {
+            o->z[((size_t)0 * s + k) * m + d] = start_derivs ? (real_t)start_derivs[(k - 1) * m + d] : 0;
+            o->z[((size_t)N * s + k) * m + d] = end_derivs ? (real_t)end_derivs[(k - 1) * m + d] : 0;
+        }
+    memcpy(o->zprev, o->z, sizeof(real_t) * (size_t)(N + 1) * s * m);
+    for (int i = 0; i < N; ++i)            /* slacks / phi of the chord samples; all duals 0 */
+        for (int j = 0; j < Ms; ++j) {
+            real_t P[3] = {0, 0, 0}, V[3] = {0, 0, 0}, A[3] = {0, 0, 0};
+            for (int d = 0; d < m; ++d)
+                for (int a = 0; a < n; ++a) {
+                    real_t c = o->C[((size_t)i * n + a) * m + d];
+                    P[d] += o->E0[((size_t)i * Ms + j) * n + a] * c;
+                    V[d] += o->E1[((size_t)i * Ms + j) * n + a] * c;
+                    A[d] += o->E2[((size_t)i * Ms + j) * n + a] * c;
+                }
+            size_t q = ((size_t)i * Ms + j) * m;
+            if (o->has_box) for (int d = 0; d < m; ++d) {
+                real_t a = o->hi[(size_t)i * m + d] - P[d], b = P[d] - o->lo[(size_t)i * m + d];
+                o->Sp[q + d] = a > 0 ? a : 0; o->Sn[q + d] = b > 0 ? b : 0;
+            }
+            if (o->has_vel) proj_ball(m, V, o->vmax, o->PhiV + q);
+            if (o->has_acc) proj_ball(m, A, o->amax, o->PhiA + q);
+        }
+    o->iter = 0; o->rp = o->rd = o->rd_norm = o->rp_gap = NAN;
+    return o;
+}
+
+/* ------------------------------------------------------------------ one sweep (Alg. 1 lines 3-13) */
+
+static void sweep_once(oracle_t *o) {
+    const int N = o->N, s = o->s, n = o->n, m = o->m, Ms = o->Ms;
+    const real_t rho = o->rho;
+
+    /* ClosedFormSolve: Eq. 20a with rho on the right-hand side (A3) */
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        real_t R[NMAX * 3];
+        for (int a = 0; a < n * m; ++a) R[a] = 0;
+        const real_t *M = o->M + (size_t)i * 2 * s * n;
+        for (int r = 0; r < 2 * s; ++r) {          /* M'(z~_i - u_i), z~_i = (z_{i-1}; z_i) */
+            const real_t *zr = o->z + ((size_t)(i + (r >= s)) * s + (r % s)) * m;
+            const real_t *ur = o->u + ((size_t)i * 2 * s + r) * m;
+            for (int d = 0; d < m; ++d) {
+                real_t g = zr[d] - ur[d];
+                for (int a = 0; a < n; ++a) R[a * m + d] += M[r * n + a] * g;
+            }
+        }
+        for (int j = 0; j < Ms; ++j) {
+            size_t q = ((size_t)i * Ms + j) * m;
+            const real_t *e0 = o->E0 + ((size_t)i * Ms + j) * n;
+            const real_t *e1 = o->E1 + ((size_t)i * Ms + j) * n;
+            const real_t *e2 = o->E2 + ((size_t)i * Ms + j) * n;
+            for (int d = 0; d < m; ++d) {
+                if (o->has_box) {                  /* Ao'(b - s - v) with Ao = [E0; -E0], b = [hi; -lo] */
+                    real_t gp = o->hi[(size_t)i * m + d] - o->Sp[q + d] - o->Vp[q + d];
+                    real_t gn = -o->lo[(size_t)i * m + d] - o->Sn[q + d] - o->Vn[q + d];
+                    for (int a = 0; a < n; ++a) R[a * m + d] += e0[a] * gp + (-e0[a]) * gn;
+                }
+                if (o->has_vel) { real_t g = o->PhiV[q + d] - o->WV[q + d]; for (int a = 0; a < n; ++a) R[a * m + d] += e1[a] * g; }
+                if (o->has_acc) { real_t g = o->PhiA[q + d] - o->WA[q + d]; for (int a = 0; a < n; ++a) R[a * m + d] += e2[a] * g; }
+            }
+        }
+        const real_t *Pm = o->Pm + (size_t)i * n * n;
+        for (int a = 0; a < n; ++a)
+            for (int d = 0; d < m; ++d) {
+                real_t acc = 0;
+                for (int b = 0; b < n; ++b) acc += Pm[a * n + b] * (rho * R[b * m + d]);
+                o->C[((size_t)i * n + a) * m + d] = acc + o->c0[((size_t)i * n + a) * m + d];
+            }
+    }
+
+    /* phi, w: Eq. 20f, 20g */
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i)
+        for (int j = 0; j < Ms; ++j) {
+            size_t q = ((size_t)i * Ms + j) * m;
+            for (int kind = 1; kind <= 2; ++kind) {
+                if (kind == 1 ? !o->has_vel : !o->has_acc) continue;
+                const real_t *e = (kind == 1 ? o->E1 : o->E2) + ((size_t)i * Ms + j) * n;
+                real_t *Phi = (kind == 1 ? o->PhiV : o->PhiA) + q, *W = (kind == 1 ? o->WV : o->WA) + q;
+                real_t Y[3];
+                for (int d = 0; d < m; ++d) {
+                    real_t acc = 0;
+                    for (int a = 0; a < n; ++a) acc += e[a] * o->C[((size_t)i * n + a) * m + d];
+                    Y[d] = acc + W[d];
+                }
+                proj_ball(m, Y, kind == 1 ? o->vmax : o->amax, Phi);
+                for (int d = 0; d < m; ++d) W[d] = Y[d] - Phi[d];
+            }
+        }
+
+    /* UpdateConsensus: Eq. 6b / 20b. z_0, z_N fixed (L141). */
+    memcpy(o->zprev, o->z, sizeof(real_t) * (size_t)(N + 1) * s * m);
+#pragma omp parallel for schedule(static)
+    for (int j = 1; j <= N - 1; ++j) {
+        const real_t *Ml = o->M + (size_t)(j - 1) * 2 * s * n, *Mr = o->M + (size_t)j * 2 * s * n;
+        for (int k = 0; k < s; ++k) {
+            if (k == 0 && o->mode == MODE_PINNED_Z) continue;   /* position row held at p_j */
+            for (int d = 0; d < m; ++d) {
+                real_t bl = 0, br = 0;
+                for (int a = 0; a < n; ++a) {
+                    bl += Ml[(s + k) * n + a] * o->C[((size_t)(j - 1) * n + a) * m + d];
+                    br += Mr[k * n + a] * o->C[((size_t)j * n + a) * m + d];
+                }
+                o->z[((size_t)j * s + k) * m + d] = (real_t)0.5 * (bl + br);
+            }
+        }
+    }
+
+    /* UpdateResidual (Eq. 21, 22; A7, A8), ProjectNonNeg (20d), UpdateDual (20c, 20e) */
+#pragma omp parallel for schedule(static)
+    for (int i = 0; i < N; ++i) {
+        const real_t *M = o->M + (size_t)i * 2 * s * n;
+        real_t rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
+        real_t dz[NMAX * 3];
+        for (int r = 0; r < 2 * s; ++r) {
+            size_t zi = ((size_t)(i + (r >= s)) * s + (r % s)) * m;
+            for (int d = 0; d < m; ++d) {
+                real_t b = 0;
+                for (int a = 0; a < n; ++a) b += M[r * n + a] * o->C[((size_t)i * n + a) * m + d];
+                real_t res = b - o->z[zi + d];
+                rp2 += res * res;
+                o->u[((size_t)i * 2 * s + r) * m + d] += res;           /* Eq. 20c */
+                dz[r * m + d] = o->z[zi + d] - o->zprev[zi + d];
+                if (r >= s && i < N - 1) {                              /* Eq. 21 verbatim: junction gap */
+                    real_t br = 0;
+                    const real_t *Mn = o->M + (size_t)(i + 1) * 2 * s * n;
+                    for (int a = 0; a < n; ++a) br += Mn[(r - s) * n + a] * o->C[((size_t)(i + 1) * n + a) * m + d];
+                    gap2 += (b - br) * (b - br);
+                }
+            }
+        }
+        real_t Tp = 1;
+        for (int a = 0; a < n; ++a) {                                   /* rho M'(dz~): Eq. 22 */
+            for (int d = 0; d < m; ++d) {
+                real_t acc = 0;
+                for (int r = 0; r < 2 * s; ++r) acc += M[r * n + a] * dz[r * m + d];
+                acc *= rho;
+                rd2 += acc * acc;
+                rdn2 += (acc / Tp) * (acc / Tp);
+            }
+            Tp *= o->T[i];
+        }
+        o->part[(size_t)i * 4 + 0] = rp2; o->part[(size_t)i * 4 + 1] = rd2;
+        o->part[(size_t)i * 4 + 2] = rdn2; o->part[(size_t)i * 4 + 3] = gap2;
+
+        if (o->has_box)
+            for (int j = 0; j < Ms; ++j) {
+                const real_t *e0 = o->E0 + ((size_t)i * Ms + j) * n;
+                size_t q = ((size_t)i * Ms + j) * m;
+                for (int d = 0; d < m; ++d) {
+                    real_t P = 0;
+                    for (int a = 0; a < n; ++a) P += e0[a] * o->C[((size_t)i * n + a) * m + d];
+                    real_t hi = o->hi[(size_t)i * m + d], lo = o->lo[(size_t)i * m + d];
+                    real_t sp = -(P - hi + o->Vp[q + d]);            /* Eq. 20d, + side: A=E0,  b=hi  */
+                    real_t sn = -(-P + lo + o->Vn[q + d]);           /*          - side: A=-E0, b=-lo */
+                    o->Sp[q + d] = sp > 0 ? sp : 0;
+                    o->Sn[q + d] = sn > 0 ? sn : 0;
+                    o->Vp[q + d] += P + o->Sp[q + d] - hi;           /* Eq. 20e */
+                    o->Vn[q + d] += -P + o->Sn[q + d] + lo;
+                }
+            }
+    }
+    real_t a0 = 0, a1 = 0, a2 = 0, a3 = 0;       /* fixed-order (serial) reduction */
+    for (int i = 0; i < N; ++i) { a0 += o->part[(size_t)i * 4]; a1 += o->part[(size_t)i * 4 + 1];
+                                  a2 += o->part[(size_t)i * 4 + 2]; a3 += o->part[(size_t)i * 4 + 3]; }
+    o->rp = (double)R_SQRT(a0); o->rd = (double)R_SQRT(a1); o->rd_norm = (double)R_SQRT(a2); o->rp_gap = (double)R_SQRT(a3);
+    o->iter += 1;
+}
+
+/* run k sweeps on `threads` OpenMP threads (<=0: leave the runtime default) */
+void oracle_sweep(oracle_t *o, int64_t k, int threads) {
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#else
+    (void)threads;
+#endif
+    for (int64_t it = 0; it < k; ++it) sweep_once(o);
+}
+
+int oracle_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+/* sweep until rp < eps and rd (or its normalised variant) < eps, or max_iter; returns sweeps done in this call */
+int64_t oracle_solve(oracle_t *o, double eps, int64_t max_iter, int use_rd_norm, int threads) {
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#else
+    (void)threads;
+#endif
+    int64_t it = 0;
+    while (it < max_iter) {
+        sweep_once(o); ++it;
+        double rd = use_rd_norm ? o->rd_norm : o->rd;
+        if (o->rp < eps && rd < eps) break;
+    }
+    return it;
+}
+
+/* out[0..3] = r_p (A7), r_d (Eq. 22, A8), r_d normalised, r_p of Eq. 21 verbatim (junction gaps) */
+void oracle_residuals(const oracle_t *o, double *out) {
+    out[0] = o->rp; out[1] = o->rd; out[2] = o->rd_norm; out[3] = o->rp_gap;
+}
+
+/* J = sum_i tr(C_i' Q(T_i) C_i)   (Eq. 2a with W = I, A19) */
+double oracle_objective(const oracle_t *o) {
+    real_t J = 0;
+    for (int i = 0; i < o->N; ++i)
+        for (int d = 0; d < o->m; ++d)
+            for (int a = 0; a < o->n; ++a)
+                for (int b = 0; b < o->n; ++b)
+                    J += o->C[((size_t)i * o->n + a) * o->m + d] * o->Q[((size_t)i * o->n + a) * o->n + b]
+                       * o->C[((size_t)i * o->n + b) * o->m + d];
+    return (double)J;
+}
+
+int64_t oracle_iter(const oracle_t *o) { return o->iter; }
+
+/* copy a field as doubles. returns the element count, or -1 for an unknown name.
+ * "coeffs" is [N][m][n] (dim-major per segment, the paper's squeezed c_i); every other field is in its
+ * native layout: C [N][n][m], z [N+1][s][m], u [N][2s][m], sample fields [N][Ms][m], Pm [N][n][n] ... */
+int64_t oracle_get(const oracle_t *o, const char *name, double *out) {
+    const int N = o->N, s = o->s, n = o->n, m = o->m, Ms = o->Ms;
+    const real_t *src = NULL; size_t cnt = 0;
+    if (!strcmp(name, "coeffs")) {
+        for (int i = 0; i < N; ++i) for (int d = 0; d < m; ++d) for (int a = 0; a < n; ++a)
+            out[((size_t)i * m + d) * n + a] = (double)o->C[((size_t)i * n + a) * m + d];
+        return (int64_t)N * m * n;
+    }
+#define FIELD(nm, ptr, count) else if (!strcmp(name, nm)) { src = (ptr); cnt = (size_t)(count); }
+    if (0) {}
+    FIELD("C", o->C, (size_t)N * n * m) FIELD("z", o->z, (size_t)(N + 1) * s * m) FIELD("u", o->u, (size_t)N * 2 * s * m)
+    FIELD("s_pos", o->Sp, (size_t)N * Ms * m) FIELD("s_neg", o->Sn, (size_t)N * Ms * m)
+    FIELD("v_pos", o->Vp, (size_t)N * Ms * m) FIELD("v_neg", o->Vn, (size_t)N * Ms * m)
+    FIELD("phi_v", o->PhiV, (size_t)N * Ms * m) FIELD("w_v", o->WV, (size_t)N * Ms * m)
+    FIELD("phi_a", o->PhiA, (size_t)N * Ms * m) FIELD("w_a", o->WA, (size_t)N * Ms * m)
+    FIELD("Pm", o->Pm, (size_t)N * n * n) FIELD("c0", o->c0, (size_t)N * n * m) FIELD("Q", o->Q, (size_t)N * n * n)
+    FIELD("M", o->M, (size_t)N * 2 * s * n) FIELD("E0", o->E0, (size_t)N * Ms * n) FIELD("E1", o->E1, (size_t)N * Ms * n)
+    FIELD("E2", o->E2, (size_t)N * Ms * n)
+    else return -1;
+#undef FIELD
+    for (size_t a = 0; a < cnt; ++a) out[a] = (double)src[a];
+    return (int64_t)cnt;
+}
