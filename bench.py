@@ -1,0 +1,289 @@
+#!/usr/bin/env python
+"""bench.py -- CADMM segment-iterations/s of the fused sweep on B200 (BASELINE.json's metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload cfg4|cfg2|cfg3|cfg5]
+
+One "step" = `--sweeps` CADMM sweeps (all five parts of the hot path: x-update, projections, z-update, dual
+update, residual reduction) over one batch of seeded synthetic trajectories = one top_iterate call.
+Default workload: BASELINE.json configs[3] (N=10,000 segments, minimum snap, box + velocity + acceleration
+sets, fp64) -- the N >= 10,000 case north_star quotes the roofline fraction on.  Prints ONE JSON line.
+
+The oracle (oracle/) is used only for the `cpu_baseline` leg and for `--impl reference`.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2507_10290_b200 import workloads as W  # noqa: E402
+
+METRIC = "cadmm_segment_iterations_per_s"
+UNIT = "segment-iterations/s"
+
+# Algorithmic FLOPs per segment-sweep (FMA = 2), counted from the kernel's arithmetic in DESIGN.md "Roofline":
+# rhs assembly + operator apply + evaluation + projections + consensus/dual updates (residuals excluded: they
+# are computed on the last sweep of a launch only).
+FLOPS_PER_SEG_SWEEP = {"cfg4": 4260.0, "cfg2": 3330.0, "cfg5": 3330.0, "cfg3": 740.0, "cfg1": 740.0}
+
+
+def make_workload(name: str, rank: int = 0):
+    if name == "cfg4":
+        return W.config4(seed=1004 + rank)
+    if name == "cfg2":
+        return W.config2(seed=1002 + rank)
+    if name == "cfg3":
+        return W.config3(seed=1003 + rank)
+    if name == "cfg3f32":
+        return W.config3(seed=1003 + rank, dtype="f32")
+    if name == "cfg5":
+        return W.config5(seed0=5000 + 1000 * rank)
+    if name == "cfg1":
+        return W.config1(seed=1001 + rank)
+    raise SystemExit("unknown workload " + name)
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (profiling recipe's clocks line)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows, self.proc, self.thread = [], None, None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def oracle_rate(w, seconds: float, threads: int):
+    """Oracle (as it stands) on the host cores: a bounded number of sweeps of trajectory 0 of the workload."""
+    from oracle.top_oracle import Oracle
+    o = Oracle(w.waypoints[0], w.durations[0], w.s, w.rho, samples=w.samples,
+               box_lo=None if w.box_lo is None else w.box_lo[0], box_hi=None if w.box_hi is None else w.box_hi[0],
+               vmax=w.vmax, amax=w.amax)
+    if threads <= 0:
+        threads = min(o.max_threads(), os.cpu_count() or 1)
+    t0 = time.perf_counter(); o.sweep(2, threads); probe = (time.perf_counter() - t0) / 2
+    sweeps = int(max(3, min(200000, seconds / max(probe, 1e-9))))
+    t0 = time.perf_counter(); o.sweep(sweeps, threads); dt = time.perf_counter() - t0
+    return {"value": w.N * sweeps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
+            "sample": "%d sweeps of trajectory 0 (N=%d) of %s, %.1f s, gcc -O2 -fopenmp" % (sweeps, w.N, w.name, dt)}, sweeps, dt
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    w = make_workload(args.workload)
+    per_step = max(1.0, min(20.0, 120.0 / max(1, args.steps + args.warmup)))
+    for _ in range(args.warmup):
+        oracle_rate(w, per_step / 4, args.oracle_threads)
+    vals, tot_units, tot_t = [], 0.0, 0.0
+    info = None
+    for _ in range(args.steps):
+        info, sweeps, dt = oracle_rate(w, per_step, args.oracle_threads)
+        tot_units += w.N * sweeps; tot_t += dt
+    value = tot_units / tot_t
+    info["value"] = value
+    info["sample"] = "per step: ~%.0f s of oracle sweeps on trajectory 0 of %s" % (per_step, w.name)
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+                      "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps,
+                      "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                      "data": "synthetic", "config": {"workload": w.name, "note": "CPU oracle, bounded sample"},
+                      "cpu_baseline": info,
+                      "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="cfg4")
+    ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (0 = the config's count, or 2000)")
+    ap.add_argument("--sync", default="auto")
+    ap.add_argument("--segs-per-cta", type=int, default=0)
+    ap.add_argument("--oracle-seconds", type=float, default=12.0)
+    ap.add_argument("--oracle-threads", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip time-to-eps and the e2e leg")
+    args = ap.parse_args()
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from paper_2507_10290_b200 import build as top_build
+    from paper_2507_10290_b200 import top
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the CADMM sweep has no CPU path")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    if local_rank == 0:
+        top_build.build()
+    if world > 1:
+        dist.barrier()
+
+    w = make_workload(args.workload, rank)      # weak scaling: every rank sweeps its own trajectories, no collective
+    sweeps = args.sweeps or w.sweeps or 2000
+    stream = torch.cuda.current_stream()
+    sol = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync,
+                            segs_per_cta=args.segs_per_cta)
+    info = sol.launch_info()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        sol.iterate(sweeps)
+    barrier()
+    launches0 = sol.launch_info()["launches"]
+    sampler = ClockSampler(local_rank)
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t_wall0 = time.perf_counter()
+    for a, b in ev:
+        flush.fill_(1)                    # L2 flush between timed iterations (not inside the event pair)
+        a.record(stream)
+        sol.iterate(sweeps)
+        b.record(stream)
+    barrier()
+    t_wall = time.perf_counter() - t_wall0
+    clocks = sampler.stop()
+    ms = [a.elapsed_time(b) for a, b in ev]
+    total_ms = float(sum(ms))
+    gpu_launches = sol.launch_info()["launches"] - launches0
+    units = float(w.batch * w.N) * sweeps * args.steps
+    if world > 1:
+        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+        u = torch.tensor([units], device="cuda", dtype=torch.float64)
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        units = float(u.item())
+    value = units / (total_ms * 1e-3)
+    res = sol.residuals()
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": max(3, args.warmup), "ms_per_step": total_ms / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": w.dtype, "data": "synthetic",
+           "config": {"workload": w.name, "baseline_config_index": {"cfg1": 0, "cfg2": 1, "cfg3": 2, "cfg4": 3, "cfg5": 4}.get(args.workload),
+                      "segments": w.N, "batch": w.batch, "s": w.s, "rho": w.rho, "sweeps_per_step": sweeps,
+                      "l2": "flushed between steps (256 MiB write); state is on-chip during a step",
+                      "sync": args.sync, **info, "parallelism": "replicas x%d (no collective)" % world},
+           "clocks": clocks, "gpu_launches": int(gpu_launches), "wall_s": t_wall,
+           "us_per_sweep": 1e3 * total_ms / args.steps / sweeps,
+           "residuals_after": {k: float(v[0]) for k, v in res.items()}}
+
+    if rank == 0:
+        # ---- roofline of the dominant kernel (cadmm_sweeps_kernel): plain FP64/FP32 ALU bound, state on chip
+        fl = FLOPS_PER_SEG_SWEEP.get(args.workload.replace("f32", ""), None)
+        dt_name = "f64" if w.dtype == "f64" else "f32"
+        peak = top.fma_peak(dt_name, reps=5, device=local_rank, stream=stream.cuda_stream)
+        if fl is not None:
+            waves = info["waves"]
+            per_launch_flops = fl * w.batch * w.N * sweeps / waves
+            per_launch_s = (sum(ms) / args.steps) * 1e-3 / waves
+            ach = per_launch_flops / per_launch_s
+            out["roofline"] = {"bound": "alu", "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
+                               "frac": ach / peak, "traffic": None,
+                               "peak_source": "measured in this run: top_fma_peak (%s FMA loop, all SMs)" % dt_name,
+                               "flops_per_segment_sweep": fl}
+        peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+        if os.path.exists(peaks_path):
+            out["measured_peaks"] = {k: v for k, v in json.load(open(peaks_path)).items() if k in ("hbm_gbs", "sm_max_mhz")}
+
+        if not args.no_extras:
+            # ---- e2e: the user's calls with HOST buffers: top_create (H2D) + top_iterate + top_get_coeffs (D2H)
+            torch.cuda.synchronize()
+            e2e_t, nrep = 0.0, 3
+            h2d = d2h = 0
+            for _ in range(nrep):
+                t0 = time.perf_counter()
+                s2 = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync,
+                                       segs_per_cta=args.segs_per_cta)
+                s2.iterate(sweeps)
+                c = s2.coeffs()
+                e2e_t += time.perf_counter() - t0
+                h2d = w.waypoints.nbytes + w.durations.nbytes + (0 if w.box_lo is None else w.box_lo.nbytes + w.box_hi.nbytes)
+                d2h = c.nbytes
+                s2.close()
+            out["e2e"] = {"value": float(w.batch * w.N) * sweeps * nrep / e2e_t, "unit": UNIT,
+                          "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                          "what": "top_create(host arrays: validate, fp80 operator precompute, upload) + top_iterate(%d) + top_get_coeffs(host), wall clock" % sweeps}
+            # ---- time-to-eps (BASELINE.json's second figure)
+            s3 = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync, check_every=64,
+                                   max_iter=200000, segs_per_cta=args.segs_per_cta)
+            eps = w.eps or 1e-4
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            ok, iters = s3.solve(eps)
+            torch.cuda.synchronize(); dt = time.perf_counter() - t0
+            r3 = s3.residuals()
+            out["time_to_eps"] = {"eps": eps, "converged": bool(ok), "sweeps": int(iters.max()), "seconds": dt,
+                                  "r_p": float(r3["r_p"].max()), "r_d": float(r3["r_d"].max()),
+                                  "note": "cap reached (max_iter=200000)" if not ok else "ok"}
+            s3.close()
+        if not args.no_cpu_baseline and world == 1:
+            out["cpu_baseline"], _, _ = oracle_rate(w, args.oracle_seconds, args.oracle_threads)
+        print(json.dumps(out))
+    sol.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

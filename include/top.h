@@ -1,0 +1,195 @@
+/*
+ * top.h -- C ABI of the B200-native Consensus-ADMM (CADMM) segment sweep of TOP
+ * (arXiv 2507.10290).  Citations are PAPER.md:L<line> (+ equation) of the paper text.
+ *
+ * What the library computes: Algorithm 1 of the paper, closed-form
+ * branch -- per sweep and per polynomial segment i of a piecewise polynomial trajectory
+ * (Eq. 18; order 2s-1, s=3 jerk / s=4 snap):
+ *     x-update  (Eq. 20a)      c_i  <- closed-form QP solve
+ *     phi, w    (Eq. 14/20f/20g, L186-191, L250-252)  ball projections + their scaled duals
+ *     z-update  (Eq. 6b/20b, L136, L235)      average of adjacent boundary derivatives
+ *     residuals (Eq. 21-22)         r_p, r_d (two global sums per trajectory)
+ *     s-update  (Eq. 10/20d, L166, L244)      slack projection of the box corridor
+ *     u, v      (Eq. 6c/20c/20e, L139, L239-247)  scaled dual updates
+ * Every step runs in CUDA kernels for sm_100a.  There is NO CPU fallback: without a CUDA
+ * device every compute entry point returns TOP_E_CUDA.  The readings of the paper taken
+ * where it is silent or garbled are listed in DESIGN.md ("Readings", A1-A19).
+ *
+ * Conventions
+ *  - All INPUT pointers are HOST pointers to fp64 data and are copied inside top_create
+ *    (the caller may free them as soon as top_create returns).
+ *  - Output buffers are caller-owned.  Where an argument says "host or device" a flag tells
+ *    which; device pointers must belong to the solver's device.
+ *  - The handle owns all other host and device memory; top_destroy frees it.
+ *  - Every call returns a top_status; nothing throws or aborts across the ABI.  A negative
+ *    status leaves a message in top_last_error().  A handle is not thread-safe.
+ *  - Kernels are enqueued on top_options.cuda_stream (a cudaStream_t passed as void*;
+ *    NULL = the legacy default stream).  top_iterate is asynchronous with respect to the
+ *    host; every call that returns data to the host synchronises that stream first.
+ */
+#ifndef TOP_H
+#define TOP_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define TOP_API __attribute__((visibility("default")))
+#else
+#define TOP_API
+#endif
+
+typedef struct top_solver top_solver;
+
+typedef enum {
+    TOP_OK = 0,
+    TOP_NOT_CONVERGED = 1,   /* top_solve hit max_iter; the state is valid */
+    TOP_E_INVALID = -1,      /* bad argument (see top_create)                      */
+    TOP_E_NOMEM = -2,        /* host or device allocation failed                   */
+    TOP_E_CUDA = -3,         /* CUDA runtime error, no device, or barrier time-out */
+    TOP_E_UNSUPPORTED = -4,  /* valid request this build cannot run (size limits)  */
+    TOP_E_NONFINITE = -5     /* a residual became NaN/Inf                          */
+} top_status;
+
+typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
+/* TOP_F64: state, evaluation, projections and the x-update all in fp64.
+ * TOP_F32: state, evaluation and projections in fp32; the 2s x 2s x-update operator is kept
+ *          and applied in fp64 (an all-fp32 operator loses Q against rho*G; R5). */
+
+/* Waypoint handling (reading A2 of DESIGN.md; the paper's Alg. 1 leaves waypoints free). */
+#define TOP_WAYPOINT_HARD     0u  /* sigma_i(0)=p_{i-1}, sigma_i(T_i)=p_i as equalities inside each segment QP (default) */
+#define TOP_WAYPOINT_PINNED_Z 1u  /* Eq. 20a verbatim; the position row of every z_j is held at p_j */
+#define TOP_WAYPOINT_FREE     2u  /* Alg. 1 verbatim: position rows are averaged as well */
+#define TOP_WAYPOINT_MASK     3u
+/* Which dual residual top_solve compares with eps (reading A8). */
+#define TOP_RD_PAPER          0u  /* Eq. 22 in monomial physical-time coefficient space (default) */
+#define TOP_RD_NORMALISED     4u  /* component k divided by T_i^k */
+/* Tolerance scaling (reading A13). */
+#define TOP_EPS_ABSOLUTE      0u  /* ||r|| < eps (default) */
+#define TOP_EPS_N_SCALED      8u  /* ||r|| < N*eps, the paper's rule */
+/* Inter-CTA synchronisation of the persistent kernel (a performance knob; results are identical). */
+#define TOP_SYNC_AUTO         0u
+#define TOP_SYNC_GRID         16u /* one grid-wide barrier per sweep */
+#define TOP_SYNC_NEIGHBOUR    32u /* release/acquire flags with the two neighbouring CTAs only */
+#define TOP_SYNC_MASK         48u
+
+/* The paper's convex sets, specialised as BASELINE.json's configs use them:
+ * an axis-aligned box corridor per segment (K=6 half-spaces, linear set, Eq. 7-10) and Euclidean balls on
+ * velocity and acceleration (quadratic sets, Eq. 11-14), all enforced at `samples` interior sample times
+ * t_ij = T_i*j/(samples+1), j=1..samples (reading A10). */
+typedef struct {
+    int32_t samples;        /* Ms: 0 => no inequality constraints; otherwise must be 8 in this build */
+    const double* box_lo;   /* host [batch][N][dims] or NULL => no box */
+    const double* box_hi;   /* host [batch][N][dims]; lo < hi elementwise */
+    double vmax;            /* > 0: ||sigma'(t_ij)||_2  <= vmax ; <= 0: off */
+    double amax;            /* > 0: ||sigma''(t_ij)||_2 <= amax ; <= 0: off */
+} top_constraints;
+
+typedef struct {
+    uint32_t struct_size;   /* = sizeof(top_options); lets the struct grow */
+    uint32_t flags;         /* OR of TOP_WAYPOINT_*, TOP_RD_*, TOP_EPS_*, TOP_SYNC_* */
+    int32_t check_every;    /* top_solve evaluates the residuals every this many sweeps (default 32) */
+    int32_t device;         /* CUDA device ordinal; -1 = current device */
+    int64_t max_iter;       /* top_solve gives up after this many sweeps (default 1000000) */
+    void* cuda_stream;      /* cudaStream_t; NULL = default stream */
+    int32_t segs_per_cta;   /* segments per thread block, 0 = choose (a tuning knob; multiple of 4) */
+    int32_t reserved;
+} top_options;
+
+/*
+ * top_create -- Init of Alg. 1 (PAPER.md:L270 line 1, L301): validates, precomputes per segment (host,
+ * extended precision) the x-update operator of Eq. 20a from T_i, rho and the enabled constraint sets,
+ * uploads it in segment-major SoA form, and sets iterate 0 (reading A9: chord at constant speed, z0 from
+ * the chord, duals 0, slacks/phi = projections of the chord samples).
+ *   batch        number of independent trajectories (>= 1), each with N segments
+ *   N            segments per trajectory (>= 1);  s in {3,4};  dims in {1,2,3}
+ *   waypoints    host [batch][N+1][dims] metres       (the path P of Alg. 1)
+ *   durations    host [batch][N] seconds, > 0
+ *   start_derivs host [batch][s-1][dims], derivative orders 1..s-1 at t_0, or NULL = rest (Eq. 2c)
+ *   end_derivs   same at t_N
+ *   cons         NULL = unconstrained
+ *   rho          > 0, penalty of Eq. 5; one rho for every penalty (A18)
+ *   opt          NULL = defaults
+ * Errors: TOP_E_INVALID (sizes, non-finite input, T<=0, lo>=hi, rho<=0, samples not in {0,8}),
+ * TOP_E_NOMEM, TOP_E_CUDA, TOP_E_UNSUPPORTED (one trajectory longer than the on-chip capacity of the
+ * persistent kernel, see top_capacity).  On error *out is NULL; top_last_error(NULL) has the message.
+ */
+TOP_API top_status top_create(top_solver** out, int32_t batch, int32_t N, int32_t s, int32_t dims, top_dtype dtype,
+                      const double* waypoints, const double* durations,
+                      const double* start_derivs, const double* end_derivs,
+                      const top_constraints* cons, double rho, const top_options* opt);
+
+/* top_iterate -- exactly k sweeps of Alg. 1 lines 3-13 (k >= 0; k == 0 is a no-op), enqueued on the
+ * stream, no host synchronisation.  Afterwards the observable state is iterate (previous + k) and the
+ * residuals are those of the last sweep. */
+TOP_API top_status top_iterate(top_solver* h, int64_t k);
+
+/* top_solve -- sweep until, for every trajectory, r_p < eps and r_d < eps (Eq. 23, PAPER.md:L283-288;
+ * readings A6, A7, A8, A13), testing every check_every sweeps, or until max_iter sweeps (of this call).
+ *   iters  host [batch] or NULL: sweeps done (in this call) when that trajectory first passed the test,
+ *          or the total if it never did.
+ * Returns TOP_OK, TOP_NOT_CONVERGED, TOP_E_NONFINITE, TOP_E_CUDA.  Synchronises the stream. */
+TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iters);
+
+/* top_get_residuals -- residuals of the last sweep, host [batch] each, any pointer may be NULL:
+ *   r_primal       || stack_i (M c_i - z~_i) ||_2  over all consensus rows (reading A7)
+ *   r_dual         rho || stack_i M(T_i)'(z~_i^{k+1} - z~_i^k) ||_2   (Eq. 22, reading A8)
+ *   r_dual_norm    the same with component k divided by T_i^k
+ *   r_primal_gap   Eq. 21 verbatim: junction gaps only
+ * NaN before the first sweep.  Synchronises the stream. */
+TOP_API top_status top_get_residuals(top_solver* h, double* r_primal, double* r_dual, double* r_dual_norm,
+                             double* r_primal_gap);
+
+/* top_get_coeffs -- the trajectory C of the current iterate in the paper's basis (Eq. 18, PAPER.md:L220:
+ * ascending powers of (t - t_{i-1}), seconds, global frame), layout [batch][N][dims][2s] (dim-major per
+ * segment, the "squeezed" c_i of PAPER.md:L231), element type = the solver's dtype.
+ * out_is_device != 0: `out` is a device pointer, written on the stream without host synchronisation. */
+TOP_API top_status top_get_coeffs(top_solver* h, void* out, int32_t out_is_device);
+
+/* top_get_state -- one field of the current iterate as host fp64 (parity tests, warm-start snapshots).
+ * field / layout:  "z" [batch][N+1][s][dims]   "u" [batch][N][2s][dims]
+ *                  "s_pos","s_neg","v_pos","v_neg","phi_v","w_v","phi_a","w_a" [batch][N][Ms][dims]
+ * count = number of doubles `out` holds; TOP_E_INVALID if it does not match or the field is unknown. */
+TOP_API top_status top_get_state(top_solver* h, const char* field, double* out, size_t count);
+
+/* Sweeps done since top_create. */
+TOP_API int64_t top_iteration(const top_solver* h);
+
+/* Launch facts of this solver (for the bench's roofline arithmetic); any pointer may be NULL:
+ * CTAs per launch, threads per CTA, segments per CTA, dynamic shared memory bytes per CTA,
+ * waves (launches per top_iterate call) and kernels launched so far. */
+TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas, int32_t* threads, int32_t* segs_per_cta,
+                           int32_t* smem_bytes, int32_t* waves, int64_t* launches);
+
+/* Largest N (segments of ONE trajectory) the persistent kernel can hold on the given device
+ * (-1 = current) for this s / dtype / constraint selection; < 0 on error. */
+TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dtype, int32_t constrained);
+
+/* top_fma_peak -- measured plain-ALU FMA throughput of the device in FLOP/s (2 per FMA) for the given
+ * dtype, from a dependent-chain-free FMA loop on all SMs (the denominator of the ALU roofline).
+ * Runs `reps` launches on `stream` and returns the best.  < 0 on error. */
+TOP_API double top_fma_peak(int32_t device, top_dtype dtype, int32_t reps, void* cuda_stream);
+
+/* top_precompute_operator -- the host-side precompute top_create runs per segment, exposed so that it can
+ * be checked without a device (it launches nothing): the x-update operator of Eq. 20a in the
+ * library's internal normalised-time basis c^_a = c_a T^a, for one segment of duration T between waypoints
+ * p0, p1 (host [3]):  c^ = Pm_hat (rho R^) + c0_hat.   Pm_hat host [8][8] row-major (zero padded beyond 2s),
+ * c0_hat host [8][3].  flags: TOP_WAYPOINT_*.  box/vel/acc != 0 enable the constraint blocks (8 samples). */
+TOP_API top_status top_precompute_operator(int32_t s, double T, double rho, int32_t box, int32_t vel, int32_t acc,
+                                           uint32_t flags, const double* p0, const double* p1,
+                                           double* Pm_hat, double* c0_hat);
+
+TOP_API top_status top_destroy(top_solver* h);
+
+/* Message of the last failing call on this handle (h == NULL: of the last failing top_create on this
+ * thread).  Never NULL. */
+TOP_API const char* top_last_error(const top_solver* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TOP_H */

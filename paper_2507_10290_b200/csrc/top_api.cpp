@@ -1,0 +1,727 @@
+// top_api.cpp -- host side of the C ABI in include/top.h: validation, the one-off per-segment precompute of
+// the x-update operator (Eq. 20a), SoA packing, launch planning and the calls themselves.
+// Product code: shares nothing with oracle/.  Every sweep step runs in top_kernels.cu; there is no CPU path.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/top.h"
+#include "top_internal.h"
+
+using namespace top;
+
+namespace {
+
+typedef long double xreal;   // precision of the one-off operator precompute (cond(H) reaches 1e13, R6)
+
+thread_local std::string g_create_error;
+
+}  // namespace
+
+struct top_solver {
+    int batch = 0, N = 0, s = 0, dims = 0, dtype = 0, n = 0;
+    uint32_t opt_flags = 0, kflags = 0;
+    bool constrained = false, has_box = false, has_vel = false, has_acc = false;
+    double rho = 0, vmax = 0, amax = 0;
+    int check_every = 32;
+    int64_t max_iter = 1000000;
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    long long nseg = 0, nseg_pad = 0, stride = 0;
+    int num_sms = 0, max_ctas = 0, user_segs = 0;
+    struct Wave { long long seg_begin, seg_end; int segs_per_cta, ctas, threads; size_t smem; };
+    std::vector<Wave> waves;
+    // device buffers
+    std::vector<void*> allocs;
+    double *d_Pm = nullptr, *d_c0 = nullptr, *d_part = nullptr, *d_res = nullptr;
+    void *d_invTk = nullptr, *d_Tpow = nullptr, *d_invT = nullptr, *d_lohi = nullptr;
+    uint8_t* d_segflags = nullptr;
+    void *d_zt = nullptr, *d_u = nullptr, *d_qp = nullptr, *d_qn = nullptr, *d_phv = nullptr, *d_wv = nullptr,
+         *d_pha = nullptr, *d_wa = nullptr, *d_chat = nullptr, *d_Bedge = nullptr, *d_coef = nullptr;
+    unsigned char* d_sync = nullptr;   // [u64 barrier counter][u32 flag x max_ctas]
+    int* d_abort = nullptr;
+    double* h_res = nullptr;           // pinned [batch][4]
+    int* h_abort = nullptr;            // pinned
+    bool have_residuals = false;
+    int64_t iter = 0, launches = 0;
+    std::string err;
+};
+
+namespace {
+
+size_t real_bytes(const top_solver* h) { return h->dtype == TOP_F64 ? 8 : 4; }
+
+top_status fail(top_solver* h, top_status st, const std::string& msg) {
+    if (h) h->err = msg; else g_create_error = msg;
+    return st;
+}
+top_status cuda_fail(top_solver* h, cudaError_t e, const char* what) {
+    return fail(h, TOP_E_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define CU(call, what) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return cuda_fail(h, e_, what); } while (0)
+
+// ---------------------------------------------------------------------------------- small dense linear algebra
+
+// [beta_k(tau)]_a = a!/(a-k)! tau^(a-k)   (Eq. 18 differentiated, normalised time)
+xreal beta_hat(int k, int a, xreal tau) {
+    if (a < k) return 0;
+    xreal f = 1;
+    for (int q = 0; q < k; ++q) f *= (xreal)(a - q);
+    return f * std::pow(tau, (xreal)(a - k));
+}
+
+// In-place inverse of a symmetric positive definite q x q matrix: symmetric diagonal scaling, then
+// Gauss-Jordan elimination without pivoting (safe for SPD), in extended precision.  false if not SPD.
+bool spd_invert(int q, std::vector<xreal>& A) {
+    std::vector<xreal> sc(q);
+    for (int i = 0; i < q; ++i) {
+        if (!(A[i * q + i] > 0)) return false;
+        sc[i] = 1 / std::sqrt(A[i * q + i]);
+    }
+    std::vector<xreal> W(q * 2 * q, 0);
+    for (int i = 0; i < q; ++i) {
+        for (int j = 0; j < q; ++j) W[i * 2 * q + j] = A[i * q + j] * sc[i] * sc[j];
+        W[i * 2 * q + q + i] = 1;
+    }
+    for (int c = 0; c < q; ++c) {
+        const xreal piv = W[c * 2 * q + c];
+        if (!(piv > 0)) return false;
+        for (int j = 0; j < 2 * q; ++j) W[c * 2 * q + j] /= piv;
+        for (int r = 0; r < q; ++r) {
+            if (r == c) continue;
+            const xreal f = W[r * 2 * q + c];
+            if (f == 0) continue;
+            for (int j = 0; j < 2 * q; ++j) W[r * 2 * q + j] -= f * W[c * 2 * q + j];
+        }
+    }
+    for (int i = 0; i < q; ++i)
+        for (int j = 0; j < q; ++j) A[i * q + j] = W[i * 2 * q + q + j] * sc[i] * sc[j];
+    for (int i = 0; i < q; ++i)          // symmetrise the rounding
+        for (int j = 0; j < i; ++j) { const xreal m = (A[i * q + j] + A[j * q + i]) / 2; A[i * q + j] = A[j * q + i] = m; }
+    return true;
+}
+
+// Per-segment operator in the normalised-time basis c^_a = c_a T^a:
+//   H^ = 2 T^(1-2s) Q(1) + rho [ sum_r m^_r m^_r' + 2 sum_j e0_j e0_j' + sum_j e1_j e1_j'/T^2 + sum_j e2_j e2_j'/T^4 ]
+// (Eq. 20a first bracket; Q, M, Ao, Av of PAPER.md:L231; cost without 1/2 => 2Q, reading A19).
+// HARD waypoint mode (reading A2): the two equalities c^_0 = p_{i-1}, sum_a c^_a = p_i are eliminated with the
+// null-space basis Z = {e_a - e_1, a >= 2}:  Pm^ = Z (Z'H^Z)^-1 Z',  c0^ = (I - Pm^ H^) c_chord.
+// Other modes: Pm^ = H^^-1, c0^ = 0.
+bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int mode,
+                    const xreal* p0, const xreal* p1, xreal* Pm /*[8][8]*/, xreal* c0 /*[8][3]*/) {
+    const int n = 2 * s;
+    std::vector<xreal> H(n * n, 0);
+    for (int j = s; j < n; ++j)
+        for (int l = s; l < n; ++l) {
+            xreal fj = 1, fl = 1;
+            for (int q = 0; q < s; ++q) { fj *= (xreal)(j - q); fl *= (xreal)(l - q); }
+            H[j * n + l] = 2 * std::pow(T, (xreal)(1 - 2 * s)) * fj * fl / (xreal)(j + l - 2 * s + 1);
+        }
+    auto add_row = [&](int k, xreal tau, xreal w) {
+        xreal row[MAXN];
+        for (int a = 0; a < n; ++a) row[a] = beta_hat(k, a, tau) / std::pow(T, (xreal)k);
+        for (int a = 0; a < n; ++a)
+            for (int b = 0; b < n; ++b) H[a * n + b] += rho * w * row[a] * row[b];
+    };
+    for (int k = 0; k < s; ++k) { add_row(k, 0, 1); add_row(k, 1, 1); }
+    for (int j = 1; j <= MS; ++j) {
+        const xreal tau = (xreal)j / (xreal)(MS + 1);          // reading A10
+        if (box) add_row(0, tau, 2);                            // two sides of the box (A11)
+        if (vel) add_row(1, tau, 1);
+        if (acc) add_row(2, tau, 1);
+    }
+    for (int i = 0; i < MAXN * MAXN; ++i) Pm[i] = 0;
+    for (int i = 0; i < MAXN * 3; ++i) c0[i] = 0;
+    if (mode == (int)TOP_WAYPOINT_HARD) {
+        const int q = n - 2;
+        std::vector<xreal> A(q * q);
+        auto Hz = [&](int a, int b) { return H[a * n + b]; };
+        for (int i = 0; i < q; ++i)
+            for (int j = 0; j < q; ++j) {
+                const int a = i + 2, b = j + 2;            // Z column i = e_a - e_1
+                A[i * q + j] = Hz(a, b) - Hz(a, 1) - Hz(1, b) + Hz(1, 1);
+            }
+        if (!spd_invert(q, A)) return false;
+        // Pm^ = Z A^-1 Z'
+        for (int i = 0; i < q; ++i)
+            for (int j = 0; j < q; ++j) {
+                const xreal v = A[i * q + j];
+                Pm[(i + 2) * MAXN + (j + 2)] += v;
+                Pm[1 * MAXN + (j + 2)] -= v;
+                Pm[(i + 2) * MAXN + 1] -= v;
+                Pm[1 * MAXN + 1] += v;
+            }
+        for (int d = 0; d < 3; ++d) {
+            xreal cp[MAXN] = {0}, Hc[MAXN] = {0};
+            cp[0] = p0[d]; cp[1] = p1[d] - p0[d];
+            for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) Hc[a] += H[a * n + b] * cp[b];
+            for (int a = 0; a < n; ++a) {
+                xreal acc2 = 0;
+                for (int b = 0; b < n; ++b) acc2 += Pm[a * MAXN + b] * Hc[b];
+                c0[a * 3 + d] = cp[a] - acc2;
+            }
+        }
+    } else {
+        std::vector<xreal> A(H);
+        if (!spd_invert(n, A)) return false;
+        for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) Pm[a * MAXN + b] = A[a * n + b];
+    }
+    return true;
+}
+
+template <typename Real>
+void project_ball_host(const double* y, double bound, Real* phi) {
+    const double n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+    double sc = 1;
+    if (n2 > bound * bound) sc = bound / std::sqrt(n2);
+    for (int d = 0; d < 3; ++d) phi[d] = (Real)(sc * y[d]);
+}
+
+top_status dev_alloc(top_solver* h, void** out, size_t bytes, bool zero) {
+    void* p = nullptr;
+    cudaError_t e = cudaMalloc(&p, bytes ? bytes : 16);
+    if (e != cudaSuccess) { *out = nullptr; return fail(h, e == cudaErrorMemoryAllocation ? TOP_E_NOMEM : TOP_E_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
+    h->allocs.push_back(p);
+    if (zero) { e = cudaMemsetAsync(p, 0, bytes ? bytes : 16, h->stream); if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync"); }
+    *out = p;
+    return TOP_OK;
+}
+
+// host fp64 staging -> device array of the solver's Real type
+top_status upload_real(top_solver* h, void* dst, const std::vector<double>& src) {
+    if (src.empty()) return TOP_OK;
+    if (h->dtype == TOP_F64) {
+        CU(cudaMemcpyAsync(dst, src.data(), src.size() * 8, cudaMemcpyHostToDevice, h->stream), "H2D");
+        CU(cudaStreamSynchronize(h->stream), "sync");
+    } else {
+        std::vector<float> f(src.size());
+        for (size_t i = 0; i < src.size(); ++i) f[i] = (float)src[i];
+        CU(cudaMemcpyAsync(dst, f.data(), f.size() * 4, cudaMemcpyHostToDevice, h->stream), "H2D");
+        CU(cudaStreamSynchronize(h->stream), "sync");
+    }
+    return TOP_OK;
+}
+
+top_status download_real(top_solver* h, const void* src, std::vector<double>& dst, size_t count) {
+    dst.resize(count);
+    if (h->dtype == TOP_F64) {
+        CU(cudaMemcpyAsync(dst.data(), src, count * 8, cudaMemcpyDeviceToHost, h->stream), "D2H");
+        CU(cudaStreamSynchronize(h->stream), "sync");
+    } else {
+        std::vector<float> f(count);
+        CU(cudaMemcpyAsync(f.data(), src, count * 4, cudaMemcpyDeviceToHost, h->stream), "D2H");
+        CU(cudaStreamSynchronize(h->stream), "sync");
+        for (size_t i = 0; i < count; ++i) dst[i] = (double)f[i];
+    }
+    return TOP_OK;
+}
+
+int round_up(int x, int m) { return (x + m - 1) / m * m; }
+
+// largest segments-per-CTA (multiple of 4) whose threads and shared memory fit one CTA
+int max_segs_per_cta(int dtype, int s, bool constrained, uint32_t kflags, size_t smem_limit) {
+    int best = 0;
+    for (int segs = 4; segs * LANES <= max_threads_for(dtype); segs += 4)
+        if (sweep_smem_bytes(dtype, s, constrained, kflags, segs) <= smem_limit) best = segs;
+    return best;
+}
+
+}  // namespace
+
+// =================================================================================== top_create
+
+extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_t N, int32_t s, int32_t dims, top_dtype dtype,
+                                 const double* waypoints, const double* durations, const double* start_derivs,
+                                 const double* end_derivs, const top_constraints* cons, double rho,
+                                 const top_options* opt) {
+    top_solver* h = nullptr;   // errors before the handle exists go to the thread-local message
+    if (!out) return fail(h, TOP_E_INVALID, "out is NULL");
+    *out = nullptr;
+    if (batch < 1 || N < 1) return fail(h, TOP_E_INVALID, "batch and N must be >= 1");
+    if (s != 3 && s != 4) return fail(h, TOP_E_INVALID, "s must be 3 (jerk) or 4 (snap)");
+    if (dims < 1 || dims > 3) return fail(h, TOP_E_INVALID, "dims must be 1..3");
+    if (dtype != TOP_F64 && dtype != TOP_F32) return fail(h, TOP_E_INVALID, "unknown dtype");
+    if (!waypoints || !durations) return fail(h, TOP_E_INVALID, "waypoints and durations are required");
+    if (!(rho > 0) || !std::isfinite(rho)) return fail(h, TOP_E_INVALID, "rho must be finite and > 0");
+    const long long nseg = (long long)batch * N;
+    if (nseg > (1ll << 28)) return fail(h, TOP_E_UNSUPPORTED, "more than 2^28 segments");
+    for (long long i = 0; i < (long long)batch * (N + 1) * dims; ++i)
+        if (!std::isfinite(waypoints[i])) return fail(h, TOP_E_INVALID, "non-finite waypoint");
+    for (long long i = 0; i < nseg; ++i)
+        if (!(durations[i] > 0) || !std::isfinite(durations[i])) return fail(h, TOP_E_INVALID, "durations must be finite and > 0");
+    for (int e = 0; e < 2; ++e) {
+        const double* dv = e ? end_derivs : start_derivs;
+        if (dv) for (long long i = 0; i < (long long)batch * (s - 1) * dims; ++i)
+            if (!std::isfinite(dv[i])) return fail(h, TOP_E_INVALID, "non-finite end state");
+    }
+    bool has_box = false, has_vel = false, has_acc = false;
+    if (cons && cons->samples != 0) {
+        if (cons->samples != MS) return fail(h, TOP_E_INVALID, "constraints.samples must be 0 or 8");
+        if ((cons->box_lo == nullptr) != (cons->box_hi == nullptr)) return fail(h, TOP_E_INVALID, "box_lo and box_hi go together");
+        has_box = cons->box_lo != nullptr;
+        if (has_box) for (long long i = 0; i < nseg * dims; ++i) {
+            if (!std::isfinite(cons->box_lo[i]) || !std::isfinite(cons->box_hi[i]) || !(cons->box_lo[i] < cons->box_hi[i]))
+                return fail(h, TOP_E_INVALID, "box needs finite lo < hi");
+        }
+        if (std::isnan(cons->vmax) || std::isnan(cons->amax) || std::isinf(cons->vmax) || std::isinf(cons->amax))
+            return fail(h, TOP_E_INVALID, "vmax/amax must be finite");
+        has_vel = cons->vmax > 0;
+        has_acc = cons->amax > 0;
+    }
+    top_options o;
+    std::memset(&o, 0, sizeof o);
+    o.check_every = 32; o.device = -1; o.max_iter = 1000000;
+    if (opt) {
+        if (opt->struct_size < 8 || opt->struct_size > sizeof(top_options)) return fail(h, TOP_E_INVALID, "options.struct_size");
+        top_options in;
+        std::memset(&in, 0, sizeof in);
+        std::memcpy(&in, opt, opt->struct_size);
+        o.flags = in.flags;
+        if (opt->struct_size >= offsetof(top_options, device)) if (in.check_every > 0) o.check_every = in.check_every;
+        if (opt->struct_size >= offsetof(top_options, max_iter)) o.device = in.device;
+        if (opt->struct_size >= offsetof(top_options, cuda_stream)) if (in.max_iter > 0) o.max_iter = in.max_iter;
+        if (opt->struct_size >= offsetof(top_options, segs_per_cta)) o.cuda_stream = in.cuda_stream;
+        if (opt->struct_size >= offsetof(top_options, reserved)) o.segs_per_cta = in.segs_per_cta;
+    }
+    const uint32_t mode = o.flags & TOP_WAYPOINT_MASK;
+    if (mode > TOP_WAYPOINT_FREE) return fail(h, TOP_E_INVALID, "unknown waypoint mode");
+    if (o.segs_per_cta < 0 || (o.segs_per_cta % 4) != 0) return fail(h, TOP_E_INVALID, "segs_per_cta must be a multiple of 4");
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(h, TOP_E_CUDA, "no CUDA device: this library has no CPU path");
+    }
+    int dev = o.device;
+    if (dev < 0) { if (cudaGetDevice(&dev) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaGetDevice failed"); }
+    if (dev >= ndev) return fail(h, TOP_E_INVALID, "device ordinal out of range");
+    if (cudaSetDevice(dev) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
+
+    h = new (std::nothrow) top_solver();
+    if (!h) return fail(nullptr, TOP_E_NOMEM, "host allocation failed");
+    // from here on errors are reported through the thread-local message and the handle is destroyed
+#define CREATE_FAIL(st_) do { top_status s__ = (st_); g_create_error = h->err; top_destroy(h); return s__; } while (0)
+    h->batch = batch; h->N = N; h->s = s; h->n = 2 * s; h->dims = dims; h->dtype = (int)dtype;
+    h->opt_flags = o.flags; h->rho = rho; h->check_every = o.check_every; h->max_iter = o.max_iter;
+    h->device = dev; h->stream = (cudaStream_t)o.cuda_stream; h->user_segs = o.segs_per_cta;
+    h->has_box = has_box; h->has_vel = has_vel; h->has_acc = has_acc;
+    h->constrained = has_box || has_vel || has_acc;
+    h->vmax = has_vel ? cons->vmax : 0; h->amax = has_acc ? cons->amax : 0;
+    h->kflags = (has_box ? KF_BOX : 0) | (has_vel ? KF_VEL : 0) | (has_acc ? KF_ACC : 0) |
+                (mode == TOP_WAYPOINT_PINNED_Z ? KF_PIN_POS : 0);
+    h->nseg = nseg; h->nseg_pad = (nseg + 31) / 32 * 32; h->stride = h->nseg_pad * LANES;
+
+    // ---- launch plan: waves of whole trajectories, each wave resident on chip for all its sweeps
+    int smem_optin = 0;
+    if (cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess)
+        CREATE_FAIL(fail(h, TOP_E_CUDA, "cudaDeviceGetAttribute failed"));
+    int coop = 0;
+    cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+    if (!coop) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "device lacks cooperative launch"));
+    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->kflags, (size_t)smem_optin - 1024);
+    if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
+    h->max_ctas = h->num_sms;
+    const long long capacity = (long long)h->max_ctas * std::min(segs_max, h->user_segs ? h->user_segs : segs_max);
+    if ((long long)N > capacity) {
+        char msg[160];
+        std::snprintf(msg, sizeof msg, "one trajectory of N=%d segments exceeds the on-chip capacity of %lld segments", N, capacity);
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, msg));
+    }
+    {
+        const long long traj_cap = capacity / N;
+        const long long nwaves = (batch + traj_cap - 1) / traj_cap;
+        const long long per_wave = (batch + nwaves - 1) / nwaves;
+        for (long long b0 = 0; b0 < batch; b0 += per_wave) {
+            const long long b1 = std::min<long long>(batch, b0 + per_wave);
+            top_solver::Wave w;
+            w.seg_begin = b0 * N; w.seg_end = b1 * N;
+            const long long cnt = w.seg_end - w.seg_begin;
+            int segs = h->user_segs ? h->user_segs : round_up((int)((cnt + h->max_ctas - 1) / h->max_ctas), 4);
+            segs = std::max(4, std::min(segs, segs_max));
+            w.segs_per_cta = segs;
+            w.ctas = (int)((cnt + segs - 1) / segs);
+            w.threads = segs * LANES;
+            w.smem = sweep_smem_bytes(h->dtype, s, h->constrained, h->kflags, segs);
+            if (w.ctas > h->max_ctas) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "launch plan exceeds one CTA per SM"));
+            h->waves.push_back(w);
+        }
+    }
+    for (const auto& w : h->waves) {
+        int per_sm = 0;
+        cudaError_t e = sweep_kernel_limits(h->dtype, s, h->constrained, w.threads, w.smem, &per_sm);
+        if (e != cudaSuccess) CREATE_FAIL(cuda_fail(h, e, "occupancy query"));
+        if (per_sm < 1) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "sweep kernel does not fit an SM"));
+    }
+
+    // ---- host precompute (extended precision) and iterate 0 (reading A9), packed per lane
+    const size_t LS = (size_t)h->stride, NP = (size_t)h->nseg_pad;
+    std::vector<double> Pm(MAXN * LS, 0.0), c0(3 * LS, 0.0), invTk(LS, 0.0), Tpow(LS, 0.0), invT(2 * NP, 0.0),
+        lohi(6 * NP, 0.0), zt(3 * LS, 0.0), chat(3 * LS, 0.0), qp, qn, phv, pha;
+    std::vector<uint8_t> segflags(NP, 0);
+    if (has_box) { qp.assign(3 * LS, 0.0); qn.assign(3 * LS, 0.0); }
+    if (has_vel) phv.assign(3 * LS, 0.0);
+    const int n = 2 * s;
+    auto wp = [&](long long b, long long j, int d) -> double { return d < dims ? waypoints[((size_t)b * (N + 1) + j) * dims + d] : 0.0; };
+    for (long long b = 0; b < batch; ++b)
+        for (long long i = 0; i < N; ++i) {
+            const size_t g = (size_t)(b * N + i);
+            const double Td = durations[g];
+            const xreal T = (xreal)Td;
+            xreal p0[3], p1[3], PmX[MAXN * MAXN], c0X[MAXN * 3];
+            for (int d = 0; d < 3; ++d) { p0[d] = wp(b, i, d); p1[d] = wp(b, i + 1, d); }
+            if (!build_operator(s, T, (xreal)rho, has_box, has_vel, has_acc, (int)mode, p0, p1, PmX, c0X))
+                CREATE_FAIL(fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)"));
+            segflags[g] = (uint8_t)((i == 0 ? SEG_FIRST : 0) | (i == N - 1 ? SEG_LAST : 0));
+            invT[g] = (double)(1 / T); invT[NP + g] = (double)(1 / (T * T));
+            for (int d = 0; d < 3; ++d) {
+                lohi[(size_t)d * NP + g] = (has_box && d < dims) ? cons->box_lo[g * dims + d] : -1.0;
+                lohi[(size_t)(3 + d) * NP + g] = (has_box && d < dims) ? cons->box_hi[g * dims + d] : 1.0;
+            }
+            for (int lane = 0; lane < LANES; ++lane) {
+                const size_t gt = g * LANES + lane;
+                for (int bb = 0; bb < MAXN; ++bb) Pm[(size_t)bb * LS + gt] = (double)((xreal)rho * PmX[lane * MAXN + bb]);
+                for (int d = 0; d < 3; ++d) c0[(size_t)d * LS + gt] = d < dims ? (double)c0X[lane * 3 + d] : 0.0;
+                Tpow[gt] = (double)std::pow(T, (xreal)lane);
+                if (lane < n) {
+                    const int k = lane % s;
+                    invTk[gt] = (double)(1 / std::pow(T, (xreal)k));
+                    // z0: position = waypoint; velocity = mean of the adjacent chord velocities; higher orders 0;
+                    // z_0 and z_N carry the given end states (Eq. 2c)
+                    const long long j = lane < s ? i : i + 1;
+                    for (int d = 0; d < dims; ++d) {
+                        double v = 0;
+                        if (k == 0) v = wp(b, j, d);
+                        else if (j == 0) v = start_derivs ? start_derivs[((size_t)b * (s - 1) + (k - 1)) * dims + d] : 0.0;
+                        else if (j == N) v = end_derivs ? end_derivs[((size_t)b * (s - 1) + (k - 1)) * dims + d] : 0.0;
+                        else if (k == 1) {
+                            const double vl = (wp(b, j, d) - wp(b, j - 1, d)) / durations[b * N + j - 1];
+                            const double vr = (wp(b, j + 1, d) - wp(b, j, d)) / durations[b * N + j];
+                            v = 0.5 * (vl + vr);
+                        }
+                        zt[(size_t)d * LS + gt] = v;
+                    }
+                }
+                // C0 = chord at constant speed: c^_0 = p_{i-1}, c^_1 = p_i - p_{i-1}
+                for (int d = 0; d < dims; ++d)
+                    chat[(size_t)d * LS + gt] = lane == 0 ? (double)p0[d] : (lane == 1 ? (double)(p1[d] - p0[d]) : 0.0);
+                // samples of the chord: slack = max(0, .), phi = projection of the chord velocity, duals 0
+                const double tau = (double)(lane + 1) / (double)(MS + 1);
+                double V0[3] = {0, 0, 0};
+                for (int d = 0; d < dims; ++d) {
+                    const double P0 = (double)p0[d] + tau * (double)(p1[d] - p0[d]);
+                    V0[d] = (double)(p1[d] - p0[d]) / Td;
+                    if (has_box) {
+                        qp[(size_t)d * LS + gt] = std::max(0.0, cons->box_hi[g * dims + d] - P0);
+                        qn[(size_t)d * LS + gt] = std::max(0.0, P0 - cons->box_lo[g * dims + d]);
+                    }
+                }
+                if (has_box) for (int d = dims; d < 3; ++d) { qp[(size_t)d * LS + gt] = 1.0; qn[(size_t)d * LS + gt] = 1.0; }
+                if (has_vel) {
+                    double phi[3];
+                    project_ball_host<double>(V0, h->vmax, phi);
+                    for (int d = 0; d < 3; ++d) phv[(size_t)d * LS + gt] = phi[d];
+                }
+            }
+        }
+
+    // ---- device memory
+    const size_t rb = real_bytes(h);
+    top_status st;
+#define ALLOC(ptr, bytes, zero) do { void* p__ = nullptr; st = dev_alloc(h, &p__, (bytes), (zero)); if (st != TOP_OK) CREATE_FAIL(st); ptr = static_cast<decltype(ptr)>(p__); } while (0)
+    ALLOC(h->d_Pm, MAXN * LS * 8, false); ALLOC(h->d_c0, 3 * LS * 8, false);
+    ALLOC(h->d_invTk, LS * rb, false); ALLOC(h->d_Tpow, LS * rb, false); ALLOC(h->d_invT, 2 * NP * rb, false);
+    ALLOC(h->d_lohi, 6 * NP * rb, false); ALLOC(h->d_segflags, NP, false);
+    ALLOC(h->d_zt, 3 * LS * rb, false); ALLOC(h->d_u, 3 * LS * rb, true); ALLOC(h->d_chat, 3 * LS * rb, false);
+    if (has_box) { ALLOC(h->d_qp, 3 * LS * rb, false); ALLOC(h->d_qn, 3 * LS * rb, false); }
+    if (has_vel) { ALLOC(h->d_phv, 3 * LS * rb, false); ALLOC(h->d_wv, 3 * LS * rb, true); }
+    if (has_acc) { ALLOC(h->d_pha, 3 * LS * rb, true); ALLOC(h->d_wa, 3 * LS * rb, true); }
+    ALLOC(h->d_Bedge, (size_t)2 * h->max_ctas * 24 * rb, true);
+    ALLOC(h->d_part, NP * 4 * 8, true); ALLOC(h->d_res, (size_t)batch * 4 * 8, true);
+    ALLOC(h->d_sync, 8 + (size_t)h->max_ctas * 4, true); ALLOC(h->d_abort, 16, true);
+    ALLOC(h->d_coef, (size_t)nseg * dims * n * rb, false);
+#undef ALLOC
+    if (cudaMallocHost((void**)&h->h_res, (size_t)batch * 4 * 8) != cudaSuccess ||
+        cudaMallocHost((void**)&h->h_abort, 16) != cudaSuccess)
+        CREATE_FAIL(fail(h, TOP_E_NOMEM, "pinned host allocation failed"));
+    for (long long i = 0; i < (long long)batch * 4; ++i) h->h_res[i] = std::numeric_limits<double>::quiet_NaN();
+    h->h_abort[0] = 0;
+
+    cudaError_t ce;
+    if ((ce = cudaMemcpyAsync(h->d_Pm, Pm.data(), MAXN * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_c0, c0.data(), 3 * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_segflags, segflags.data(), NP, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
+        CREATE_FAIL(cuda_fail(h, ce, "upload"));
+#define UP(dst, src) do { st = upload_real(h, dst, src); if (st != TOP_OK) CREATE_FAIL(st); } while (0)
+    UP(h->d_invTk, invTk); UP(h->d_Tpow, Tpow); UP(h->d_invT, invT); UP(h->d_lohi, lohi);
+    UP(h->d_zt, zt); UP(h->d_chat, chat);
+    if (has_box) { UP(h->d_qp, qp); UP(h->d_qn, qn); }
+    if (has_vel) UP(h->d_phv, phv);
+#undef UP
+#undef CREATE_FAIL
+    *out = h;
+    return TOP_OK;
+}
+
+// =================================================================================== sweeps
+
+namespace {
+
+top_status check_abort(top_solver* h) {
+    CU(cudaMemcpyAsync(h->h_abort, h->d_abort, sizeof(int), cudaMemcpyDeviceToHost, h->stream), "D2H abort flag");
+    CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+    if (h->h_abort[0]) return fail(h, TOP_E_CUDA, "inter-CTA barrier timed out inside the sweep kernel");
+    return TOP_OK;
+}
+
+uint32_t sync_flag(const top_solver* h) {
+    const uint32_t m = h->opt_flags & TOP_SYNC_MASK;
+    if (m == TOP_SYNC_GRID) return 0;
+    return KF_NEIGHBOUR_SYNC;     // TOP_SYNC_AUTO and TOP_SYNC_NEIGHBOUR
+}
+
+// k sweeps on every wave, then the per-trajectory residual reduction.  Asynchronous.
+top_status run_sweeps(top_solver* h, int64_t k) {
+    if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
+    while (k > 0) {
+        const int kk = (int)std::min<int64_t>(k, 1 << 30);
+        for (const auto& w : h->waves) {
+            KParams p;
+            std::memset(&p, 0, sizeof p);
+            p.Pm = h->d_Pm; p.c0 = h->d_c0; p.invTk = h->d_invTk; p.Tpow = h->d_Tpow; p.invT = h->d_invT;
+            p.lohi = h->d_lohi; p.segflags = h->d_segflags;
+            p.zt = h->d_zt; p.u = h->d_u; p.qp = h->d_qp; p.qn = h->d_qn; p.phv = h->d_phv; p.wv = h->d_wv;
+            p.pha = h->d_pha; p.wa = h->d_wa; p.chat = h->d_chat;
+            p.Bedge = h->d_Bedge; p.part = h->d_part;
+            p.bar = reinterpret_cast<unsigned long long*>(h->d_sync);
+            p.nflag = reinterpret_cast<unsigned int*>(h->d_sync + 8);
+            p.abort_flag = h->d_abort;
+            p.stride = h->stride; p.nseg_pad = h->nseg_pad; p.seg_begin = w.seg_begin; p.seg_end = w.seg_end;
+            p.segs_per_cta = w.segs_per_cta; p.k_sweeps = kk; p.flags = h->kflags | sync_flag(h);
+            p.max_ctas = h->max_ctas; p.rho = h->rho; p.vmax = h->vmax; p.amax = h->amax;
+            if (w.ctas > 1)
+                CU(cudaMemsetAsync(h->d_sync, 0, 8 + (size_t)h->max_ctas * 4, h->stream), "cudaMemsetAsync");
+            CU(launch_sweeps(p, h->dtype, h->s, h->constrained, w.ctas, w.threads, w.smem, h->stream), "sweep kernel launch");
+            h->launches += 1;
+        }
+        k -= kk;
+        h->iter += kk;
+    }
+    CU(launch_residual_reduce(h->d_part, h->d_res, h->N, h->batch, h->stream), "residual reduction launch");
+    h->launches += 1;
+    h->have_residuals = true;
+    return TOP_OK;
+}
+
+top_status fetch_residuals(top_solver* h) {
+    if (!h->have_residuals) return TOP_OK;
+    CU(cudaMemcpyAsync(h->h_res, h->d_res, (size_t)h->batch * 4 * 8, cudaMemcpyDeviceToHost, h->stream), "D2H residuals");
+    return check_abort(h);   // synchronises
+}
+
+}  // namespace
+
+extern "C" TOP_API top_status top_iterate(top_solver* h, int64_t k) {
+    if (!h) return TOP_E_INVALID;
+    if (k < 0) return fail(h, TOP_E_INVALID, "k must be >= 0");
+    if (k == 0) return TOP_OK;
+    return run_sweeps(h, k);
+}
+
+extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iters) {
+    if (!h) return TOP_E_INVALID;
+    if (!(eps > 0)) return fail(h, TOP_E_INVALID, "eps must be > 0");
+    const double tol = (h->opt_flags & TOP_EPS_N_SCALED) ? eps * h->N : eps;
+    const int rd_idx = (h->opt_flags & TOP_RD_NORMALISED) ? 2 : 1;
+    std::vector<int64_t> first(h->batch, -1);
+    int64_t done = 0;
+    bool all = false;
+    while (done < h->max_iter && !all) {
+        const int64_t k = std::min<int64_t>(h->check_every, h->max_iter - done);
+        top_status st = run_sweeps(h, k);
+        if (st != TOP_OK) return st;
+        done += k;
+        st = fetch_residuals(h);
+        if (st != TOP_OK) return st;
+        all = true;
+        for (int b = 0; b < h->batch; ++b) {
+            const double rp = h->h_res[b * 4 + 0], rd = h->h_res[b * 4 + rd_idx];
+            if (!std::isfinite(rp) || !std::isfinite(rd)) return fail(h, TOP_E_NONFINITE, "non-finite residual");
+            if (rp < tol && rd < tol) { if (first[b] < 0) first[b] = done; }
+            else { all = false; first[b] = -1; }     // a trajectory counts as converged only while it stays below
+        }
+    }
+    if (iters) for (int b = 0; b < h->batch; ++b) iters[b] = first[b] >= 0 ? first[b] : done;
+    return all ? TOP_OK : TOP_NOT_CONVERGED;
+}
+
+extern "C" TOP_API top_status top_get_residuals(top_solver* h, double* r_primal, double* r_dual, double* r_dual_norm,
+                                        double* r_primal_gap) {
+    if (!h) return TOP_E_INVALID;
+    top_status st = fetch_residuals(h);
+    if (st != TOP_OK) return st;
+    for (int b = 0; b < h->batch; ++b) {
+        if (r_primal) r_primal[b] = h->h_res[b * 4 + 0];
+        if (r_dual) r_dual[b] = h->h_res[b * 4 + 1];
+        if (r_dual_norm) r_dual_norm[b] = h->h_res[b * 4 + 2];
+        if (r_primal_gap) r_primal_gap[b] = h->h_res[b * 4 + 3];
+    }
+    return TOP_OK;
+}
+
+extern "C" TOP_API top_status top_get_coeffs(top_solver* h, void* out, int32_t out_is_device) {
+    if (!h) return TOP_E_INVALID;
+    if (!out) return fail(h, TOP_E_INVALID, "out is NULL");
+    if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
+    ConvParams p;
+    p.chat = h->d_chat; p.invT = h->d_invT; p.out = out_is_device ? out : h->d_coef;
+    p.stride = h->stride; p.nseg = h->nseg; p.s = h->s; p.dims = h->dims;
+    CU(launch_convert(p, h->dtype, h->stream), "coefficient conversion launch");
+    h->launches += 1;
+    if (!out_is_device) {
+        CU(cudaMemcpyAsync(out, h->d_coef, (size_t)h->nseg * h->dims * h->n * real_bytes(h), cudaMemcpyDeviceToHost, h->stream), "D2H coefficients");
+        return check_abort(h);
+    }
+    return TOP_OK;
+}
+
+extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, double* out, size_t count) {
+    if (!h) return TOP_E_INVALID;
+    if (!field || !out) return fail(h, TOP_E_INVALID, "field and out are required");
+    const std::string f(field);
+    const int s = h->s, dims = h->dims, N = h->N, batch = h->batch;
+    const size_t LS = (size_t)h->stride;
+    std::vector<double> buf;
+    top_status st;
+    if (f == "z" || f == "u") {
+        const size_t want = f == "z" ? (size_t)batch * (N + 1) * s * dims : (size_t)batch * N * 2 * s * dims;
+        if (count != want) return fail(h, TOP_E_INVALID, "top_get_state: count does not match the field");
+        if ((st = download_real(h, f == "z" ? h->d_zt : h->d_u, buf, 3 * LS)) != TOP_OK) return st;
+        for (int b = 0; b < batch; ++b)
+            for (int i = 0; i < N; ++i) {
+                const size_t g = (size_t)b * N + i;
+                for (int r = 0; r < 2 * s; ++r)
+                    for (int d = 0; d < dims; ++d) {
+                        const double v = buf[(size_t)d * LS + g * LANES + r];
+                        if (f == "u") out[((g * 2 * s) + r) * dims + d] = v;
+                        else if (r < s) out[(((size_t)b * (N + 1) + i) * s + r) * dims + d] = v;
+                        else if (i == N - 1) out[(((size_t)b * (N + 1) + N) * s + (r - s)) * dims + d] = v;
+                    }
+            }
+        return check_abort(h);
+    }
+    struct { const char* name; void* ptr; int how; bool on; } tab[] = {
+        {"s_pos", h->d_qp, 1, h->has_box}, {"v_pos", h->d_qp, 2, h->has_box},
+        {"s_neg", h->d_qn, 1, h->has_box}, {"v_neg", h->d_qn, 2, h->has_box},
+        {"phi_v", h->d_phv, 0, h->has_vel}, {"w_v", h->d_wv, 0, h->has_vel},
+        {"phi_a", h->d_pha, 0, h->has_acc}, {"w_a", h->d_wa, 0, h->has_acc}};
+    for (auto& t : tab) {
+        if (f != t.name) continue;
+        const size_t want = (size_t)batch * N * MS * dims;
+        if (count != want) return fail(h, TOP_E_INVALID, "top_get_state: count does not match the field");
+        if (!t.on) { std::fill(out, out + count, 0.0); return TOP_OK; }
+        if ((st = download_real(h, t.ptr, buf, 3 * LS)) != TOP_OK) return st;
+        for (size_t g = 0; g < (size_t)batch * N; ++g)
+            for (int j = 0; j < MS; ++j)
+                for (int d = 0; d < dims; ++d) {
+                    const double v = buf[(size_t)d * LS + g * LANES + j];
+                    // Moreau pair of the slack projection (Eq. 10 / 20d-e): s = max(0,q), v = max(0,-q)
+                    out[(g * MS + j) * dims + d] = t.how == 0 ? v : (t.how == 1 ? std::max(0.0, v) : std::max(0.0, -v));
+                }
+        return check_abort(h);
+    }
+    return fail(h, TOP_E_INVALID, "top_get_state: unknown field '" + f + "'");
+}
+
+extern "C" TOP_API int64_t top_iteration(const top_solver* h) { return h ? h->iter : -1; }
+
+extern "C" TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas, int32_t* threads, int32_t* segs_per_cta,
+                                      int32_t* smem_bytes, int32_t* waves, int64_t* launches) {
+    if (!h || h->waves.empty()) return TOP_E_INVALID;
+    const auto& w = h->waves[0];
+    if (ctas) *ctas = w.ctas;
+    if (threads) *threads = w.threads;
+    if (segs_per_cta) *segs_per_cta = w.segs_per_cta;
+    if (smem_bytes) *smem_bytes = (int32_t)w.smem;
+    if (waves) *waves = (int32_t)h->waves.size();
+    if (launches) *launches = h->launches;
+    return TOP_OK;
+}
+
+extern "C" TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dtype, int32_t constrained) {
+    if ((s != 3 && s != 4) || (dtype != TOP_F64 && dtype != TOP_F32)) return -1;
+    int dev = device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return -1; }
+    int sms = 0, smem = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) { cudaGetLastError(); return -1; }
+    const uint32_t kf = constrained ? (KF_BOX | KF_VEL | KF_ACC) : 0;
+    return (int64_t)sms * max_segs_per_cta((int)dtype, s, constrained != 0, kf, (size_t)smem - 1024);
+}
+
+extern "C" TOP_API double top_fma_peak(int32_t device, top_dtype dtype, int32_t reps, void* cuda_stream) {
+    int dev = device;
+    if (dev < 0 && cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return -1; }
+    if (cudaSetDevice(dev) != cudaSuccess) return -1;
+    int sms = 0;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return -1;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    float* sink = nullptr;
+    if (cudaMalloc(&sink, 16) != cudaSuccess) return -1;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = sms * 4, threads = 512;
+    const long long iters = dtype == TOP_F64 ? 4000 : 8000;
+    double best = -1;
+    launch_fma_peak((int)dtype, blocks, threads, 100, sink, st);   // warm-up
+    for (int r = 0; r < std::max(1, reps); ++r) {
+        cudaEventRecord(e0, st);
+        if (launch_fma_peak((int)dtype, blocks, threads, iters, sink, st) != cudaSuccess) { best = -1; break; }
+        cudaEventRecord(e1, st);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { best = -1; break; }
+        float ms = 0;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double flops = 2.0 * 32.0 * (double)iters * blocks * threads;
+        if (ms > 0) best = std::max(best, flops / (ms * 1e-3));
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(sink);
+    return best;
+}
+
+extern "C" TOP_API top_status top_precompute_operator(int32_t s, double T, double rho, int32_t box, int32_t vel,
+                                                      int32_t acc, uint32_t flags, const double* p0, const double* p1,
+                                                      double* Pm_hat, double* c0_hat) {
+    if ((s != 3 && s != 4) || !(T > 0) || !(rho > 0) || !p0 || !p1 || !Pm_hat || !c0_hat ||
+        (flags & TOP_WAYPOINT_MASK) > TOP_WAYPOINT_FREE)
+        return fail(nullptr, TOP_E_INVALID, "top_precompute_operator: bad argument");
+    xreal a[3], b[3], PmX[MAXN * MAXN], c0X[MAXN * 3];
+    for (int d = 0; d < 3; ++d) { a[d] = p0[d]; b[d] = p1[d]; }
+    if (!build_operator(s, (xreal)T, (xreal)rho, box != 0, vel != 0, acc != 0, (int)(flags & TOP_WAYPOINT_MASK), a, b, PmX, c0X))
+        return fail(nullptr, TOP_E_INVALID, "operator is not positive definite");
+    for (int i = 0; i < MAXN * MAXN; ++i) Pm_hat[i] = (double)PmX[i];
+    for (int i = 0; i < MAXN * 3; ++i) c0_hat[i] = (double)c0X[i];
+    return TOP_OK;
+}
+
+extern "C" TOP_API top_status top_destroy(top_solver* h) {
+    if (!h) return TOP_OK;
+    cudaSetDevice(h->device);
+    cudaStreamSynchronize(h->stream);
+    for (void* p : h->allocs) cudaFree(p);
+    if (h->h_res) cudaFreeHost(h->h_res);
+    if (h->h_abort) cudaFreeHost(h->h_abort);
+    cudaGetLastError();
+    delete h;
+    return TOP_OK;
+}
+
+extern "C" TOP_API const char* top_last_error(const top_solver* h) { return h ? h->err.c_str() : g_create_error.c_str(); }

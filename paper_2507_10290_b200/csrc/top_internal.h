@@ -1,0 +1,78 @@
+// top_internal.h -- structures shared by the host side (top_api.cpp) and the kernels (top_kernels.cu).
+// Product code: shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace top {
+
+constexpr int LANES = 8;        // threads per segment: lane j <-> sample j, lane a <-> coefficient / consensus row a
+constexpr int MS = 8;           // samples per segment (Ms)
+constexpr int MAXN = 8;         // n = 2s <= 8
+constexpr int DIMS = 3;         // flat dimensions are padded to 3 (unused ones carry zeros)
+
+// segment flags
+constexpr uint8_t SEG_FIRST = 1;  // first segment of its trajectory: left junction (z_0) is fixed
+constexpr uint8_t SEG_LAST = 2;   // last segment: right junction (z_N) is fixed
+
+// kernel flags
+constexpr uint32_t KF_BOX = 1, KF_VEL = 2, KF_ACC = 4, KF_PIN_POS = 8 /* PINNED_Z: position row of z held */,
+                   KF_NEIGHBOUR_SYNC = 16;
+
+// Per-lane field arrays: element [f * stride + gseg * LANES + lane]; stride = padded lane count.
+// "Real" is double (TOP_F64) or float (TOP_F32); the x-update operator is always double.
+struct KParams {
+    // ---- constants (read only)
+    const double* Pm;       // [MAXN][stride]  row `lane` of rho * Pm_hat (normalised-time basis), zero padded
+    const double* c0;       // [DIMS][stride]  row `lane` of c0_hat
+    const void* invTk;      // Real [stride]   1 / T^k, k = derivative order of consensus row `lane`
+    const void* Tpow;       // Real [stride]   T^lane (physical-time scaling of the dual residual, Eq. 22)
+    const void* invT;       // Real [2][nseg_pad]  1/T, 1/T^2 per segment
+    const void* lohi;       // Real [6][nseg_pad]  lo[3], hi[3] per segment
+    const uint8_t* segflags;// [nseg_pad]
+    // ---- state of iterate k (read at launch start, written at launch end)
+    void* zt;               // Real [DIMS][stride]  consensus row `lane` of z~_i = (z_{i-1}; z_i)
+    void* u;                // Real [DIMS][stride]  scaled dual of that row (Eq. 20c)
+    void* qp;               // Real [DIMS][stride]  box + side: S+ = max(0,q), V+ = max(0,-q)  (Moreau pair)
+    void* qn;               // Real [DIMS][stride]  box - side
+    void* phv;              // Real [DIMS][stride]  phi of the velocity ball (Eq. 20f)
+    void* wv;               // Real [DIMS][stride]  its scaled dual (Eq. 20g)
+    void* pha;              // Real [DIMS][stride]
+    void* wa;               // Real [DIMS][stride]
+    void* chat;             // Real [DIMS][stride]  coefficient row `lane` in normalised time (c^_a = c_a T^a)
+    // ---- exchange / reduction
+    void* Bedge;            // Real [2 parity][max_ctas][2 sides][4][DIMS]  boundary rows at chunk edges
+    double* part;           // [nseg_pad][4]  per-segment residual partial sums (rp2, rd2, rdn2, gap2)
+    unsigned long long* bar;// [0] grid barrier counter (reset before each launch)
+    unsigned int* nflag;    // [max_ctas]  neighbour flags: sweeps published by each CTA (reset before each launch)
+    int* abort_flag;        // set when a barrier wait times out
+    // ---- sizes
+    long long stride;       // lanes per field (>= nseg_pad * LANES)
+    long long nseg_pad;
+    long long seg_begin, seg_end;   // global segment range of this launch (a wave of whole trajectories)
+    int segs_per_cta;
+    int k_sweeps;
+    uint32_t flags;
+    int max_ctas;
+    double rho, vmax, amax;
+};
+
+struct ConvParams {       // coefficient conversion to the paper's basis (Eq. 18)
+    const void* chat;     // Real [DIMS][stride]
+    const void* invT;     // Real [2][nseg_pad]
+    void* out;            // Real [nseg][dims][2s]
+    long long stride, nseg;
+    int s, dims;
+};
+
+// launchers (top_kernels.cu).  dtype: 0 = f64, 1 = f32.  Return cudaError_t.
+cudaError_t launch_sweeps(const KParams& p, int dtype, int s, bool constrained, int ctas, int threads,
+                          size_t smem, cudaStream_t st);
+size_t sweep_smem_bytes(int dtype, int s, bool constrained, uint32_t flags, int segs_per_cta);
+int max_threads_for(int dtype);
+cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int threads, size_t smem, int* max_ctas_per_sm);
+cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
+cudaError_t launch_residual_reduce(const double* part, double* res, long long N, int batch, cudaStream_t st);
+cudaError_t launch_fma_peak(int dtype, int blocks, int threads, long long iters, float* sink, cudaStream_t st);
+
+}  // namespace top

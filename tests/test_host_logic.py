@@ -1,0 +1,113 @@
+"""`not gpu` tests of the product's host side: the C-ABI library loads and exports every symbol that
+include/top.h declares, argument validation works without a device, and the per-segment operator precompute
+(top_precompute_operator, the code top_create runs) agrees with the oracle's independently written operator
+(different formulation: null-space elimination in normalised time vs. Schur complement in physical time)."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from oracle.top_oracle import Oracle
+from paper_2507_10290_b200 import build as top_build
+from paper_2507_10290_b200 import top
+from paper_2507_10290_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built():
+    top_build.build()
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "top.h")).read()
+    declared = sorted(set(re.findall(r"TOP_API\s+[\w\s\*]+?\b(top_\w+)\s*\(", header)))
+    assert len(declared) >= 12
+    assert sorted(top.EXPORTS) == declared
+    L = ctypes.CDLL(top.LIB_PATH)
+    for name in declared:
+        assert hasattr(L, name), name
+
+
+def test_no_oracle_in_product_path():
+    """The product package never imports, links or executes oracle/."""
+    pkg = os.path.join(ROOT, "paper_2507_10290_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cpp", ".h", ".cuh")):
+                txt = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(from|import)\s+oracle", txt, re.M), f
+                assert "top_oracle" not in txt, f
+
+
+def test_validation_happens_before_the_device_is_needed():
+    wp, T = np.zeros((3, 3)), np.ones(2)
+    cases = [
+        dict(waypoints=wp, durations=T, s=5, rho=1.0),                       # s
+        dict(waypoints=wp, durations=T, s=3, rho=0.0),                       # rho
+        dict(waypoints=wp, durations=np.array([1.0, -1.0]), s=3, rho=1.0),   # T <= 0
+        dict(waypoints=wp * np.nan, durations=T, s=3, rho=1.0),              # non-finite
+        dict(waypoints=wp, durations=T, s=3, rho=1.0, samples=4, vmax=1.0),  # samples
+        dict(waypoints=wp, durations=T, s=3, rho=1.0, samples=8, box_lo=np.ones((2, 3)), box_hi=np.zeros((2, 3))),
+        dict(waypoints=wp, durations=T, s=3, rho=1.0, segs_per_cta=6),
+    ]
+    for kw in cases:
+        with pytest.raises(top.TopError) as e:
+            top.TopSolver(**kw)
+        assert e.value.status == top.TOP_E_INVALID, kw
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a device is present")
+    with pytest.raises(top.TopError) as e:
+        top.TopSolver(np.zeros((3, 3)), np.ones(2), 3, 1.0)
+    assert e.value.status == top.TOP_E_CUDA
+
+
+@pytest.mark.parametrize("s", [3, 4])
+@pytest.mark.parametrize("mode", ["hard", "pinned_z", "free"])
+@pytest.mark.parametrize("cons", [(0, 0, 0), (1, 1, 0), (1, 1, 1)])
+def test_operator_precompute_matches_oracle_operator(s, mode, cons):
+    """c = Pm rho R + c0 (oracle, physical time)  <=>  c^ = Pm^ rho R^ + c0^ with c^ = D c, R^ = D^-1 R:
+    Pm^ = D Pm D, c0^ = D c0, D = diag(T^a)."""
+    rng = np.random.default_rng(11 * s + sum(cons))
+    box, vel, acc = cons
+    n = 2 * s
+    for T in (0.37, 1.0, 2.9, 7.5):
+        p = rng.uniform(-20, 20, size=(2, 3))
+        rho = float(rng.choice([0.5, 1.0, 10.0, 300.0]))
+        kw = {}
+        if box or vel or acc:
+            kw = dict(samples=8, vmax=3.0 if vel else 0.0, amax=5.0 if acc else 0.0)
+            if box:
+                kw.update(box_lo=np.minimum(p[0], p[1])[None] - 1.0, box_hi=np.maximum(p[0], p[1])[None] + 1.0)
+        o = Oracle(p, np.array([T]), s, rho, mode=mode, **kw)
+        D = T ** np.arange(n)
+        Pm_ref = o.get("Pm")[0] * D[:, None] * D[None, :]
+        c0_ref = o.get("c0")[0] * D[:, None]
+        Pm, c0 = top.precompute_operator(s, T, rho, p[0], p[1], box=box, vel=vel, acc=acc, mode=mode)
+        assert np.all(Pm[n:] == 0) and np.all(Pm[:, n:] == 0) and np.all(c0[n:] == 0)
+        lo = 0
+        if mode == "hard":      # row/column 0 (c^_0 = p_{i-1} is fixed) is zero up to rounding on both sides
+            lo = 1
+            assert max(np.abs(Pm_ref[0]).max(), np.abs(Pm_ref[:, 0]).max(), np.abs(Pm[0]).max()) < 1e-12 * np.abs(Pm_ref).max()
+        scale = np.sqrt(np.abs(np.diag(Pm_ref)))[lo:]
+        errP = np.abs((Pm[lo:n, lo:n] - Pm_ref[lo:, lo:]) / (scale[:, None] * scale[None, :])).max()
+        assert errP < 1e-10, (T, rho, errP)
+        assert np.abs(c0[:n] - c0_ref).max() < 1e-10 * max(1.0, np.abs(c0_ref).max()), (T, rho)
+
+
+def test_hard_mode_operator_keeps_the_waypoints():
+    """Pm^ maps into polynomials vanishing at both ends and c0^ hits the waypoints: E_w Pm^ = 0, E_w c0^ = p."""
+    for s in (3, 4):
+        n = 2 * s
+        p0, p1 = np.array([1.0, -2.0, 30.0]), np.array([4.0, 0.5, 28.0])
+        Pm, c0 = top.precompute_operator(s, 1.7, 10.0, p0, p1, box=True, vel=True, acc=True)
+        assert np.abs(Pm[0]).max() == 0.0
+        assert np.abs(Pm[:n, :n].sum(axis=0)).max() < 1e-14 * np.abs(Pm).max()
+        assert np.abs(c0[0] - p0).max() < 1e-13 and np.abs(c0[:n].sum(axis=0) - p1).max() < 1e-12
