@@ -45,12 +45,13 @@ struct top_solver {
     uint8_t* d_segflags = nullptr;
     void *d_zt = nullptr, *d_u = nullptr, *d_qp = nullptr, *d_qn = nullptr, *d_phv = nullptr, *d_wv = nullptr,
          *d_pha = nullptr, *d_wa = nullptr, *d_chat = nullptr, *d_Bedge = nullptr, *d_coef = nullptr;
-    unsigned char* d_sync = nullptr;   // [u64 barrier counter][u32 flag x max_ctas]
+    unsigned char* d_sync = nullptr;   // u64 grid-barrier counter
     int* d_abort = nullptr;
     double* h_res = nullptr;           // pinned [batch][4]
     int* h_abort = nullptr;            // pinned
     bool have_residuals = false;
     int64_t iter = 0, launches = 0;
+    unsigned long long seq_counter = 0;   // sweeps launched so far over all waves (mailbox sequence space)
     std::string err;
 };
 
@@ -444,9 +445,9 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     if (has_box) { ALLOC(h->d_qp, 3 * LS * rb, false); ALLOC(h->d_qn, 3 * LS * rb, false); }
     if (has_vel) { ALLOC(h->d_phv, 3 * LS * rb, false); ALLOC(h->d_wv, 3 * LS * rb, true); }
     if (has_acc) { ALLOC(h->d_pha, 3 * LS * rb, true); ALLOC(h->d_wa, 3 * LS * rb, true); }
-    ALLOC(h->d_Bedge, (size_t)2 * h->max_ctas * 24 * rb, true);
+    ALLOC(h->d_Bedge, (size_t)2 * h->max_ctas * 24 * 16, true);
     ALLOC(h->d_part, NP * 4 * 8, true); ALLOC(h->d_res, (size_t)batch * 4 * 8, true);
-    ALLOC(h->d_sync, 8 + (size_t)h->max_ctas * 4, true); ALLOC(h->d_abort, 16, true);
+    ALLOC(h->d_sync, 16, true); ALLOC(h->d_abort, 16, true);
     ALLOC(h->d_coef, (size_t)nseg * dims * n * rb, false);
 #undef ALLOC
     if (cudaMallocHost((void**)&h->h_res, (size_t)batch * 4 * 8) != cudaSuccess ||
@@ -503,13 +504,14 @@ top_status run_sweeps(top_solver* h, int64_t k) {
             p.pha = h->d_pha; p.wa = h->d_wa; p.chat = h->d_chat;
             p.Bedge = h->d_Bedge; p.part = h->d_part;
             p.bar = reinterpret_cast<unsigned long long*>(h->d_sync);
-            p.nflag = reinterpret_cast<unsigned int*>(h->d_sync + 8);
             p.abort_flag = h->d_abort;
             p.stride = h->stride; p.nseg_pad = h->nseg_pad; p.seg_begin = w.seg_begin; p.seg_end = w.seg_end;
             p.segs_per_cta = w.segs_per_cta; p.k_sweeps = kk; p.flags = h->kflags | sync_flag(h);
             p.max_ctas = h->max_ctas; p.rho = h->rho; p.vmax = h->vmax; p.amax = h->amax;
-            if (w.ctas > 1)
-                CU(cudaMemsetAsync(h->d_sync, 0, 8 + (size_t)h->max_ctas * 4, h->stream), "cudaMemsetAsync");
+            p.seq_base = (unsigned int)(h->seq_counter & 0xffffffffull);
+            h->seq_counter += (unsigned long long)kk;
+            if (w.ctas > 1 && !(p.flags & KF_NEIGHBOUR_SYNC))
+                CU(cudaMemsetAsync(h->d_sync, 0, 8, h->stream), "cudaMemsetAsync");
             CU(launch_sweeps(p, h->dtype, h->s, h->constrained, w.ctas, w.threads, w.smem, h->stream), "sweep kernel launch");
             h->launches += 1;
         }

@@ -41,10 +41,9 @@ struct KParams {
     void* wa;               // Real [DIMS][stride]
     void* chat;             // Real [DIMS][stride]  coefficient row `lane` in normalised time (c^_a = c_a T^a)
     // ---- exchange / reduction
-    void* Bedge;            // Real [2 parity][max_ctas][2 sides][4][DIMS]  boundary rows at chunk edges
+    void* Bedge;            // mailbox [2 parity][max_ctas][2 sides][4][DIMS] x 16-byte LL slots: boundary rows at CTA edges
     double* part;           // [nseg_pad][4]  per-segment residual partial sums (rp2, rd2, rdn2, gap2)
     unsigned long long* bar;// [0] grid barrier counter (reset before each launch)
-    unsigned int* nflag;    // [max_ctas]  neighbour flags: sweeps published by each CTA (reset before each launch)
     int* abort_flag;        // set when a barrier wait times out
     // ---- sizes
     long long stride;       // lanes per field (>= nseg_pad * LANES)
@@ -54,6 +53,7 @@ struct KParams {
     int k_sweeps;
     uint32_t flags;
     int max_ctas;
+    unsigned int seq_base;  // sweeps launched before this launch (mod 2^32): mailbox sequence numbers never repeat
     double rho, vmax, amax;
 };
 

@@ -2,8 +2,8 @@
 //
 // One launch runs k sweeps of Algorithm 1 (closed-form branch) over a contiguous range of
 // segments.  Mapping:
-//   * one CTA owns `segs_per_cta` consecutive segments for the whole launch; their state stays in shared
-//     memory / registers across all k sweeps (HBM is touched at launch start and end only);
+//   * one CTA owns `segs_per_cta` consecutive segments for the whole launch; their state stays in registers
+//     across all k sweeps (HBM is touched at launch start and end only);
 //   * 8 lanes per segment: lane j owns inequality sample j (its box slack pair and velocity / acceleration
 //     ball variables, 3 dims), lane a owns coefficient row a and consensus row a (u, z~);
 //   * the internal basis is normalised time, c^_a = c_a T^a (an exact change of variable of Eq. 18), so the
@@ -11,10 +11,14 @@
 //     segment, scaled by 1/T^k per derivative order k;
 //   * a sweep is split at its only cross-segment dependency (the neighbour read of Eq. 20b):
 //       phase A (segment local):  x-update (20a), phi/w (20f,g), slack + its dual (20d,e), boundary B = M c
-//       exchange: neighbours inside the CTA through shared memory, across CTAs through an L2 mailbox
+//         - the right-hand side is a lane -> row reduce-scatter through warp shuffles (no tables: the rows of
+//           E_k' are powers of the lane's own sample time), the two all-gathers (rhs rows, coefficient rows) go
+//           through shared memory with broadcast 128-bit reads, evaluation is repeated synthetic division;
+//       exchange: neighbours inside the CTA through shared memory, across CTAs through an L2 mailbox of
+//         16-byte "LL" slots {lo32, seq, hi32, seq} (the value is its own flag: no fence, no L1 invalidation)
 //       phase B:                  z-update (20b), u-update (20c), residual partial sums (Eq. 21-22)
-//   * CTAs synchronise once per sweep: either a grid-wide barrier or release/acquire flags with the two
-//     neighbouring CTAs only (the dependency radius of a sweep is exactly one segment).
+//   * CTAs synchronise once per sweep through that mailbox with their two neighbouring CTAs only (the dependency
+//     radius of a sweep is exactly one segment); a grid-wide barrier per sweep is kept as an option.
 #include <cooperative_groups.h>
 #include <cuda_runtime.h>
 #include <math.h>
@@ -27,24 +31,14 @@ namespace {
 
 // ------------------------------------------------------------------------------------------------ helpers
 
-template <typename Real> struct Traits;
-template <> struct Traits<double> { static constexpr int GSTRIDE = 98; };   // Reals of per-segment scratch (padded:
-template <> struct Traits<float>  { static constexpr int GSTRIDE = 100; };  //  4 segments of a warp hit distinct banks)
-
-constexpr int GSLOT = 12;  // per lane: gM[3], g0[3], g1[3], g2[3]
+// per-segment strides of the all-gather buffers (24 values used; padded so that the four segments of a warp
+// read distinct 16-byte bank groups): rhs rows in doubles; coefficient rows 26 doubles / 28 floats
+constexpr int XSTRIDE = 26;
 
 __device__ __forceinline__ unsigned long long ld_acquire_u64(const unsigned long long* p) {
     unsigned long long v;
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
-}
-__device__ __forceinline__ unsigned int ld_acquire_u32(const unsigned int* p) {
-    unsigned int v;
-    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void st_release_u32(unsigned int* p, unsigned int v) {
-    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
 }
 __device__ __forceinline__ long long global_ns() {
     long long t;
@@ -81,13 +75,28 @@ __device__ __forceinline__ bool grid_barrier(unsigned long long* bar, unsigned l
     return ok_sh != 0;
 }
 
-// wait until CTA `who` has published sweep `want` (neighbour synchronisation)
-__device__ __forceinline__ bool wait_flag(const unsigned int* flag, unsigned int want, int* abort_flag) {
-    if (ld_acquire_u32(flag) >= want) return true;
+// ---- inter-CTA mailbox: "LL" slots.  One 16-byte slot carries one fp64 value as {lo32, seq, hi32, seq}, written
+// with a single 128-bit store and read with a single 128-bit load; each aligned 8-byte half is atomic, so a
+// reader that sees `seq` in both halves has the whole value.  No fence, no separate flag: the data is the flag,
+// and neither side invalidates L1 (an acquire/fence at gpu scope would: CCTL.IVALL).
+__device__ __forceinline__ void ll_store(void* slot, double v, unsigned seq) {
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(slot), "r"((unsigned)b), "r"(seq),
+                 "r"((unsigned)(b >> 32)), "r"(seq) : "memory");
+}
+__device__ __forceinline__ bool ll_try_load(const void* slot, unsigned seq, double& v) {
+    unsigned a, f0, b, f1;
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(f0), "=r"(b), "=r"(f1) : "l"(slot) : "memory");
+    v = __longlong_as_double((long long)(((unsigned long long)b << 32) | a));
+    return f0 == seq && f1 == seq;
+}
+// spin until the slot carries `seq`; bounded (returns false after WAIT_TIMEOUT_NS or when another CTA aborted)
+__device__ __forceinline__ bool ll_wait(const void* slot, unsigned seq, double& v, int* abort_flag) {
+    if (ll_try_load(slot, seq, v)) return true;
     const long long t0 = global_ns();
     unsigned spins = 0;
-    while (ld_acquire_u32(flag) < want) {
-        if ((++spins & 1023u) == 0) {
+    while (!ll_try_load(slot, seq, v)) {
+        if ((++spins & 255u) == 0) {
             if (*(volatile int*)abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS) {
                 atomicExch(abort_flag, 1);
                 return false;
@@ -110,26 +119,6 @@ __device__ __forceinline__ double beta_entry(int k, int a, double tau) {
     return f * pw;
 }
 
-// table entry (row r, coefficient a, kind): kind 0 = consensus row r of M (derivative r%S at tau = 0 for r < S,
-// at tau = 1 for S <= r < 2S); kind 1..3 = sample r of E_0, E_1, E_2 at tau_r = (r+1)/(MS+1)  (reading A10)
-template <int S> __device__ __forceinline__ double table_entry(int r, int a, int kind) {
-    if (a >= 2 * S) return 0.0;
-    if (kind == 0) {
-        if (r >= 2 * S) return 0.0;
-        return beta_entry(r % S, a, r < S ? 0.0 : 1.0);
-    }
-    return beta_entry(kind - 1, a, (double)(r + 1) / (double)(MS + 1));
-}
-
-// projection onto the Euclidean ball ||y|| <= bound  (Eq. 14 / 20f; reading A15: y = 0 -> scale 1)
-template <typename Real>
-__device__ __forceinline__ void project_ball(const Real (&y)[3], Real bound, Real (&phi)[3]) {
-    const Real n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
-    Real scale = (Real)1;
-    if (n2 > bound * bound) scale = bound / sqrt(n2);
-    phi[0] = scale * y[0]; phi[1] = scale * y[1]; phi[2] = scale * y[2];
-}
-
 template <typename Real> __device__ __forceinline__ Real shfl_xor(Real v, int m) { return __shfl_xor_sync(0xffffffffu, v, m); }
 
 }  // namespace
@@ -140,32 +129,66 @@ namespace {
 
 // shared-memory carve-up, identical on host (size) and device (pointers)
 struct SmemLayout {
-    size_t pm, tabA, tabJ, gs, bs, segc, sst, total;
-    int nsample_fields;
+    size_t pm, bco, lohi, xs, cs, bs, total;
 };
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
-__host__ __device__ inline SmemLayout smem_layout(int real_bytes, int S, bool cons, uint32_t flags, int segs, int gstride) {
+__host__ __device__ inline SmemLayout smem_layout(int real_bytes, int S, bool cons, int segs) {
     SmemLayout L;
+    const int CSTRIDE = real_bytes == 8 ? 26 : 28;
     const int T = segs * LANES;
     size_t off = 0;
-    L.pm = off;   off = align16(off + (size_t)2 * S * T * sizeof(double));
-    L.tabA = off; off = align16(off + (size_t)8 * 8 * 4 * real_bytes);
-    L.tabJ = off; off = align16(off + (size_t)8 * 8 * 4 * real_bytes);
-    L.gs = off;   off = align16(off + (size_t)segs * gstride * real_bytes);
-    L.bs = off;   off = align16(off + (size_t)2 * (segs + 2) * 24 * real_bytes);
-    L.segc = off; off = align16(off + (size_t)8 * segs * real_bytes);
-    int nf = 0;
-    if (cons) nf = ((flags & KF_BOX) ? 6 : 0) + ((flags & KF_VEL) ? 6 : 0) + ((flags & KF_ACC) ? 6 : 0);
-    L.nsample_fields = nf;
-    L.sst = off;  off = align16(off + (size_t)nf * T * real_bytes);
+    L.pm = off;   off = align16(off + (size_t)2 * S * T * sizeof(double));           // rho*Pm^ rows, [b][thread]
+    L.bco = off;  off = align16(off + (size_t)8 * 8 * real_bytes);                     // consensus-row coefficients [a][lane]
+    L.lohi = off; off = align16(off + (size_t)(cons ? 6 : 0) * segs * real_bytes);     // box lo[3], hi[3] per segment
+    L.xs = off;   off = align16(off + (size_t)segs * XSTRIDE * sizeof(double));        // rhs rows, all-gather
+    L.cs = off;   off = align16(off + (size_t)segs * CSTRIDE * real_bytes);            // coefficient rows, all-gather
+    L.bs = off;   off = align16(off + (size_t)2 * (segs + 2) * 24 * real_bytes);       // boundary rows, double buffered
     L.total = off;
     return L;
+}
+
+template <typename Real> __device__ __forceinline__ Real sel(bool c, Real a, Real b) { return c ? a : b; }
+
+// Reduce-scatter of v[0..7] over the 8 lanes of a segment: afterwards lane a holds sum_j v_j[a].
+// Three xor-butterfly stages (4 + 2 + 1 shuffles); the order of additions is fixed per lane (deterministic).
+template <typename Real>
+__device__ __forceinline__ Real reduce_scatter8(const Real (&v)[8], int lane) {
+    const bool b2 = lane & 4, b1 = lane & 2, b0 = lane & 1;
+    Real w[4], x[2];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const Real send = sel(b2, v[i], v[i + 4]), keep = sel(b2, v[i + 4], v[i]);
+        w[i] = keep + shfl_xor(send, 4);
+    }
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+        const Real send = sel(b1, w[i], w[i + 2]), keep = sel(b1, w[i + 2], w[i]);
+        x[i] = keep + shfl_xor(send, 2);
+    }
+    const Real send = sel(b0, x[0], x[1]), keep = sel(b0, x[1], x[0]);
+    return keep + shfl_xor(send, 1);
+}
+
+template <typename Real> __device__ __forceinline__ Real rsqrt_real(Real x);
+template <> __device__ __forceinline__ double rsqrt_real<double>(double x) { return rsqrt(x); }
+template <> __device__ __forceinline__ float rsqrt_real<float>(float x) { return rsqrtf(x); }
+
+// Eq. 20f, 20g: y = A c + w;  phi = projection of y onto ||.|| <= bound (reading A15);  w = y - phi
+template <typename Real>
+__device__ __forceinline__ void ball_update(const Real (&val)[3], Real bound, Real (&phi)[3], Real (&w)[3]) {
+    Real y[3];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) y[d] = val[d] + w[d];
+    const Real n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+    Real scale = (Real)1;
+    if (n2 > bound * bound) scale = bound * rsqrt_real<Real>(n2);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) { phi[d] = scale * y[d]; w[d] = y[d] - phi[d]; }
 }
 
 template <typename Real, int S, bool CONS, int MAXT>
 __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) {
     constexpr int N2 = 2 * S;                      // n = 2s coefficients = 2s consensus rows per segment
-    constexpr int GST = Traits<Real>::GSTRIDE;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int T = blockDim.x, tid = threadIdx.x, lane = tid & (LANES - 1), sl = tid >> 3;
@@ -176,215 +199,196 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     const bool pin_pos = flags & KF_PIN_POS;
     const bool nb_sync = flags & KF_NEIGHBOUR_SYNC;
 
-    const SmemLayout L = smem_layout((int)sizeof(Real), S, CONS, flags, SEGS, GST);
+    const SmemLayout L = smem_layout((int)sizeof(Real), S, CONS, SEGS);
     double* Pms = reinterpret_cast<double*>(smem_raw + L.pm);
-    Real* tabA = reinterpret_cast<Real*>(smem_raw + L.tabA);   // [row/sample j][coef a][kind]
-    Real* tabJ = reinterpret_cast<Real*>(smem_raw + L.tabJ);   // [coef b][row/sample j][kind]
-    Real* Gs = reinterpret_cast<Real*>(smem_raw + L.gs);
+    Real* bco = reinterpret_cast<Real*>(smem_raw + L.bco);     // [a][lane]: beta_k(tau_b)[a] of consensus row `lane`
+    Real* lohi = reinterpret_cast<Real*>(smem_raw + L.lohi);   // [6][SEGS]
+    double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE;   // this segment: [d][a]
+    Real* Cs = reinterpret_cast<Real*>(smem_raw + L.cs) + (size_t)sl * (sizeof(Real) == 8 ? 26 : 28);   // this segment: [d][a]
     Real* Bs = reinterpret_cast<Real*>(smem_raw + L.bs);       // [2 parity][SEGS+2][8 rows][3]
-    Real* segc = reinterpret_cast<Real*>(smem_raw + L.segc);   // [8][SEGS]: 1/T, 1/T^2, lo[3], hi[3]
-    Real* sst = reinterpret_cast<Real*>(smem_raw + L.sst);     // [field][T] per-lane sample state
-    // sample-state field offsets (in units of T)
-    const int F_QP = 0, F_QN = 3;
-    const int F_PHV = has_box ? 6 : 0, F_WV = F_PHV + 3;
-    const int F_PHA = F_PHV + (has_vel ? 6 : 0), F_WA = F_PHA + 3;
 
     const long long cta_first = p.seg_begin + (long long)cta * SEGS;
     const long long remaining = p.seg_end - cta_first;
     const int nact = remaining < SEGS ? (int)remaining : SEGS;     // active segments of this CTA (>= 1)
     const bool active = sl < nact;
-    const long long gseg = active ? cta_first + sl : cta_first;     // inactive threads alias a valid segment (loads only)
+    // inactive lanes of a ragged CTA compute on a copy of the CTA's first segment (shuffles need full warps)
+    // and never write to global memory
+    const long long gseg = active ? cta_first + sl : cta_first;
     const long long gt = gseg * LANES + lane;
     const long long stride = p.stride;
     const bool isrow = lane < N2;
     const bool right = lane >= S;
     const int korder = right ? lane - S : lane;
 
-    // ---- tables (same for every segment: normalised time)
-    for (int idx = tid; idx < 8 * 8 * 4; idx += T) {
-        const int kind = idx & 3, a = (idx >> 2) & 7, r = idx >> 5;
-        const Real v = (Real)table_entry<S>(r, a, kind);
-        tabA[(r * 8 + a) * 4 + kind] = v;
-        tabJ[(a * 8 + r) * 4 + kind] = v;
-    }
     // ---- constants
+    for (int idx = tid; idx < 64; idx += T) {
+        const int a = idx >> 3, r = idx & 7;
+        double v = 0.0;
+        if (r < N2 && a < N2) v = beta_entry(r % S, a, r < S ? 0.0 : 1.0);
+        bco[a * 8 + r] = (Real)v;
+    }
 #pragma unroll
     for (int b = 0; b < N2; ++b) Pms[b * T + tid] = p.Pm[b * stride + gt];
     double c0[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) c0[d] = p.c0[d * stride + gt];
     const Real invTk = static_cast<const Real*>(p.invTk)[gt];
-    if (active) {
-        Real v;
-        if (lane < 2) v = static_cast<const Real*>(p.invT)[lane * p.nseg_pad + gseg];
-        else v = static_cast<const Real*>(p.lohi)[(lane - 2) * p.nseg_pad + gseg];
-        segc[lane * SEGS + sl] = v;
-    }
+    const Real invT = static_cast<const Real*>(p.invT)[gseg], invT2 = static_cast<const Real*>(p.invT)[p.nseg_pad + gseg];
+    if (CONS && lane < 6) lohi[lane * SEGS + sl] = static_cast<const Real*>(p.lohi)[lane * p.nseg_pad + gseg];
     const uint8_t sf = p.segflags[gseg];
+    const Real tau = (Real)((double)(lane + 1) / (double)(MS + 1));       // sample time of this lane (reading A10)
+    const Real itau2 = (Real)(1.0 / (((double)(lane + 1) / (double)(MS + 1)) * ((double)(lane + 1) / (double)(MS + 1))));
     // ---- state of iterate k
-    Real zt[3], u[3], chat[3];
+    Real zt[3], u[3], qp[3], qn[3], phv[3], wv[3], pha[3], wa[3];
 #pragma unroll
     for (int d = 0; d < 3; ++d) {
         zt[d] = static_cast<const Real*>(p.zt)[d * stride + gt];
         u[d] = static_cast<const Real*>(p.u)[d * stride + gt];
-        chat[d] = static_cast<const Real*>(p.chat)[d * stride + gt];
-    }
-    if (CONS) {
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            if (has_box) {
-                sst[(F_QP + d) * T + tid] = static_cast<const Real*>(p.qp)[d * stride + gt];
-                sst[(F_QN + d) * T + tid] = static_cast<const Real*>(p.qn)[d * stride + gt];
-            }
-            if (has_vel) {
-                sst[(F_PHV + d) * T + tid] = static_cast<const Real*>(p.phv)[d * stride + gt];
-                sst[(F_WV + d) * T + tid] = static_cast<const Real*>(p.wv)[d * stride + gt];
-            }
-            if (has_acc) {
-                sst[(F_PHA + d) * T + tid] = static_cast<const Real*>(p.pha)[d * stride + gt];
-                sst[(F_WA + d) * T + tid] = static_cast<const Real*>(p.wa)[d * stride + gt];
-            }
-        }
+        qp[d] = has_box ? static_cast<const Real*>(p.qp)[d * stride + gt] : (Real)0;
+        qn[d] = has_box ? static_cast<const Real*>(p.qn)[d * stride + gt] : (Real)0;
+        phv[d] = has_vel ? static_cast<const Real*>(p.phv)[d * stride + gt] : (Real)0;
+        wv[d] = has_vel ? static_cast<const Real*>(p.wv)[d * stride + gt] : (Real)0;
+        pha[d] = has_acc ? static_cast<const Real*>(p.pha)[d * stride + gt] : (Real)0;
+        wa[d] = has_acc ? static_cast<const Real*>(p.wa)[d * stride + gt] : (Real)0;
     }
     __syncthreads();
 
-    const Real invT = segc[0 * SEGS + (active ? sl : 0)], invT2 = segc[1 * SEGS + (active ? sl : 0)];
-    const Real rho = (Real)p.rho, vmax = (Real)p.vmax, amax = (Real)p.amax;
-    Real* const G = Gs + (size_t)sl * GST;                 // this segment's scratch
-    double* const X = reinterpret_cast<double*>(G);         // [8][3] rhs rows (aliases the g slots)
-    Real* const Cs = G + 48;                                // [8][3] coefficient rows
-    Real* const Bedge = static_cast<Real*>(p.Bedge);
-    const size_t edge_par_stride = (size_t)p.max_ctas * 2 * 4 * 3;
+    const Real vmax = (Real)p.vmax, amax = (Real)p.amax;
+    // mailbox: [2 parity][max_ctas][2 sides][4 rows][3 dims] LL slots of 16 bytes
+    unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
+    const size_t mbox_par_stride = (size_t)p.max_ctas * 24 * 16;
+    Real bc[N2];                               // consensus-row coefficients of this lane: M^[lane][a] = bc[a] / T^k
+#pragma unroll
+    for (int a = 0; a < N2; ++a) bc[a] = bco[a * 8 + lane];
 
-    int wait_failed = 0;
+    __shared__ int abort_sh[2];
+    if (tid < 2) abort_sh[tid] = 0;
+    __syncthreads();
     for (int it = 0; it < p.k_sweeps; ++it) {
-        const int par = it & 1;
+        int wait_failed = 0;
+        const unsigned seq = p.seq_base + (unsigned)it + 1u;     // launch-unique sweep number (never reused)
+        const int par = (int)(seq & 1u);
         const bool last_sweep = (it == p.k_sweeps - 1);
         Real* const Bcur = Bs + (size_t)par * (SEGS + 2) * 24;
 
         // ================= phase A: segment local =================
-        // right-hand side of Eq. 20a (second bracket; rho is applied with the operator, reading A3)
-        if (active) {
-            Real* g = G + lane * GSLOT;
+        // a1: right-hand side of Eq. 20a (second bracket; rho is folded into the operator, A3).
+        // Lane j adds the terms of ITS sample j and ITS consensus row to all n rows, then the 8 lanes
+        // reduce-scatter: lane a ends with row a.  In normalised time row a of E_k' at tau is
+        // a!/(a-k)! tau^(a-k) / T^k, so  contribution_a = tau^(a-2) (tau^2 g0 + a tau g1/T + a(a-1) g2/T^2).
+        Real R[3];
 #pragma unroll
-            for (int d = 0; d < 3; ++d) g[d] = isrow ? (zt[d] - u[d]) * invTk : (Real)0;   // M'(z~ - u)
+        for (int d = 0; d < 3; ++d) {
+            const Real gM = isrow ? (zt[d] - u[d]) * invTk : (Real)0;               // M'(z~ - u)
+            Real v[8];
             if (CONS) {
+                Real A0 = 0, A1 = 0, A2 = 0;
+                if (has_box) {      // Ao'(b - s - v), Ao = [E0; -E0], b = [hi; -lo];  s + v = |q| (Moreau pair)
+                    const Real lo = lohi[d * SEGS + sl], hi = lohi[(3 + d) * SEGS + sl];
+                    A0 = ((hi - fabs(qp[d])) + (lo + fabs(qn[d]))) * (tau * tau);
+                }
+                if (has_vel) A1 = (phv[d] - wv[d]) * (invT * tau);                   // Av'(phi - w), velocity
+                if (has_acc) A2 = (pha[d] - wa[d]) * invT2;                          //               acceleration
+                Real tp = itau2;                                                      // tau^(a-2)
 #pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    Real g0 = 0, g1 = 0, g2 = 0;
-                    if (has_box) {      // Ao'(b - s - v), Ao = [E0; -E0], b = [hi; -lo];  s + v = |q| (Moreau pair)
-                        const Real lo = segc[(2 + d) * SEGS + sl], hi = segc[(5 + d) * SEGS + sl];
-                        g0 = (hi - fabs(sst[(F_QP + d) * T + tid])) + (lo + fabs(sst[(F_QN + d) * T + tid]));
+                for (int a = 0; a < 8; ++a) {
+                    if (a < N2) {
+                        const Real inner = A0 + (Real)a * A1 + (Real)(a * (a - 1)) * A2;
+                        v[a] = tp * inner + bc[a] * gM;
+                        tp *= tau;
+                    } else {
+                        v[a] = (Real)0;
                     }
-                    if (has_vel) g1 = (sst[(F_PHV + d) * T + tid] - sst[(F_WV + d) * T + tid]) * invT;    // Av'(phi - w)
-                    if (has_acc) g2 = (sst[(F_PHA + d) * T + tid] - sst[(F_WA + d) * T + tid]) * invT2;
-                    g[3 + d] = g0; g[6 + d] = g1; g[9 + d] = g2;
                 }
+            } else {
+#pragma unroll
+                for (int a = 0; a < 8; ++a) v[a] = a < N2 ? bc[a] * gM : (Real)0;
             }
+            R[d] = reduce_scatter8(v, lane);
         }
-        __syncwarp();
-        Real R[3] = {0, 0, 0};
-        if (active) {
 #pragma unroll
-            for (int j = 0; j < (CONS ? 8 : N2); ++j) {
-                const Real* gj = G + j * GSLOT;
-                const Real* t = tabA + (j * 8 + lane) * 4;
-#pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    if (CONS) R[d] += t[0] * gj[d] + t[1] * gj[3 + d] + t[2] * gj[6 + d] + t[3] * gj[9 + d];
-                    else R[d] += t[0] * gj[d];
-                }
-            }
-        }
+        for (int d = 0; d < 3; ++d) Xs[d * 8 + lane] = (double)R[d];
         __syncwarp();
-        if (active) {
-#pragma unroll
-            for (int d = 0; d < 3; ++d) X[lane * 3 + d] = (double)R[d];
-        }
-        __syncwarp();
-        // x-update: c^ = (rho Pm^) R^ + c0^   (Eq. 20a, first bracket precomputed per segment from T_i; fp64 always)
-        if (active) {
+        // a2: x-update  c^ = (rho Pm^) R^ + c0^   (Eq. 20a first bracket, precomputed per segment; fp64 always)
+        {
             double c[3] = {c0[0], c0[1], c0[2]};
 #pragma unroll
-            for (int b = 0; b < N2; ++b) {
-                const double pm = Pms[b * T + tid];
+            for (int d = 0; d < 3; ++d) {
+                double x[N2];
 #pragma unroll
-                for (int d = 0; d < 3; ++d) c[d] += pm * X[b * 3 + d];
+                for (int b = 0; b < N2; b += 2) {
+                    const double2 t = *reinterpret_cast<const double2*>(Xs + d * 8 + b);
+                    x[b] = t.x; x[b + 1] = t.y;
+                }
+#pragma unroll
+                for (int b = 0; b < N2; ++b) c[d] += Pms[b * T + tid] * x[b];
             }
 #pragma unroll
-            for (int d = 0; d < 3; ++d) { chat[d] = (Real)c[d]; Cs[lane * 3 + d] = chat[d]; }
+            for (int d = 0; d < 3; ++d) Cs[d * 8 + lane] = (Real)c[d];
+            if (last_sweep && active) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) static_cast<Real*>(p.chat)[d * stride + gt] = (Real)c[d];
+            }
         }
         __syncwarp();
-        Real Bnd[3] = {0, 0, 0};
-        if (active) {
-            Real C[N2][3];
+        // a3: evaluate the new polynomial: consensus row `lane` of B = M c, and sample `lane` of E0 c, E1 c, E2 c
+        Real Bnd[3], Pv[3], Vv[3], Av[3];
 #pragma unroll
-            for (int b = 0; b < N2; ++b)
+        for (int d = 0; d < 3; ++d) {
+            Real C[8];
+            if (sizeof(Real) == 8) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) C[b][d] = Cs[b * 3 + d];
-            // boundary derivative row `lane` of B = M c  (Eq. 20b's sigma~)
-            if (isrow) {
-                Real acc[3] = {0, 0, 0};
-#pragma unroll
-                for (int b = 0; b < N2; ++b) {
-                    const Real m = tabJ[(b * 8 + lane) * 4 + 0];
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) acc[d] += m * C[b][d];
+                for (int b = 0; b < N2; b += 2) {
+                    const double2 t = *reinterpret_cast<const double2*>(Cs + d * 8 + b);
+                    C[b] = (Real)t.x; C[b + 1] = (Real)t.y;
                 }
+            } else {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    Bnd[d] = acc[d] * invTk;
-                    Bcur[(sl + 1) * 24 + lane * 3 + d] = Bnd[d];
-                }
-                if (nctas > 1) {
-                    Real* e = Bedge + par * edge_par_stride + (size_t)cta * 24;
-                    if (sl == 0 && !right) {
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) stcg(e + 0 * 12 + korder * 3 + d, Bnd[d]);
-                    }
-                    if (sl == nact - 1 && right) {
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) stcg(e + 1 * 12 + korder * 3 + d, Bnd[d]);
-                    }
+                for (int b = 0; b < N2; b += 2) {
+                    const float2 t = *reinterpret_cast<const float2*>(Cs + d * 8 + b);
+                    C[b] = (Real)t.x; C[b + 1] = (Real)t.y;
                 }
             }
+            Real acc = 0;
+#pragma unroll
+            for (int b = 0; b < N2; ++b) acc += bc[b] * C[b];
+            Bnd[d] = acc * invTk;
             if (CONS) {
-                Real P[3] = {0, 0, 0}, V[3] = {0, 0, 0}, A[3] = {0, 0, 0};
+                // repeated synthetic division at tau: value, first derivative, second derivative / 2
 #pragma unroll
-                for (int b = 0; b < N2; ++b) {
-                    const Real* t = tabJ + (b * 8 + lane) * 4;
+                for (int b = N2 - 2; b >= 0; --b) C[b] += tau * C[b + 1];
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) {
-                        if (has_box) P[d] += t[1] * C[b][d];
-                        if (has_vel) V[d] += t[2] * C[b][d];
-                        if (has_acc) A[d] += t[3] * C[b][d];
-                    }
+                for (int b = N2 - 2; b >= 1; --b) C[b] += tau * C[b + 1];
+#pragma unroll
+                for (int b = N2 - 2; b >= 2; --b) C[b] += tau * C[b + 1];
+                Pv[d] = C[0]; Vv[d] = C[1] * invT; Av[d] = (C[2] + C[2]) * invT2;
+            }
+        }
+        if (isrow) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) Bcur[(sl + 1) * 24 + lane * 3 + d] = Bnd[d];
+            if (nctas > 1 && active) {      // publish the rows the neighbouring CTAs need, as early as possible
+                unsigned char* e = mbox + par * mbox_par_stride + (size_t)cta * 24 * 16;
+                if (sl == 0 && !right && cta > 0) {
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) ll_store(e + (0 * 12 + korder * 3 + d) * 16, (double)Bnd[d], seq);
                 }
-                if (has_vel) {      // Eq. 20f, 20g: y = Av c + w;  phi = proj(y);  w = y - phi
-                    Real Y[3], phi[3];
+                if (sl == nact - 1 && right && cta + 1 < nctas) {
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) Y[d] = V[d] * invT + sst[(F_WV + d) * T + tid];
-                    project_ball(Y, vmax, phi);
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) { sst[(F_PHV + d) * T + tid] = phi[d]; sst[(F_WV + d) * T + tid] = Y[d] - phi[d]; }
+                    for (int d = 0; d < 3; ++d) ll_store(e + (1 * 12 + korder * 3 + d) * 16, (double)Bnd[d], seq);
                 }
-                if (has_acc) {
-                    Real Y[3], phi[3];
+            }
+        }
+        if (CONS) {
+            if (has_vel) ball_update(Vv, vmax, phv, wv);      // a4: Eq. 20f, 20g
+            if (has_acc) ball_update(Av, amax, pha, wa);
+            if (has_box) {      // a7 + a8: Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q)
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) Y[d] = A[d] * invT2 + sst[(F_WA + d) * T + tid];
-                    project_ball(Y, amax, phi);
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) { sst[(F_PHA + d) * T + tid] = phi[d]; sst[(F_WA + d) * T + tid] = Y[d] - phi[d]; }
-                }
-                if (has_box) {      // Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q)
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) {
-                        const Real lo = segc[(2 + d) * SEGS + sl], hi = segc[(5 + d) * SEGS + sl];
-                        const Real qp = sst[(F_QP + d) * T + tid], qn = sst[(F_QN + d) * T + tid];
-                        const Real vp = qp < 0 ? -qp : (Real)0, vn = qn < 0 ? -qn : (Real)0;
-                        sst[(F_QP + d) * T + tid] = (hi - P[d]) - vp;
-                        sst[(F_QN + d) * T + tid] = (P[d] - lo) - vn;
-                    }
+                for (int d = 0; d < 3; ++d) {
+                    const Real lo = lohi[d * SEGS + sl], hi = lohi[(3 + d) * SEGS + sl];
+                    const Real vp = qp[d] < 0 ? -qp[d] : (Real)0, vn = qn[d] < 0 ? -qn[d] : (Real)0;
+                    qp[d] = (hi - Pv[d]) - vp;
+                    qn[d] = (Pv[d] - lo) - vn;
                 }
             }
         }
@@ -395,66 +399,59 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
         } else if (!nb_sync) {
             if (!grid_barrier(p.bar, (unsigned long long)(it + 1) * nctas, p.abort_flag)) break;   // uniform per CTA
         } else {
-            if (__syncthreads_or(wait_failed)) break;       // a wait of the previous sweep timed out: give up together
-            if (tid == 0) { __threadfence(); st_release_u32(p.nflag + cta, (unsigned)(it + 1)); }
-            if (active && isrow) {
-                if (sl == 0 && !right && cta > 0)
-                    wait_failed |= !wait_flag(p.nflag + cta - 1, (unsigned)(it + 1), p.abort_flag);
-                if (sl == nact - 1 && right && cta + 1 < nctas)
-                    wait_failed |= !wait_flag(p.nflag + cta + 1, (unsigned)(it + 1), p.abort_flag);
-            }
+            // a mailbox wait of the previous sweep timed out: give up together.  The flag is double buffered by
+            // sweep parity so that every thread of the CTA reads the same value after this barrier.
+            __syncthreads();
+            if (abort_sh[(it + 1) & 1]) break;
         }
 
         // ================= phase B: consensus, dual, residuals =================
         double rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
         Real dz[3] = {0, 0, 0};
-        if (active && isrow) {
+        if (isrow) {
             Real nb[3];
-            if (nctas > 1 && sl == 0 && !right) {             // left neighbour lives in the previous CTA
-                const Real* e = Bedge + par * edge_par_stride + (size_t)(cta > 0 ? cta - 1 : 0) * 24 + 1 * 12 + korder * 3;
+            if (active && sl == 0 && !right && cta > 0) {                // left neighbour lives in the previous CTA
+                const unsigned char* e = mbox + par * mbox_par_stride + (size_t)(cta - 1) * 24 * 16 + (1 * 12 + korder * 3) * 16;
 #pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] = ldcg(e + d);
-            } else if (nctas > 1 && sl == nact - 1 && right) { // right neighbour lives in the next CTA
-                const Real* e = Bedge + par * edge_par_stride + (size_t)(cta + 1 < nctas ? cta + 1 : cta) * 24 + 0 * 12 + korder * 3;
+                for (int d = 0; d < 3; ++d) { double t; wait_failed |= !ll_wait(e + d * 16, seq, t, p.abort_flag); nb[d] = (Real)t; }
+            } else if (active && sl == nact - 1 && right && cta + 1 < nctas) {   // right neighbour lives in the next CTA
+                const unsigned char* e = mbox + par * mbox_par_stride + (size_t)(cta + 1) * 24 * 16 + (0 * 12 + korder * 3) * 16;
 #pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] = ldcg(e + d);
+                for (int d = 0; d < 3; ++d) { double t; wait_failed |= !ll_wait(e + d * 16, seq, t, p.abort_flag); nb[d] = (Real)t; }
             } else {
                 const Real* e = right ? Bcur + (sl + 2) * 24 + korder * 3 : Bcur + sl * 24 + (korder + S) * 3;
 #pragma unroll
                 for (int d = 0; d < 3; ++d) nb[d] = e[d];
             }
+            if (wait_failed) abort_sh[it & 1] = 1;
             const bool fixed = (right ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder == 0);
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const Real bl = right ? Bnd[d] : nb[d], br = right ? nb[d] : Bnd[d];
-                const Real znew = fixed ? zt[d] : (Real)0.5 * (bl + br);      // Eq. 6b / 20b
+                const Real znew = fixed ? zt[d] : (Real)0.5 * (bl + br);      // a5: Eq. 6b / 20b
                 dz[d] = znew - zt[d];
                 zt[d] = znew;
                 const Real res = Bnd[d] - znew;
-                u[d] += res;                                                 // Eq. 6c / 20c (scaled dual, A5)
-                rp2 += (double)res * (double)res;
-                if (right && !(sf & SEG_LAST)) { const double gp = (double)Bnd[d] - (double)nb[d]; gap2 += gp * gp; }   // Eq. 21
+                u[d] += res;                                                 // a8: Eq. 6c / 20c (scaled dual, A5)
+                if (last_sweep) {
+                    rp2 += (double)res * (double)res;
+                    if (right && !(sf & SEG_LAST)) { const double gp = (double)Bnd[d] - (double)nb[d]; gap2 += gp * gp; }   // Eq. 21
+                }
             }
         }
         if (last_sweep) {
-            // dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8)
-            __syncwarp();
-            if (active) {
+            // a6: dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8):
+            // the same lane-to-row reduce-scatter as the right-hand side
+            const double Tp = (double)static_cast<const Real*>(p.Tpow)[gt];
 #pragma unroll
-                for (int d = 0; d < 3; ++d) G[lane * GSLOT + d] = isrow ? dz[d] * invTk : (Real)0;
-            }
-            __syncwarp();
-            if (active && isrow) {
-                const double Tp = (double)static_cast<const Real*>(p.Tpow)[gt];
+            for (int d = 0; d < 3; ++d) {
+                const Real gd = isrow ? dz[d] * invTk : (Real)0;
+                Real v[8];
 #pragma unroll
-                for (int d = 0; d < 3; ++d) {
-                    Real x = 0;
-#pragma unroll
-                    for (int r = 0; r < N2; ++r) x += tabA[(r * 8 + lane) * 4 + 0] * G[r * GSLOT + d];
-                    const double xr = p.rho * (double)x;
-                    rdn2 += xr * xr;
-                    rd2 += (xr * Tp) * (xr * Tp);
-                }
+                for (int a = 0; a < 8; ++a) v[a] = a < N2 ? bc[a] * gd : (Real)0;
+                const double xr = p.rho * (double)reduce_scatter8(v, lane);
+                rdn2 += xr * xr;
+                rd2 += (xr * Tp) * (xr * Tp);
             }
 #pragma unroll
             for (int m = 1; m < LANES; m <<= 1) {     // fixed-order tree over the 8 lanes of the segment
@@ -464,7 +461,6 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
                 double* o = p.part + gseg * 4;
                 o[0] = rp2; o[1] = rd2; o[2] = rdn2; o[3] = gap2;
             }
-            __syncwarp();
         }
     }
 
@@ -474,18 +470,17 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
         for (int d = 0; d < 3; ++d) {
             static_cast<Real*>(p.zt)[d * stride + gt] = zt[d];
             static_cast<Real*>(p.u)[d * stride + gt] = u[d];
-            static_cast<Real*>(p.chat)[d * stride + gt] = chat[d];
             if (has_box) {
-                static_cast<Real*>(p.qp)[d * stride + gt] = sst[(F_QP + d) * T + tid];
-                static_cast<Real*>(p.qn)[d * stride + gt] = sst[(F_QN + d) * T + tid];
+                static_cast<Real*>(p.qp)[d * stride + gt] = qp[d];
+                static_cast<Real*>(p.qn)[d * stride + gt] = qn[d];
             }
             if (has_vel) {
-                static_cast<Real*>(p.phv)[d * stride + gt] = sst[(F_PHV + d) * T + tid];
-                static_cast<Real*>(p.wv)[d * stride + gt] = sst[(F_WV + d) * T + tid];
+                static_cast<Real*>(p.phv)[d * stride + gt] = phv[d];
+                static_cast<Real*>(p.wv)[d * stride + gt] = wv[d];
             }
             if (has_acc) {
-                static_cast<Real*>(p.pha)[d * stride + gt] = sst[(F_PHA + d) * T + tid];
-                static_cast<Real*>(p.wa)[d * stride + gt] = sst[(F_WA + d) * T + tid];
+                static_cast<Real*>(p.pha)[d * stride + gt] = pha[d];
+                static_cast<Real*>(p.wa)[d * stride + gt] = wa[d];
             }
         }
     }
@@ -605,9 +600,8 @@ cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int threads,
 }
 
 size_t sweep_smem_bytes(int dtype, int s, bool constrained, uint32_t flags, int segs_per_cta) {
-    const int rb = dtype == 0 ? 8 : 4;
-    const int gst = dtype == 0 ? Traits<double>::GSTRIDE : Traits<float>::GSTRIDE;
-    return smem_layout(rb, s, constrained, flags, segs_per_cta, gst).total;
+    (void)flags;
+    return smem_layout(dtype == 0 ? 8 : 4, s, constrained, segs_per_cta).total;
 }
 
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st) {
