@@ -90,6 +90,14 @@ __device__ __forceinline__ bool ll_try_load(const void* slot, unsigned seq, doub
     v = __longlong_as_double((long long)(((unsigned long long)b << 32) | a));
     return f0 == seq && f1 == seq;
 }
+struct LLRaw { unsigned a, f0, b, f1; };
+__device__ __forceinline__ void ll_issue(const void* slot, LLRaw& r) {      // the load is issued here, consumed later
+    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.a), "=r"(r.f0), "=r"(r.b), "=r"(r.f1) : "l"(slot) : "memory");
+}
+__device__ __forceinline__ bool ll_ok(const LLRaw& r, unsigned seq) { return r.f0 == seq && r.f1 == seq; }
+__device__ __forceinline__ double ll_value(const LLRaw& r) {
+    return __longlong_as_double((long long)(((unsigned long long)r.b << 32) | r.a));
+}
 // spin until the slot carries `seq`; bounded (returns false after WAIT_TIMEOUT_NS or when another CTA aborted)
 __device__ __forceinline__ bool ll_wait(const void* slot, unsigned seq, double& v, int* abort_flag) {
     if (ll_try_load(slot, seq, v)) return true;
@@ -265,7 +273,6 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     if (tid < 2) abort_sh[tid] = 0;
     __syncthreads();
     for (int it = 0; it < p.k_sweeps; ++it) {
-        int wait_failed = 0;
         const unsigned seq = p.seq_base + (unsigned)it + 1u;     // launch-unique sweep number (never reused)
         const int par = (int)(seq & 1u);
         const bool last_sweep = (it == p.k_sweeps - 1);
@@ -379,6 +386,18 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
                 }
             }
         }
+        // prefetch the rows of the neighbouring CTAs (published at the same point of their sweep): the loads fly
+        // while this warp does its projections and are checked before the CTA barrier
+        const bool need_l = active && isrow && sl == 0 && !right && cta > 0;
+        const bool need_r = active && isrow && sl == nact - 1 && right && cta + 1 < nctas;
+        const bool need = need_l || need_r;
+        const unsigned char* rslot = mbox + par * mbox_par_stride +
+            (need_l ? ((size_t)(cta - 1) * 24 + 12 + korder * 3) * 16 : ((size_t)(cta + 1) * 24 + korder * 3) * 16);
+        LLRaw rr[3];
+        if (need) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) ll_issue(rslot + d * 16, rr[d]);
+        }
         if (CONS) {
             if (has_vel) ball_update(Vv, vmax, phv, wv);      // a4: Eq. 20f, 20g
             if (has_acc) ball_update(Av, amax, pha, wa);
@@ -394,15 +413,36 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
         }
 
         // ================= exchange of boundary rows =================
+        // warp-uniform wait for the prefetched mailbox rows (normally they have arrived: no iteration)
+        int wait_failed = 0;
+        {
+            bool okk = !need || (ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq));
+            if (!__all_sync(0xffffffffu, okk)) {
+                const long long t0 = global_ns();
+                unsigned spins = 0;
+                do {
+                    if (!okk) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) ll_issue(rslot + d * 16, rr[d]);
+                        okk = ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq);
+                    }
+                    bool bail = false;
+                    if ((++spins & 255u) == 0) bail = *(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS;
+                    if (__any_sync(0xffffffffu, bail)) { if (!okk) { atomicExch(p.abort_flag, 1); wait_failed = 1; } break; }
+                } while (!__all_sync(0xffffffffu, okk));
+            }
+        }
+        if (wait_failed) abort_sh[it & 1] = 1;
         if (nctas == 1) {
             __syncthreads();
         } else if (!nb_sync) {
             if (!grid_barrier(p.bar, (unsigned long long)(it + 1) * nctas, p.abort_flag)) break;   // uniform per CTA
+            if (abort_sh[it & 1]) break;
         } else {
             // a mailbox wait of the previous sweep timed out: give up together.  The flag is double buffered by
             // sweep parity so that every thread of the CTA reads the same value after this barrier.
             __syncthreads();
-            if (abort_sh[(it + 1) & 1]) break;
+            if (abort_sh[it & 1]) break;
         }
 
         // ================= phase B: consensus, dual, residuals =================
@@ -410,20 +450,14 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
         Real dz[3] = {0, 0, 0};
         if (isrow) {
             Real nb[3];
-            if (active && sl == 0 && !right && cta > 0) {                // left neighbour lives in the previous CTA
-                const unsigned char* e = mbox + par * mbox_par_stride + (size_t)(cta - 1) * 24 * 16 + (1 * 12 + korder * 3) * 16;
+            if (need) {                 // the neighbour lives in another CTA: prefetched mailbox rows
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double t; wait_failed |= !ll_wait(e + d * 16, seq, t, p.abort_flag); nb[d] = (Real)t; }
-            } else if (active && sl == nact - 1 && right && cta + 1 < nctas) {   // right neighbour lives in the next CTA
-                const unsigned char* e = mbox + par * mbox_par_stride + (size_t)(cta + 1) * 24 * 16 + (0 * 12 + korder * 3) * 16;
-#pragma unroll
-                for (int d = 0; d < 3; ++d) { double t; wait_failed |= !ll_wait(e + d * 16, seq, t, p.abort_flag); nb[d] = (Real)t; }
+                for (int d = 0; d < 3; ++d) nb[d] = (Real)ll_value(rr[d]);
             } else {
                 const Real* e = right ? Bcur + (sl + 2) * 24 + korder * 3 : Bcur + sl * 24 + (korder + S) * 3;
 #pragma unroll
                 for (int d = 0; d < 3; ++d) nb[d] = e[d];
             }
-            if (wait_failed) abort_sh[it & 1] = 1;
             const bool fixed = (right ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder == 0);
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
