@@ -84,12 +84,6 @@ __device__ __forceinline__ void ll_store(void* slot, double v, unsigned seq) {
     asm volatile("st.relaxed.gpu.global.v4.u32 [%0], {%1, %2, %3, %4};" ::"l"(slot), "r"((unsigned)b), "r"(seq),
                  "r"((unsigned)(b >> 32)), "r"(seq) : "memory");
 }
-__device__ __forceinline__ bool ll_try_load(const void* slot, unsigned seq, double& v) {
-    unsigned a, f0, b, f1;
-    asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(f0), "=r"(b), "=r"(f1) : "l"(slot) : "memory");
-    v = __longlong_as_double((long long)(((unsigned long long)b << 32) | a));
-    return f0 == seq && f1 == seq;
-}
 struct LLRaw { unsigned a, f0, b, f1; };
 __device__ __forceinline__ void ll_issue(const void* slot, LLRaw& r) {      // the load is issued here, consumed later
     asm volatile("ld.relaxed.gpu.global.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.a), "=r"(r.f0), "=r"(r.b), "=r"(r.f1) : "l"(slot) : "memory");
@@ -98,24 +92,6 @@ __device__ __forceinline__ bool ll_ok(const LLRaw& r, unsigned seq) { return r.f
 __device__ __forceinline__ double ll_value(const LLRaw& r) {
     return __longlong_as_double((long long)(((unsigned long long)r.b << 32) | r.a));
 }
-// spin until the slot carries `seq`; bounded (returns false after WAIT_TIMEOUT_NS or when another CTA aborted)
-__device__ __forceinline__ bool ll_wait(const void* slot, unsigned seq, double& v, int* abort_flag) {
-    if (ll_try_load(slot, seq, v)) return true;
-    const long long t0 = global_ns();
-    unsigned spins = 0;
-    while (!ll_try_load(slot, seq, v)) {
-        if ((++spins & 255u) == 0) {
-            if (*(volatile int*)abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS) {
-                atomicExch(abort_flag, 1);
-                return false;
-            }
-        }
-    }
-    return true;
-}
-
-template <typename Real> __device__ __forceinline__ Real ldcg(const Real* p) { return __ldcg(p); }
-template <typename Real> __device__ __forceinline__ void stcg(Real* p, Real v) { __stcg(p, v); }
 
 // [beta_k(tau)]_a = a!/(a-k)! tau^(a-k), a >= k   (Eq. 18 differentiated k times, normalised time)
 __device__ __forceinline__ double beta_entry(int k, int a, double tau) {
