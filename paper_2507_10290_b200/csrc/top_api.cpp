@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <atomic>
+#include <thread>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -116,29 +118,55 @@ bool spd_invert(int q, std::vector<xreal>& A) {
 // HARD waypoint mode (reading A2): the two equalities c^_0 = p_{i-1}, sum_a c^_a = p_i are eliminated with the
 // null-space basis Z = {e_a - e_1, a >= 2}:  Pm^ = Z (Z'H^Z)^-1 Z',  c0^ = (I - Pm^ H^) c_chord.
 // Other modes: Pm^ = H^^-1, c0^ = 0.
-bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int mode,
-                    const xreal* p0, const xreal* p1, xreal* Pm /*[8][8]*/, xreal* c0 /*[8][3]*/) {
+// Gram matrices of the constant (normalised-time) rows, built once per s: H^ is a T-weighted sum of them.
+struct GramTables {
+    xreal Q1[MAXN * MAXN];        // int_0^1 beta^(s) beta^(s)'
+    xreal Gc[4][MAXN * MAXN];     // consensus rows of derivative order k: beta_k(0)beta_k(0)' + beta_k(1)beta_k(1)'
+    xreal Ge[3][MAXN * MAXN];     // sample rows of E_0, E_1, E_2: sum_j beta_k(tau_j) beta_k(tau_j)'
+};
+const GramTables& gram_tables(int s) {
+    static GramTables tab[2];
+    static bool ready[2] = {false, false};
+    GramTables& G = tab[s - 3];
+    if (ready[s - 3]) return G;        // benign race: concurrent builders write identical values
     const int n = 2 * s;
-    std::vector<xreal> H(n * n, 0);
+    std::memset(&G, 0, sizeof G);
     for (int j = s; j < n; ++j)
         for (int l = s; l < n; ++l) {
             xreal fj = 1, fl = 1;
             for (int q = 0; q < s; ++q) { fj *= (xreal)(j - q); fl *= (xreal)(l - q); }
-            H[j * n + l] = 2 * std::pow(T, (xreal)(1 - 2 * s)) * fj * fl / (xreal)(j + l - 2 * s + 1);
+            G.Q1[j * MAXN + l] = fj * fl / (xreal)(j + l - 2 * s + 1);
         }
-    auto add_row = [&](int k, xreal tau, xreal w) {
+    auto add = [&](xreal* M, int k, xreal tau) {
         xreal row[MAXN];
-        for (int a = 0; a < n; ++a) row[a] = beta_hat(k, a, tau) / std::pow(T, (xreal)k);
-        for (int a = 0; a < n; ++a)
-            for (int b = 0; b < n; ++b) H[a * n + b] += rho * w * row[a] * row[b];
+        for (int a = 0; a < n; ++a) row[a] = beta_hat(k, a, tau);
+        for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) M[a * MAXN + b] += row[a] * row[b];
     };
-    for (int k = 0; k < s; ++k) { add_row(k, 0, 1); add_row(k, 1, 1); }
-    for (int j = 1; j <= MS; ++j) {
-        const xreal tau = (xreal)j / (xreal)(MS + 1);          // reading A10
-        if (box) add_row(0, tau, 2);                            // two sides of the box (A11)
-        if (vel) add_row(1, tau, 1);
-        if (acc) add_row(2, tau, 1);
-    }
+    for (int k = 0; k < s; ++k) { add(G.Gc[k], k, 0); add(G.Gc[k], k, 1); }
+    for (int j = 1; j <= MS; ++j)
+        for (int k = 0; k < 3; ++k) add(G.Ge[k], k, (xreal)j / (xreal)(MS + 1));     // reading A10
+    ready[s - 3] = true;
+    return G;
+}
+
+bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int mode,
+                    const xreal* p0, const xreal* p1, xreal* Pm /*[8][8]*/, xreal* c0 /*[8][3]*/) {
+    const int n = 2 * s;
+    const GramTables& G = gram_tables(s);
+    xreal iT[8];                       // T^-k
+    iT[0] = 1;
+    for (int k = 1; k < 8; ++k) iT[k] = iT[k - 1] / T;
+    const xreal wq = 2 * T * iT[2 * s - 1] * iT[1];             // 2 T^(1-2s)
+    const xreal wb = box ? 2 * rho : 0;                        // two sides of the box (A11)
+    const xreal wv = vel ? rho * iT[2] : 0, wa = acc ? rho * iT[4] : 0;
+    std::vector<xreal> H(n * n, 0);
+    for (int a = 0; a < n; ++a)
+        for (int b = 0; b < n; ++b) {
+            const int i = a * MAXN + b;
+            xreal v = wq * G.Q1[i] + wb * G.Ge[0][i] + wv * G.Ge[1][i] + wa * G.Ge[2][i];
+            for (int k = 0; k < s; ++k) v += rho * iT[2 * k] * G.Gc[k][i];
+            H[a * n + b] = v;
+        }
     for (int i = 0; i < MAXN * MAXN; ++i) Pm[i] = 0;
     for (int i = 0; i < MAXN * 3; ++i) c0[i] = 0;
     if (mode == (int)TOP_WAYPOINT_HARD) {
@@ -372,15 +400,20 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     if (has_vel) phv.assign(3 * LS, 0.0);
     const int n = 2 * s;
     auto wp = [&](long long b, long long j, int d) -> double { return d < dims ? waypoints[((size_t)b * (N + 1) + j) * dims + d] : 0.0; };
-    for (long long b = 0; b < batch; ++b)
-        for (long long i = 0; i < N; ++i) {
-            const size_t g = (size_t)(b * N + i);
+    gram_tables(s);                       // build the shared tables before the worker threads start
+    std::atomic<int> bad_operator(0);
+    auto do_segments = [&](long long g0, long long g1) {
+        for (long long gg = g0; gg < g1; ++gg) {
+            const long long b = gg / N, i = gg % N;
+            const size_t g = (size_t)gg;
             const double Td = durations[g];
             const xreal T = (xreal)Td;
             xreal p0[3], p1[3], PmX[MAXN * MAXN], c0X[MAXN * 3];
             for (int d = 0; d < 3; ++d) { p0[d] = wp(b, i, d); p1[d] = wp(b, i + 1, d); }
-            if (!build_operator(s, T, (xreal)rho, has_box, has_vel, has_acc, (int)mode, p0, p1, PmX, c0X))
-                CREATE_FAIL(fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)"));
+            if (!build_operator(s, T, (xreal)rho, has_box, has_vel, has_acc, (int)mode, p0, p1, PmX, c0X)) {
+                bad_operator.store(1);
+                return;
+            }
             segflags[g] = (uint8_t)((i == 0 ? SEG_FIRST : 0) | (i == N - 1 ? SEG_LAST : 0));
             invT[g] = (double)(1 / T); invT[NP + g] = (double)(1 / (T * T));
             for (int d = 0; d < 3; ++d) {
@@ -433,6 +466,20 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
                 }
             }
         }
+    };
+    {   // segments are independent: spread the precompute over the host cores
+        unsigned nt = std::thread::hardware_concurrency();
+        nt = std::max(1u, std::min(nt, 32u));
+        if (nseg < 2048) nt = 1;
+        std::vector<std::thread> pool;
+        const long long chunk = (nseg + nt - 1) / nt;
+        for (unsigned t = 1; t < nt; ++t)
+            if ((long long)t * chunk < nseg) pool.emplace_back(do_segments, (long long)t * chunk, std::min(nseg, (long long)(t + 1) * chunk));
+        do_segments(0, std::min(nseg, chunk));
+        for (auto& th : pool) th.join();
+    }
+    if (bad_operator.load())
+        CREATE_FAIL(fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)"));
 
     // ---- device memory
     const size_t rb = real_bytes(h);
