@@ -575,7 +575,8 @@ cudaError_t limits_one(int threads, size_t smem, int* per_sm) {
 }
 
 // f64 kernels are compiled for <= 576 threads (112 registers per thread); f32 for <= 1024 (64 registers)
-constexpr int MAXT_F64 = 576, MAXT_F32 = 1024;
+// plus a variant for small CTAs (<= 256 threads: up to 255 registers, no spills, more ILP across dims)
+constexpr int MAXT_F64 = 576, MAXT_F32 = 1024, MAXT_SMALL = 256;
 
 }  // namespace
 
@@ -592,8 +593,10 @@ int max_threads_for(int dtype) { return dtype == 0 ? MAXT_F64 : MAXT_F32; }
 
 cudaError_t launch_sweeps(const KParams& p, int dtype, int s, bool constrained, int ctas, int threads,
                           size_t smem, cudaStream_t st) {
-#define F64(S_, C_) return launch_one<double, S_, C_, MAXT_F64>(p, ctas, threads, smem, st);
-#define F32(S_, C_) return launch_one<float, S_, C_, MAXT_F32>(p, ctas, threads, smem, st);
+#define F64(S_, C_) return threads <= MAXT_SMALL ? launch_one<double, S_, C_, MAXT_SMALL>(p, ctas, threads, smem, st) \
+                                                 : launch_one<double, S_, C_, MAXT_F64>(p, ctas, threads, smem, st);
+#define F32(S_, C_) return threads <= MAXT_SMALL ? launch_one<float, S_, C_, MAXT_SMALL>(p, ctas, threads, smem, st) \
+                                                 : launch_one<float, S_, C_, MAXT_F32>(p, ctas, threads, smem, st);
     TOP_DISPATCH(F64, F32)
 #undef F64
 #undef F32
@@ -601,8 +604,10 @@ cudaError_t launch_sweeps(const KParams& p, int dtype, int s, bool constrained, 
 }
 
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int threads, size_t smem, int* max_ctas_per_sm) {
-#define F64(S_, C_) return limits_one<double, S_, C_, MAXT_F64>(threads, smem, max_ctas_per_sm);
-#define F32(S_, C_) return limits_one<float, S_, C_, MAXT_F32>(threads, smem, max_ctas_per_sm);
+#define F64(S_, C_) return threads <= MAXT_SMALL ? limits_one<double, S_, C_, MAXT_SMALL>(threads, smem, max_ctas_per_sm) \
+                                                 : limits_one<double, S_, C_, MAXT_F64>(threads, smem, max_ctas_per_sm);
+#define F32(S_, C_) return threads <= MAXT_SMALL ? limits_one<float, S_, C_, MAXT_SMALL>(threads, smem, max_ctas_per_sm) \
+                                                 : limits_one<float, S_, C_, MAXT_F32>(threads, smem, max_ctas_per_sm);
     TOP_DISPATCH(F64, F32)
 #undef F64
 #undef F32
