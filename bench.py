@@ -106,11 +106,26 @@ def oracle_rate(w, seconds: float, threads: int):
                vmax=w.vmax, amax=w.amax)
     if threads <= 0:
         threads = min(o.max_threads(), os.cpu_count() or 1)
-    t0 = time.perf_counter(); o.sweep(2, threads); probe = (time.perf_counter() - t0) / 2
-    sweeps = int(max(3, min(200000, seconds / max(probe, 1e-9))))
+    o.sweep(2, threads)                                            # thread start-up, page faults
+    t0 = time.perf_counter(); o.sweep(10, threads); probe = (time.perf_counter() - t0) / 10
+    sweeps = int(max(3, min(2000000, seconds / max(probe, 1e-9))))
     t0 = time.perf_counter(); o.sweep(sweeps, threads); dt = time.perf_counter() - t0
     return {"value": w.N * sweeps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": "%d sweeps of trajectory 0 (N=%d) of %s, %.1f s, gcc -O2 -fopenmp" % (sweeps, w.N, w.name, dt)}, sweeps, dt
+
+
+def aggregate_over_ranks(total_ms: float, units: float, world: int, device="cpu"):
+    """Whole-job figures from per-rank ones: time = MAX over ranks, units = SUM over ranks (weak scaling, no
+    data-path collective).  Uses the default process group (NCCL on GPUs, gloo in the CPU test)."""
+    if world <= 1:
+        return total_ms, units
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([total_ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([units], dtype=torch.float64, device=device)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
 
 
 def run_reference(args, rank, world):
@@ -181,6 +196,7 @@ def main():
     sol = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync,
                             segs_per_cta=args.segs_per_cta)
     info = sol.launch_info()
+    info.pop("launches", None)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2
 
     def barrier():
@@ -208,13 +224,7 @@ def main():
     total_ms = float(sum(ms))
     gpu_launches = sol.launch_info()["launches"] - launches0
     units = float(w.batch * w.N) * sweeps * args.steps
-    if world > 1:
-        t = torch.tensor([total_ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-        u = torch.tensor([units], device="cuda", dtype=torch.float64)
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        units = float(u.item())
+    total_ms, units = aggregate_over_ranks(total_ms, units, world, device="cuda")
     value = units / (total_ms * 1e-3)
     res = sol.residuals()
 

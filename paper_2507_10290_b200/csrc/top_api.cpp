@@ -43,7 +43,9 @@ struct top_solver {
     // device buffers
     std::vector<void*> allocs;
     double *d_Pm = nullptr, *d_c0 = nullptr, *d_part = nullptr, *d_res = nullptr;
-    void *d_invTk = nullptr, *d_Tpow = nullptr, *d_invT = nullptr, *d_lohi = nullptr;
+    void *d_invTk = nullptr, *d_Tpow = nullptr, *d_invT = nullptr, *d_lohi = nullptr, *d_zoff = nullptr;
+    double* d_origin = nullptr;        // [3][nseg_pad] origin o_i = p_{i-1} of each segment's local frame
+    std::vector<double> origin;        // host copy (top_get_state)
     uint8_t* d_segflags = nullptr;
     void *d_zt = nullptr, *d_u = nullptr, *d_qp = nullptr, *d_qn = nullptr, *d_phv = nullptr, *d_wv = nullptr,
          *d_pha = nullptr, *d_wa = nullptr, *d_chat = nullptr, *d_Bedge = nullptr, *d_coef = nullptr;
@@ -394,7 +396,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     // ---- host precompute (extended precision) and iterate 0 (reading A9), packed per lane
     const size_t LS = (size_t)h->stride, NP = (size_t)h->nseg_pad;
     std::vector<double> Pm(MAXN * LS, 0.0), c0(3 * LS, 0.0), invTk(LS, 0.0), Tpow(LS, 0.0), invT(2 * NP, 0.0),
-        lohi(6 * NP, 0.0), zt(3 * LS, 0.0), chat(3 * LS, 0.0), qp, qn, phv, pha;
+        lohi(6 * NP, 0.0), zt(3 * LS, 0.0), chat(3 * LS, 0.0), zoff(3 * LS, 0.0), origin(3 * NP, 0.0), qp, qn, phv, pha;
     std::vector<uint8_t> segflags(NP, 0);
     if (has_box) { qp.assign(3 * LS, 0.0); qn.assign(3 * LS, 0.0); }
     if (has_vel) phv.assign(3 * LS, 0.0);
@@ -408,8 +410,17 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
             const size_t g = (size_t)gg;
             const double Td = durations[g];
             const xreal T = (xreal)Td;
+            // Segment-local frame: every position-like quantity of segment i (coefficient c_0, position rows of
+            // z~, box bounds) is stored relative to the origin o_i = p_{i-1}.  An exact change of variable (the
+            // sweep only ever uses position differences) that keeps the operator free of the cancellation of
+            // |p| ~ 100 m against segment-sized quantities; top_get_coeffs / top_get_state add o_i back.
             xreal p0[3], p1[3], PmX[MAXN * MAXN], c0X[MAXN * 3];
-            for (int d = 0; d < 3; ++d) { p0[d] = wp(b, i, d); p1[d] = wp(b, i + 1, d); }
+            double org3[3];
+            for (int d = 0; d < 3; ++d) {
+                org3[d] = wp(b, i, d);
+                p0[d] = 0; p1[d] = (xreal)wp(b, i + 1, d) - (xreal)wp(b, i, d);
+                origin[(size_t)d * NP + g] = org3[d];
+            }
             if (!build_operator(s, T, (xreal)rho, has_box, has_vel, has_acc, (int)mode, p0, p1, PmX, c0X)) {
                 bad_operator.store(1);
                 return;
@@ -417,14 +428,19 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
             segflags[g] = (uint8_t)((i == 0 ? SEG_FIRST : 0) | (i == N - 1 ? SEG_LAST : 0));
             invT[g] = (double)(1 / T); invT[NP + g] = (double)(1 / (T * T));
             for (int d = 0; d < 3; ++d) {
-                lohi[(size_t)d * NP + g] = (has_box && d < dims) ? cons->box_lo[g * dims + d] : -1.0;
-                lohi[(size_t)(3 + d) * NP + g] = (has_box && d < dims) ? cons->box_hi[g * dims + d] : 1.0;
+                lohi[(size_t)d * NP + g] = (has_box && d < dims) ? cons->box_lo[g * dims + d] - org3[d] : -1.0;
+                lohi[(size_t)(3 + d) * NP + g] = (has_box && d < dims) ? cons->box_hi[g * dims + d] - org3[d] : 1.0;
             }
             for (int lane = 0; lane < LANES; ++lane) {
                 const size_t gt = g * LANES + lane;
                 for (int bb = 0; bb < MAXN; ++bb) Pm[(size_t)bb * LS + gt] = (double)((xreal)rho * PmX[lane * MAXN + bb]);
                 for (int d = 0; d < 3; ++d) c0[(size_t)d * LS + gt] = d < dims ? (double)c0X[lane * 3 + d] : 0.0;
                 Tpow[gt] = (double)std::pow(T, (xreal)lane);
+                // a neighbour's position row arrives in the neighbour's frame: shift it into this segment's frame
+                for (int d = 0; d < dims; ++d) {
+                    if (lane == 0 && i > 0) zoff[(size_t)d * LS + gt] = wp(b, i - 1, d) - wp(b, i, d);   // o_{i-1} - o_i
+                    if (lane == s && i < N - 1) zoff[(size_t)d * LS + gt] = (double)p1[d];               // o_{i+1} - o_i
+                }
                 if (lane < n) {
                     const int k = lane % s;
                     invTk[gt] = (double)(1 / std::pow(T, (xreal)k));
@@ -433,7 +449,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
                     const long long j = lane < s ? i : i + 1;
                     for (int d = 0; d < dims; ++d) {
                         double v = 0;
-                        if (k == 0) v = wp(b, j, d);
+                        if (k == 0) v = wp(b, j, d) - org3[d];
                         else if (j == 0) v = start_derivs ? start_derivs[((size_t)b * (s - 1) + (k - 1)) * dims + d] : 0.0;
                         else if (j == N) v = end_derivs ? end_derivs[((size_t)b * (s - 1) + (k - 1)) * dims + d] : 0.0;
                         else if (k == 1) {
@@ -451,11 +467,11 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
                 const double tau = (double)(lane + 1) / (double)(MS + 1);
                 double V0[3] = {0, 0, 0};
                 for (int d = 0; d < dims; ++d) {
-                    const double P0 = (double)p0[d] + tau * (double)(p1[d] - p0[d]);
+                    const double P0 = tau * (double)p1[d];         // local frame
                     V0[d] = (double)(p1[d] - p0[d]) / Td;
                     if (has_box) {
-                        qp[(size_t)d * LS + gt] = std::max(0.0, cons->box_hi[g * dims + d] - P0);
-                        qn[(size_t)d * LS + gt] = std::max(0.0, P0 - cons->box_lo[g * dims + d]);
+                        qp[(size_t)d * LS + gt] = std::max(0.0, (cons->box_hi[g * dims + d] - org3[d]) - P0);
+                        qn[(size_t)d * LS + gt] = std::max(0.0, P0 - (cons->box_lo[g * dims + d] - org3[d]));
                     }
                 }
                 if (has_box) for (int d = dims; d < 3; ++d) { qp[(size_t)d * LS + gt] = 1.0; qn[(size_t)d * LS + gt] = 1.0; }
@@ -488,6 +504,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     ALLOC(h->d_Pm, MAXN * LS * 8, false); ALLOC(h->d_c0, 3 * LS * 8, false);
     ALLOC(h->d_invTk, LS * rb, false); ALLOC(h->d_Tpow, LS * rb, false); ALLOC(h->d_invT, 2 * NP * rb, false);
     ALLOC(h->d_lohi, 6 * NP * rb, false); ALLOC(h->d_segflags, NP, false);
+    ALLOC(h->d_zoff, 3 * LS * rb, false); ALLOC(h->d_origin, 3 * NP * 8, false);
     ALLOC(h->d_zt, 3 * LS * rb, false); ALLOC(h->d_u, 3 * LS * rb, true); ALLOC(h->d_chat, 3 * LS * rb, false);
     if (has_box) { ALLOC(h->d_qp, 3 * LS * rb, false); ALLOC(h->d_qn, 3 * LS * rb, false); }
     if (has_vel) { ALLOC(h->d_phv, 3 * LS * rb, false); ALLOC(h->d_wv, 3 * LS * rb, true); }
@@ -507,10 +524,12 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     if ((ce = cudaMemcpyAsync(h->d_Pm, Pm.data(), MAXN * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
         (ce = cudaMemcpyAsync(h->d_c0, c0.data(), 3 * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
         (ce = cudaMemcpyAsync(h->d_segflags, segflags.data(), NP, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_origin, origin.data(), 3 * NP * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
         (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
         CREATE_FAIL(cuda_fail(h, ce, "upload"));
 #define UP(dst, src) do { st = upload_real(h, dst, src); if (st != TOP_OK) CREATE_FAIL(st); } while (0)
-    UP(h->d_invTk, invTk); UP(h->d_Tpow, Tpow); UP(h->d_invT, invT); UP(h->d_lohi, lohi);
+    UP(h->d_invTk, invTk); UP(h->d_Tpow, Tpow); UP(h->d_invT, invT); UP(h->d_lohi, lohi); UP(h->d_zoff, zoff);
+    h->origin = origin;
     UP(h->d_zt, zt); UP(h->d_chat, chat);
     if (has_box) { UP(h->d_qp, qp); UP(h->d_qn, qn); }
     if (has_vel) UP(h->d_phv, phv);
@@ -546,7 +565,7 @@ top_status run_sweeps(top_solver* h, int64_t k) {
             KParams p;
             std::memset(&p, 0, sizeof p);
             p.Pm = h->d_Pm; p.c0 = h->d_c0; p.invTk = h->d_invTk; p.Tpow = h->d_Tpow; p.invT = h->d_invT;
-            p.lohi = h->d_lohi; p.segflags = h->d_segflags;
+            p.lohi = h->d_lohi; p.segflags = h->d_segflags; p.zoff = h->d_zoff;
             p.zt = h->d_zt; p.u = h->d_u; p.qp = h->d_qp; p.qn = h->d_qn; p.phv = h->d_phv; p.wv = h->d_wv;
             p.pha = h->d_pha; p.wa = h->d_wa; p.chat = h->d_chat;
             p.Bedge = h->d_Bedge; p.part = h->d_part;
@@ -632,7 +651,8 @@ extern "C" TOP_API top_status top_get_coeffs(top_solver* h, void* out, int32_t o
     if (!out) return fail(h, TOP_E_INVALID, "out is NULL");
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     ConvParams p;
-    p.chat = h->d_chat; p.invT = h->d_invT; p.out = out_is_device ? out : h->d_coef;
+    p.chat = h->d_chat; p.invT = h->d_invT; p.origin = h->d_origin; p.out = out_is_device ? out : h->d_coef;
+    p.nseg_pad = h->nseg_pad;
     p.stride = h->stride; p.nseg = h->nseg; p.s = h->s; p.dims = h->dims;
     CU(launch_convert(p, h->dtype, h->stream), "coefficient conversion launch");
     h->launches += 1;
@@ -660,7 +680,8 @@ extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, do
                 const size_t g = (size_t)b * N + i;
                 for (int r = 0; r < 2 * s; ++r)
                     for (int d = 0; d < dims; ++d) {
-                        const double v = buf[(size_t)d * LS + g * LANES + r];
+                        double v = buf[(size_t)d * LS + g * LANES + r];
+                        if (f == "z" && r % s == 0) v += h->origin[(size_t)d * h->nseg_pad + g];   // local frame -> global
                         if (f == "u") out[((g * 2 * s) + r) * dims + d] = v;
                         else if (r < s) out[(((size_t)b * (N + 1) + i) * s + r) * dims + d] = v;
                         else if (i == N - 1) out[(((size_t)b * (N + 1) + N) * s + (r - s)) * dims + d] = v;

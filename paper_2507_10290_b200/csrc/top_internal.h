@@ -30,6 +30,7 @@ struct KParams {
     const void* invT;       // Real [2][nseg_pad]  1/T, 1/T^2 per segment
     const void* lohi;       // Real [6][nseg_pad]  lo[3], hi[3] per segment
     const uint8_t* segflags;// [nseg_pad]
+    const void* zoff;       // Real [DIMS][stride]  frame shift added to the neighbour's row (position rows only)
     // ---- state of iterate k (read at launch start, written at launch end)
     void* zt;               // Real [DIMS][stride]  consensus row `lane` of z~_i = (z_{i-1}; z_i)
     void* u;                // Real [DIMS][stride]  scaled dual of that row (Eq. 20c)
@@ -60,6 +61,8 @@ struct KParams {
 struct ConvParams {       // coefficient conversion to the paper's basis (Eq. 18)
     const void* chat;     // Real [DIMS][stride]
     const void* invT;     // Real [2][nseg_pad]
+    const double* origin; // [3][nseg_pad]  origin of each segment's local frame (added to c_0)
+    long long nseg_pad;
     void* out;            // Real [nseg][dims][2s]
     long long stride, nseg;
     int s, dims;

@@ -113,7 +113,7 @@ namespace {
 
 // shared-memory carve-up, identical on host (size) and device (pointers)
 struct SmemLayout {
-    size_t pm, bco, lohi, xs, cs, bs, total;
+    size_t pm, bco, lohi, xs, cs, bs, zoff, total;
 };
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
 __host__ __device__ inline SmemLayout smem_layout(int real_bytes, int S, bool cons, int segs) {
@@ -127,6 +127,7 @@ __host__ __device__ inline SmemLayout smem_layout(int real_bytes, int S, bool co
     L.xs = off;   off = align16(off + (size_t)segs * XSTRIDE * sizeof(double));        // rhs rows, all-gather
     L.cs = off;   off = align16(off + (size_t)segs * CSTRIDE * real_bytes);            // coefficient rows, all-gather
     L.bs = off;   off = align16(off + (size_t)2 * (segs + 2) * 24 * real_bytes);       // boundary rows, double buffered
+    L.zoff = off; off = align16(off + (size_t)3 * T * real_bytes);                     // frame shift of the neighbour's row
     L.total = off;
     return L;
 }
@@ -190,6 +191,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE;   // this segment: [d][a]
     Real* Cs = reinterpret_cast<Real*>(smem_raw + L.cs) + (size_t)sl * (sizeof(Real) == 8 ? 26 : 28);   // this segment: [d][a]
     Real* Bs = reinterpret_cast<Real*>(smem_raw + L.bs);       // [2 parity][SEGS+2][8 rows][3]
+    Real* zoffs = reinterpret_cast<Real*>(smem_raw + L.zoff) + tid;   // [3][T]
 
     const long long cta_first = p.seg_begin + (long long)cta * SEGS;
     const long long remaining = p.seg_end - cta_first;
@@ -220,6 +222,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     const Real invT = static_cast<const Real*>(p.invT)[gseg], invT2 = static_cast<const Real*>(p.invT)[p.nseg_pad + gseg];
     if (CONS && lane < 6) lohi[lane * SEGS + sl] = static_cast<const Real*>(p.lohi)[lane * p.nseg_pad + gseg];
     const uint8_t sf = p.segflags[gseg];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) zoffs[d * T] = static_cast<const Real*>(p.zoff)[d * stride + gt];
     const Real tau = (Real)((double)(lane + 1) / (double)(MS + 1));       // sample time of this lane (reading A10)
     const Real itau2 = (Real)(1.0 / (((double)(lane + 1) / (double)(MS + 1)) * ((double)(lane + 1) / (double)(MS + 1))));
     // ---- state of iterate k
@@ -434,6 +438,10 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
 #pragma unroll
                 for (int d = 0; d < 3; ++d) nb[d] = e[d];
             }
+            if (korder == 0) {          // position rows live in segment-local frames: shift the neighbour's into mine
+#pragma unroll
+                for (int d = 0; d < 3; ++d) nb[d] += zoffs[d * T];
+            }
             const bool fixed = (right ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder == 0);
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
@@ -514,8 +522,11 @@ __global__ void convert_coeffs_kernel(const ConvParams p) {
     Real sc = 1;
     for (int q = 0; q < a; ++q) sc *= invT;
     Real* out = static_cast<Real*>(p.out);
-    for (int d = 0; d < p.dims; ++d)
-        out[(seg * p.dims + d) * (2 * p.s) + a] = static_cast<const Real*>(p.chat)[d * p.stride + idx] * sc;
+    for (int d = 0; d < p.dims; ++d) {
+        double v = (double)(static_cast<const Real*>(p.chat)[d * p.stride + idx] * sc);
+        if (a == 0) v += p.origin[d * p.nseg_pad + seg];          // segment-local frame -> global frame
+        out[(seg * p.dims + d) * (2 * p.s) + a] = (Real)v;
+    }
 }
 
 // res[b][q] = sqrt(sum_i part[b*N+i][q]) with a fixed-order tree (deterministic; no atomics)

@@ -27,9 +27,9 @@ def check_fields(errs, where):
         assert v < tol, (where, k, v, errs)
 
 
-def run_parity(w, checkpoints, mode="hard", sync="auto", segs_per_cta=0, b_list=None):
+def run_parity(w, checkpoints, mode="hard", sync="auto", segs_per_cta=0, b_list=None, long_double=False, threads=1):
     b_list = list(range(w.batch)) if b_list is None else b_list
-    oracles = [make_oracle(w, b, mode=mode) for b in b_list]
+    oracles = [make_oracle(w, b, mode=mode, long_double=long_double) for b in b_list]
     sol = top.from_workload(w, mode=mode, sync=sync, segs_per_cta=segs_per_cta, dtype="f64")
     errs0 = field_errors(sol, oracles, w, b_list)       # iterate 0 (Init, reading A9)
     check_fields(errs0, "iterate 0")
@@ -38,7 +38,7 @@ def run_parity(w, checkpoints, mode="hard", sync="auto", segs_per_cta=0, b_list=
     for cp in checkpoints:
         sol.iterate(cp - done)
         for o in oracles:
-            o.sweep(cp - done)
+            o.sweep(cp - done, threads)
         done = cp
         assert sol.iteration == done
         errs = field_errors(sol, oracles, w, b_list)
@@ -168,3 +168,86 @@ def test_capacity_and_unsupported():
         top.TopSolver(w.waypoints, w.durations, 4, 1.0, samples=8, vmax=3.0, amax=5.0,
                       box_lo=w.waypoints[:, :-1] - 50, box_hi=w.waypoints[:, :-1] + 50)
     assert e.value.status == top.TOP_E_UNSUPPORTED
+
+
+# ------------------------------------------------------------------ BASELINE.json's full sizes, bench.py's launch plan
+
+def test_config4_full_size_iterates():
+    """N=10,000 (148 CTAs x 68 segments, the configuration bench.py times): every field, element by element."""
+    # The fp64 oracle works in the paper's raw monomial basis (cond(H) up to 1e13, reading A12): at this size its
+    # own rounding error against the same oracle in long double is 1e-10..5e-10 norm-relative (measured in
+    # test_fp64_oracle_rounding_error_at_full_size), i.e. it would consume the 1e-9 budget.  The CUDA path is
+    # therefore held to 1e-9 against the oracle run in long double (same algorithm, same order, more digits).
+    w = W.config4()
+    sol, (o,), worst = run_parity(w, [1, 2, 10, 100, 300], long_double=True, threads=0)
+    info = sol.launch_info()
+    assert info["ctas"] >= 140 and info["waves"] == 1
+    # per-iterate invariants on the GPU state (P10)
+    for side in ("pos", "neg"):
+        sp, vp = sol.state("s_" + side), sol.state("v_" + side)
+        assert sp.min() >= 0 and vp.min() >= 0 and np.abs(sp * vp).max() == 0
+    assert np.sqrt((sol.state("phi_v") ** 2).sum(-1)).max() <= w.vmax * (1 + 1e-15)
+    assert np.sqrt((sol.state("phi_a") ** 2).sum(-1)).max() <= w.amax * (1 + 1e-15)
+    z = sol.state("z")
+    assert np.abs(z[0, :, 0, :] - w.waypoints[0]).max() < 1e-9          # HARD mode: position rows are the waypoints
+
+
+def test_config4_launch_chunking_is_invisible():
+    """top_iterate(k1) then top_iterate(k2) is iterate k1+k2, bit for bit, in both inter-CTA sync modes."""
+    w = W.config4(N=1500)
+    a = top.from_workload(w, sync="neighbour"); a.iterate(37)
+    b = top.from_workload(w, sync="neighbour"); b.iterate(20); b.iterate(1); b.iterate(16)
+    c = top.from_workload(w, sync="grid"); c.iterate(37)
+    for f in ("z", "u", "s_pos", "v_neg", "phi_v", "w_a"):
+        assert np.array_equal(a.state(f), b.state(f)), f
+        assert np.array_equal(a.state(f), c.state(f)), f
+    assert np.array_equal(a.coeffs(), b.coeffs()) and np.array_equal(a.coeffs(), c.coeffs())
+    ra, rb = a.residuals(), b.residuals()
+    assert ra["r_p"][0] == rb["r_p"][0] and ra["r_d"][0] == rb["r_d"][0]
+
+
+def test_config5_batch_fp32_positions():
+    """256 x 512 segments, fp32 (mixed), 500 sweeps, 7 waves of whole trajectories: sampled positions of 24
+    trajectories spread over the batch (every wave) against the fp64 oracle, 1e-3 m (north_star)."""
+    w = W.config5()
+    sol = top.from_workload(w)
+    assert sol.launch_info()["waves"] > 1
+    sol.iterate(500)
+    c = sol.coeffs()
+    worst = 0.0
+    for b in list(range(0, 256, 11)):
+        o = make_oracle(w, b)
+        o.sweep(500)
+        T = w.durations[b]
+        err = np.abs(sampled_positions(c[b], T) - sampled_positions(o.get("coeffs"), T)).max()
+        worst = max(worst, err)
+    assert worst < 1e-3, worst
+    r = sol.residuals()
+    assert np.all(np.isfinite(r["r_p"])) and r["r_p"].shape == (256,)
+
+
+def test_config5_batch_fp64_waves_match_oracle():
+    """The same batch in fp64 (more waves): wave boundaries and trajectory ends inside CTAs do not leak."""
+    w = W.config5(batch=40)
+    sol = top.from_workload(w, dtype="f64")
+    sol.iterate(60)
+    bl = [0, 1, 18, 19, 20, 38, 39]
+    oracles = [make_oracle(w, b) for b in bl]
+    for o in oracles:
+        o.sweep(60)
+    check_fields(field_errors(sol, oracles, w, bl), "cfg5 fp64 batch=40")
+
+
+def test_fp64_oracle_rounding_error_at_full_size():
+    """Context for the test above: fp64 oracle vs long-double oracle on config 4, and the CUDA path vs both."""
+    w = W.config4()
+    o, ol = make_oracle(w), make_oracle(w, long_double=True)
+    sol = top.from_workload(w)
+    o.sweep(100, 0); ol.sweep(100, 0); sol.iterate(100)
+    T = w.durations[0]
+    ref = scaled(ol.get("coeffs"), T)
+    e_oracle = np.abs(scaled(o.get("coeffs"), T) - ref).max() / np.abs(ref).max()
+    e_gpu = np.abs(scaled(sol.coeffs()[0], T) - ref).max() / np.abs(ref).max()
+    assert e_gpu < 1e-9
+    assert e_oracle < 2e-9            # the fp64 oracle itself stays close to the bar ...
+    assert np.abs(scaled(sol.coeffs()[0], T) - scaled(o.get("coeffs"), T)).max() / np.abs(ref).max() < 1e-9 + e_oracle
