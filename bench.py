@@ -250,7 +250,10 @@ def main():
             per_launch_s = (sum(ms) / args.steps) * 1e-3 / waves
             ach = per_launch_flops / per_launch_s
             out["roofline"] = {"bound": "alu", "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
-                               "frac": ach / peak, "traffic": None,
+                               "frac": ach / peak,
+                               # DRAM bytes per launch (read + write) from the committed ncu capture of this command
+                               # (profiles/r1_v1_cfg4_ncu_summary.md); independent of the sweep count: state is on chip
+                               "traffic": 27513088 if args.workload == "cfg4" else None,
                                "peak_source": "measured in this run: top_fma_peak (%s FMA loop, all SMs)" % dt_name,
                                "flops_per_segment_sweep": fl}
         peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
