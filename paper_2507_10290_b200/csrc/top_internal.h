@@ -17,7 +17,7 @@ constexpr uint8_t SEG_LAST = 2;   // last segment: right junction (z_N) is fixed
 
 // kernel flags
 constexpr uint32_t KF_BOX = 1, KF_VEL = 2, KF_ACC = 4, KF_PIN_POS = 8 /* PINNED_Z: position row of z held */,
-                   KF_NEIGHBOUR_SYNC = 16;
+                   KF_NEIGHBOUR_SYNC = 16, KF_PAIRWISE = 32 /* warp-pair named barriers instead of the CTA barrier */;
 
 // Per-lane field arrays: element [f * stride + gseg * LANES + lane]; stride = padded lane count.
 // "Real" is double (TOP_F64) or float (TOP_F32); the x-update operator is always double.

@@ -250,7 +250,14 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     for (int a = 0; a < N2; ++a) bc[a] = bco[a * 8 + lane];
 
     __shared__ int abort_sh[2];
+    __shared__ int abort_any;                  // pairwise-barrier mode: a mailbox wait timed out somewhere in this CTA
     if (tid < 2) abort_sh[tid] = 0;
+    if (tid == 0) abort_any = 0;
+    const int warp = tid >> 5, nwarps = T >> 5;
+    // Pairwise mode: instead of one CTA-wide barrier per sweep, a warp meets only its two neighbouring warps, on
+    // hardware named barriers (pair (w, w+1) <-> barrier id w; even pairs first, then odd pairs: no deadlock).
+    // Warps may then drift up to one sweep apart, which de-synchronises their use of the fp64 pipe.
+    const bool pairwise = nb_sync && nctas > 1 && nwarps <= 17 && (flags & KF_PAIRWISE);
     __syncthreads();
     for (int it = 0; it < p.k_sweeps; ++it) {
         const unsigned seq = p.seq_base + (unsigned)it + 1u;     // launch-unique sweep number (never reused)
@@ -397,6 +404,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
         int wait_failed = 0;
         {
             bool okk = !need || (ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq));
+            if (pairwise && *(volatile int*)&abort_any) okk = true;      // already failed: run out the sweeps without waiting
             if (!__all_sync(0xffffffffu, okk)) {
                 const long long t0 = global_ns();
                 unsigned spins = 0;
@@ -412,8 +420,14 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
                 } while (!__all_sync(0xffffffffu, okk));
             }
         }
-        if (wait_failed) abort_sh[it & 1] = 1;
-        if (nctas == 1) {
+        if (wait_failed) { abort_sh[it & 1] = 1; *(volatile int*)&abort_any = 1; }
+        if (pairwise) {
+            // no thread may leave the loop early in this mode (its partners would wait for ever at a named barrier):
+            // after a time-out the CTA runs its remaining sweeps without waiting and the host reports TOP_E_CUDA
+            const int first = (warp & 1) ? warp - 1 : warp, second = (warp & 1) ? warp : warp - 1;
+            if (first >= 0 && first + 1 < nwarps) asm volatile("bar.sync %0, 64;" ::"r"(first) : "memory");
+            if (second >= 0 && second + 1 < nwarps) asm volatile("bar.sync %0, 64;" ::"r"(second) : "memory");
+        } else if (nctas == 1) {
             __syncthreads();
         } else if (!nb_sync) {
             if (!grid_barrier(p.bar, (unsigned long long)(it + 1) * nctas, p.abort_flag)) break;   // uniform per CTA

@@ -20,7 +20,7 @@ TOP_F64, TOP_F32 = 0, 1
 WAYPOINT = {"hard": 0, "pinned_z": 1, "free": 2}
 TOP_RD_NORMALISED = 4
 TOP_EPS_N_SCALED = 8
-SYNC = {"auto": 0, "grid": 16, "neighbour": 32}
+SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
 EXPORTS = ["top_create", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
            "top_iteration", "top_launch_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
