@@ -74,7 +74,8 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
 /* Inter-CTA synchronisation of the persistent kernel (a performance knob; results are identical). */
 #define TOP_SYNC_AUTO         0u
 #define TOP_SYNC_GRID         16u /* one grid-wide barrier per sweep */
-#define TOP_SYNC_NEIGHBOUR    32u /* release/acquire flags with the two neighbouring CTAs only */
+#define TOP_SYNC_NEIGHBOUR    32u /* mailbox exchange with the two neighbouring CTAs only; one CTA barrier per sweep */
+#define TOP_SYNC_PAIRWISE     48u /* the same, with warp-pair named barriers instead of the CTA barrier (what AUTO picks) */
 #define TOP_SYNC_MASK         48u
 
 /* The paper's convex sets, specialised as BASELINE.json's configs use them:

@@ -553,8 +553,8 @@ top_status check_abort(top_solver* h) {
 uint32_t sync_flag(const top_solver* h) {
     const uint32_t m = h->opt_flags & TOP_SYNC_MASK;
     if (m == TOP_SYNC_GRID) return 0;
-    if (m == TOP_SYNC_MASK) return KF_NEIGHBOUR_SYNC | KF_PAIRWISE;   // experimental: both bits
-    return KF_NEIGHBOUR_SYNC;     // TOP_SYNC_AUTO and TOP_SYNC_NEIGHBOUR
+    if (m == TOP_SYNC_NEIGHBOUR) return KF_NEIGHBOUR_SYNC;            // CTA barrier + mailbox
+    return KF_NEIGHBOUR_SYNC | KF_PAIRWISE;   // TOP_SYNC_AUTO / TOP_SYNC_PAIRWISE: warp-pair barriers + mailbox
 }
 
 // k sweeps on every wave, then the per-trajectory residual reduction.  Asynchronous.

@@ -67,7 +67,7 @@ def test_config1_other_waypoint_modes(mode):
 
 
 @pytest.mark.parametrize("s,acc", [(3, False), (3, True), (4, False), (4, True)])
-@pytest.mark.parametrize("sync", ["grid", "neighbour"])
+@pytest.mark.parametrize("sync", ["grid", "neighbour", "pairwise"])
 def test_small_constrained_ragged(s, acc, sync):
     """N=37: several CTAs (segs_per_cta=8 -> 5 CTAs, last one ragged with 5 of 8 segments)."""
     w = W.small_constrained(N=37, s=s, acc=acc)
@@ -198,6 +198,8 @@ def test_config4_launch_chunking_is_invisible():
     a = top.from_workload(w, sync="neighbour"); a.iterate(37)
     b = top.from_workload(w, sync="neighbour"); b.iterate(20); b.iterate(1); b.iterate(16)
     c = top.from_workload(w, sync="grid"); c.iterate(37)
+    e = top.from_workload(w, sync="pairwise"); e.iterate(30); e.iterate(7)
+    assert np.array_equal(a.coeffs(), e.coeffs()) and np.array_equal(a.state("u"), e.state("u"))
     for f in ("z", "u", "s_pos", "v_neg", "phi_v", "w_a"):
         assert np.array_equal(a.state(f), b.state(f)), f
         assert np.array_equal(a.state(f), c.state(f)), f
