@@ -290,6 +290,38 @@ def main():
                                   "r_p": float(r3["r_p"].max()), "r_d": float(r3["r_d"].max()),
                                   "note": "cap reached (max_iter=200000)" if not ok else "ok"}
             s3.close()
+            if args.workload == "cfg4":
+                # flagged feasible variant "4f" (every T_i x 3): stop on r_p and the normalised r_d
+                wf = W.config4(seed=1004 + rank, time_stretch=3.0)
+                s4 = top.from_workload(wf, device=local_rank, stream=stream.cuda_stream, sync=args.sync, check_every=64,
+                                       max_iter=400000, rd_normalised=True)
+                torch.cuda.synchronize(); t0 = time.perf_counter()
+                ok4, it4 = s4.solve(1e-4)
+                torch.cuda.synchronize(); dt4 = time.perf_counter() - t0
+                r4 = s4.residuals()
+                out["time_to_eps_feasible_variant"] = {
+                    "workload": wf.name, "eps": 1e-4, "stop": "r_p and r_d_norm (TOP_RD_NORMALISED)", "converged": bool(ok4),
+                    "sweeps": int(it4.max()), "seconds": dt4, "r_p": float(r4["r_p"].max()),
+                    "r_d_norm": float(r4["r_d_norm"].max()), "r_d": float(r4["r_d"].max())}
+                s4.close()
+            # ---- the other BASELINE.json configs, device-resident throughput (parity-test cases, context only)
+            others = {}
+            for name in ("cfg1", "cfg2", "cfg3", "cfg3f32", "cfg5"):
+                if name == args.workload:
+                    continue
+                wo = make_workload(name, rank)
+                so = top.from_workload(wo, device=local_rank, stream=stream.cuda_stream, sync=args.sync)
+                k = wo.sweeps or 2000
+                so.iterate(k)
+                torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream); so.iterate(k); so.iterate(k); so.iterate(k); e1.record(stream)
+                torch.cuda.synchronize()
+                msk = e0.elapsed_time(e1) / 3
+                others[wo.name] = {"segment_iterations_per_s": wo.batch * wo.N * k / (msk * 1e-3), "sweeps": k,
+                                   "us_per_sweep_per_wave": 1e3 * msk / k / so.launch_info()["waves"], "dtype": wo.dtype}
+                so.close()
+            out["other_workloads"] = others
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"], _, _ = oracle_rate(w, args.oracle_seconds, args.oracle_threads)
         print(json.dumps(out))
