@@ -322,6 +322,22 @@ def main():
                                    "us_per_sweep_per_wave": 1e3 * msk / k / so.launch_info()["waves"], "dtype": wo.dtype}
                 so.close()
             out["other_workloads"] = others
+            # ---- the paper's own regime (Tables I-II): tolerance ||r|| < N*0.05 on config 2, fixed rho
+            # vs adaptive rho (Eq. 24, rho0 = 1, updated every sweep as in Alg. 1 line 14)
+            w2 = make_workload("cfg2", rank)
+            reg = {}
+            for label, kw in (("fixed_rho10", dict()), ("adaptive_rho0_1", dict(adaptive_rho=True))):
+                sa = top.TopSolver(w2.waypoints, w2.durations, w2.s, 1.0 if kw else w2.rho, samples=w2.samples,
+                                   box_lo=w2.box_lo, box_hi=w2.box_hi, vmax=w2.vmax, eps_n_scaled=True, check_every=1,
+                                   max_iter=300000, device=local_rank, stream=stream.cuda_stream, **kw)
+                torch.cuda.synchronize(); t0 = time.perf_counter()
+                oka, ita = sa.solve(0.05)
+                torch.cuda.synchronize(); dta = time.perf_counter() - t0
+                ra = sa.residuals()
+                reg[label] = {"converged": bool(oka), "sweeps": int(ita.max()), "seconds": dta, "rho_final": sa.rho,
+                              "r_p": float(ra["r_p"][0]), "r_d": float(ra["r_d"][0])}
+                sa.close()
+            out["paper_tolerance_cfg2"] = {"eps": "N*0.05", "check_every": 1, **reg}
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"], _, _ = oracle_rate(w, args.oracle_seconds, args.oracle_threads)
         print(json.dumps(out))

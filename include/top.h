@@ -77,6 +77,10 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
 #define TOP_SYNC_NEIGHBOUR    32u /* mailbox exchange with the two neighbouring CTAs only; one CTA barrier per sweep */
 #define TOP_SYNC_PAIRWISE     48u /* the same, with warp-pair named barriers instead of the CTA barrier (what AUTO picks) */
 #define TOP_SYNC_MASK         48u
+/* Adaptive penalty (Eq. 24; Alg. 1 line 14): at every residual check of top_solve (every
+ * check_every sweeps; the paper: every sweep) rho <- tau_incr*rho if r_p > mu*r_d, rho <- rho/tau_decr if
+ * r_d > mu*r_p.  The change goes through top_set_rho. */
+#define TOP_RHO_ADAPTIVE      64u
 
 /* The paper's convex sets, specialised as BASELINE.json's configs use them:
  * an axis-aligned box corridor per segment (K=6 half-spaces, linear set, Eq. 7-10) and Euclidean balls on
@@ -99,6 +103,9 @@ typedef struct {
     void* cuda_stream;      /* cudaStream_t; NULL = default stream */
     int32_t segs_per_cta;   /* segments per thread block, 0 = choose (a tuning knob; multiple of 4) */
     int32_t reserved;
+    double adapt_mu;        /* Eq. 24: mu (> 1),       0 = the paper's 10 */
+    double adapt_tau_incr;  /*         tau_incr (> 1), 0 = the paper's 1.1 */
+    double adapt_tau_decr;  /*         tau_decr (> 1), 0 = the paper's 1.1 */
 } top_options;
 
 /*
@@ -135,6 +142,16 @@ TOP_API top_status top_iterate(top_solver* h, int64_t k);
  *          or the total if it never did.
  * Returns TOP_OK, TOP_NOT_CONVERGED, TOP_E_NONFINITE, TOP_E_CUDA.  Synchronises the stream. */
 TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iters);
+
+/* top_set_rho -- change the penalty parameter between sweeps (the primitive under Eq. 24).  The x-update operator
+ * of every segment is rebuilt for the new rho (host, extended precision, as in top_create) and uploaded, and the
+ * SCALED duals u, v, w on the device are multiplied by rho_old/rho_new so that the multipliers y = rho*u are
+ * unchanged (reading A16; the paper is silent; Boyd et al. 3.4.1).  Synchronises the stream.
+ * TOP_E_INVALID if rho <= 0 or not finite. */
+TOP_API top_status top_set_rho(top_solver* h, double rho);
+
+/* Current penalty parameter (NaN if h is NULL). */
+TOP_API double top_get_rho(const top_solver* h);
 
 /* top_get_residuals -- residuals of the last sweep, host [batch] each, any pointer may be NULL:
  *   r_primal       || stack_i (M c_i - z~_i) ||_2  over all consensus rows (reading A7)

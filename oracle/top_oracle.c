@@ -487,6 +487,47 @@ int64_t oracle_solve(oracle_t *o, double eps, int64_t max_iter, int use_rd_norm,
     return it;
 }
 
+/*
+ * Adaptive rho (Eq. 24; Alg. 1 line 14).  Changing rho changes the x-update operator
+ * (rebuilt from scratch) and -- reading A16, the paper is silent -- the SCALED duals u = y/rho, v, w are
+ * multiplied by rho_old/rho_new so that the unscaled multipliers y = rho*u are unchanged (Boyd et al. [8] 3.4.1).
+ * Returns 0 on success.
+ */
+int oracle_set_rho(oracle_t *o, double rho_new) {
+    if (!(rho_new > 0)) return -1;
+    const int N = o->N, s = o->s, m = o->m, Ms = o->Ms;
+    const real_t r = o->rho / (real_t)rho_new;
+    for (size_t a = 0; a < (size_t)N * 2 * s * m; ++a) o->u[a] *= r;
+    for (size_t a = 0; a < (size_t)N * Ms * m; ++a) { o->Vp[a] *= r; o->Vn[a] *= r; o->WV[a] *= r; o->WA[a] *= r; }
+    o->rho = (real_t)rho_new;
+    for (int i = 0; i < N; ++i) if (build_operator(o, i)) return -1;
+    return 0;
+}
+
+double oracle_rho(const oracle_t *o) { return (double)o->rho; }
+
+/* Alg. 1 with line 14: sweep; test the stop rule (Eq. 23); every `every` sweeps apply Eq. 24 with the residuals of
+ * that sweep:  rho <- tau_incr*rho if r_p > mu r_d;  rho <- rho/tau_decr if r_d > mu r_p.  Returns sweeps done. */
+int64_t oracle_solve_adaptive(oracle_t *o, double eps, int64_t max_iter, int use_rd_norm, double mu, double tau_incr,
+                              double tau_decr, int every, int threads) {
+#ifdef _OPENMP
+    if (threads > 0) omp_set_num_threads(threads);
+#else
+    (void)threads;
+#endif
+    int64_t it = 0;
+    while (it < max_iter) {
+        sweep_once(o); ++it;
+        double rd = use_rd_norm ? o->rd_norm : o->rd;
+        if (o->rp < eps && rd < eps) break;
+        if (every > 0 && it % every == 0) {
+            if (o->rp > mu * rd) oracle_set_rho(o, (double)o->rho * tau_incr);
+            else if (rd > mu * o->rp) oracle_set_rho(o, (double)o->rho / tau_decr);
+        }
+    }
+    return it;
+}
+
 /* out[0..3] = r_p (A7), r_d (Eq. 22, A8), r_d normalised, r_p of Eq. 21 verbatim (junction gaps) */
 void oracle_residuals(const oracle_t *o, double *out) {
     out[0] = o->rp; out[1] = o->rd; out[2] = o->rd_norm; out[3] = o->rp_gap;

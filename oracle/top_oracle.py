@@ -44,6 +44,13 @@ def _lib(long_double: bool):
         L.oracle_sweep.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int]
         L.oracle_solve.restype = ctypes.c_int64
         L.oracle_solve.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int64, ctypes.c_int, ctypes.c_int]
+        L.oracle_set_rho.restype = ctypes.c_int
+        L.oracle_set_rho.argtypes = [ctypes.c_void_p, ctypes.c_double]
+        L.oracle_rho.restype = ctypes.c_double
+        L.oracle_rho.argtypes = [ctypes.c_void_p]
+        L.oracle_solve_adaptive.restype = ctypes.c_int64
+        L.oracle_solve_adaptive.argtypes = [ctypes.c_void_p, ctypes.c_double, ctypes.c_int64, ctypes.c_int, ctypes.c_double,
+                                            ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int]
         L.oracle_residuals.argtypes = [ctypes.c_void_p, dp]
         L.oracle_objective.restype = ctypes.c_double
         L.oracle_objective.argtypes = [ctypes.c_void_p]
@@ -96,6 +103,18 @@ class Oracle:
 
     def solve(self, eps, max_iter, use_rd_norm=False, threads=1):
         return int(self._L.oracle_solve(self._h, float(eps), int(max_iter), int(use_rd_norm), int(threads)))
+
+    def set_rho(self, rho):
+        if self._L.oracle_set_rho(self._h, float(rho)) != 0:
+            raise ValueError("oracle_set_rho failed")
+
+    @property
+    def rho(self):
+        return float(self._L.oracle_rho(self._h))
+
+    def solve_adaptive(self, eps, max_iter, mu=10.0, tau_incr=1.1, tau_decr=1.1, every=1, use_rd_norm=False, threads=1):
+        return int(self._L.oracle_solve_adaptive(self._h, float(eps), int(max_iter), int(use_rd_norm), float(mu),
+                                                 float(tau_incr), float(tau_decr), int(every), int(threads)))
 
     def residuals(self):
         out = np.zeros(4)

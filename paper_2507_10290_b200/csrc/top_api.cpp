@@ -46,6 +46,10 @@ struct top_solver {
     void *d_invTk = nullptr, *d_Tpow = nullptr, *d_invT = nullptr, *d_lohi = nullptr, *d_zoff = nullptr;
     double* d_origin = nullptr;        // [3][nseg_pad] origin o_i = p_{i-1} of each segment's local frame
     std::vector<double> origin;        // host copy (top_get_state)
+    std::vector<double> h_T;           // [nseg] durations (operator rebuild on top_set_rho)
+    std::vector<xreal> h_dp;           // [nseg][3] p_i - p_{i-1} in extended precision
+    uint32_t wp_mode = 0;
+    double adapt_mu = 10.0, adapt_incr = 1.1, adapt_decr = 1.1;
     uint8_t* d_segflags = nullptr;
     void *d_zt = nullptr, *d_u = nullptr, *d_qp = nullptr, *d_qn = nullptr, *d_phv = nullptr, *d_wv = nullptr,
          *d_pha = nullptr, *d_wa = nullptr, *d_chat = nullptr, *d_Bedge = nullptr, *d_coef = nullptr;
@@ -267,6 +271,21 @@ int max_segs_per_cta(int dtype, int s, bool constrained, uint32_t kflags, size_t
 
 }  // namespace
 
+namespace {
+// run fn(g0, g1) over [0, n) on the host cores (segments are independent)
+template <typename F> void parallel_segments(long long n, F fn) {
+    unsigned nt = std::thread::hardware_concurrency();
+    nt = std::max(1u, std::min(nt, 32u));
+    if (n < 2048) nt = 1;
+    std::vector<std::thread> pool;
+    const long long chunk = (n + nt - 1) / nt;
+    for (unsigned t = 1; t < nt; ++t)
+        if ((long long)t * chunk < n) pool.emplace_back(fn, (long long)t * chunk, std::min(n, (long long)(t + 1) * chunk));
+    fn(0, std::min(n, chunk));
+    for (auto& th : pool) th.join();
+}
+}  // namespace
+
 // =================================================================================== top_create
 
 extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_t N, int32_t s, int32_t dims, top_dtype dtype,
@@ -321,10 +340,15 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
         if (opt->struct_size >= offsetof(top_options, cuda_stream)) if (in.max_iter > 0) o.max_iter = in.max_iter;
         if (opt->struct_size >= offsetof(top_options, segs_per_cta)) o.cuda_stream = in.cuda_stream;
         if (opt->struct_size >= offsetof(top_options, reserved)) o.segs_per_cta = in.segs_per_cta;
+        if (opt->struct_size >= sizeof(top_options)) {
+            o.adapt_mu = in.adapt_mu; o.adapt_tau_incr = in.adapt_tau_incr; o.adapt_tau_decr = in.adapt_tau_decr;
+        }
     }
     const uint32_t mode = o.flags & TOP_WAYPOINT_MASK;
     if (mode > TOP_WAYPOINT_FREE) return fail(h, TOP_E_INVALID, "unknown waypoint mode");
     if (o.segs_per_cta < 0 || (o.segs_per_cta % 4) != 0) return fail(h, TOP_E_INVALID, "segs_per_cta must be a multiple of 4");
+    for (double v : {o.adapt_mu, o.adapt_tau_incr, o.adapt_tau_decr})
+        if (v != 0 && !(v > 1 && std::isfinite(v))) return fail(h, TOP_E_INVALID, "adapt_mu / adapt_tau_* must be > 1 (or 0 = default)");
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
@@ -346,6 +370,10 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     h->has_box = has_box; h->has_vel = has_vel; h->has_acc = has_acc;
     h->constrained = has_box || has_vel || has_acc;
     h->vmax = has_vel ? cons->vmax : 0; h->amax = has_acc ? cons->amax : 0;
+    h->wp_mode = mode;
+    if (o.adapt_mu > 0) h->adapt_mu = o.adapt_mu;
+    if (o.adapt_tau_incr > 0) h->adapt_incr = o.adapt_tau_incr;
+    if (o.adapt_tau_decr > 0) h->adapt_decr = o.adapt_tau_decr;
     h->kflags = (has_box ? KF_BOX : 0) | (has_vel ? KF_VEL : 0) | (has_acc ? KF_ACC : 0) |
                 (mode == TOP_WAYPOINT_PINNED_Z ? KF_PIN_POS : 0);
     h->nseg = nseg; h->nseg_pad = (nseg + 31) / 32 * 32; h->stride = h->nseg_pad * LANES;
@@ -403,6 +431,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     const int n = 2 * s;
     auto wp = [&](long long b, long long j, int d) -> double { return d < dims ? waypoints[((size_t)b * (N + 1) + j) * dims + d] : 0.0; };
     gram_tables(s);                       // build the shared tables before the worker threads start
+    h->h_T.assign((size_t)nseg, 0.0); h->h_dp.assign((size_t)nseg * 3, 0);
     std::atomic<int> bad_operator(0);
     auto do_segments = [&](long long g0, long long g1) {
         for (long long gg = g0; gg < g1; ++gg) {
@@ -420,7 +449,9 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
                 org3[d] = wp(b, i, d);
                 p0[d] = 0; p1[d] = (xreal)wp(b, i + 1, d) - (xreal)wp(b, i, d);
                 origin[(size_t)d * NP + g] = org3[d];
+                h->h_dp[g * 3 + d] = p1[d];
             }
+            h->h_T[g] = Td;
             if (!build_operator(s, T, (xreal)rho, has_box, has_vel, has_acc, (int)mode, p0, p1, PmX, c0X)) {
                 bad_operator.store(1);
                 return;
@@ -483,17 +514,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
             }
         }
     };
-    {   // segments are independent: spread the precompute over the host cores
-        unsigned nt = std::thread::hardware_concurrency();
-        nt = std::max(1u, std::min(nt, 32u));
-        if (nseg < 2048) nt = 1;
-        std::vector<std::thread> pool;
-        const long long chunk = (nseg + nt - 1) / nt;
-        for (unsigned t = 1; t < nt; ++t)
-            if ((long long)t * chunk < nseg) pool.emplace_back(do_segments, (long long)t * chunk, std::min(nseg, (long long)(t + 1) * chunk));
-        do_segments(0, std::min(nseg, chunk));
-        for (auto& th : pool) th.join();
-    }
+    parallel_segments(nseg, do_segments);
     if (bad_operator.load())
         CREATE_FAIL(fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)"));
 
@@ -628,10 +649,60 @@ extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iter
             if (rp < tol && rd < tol) { if (first[b] < 0) first[b] = done; }
             else { all = false; first[b] = -1; }     // a trajectory counts as converged only while it stays below
         }
+        if (!all && (h->opt_flags & TOP_RHO_ADAPTIVE) && done < h->max_iter) {
+            // Eq. 24 with the residuals of this check; one rho for the whole batch: the norms are
+            // taken over all trajectories
+            double rp2 = 0, rd2 = 0;
+            for (int b = 0; b < h->batch; ++b) {
+                rp2 += h->h_res[b * 4 + 0] * h->h_res[b * 4 + 0];
+                rd2 += h->h_res[b * 4 + rd_idx] * h->h_res[b * 4 + rd_idx];
+            }
+            const double rp = std::sqrt(rp2), rd = std::sqrt(rd2);
+            double rho_new = h->rho;
+            if (rp > h->adapt_mu * rd) rho_new = h->rho * h->adapt_incr;
+            else if (rd > h->adapt_mu * rp) rho_new = h->rho / h->adapt_decr;
+            if (rho_new != h->rho) { st = top_set_rho(h, rho_new); if (st != TOP_OK) return st; }
+        }
     }
     if (iters) for (int b = 0; b < h->batch; ++b) iters[b] = first[b] >= 0 ? first[b] : done;
     return all ? TOP_OK : TOP_NOT_CONVERGED;
 }
+
+extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
+    if (!h) return TOP_E_INVALID;
+    if (!(rho > 0) || !std::isfinite(rho)) return fail(h, TOP_E_INVALID, "rho must be finite and > 0");
+    if (rho == h->rho) return TOP_OK;
+    if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
+    const size_t LS = (size_t)h->stride;
+    std::vector<double> Pm(MAXN * LS, 0.0), c0(3 * LS, 0.0);
+    std::atomic<int> bad(0);
+    const int s = h->s, dims = h->dims;
+    parallel_segments(h->nseg, [&](long long g0, long long g1) {
+        for (long long g = g0; g < g1; ++g) {
+            xreal p0[3] = {0, 0, 0}, PmX[MAXN * MAXN], c0X[MAXN * 3];
+            if (!build_operator(s, (xreal)h->h_T[g], (xreal)rho, h->has_box, h->has_vel, h->has_acc, (int)h->wp_mode, p0,
+                                &h->h_dp[(size_t)g * 3], PmX, c0X)) { bad.store(1); return; }
+            for (int lane = 0; lane < LANES; ++lane) {
+                const size_t gt = (size_t)g * LANES + lane;
+                for (int bb = 0; bb < MAXN; ++bb) Pm[(size_t)bb * LS + gt] = (double)((xreal)rho * PmX[lane * MAXN + bb]);
+                for (int d = 0; d < dims; ++d) c0[(size_t)d * LS + gt] = (double)c0X[lane * 3 + d];
+            }
+        }
+    });
+    if (bad.load()) return fail(h, TOP_E_INVALID, "x-update operator is not positive definite for this rho");
+    CU(cudaMemcpyAsync(h->d_Pm, Pm.data(), MAXN * LS * 8, cudaMemcpyHostToDevice, h->stream), "H2D operator");
+    CU(cudaMemcpyAsync(h->d_c0, c0.data(), 3 * LS * 8, cudaMemcpyHostToDevice, h->stream), "H2D operator");
+    RescaleParams r;
+    r.u = h->d_u; r.qp = h->d_qp; r.qn = h->d_qn; r.wv = h->d_wv; r.wa = h->d_wa;
+    r.count = 3 * (long long)LS; r.ratio = h->rho / rho;
+    CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
+    h->launches += 1;
+    CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");     // Pm / c0 staging buffers die here
+    h->rho = rho;
+    return TOP_OK;
+}
+
+extern "C" TOP_API double top_get_rho(const top_solver* h) { return h ? h->rho : std::numeric_limits<double>::quiet_NaN(); }
 
 extern "C" TOP_API top_status top_get_residuals(top_solver* h, double* r_primal, double* r_dual, double* r_dual_norm,
                                         double* r_primal_gap) {

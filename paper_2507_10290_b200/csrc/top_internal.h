@@ -75,6 +75,9 @@ size_t sweep_smem_bytes(int dtype, int s, bool constrained, uint32_t flags, int 
 int max_threads_for(int dtype);
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int threads, size_t smem, int* max_ctas_per_sm);
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
+// duals *= ratio after a change of rho: u, w (both balls), and the negative part of the Moreau values q (= -v)
+struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; };
+cudaError_t launch_rescale_duals(const RescaleParams& p, int dtype, cudaStream_t st);
 cudaError_t launch_residual_reduce(const double* part, double* res, long long N, int batch, cudaStream_t st);
 cudaError_t launch_fma_peak(int dtype, int blocks, int threads, long long iters, float* sink, cudaStream_t st);
 

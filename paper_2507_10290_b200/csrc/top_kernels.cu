@@ -561,6 +561,22 @@ __global__ void residual_reduce_kernel(const double* __restrict__ part, double* 
     if (t < 4) res[b * 4 + t] = sqrt(sh[t][0]);
 }
 
+// scaled duals after rho_old -> rho_new (reading A16): u, w_v, w_a *= ratio; box: v = max(0,-q) *= ratio, s unchanged
+template <typename Real>
+__global__ void rescale_duals_kernel(const RescaleParams p) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= p.count) return;
+    const Real r = (Real)p.ratio;
+    static_cast<Real*>(p.u)[i] *= r;
+    if (p.wv) static_cast<Real*>(p.wv)[i] *= r;
+    if (p.wa) static_cast<Real*>(p.wa)[i] *= r;
+    if (p.qp) {
+        Real* qp = static_cast<Real*>(p.qp); Real* qn = static_cast<Real*>(p.qn);
+        if (qp[i] < 0) qp[i] *= r;
+        if (qn[i] < 0) qn[i] *= r;
+    }
+}
+
 // dependent-chain-free FMA loop: 8 independent accumulators per thread; 2 flops per FMA
 template <typename Real>
 __global__ void fma_peak_kernel(long long iters, float* sink) {
@@ -650,6 +666,14 @@ cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st) {
     const int blocks = (int)((n + 255) / 256);
     if (dtype == 0) convert_coeffs_kernel<double><<<blocks, 256, 0, st>>>(p);
     else convert_coeffs_kernel<float><<<blocks, 256, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_rescale_duals(const RescaleParams& p, int dtype, cudaStream_t st) {
+    if (p.count == 0) return cudaSuccess;
+    const int blocks = (int)((p.count + 255) / 256);
+    if (dtype == 0) rescale_duals_kernel<double><<<blocks, 256, 0, st>>>(p);
+    else rescale_duals_kernel<float><<<blocks, 256, 0, st>>>(p);
     return cudaGetLastError();
 }
 

@@ -20,10 +20,11 @@ TOP_F64, TOP_F32 = 0, 1
 WAYPOINT = {"hard": 0, "pinned_z": 1, "free": 2}
 TOP_RD_NORMALISED = 4
 TOP_EPS_N_SCALED = 8
+TOP_RHO_ADAPTIVE = 64
 SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
 EXPORTS = ["top_create", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
-           "top_iteration", "top_launch_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
+           "top_iteration", "top_set_rho", "top_get_rho", "top_launch_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
            "top_destroy", "top_last_error"]
 
 
@@ -41,7 +42,8 @@ class _Constraints(ctypes.Structure):
 class _Options(ctypes.Structure):
     _fields_ = [("struct_size", ctypes.c_uint32), ("flags", ctypes.c_uint32), ("check_every", ctypes.c_int32),
                 ("device", ctypes.c_int32), ("max_iter", ctypes.c_int64), ("cuda_stream", ctypes.c_void_p),
-                ("segs_per_cta", ctypes.c_int32), ("reserved", ctypes.c_int32)]
+                ("segs_per_cta", ctypes.c_int32), ("reserved", ctypes.c_int32), ("adapt_mu", ctypes.c_double),
+                ("adapt_tau_incr", ctypes.c_double), ("adapt_tau_decr", ctypes.c_double)]
 
 
 _lib = None
@@ -73,6 +75,10 @@ def lib():
     L.top_get_coeffs.argtypes = [vp, vp, ctypes.c_int32]
     L.top_get_state.restype = ctypes.c_int
     L.top_get_state.argtypes = [vp, ctypes.c_char_p, dp, ctypes.c_size_t]
+    L.top_set_rho.restype = ctypes.c_int
+    L.top_set_rho.argtypes = [vp, ctypes.c_double]
+    L.top_get_rho.restype = ctypes.c_double
+    L.top_get_rho.argtypes = [vp]
     L.top_iteration.restype = ctypes.c_int64
     L.top_iteration.argtypes = [vp]
     L.top_launch_info.restype = ctypes.c_int
@@ -138,7 +144,8 @@ class TopSolver:
 
     def __init__(self, waypoints, durations, s, rho, dtype="f64", samples=0, box_lo=None, box_hi=None, vmax=0.0,
                  amax=0.0, start_derivs=None, end_derivs=None, mode="hard", rd_normalised=False, eps_n_scaled=False,
-                 sync="auto", check_every=0, max_iter=0, device=-1, stream=0, segs_per_cta=0):
+                 sync="auto", check_every=0, max_iter=0, device=-1, stream=0, segs_per_cta=0, adaptive_rho=False,
+                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0):
         L = lib()
         wp = np.asarray(waypoints, dtype=np.float64)
         T = np.asarray(durations, dtype=np.float64)
@@ -163,9 +170,10 @@ class TopSolver:
         if samples:
             cons = _Constraints(int(samples), _dptr(lo), _dptr(hi), float(vmax), float(amax))
         flags = WAYPOINT[mode] | (TOP_RD_NORMALISED if rd_normalised else 0) | \
-            (TOP_EPS_N_SCALED if eps_n_scaled else 0) | SYNC[sync]
+            (TOP_EPS_N_SCALED if eps_n_scaled else 0) | SYNC[sync] | (TOP_RHO_ADAPTIVE if adaptive_rho else 0)
         opt = _Options(ctypes.sizeof(_Options), flags, int(check_every), int(device), int(max_iter),
-                       ctypes.c_void_p(stream), int(segs_per_cta), 0)
+                       ctypes.c_void_p(stream), int(segs_per_cta), 0, float(adapt_mu), float(adapt_tau_incr),
+                       float(adapt_tau_decr))
         self._L = L
         self._h = ctypes.c_void_p()
         st = L.top_create(ctypes.byref(self._h), self.batch, self.N, self.s, self.dims,
@@ -200,6 +208,13 @@ class TopSolver:
         st = self._check(self._L.top_solve(self._h, float(eps), it.ctypes.data_as(ctypes.POINTER(ctypes.c_int64))),
                          ok=(TOP_OK, TOP_NOT_CONVERGED))
         return st == TOP_OK, it
+
+    def set_rho(self, rho: float):
+        self._check(self._L.top_set_rho(self._h, float(rho)))
+
+    @property
+    def rho(self) -> float:
+        return float(self._L.top_get_rho(self._h))
 
     def residuals(self):
         r = [np.zeros(self.batch) for _ in range(4)]

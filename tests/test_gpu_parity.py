@@ -253,3 +253,38 @@ def test_fp64_oracle_rounding_error_at_full_size():
     assert e_gpu < 1e-9
     assert e_oracle < 2e-9            # the fp64 oracle itself stays close to the bar ...
     assert np.abs(scaled(sol.coeffs()[0], T) - scaled(o.get("coeffs"), T)).max() / np.abs(ref).max() < 1e-9 + e_oracle
+
+
+# ------------------------------------------------------------------ adaptive rho (Eq. 24)
+
+def test_set_rho_matches_oracle_iterates():
+    w = W.small_constrained(N=37, s=4, acc=True)
+    o = make_oracle(w)
+    sol = top.from_workload(w, segs_per_cta=8)
+    for rho, k in [(10.0, 20), (3.0, 15), (47.0, 30), (10.0, 10)]:
+        sol.set_rho(rho); o.set_rho(rho)
+        assert sol.rho == rho
+        sol.iterate(k); o.sweep(k)
+        check_fields(field_errors(sol, [o], w), "after rho=%g" % rho)
+
+
+@pytest.mark.parametrize("every", [1, 8])
+def test_adaptive_solve_matches_oracle(every):
+    w = W.config2(N=40)
+    o = make_oracle(w)
+    n_ref = o.solve_adaptive(1e-3, 3000, every=every)
+    sol = top.from_workload(w, adaptive_rho=True, check_every=every, max_iter=3000)
+    ok, iters = sol.solve(1e-3)
+    assert sol.rho == pytest.approx(o.rho, rel=1e-12)        # the same sequence of Eq. 24 decisions
+    assert int(iters[0]) == n_ref and sol.iteration == o.iter
+    check_fields(field_errors(sol, [o], w), "adaptive, every=%d" % every)
+
+
+def test_adaptive_rho_config1_reaches_direct_solution():
+    w = W.config1()
+    sol = top.from_workload(w, adaptive_rho=True, check_every=1, max_iter=200000)
+    ok, iters = sol.solve(1e-6)
+    assert ok and sol.rho != 1.0
+    T = w.durations[0]
+    ref = direct.banded_optimality(w.waypoints[0], T, w.s)
+    assert np.abs(scaled(sol.coeffs()[0] - ref, T)).max() / np.abs(scaled(ref, T)).max() < 1e-6
