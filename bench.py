@@ -161,6 +161,7 @@ def main():
     ap.add_argument("--sweeps", type=int, default=0, help="sweeps per step (0 = the config's count, or 2000)")
     ap.add_argument("--sync", default="auto")
     ap.add_argument("--segs-per-cta", type=int, default=0)
+    ap.add_argument("--lanes", type=int, default=0, help="threads per segment: 0 = library default, 4 or 8")
     ap.add_argument("--oracle-seconds", type=float, default=12.0)
     ap.add_argument("--oracle-threads", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -194,7 +195,7 @@ def main():
     sweeps = args.sweeps or w.sweeps or 2000
     stream = torch.cuda.current_stream()
     sol = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync,
-                            segs_per_cta=args.segs_per_cta)
+                            segs_per_cta=args.segs_per_cta, lanes=args.lanes)
     info = sol.launch_info()
     info.pop("launches", None)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device="cuda")   # > 126 MB L2

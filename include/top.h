@@ -102,7 +102,7 @@ typedef struct {
     int64_t max_iter;       /* top_solve gives up after this many sweeps (default 1000000) */
     void* cuda_stream;      /* cudaStream_t; NULL = default stream */
     int32_t segs_per_cta;   /* segments per thread block, 0 = choose (a tuning knob; multiple of 4) */
-    int32_t reserved;
+    int32_t lanes_per_segment; /* threads per segment of the sweep kernel: 0 = choose, 4 or 8 (a tuning knob) */
     double adapt_mu;        /* Eq. 24: mu (> 1),       0 = the paper's 10 */
     double adapt_tau_incr;  /*         tau_incr (> 1), 0 = the paper's 1.1 */
     double adapt_tau_decr;  /*         tau_decr (> 1), 0 = the paper's 1.1 */

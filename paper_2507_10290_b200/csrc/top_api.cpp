@@ -37,7 +37,7 @@ struct top_solver {
     int device = 0;
     cudaStream_t stream = nullptr;
     long long nseg = 0, nseg_pad = 0, stride = 0;
-    int num_sms = 0, max_ctas = 0, user_segs = 0;
+    int num_sms = 0, max_ctas = 0, user_segs = 0, lanes = 8;
     struct Wave { long long seg_begin, seg_end; int segs_per_cta, ctas, threads; size_t smem; };
     std::vector<Wave> waves;
     // device buffers
@@ -262,10 +262,10 @@ top_status download_real(top_solver* h, const void* src, std::vector<double>& ds
 int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 // largest segments-per-CTA (multiple of 4) whose threads and shared memory fit one CTA
-int max_segs_per_cta(int dtype, int s, bool constrained, uint32_t kflags, size_t smem_limit) {
+int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, size_t smem_limit) {
     int best = 0;
-    for (int segs = 4; segs * LANES <= max_threads_for(dtype); segs += 4)
-        if (sweep_smem_bytes(dtype, s, constrained, kflags, segs) <= smem_limit) best = segs;
+    for (int segs = 4; (segs * lanes + 31) / 32 * 32 <= max_threads_for(dtype, lanes); segs += 4)
+        if (sweep_smem_bytes(dtype, s, constrained, lanes, segs) <= smem_limit) best = segs;
     return best;
 }
 
@@ -339,7 +339,8 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
         if (opt->struct_size >= offsetof(top_options, max_iter)) o.device = in.device;
         if (opt->struct_size >= offsetof(top_options, cuda_stream)) if (in.max_iter > 0) o.max_iter = in.max_iter;
         if (opt->struct_size >= offsetof(top_options, segs_per_cta)) o.cuda_stream = in.cuda_stream;
-        if (opt->struct_size >= offsetof(top_options, reserved)) o.segs_per_cta = in.segs_per_cta;
+        if (opt->struct_size >= offsetof(top_options, lanes_per_segment)) o.segs_per_cta = in.segs_per_cta;
+        if (opt->struct_size >= offsetof(top_options, adapt_mu)) o.lanes_per_segment = in.lanes_per_segment;
         if (opt->struct_size >= sizeof(top_options)) {
             o.adapt_mu = in.adapt_mu; o.adapt_tau_incr = in.adapt_tau_incr; o.adapt_tau_decr = in.adapt_tau_decr;
         }
@@ -347,6 +348,8 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     const uint32_t mode = o.flags & TOP_WAYPOINT_MASK;
     if (mode > TOP_WAYPOINT_FREE) return fail(h, TOP_E_INVALID, "unknown waypoint mode");
     if (o.segs_per_cta < 0 || (o.segs_per_cta % 4) != 0) return fail(h, TOP_E_INVALID, "segs_per_cta must be a multiple of 4");
+    if (o.lanes_per_segment != 0 && o.lanes_per_segment != 4 && o.lanes_per_segment != 8)
+        return fail(h, TOP_E_INVALID, "lanes_per_segment must be 0 (choose), 4 or 8");
     for (double v : {o.adapt_mu, o.adapt_tau_incr, o.adapt_tau_decr})
         if (v != 0 && !(v > 1 && std::isfinite(v))) return fail(h, TOP_E_INVALID, "adapt_mu / adapt_tau_* must be > 1 (or 0 = default)");
 
@@ -386,7 +389,12 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     int coop = 0;
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
     if (!coop) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "device lacks cooperative launch"));
-    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->kflags, (size_t)smem_optin - 1024);
+    // 8 lanes per segment unless told otherwise; 4 lanes (twice the registers per thread, two samples per lane) win
+    // for fp32 once every SM is full of segments (measured on config 5: 4.1e9 vs 3.3e9 segment-iterations/s), and
+    // lose for fp64 (register spills) and for short chains (longer serial path per warp)
+    h->lanes = o.lanes_per_segment ? o.lanes_per_segment : 8;
+    if (!o.lanes_per_segment && dtype == TOP_F32 && nseg >= (long long)h->num_sms * 96) h->lanes = 4;
+    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, (size_t)smem_optin - 1024);
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
     h->max_ctas = h->num_sms;
     const long long capacity = (long long)h->max_ctas * std::min(segs_max, h->user_segs ? h->user_segs : segs_max);
@@ -408,15 +416,15 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
             segs = std::max(4, std::min(segs, segs_max));
             w.segs_per_cta = segs;
             w.ctas = (int)((cnt + segs - 1) / segs);
-            w.threads = segs * LANES;
-            w.smem = sweep_smem_bytes(h->dtype, s, h->constrained, h->kflags, segs);
+            w.threads = (segs * h->lanes + 31) / 32 * 32;
+            w.smem = sweep_smem_bytes(h->dtype, s, h->constrained, h->lanes, segs);
             if (w.ctas > h->max_ctas) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "launch plan exceeds one CTA per SM"));
             h->waves.push_back(w);
         }
     }
     for (const auto& w : h->waves) {
         int per_sm = 0;
-        cudaError_t e = sweep_kernel_limits(h->dtype, s, h->constrained, w.threads, w.smem, &per_sm);
+        cudaError_t e = sweep_kernel_limits(h->dtype, s, h->constrained, h->lanes, w.threads, w.smem, &per_sm);
         if (e != cudaSuccess) CREATE_FAIL(cuda_fail(h, e, "occupancy query"));
         if (per_sm < 1) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "sweep kernel does not fit an SM"));
     }
@@ -600,7 +608,7 @@ top_status run_sweeps(top_solver* h, int64_t k) {
             h->seq_counter += (unsigned long long)kk;
             if (w.ctas > 1 && !(p.flags & KF_NEIGHBOUR_SYNC))
                 CU(cudaMemsetAsync(h->d_sync, 0, 8, h->stream), "cudaMemsetAsync");
-            CU(launch_sweeps(p, h->dtype, h->s, h->constrained, w.ctas, w.threads, w.smem, h->stream), "sweep kernel launch");
+            CU(launch_sweeps(p, h->dtype, h->s, h->constrained, h->lanes, w.ctas, w.threads, w.smem, h->stream), "sweep kernel launch");
             h->launches += 1;
         }
         k -= kk;
@@ -807,7 +815,9 @@ extern "C" TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dty
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) { cudaGetLastError(); return -1; }
     const uint32_t kf = constrained ? (KF_BOX | KF_VEL | KF_ACC) : 0;
-    return (int64_t)sms * max_segs_per_cta((int)dtype, s, constrained != 0, kf, (size_t)smem - 1024);
+    (void)kf;
+    return (int64_t)sms * std::max(max_segs_per_cta((int)dtype, s, constrained != 0, 8, (size_t)smem - 1024),
+                                   max_segs_per_cta((int)dtype, s, constrained != 0, 4, (size_t)smem - 1024));
 }
 
 extern "C" TOP_API double top_fma_peak(int32_t device, top_dtype dtype, int32_t reps, void* cuda_stream) {

@@ -69,11 +69,12 @@ struct ConvParams {       // coefficient conversion to the paper's basis (Eq. 18
 };
 
 // launchers (top_kernels.cu).  dtype: 0 = f64, 1 = f32.  Return cudaError_t.
-cudaError_t launch_sweeps(const KParams& p, int dtype, int s, bool constrained, int ctas, int threads,
+// `lanes` = threads per segment of the sweep kernel: 8 (cadmm_sweeps_kernel) or 4 (cadmm_sweeps_kernel4)
+cudaError_t launch_sweeps(const KParams& p, int dtype, int s, bool constrained, int lanes, int ctas, int threads,
                           size_t smem, cudaStream_t st);
-size_t sweep_smem_bytes(int dtype, int s, bool constrained, uint32_t flags, int segs_per_cta);
-int max_threads_for(int dtype);
-cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int threads, size_t smem, int* max_ctas_per_sm);
+size_t sweep_smem_bytes(int dtype, int s, bool constrained, int lanes, int segs_per_cta);
+int max_threads_for(int dtype, int lanes);
+cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, int threads, size_t smem, int* max_ctas_per_sm);
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
 // duals *= ratio after a change of rho: u, w (both balls), and the negative part of the Moreau values q (= -v)
 struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; };

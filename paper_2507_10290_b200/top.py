@@ -42,7 +42,7 @@ class _Constraints(ctypes.Structure):
 class _Options(ctypes.Structure):
     _fields_ = [("struct_size", ctypes.c_uint32), ("flags", ctypes.c_uint32), ("check_every", ctypes.c_int32),
                 ("device", ctypes.c_int32), ("max_iter", ctypes.c_int64), ("cuda_stream", ctypes.c_void_p),
-                ("segs_per_cta", ctypes.c_int32), ("reserved", ctypes.c_int32), ("adapt_mu", ctypes.c_double),
+                ("segs_per_cta", ctypes.c_int32), ("lanes_per_segment", ctypes.c_int32), ("adapt_mu", ctypes.c_double),
                 ("adapt_tau_incr", ctypes.c_double), ("adapt_tau_decr", ctypes.c_double)]
 
 
@@ -144,7 +144,7 @@ class TopSolver:
 
     def __init__(self, waypoints, durations, s, rho, dtype="f64", samples=0, box_lo=None, box_hi=None, vmax=0.0,
                  amax=0.0, start_derivs=None, end_derivs=None, mode="hard", rd_normalised=False, eps_n_scaled=False,
-                 sync="auto", check_every=0, max_iter=0, device=-1, stream=0, segs_per_cta=0, adaptive_rho=False,
+                 sync="auto", check_every=0, max_iter=0, device=-1, stream=0, segs_per_cta=0, lanes=0, adaptive_rho=False,
                  adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0):
         L = lib()
         wp = np.asarray(waypoints, dtype=np.float64)
@@ -172,7 +172,7 @@ class TopSolver:
         flags = WAYPOINT[mode] | (TOP_RD_NORMALISED if rd_normalised else 0) | \
             (TOP_EPS_N_SCALED if eps_n_scaled else 0) | SYNC[sync] | (TOP_RHO_ADAPTIVE if adaptive_rho else 0)
         opt = _Options(ctypes.sizeof(_Options), flags, int(check_every), int(device), int(max_iter),
-                       ctypes.c_void_p(stream), int(segs_per_cta), 0, float(adapt_mu), float(adapt_tau_incr),
+                       ctypes.c_void_p(stream), int(segs_per_cta), int(lanes), float(adapt_mu), float(adapt_tau_incr),
                        float(adapt_tau_decr))
         self._L = L
         self._h = ctypes.c_void_p()

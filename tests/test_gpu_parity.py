@@ -27,10 +27,10 @@ def check_fields(errs, where):
         assert v < tol, (where, k, v, errs)
 
 
-def run_parity(w, checkpoints, mode="hard", sync="auto", segs_per_cta=0, b_list=None, long_double=False, threads=1):
+def run_parity(w, checkpoints, mode="hard", sync="auto", segs_per_cta=0, b_list=None, long_double=False, threads=1, lanes=0):
     b_list = list(range(w.batch)) if b_list is None else b_list
     oracles = [make_oracle(w, b, mode=mode, long_double=long_double) for b in b_list]
-    sol = top.from_workload(w, mode=mode, sync=sync, segs_per_cta=segs_per_cta, dtype="f64")
+    sol = top.from_workload(w, mode=mode, sync=sync, segs_per_cta=segs_per_cta, dtype="f64", lanes=lanes)
     errs0 = field_errors(sol, oracles, w, b_list)       # iterate 0 (Init, reading A9)
     check_fields(errs0, "iterate 0")
     done = 0
@@ -288,3 +288,22 @@ def test_adaptive_rho_config1_reaches_direct_solution():
     T = w.durations[0]
     ref = direct.banded_optimality(w.waypoints[0], T, w.s)
     assert np.abs(scaled(sol.coeffs()[0] - ref, T)).max() / np.abs(scaled(ref, T)).max() < 1e-6
+
+
+# ------------------------------------------------------------------ the 4-lanes-per-segment kernel (cadmm_sweeps_kernel4)
+
+@pytest.mark.parametrize("s,acc,segs", [(3, False, 12), (3, True, 8), (4, False, 8), (4, True, 20)])
+@pytest.mark.parametrize("sync", ["grid", "pairwise"])
+def test_four_lane_kernel_small_ragged(s, acc, segs, sync):
+    w = W.small_constrained(N=37, s=s, acc=acc)
+    run_parity(w, [1, 2, 3, 10, 50, 200], sync=sync, segs_per_cta=segs, lanes=4)
+
+
+def test_four_lane_kernel_configs():
+    run_parity(W.config1(), [1, 10, 300], lanes=4)
+    run_parity(W.config1(), [1, 10, 100], lanes=4, mode="free")
+    run_parity(W.config2(), [1, 100, 1000], lanes=4)
+    run_parity(W.config3(), [1, 100], lanes=4)
+    run_parity(W.config4(), [1, 20, 100], lanes=4, long_double=True, threads=0)
+    w = W.small_constrained(N=19, s=4, acc=True, batch=5, seed=3)
+    run_parity(w, [1, 20, 100], segs_per_cta=8, lanes=4)
