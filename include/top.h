@@ -123,8 +123,9 @@ typedef struct {
  *   rho          > 0, penalty of Eq. 5; one rho for every penalty (A18)
  *   opt          NULL = defaults
  * Errors: TOP_E_INVALID (sizes, non-finite input, T<=0, lo>=hi, rho<=0, samples not in {0,8}),
- * TOP_E_NOMEM, TOP_E_CUDA, TOP_E_UNSUPPORTED (one trajectory longer than the on-chip capacity of the
- * persistent kernel, see top_capacity).  On error *out is NULL; top_last_error(NULL) has the message.
+ * TOP_E_NOMEM, TOP_E_CUDA, TOP_E_UNSUPPORTED.  A trajectory longer than the on-chip capacity of the persistent
+ * kernel (top_capacity) is streamed in pieces with halo segments (temporal blocking: same results, state
+ * round-trips through device memory every 64 sweeps).  On error *out is NULL; top_last_error(NULL) has the message.
  */
 TOP_API top_status top_create(top_solver** out, int32_t batch, int32_t N, int32_t s, int32_t dims, top_dtype dtype,
                       const double* waypoints, const double* durations,
@@ -183,7 +184,8 @@ TOP_API int64_t top_iteration(const top_solver* h);
 TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas, int32_t* threads, int32_t* segs_per_cta,
                            int32_t* smem_bytes, int32_t* waves, int64_t* launches);
 
-/* Largest N (segments of ONE trajectory) the persistent kernel can hold on the given device
+/* Largest N (segments of ONE trajectory) the persistent kernel can hold ON CHIP on the given device (longer
+ * trajectories are streamed)
  * (-1 = current) for this s / dtype / constraint selection; < 0 on error. */
 TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dtype, int32_t constrained);
 

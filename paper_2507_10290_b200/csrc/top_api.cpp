@@ -38,7 +38,13 @@ struct top_solver {
     cudaStream_t stream = nullptr;
     long long nseg = 0, nseg_pad = 0, stride = 0;
     int num_sms = 0, max_ctas = 0, user_segs = 0, lanes = 8;
-    struct Wave { long long seg_begin, seg_end; int segs_per_cta, ctas, threads; size_t smem; };
+    struct Wave { long long seg_begin, seg_end, own_begin, own_end; uint32_t kflags; int segs_per_cta, ctas, threads; size_t smem; };
+    // streaming (temporal blocking) for chains longer than the on-chip capacity: pieces with `halo` extra segments on
+    // each open side run `halo` sweeps per launch (the dependency radius of a sweep is one segment), reading iterate
+    // k from one set of state buffers and writing iterate k + halo of their own segments to the other set
+    bool streaming = false;
+    int halo = 0;
+    void* alt[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     std::vector<Wave> waves;
     // device buffers
     std::vector<void*> allocs;
@@ -398,28 +404,42 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
     h->max_ctas = h->num_sms;
     const long long capacity = (long long)h->max_ctas * std::min(segs_max, h->user_segs ? h->user_segs : segs_max);
+    auto make_wave = [&](long long r0, long long r1, long long o0, long long o1, uint32_t kf) -> bool {
+        top_solver::Wave w;
+        w.seg_begin = r0; w.seg_end = r1; w.own_begin = o0; w.own_end = o1; w.kflags = kf;
+        const long long cnt = r1 - r0;
+        int segs = h->user_segs ? h->user_segs : round_up((int)((cnt + h->max_ctas - 1) / h->max_ctas), 4);
+        segs = std::max(4, std::min(segs, segs_max));
+        w.segs_per_cta = segs;
+        w.ctas = (int)((cnt + segs - 1) / segs);
+        w.threads = (segs * h->lanes + 31) / 32 * 32;
+        w.smem = sweep_smem_bytes(h->dtype, s, h->constrained, h->lanes, segs);
+        if (w.ctas > h->max_ctas) return false;
+        h->waves.push_back(w);
+        return true;
+    };
     if ((long long)N > capacity) {
-        char msg[160];
-        std::snprintf(msg, sizeof msg, "one trajectory of N=%d segments exceeds the on-chip capacity of %lld segments", N, capacity);
-        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, msg));
-    }
-    {
+        // one trajectory does not fit on chip: stream the whole segment index space in pieces with halos
+        h->streaming = true;
+        h->halo = (int)std::min<long long>(64, std::max<long long>(1, capacity / 8));
+        const long long own_max = capacity - 2 * h->halo;
+        if (own_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "on-chip capacity too small to stream this trajectory"));
+        const long long npieces = (nseg + own_max - 1) / own_max;
+        const long long own = (nseg + npieces - 1) / npieces;
+        for (long long o0 = 0; o0 < nseg; o0 += own) {
+            const long long o1 = std::min(nseg, o0 + own);
+            const long long r0 = std::max<long long>(0, o0 - h->halo), r1 = std::min(nseg, o1 + h->halo);
+            if (!make_wave(r0, r1, o0, o1, (r0 > 0 ? KF_OPEN_LEFT : 0) | (r1 < nseg ? KF_OPEN_RIGHT : 0)))
+                CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "launch plan exceeds one CTA per SM"));
+        }
+    } else {
         const long long traj_cap = capacity / N;
         const long long nwaves = (batch + traj_cap - 1) / traj_cap;
         const long long per_wave = (batch + nwaves - 1) / nwaves;
         for (long long b0 = 0; b0 < batch; b0 += per_wave) {
             const long long b1 = std::min<long long>(batch, b0 + per_wave);
-            top_solver::Wave w;
-            w.seg_begin = b0 * N; w.seg_end = b1 * N;
-            const long long cnt = w.seg_end - w.seg_begin;
-            int segs = h->user_segs ? h->user_segs : round_up((int)((cnt + h->max_ctas - 1) / h->max_ctas), 4);
-            segs = std::max(4, std::min(segs, segs_max));
-            w.segs_per_cta = segs;
-            w.ctas = (int)((cnt + segs - 1) / segs);
-            w.threads = (segs * h->lanes + 31) / 32 * 32;
-            w.smem = sweep_smem_bytes(h->dtype, s, h->constrained, h->lanes, segs);
-            if (w.ctas > h->max_ctas) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "launch plan exceeds one CTA per SM"));
-            h->waves.push_back(w);
+            if (!make_wave(b0 * N, b1 * N, b0 * N, b1 * N, 0))
+                CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "launch plan exceeds one CTA per SM"));
         }
     }
     for (const auto& w : h->waves) {
@@ -538,6 +558,10 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     if (has_box) { ALLOC(h->d_qp, 3 * LS * rb, false); ALLOC(h->d_qn, 3 * LS * rb, false); }
     if (has_vel) { ALLOC(h->d_phv, 3 * LS * rb, false); ALLOC(h->d_wv, 3 * LS * rb, true); }
     if (has_acc) { ALLOC(h->d_pha, 3 * LS * rb, true); ALLOC(h->d_wa, 3 * LS * rb, true); }
+    if (h->streaming) {
+        void* cur[8] = {h->d_zt, h->d_u, h->d_qp, h->d_qn, h->d_phv, h->d_wv, h->d_pha, h->d_wa};
+        for (int i = 0; i < 8; ++i) if (cur[i]) ALLOC(h->alt[i], 3 * LS * rb, true);
+    }
     ALLOC(h->d_Bedge, (size_t)2 * h->max_ctas * 24 * 16, true);
     ALLOC(h->d_part, NP * 4 * 8, true); ALLOC(h->d_res, (size_t)batch * 4 * 8, true);
     ALLOC(h->d_sync, 16, true); ALLOC(h->d_abort, 16, true);
@@ -590,7 +614,9 @@ uint32_t sync_flag(const top_solver* h) {
 top_status run_sweeps(top_solver* h, int64_t k) {
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     while (k > 0) {
-        const int kk = (int)std::min<int64_t>(k, 1 << 30);
+        // streaming: at most `halo` sweeps per launch (that is how far a piece can run before the staleness of
+        // its halo reaches the segments it owns)
+        const int kk = (int)std::min<int64_t>(k, h->streaming ? h->halo : (1 << 30));
         for (const auto& w : h->waves) {
             KParams p;
             std::memset(&p, 0, sizeof p);
@@ -598,11 +624,19 @@ top_status run_sweeps(top_solver* h, int64_t k) {
             p.lohi = h->d_lohi; p.segflags = h->d_segflags; p.zoff = h->d_zoff;
             p.zt = h->d_zt; p.u = h->d_u; p.qp = h->d_qp; p.qn = h->d_qn; p.phv = h->d_phv; p.wv = h->d_wv;
             p.pha = h->d_pha; p.wa = h->d_wa; p.chat = h->d_chat;
+            if (h->streaming) {
+                p.zt_out = h->alt[0]; p.u_out = h->alt[1]; p.qp_out = h->alt[2]; p.qn_out = h->alt[3];
+                p.phv_out = h->alt[4]; p.wv_out = h->alt[5]; p.pha_out = h->alt[6]; p.wa_out = h->alt[7];
+            } else {
+                p.zt_out = p.zt; p.u_out = p.u; p.qp_out = p.qp; p.qn_out = p.qn;
+                p.phv_out = p.phv; p.wv_out = p.wv; p.pha_out = p.pha; p.wa_out = p.wa;
+            }
+            p.own_begin = w.own_begin; p.own_end = w.own_end;
             p.Bedge = h->d_Bedge; p.part = h->d_part;
             p.bar = reinterpret_cast<unsigned long long*>(h->d_sync);
             p.abort_flag = h->d_abort;
             p.stride = h->stride; p.nseg_pad = h->nseg_pad; p.seg_begin = w.seg_begin; p.seg_end = w.seg_end;
-            p.segs_per_cta = w.segs_per_cta; p.k_sweeps = kk; p.flags = h->kflags | sync_flag(h);
+            p.segs_per_cta = w.segs_per_cta; p.k_sweeps = kk; p.flags = h->kflags | sync_flag(h) | w.kflags;
             p.max_ctas = h->max_ctas; p.rho = h->rho; p.vmax = h->vmax; p.amax = h->amax;
             p.seq_base = (unsigned int)(h->seq_counter & 0xffffffffull);
             h->seq_counter += (unsigned long long)kk;
@@ -610,6 +644,11 @@ top_status run_sweeps(top_solver* h, int64_t k) {
                 CU(cudaMemsetAsync(h->d_sync, 0, 8, h->stream), "cudaMemsetAsync");
             CU(launch_sweeps(p, h->dtype, h->s, h->constrained, h->lanes, w.ctas, w.threads, w.smem, h->stream), "sweep kernel launch");
             h->launches += 1;
+        }
+        if (h->streaming) {       // every piece has written iterate k + kk of its own segments: swap the buffer sets
+            std::swap(h->d_zt, h->alt[0]); std::swap(h->d_u, h->alt[1]); std::swap(h->d_qp, h->alt[2]);
+            std::swap(h->d_qn, h->alt[3]); std::swap(h->d_phv, h->alt[4]); std::swap(h->d_wv, h->alt[5]);
+            std::swap(h->d_pha, h->alt[6]); std::swap(h->d_wa, h->alt[7]);
         }
         k -= kk;
         h->iter += kk;

@@ -17,7 +17,8 @@ constexpr uint8_t SEG_LAST = 2;   // last segment: right junction (z_N) is fixed
 
 // kernel flags
 constexpr uint32_t KF_BOX = 1, KF_VEL = 2, KF_ACC = 4, KF_PIN_POS = 8 /* PINNED_Z: position row of z held */,
-                   KF_NEIGHBOUR_SYNC = 16, KF_PAIRWISE = 32 /* warp-pair named barriers instead of the CTA barrier */;
+                   KF_NEIGHBOUR_SYNC = 16, KF_PAIRWISE = 32 /* warp-pair named barriers instead of the CTA barrier */,
+                   KF_OPEN_LEFT = 64, KF_OPEN_RIGHT = 128 /* streaming: the launch range starts / ends inside a chain (halo) */;
 
 // Per-lane field arrays: element [f * stride + gseg * LANES + lane]; stride = padded lane count.
 // "Real" is double (TOP_F64) or float (TOP_F32); the x-update operator is always double.
@@ -41,6 +42,8 @@ struct KParams {
     void* pha;              // Real [DIMS][stride]
     void* wa;               // Real [DIMS][stride]
     void* chat;             // Real [DIMS][stride]  coefficient row `lane` in normalised time (c^_a = c_a T^a)
+    // where the iterate is written at launch end (= the input arrays except in streaming mode: ping-pong buffers)
+    void *zt_out, *u_out, *qp_out, *qn_out, *phv_out, *wv_out, *pha_out, *wa_out;
     // ---- exchange / reduction
     void* Bedge;            // mailbox [2 parity][max_ctas][2 sides][4][DIMS] x 16-byte LL slots: boundary rows at CTA edges
     double* part;           // [nseg_pad][4]  per-segment residual partial sums (rp2, rd2, rdn2, gap2)
@@ -50,6 +53,7 @@ struct KParams {
     long long stride;       // lanes per field (>= nseg_pad * LANES)
     long long nseg_pad;
     long long seg_begin, seg_end;   // global segment range of this launch (a wave of whole trajectories)
+    long long own_begin, own_end;   // segments whose results are written back (streaming: range minus its halos)
     int segs_per_cta;
     int k_sweeps;
     uint32_t flags;

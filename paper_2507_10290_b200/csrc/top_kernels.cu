@@ -200,6 +200,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     // inactive lanes of a ragged CTA compute on a copy of the CTA's first segment (shuffles need full warps)
     // and never write to global memory
     const long long gseg = active ? cta_first + sl : cta_first;
+    // streaming (temporal blocking): the launch range carries halo segments that are computed but never written
+    const bool owned = active && gseg >= p.own_begin && gseg < p.own_end;
     const long long gt = gseg * LANES + lane;
     const long long stride = p.stride;
     const bool isrow = lane < N2;
@@ -222,6 +224,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     const Real invT = static_cast<const Real*>(p.invT)[gseg], invT2 = static_cast<const Real*>(p.invT)[p.nseg_pad + gseg];
     if (CONS && lane < 6) lohi[lane * SEGS + sl] = static_cast<const Real*>(p.lohi)[lane * p.nseg_pad + gseg];
     const uint8_t sf = p.segflags[gseg];
+    const bool open_l = (flags & KF_OPEN_LEFT) && gseg == p.seg_begin, open_r = (flags & KF_OPEN_RIGHT) && gseg == p.seg_end - 1;
 #pragma unroll
     for (int d = 0; d < 3; ++d) zoffs[d * T] = static_cast<const Real*>(p.zoff)[d * stride + gt];
     const Real tau = (Real)((double)(lane + 1) / (double)(MS + 1));       // sample time of this lane (reading A10)
@@ -319,7 +322,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
             }
 #pragma unroll
             for (int d = 0; d < 3; ++d) Cs[d * 8 + lane] = (Real)c[d];
-            if (last_sweep && active) {
+            if (last_sweep && owned) {
 #pragma unroll
                 for (int d = 0; d < 3; ++d) static_cast<Real*>(p.chat)[d * stride + gt] = (Real)c[d];
             }
@@ -456,7 +459,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
 #pragma unroll
                 for (int d = 0; d < 3; ++d) nb[d] += zoffs[d * T];
             }
-            const bool fixed = (right ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder == 0);
+            const bool fixed = (right ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder == 0) ||
+                               (right ? open_r : open_l);      // outer end of a halo: no neighbour in this launch
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const Real bl = right ? Bnd[d] : nb[d], br = right ? nb[d] : Bnd[d];
@@ -489,7 +493,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
             for (int m = 1; m < LANES; m <<= 1) {     // fixed-order tree over the 8 lanes of the segment
                 rp2 += shfl_xor(rp2, m); rd2 += shfl_xor(rd2, m); rdn2 += shfl_xor(rdn2, m); gap2 += shfl_xor(gap2, m);
             }
-            if (active && lane == 0) {
+            if (owned && lane == 0) {
                 double* o = p.part + gseg * 4;
                 o[0] = rp2; o[1] = rd2; o[2] = rdn2; o[3] = gap2;
             }
@@ -497,22 +501,22 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     }
 
     // ---- write iterate k + k_sweeps back
-    if (active) {
+    if (owned) {
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            static_cast<Real*>(p.zt)[d * stride + gt] = zt[d];
-            static_cast<Real*>(p.u)[d * stride + gt] = u[d];
+            static_cast<Real*>(p.zt_out)[d * stride + gt] = zt[d];
+            static_cast<Real*>(p.u_out)[d * stride + gt] = u[d];
             if (has_box) {
-                static_cast<Real*>(p.qp)[d * stride + gt] = qp[d];
-                static_cast<Real*>(p.qn)[d * stride + gt] = qn[d];
+                static_cast<Real*>(p.qp_out)[d * stride + gt] = qp[d];
+                static_cast<Real*>(p.qn_out)[d * stride + gt] = qn[d];
             }
             if (has_vel) {
-                static_cast<Real*>(p.phv)[d * stride + gt] = phv[d];
-                static_cast<Real*>(p.wv)[d * stride + gt] = wv[d];
+                static_cast<Real*>(p.phv_out)[d * stride + gt] = phv[d];
+                static_cast<Real*>(p.wv_out)[d * stride + gt] = wv[d];
             }
             if (has_acc) {
-                static_cast<Real*>(p.pha)[d * stride + gt] = pha[d];
-                static_cast<Real*>(p.wa)[d * stride + gt] = wa[d];
+                static_cast<Real*>(p.pha_out)[d * stride + gt] = pha[d];
+                static_cast<Real*>(p.wa_out)[d * stride + gt] = wa[d];
             }
         }
     }
@@ -597,6 +601,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel4(const KParams p)
     const int nact = remaining < SEGS ? (int)remaining : SEGS;
     const bool active = sl < nact;
     const long long gseg = active ? cta_first + sl : cta_first;
+    const bool owned = active && gseg >= p.own_begin && gseg < p.own_end;
     const long long stride = p.stride;
 
     // the two items of this lane: sample / row index jj[h], global lane slot gt[h]
@@ -638,6 +643,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel4(const KParams p)
         if (lane < 2) lohi[(lane + 4) * SA + sl] = static_cast<const Real*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
     }
     const uint8_t sf = p.segflags[gseg];
+    const bool open_l = (flags & KF_OPEN_LEFT) && gseg == p.seg_begin, open_r = (flags & KF_OPEN_RIGHT) && gseg == p.seg_end - 1;
     // ---- state of iterate k
     Real zt[2][3], u[2][3], qp[2][3], qn[2][3], phv[2][3], wv[2][3], pha[2][3], wa[2][3];
 #pragma unroll
@@ -731,7 +737,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel4(const KParams p)
                 Cs[d * 8 + jj[h]] = (Real)c;
             }
         }
-        if (last_sweep && active) {
+        if (last_sweep && owned) {
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
@@ -888,7 +894,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel4(const KParams p)
 #pragma unroll
                 for (int d = 0; d < 3; ++d) nb[d] += zoff[h][d];
             }
-            const bool fixed = (right[h] ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder[h] == 0);
+            const bool fixed = (right[h] ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder[h] == 0) ||
+                               (right[h] ? open_r : open_l);
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const Real bl = right[h] ? Bnd[h][d] : nb[d], br = right[h] ? nb[d] : Bnd[h][d];
@@ -929,7 +936,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel4(const KParams p)
             for (int m = 1; m < LPS; m <<= 1) {     // fixed-order tree over the 4 lanes of the segment
                 rp2 += shfl_xor(rp2, m); rd2 += shfl_xor(rd2, m); rdn2 += shfl_xor(rdn2, m); gap2 += shfl_xor(gap2, m);
             }
-            if (active && lane == 0) {
+            if (owned && lane == 0) {
                 double* o = p.part + gseg * 4;
                 o[0] = rp2; o[1] = rd2; o[2] = rdn2; o[3] = gap2;
             }
@@ -937,17 +944,17 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel4(const KParams p)
     }
 
     // ---- write iterate k + k_sweeps back
-    if (active) {
+    if (owned) {
 #pragma unroll
         for (int h = 0; h < 2; ++h)
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const long long i = d * stride + gt[h];
-                static_cast<Real*>(p.zt)[i] = zt[h][d];
-                static_cast<Real*>(p.u)[i] = u[h][d];
-                if (has_box) { static_cast<Real*>(p.qp)[i] = qp[h][d]; static_cast<Real*>(p.qn)[i] = qn[h][d]; }
-                if (has_vel) { static_cast<Real*>(p.phv)[i] = phv[h][d]; static_cast<Real*>(p.wv)[i] = wv[h][d]; }
-                if (has_acc) { static_cast<Real*>(p.pha)[i] = pha[h][d]; static_cast<Real*>(p.wa)[i] = wa[h][d]; }
+                static_cast<Real*>(p.zt_out)[i] = zt[h][d];
+                static_cast<Real*>(p.u_out)[i] = u[h][d];
+                if (has_box) { static_cast<Real*>(p.qp_out)[i] = qp[h][d]; static_cast<Real*>(p.qn_out)[i] = qn[h][d]; }
+                if (has_vel) { static_cast<Real*>(p.phv_out)[i] = phv[h][d]; static_cast<Real*>(p.wv_out)[i] = wv[h][d]; }
+                if (has_acc) { static_cast<Real*>(p.pha_out)[i] = pha[h][d]; static_cast<Real*>(p.wa_out)[i] = wa[h][d]; }
             }
     }
 }

@@ -160,14 +160,39 @@ def test_dims_1_and_2():
         run_parity(w, [1, 5, 50])
 
 
-def test_capacity_and_unsupported():
-    cap = top.capacity(4, "f64", True)
-    assert cap >= 10000
-    w = W.config3(N=cap + 8)
-    with pytest.raises(top.TopError) as e:
-        top.TopSolver(w.waypoints, w.durations, 4, 1.0, samples=8, vmax=3.0, amax=5.0,
-                      box_lo=w.waypoints[:, :-1] - 50, box_hi=w.waypoints[:, :-1] + 50)
-    assert e.value.status == top.TOP_E_UNSUPPORTED
+def test_capacity_is_reported():
+    assert top.capacity(4, "f64", True) >= 10000
+    assert top.capacity(3, "f32", False) >= 18000
+
+
+@pytest.mark.parametrize("lanes", [8, 4])
+def test_streaming_long_chain_matches_oracle(lanes):
+    """A chain longer than the on-chip capacity is streamed in pieces with halos (temporal blocking).  Forced here
+    with a small segs_per_cta (capacity = #SMs x 4 segments); N = 2000 -> several pieces, halo 64, so 150 sweeps
+    cross two halo refreshes.  Results must be those of the resident kernel: iterate parity with the oracle."""
+    w = W.small_constrained(N=2000, s=4, acc=True, seed=77)
+    # (long-double oracle: at this size the fp64 oracle's own rounding error is the size of the 1e-9 bar, see
+    # test_config4_full_size_iterates)
+    sol, (o,), worst = run_parity(w, [1, 2, 63, 64, 65, 150], segs_per_cta=4, lanes=lanes, threads=0, long_double=True)
+    assert sol.launch_info()["waves"] >= 3
+    # bitwise equal to the resident run (same per-segment arithmetic, same order)
+    ref = top.from_workload(w, segs_per_cta=16, lanes=lanes)
+    assert ref.launch_info()["waves"] == 1
+    ref.iterate(150)
+    for f in ("z", "u", "s_pos", "v_neg", "phi_v", "w_a"):
+        assert np.array_equal(sol.state(f), ref.state(f)), f
+    assert np.array_equal(sol.coeffs(), ref.coeffs())
+
+
+def test_streaming_beyond_capacity_unconstrained():
+    cap = top.capacity(3, "f64", False)
+    w = W.config3(N=cap + 1000, rho=10.0)
+    sol = top.from_workload(w)
+    assert sol.launch_info()["waves"] >= 2
+    sol.iterate(300)
+    T = w.durations[0]
+    ref = direct.banded_optimality(w.waypoints[0], T, w.s)
+    assert np.abs(scaled(sol.coeffs()[0] - ref, T)).max() / np.abs(scaled(ref, T)).max() < 1e-6
 
 
 # ------------------------------------------------------------------ BASELINE.json's full sizes, bench.py's launch plan
