@@ -145,9 +145,10 @@ TOP_API top_status top_iterate(top_solver* h, int64_t k);
 TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iters);
 
 /* top_set_rho -- change the penalty parameter between sweeps (the primitive under Eq. 24).  The x-update operator
- * of every segment is rebuilt for the new rho (host, extended precision, as in top_create) and uploaded, and the
- * SCALED duals u, v, w on the device are multiplied by rho_old/rho_new so that the multipliers y = rho*u are
- * unchanged (reading A16; the paper is silent; Boyd et al. 3.4.1).  Synchronises the stream.
+ * of every segment is re-evaluated on the device for the new rho (from the rho-independent spectral form that
+ * top_create precomputes in extended precision), and the SCALED duals u, v, w are multiplied by rho_old/rho_new
+ * so that the multipliers y = rho*u are unchanged (reading A16; the paper is silent; Boyd et al. 3.4.1).
+ * Two small kernels on the stream; no host synchronisation.
  * TOP_E_INVALID if rho <= 0 or not finite. */
 TOP_API top_status top_set_rho(top_solver* h, double rho);
 

@@ -49,11 +49,10 @@ struct top_solver {
     // device buffers
     std::vector<void*> allocs;
     double *d_Pm = nullptr, *d_c0 = nullptr, *d_part = nullptr, *d_res = nullptr;
+    double *d_W = nullptr, *d_lam = nullptr, *d_g0 = nullptr, *d_dp = nullptr;   // spectral operator data (rho-independent)
     void *d_invTk = nullptr, *d_Tpow = nullptr, *d_invT = nullptr, *d_lohi = nullptr, *d_zoff = nullptr;
     double* d_origin = nullptr;        // [3][nseg_pad] origin o_i = p_{i-1} of each segment's local frame
     std::vector<double> origin;        // host copy (top_get_state)
-    std::vector<double> h_T;           // [nseg] durations (operator rebuild on top_set_rho)
-    std::vector<xreal> h_dp;           // [nseg][3] p_i - p_{i-1} in extended precision
     uint32_t wp_mode = 0;
     double adapt_mu = 10.0, adapt_incr = 1.1, adapt_decr = 1.1;
     uint8_t* d_segflags = nullptr;
@@ -218,6 +217,148 @@ bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int
     return true;
 }
 
+// ---- rho-independent (spectral) form of the same operator, so that rho is a run-time parameter on the device.
+// H^(rho) = Q2 + rho G with Q2 = 2 T^(1-2s) Q(1) and G the Gram matrix of all penalty rows (Eq. 20a first bracket).
+// In the reduced basis Z (HARD: polynomials vanishing at both ends; else Z = I):  A_Q = Z'Q2 Z, A_G = Z'G Z (SPD).
+// Generalised symmetric eigenproblem A_Q v = lambda A_G v with V'A_G V = I, V'A_Q V = Lambda gives
+//     (A_Q + rho A_G)^-1 = V diag(1/(lambda_i + rho)) V'      =>     rho Pm^ = W diag(rho/(lambda_i + rho)) W',  W = Z V,
+// and, because the chord (degree 1 < s) is in the null space of Q2,  c0^ = c_chord - (rho Pm^) (G c_chord).
+// Everything below is done once per segment in extended precision (diagonal scaling, Cholesky of A_G, cyclic Jacobi
+// on L^-1 A_Q L^-T); the device only evaluates the two formulas above (refresh_operator_kernel).
+struct Spectral {
+    xreal W[MAXN * MAXN];     // [a][i], zero padded
+    xreal lam[MAXN];
+    xreal g0[MAXN * 3];       // G c_chord, [a][d]   (HARD mode; else 0)
+    xreal gcol0[MAXN];        // G e_0 (only top_precompute_operator needs it: a frame other than the local one)
+    int q;
+};
+
+bool jacobi_eigen(int q, std::vector<xreal>& C, std::vector<xreal>& U) {       // C symmetric -> diag; U its eigenvectors
+    U.assign(q * q, 0);
+    for (int i = 0; i < q; ++i) U[i * q + i] = 1;
+    for (int sweep = 0; sweep < 60; ++sweep) {
+        xreal off = 0, diag = 0;
+        for (int i = 0; i < q; ++i) for (int j = 0; j < q; ++j) (i == j ? diag : off) += C[i * q + j] * C[i * q + j];
+        if (off <= diag * (xreal)1e-40 || off == 0) return true;
+        for (int pp = 0; pp < q; ++pp)
+            for (int r = pp + 1; r < q; ++r) {
+                const xreal apq = C[pp * q + r];
+                if (apq == 0) continue;
+                const xreal theta = (C[r * q + r] - C[pp * q + pp]) / (2 * apq);
+                const xreal t = (theta >= 0 ? 1 : -1) / (std::fabs(theta) + std::sqrt(theta * theta + 1));
+                const xreal c = 1 / std::sqrt(t * t + 1), sn = t * c;
+                for (int k = 0; k < q; ++k) {       // columns
+                    const xreal a = C[k * q + pp], b = C[k * q + r];
+                    C[k * q + pp] = c * a - sn * b; C[k * q + r] = sn * a + c * b;
+                }
+                for (int k = 0; k < q; ++k) {       // rows
+                    const xreal a = C[pp * q + k], b = C[r * q + k];
+                    C[pp * q + k] = c * a - sn * b; C[r * q + k] = sn * a + c * b;
+                }
+                for (int k = 0; k < q; ++k) {
+                    const xreal a = U[k * q + pp], b = U[k * q + r];
+                    U[k * q + pp] = c * a - sn * b; U[k * q + r] = sn * a + c * b;
+                }
+            }
+    }
+    return true;
+}
+
+bool build_spectral(int s, xreal T, bool box, bool vel, bool acc, int mode, const xreal* dp, Spectral& S) {
+    const int n = 2 * s;
+    const GramTables& G = gram_tables(s);
+    xreal iT[8];
+    iT[0] = 1;
+    for (int k = 1; k < 8; ++k) iT[k] = iT[k - 1] / T;
+    const xreal wq = 2 * T * iT[2 * s - 1] * iT[1];             // 2 T^(1-2s)
+    std::vector<xreal> Q2(n * n), Gm(n * n);
+    for (int a = 0; a < n; ++a)
+        for (int b = 0; b < n; ++b) {
+            const int i = a * MAXN + b;
+            Q2[a * n + b] = wq * G.Q1[i];
+            xreal v = (box ? 2 * G.Ge[0][i] : 0) + (vel ? iT[2] * G.Ge[1][i] : 0) + (acc ? iT[4] * G.Ge[2][i] : 0);
+            for (int k = 0; k < s; ++k) v += iT[2 * k] * G.Gc[k][i];
+            Gm[a * n + b] = v;
+        }
+    const bool hard = mode == (int)TOP_WAYPOINT_HARD;
+    const int q = hard ? n - 2 : n;
+    std::vector<xreal> AQ(q * q), AG(q * q);
+    auto red = [&](const std::vector<xreal>& M, int i, int j) -> xreal {
+        if (!hard) return M[i * n + j];
+        const int a = i + 2, b = j + 2;                         // Z column i = e_a - e_1
+        return M[a * n + b] - M[a * n + 1] - M[1 * n + b] + M[1 * n + 1];
+    };
+    for (int i = 0; i < q; ++i) for (int j = 0; j < q; ++j) { AQ[i * q + j] = red(Q2, i, j); AG[i * q + j] = red(Gm, i, j); }
+    std::vector<xreal> sc(q);
+    for (int i = 0; i < q; ++i) { if (!(AG[i * q + i] > 0)) return false; sc[i] = 1 / std::sqrt(AG[i * q + i]); }
+    for (int i = 0; i < q; ++i) for (int j = 0; j < q; ++j) { AQ[i * q + j] *= sc[i] * sc[j]; AG[i * q + j] *= sc[i] * sc[j]; }
+    // Cholesky A_G = L L'
+    std::vector<xreal> Lm(q * q, 0);
+    for (int i = 0; i < q; ++i)
+        for (int j = 0; j <= i; ++j) {
+            xreal v = AG[i * q + j];
+            for (int k = 0; k < j; ++k) v -= Lm[i * q + k] * Lm[j * q + k];
+            if (i == j) { if (!(v > 0)) return false; Lm[i * q + i] = std::sqrt(v); }
+            else Lm[i * q + j] = v / Lm[j * q + j];
+        }
+    // C = L^-1 A_Q L^-T  (two triangular solves)
+    std::vector<xreal> Y(q * q), C(q * q), U;
+    for (int c = 0; c < q; ++c)                                   // Y = L^-1 A_Q
+        for (int i = 0; i < q; ++i) {
+            xreal v = AQ[i * q + c];
+            for (int k = 0; k < i; ++k) v -= Lm[i * q + k] * Y[k * q + c];
+            Y[i * q + c] = v / Lm[i * q + i];
+        }
+    for (int r = 0; r < q; ++r)                                   // C = Y L^-T  <=>  C L' = Y, row by row
+        for (int j = 0; j < q; ++j) {
+            xreal v = Y[r * q + j];
+            for (int k = 0; k < j; ++k) v -= C[r * q + k] * Lm[j * q + k];
+            C[r * q + j] = v / Lm[j * q + j];
+        }
+    for (int i = 0; i < q; ++i) for (int j = 0; j < i; ++j) { const xreal m = (C[i * q + j] + C[j * q + i]) / 2; C[i * q + j] = C[j * q + i] = m; }
+    if (!jacobi_eigen(q, C, U)) return false;
+    // V = S L^-T U
+    std::vector<xreal> V(q * q);
+    for (int c = 0; c < q; ++c)
+        for (int i = q - 1; i >= 0; --i) {
+            xreal v = U[i * q + c];
+            for (int k = i + 1; k < q; ++k) v -= Lm[k * q + i] * V[k * q + c];
+            V[i * q + c] = v / Lm[i * q + i];
+        }
+    for (int i = 0; i < q; ++i) for (int c = 0; c < q; ++c) V[i * q + c] *= sc[i];
+    std::memset(&S, 0, sizeof S);
+    S.q = q;
+    for (int i = 0; i < q; ++i) S.lam[i] = C[i * q + i] > 0 ? C[i * q + i] : 0;
+    for (int i = 0; i < q; ++i) {
+        if (hard) {
+            xreal sum = 0;
+            for (int a = 2; a < n; ++a) { S.W[a * MAXN + i] = V[(a - 2) * q + i]; sum += V[(a - 2) * q + i]; }
+            S.W[1 * MAXN + i] = -sum;
+        } else {
+            for (int a = 0; a < n; ++a) S.W[a * MAXN + i] = V[a * q + i];
+        }
+    }
+    if (hard) for (int a = 0; a < n; ++a) for (int d = 0; d < 3; ++d) S.g0[a * 3 + d] = Gm[a * n + 1] * dp[d];
+    for (int a = 0; a < n; ++a) S.gcol0[a] = Gm[a * n + 0];
+    return true;
+}
+
+// host twin of refresh_operator_kernel (extended precision): rho Pm^ and c0^ from the spectral form
+void spectral_operator(const Spectral& S, int n, bool hard, xreal rho, const xreal* dp, xreal* rhoPm /*[8][8]*/, xreal* c0 /*[8][3]*/) {
+    for (int a = 0; a < MAXN; ++a)
+        for (int b = 0; b < MAXN; ++b) {
+            xreal v = 0;
+            for (int i = 0; i < S.q; ++i) v += S.W[a * MAXN + i] * S.W[b * MAXN + i] * (rho / (S.lam[i] + rho));
+            rhoPm[a * MAXN + b] = v;
+        }
+    for (int a = 0; a < MAXN; ++a)
+        for (int d = 0; d < 3; ++d) {
+            xreal v = (hard && a == 1) ? dp[d] : 0;
+            for (int b = 0; b < n; ++b) v -= rhoPm[a * MAXN + b] * S.g0[b * 3 + d];
+            c0[a * 3 + d] = v;
+        }
+}
+
 template <typename Real>
 void project_ball_host(const double* y, double bound, Real* phi) {
     const double n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
@@ -278,6 +419,16 @@ int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, size_t smem_
 }  // namespace
 
 namespace {
+// (re)build rho*Pm^ and c0^ on the device for `rho` from the spectral data
+cudaError_t refresh_operator(top_solver* h, double rho) {
+    RefreshParams r;
+    r.W = h->d_W; r.lam = h->d_lam; r.g0 = h->d_g0; r.dp = h->d_dp; r.Pm = h->d_Pm; r.c0 = h->d_c0;
+    r.stride = h->stride; r.nseg_pad = h->nseg_pad; r.nseg = h->nseg;
+    r.q = h->wp_mode == TOP_WAYPOINT_HARD ? h->n - 2 : h->n;
+    r.rho = rho;
+    h->launches += 1;
+    return launch_refresh_operator(r, h->stream);
+}
 // run fn(g0, g1) over [0, n) on the host cores (segments are independent)
 template <typename F> void parallel_segments(long long n, F fn) {
     unsigned nt = std::thread::hardware_concurrency();
@@ -451,7 +602,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
 
     // ---- host precompute (extended precision) and iterate 0 (reading A9), packed per lane
     const size_t LS = (size_t)h->stride, NP = (size_t)h->nseg_pad;
-    std::vector<double> Pm(MAXN * LS, 0.0), c0(3 * LS, 0.0), invTk(LS, 0.0), Tpow(LS, 0.0), invT(2 * NP, 0.0),
+    std::vector<double> Wv(MAXN * LS, 0.0), g0v(3 * LS, 0.0), lamv(MAXN * NP, 0.0), dpv(3 * NP, 0.0), invTk(LS, 0.0), Tpow(LS, 0.0), invT(2 * NP, 0.0),
         lohi(6 * NP, 0.0), zt(3 * LS, 0.0), chat(3 * LS, 0.0), zoff(3 * LS, 0.0), origin(3 * NP, 0.0), qp, qn, phv, pha;
     std::vector<uint8_t> segflags(NP, 0);
     if (has_box) { qp.assign(3 * LS, 0.0); qn.assign(3 * LS, 0.0); }
@@ -459,7 +610,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     const int n = 2 * s;
     auto wp = [&](long long b, long long j, int d) -> double { return d < dims ? waypoints[((size_t)b * (N + 1) + j) * dims + d] : 0.0; };
     gram_tables(s);                       // build the shared tables before the worker threads start
-    h->h_T.assign((size_t)nseg, 0.0); h->h_dp.assign((size_t)nseg * 3, 0);
+
     std::atomic<int> bad_operator(0);
     auto do_segments = [&](long long g0, long long g1) {
         for (long long gg = g0; gg < g1; ++gg) {
@@ -471,19 +622,20 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
             // z~, box bounds) is stored relative to the origin o_i = p_{i-1}.  An exact change of variable (the
             // sweep only ever uses position differences) that keeps the operator free of the cancellation of
             // |p| ~ 100 m against segment-sized quantities; top_get_coeffs / top_get_state add o_i back.
-            xreal p0[3], p1[3], PmX[MAXN * MAXN], c0X[MAXN * 3];
+            xreal p0[3], p1[3];
             double org3[3];
             for (int d = 0; d < 3; ++d) {
                 org3[d] = wp(b, i, d);
                 p0[d] = 0; p1[d] = (xreal)wp(b, i + 1, d) - (xreal)wp(b, i, d);
                 origin[(size_t)d * NP + g] = org3[d];
-                h->h_dp[g * 3 + d] = p1[d];
             }
-            h->h_T[g] = Td;
-            if (!build_operator(s, T, (xreal)rho, has_box, has_vel, has_acc, (int)mode, p0, p1, PmX, c0X)) {
+            Spectral SP;
+            if (!build_spectral(s, T, has_box, has_vel, has_acc, (int)mode, p1, SP)) {
                 bad_operator.store(1);
                 return;
             }
+            for (int ii = 0; ii < MAXN; ++ii) lamv[(size_t)ii * NP + g] = ii < SP.q ? (double)SP.lam[ii] : 0.0;
+            for (int d = 0; d < 3; ++d) dpv[(size_t)d * NP + g] = (mode == TOP_WAYPOINT_HARD && d < dims) ? (double)p1[d] : 0.0;
             segflags[g] = (uint8_t)((i == 0 ? SEG_FIRST : 0) | (i == N - 1 ? SEG_LAST : 0));
             invT[g] = (double)(1 / T); invT[NP + g] = (double)(1 / (T * T));
             for (int d = 0; d < 3; ++d) {
@@ -492,8 +644,8 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
             }
             for (int lane = 0; lane < LANES; ++lane) {
                 const size_t gt = g * LANES + lane;
-                for (int bb = 0; bb < MAXN; ++bb) Pm[(size_t)bb * LS + gt] = (double)((xreal)rho * PmX[lane * MAXN + bb]);
-                for (int d = 0; d < 3; ++d) c0[(size_t)d * LS + gt] = d < dims ? (double)c0X[lane * 3 + d] : 0.0;
+                for (int ii = 0; ii < MAXN; ++ii) Wv[(size_t)ii * LS + gt] = (double)SP.W[lane * MAXN + ii];
+                for (int d = 0; d < 3; ++d) g0v[(size_t)d * LS + gt] = d < dims ? (double)SP.g0[lane * 3 + d] : 0.0;
                 Tpow[gt] = (double)std::pow(T, (xreal)lane);
                 // a neighbour's position row arrives in the neighbour's frame: shift it into this segment's frame
                 for (int d = 0; d < dims; ++d) {
@@ -551,6 +703,8 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     top_status st;
 #define ALLOC(ptr, bytes, zero) do { void* p__ = nullptr; st = dev_alloc(h, &p__, (bytes), (zero)); if (st != TOP_OK) CREATE_FAIL(st); ptr = static_cast<decltype(ptr)>(p__); } while (0)
     ALLOC(h->d_Pm, MAXN * LS * 8, false); ALLOC(h->d_c0, 3 * LS * 8, false);
+    ALLOC(h->d_W, MAXN * LS * 8, false); ALLOC(h->d_g0, 3 * LS * 8, false);
+    ALLOC(h->d_lam, MAXN * NP * 8, false); ALLOC(h->d_dp, 3 * NP * 8, false);
     ALLOC(h->d_invTk, LS * rb, false); ALLOC(h->d_Tpow, LS * rb, false); ALLOC(h->d_invT, 2 * NP * rb, false);
     ALLOC(h->d_lohi, 6 * NP * rb, false); ALLOC(h->d_segflags, NP, false);
     ALLOC(h->d_zoff, 3 * LS * rb, false); ALLOC(h->d_origin, 3 * NP * 8, false);
@@ -574,8 +728,11 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     h->h_abort[0] = 0;
 
     cudaError_t ce;
-    if ((ce = cudaMemcpyAsync(h->d_Pm, Pm.data(), MAXN * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
-        (ce = cudaMemcpyAsync(h->d_c0, c0.data(), 3 * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+    if ((ce = cudaMemcpyAsync(h->d_W, Wv.data(), MAXN * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_g0, g0v.data(), 3 * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_lam, lamv.data(), MAXN * NP * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = cudaMemcpyAsync(h->d_dp, dpv.data(), 3 * NP * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
+        (ce = refresh_operator(h, rho)) != cudaSuccess ||
         (ce = cudaMemcpyAsync(h->d_segflags, segflags.data(), NP, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
         (ce = cudaMemcpyAsync(h->d_origin, origin.data(), 3 * NP * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
         (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
@@ -721,30 +878,12 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
     if (rho == h->rho) return TOP_OK;
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     const size_t LS = (size_t)h->stride;
-    std::vector<double> Pm(MAXN * LS, 0.0), c0(3 * LS, 0.0);
-    std::atomic<int> bad(0);
-    const int s = h->s, dims = h->dims;
-    parallel_segments(h->nseg, [&](long long g0, long long g1) {
-        for (long long g = g0; g < g1; ++g) {
-            xreal p0[3] = {0, 0, 0}, PmX[MAXN * MAXN], c0X[MAXN * 3];
-            if (!build_operator(s, (xreal)h->h_T[g], (xreal)rho, h->has_box, h->has_vel, h->has_acc, (int)h->wp_mode, p0,
-                                &h->h_dp[(size_t)g * 3], PmX, c0X)) { bad.store(1); return; }
-            for (int lane = 0; lane < LANES; ++lane) {
-                const size_t gt = (size_t)g * LANES + lane;
-                for (int bb = 0; bb < MAXN; ++bb) Pm[(size_t)bb * LS + gt] = (double)((xreal)rho * PmX[lane * MAXN + bb]);
-                for (int d = 0; d < dims; ++d) c0[(size_t)d * LS + gt] = (double)c0X[lane * 3 + d];
-            }
-        }
-    });
-    if (bad.load()) return fail(h, TOP_E_INVALID, "x-update operator is not positive definite for this rho");
-    CU(cudaMemcpyAsync(h->d_Pm, Pm.data(), MAXN * LS * 8, cudaMemcpyHostToDevice, h->stream), "H2D operator");
-    CU(cudaMemcpyAsync(h->d_c0, c0.data(), 3 * LS * 8, cudaMemcpyHostToDevice, h->stream), "H2D operator");
+    CU(refresh_operator(h, rho), "operator refresh launch");      // on the device, from the spectral data: no host work
     RescaleParams r;
     r.u = h->d_u; r.qp = h->d_qp; r.qn = h->d_qn; r.wv = h->d_wv; r.wa = h->d_wa;
     r.count = 3 * (long long)LS; r.ratio = h->rho / rho;
     CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
     h->launches += 1;
-    CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");     // Pm / c0 staging buffers die here
     h->rho = rho;
     return TOP_OK;
 }
@@ -896,8 +1035,28 @@ extern "C" TOP_API top_status top_precompute_operator(int32_t s, double T, doubl
         return fail(nullptr, TOP_E_INVALID, "top_precompute_operator: bad argument");
     xreal a[3], b[3], PmX[MAXN * MAXN], c0X[MAXN * 3];
     for (int d = 0; d < 3; ++d) { a[d] = p0[d]; b[d] = p1[d]; }
-    if (!build_operator(s, (xreal)T, (xreal)rho, box != 0, vel != 0, acc != 0, (int)(flags & TOP_WAYPOINT_MASK), a, b, PmX, c0X))
-        return fail(nullptr, TOP_E_INVALID, "operator is not positive definite");
+    {
+        // the spectral path top_create and top_set_rho use (local frame: p0 is the origin); the direct inverse
+        // build_operator() is kept as an in-library cross-check of it
+        const int mode = (int)(flags & TOP_WAYPOINT_MASK);
+        xreal dp[3] = {b[0] - a[0], b[1] - a[1], b[2] - a[2]}, zero[3] = {0, 0, 0}, PmD[MAXN * MAXN], c0D[MAXN * 3], rPm[MAXN * MAXN];
+        Spectral S;
+        if (!build_spectral(s, (xreal)T, box != 0, vel != 0, acc != 0, mode, dp, S))
+            return fail(nullptr, TOP_E_INVALID, "operator is not positive definite");
+        spectral_operator(S, 2 * s, mode == (int)TOP_WAYPOINT_HARD, (xreal)rho, dp, rPm, c0X);
+        if (!build_operator(s, (xreal)T, (xreal)rho, box != 0, vel != 0, acc != 0, mode, zero, dp, PmD, c0D))
+            return fail(nullptr, TOP_E_INVALID, "operator is not positive definite");
+        xreal worst = 0, scale = 0;
+        for (int i = 0; i < MAXN * MAXN; ++i) { PmX[i] = rPm[i] / (xreal)rho; worst = std::max(worst, std::fabs(PmX[i] - PmD[i])); scale = std::max(scale, std::fabs(PmD[i])); }
+        if (worst > (xreal)1e-13 * scale) return fail(nullptr, TOP_E_INVALID, "spectral and direct operators disagree");
+        if (mode == (int)TOP_WAYPOINT_HARD)     // the caller's frame: the chord also carries p0 in c^_0
+            for (int r = 0; r < MAXN; ++r)
+                for (int d = 0; d < 3; ++d) {
+                    xreal v = (r == 0) ? a[d] : 0;
+                    for (int c = 0; c < 2 * s; ++c) v -= rPm[r * MAXN + c] * S.gcol0[c] * a[d];
+                    c0X[r * 3 + d] += v;
+                }
+    }
     for (int i = 0; i < MAXN * MAXN; ++i) Pm_hat[i] = (double)PmX[i];
     for (int i = 0; i < MAXN * 3; ++i) c0_hat[i] = (double)c0X[i];
     return TOP_OK;

@@ -80,6 +80,19 @@ size_t sweep_smem_bytes(int dtype, int s, bool constrained, int lanes, int segs_
 int max_threads_for(int dtype, int lanes);
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, int threads, size_t smem, int* max_ctas_per_sm);
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
+// rho Pm^ = W diag(rho/(lambda_i+rho)) W',  c0^ = c_chord - (rho Pm^) g0   (spectral form; top_api.cpp build_spectral)
+struct RefreshParams {
+    const double* W;      // [MAXN i][stride]  W[lane][i]
+    const double* lam;    // [MAXN i][nseg_pad]
+    const double* g0;     // [DIMS][stride]    (G c_chord)[lane][d]
+    const double* dp;     // [DIMS][nseg_pad]  p_i - p_{i-1} (c_chord row 1; HARD mode), else zeros
+    double* Pm;           // out [MAXN b][stride]
+    double* c0;           // out [DIMS][stride]
+    long long stride, nseg_pad, nseg;
+    int q;                // number of spectral components (n-2 in HARD mode, else n)
+    double rho;
+};
+cudaError_t launch_refresh_operator(const RefreshParams& p, cudaStream_t st);
 // duals *= ratio after a change of rho: u, w (both balls), and the negative part of the Moreau values q (= -v)
 struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; };
 cudaError_t launch_rescale_duals(const RescaleParams& p, int dtype, cudaStream_t st);

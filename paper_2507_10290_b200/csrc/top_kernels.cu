@@ -1002,6 +1002,32 @@ __global__ void residual_reduce_kernel(const double* __restrict__ part, double* 
     if (t < 4) res[b * 4 + t] = sqrt(sh[t][0]);
 }
 
+// Operator refresh for a new rho, fp64: one thread per (segment, lane a) evaluates row a of rho Pm^ and of c0^ from the
+// rho-independent spectral data (Eq. 20a first bracket as a function of rho; SURVEY 8(f)-1 "operator refresh").
+__global__ void refresh_operator_kernel(const RefreshParams p) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= p.nseg * LANES) return;
+    const long long seg = idx / LANES;
+    double wd[MAXN];
+    for (int i = 0; i < MAXN; ++i) {
+        const double lam = i < p.q ? p.lam[i * p.nseg_pad + seg] : 0.0;
+        wd[i] = i < p.q ? p.W[i * p.stride + idx] * (p.rho / (lam + p.rho)) : 0.0;
+    }
+    double pm[MAXN];
+    for (int b = 0; b < MAXN; ++b) {
+        double v = 0.0;
+        for (int i = 0; i < p.q; ++i) v += wd[i] * p.W[i * p.stride + seg * LANES + b];
+        pm[b] = v;
+        p.Pm[b * p.stride + idx] = v;
+    }
+    const int a = (int)(idx % LANES);
+    for (int d = 0; d < 3; ++d) {
+        double v = a == 1 ? p.dp[d * p.nseg_pad + seg] : 0.0;
+        for (int b = 0; b < MAXN; ++b) v -= pm[b] * p.g0[d * p.stride + seg * LANES + b];
+        p.c0[d * p.stride + idx] = v;
+    }
+}
+
 // scaled duals after rho_old -> rho_new (reading A16): u, w_v, w_a *= ratio; box: v = max(0,-q) *= ratio, s unchanged
 template <typename Real>
 __global__ void rescale_duals_kernel(const RescaleParams p) {
@@ -1150,6 +1176,13 @@ cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st) {
     const int blocks = (int)((n + 255) / 256);
     if (dtype == 0) convert_coeffs_kernel<double><<<blocks, 256, 0, st>>>(p);
     else convert_coeffs_kernel<float><<<blocks, 256, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_refresh_operator(const RefreshParams& p, cudaStream_t st) {
+    const long long n = p.nseg * LANES;
+    if (n == 0) return cudaSuccess;
+    refresh_operator_kernel<<<(int)((n + 127) / 128), 128, 0, st>>>(p);
     return cudaGetLastError();
 }
 
