@@ -239,7 +239,7 @@ bool jacobi_eigen(int q, std::vector<xreal>& C, std::vector<xreal>& U) {       /
     for (int sweep = 0; sweep < 60; ++sweep) {
         xreal off = 0, diag = 0;
         for (int i = 0; i < q; ++i) for (int j = 0; j < q; ++j) (i == j ? diag : off) += C[i * q + j] * C[i * q + j];
-        if (off <= diag * (xreal)1e-40 || off == 0) return true;
+        if (off <= diag * (xreal)1e-37 || off == 0) return true;   // off-diagonal mass below the rounding of long double
         for (int pp = 0; pp < q; ++pp)
             for (int r = pp + 1; r < q; ++r) {
                 const xreal apq = C[pp * q + r];
