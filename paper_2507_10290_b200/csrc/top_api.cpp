@@ -62,6 +62,9 @@ struct top_solver {
     int* d_abort = nullptr;
     double* h_res = nullptr;           // pinned [batch][4]
     int* h_abort = nullptr;            // pinned
+    void* d_resbox = nullptr;          // in-kernel solve: LL slots of the per-CTA residual partial sums
+    double* d_solve = nullptr;         // in-kernel solve result [8]
+    double* h_solve = nullptr;         // pinned
     bool have_residuals = false;
     int64_t iter = 0, launches = 0;
     unsigned long long seq_counter = 0;   // sweeps launched so far over all waves (mailbox sequence space)
@@ -551,7 +554,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     // lose for fp64 (register spills) and for short chains (longer serial path per warp)
     h->lanes = o.lanes_per_segment ? o.lanes_per_segment : 8;
     if (!o.lanes_per_segment && dtype == TOP_F32 && nseg >= (long long)h->num_sms * 96) h->lanes = 4;
-    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, (size_t)smem_optin - 1024);
+    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, (size_t)smem_optin - 8192);
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
     h->max_ctas = h->num_sms;
     const long long capacity = (long long)h->max_ctas * std::min(segs_max, h->user_segs ? h->user_segs : segs_max);
@@ -720,9 +723,10 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     ALLOC(h->d_part, NP * 4 * 8, true); ALLOC(h->d_res, (size_t)batch * 4 * 8, true);
     ALLOC(h->d_sync, 16, true); ALLOC(h->d_abort, 16, true);
     ALLOC(h->d_coef, (size_t)nseg * dims * n * rb, false);
+    ALLOC(h->d_resbox, (size_t)2 * h->max_ctas * 4 * 16, true); ALLOC(h->d_solve, 64, true);
 #undef ALLOC
     if (cudaMallocHost((void**)&h->h_res, (size_t)batch * 4 * 8) != cudaSuccess ||
-        cudaMallocHost((void**)&h->h_abort, 16) != cudaSuccess)
+        cudaMallocHost((void**)&h->h_abort, 16) != cudaSuccess || cudaMallocHost((void**)&h->h_solve, 64) != cudaSuccess)
         CREATE_FAIL(fail(h, TOP_E_NOMEM, "pinned host allocation failed"));
     for (long long i = 0; i < (long long)batch * 4; ++i) h->h_res[i] = std::numeric_limits<double>::quiet_NaN();
     h->h_abort[0] = 0;
@@ -768,7 +772,9 @@ uint32_t sync_flag(const top_solver* h) {
 }
 
 // k sweeps on every wave, then the per-trajectory residual reduction.  Asynchronous.
-top_status run_sweeps(top_solver* h, int64_t k) {
+struct InKernelSolve { int check_every; int rd_sel; int adaptive; double tol; };
+
+top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullptr) {
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     while (k > 0) {
         // streaming: at most `halo` sweeps per launch (that is how far a piece can run before the staleness of
@@ -794,6 +800,14 @@ top_status run_sweeps(top_solver* h, int64_t k) {
             p.abort_flag = h->d_abort;
             p.stride = h->stride; p.nseg_pad = h->nseg_pad; p.seg_begin = w.seg_begin; p.seg_end = w.seg_end;
             p.segs_per_cta = w.segs_per_cta; p.k_sweeps = kk; p.flags = h->kflags | sync_flag(h) | w.kflags;
+            if (iks) {      // device-side stop rule / Eq. 24 (one CTA-wide barrier per sweep: no warp-pair barriers)
+                p.flags &= ~KF_PAIRWISE;
+                p.check_every = iks->check_every; p.rd_sel = iks->rd_sel; p.adaptive = iks->adaptive; p.tol = iks->tol;
+                p.mu = h->adapt_mu; p.tau_incr = h->adapt_incr; p.tau_decr = h->adapt_decr;
+                p.q = h->wp_mode == TOP_WAYPOINT_HARD ? h->n - 2 : h->n;
+                p.resbox = h->d_resbox; p.solve_out = h->d_solve;
+                p.W = h->d_W; p.lam = h->d_lam; p.g0 = h->d_g0; p.dp = h->d_dp;
+            }
             p.max_ctas = h->max_ctas; p.rho = h->rho; p.vmax = h->vmax; p.amax = h->amax;
             p.seq_base = (unsigned int)(h->seq_counter & 0xffffffffull);
             h->seq_counter += (unsigned long long)kk;
@@ -808,7 +822,20 @@ top_status run_sweeps(top_solver* h, int64_t k) {
             std::swap(h->d_pha, h->alt[6]); std::swap(h->d_wa, h->alt[7]);
         }
         k -= kk;
-        h->iter += kk;
+        if (iks) {
+            // how far did the kernel get, and with which rho?
+            CU(cudaMemcpyAsync(h->h_solve, h->d_solve, 64, cudaMemcpyDeviceToHost, h->stream), "D2H solve result");
+            CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+            const int64_t done = (int64_t)h->h_solve[0];
+            h->iter += done;
+            if (h->h_solve[2] != h->rho) {      // the kernel refreshed its on-chip operator only: bring the arrays along
+                h->rho = h->h_solve[2];
+                CU(refresh_operator(h, h->rho), "operator refresh launch");
+            }
+            if (h->h_solve[1] != 0.0 || done < kk) break;
+        } else {
+            h->iter += kk;
+        }
     }
     CU(launch_residual_reduce(h->d_part, h->d_res, h->N, h->batch, h->stream), "residual reduction launch");
     h->launches += 1;
@@ -836,6 +863,24 @@ extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iter
     if (!(eps > 0)) return fail(h, TOP_E_INVALID, "eps must be > 0");
     const double tol = (h->opt_flags & TOP_EPS_N_SCALED) ? eps * h->N : eps;
     const int rd_idx = (h->opt_flags & TOP_RD_NORMALISED) ? 2 : 1;
+    // (large CTAs run the plain kernel faster than the solve instantiation -- 96-register cap -- so with a sparse
+    // test cadence they keep the host loop below)
+    if (h->batch == 1 && h->waves.size() == 1 && !h->streaming && h->lanes == 8 && h->waves[0].ctas <= 160 &&
+        (h->waves[0].threads <= 256 || h->check_every < 16)) {
+        // one resident trajectory: the stop rule (and Eq. 24) runs inside the kernel, one launch for the whole solve
+        InKernelSolve iks;
+        iks.check_every = h->check_every; iks.rd_sel = rd_idx; iks.adaptive = (h->opt_flags & TOP_RHO_ADAPTIVE) ? 1 : 0;
+        iks.tol = tol;
+        const int64_t it0 = h->iter;
+        top_status st = run_sweeps(h, h->max_iter, &iks);
+        if (st != TOP_OK) return st;
+        st = fetch_residuals(h);
+        if (st != TOP_OK) return st;
+        if (iters) iters[0] = h->iter - it0;
+        const double rp = h->h_res[0], rd = h->h_res[rd_idx];
+        if (!std::isfinite(rp) || !std::isfinite(rd)) return fail(h, TOP_E_NONFINITE, "non-finite residual");
+        return h->h_solve[1] != 0.0 ? TOP_OK : TOP_NOT_CONVERGED;
+    }
     std::vector<int64_t> first(h->batch, -1);
     int64_t done = 0;
     bool all = false;
@@ -853,7 +898,7 @@ extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iter
             if (rp < tol && rd < tol) { if (first[b] < 0) first[b] = done; }
             else { all = false; first[b] = -1; }     // a trajectory counts as converged only while it stays below
         }
-        if (!all && (h->opt_flags & TOP_RHO_ADAPTIVE) && done < h->max_iter) {
+        if (!all && (h->opt_flags & TOP_RHO_ADAPTIVE)) {
             // Eq. 24 with the residuals of this check; one rho for the whole batch: the norms are
             // taken over all trajectories
             double rp2 = 0, rd2 = 0;
@@ -1069,6 +1114,7 @@ extern "C" TOP_API top_status top_destroy(top_solver* h) {
     for (void* p : h->allocs) cudaFree(p);
     if (h->h_res) cudaFreeHost(h->h_res);
     if (h->h_abort) cudaFreeHost(h->h_abort);
+    if (h->h_solve) cudaFreeHost(h->h_solve);
     cudaGetLastError();
     delete h;
     return TOP_OK;

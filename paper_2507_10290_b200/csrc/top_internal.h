@@ -60,6 +60,15 @@ struct KParams {
     int max_ctas;
     unsigned int seq_base;  // sweeps launched before this launch (mod 2^32): mailbox sequence numbers never repeat
     double rho, vmax, amax;
+    // ---- in-kernel solve (cadmm_sweeps_kernel only; check_every == 0: plain k sweeps)
+    int check_every;        // test the stop rule (Eq. 23) inside the kernel every this many sweeps
+    int rd_sel;             // which dual residual is tested: 1 = Eq. 22, 2 = normalised
+    int adaptive;           // apply Eq. 24 after every test
+    int q;                  // spectral components (operator refresh)
+    double tol, mu, tau_incr, tau_decr;
+    void* resbox;           // [2][max_ctas][4] LL slots: per-CTA residual partial sums, all-gathered by every CTA
+    double* solve_out;      // [8]: sweeps done, stopped (0/1), rho, r_p, r_d, r_d_norm, r_p_gap, unused
+    const double *W, *lam, *g0, *dp;   // spectral operator data (RefreshParams)
 };
 
 struct ConvParams {       // coefficient conversion to the paper's basis (Eq. 18)

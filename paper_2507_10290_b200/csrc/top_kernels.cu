@@ -171,7 +171,9 @@ __device__ __forceinline__ void ball_update(const Real (&val)[3], Real bound, Re
     for (int d = 0; d < 3; ++d) { phi[d] = scale * y[d]; w[d] = y[d] - phi[d]; }
 }
 
-template <typename Real, int S, bool CONS, int MAXT>
+// SOLVE = true adds the device-side stop rule / Eq. 24 (a separate instantiation: the plain sweep loop keeps its
+// register allocation)
+template <typename Real, int S, bool CONS, int MAXT, bool SOLVE>
 __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) {
     constexpr int N2 = 2 * S;                      // n = 2s coefficients = 2s consensus rows per segment
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -262,10 +264,20 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
     // Warps may then drift up to one sweep apart, which de-synchronises their use of the fp64 pipe.
     const bool pairwise = nb_sync && nctas > 1 && nwarps <= 17 && (flags & KF_PAIRWISE);
     __syncthreads();
+    // in-kernel solve: stop rule and Eq. 24 evaluated on the device (all CTAs all-gather their residual partial
+    // sums through LL slots and take the same decision from the same numbers)
+    const int ce = SOLVE ? p.check_every : 0;
+    double rho_cur = p.rho;
+    __shared__ double wsum_sh[SOLVE ? 32 : 1][4];
+    __shared__ double allp_sh[SOLVE ? 160 : 1][4];
+    __shared__ double tot_sh[4];
+    int ncheck = 0, sweeps_done = p.k_sweeps, stopped = 0;
     for (int it = 0; it < p.k_sweeps; ++it) {
         const unsigned seq = p.seq_base + (unsigned)it + 1u;     // launch-unique sweep number (never reused)
         const int par = (int)(seq & 1u);
-        const bool last_sweep = (it == p.k_sweeps - 1);
+        const bool final_sweep = (it == p.k_sweeps - 1);
+        // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
+        const bool last_sweep = final_sweep || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
         Real* const Bcur = Bs + (size_t)par * (SEGS + 2) * 24;
 
         // ================= phase A: segment local =================
@@ -322,7 +334,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
             }
 #pragma unroll
             for (int d = 0; d < 3; ++d) Cs[d * 8 + lane] = (Real)c[d];
-            if (last_sweep && owned) {
+            if (last_sweep && owned) {      // (every test sweep as well: the solve may stop there)
 #pragma unroll
                 for (int d = 0; d < 3; ++d) static_cast<Real*>(p.chat)[d * stride + gt] = (Real)c[d];
             }
@@ -485,7 +497,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
                 Real v[8];
 #pragma unroll
                 for (int a = 0; a < 8; ++a) v[a] = a < N2 ? bc[a] * gd : (Real)0;
-                const double xr = p.rho * (double)reduce_scatter8(v, lane);
+                const double xr = rho_cur * (double)reduce_scatter8(v, lane);
                 rdn2 += xr * xr;
                 rd2 += (xr * Tp) * (xr * Tp);
             }
@@ -497,7 +509,86 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
                 double* o = p.part + gseg * 4;
                 o[0] = rp2; o[1] = rd2; o[2] = rdn2; o[3] = gap2;
             }
+            if (SOLVE && ce > 0) {
+                // ---- CTA partial (fixed order), all-gather over the CTAs, decision
+                double q4[4] = {rp2, rd2, rdn2, gap2};
+                if (!(owned && lane == 0)) { q4[0] = q4[1] = q4[2] = q4[3] = 0.0; }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) { q4[k] += shfl_xor(q4[k], 8); q4[k] += shfl_xor(q4[k], 16); }
+                if ((tid & 31) == 0) { for (int k = 0; k < 4; ++k) wsum_sh[tid >> 5][k] = q4[k]; }
+                __syncthreads();
+                unsigned char* const rb = static_cast<unsigned char*>(p.resbox) + (size_t)(ncheck & 1) * p.max_ctas * 4 * 16;
+                if (tid == 0) {
+                    for (int k = 0; k < 4; ++k) {
+                        double acc = 0.0;
+                        for (int w = 0; w < (T >> 5); ++w) acc += wsum_sh[w][k];
+                        ll_store(rb + ((size_t)cta * 4 + k) * 16, acc, seq);
+                    }
+                }
+                int gather_failed = 0;
+                for (int t = tid; t < nctas; t += T) {
+                    const long long t0 = global_ns();
+                    unsigned spins = 0;
+                    for (int k = 0; k < 4; ++k) {
+                        LLRaw r;
+                        ll_issue(rb + ((size_t)t * 4 + k) * 16, r);
+                        while (!ll_ok(r, seq)) {
+                            if ((++spins & 255u) == 0 && (*(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS)) {
+                                atomicExch(p.abort_flag, 1); gather_failed = 1; break;
+                            }
+                            ll_issue(rb + ((size_t)t * 4 + k) * 16, r);
+                        }
+                        allp_sh[t][k] = ll_value(r);
+                    }
+                }
+                gather_failed = __syncthreads_or(gather_failed);
+                if (tid < 4) {
+                    double acc = 0.0;
+                    for (int t = 0; t < nctas; ++t) acc += allp_sh[t][tid];
+                    tot_sh[tid] = acc;
+                }
+                __syncthreads();
+                ++ncheck;
+                const double rp = sqrt(tot_sh[0]), rd = sqrt(tot_sh[p.rd_sel]);
+                const bool conv = rp < p.tol && rd < p.tol;
+                if (conv || gather_failed || !(rp == rp) || !(rd == rd)) { stopped = conv ? 1 : 0; sweeps_done = it + 1; break; }
+                if (p.adaptive) {      // Eq. 24, then reading A16 for the scaled duals
+                    double rho_new = rho_cur;
+                    if (rp > p.mu * rd) rho_new = rho_cur * p.tau_incr;
+                    else if (rd > p.mu * rp) rho_new = rho_cur / p.tau_decr;
+                    if (rho_new != rho_cur) {
+                        const Real ratio = (Real)(rho_cur / rho_new);
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) {
+                            u[d] *= ratio; wv[d] *= ratio; wa[d] *= ratio;
+                            if (qp[d] < 0) qp[d] *= ratio;
+                            if (qn[d] < 0) qn[d] *= ratio;
+                        }
+                        // operator refresh from the spectral form (as refresh_operator_kernel): my row of rho Pm^, c0^
+                        double wd[MAXN];
+                        for (int i = 0; i < MAXN; ++i) {
+                            const double lam = i < p.q ? p.lam[i * p.nseg_pad + gseg] : 0.0;
+                            wd[i] = i < p.q ? p.W[i * stride + gt] * (rho_new / (lam + rho_new)) : 0.0;
+                        }
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) c0[d] = lane == 1 ? p.dp[d * p.nseg_pad + gseg] : 0.0;
+                        for (int b = 0; b < N2; ++b) {
+                            double v = 0.0;
+                            for (int i = 0; i < p.q; ++i) v += wd[i] * p.W[i * stride + gseg * LANES + b];
+                            Pms[b * T + tid] = v;
+#pragma unroll
+                            for (int d = 0; d < 3; ++d) c0[d] -= v * p.g0[d * stride + gseg * LANES + b];
+                        }
+                        rho_cur = rho_new;
+                    }
+                }
+            }
         }
+    }
+    if (SOLVE && ce > 0 && cta == 0 && tid == 0) {
+        double* o = p.solve_out;
+        o[0] = (double)sweeps_done; o[1] = (double)stopped; o[2] = rho_cur;
+        o[3] = sqrt(tot_sh[0]); o[4] = sqrt(tot_sh[1]); o[5] = sqrt(tot_sh[2]); o[6] = sqrt(tot_sh[3]);
     }
 
     // ---- write iterate k + k_sweeps back
@@ -1065,7 +1156,7 @@ __global__ void fma_peak_kernel(long long iters, float* sink) {
 
 template <typename Real, int S, bool CONS, int MAXT>
 cudaError_t launch_one(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
-    auto kern = cadmm_sweeps_kernel<Real, S, CONS, MAXT>;
+    auto kern = p.check_every > 0 ? cadmm_sweeps_kernel<Real, S, CONS, MAXT, true> : cadmm_sweeps_kernel<Real, S, CONS, MAXT, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     KParams pc = p;
@@ -1095,7 +1186,7 @@ cudaError_t limits_one4(int threads, size_t smem, int* per_sm) {
 
 template <typename Real, int S, bool CONS, int MAXT>
 cudaError_t limits_one(int threads, size_t smem, int* per_sm) {
-    auto kern = cadmm_sweeps_kernel<Real, S, CONS, MAXT>;
+    auto kern = cadmm_sweeps_kernel<Real, S, CONS, MAXT, true>;     // the larger of the two instantiations
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);

@@ -332,3 +332,40 @@ def test_four_lane_kernel_configs():
     run_parity(W.config4(), [1, 20, 100], lanes=4, long_double=True, threads=0)
     w = W.small_constrained(N=19, s=4, acc=True, batch=5, seed=3)
     run_parity(w, [1, 20, 100], segs_per_cta=8, lanes=4)
+
+
+# ------------------------------------------------------------------ device-side stop rule (in-kernel top_solve)
+
+def test_in_kernel_solve_many_ctas_matches_oracle_count():
+    """N=1000 -> 125 CTAs of 64 threads: every CTA all-gathers the 125 residual partial sums and stops at the same
+    sweep as the oracle (check every sweep)."""
+    w = W.config3(rho=10.0)
+    o = make_oracle(w)
+    n_ref = o.solve(1e-3, 5000)
+    sol = top.from_workload(w, check_every=1, max_iter=5000)
+    ok, iters = sol.solve(1e-3)
+    assert ok and int(iters[0]) == n_ref and sol.iteration == n_ref
+    check_fields(field_errors(sol, [o], w), "in-kernel solve, 125 CTAs")
+    r, ro = sol.residuals(), o.residuals()
+    assert r["r_p"][0] < 1e-3 and abs(r["r_p"][0] - ro["r_p"]) < 1e-9 * max(1.0, ro["r_p"])
+
+
+def test_in_kernel_solve_equals_host_loop():
+    """batch = 1 uses the in-kernel stop rule, batch = 2 (two copies) the host loop: same count, same iterate."""
+    w1 = W.config2(N=40)
+    a = top.from_workload(w1, check_every=8, max_iter=40000, rd_normalised=True)
+    ok_a, it_a = a.solve(1.0)
+    w2 = W.config2(N=40)
+    w2.batch = 2
+    for name in ("waypoints", "durations", "box_lo", "box_hi"):
+        setattr(w2, name, np.concatenate([getattr(w1, name)] * 2, axis=0))
+    b = top.from_workload(w2, check_every=8, max_iter=40000, rd_normalised=True)
+    ok_b, it_b = b.solve(1.0)
+    assert ok_a and ok_b and int(it_a[0]) == int(it_b[0]) == int(it_b[1])
+    assert np.array_equal(a.coeffs()[0], b.coeffs()[0]) and np.array_equal(a.coeffs()[0], b.coeffs()[1])
+    # cap reached: both report the cap and stay usable
+    c = top.from_workload(w1, check_every=8, max_iter=24)
+    ok_c, it_c = c.solve(1e-12)
+    assert not ok_c and int(it_c[0]) == 24 and c.iteration == 24
+    c.iterate(8)
+    assert c.iteration == 32
