@@ -369,3 +369,50 @@ def test_in_kernel_solve_equals_host_loop():
     assert not ok_c and int(it_c[0]) == 24 and c.iteration == 24
     c.iterate(8)
     assert c.iteration == 32
+
+
+# ------------------------------------------------------------------ API surface
+
+def test_device_output_and_user_stream():
+    """top_get_coeffs into a device buffer, everything enqueued on a caller-provided (non-default) stream."""
+    import torch
+    w = W.small_constrained(N=37, s=4, acc=True)
+    st = torch.cuda.Stream()
+    with torch.cuda.stream(st):
+        sol = top.from_workload(w, stream=st.cuda_stream, segs_per_cta=8)
+        sol.iterate(25)
+        out = torch.zeros((1, w.N, 3, 8), dtype=torch.float64, device="cuda")
+        sol.coeffs_to_device(out.data_ptr())
+        st.synchronize()
+    host = sol.coeffs()
+    assert np.array_equal(out.cpu().numpy(), host)
+    o = make_oracle(w)
+    o.sweep(25)
+    T = w.durations[0]
+    assert np.abs(scaled(host[0] - o.get("coeffs"), T)).max() / np.abs(scaled(o.get("coeffs"), T)).max() < 1e-9
+    # fp32 solver writes fp32 coefficients
+    s32 = top.from_workload(w, dtype="f32")
+    s32.iterate(5)
+    assert s32.coeffs().dtype == np.float32
+
+
+def test_state_accessor_errors_and_iterate_zero():
+    import ctypes
+    w = W.small_constrained(N=5, s=3, acc=False)
+    sol = top.from_workload(w)
+    assert np.all(np.isnan(sol.residuals()["r_p"]))            # NaN before the first sweep
+    sol.iterate(0)
+    assert sol.iteration == 0
+    with pytest.raises(top.TopError) as e:
+        sol.state("no_such_field")
+    assert e.value.status == top.TOP_E_INVALID
+    buf = np.zeros(7)
+    st = sol._L.top_get_state(sol._h, b"z", buf.ctypes.data_as(ctypes.POINTER(ctypes.c_double)), buf.size)
+    assert st == top.TOP_E_INVALID
+    assert np.all(sol.state("phi_a") == 0)                     # a constraint set that is off reads as zeros
+    with pytest.raises(top.TopError):
+        sol.iterate(-1)
+    with pytest.raises(top.TopError):
+        sol.set_rho(-2.0)
+    z0 = sol.state("z")
+    assert np.array_equal(z0[0, :, 0, :], w.waypoints[0])      # iterate 0: z positions are the waypoints (A9)
