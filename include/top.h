@@ -141,6 +141,9 @@ TOP_API top_status top_iterate(top_solver* h, int64_t k);
  * readings A6, A7, A8, A13), testing every check_every sweeps, or until max_iter sweeps (of this call).
  *   iters  host [batch] or NULL: sweeps done (in this call) when that trajectory first passed the test,
  *          or the total if it never did.
+ * One resident trajectory: a single launch, the test (and Eq. 24 with TOP_RHO_ADAPTIVE) runs inside the kernel.
+ * Batches and streamed chains: launches of check_every sweeps with the test on the host (32 bytes D2H per test); the
+ * call ends when every trajectory is below eps at the same test.
  * Returns TOP_OK, TOP_NOT_CONVERGED, TOP_E_NONFINITE, TOP_E_CUDA.  Synchronises the stream. */
 TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iters);
 
