@@ -253,8 +253,8 @@ def main():
             out["roofline"] = {"bound": "alu", "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
                                "frac": ach / peak,
                                # DRAM bytes per launch (read + write) from the committed ncu capture of this command
-                               # (profiles/r1_v1_cfg4_ncu_summary.md); independent of the sweep count: state is on chip
-                               "traffic": 27513088 if args.workload == "cfg4" else None,
+                               # (profiles/r1_final_cfg4_ncu_summary.md); independent of the sweep count: state is on chip
+                               "traffic": 27850240 if args.workload == "cfg4" else None,
                                "peak_source": "measured in this run: top_fma_peak (%s FMA loop, all SMs)" % dt_name,
                                "flops_per_segment_sweep": fl}
         peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
