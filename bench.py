@@ -256,7 +256,9 @@ def main():
                                # (profiles/r1_final_cfg4_ncu_summary.md); independent of the sweep count: state is on chip
                                "traffic": 27850240 if args.workload == "cfg4" else None,
                                "peak_source": "measured in this run: top_fma_peak (%s FMA loop, all SMs)" % dt_name,
-                               "flops_per_segment_sweep": fl}
+                               "flops_per_segment_sweep": fl,
+                               # unit count x clock: 148 SMs x 64 fp64 (128 fp32) FMA/clk x 2 x SM clock
+                               "peak_derived": 148 * (64 if dt_name == "f64" else 128) * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e12}
         peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
         if os.path.exists(peaks_path):
             out["measured_peaks"] = {k: v for k, v in json.load(open(peaks_path)).items() if k in ("hbm_gbs", "sm_max_mhz")}
