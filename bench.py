@@ -151,6 +151,45 @@ def run_reference(args, rank, world):
                       "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}))
 
 
+def run_fig5(args, local_rank):
+    """Stand-in for the paper's Fig. 5: solve time and similarity e_simi = lg sum_i |p_i - p_i_ref|
+    (M = 8192 points) against the number of segments, to the paper's tolerance ||r|| < N * 0.05."""
+    import torch
+    from paper_2507_10290_b200 import build as top_build
+    from paper_2507_10290_b200 import top
+    top_build.build()
+    torch.cuda.set_device(local_rank)
+    stream = torch.cuda.current_stream()
+    rows = []
+    M = 8192
+    for N in (64, 128, 256, 512, 1024, 2048, 4096, 8192):
+        w = W.fig5(N)
+        best = None
+        for rep in range(3):
+            sol = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, eps_n_scaled=True, check_every=8,
+                                    max_iter=200000)
+            torch.cuda.synchronize(); t0 = time.perf_counter()
+            ok, it = sol.solve(0.05)
+            torch.cuda.synchronize(); dt = time.perf_counter() - t0
+            if best is None or dt < best[0]:
+                best = (dt, bool(ok), int(it[0]), sol.coeffs()[0], sol.residuals())
+            sol.close()
+        dt, ok, it, c, res = best
+        # evaluate the optimised trajectory at M parameters uniform in theta (plain Horner; measurement, not method)
+        th = (np.arange(M) + 0.5) * (2.0 * np.pi / M)          # mid-points: never a knot, whatever N
+        seg = np.minimum((th / (2.0 * np.pi) * N).astype(np.int64), N - 1)
+        tau = th / (2.0 * np.pi) * N - seg
+        t = tau * w.durations[0][seg]
+        P = np.zeros((M, 3))
+        for a in range(c.shape[-1] - 1, -1, -1):
+            P = P * t[:, None] + c[seg, :, a]
+        e = np.sqrt(((P - W.fig5_curve(th)) ** 2).sum(axis=1)).sum()
+        rows.append({"N": N, "converged": ok, "sweeps": it, "solve_ms": 1e3 * dt, "e_simi": float(np.log10(e)),
+                     "r_p": float(res["r_p"][0]), "r_d": float(res["r_d"][0])})
+    print(json.dumps({"experiment": "fig5_stand_in", "curve": "(10 sin 2t, 8 sin(3t+0.5), 3 cos 5t), t in [0, 2pi]",
+                      "s": 3, "rho": 10.0, "tolerance": "N*0.05 (PAPER.md:L288)", "check_every": 8, "M": M, "rows": rows}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -165,6 +204,7 @@ def main():
     ap.add_argument("--oracle-seconds", type=float, default=12.0)
     ap.add_argument("--oracle-threads", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fig5", action="store_true", help="run the Fig. 5 stand-in (time and similarity vs N) instead")
     ap.add_argument("--no-extras", action="store_true", help="skip time-to-eps and the e2e leg")
     args = ap.parse_args()
 
@@ -173,6 +213,10 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if args.impl == "reference":
         run_reference(args, rank, world)
+        return
+    if args.fig5:
+        if rank == 0:
+            run_fig5(args, local_rank)
         return
 
     import torch

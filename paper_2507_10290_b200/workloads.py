@@ -163,4 +163,22 @@ def small_constrained(seed: int = 7, N: int = 37, s: int = 4, acc: bool = True, 
                     box_lo=LO, box_hi=HI, vmax=3.0, amax=5.0 if acc else 0.0)
 
 
+def fig5_curve(theta: np.ndarray) -> np.ndarray:
+    """The reference curve of the Fig. 5 stand-in: a closed-form 3-D Lissajous figure (metres), theta in [0, 2 pi].
+    The paper does not name its curve; any smooth parameterised curve has the workload's shape."""
+    theta = np.asarray(theta, dtype=np.float64)
+    return np.stack([10.0 * np.sin(2.0 * theta), 8.0 * np.sin(3.0 * theta + 0.5), 3.0 * np.cos(5.0 * theta)], axis=-1)
+
+
+def fig5(N: int = 1024, s: int = 3, rho: float = 10.0, speed: float = 2.0) -> Workload:
+    """PAPER.md:L355-361 (Fig. 5): N+1 points sampled uniformly in the parameter of a curve, the trajectory is forced
+    through them (HARD waypoints), no inequality constraints; durations = chord length / `speed`."""
+    theta = np.linspace(0.0, 2.0 * np.pi, N + 1)
+    pts = fig5_curve(theta)
+    chord = np.sqrt(((pts[1:] - pts[:-1]) ** 2).sum(axis=1))
+    T = np.maximum(chord / speed, 1e-3)
+    return Workload("fig5_N%d_s%d" % (N, s), 1, N, s, 3, "f64", pts[None], T[None], rho=rho,
+                    notes={"theta": theta})
+
+
 CONFIGS = {1: config1, 2: config2, 3: config3, 4: config4, 5: config5}
