@@ -416,3 +416,35 @@ def test_state_accessor_errors_and_iterate_zero():
         sol.set_rho(-2.0)
     z0 = sol.state("z")
     assert np.array_equal(z0[0, :, 0, :], w.waypoints[0])      # iterate 0: z positions are the waypoints (A9)
+
+
+def test_streaming_batch_fp32_and_solve():
+    """Streamed pieces may span trajectory ends (batch of chains longer than the forced capacity); fp32 state in the
+    ping-pong buffers; top_set_rho and top_solve (host loop) on a streamed solver."""
+    w = W.small_constrained(N=700, s=4, acc=False, batch=3, seed=31)
+    sol = top.from_workload(w, segs_per_cta=4, dtype="f64")
+    assert sol.launch_info()["waves"] >= 3
+    oracles = [make_oracle(w, b) for b in range(3)]
+    sol.iterate(70)
+    for o in oracles:
+        o.sweep(70, 0)
+    check_fields(field_errors(sol, oracles, w), "streamed batch, 70 sweeps")
+    sol.set_rho(4.0)
+    for o in oracles:
+        o.set_rho(4.0)
+    sol.iterate(70)
+    for o in oracles:
+        o.sweep(70, 0)
+    check_fields(field_errors(sol, oracles, w), "streamed batch after set_rho")
+    # fp32 (mixed) on the same streamed plan: positions against the fp64 oracle
+    s32 = top.from_workload(w, segs_per_cta=4, dtype="f32")
+    s32.set_rho(4.0)          # before any sweep: duals are zero, only the operator changes
+    ofresh = make_oracle(w, 1)
+    ofresh.set_rho(4.0)
+    s32.iterate(130); ofresh.sweep(130, 0)
+    T = w.durations[1]
+    assert np.abs(sampled_positions(s32.coeffs()[1], T) - sampled_positions(ofresh.get("coeffs"), T)).max() < 1e-3
+    # host-loop solve on a streamed solver: stops at a multiple of check_every, reports per-trajectory counts
+    s3 = top.from_workload(w, segs_per_cta=4, check_every=16, max_iter=64, rd_normalised=True)
+    ok, iters = s3.solve(1e-9)
+    assert not ok and np.all(iters == 64) and s3.iteration == 64
