@@ -233,6 +233,7 @@ struct Spectral {
     xreal lam[MAXN];
     xreal g0[MAXN * 3];       // G c_chord, [a][d]   (HARD mode; else 0)
     xreal gcol0[MAXN];        // G e_0 (only top_precompute_operator needs it: a frame other than the local one)
+    xreal gcol1[MAXN];        // G e_1: g0 = gcol1 * dp (kept so that segments of equal duration can share the rest)
     int q;
 };
 
@@ -342,7 +343,7 @@ bool build_spectral(int s, xreal T, bool box, bool vel, bool acc, int mode, cons
         }
     }
     if (hard) for (int a = 0; a < n; ++a) for (int d = 0; d < 3; ++d) S.g0[a * 3 + d] = Gm[a * n + 1] * dp[d];
-    for (int a = 0; a < n; ++a) S.gcol0[a] = Gm[a * n + 0];
+    for (int a = 0; a < n; ++a) { S.gcol0[a] = Gm[a * n + 0]; S.gcol1[a] = Gm[a * n + 1]; }
     return true;
 }
 
@@ -616,6 +617,9 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
 
     std::atomic<int> bad_operator(0);
     auto do_segments = [&](long long g0, long long g1) {
+        Spectral SP;
+        bool have_cached = false;
+        double cached_T = 0.0;
         for (long long gg = g0; gg < g1; ++gg) {
             const long long b = gg / N, i = gg % N;
             const size_t g = (size_t)gg;
@@ -632,10 +636,16 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
                 p0[d] = 0; p1[d] = (xreal)wp(b, i + 1, d) - (xreal)wp(b, i, d);
                 origin[(size_t)d * NP + g] = org3[d];
             }
-            Spectral SP;
-            if (!build_spectral(s, T, has_box, has_vel, has_acc, (int)mode, p1, SP)) {
-                bad_operator.store(1);
-                return;
+            // W, lambda and G depend on the duration only: segments of equal duration (config 3: all of them) share
+            // one factorisation; only g0 = (G e_1) dp is per segment
+            if (!(have_cached && Td == cached_T)) {
+                if (!build_spectral(s, T, has_box, has_vel, has_acc, (int)mode, p1, SP)) {
+                    bad_operator.store(1);
+                    return;
+                }
+                have_cached = true; cached_T = Td;
+            } else if (mode == TOP_WAYPOINT_HARD) {
+                for (int a = 0; a < n; ++a) for (int d = 0; d < 3; ++d) SP.g0[a * 3 + d] = SP.gcol1[a] * p1[d];
             }
             for (int ii = 0; ii < MAXN; ++ii) lamv[(size_t)ii * NP + g] = ii < SP.q ? (double)SP.lam[ii] : 0.0;
             for (int d = 0; d < 3; ++d) dpv[(size_t)d * NP + g] = (mode == TOP_WAYPOINT_HARD && d < dims) ? (double)p1[d] : 0.0;
