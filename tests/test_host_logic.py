@@ -53,6 +53,10 @@ def test_validation_happens_before_the_device_is_needed():
         dict(waypoints=wp, durations=T, s=3, rho=1.0, samples=4, vmax=1.0),  # samples
         dict(waypoints=wp, durations=T, s=3, rho=1.0, samples=8, box_lo=np.ones((2, 3)), box_hi=np.zeros((2, 3))),
         dict(waypoints=wp, durations=T, s=3, rho=1.0, segs_per_cta=6),
+        dict(waypoints=wp, durations=T, s=3, rho=1.0, lanes=3),
+        dict(waypoints=np.zeros((1, 3)), durations=np.zeros(0), s=3, rho=1.0),          # empty trajectory: N = 0
+        dict(waypoints=np.zeros((0, 3, 3)), durations=np.zeros((0, 2)), s=3, rho=1.0),  # empty batch
+        dict(waypoints=wp, durations=T, s=3, rho=1.0, adaptive_rho=True, adapt_mu=0.5),
     ]
     for kw in cases:
         with pytest.raises(top.TopError) as e:
