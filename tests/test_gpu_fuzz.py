@@ -1,0 +1,45 @@
+"""`-m gpu`: seeded random sweep over the options of the CUDA path (sizes 1..300 incl. ragged CTAs, s, constraint subsets,
+dims, batch, rho, waypoint mode, lanes per segment, inter-CTA sync mode, segments per CTA, launch chunking) against the
+oracle run in long double; every state field of every compared iterate within 1e-9 norm-relative."""
+import numpy as np
+import pytest
+
+from paper_2507_10290_b200 import build as top_build
+from paper_2507_10290_b200 import top
+from paper_2507_10290_b200 import workloads as W
+from tests.parity_util import field_errors, make_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.mark.parametrize("seed", [2, 3])
+def test_random_option_sweep(seed):
+    top_build.build()
+    rng = np.random.default_rng(seed)
+    for case in range(40):
+        N = int(rng.choice([1, 2, 3, 5, 8, 17, 33, 64, 129, 300]))
+        s = int(rng.choice([3, 4])); acc = bool(rng.integers(2))
+        batch = int(rng.choice([1, 1, 2, 4])); dims = int(rng.choice([3, 3, 2, 1]))
+        w = W.small_constrained(N=N, s=s, acc=acc, batch=batch, dims=dims, seed=int(rng.integers(1 << 30)))
+        cons = int(rng.integers(4))
+        if cons == 0:
+            w.samples, w.box_lo, w.box_hi, w.vmax, w.amax = 0, None, None, 0.0, 0.0
+        elif cons == 1:
+            w.box_lo, w.box_hi = None, None
+        elif cons == 2:
+            w.vmax = 0.0
+        w.rho = float(rng.choice([0.3, 1.0, 10.0, 80.0]))
+        mode = str(rng.choice(["hard", "hard", "pinned_z", "free"]))
+        lanes = int(rng.choice([8, 4])); sync = str(rng.choice(["pairwise", "neighbour", "grid"]))
+        segs = int(rng.choice([0, 4, 8, 16]))
+        ks = [int(k) for k in rng.integers(1, 40, size=3)]
+        sol = top.from_workload(w, mode=mode, lanes=lanes, sync=sync, segs_per_cta=segs, dtype="f64")
+        oracles = [make_oracle(w, b, mode=mode, long_double=True) for b in range(batch)]
+        for k in ks:
+            sol.iterate(k)
+            for o in oracles:
+                o.sweep(k, 1)
+            for name, v in field_errors(sol, oracles, w).items():
+                tol = 1e-6 if name.startswith("res_") else 1e-9
+                assert v < tol, (case, name, v, N, s, acc, batch, dims, cons, w.rho, mode, lanes, sync, segs, ks)
+        sol.close()
