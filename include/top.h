@@ -179,6 +179,15 @@ TOP_API top_status top_get_coeffs(top_solver* h, void* out, int32_t out_is_devic
  * count = number of doubles `out` holds; TOP_E_INVALID if it does not match or the field is unknown. */
 TOP_API top_status top_get_state(top_solver* h, const char* field, double* out, size_t count);
 
+/* Checkpoint / resume (warm start).  top_snapshot_save copies the complete iterate (z~, u, slack / ball variables and
+ * their duals, coefficients, residuals, sweep count, rho) into a caller-owned HOST buffer of top_snapshot_bytes(h)
+ * bytes; top_snapshot_restore puts it back into a solver that was created with the same sizes, dtype and constraint
+ * selection (checked: TOP_E_INVALID otherwise).  Sweeping on from a restored snapshot reproduces the uninterrupted
+ * run bit for bit.  Both synchronise the stream.  The buffer layout is private to this library version. */
+TOP_API size_t top_snapshot_bytes(const top_solver* h);
+TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, size_t bytes);
+TOP_API top_status top_snapshot_restore(top_solver* h, const void* host_buf, size_t bytes);
+
 /* Sweeps done since top_create. */
 TOP_API int64_t top_iteration(const top_solver* h);
 

@@ -1025,6 +1025,73 @@ extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, do
     return fail(h, TOP_E_INVALID, "top_get_state: unknown field '" + f + "'");
 }
 
+namespace {
+struct SnapshotHeader {
+    uint64_t magic;
+    int64_t nseg, stride, iter;
+    int32_t s, dims, dtype, batch;
+    uint32_t kflags, have_residuals;
+    double rho;
+};
+constexpr uint64_t SNAP_MAGIC = 0x544f50534e415031ull;     // "TOPSNAP1"
+// the device arrays that make up an iterate, in snapshot order (null ones are skipped)
+int snapshot_fields(top_solver* h, void** out) {
+    void* all[] = {h->d_zt, h->d_u, h->d_qp, h->d_qn, h->d_phv, h->d_wv, h->d_pha, h->d_wa, h->d_chat};
+    int n = 0;
+    for (void* p : all) if (p) out[n++] = p;
+    return n;
+}
+}  // namespace
+
+extern "C" TOP_API size_t top_snapshot_bytes(const top_solver* hc) {
+    if (!hc) return 0;
+    top_solver* h = const_cast<top_solver*>(hc);
+    void* f[9];
+    const int n = snapshot_fields(h, f);
+    return sizeof(SnapshotHeader) + (size_t)n * 3 * (size_t)h->stride * real_bytes(h) + (size_t)h->batch * 4 * 8;
+}
+
+extern "C" TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, size_t bytes) {
+    if (!h) return TOP_E_INVALID;
+    if (!host_buf || bytes != top_snapshot_bytes(h)) return fail(h, TOP_E_INVALID, "top_snapshot_save: buffer size must be top_snapshot_bytes()");
+    if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
+    SnapshotHeader hd;
+    std::memset(&hd, 0, sizeof hd);
+    hd.magic = SNAP_MAGIC; hd.nseg = h->nseg; hd.stride = h->stride; hd.iter = h->iter; hd.s = h->s; hd.dims = h->dims;
+    hd.dtype = h->dtype; hd.batch = h->batch; hd.kflags = h->kflags; hd.have_residuals = h->have_residuals ? 1u : 0u; hd.rho = h->rho;
+    unsigned char* o = static_cast<unsigned char*>(host_buf);
+    std::memcpy(o, &hd, sizeof hd); o += sizeof hd;
+    void* f[9];
+    const int n = snapshot_fields(h, f);
+    const size_t fb = 3 * (size_t)h->stride * real_bytes(h);
+    for (int i = 0; i < n; ++i) { CU(cudaMemcpyAsync(o, f[i], fb, cudaMemcpyDeviceToHost, h->stream), "D2H snapshot"); o += fb; }
+    CU(cudaMemcpyAsync(o, h->d_res, (size_t)h->batch * 4 * 8, cudaMemcpyDeviceToHost, h->stream), "D2H snapshot");
+    return check_abort(h);
+}
+
+extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* host_buf, size_t bytes) {
+    if (!h) return TOP_E_INVALID;
+    if (!host_buf || bytes != top_snapshot_bytes(h)) return fail(h, TOP_E_INVALID, "top_snapshot_restore: buffer size does not match this solver");
+    SnapshotHeader hd;
+    std::memcpy(&hd, host_buf, sizeof hd);
+    if (hd.magic != SNAP_MAGIC || hd.nseg != h->nseg || hd.stride != h->stride || hd.s != h->s || hd.dims != h->dims ||
+        hd.dtype != h->dtype || hd.batch != h->batch || hd.kflags != h->kflags || !(hd.rho > 0))
+        return fail(h, TOP_E_INVALID, "top_snapshot_restore: the snapshot belongs to a different problem");
+    if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
+    const unsigned char* o = static_cast<const unsigned char*>(host_buf) + sizeof hd;
+    void* f[9];
+    const int n = snapshot_fields(h, f);
+    const size_t fb = 3 * (size_t)h->stride * real_bytes(h);
+    for (int i = 0; i < n; ++i) { CU(cudaMemcpyAsync(f[i], o, fb, cudaMemcpyHostToDevice, h->stream), "H2D snapshot"); o += fb; }
+    CU(cudaMemcpyAsync(h->d_res, o, (size_t)h->batch * 4 * 8, cudaMemcpyHostToDevice, h->stream), "H2D snapshot");
+    if (hd.rho != h->rho) { CU(refresh_operator(h, hd.rho), "operator refresh launch"); h->rho = hd.rho; }
+    CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+    h->iter = hd.iter;
+    h->have_residuals = hd.have_residuals != 0;
+    if (!h->have_residuals) for (int i = 0; i < h->batch * 4; ++i) h->h_res[i] = std::numeric_limits<double>::quiet_NaN();
+    return TOP_OK;
+}
+
 extern "C" TOP_API int64_t top_iteration(const top_solver* h) { return h ? h->iter : -1; }
 
 extern "C" TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas, int32_t* threads, int32_t* segs_per_cta,

@@ -24,7 +24,7 @@ TOP_RHO_ADAPTIVE = 64
 SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
 EXPORTS = ["top_create", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
-           "top_iteration", "top_set_rho", "top_get_rho", "top_launch_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
+           "top_snapshot_bytes", "top_snapshot_save", "top_snapshot_restore", "top_iteration", "top_set_rho", "top_get_rho", "top_launch_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
            "top_destroy", "top_last_error"]
 
 
@@ -79,6 +79,12 @@ def lib():
     L.top_set_rho.argtypes = [vp, ctypes.c_double]
     L.top_get_rho.restype = ctypes.c_double
     L.top_get_rho.argtypes = [vp]
+    L.top_snapshot_bytes.restype = ctypes.c_size_t
+    L.top_snapshot_bytes.argtypes = [vp]
+    L.top_snapshot_save.restype = ctypes.c_int
+    L.top_snapshot_save.argtypes = [vp, vp, ctypes.c_size_t]
+    L.top_snapshot_restore.restype = ctypes.c_int
+    L.top_snapshot_restore.argtypes = [vp, vp, ctypes.c_size_t]
     L.top_iteration.restype = ctypes.c_int64
     L.top_iteration.argtypes = [vp]
     L.top_launch_info.restype = ctypes.c_int
@@ -215,6 +221,16 @@ class TopSolver:
     @property
     def rho(self) -> float:
         return float(self._L.top_get_rho(self._h))
+
+    def snapshot(self) -> np.ndarray:
+        """Complete iterate as an opaque byte array (top_snapshot_save)."""
+        buf = np.zeros(int(self._L.top_snapshot_bytes(self._h)), dtype=np.uint8)
+        self._check(self._L.top_snapshot_save(self._h, buf.ctypes.data_as(ctypes.c_void_p), buf.size))
+        return buf
+
+    def restore(self, snap: np.ndarray):
+        snap = np.ascontiguousarray(snap, dtype=np.uint8)
+        self._check(self._L.top_snapshot_restore(self._h, snap.ctypes.data_as(ctypes.c_void_p), snap.size))
 
     def residuals(self):
         r = [np.zeros(self.batch) for _ in range(4)]

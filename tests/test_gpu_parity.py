@@ -448,3 +448,26 @@ def test_streaming_batch_fp32_and_solve():
     s3 = top.from_workload(w, segs_per_cta=4, check_every=16, max_iter=64, rd_normalised=True)
     ok, iters = s3.solve(1e-9)
     assert not ok and np.all(iters == 64) and s3.iteration == 64
+
+
+def test_snapshot_restore_resumes_bit_for_bit():
+    """Checkpoint / resume: save at sweep 40 (after a rho change), restore into a fresh solver, sweep on: identical to
+    the uninterrupted run; a snapshot of another problem is refused."""
+    w = W.small_constrained(N=150, s=4, acc=True, batch=2, seed=41)
+    a = top.from_workload(w, segs_per_cta=8)
+    a.iterate(25); a.set_rho(3.0); a.iterate(15)
+    snap = a.snapshot()
+    a.iterate(33)
+    b = top.from_workload(w, segs_per_cta=8)
+    b.restore(snap)
+    assert b.iteration == 40 and b.rho == 3.0
+    assert np.all(np.isfinite(b.residuals()["r_p"]))            # the residuals of sweep 40 travel with the snapshot
+    b.iterate(33)
+    for f in ("z", "u", "s_pos", "v_neg", "phi_v", "w_a"):
+        assert np.array_equal(a.state(f), b.state(f)), f
+    assert np.array_equal(a.coeffs(), b.coeffs())
+    assert np.array_equal(a.residuals()["r_d"], b.residuals()["r_d"]) and b.iteration == a.iteration == 73
+    other = top.from_workload(W.small_constrained(N=150, s=3, acc=True, batch=2, seed=41), segs_per_cta=8)
+    with pytest.raises(top.TopError) as e:
+        other.restore(snap)
+    assert e.value.status == top.TOP_E_INVALID
