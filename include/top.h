@@ -81,6 +81,10 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
  * check_every sweeps; the paper: every sweep) rho <- tau_incr*rho if r_p > mu*r_d, rho <- rho/tau_decr if
  * r_d > mu*r_p.  The change goes through top_set_rho. */
 #define TOP_RHO_ADAPTIVE      64u
+/* Kernel selection (a tuning knob; results agree to rounding): with 4 lanes per segment the fp64 sweep runs its two
+ * constant-matrix contractions (Eq. 20a second bracket; evaluation of Eq. 20b, 20d-g) on the tensor cores
+ * (mma.sync m8n8k4 f64).  This flag keeps the shuffle / synthetic-division form of the 4-lane kernel instead. */
+#define TOP_KERNEL_NO_MMA     128u
 
 /* The paper's convex sets, specialised as BASELINE.json's configs use them:
  * an axis-aligned box corridor per segment (K=6 half-spaces, linear set, Eq. 7-10) and Euclidean balls on

@@ -38,6 +38,7 @@ struct top_solver {
     cudaStream_t stream = nullptr;
     long long nseg = 0, nseg_pad = 0, stride = 0;
     int num_sms = 0, max_ctas = 0, user_segs = 0, lanes = 8;
+    bool mma = false;                  // fp64, 4 lanes per segment: the tensor-core (DMMA) kernel of top_kernels_mma.cu
     struct Wave { long long seg_begin, seg_end, own_begin, own_end; uint32_t kflags; int segs_per_cta, ctas, threads; size_t smem; };
     // streaming (temporal blocking) for chains longer than the on-chip capacity: pieces with `halo` extra segments on
     // each open side run `halo` sweeps per launch (the dependency radius of a sweep is one segment), reading iterate
@@ -412,11 +413,17 @@ top_status download_real(top_solver* h, const void* src, std::vector<double>& ds
 
 int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
+// the sweep kernel family of a solver: 8 lanes, 4 lanes (shuffle form), or 4 lanes with fp64 tensor-core contractions
+size_t kernel_smem(int dtype, int s, bool constrained, int lanes, bool mma, int segs) {
+    return mma ? sweep_smem_bytes_mma(constrained, segs) : sweep_smem_bytes(dtype, s, constrained, lanes, segs);
+}
+int kernel_max_threads(int dtype, int lanes, bool mma) { return mma ? max_threads_mma() : max_threads_for(dtype, lanes); }
+
 // largest segments-per-CTA (multiple of 4) whose threads and shared memory fit one CTA
-int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, size_t smem_limit) {
+int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, bool mma, size_t smem_limit) {
     int best = 0;
-    for (int segs = 4; (segs * lanes + 31) / 32 * 32 <= max_threads_for(dtype, lanes); segs += 4)
-        if (sweep_smem_bytes(dtype, s, constrained, lanes, segs) <= smem_limit) best = segs;
+    for (int segs = 4; (segs * lanes + 31) / 32 * 32 <= kernel_max_threads(dtype, lanes, mma); segs += 4)
+        if (kernel_smem(dtype, s, constrained, lanes, mma, segs) <= smem_limit) best = segs;
     return best;
 }
 
@@ -555,7 +562,8 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     // lose for fp64 (register spills) and for short chains (longer serial path per warp)
     h->lanes = o.lanes_per_segment ? o.lanes_per_segment : 8;
     if (!o.lanes_per_segment && dtype == TOP_F32 && nseg >= (long long)h->num_sms * 96) h->lanes = 4;
-    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, (size_t)smem_optin - 8192);
+    h->mma = dtype == TOP_F64 && h->lanes == 4 && !(o.flags & TOP_KERNEL_NO_MMA);
+    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192);
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
     h->max_ctas = h->num_sms;
     const long long capacity = (long long)h->max_ctas * std::min(segs_max, h->user_segs ? h->user_segs : segs_max);
@@ -568,7 +576,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
         w.segs_per_cta = segs;
         w.ctas = (int)((cnt + segs - 1) / segs);
         w.threads = (segs * h->lanes + 31) / 32 * 32;
-        w.smem = sweep_smem_bytes(h->dtype, s, h->constrained, h->lanes, segs);
+        w.smem = kernel_smem(h->dtype, s, h->constrained, h->lanes, h->mma, segs);
         if (w.ctas > h->max_ctas) return false;
         h->waves.push_back(w);
         return true;
@@ -599,7 +607,8 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     }
     for (const auto& w : h->waves) {
         int per_sm = 0;
-        cudaError_t e = sweep_kernel_limits(h->dtype, s, h->constrained, h->lanes, w.threads, w.smem, &per_sm);
+        cudaError_t e = h->mma ? sweep_kernel_limits_mma(s, h->constrained, w.threads, w.smem, &per_sm)
+                               : sweep_kernel_limits(h->dtype, s, h->constrained, h->lanes, w.threads, w.smem, &per_sm);
         if (e != cudaSuccess) CREATE_FAIL(cuda_fail(h, e, "occupancy query"));
         if (per_sm < 1) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "sweep kernel does not fit an SM"));
     }
@@ -823,7 +832,8 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
             h->seq_counter += (unsigned long long)kk;
             if (w.ctas > 1 && !(p.flags & KF_NEIGHBOUR_SYNC))
                 CU(cudaMemsetAsync(h->d_sync, 0, 8, h->stream), "cudaMemsetAsync");
-            CU(launch_sweeps(p, h->dtype, h->s, h->constrained, h->lanes, w.ctas, w.threads, w.smem, h->stream), "sweep kernel launch");
+            CU(h->mma ? launch_sweeps_mma(p, h->s, h->constrained, w.ctas, w.threads, w.smem, h->stream)
+                      : launch_sweeps(p, h->dtype, h->s, h->constrained, h->lanes, w.ctas, w.threads, w.smem, h->stream), "sweep kernel launch");
             h->launches += 1;
         }
         if (h->streaming) {       // every piece has written iterate k + kk of its own segments: swap the buffer sets
@@ -875,7 +885,7 @@ extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iter
     const int rd_idx = (h->opt_flags & TOP_RD_NORMALISED) ? 2 : 1;
     // (large CTAs run the plain kernel faster than the solve instantiation -- 96-register cap -- so with a sparse
     // test cadence they keep the host loop below)
-    if (h->batch == 1 && h->waves.size() == 1 && !h->streaming && h->lanes == 8 && h->waves[0].ctas <= 160 &&
+    if (h->batch == 1 && h->waves.size() == 1 && !h->streaming && (h->lanes == 8 || h->mma) && h->waves[0].ctas <= 160 &&
         (h->waves[0].threads <= 256 || h->check_every < 16)) {
         // one resident trajectory: the stop rule (and Eq. 24) runs inside the kernel, one launch for the whole solve
         InKernelSolve iks;
@@ -1116,8 +1126,8 @@ extern "C" TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dty
         cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) { cudaGetLastError(); return -1; }
     const uint32_t kf = constrained ? (KF_BOX | KF_VEL | KF_ACC) : 0;
     (void)kf;
-    return (int64_t)sms * std::max(max_segs_per_cta((int)dtype, s, constrained != 0, 8, (size_t)smem - 1024),
-                                   max_segs_per_cta((int)dtype, s, constrained != 0, 4, (size_t)smem - 1024));
+    return (int64_t)sms * std::max(max_segs_per_cta((int)dtype, s, constrained != 0, 8, false, (size_t)smem - 1024),
+                                   max_segs_per_cta((int)dtype, s, constrained != 0, 4, false, (size_t)smem - 1024));
 }
 
 extern "C" TOP_API double top_fma_peak(int32_t device, top_dtype dtype, int32_t reps, void* cuda_stream) {

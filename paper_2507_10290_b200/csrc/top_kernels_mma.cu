@@ -1,0 +1,591 @@
+// top_kernels_mma.cu -- the fp64 CADMM sweep with its constant-matrix contractions on the tensor cores.
+//
+// Same sweep, same global-memory layout, same exchange protocol as cadmm_sweeps_kernel4 (top_kernels.cu): FOUR lanes
+// per segment, lane t owns inequality samples {t, t+4} and coefficient / consensus rows {t, t+4}; 8 segments per
+// warp.  What differs is how the two contractions with CONSTANT matrices are done.  In the normalised-time basis
+// (c^_a = c_a T^a) the evaluation matrices of Eq. 19 are the same for every segment:
+//     a1  R^ = [M^' E0' E1' E2'] G        (Eq. 20a second bracket)   8 x 32 constant, G 32 x 3 per segment
+//     a3  [B; P; V; A] = [M^; E0; E1; E2] c^   (Eq. 20b, 20d-g)   32 x 8 constant, c^ 8 x 3 per segment
+// Both are issued as mma.sync.aligned.m8n8k4.f64 (DMMA) with the (segment, dim) pairs of the warp as the M dimension
+// (8 segments x 3 dims = three m-tiles) and the constant matrix as the B operand, held in registers for the whole
+// launch.  The fragment layout of m8n8k4 puts row g of the A operand in lanes 4g..4g+3 and column k in lane 4g + (k%4):
+// exactly "lane t of segment g supplies its own items t, t+4", so operands are taken from the lane's own registers and
+// results land in the lane that owns them: no shuffle reduce-scatter, no select instructions, no second all-gather.
+// The only intra-segment exchange left is the all-gather of R^ (8 rows x 3 dims through shared memory) in front of the
+// per-segment 8 x 8 operator apply a2 (Eq. 20a first bracket), which stays on DFMA: its matrix differs per segment.
+// Measured on B200: DMMA m8n8k4 runs at the DFMA FLOP rate (16 cycles per instruction and scheduler) but
+// with 26-cycle dependent latency and independent accumulators a single warp keeps the fp64 pipe busy, where the
+// shuffle / synthetic-division form was bound by instruction issue and dependent-chain latency.
+#include "top_device.cuh"
+
+namespace top {
+
+namespace {
+
+// D (8x8, lane (g,t): row g, cols 2t, 2t+1) += A (8x4, lane (g,t): row g, col t) * B (4x8, lane (g,t): row t, col g)
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// one instantiation: <= 288 threads (9 warps of 8 segments: 224 registers per thread)
+constexpr int MAXT_MMA = 288;
+
+struct SmemLayoutMma {
+    size_t pm, c0, ctab, lohi, xs, bs, zoff, total;
+};
+__host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc) {
+    SmemLayoutMma L;
+    const int T = segs_alloc * 4;
+    size_t off = 0;
+    L.pm = off;   off = align16(off + (size_t)2 * 4 * T * sizeof(double2));            // rho*Pm^ rows, [h][b/2][thread] pairs
+    L.c0 = off;   off = align16(off + (size_t)6 * T * sizeof(double));                 // c0^ rows, [h][d][thread]
+    L.ctab = off; off = align16(off + (size_t)16 * 32 * sizeof(double));               // constant MMA operands, [16][lane of warp]
+    L.lohi = off; off = align16(off + (size_t)(cons ? 6 : 0) * segs_alloc * sizeof(double));
+    L.xs = off;   off = align16(off + (size_t)segs_alloc * XSTRIDE * sizeof(double));  // rhs rows, all-gather
+    L.bs = off;   off = align16(off + (size_t)2 * (segs_alloc + 2) * 24 * sizeof(double));   // boundary rows, double buffered
+    L.zoff = off; off = align16(off + (size_t)6 * segs_alloc * sizeof(double));        // frame shift of the neighbours' position rows
+    L.total = off;
+    return L;
+}
+
+template <int S, bool CONS, int MAXT, bool SOLVE>
+__global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams p) {
+    constexpr int N2 = 2 * S;
+    constexpr int LPS = 4;                         // lanes per segment
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+
+    const int T = blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
+    const int grp = (tid >> 2) & 7;                // segment within the warp = row / column group of the MMA fragments
+    const int SA = T >> 2;                         // segment slots of this CTA (>= segs_per_cta; T is a multiple of 32)
+    const int SEGS = p.segs_per_cta;
+    const int cta = blockIdx.x, nctas = gridDim.x;
+    const uint32_t flags = p.flags;
+    const bool has_box = CONS && (flags & KF_BOX), has_vel = CONS && (flags & KF_VEL), has_acc = CONS && (flags & KF_ACC);
+    const bool pin_pos = flags & KF_PIN_POS;
+    const bool nb_sync = flags & KF_NEIGHBOUR_SYNC;
+
+    const SmemLayoutMma L = smem_layout_mma(CONS, SA);
+    double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + tid;          // [(h*4 + b/2) * T]
+    double* c0s = reinterpret_cast<double*>(smem_raw + L.c0) + tid;            // [(h*3 + d) * T]
+    double* ctab = reinterpret_cast<double*>(smem_raw + L.ctab) + (tid & 31);  // [k * 32]: a1 k-step operands at k = 0..7, a3 operands at k = 8 + kstep*4 + block
+    double* lohi = reinterpret_cast<double*>(smem_raw + L.lohi);               // [6][SA]
+    double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE;
+    double* Bs = reinterpret_cast<double*>(smem_raw + L.bs);                   // [2 parity][SA+2][8 rows][3]
+    double* zoffs = reinterpret_cast<double*>(smem_raw + L.zoff);              // [2 sides][3][SA]
+
+    const long long cta_first = p.seg_begin + (long long)cta * SEGS;
+    const long long remaining = p.seg_end - cta_first;
+    const int nact = remaining < SEGS ? (int)remaining : SEGS;
+    const bool active = sl < nact;
+    // inactive slots of a ragged CTA compute on a copy of the CTA's first segment (the MMAs need full warps) and never
+    // write to global memory
+    const long long gseg = active ? cta_first + sl : cta_first;
+    const bool owned = active && gseg >= p.own_begin && gseg < p.own_end;
+    const long long stride = p.stride;
+
+    // the two items of this lane: sample / row index jj[h], global lane slot gt[h]
+    int jj[2]; long long gt[2]; bool isrow[2], right[2]; int korder[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        jj[h] = lane + 4 * h;
+        gt[h] = gseg * LANES + jj[h];
+        isrow[h] = jj[h] < N2;
+        right[h] = jj[h] >= S;
+        korder[h] = right[h] ? jj[h] - S : jj[h];
+    }
+
+    // ---- constant operands of the two contractions (B fragments: row k = 4*kstep + lane, column n = grp)
+    // a1: k runs over the 32 items [consensus rows | E0 samples | E1 samples | E2 samples], n = coefficient row
+    // a3: k = coefficient row, n runs over the items of one block, permuted so that the accumulator columns
+    //     2*lane, 2*lane+1 are the lane's own items lane, lane+4
+    if (tid < 32) {
+        const int a = grp;
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk) {
+            const int b = kk >> 1, item = lane + 4 * (kk & 1);
+            const double tau = (double)(item + 1) / (double)(MS + 1);       // sample time (reading A10)
+            double v = 0.0;
+            if (a < N2) {
+                if (b == 0) { if (item < N2) v = beta_entry(item % S, a, item < S ? 0.0 : 1.0); }
+                else v = beta_entry(b - 1, a, tau);
+            }
+            ctab[kk * 32] = v;
+        }
+        const int item = (grp >> 1) + 4 * (grp & 1);
+        const double tau = (double)(item + 1) / (double)(MS + 1);
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk) {
+            const int ar = 4 * kk + lane;
+#pragma unroll
+            for (int nt = 0; nt < 4; ++nt) {
+                double v = 0.0;
+                if (ar < N2) {
+                    if (nt == 0) { if (item < N2) v = beta_entry(item % S, ar, item < S ? 0.0 : 1.0); }
+                    else v = beta_entry(nt - 1, ar, tau);
+                }
+                ctab[(8 + kk * 4 + nt) * 32] = v;
+            }
+        }
+    }
+    double invTk[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+#pragma unroll
+        for (int b = 0; b < 8; b += 2)
+            Pms[(h * 4 + (b >> 1)) * T] = make_double2(b < N2 ? p.Pm[b * stride + gt[h]] : 0.0, b + 1 < N2 ? p.Pm[(b + 1) * stride + gt[h]] : 0.0);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) c0s[(h * 3 + d) * T] = p.c0[d * stride + gt[h]];
+        invTk[h] = static_cast<const double*>(p.invTk)[gt[h]];
+    }
+    const double invT = static_cast<const double*>(p.invT)[gseg], invT2 = static_cast<const double*>(p.invT)[p.nseg_pad + gseg];
+    if (CONS) {
+        lohi[lane * SA + sl] = static_cast<const double*>(p.lohi)[lane * p.nseg_pad + gseg];
+        if (lane < 2) lohi[(lane + 4) * SA + sl] = static_cast<const double*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
+    }
+    if (lane < 3) {        // frame shifts of the neighbours' position rows: left junction (row 0), right junction (row S)
+        zoffs[lane * SA + sl] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + 0];
+        zoffs[(3 + lane) * SA + sl] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + S];
+    }
+    const uint8_t sf = p.segflags[gseg];
+    const bool open_l = (flags & KF_OPEN_LEFT) && gseg == p.seg_begin, open_r = (flags & KF_OPEN_RIGHT) && gseg == p.seg_end - 1;
+    // ---- state of iterate k
+    double zt[2][3], u[2][3], qp[2][3], qn[2][3], phv[2][3], wv[2][3], pha[2][3], wa[2][3];
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const long long i = d * stride + gt[h];
+            zt[h][d] = static_cast<const double*>(p.zt)[i];
+            u[h][d] = static_cast<const double*>(p.u)[i];
+            qp[h][d] = has_box ? static_cast<const double*>(p.qp)[i] : 0.0;
+            qn[h][d] = has_box ? static_cast<const double*>(p.qn)[i] : 0.0;
+            phv[h][d] = has_vel ? static_cast<const double*>(p.phv)[i] : 0.0;
+            wv[h][d] = has_vel ? static_cast<const double*>(p.wv)[i] : 0.0;
+            pha[h][d] = has_acc ? static_cast<const double*>(p.pha)[i] : 0.0;
+            wa[h][d] = has_acc ? static_cast<const double*>(p.wa)[i] : 0.0;
+        }
+
+    const double vmax = p.vmax, amax = p.amax;
+    unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
+    const size_t mbox_par_stride = (size_t)p.max_ctas * 24 * 16;
+    __shared__ int abort_sh[2];
+    __shared__ int abort_any;
+    if (tid < 2) abort_sh[tid] = 0;
+    if (tid == 0) abort_any = 0;
+    const int warp = tid >> 5, nwarps = T >> 5;
+    const bool pairwise = nb_sync && nctas > 1 && nwarps <= 17 && (flags & KF_PAIRWISE);
+    // in-kernel solve: stop rule and Eq. 24 evaluated on the device (all CTAs all-gather their residual partial
+    // sums through LL slots and take the same decision from the same numbers)
+    const int ce = SOLVE ? p.check_every : 0;
+    double rho_cur = p.rho;
+    __shared__ double wsum_sh[SOLVE ? 32 : 1][4];
+    __shared__ double allp_sh[SOLVE ? 160 : 1][4];
+    __shared__ double tot_sh[4];
+    int ncheck = 0, sweeps_done = p.k_sweeps, stopped = 0;
+    __syncthreads();
+    for (int it = 0; it < p.k_sweeps; ++it) {
+        const unsigned seq = p.seq_base + (unsigned)it + 1u;
+        const int par = (int)(seq & 1u);
+        const bool final_sweep = (it == p.k_sweeps - 1);
+        // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
+        const bool last_sweep = final_sweep || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
+        double* const Bcur = Bs + (size_t)par * (SA + 2) * 24;
+
+        // ================= phase A: segment local =================
+        // a1: right-hand side of Eq. 20a (second bracket; rho is folded into the operator, A3):
+        // R^ = M^'[(z~ - u)/T^k] + E0'[(hi - s+ - v+) + (lo + s- + v-)] + E1'[(phi_v - w_v)/T] + E2'[(phi_a - w_a)/T^2].
+        // Three accumulator tiles (one per dim), up to 8 k-steps each; the accumulator of lane t holds rows 2t, 2t+1.
+        {
+            double acc[3][2] = {{0, 0}, {0, 0}, {0, 0}};
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], (zt[h][d] - u[h][d]) * invTk[h], ctab[(h) * 32]);
+            if (CONS) {
+                if (has_box) {      // Ao'(b - s - v), Ao = [E0; -E0], b = [hi; -lo];  s + v = |q| (Moreau pair)
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) {
+                        const double lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
+#pragma unroll
+                        for (int h = 0; h < 2; ++h)
+                            dmma884(acc[d][0], acc[d][1], (hi - fabs(qp[h][d])) + (lo + fabs(qn[h][d])), ctab[(2 + h) * 32]);
+                    }
+                }
+                if (has_vel) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], (phv[h][d] - wv[h][d]) * invT, ctab[(4 + h) * 32]);
+                }
+                if (has_acc) {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h)
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], (pha[h][d] - wa[h][d]) * invT2, ctab[(6 + h) * 32]);
+                }
+            }
+#pragma unroll
+            for (int d = 0; d < 3; ++d) *reinterpret_cast<double2*>(Xs + d * 8 + 2 * lane) = make_double2(acc[d][0], acc[d][1]);
+        }
+        __syncwarp();
+        // a2: x-update  c^ = (rho Pm^) R^ + c0^   (Eq. 20a first bracket, precomputed per segment): rows lane, lane+4
+        double c[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            double pm[8];
+#pragma unroll
+            for (int b = 0; b < N2; b += 2) {
+                const double2 t2 = Pms[(h * 4 + (b >> 1)) * T];
+                pm[b] = t2.x; pm[b + 1] = t2.y;
+            }
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                double v = c0s[(h * 3 + d) * T];
+#pragma unroll
+                for (int b = 0; b < N2; b += 2) {
+                    const double2 t2 = *reinterpret_cast<const double2*>(Xs + d * 8 + b);
+                    v += pm[b] * t2.x;
+                    v += pm[b + 1] * t2.y;
+                }
+                c[h][d] = v;
+            }
+        }
+        if (last_sweep && owned) {      // (every test sweep as well: the solve may stop there)
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int d = 0; d < 3; ++d) static_cast<double*>(p.chat)[d * stride + gt[h]] = c[h][d];
+        }
+        // a3: evaluate the new polynomial: consensus rows of B = M c (Eq. 20b), and the lane's two samples of E0 c, E1 c,
+        // E2 c (Eq. 20d-g).  A operand = the lane's own coefficient rows; accumulator columns = the lane's own items.
+        double Bnd[2][3], Pv[2][3], Vv[2][3], Av[2][3];
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            double e0 = 0, e1 = 0;
+            dmma884(e0, e1, c[0][d], ctab[(8 + (0) * 4 + 0) * 32]);
+            dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 0) * 32]);
+            Bnd[0][d] = e0 * invTk[0]; Bnd[1][d] = e1 * invTk[1];
+        }
+        // publish: shared memory for the neighbours in this CTA, mailbox for the neighbouring CTAs
+        bool need[2];
+        const unsigned char* rslot[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            if (isrow[h]) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) Bcur[(sl + 1) * 24 + jj[h] * 3 + d] = Bnd[h][d];
+                if (nctas > 1 && active) {
+                    unsigned char* e = mbox + par * mbox_par_stride + (size_t)cta * 24 * 16;
+                    if (sl == 0 && !right[h] && cta > 0) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) ll_store(e + (0 * 12 + korder[h] * 3 + d) * 16, Bnd[h][d], seq);
+                    }
+                    if (sl == nact - 1 && right[h] && cta + 1 < nctas) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) ll_store(e + (1 * 12 + korder[h] * 3 + d) * 16, Bnd[h][d], seq);
+                    }
+                }
+            }
+            const bool need_l = active && isrow[h] && sl == 0 && !right[h] && cta > 0;
+            const bool need_r = active && isrow[h] && sl == nact - 1 && right[h] && cta + 1 < nctas;
+            need[h] = need_l || need_r;
+            rslot[h] = mbox + par * mbox_par_stride +
+                (need_l ? ((size_t)(cta - 1) * 24 + 12 + korder[h] * 3) * 16 : ((size_t)(cta + 1) * 24 + korder[h] * 3) * 16);
+        }
+        // prefetch the rows of the neighbouring CTAs: the loads fly during the projections
+        LLRaw rr[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+            if (need[h]) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) ll_issue(rslot[h] + d * 16, rr[h][d]);
+            }
+        if (CONS) {
+            if (has_box) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + (0) * 4 + 1) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 1) * 32]); Pv[0][d] = e0; Pv[1][d] = e1; }
+            }
+            if (has_vel) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + (0) * 4 + 2) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 2) * 32]); Vv[0][d] = e0 * invT; Vv[1][d] = e1 * invT; }
+            }
+            if (has_acc) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + (0) * 4 + 3) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 3) * 32]); Av[0][d] = e0 * invT2; Av[1][d] = e1 * invT2; }
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (has_vel) ball_update(Vv[h], vmax, phv[h], wv[h]);      // a4: Eq. 20f, 20g
+                if (has_acc) ball_update(Av[h], amax, pha[h], wa[h]);
+            }
+            if (has_box) {      // a7 + a8: Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q)
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const double lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const double vp = fmax(-qp[h][d], 0.0), vn = fmax(-qn[h][d], 0.0);
+                        qp[h][d] = (hi - Pv[h][d]) - vp;
+                        qn[h][d] = (Pv[h][d] - lo) - vn;
+                    }
+                }
+            }
+        }
+
+        // ================= exchange of boundary rows =================
+        int wait_failed = 0;
+        {
+            bool okk = true;
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+                if (need[h]) okk = okk && ll_ok(rr[h][0], seq) && ll_ok(rr[h][1], seq) && ll_ok(rr[h][2], seq);
+            if (pairwise && *(volatile int*)&abort_any) okk = true;
+            if (!__all_sync(0xffffffffu, okk)) {
+                const long long t0 = global_ns();
+                unsigned spins = 0;
+                do {
+                    if (!okk) {
+                        okk = true;
+#pragma unroll
+                        for (int h = 0; h < 2; ++h)
+                            if (need[h]) {
+#pragma unroll
+                                for (int d = 0; d < 3; ++d) ll_issue(rslot[h] + d * 16, rr[h][d]);
+                                okk = okk && ll_ok(rr[h][0], seq) && ll_ok(rr[h][1], seq) && ll_ok(rr[h][2], seq);
+                            }
+                    }
+                    bool bail = false;
+                    if ((++spins & 255u) == 0) bail = *(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS;
+                    if (__any_sync(0xffffffffu, bail)) { if (!okk) { atomicExch(p.abort_flag, 1); wait_failed = 1; } break; }
+                } while (!__all_sync(0xffffffffu, okk));
+            }
+        }
+        if (wait_failed) { abort_sh[it & 1] = 1; *(volatile int*)&abort_any = 1; }
+        if (pairwise) {
+            const int first = (warp & 1) ? warp - 1 : warp, second = (warp & 1) ? warp : warp - 1;
+            if (first >= 0 && first + 1 < nwarps) asm volatile("bar.sync %0, 64;" ::"r"(first) : "memory");
+            if (second >= 0 && second + 1 < nwarps) asm volatile("bar.sync %0, 64;" ::"r"(second) : "memory");
+        } else if (nctas == 1) {
+            __syncthreads();
+        } else if (!nb_sync) {
+            if (!grid_barrier(p.bar, (unsigned long long)(it + 1) * nctas, p.abort_flag)) break;
+            if (abort_sh[it & 1]) break;
+        } else {
+            __syncthreads();
+            if (abort_sh[it & 1]) break;
+        }
+
+        // ================= phase B: consensus, dual, residuals =================
+        double rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
+        double dz[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) dz[h][d] = 0.0;
+            if (!isrow[h]) continue;
+            double nb[3];
+            if (need[h]) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) nb[d] = ll_value(rr[h][d]);
+            } else {
+                const double* e = right[h] ? Bcur + (sl + 2) * 24 + korder[h] * 3 : Bcur + sl * 24 + (korder[h] + S) * 3;
+#pragma unroll
+                for (int d = 0; d < 3; ++d) nb[d] = e[d];
+            }
+            if (korder[h] == 0) {       // position rows live in segment-local frames: shift the neighbour's into mine
+#pragma unroll
+                for (int d = 0; d < 3; ++d) nb[d] += zoffs[((right[h] ? 3 : 0) + d) * SA + sl];
+            }
+            const bool fixed = (right[h] ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder[h] == 0) ||
+                               (right[h] ? open_r : open_l);      // outer end of a halo: no neighbour in this launch
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const double bl = right[h] ? Bnd[h][d] : nb[d], br = right[h] ? nb[d] : Bnd[h][d];
+                const double znew = fixed ? zt[h][d] : 0.5 * (bl + br);      // a5: Eq. 6b / 20b
+                dz[h][d] = znew - zt[h][d];
+                zt[h][d] = znew;
+                const double res = Bnd[h][d] - znew;
+                u[h][d] += res;                                              // a8: Eq. 6c / 20c (scaled dual, A5)
+                if (last_sweep) {
+                    rp2 += res * res;
+                    if (right[h] && !(sf & SEG_LAST)) { const double gp = Bnd[h][d] - nb[d]; gap2 += gp * gp; }   // Eq. 21
+                }
+            }
+        }
+        if (last_sweep) {
+            // a6: dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8):
+            // the consensus block of the a1 contraction applied to dz; lane t ends with coefficient rows 2t, 2t+1
+            const double Tp0 = static_cast<const double*>(p.Tpow)[gseg * LANES + 2 * lane];
+            const double Tp1 = static_cast<const double*>(p.Tpow)[gseg * LANES + 2 * lane + 1];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                double x0 = 0, x1 = 0;
+                dmma884(x0, x1, dz[0][d] * invTk[0], ctab[(0) * 32]);
+                dmma884(x0, x1, dz[1][d] * invTk[1], ctab[(1) * 32]);
+                const double xr0 = rho_cur * x0, xr1 = rho_cur * x1;
+                rdn2 += xr0 * xr0 + xr1 * xr1;
+                rd2 += (xr0 * Tp0) * (xr0 * Tp0) + (xr1 * Tp1) * (xr1 * Tp1);
+            }
+#pragma unroll
+            for (int m = 1; m < LPS; m <<= 1) {     // fixed-order tree over the 4 lanes of the segment
+                rp2 += shfl_xor(rp2, m); rd2 += shfl_xor(rd2, m); rdn2 += shfl_xor(rdn2, m); gap2 += shfl_xor(gap2, m);
+            }
+            if (owned && lane == 0) {
+                double* o = p.part + gseg * 4;
+                o[0] = rp2; o[1] = rd2; o[2] = rdn2; o[3] = gap2;
+            }
+            if (SOLVE && ce > 0) {
+                // ---- CTA partial (fixed order), all-gather over the CTAs, decision
+                double q4[4] = {rp2, rd2, rdn2, gap2};
+                if (!(owned && lane == 0)) { q4[0] = q4[1] = q4[2] = q4[3] = 0.0; }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) { q4[k] += shfl_xor(q4[k], 4); q4[k] += shfl_xor(q4[k], 8); q4[k] += shfl_xor(q4[k], 16); }
+                if ((tid & 31) == 0) { for (int k = 0; k < 4; ++k) wsum_sh[tid >> 5][k] = q4[k]; }
+                __syncthreads();
+                unsigned char* const rb = static_cast<unsigned char*>(p.resbox) + (size_t)(ncheck & 1) * p.max_ctas * 4 * 16;
+                if (tid == 0) {
+                    for (int k = 0; k < 4; ++k) {
+                        double acc = 0.0;
+                        for (int w = 0; w < (T >> 5); ++w) acc += wsum_sh[w][k];
+                        ll_store(rb + ((size_t)cta * 4 + k) * 16, acc, seq);
+                    }
+                }
+                int gather_failed = 0;
+                for (int tt = tid; tt < nctas; tt += T) {
+                    const long long t0 = global_ns();
+                    unsigned spins = 0;
+                    for (int k = 0; k < 4; ++k) {
+                        LLRaw r;
+                        ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
+                        while (!ll_ok(r, seq)) {
+                            if ((++spins & 255u) == 0 && (*(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS)) {
+                                atomicExch(p.abort_flag, 1); gather_failed = 1; break;
+                            }
+                            ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
+                        }
+                        allp_sh[tt][k] = ll_value(r);
+                    }
+                }
+                gather_failed = __syncthreads_or(gather_failed);
+                if (tid < 4) {
+                    double acc = 0.0;
+                    for (int tt = 0; tt < nctas; ++tt) acc += allp_sh[tt][tid];
+                    tot_sh[tid] = acc;
+                }
+                __syncthreads();
+                ++ncheck;
+                const double rp = sqrt(tot_sh[0]), rd = sqrt(tot_sh[p.rd_sel]);
+                const bool conv = rp < p.tol && rd < p.tol;
+                if (conv || gather_failed || !(rp == rp) || !(rd == rd)) { stopped = conv ? 1 : 0; sweeps_done = it + 1; break; }
+                if (p.adaptive) {      // Eq. 24, then reading A16 for the scaled duals
+                    double rho_new = rho_cur;
+                    if (rp > p.mu * rd) rho_new = rho_cur * p.tau_incr;
+                    else if (rd > p.mu * rp) rho_new = rho_cur / p.tau_decr;
+                    if (rho_new != rho_cur) {
+                        const double ratio = rho_cur / rho_new;
+#pragma unroll
+                        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+                            for (int d = 0; d < 3; ++d) {
+                                u[h][d] *= ratio; wv[h][d] *= ratio; wa[h][d] *= ratio;
+                                if (qp[h][d] < 0) qp[h][d] *= ratio;
+                                if (qn[h][d] < 0) qn[h][d] *= ratio;
+                            }
+                            // operator refresh from the spectral form (as refresh_operator_kernel): my rows of rho Pm^, c0^
+                            double wd[MAXN];
+                            for (int i = 0; i < MAXN; ++i) {
+                                const double lam = i < p.q ? p.lam[i * p.nseg_pad + gseg] : 0.0;
+                                wd[i] = i < p.q ? p.W[i * stride + gt[h]] * (rho_new / (lam + rho_new)) : 0.0;
+                            }
+#pragma unroll
+                            double c0n[3];
+#pragma unroll
+                            for (int d = 0; d < 3; ++d) c0n[d] = jj[h] == 1 ? p.dp[d * p.nseg_pad + gseg] : 0.0;
+                            for (int b = 0; b < 8; b += 2) {
+                                double v2[2];
+                                for (int e = 0; e < 2; ++e) {
+                                    double v = 0.0;
+                                    if (b + e < N2) for (int i = 0; i < p.q; ++i) v += wd[i] * p.W[i * stride + gseg * LANES + b + e];
+                                    v2[e] = v;
+#pragma unroll
+                                    for (int d = 0; d < 3; ++d) c0n[d] -= v * p.g0[d * stride + gseg * LANES + b + e];
+                                }
+                                Pms[(h * 4 + (b >> 1)) * T] = make_double2(v2[0], v2[1]);
+                            }
+#pragma unroll
+                            for (int d = 0; d < 3; ++d) c0s[(h * 3 + d) * T] = c0n[d];
+                        }
+                        rho_cur = rho_new;
+                    }
+                }
+            }
+        }
+    }
+    if (SOLVE && ce > 0 && cta == 0 && tid == 0) {
+        double* o = p.solve_out;
+        o[0] = (double)sweeps_done; o[1] = (double)stopped; o[2] = rho_cur;
+        o[3] = sqrt(tot_sh[0]); o[4] = sqrt(tot_sh[1]); o[5] = sqrt(tot_sh[2]); o[6] = sqrt(tot_sh[3]);
+    }
+
+    // ---- write iterate k + k_sweeps back
+    if (owned) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const long long i = d * stride + gt[h];
+                static_cast<double*>(p.zt_out)[i] = zt[h][d];
+                static_cast<double*>(p.u_out)[i] = u[h][d];
+                if (has_box) { static_cast<double*>(p.qp_out)[i] = qp[h][d]; static_cast<double*>(p.qn_out)[i] = qn[h][d]; }
+                if (has_vel) { static_cast<double*>(p.phv_out)[i] = phv[h][d]; static_cast<double*>(p.wv_out)[i] = wv[h][d]; }
+                if (has_acc) { static_cast<double*>(p.pha_out)[i] = pha[h][d]; static_cast<double*>(p.wa_out)[i] = wa[h][d]; }
+            }
+    }
+}
+
+template <int S, bool CONS, int MAXT>
+cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
+    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<S, CONS, MAXT, true> : cadmm_sweeps_mma_kernel<S, CONS, MAXT, false>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    KParams pc = p;
+    void* args[] = {&pc};
+    if (ctas > 1) return cudaLaunchCooperativeKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+    return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+}
+
+template <int S, bool CONS, int MAXT>
+cudaError_t limits_mma(int threads, size_t smem, int* per_sm) {
+    auto kern = cadmm_sweeps_mma_kernel<S, CONS, MAXT, true>;     // the larger of the two instantiations
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
+}
+
+}  // namespace
+
+#define TOP_DISPATCH_MMA(CALL)                                                         \
+    if (s == 3) { if (constrained) { CALL(3, true) } else { CALL(3, false) } }         \
+    else        { if (constrained) { CALL(4, true) } else { CALL(4, false) } }
+
+int max_threads_mma() { return MAXT_MMA; }
+
+cudaError_t launch_sweeps_mma(const KParams& p, int s, bool constrained, int ctas, int threads, size_t smem, cudaStream_t st) {
+#define CALL(S_, C_) return launch_mma<S_, C_, MAXT_MMA>(p, ctas, threads, smem, st);
+    TOP_DISPATCH_MMA(CALL)
+#undef CALL
+    return cudaErrorInvalidValue;
+}
+
+cudaError_t sweep_kernel_limits_mma(int s, bool constrained, int threads, size_t smem, int* max_ctas_per_sm) {
+#define CALL(S_, C_) return limits_mma<S_, C_, MAXT_MMA>(threads, smem, max_ctas_per_sm);
+    TOP_DISPATCH_MMA(CALL)
+#undef CALL
+    return cudaErrorInvalidValue;
+}
+
+size_t sweep_smem_bytes_mma(bool constrained, int segs_per_cta) {
+    return smem_layout_mma(constrained, (segs_per_cta * 4 + 31) / 32 * 8).total;
+}
+
+}  // namespace top

@@ -21,6 +21,7 @@ WAYPOINT = {"hard": 0, "pinned_z": 1, "free": 2}
 TOP_RD_NORMALISED = 4
 TOP_EPS_N_SCALED = 8
 TOP_RHO_ADAPTIVE = 64
+TOP_KERNEL_NO_MMA = 128
 SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
 EXPORTS = ["top_create", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
@@ -151,7 +152,7 @@ class TopSolver:
     def __init__(self, waypoints, durations, s, rho, dtype="f64", samples=0, box_lo=None, box_hi=None, vmax=0.0,
                  amax=0.0, start_derivs=None, end_derivs=None, mode="hard", rd_normalised=False, eps_n_scaled=False,
                  sync="auto", check_every=0, max_iter=0, device=-1, stream=0, segs_per_cta=0, lanes=0, adaptive_rho=False,
-                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0):
+                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0, no_mma=False):
         L = lib()
         wp = np.asarray(waypoints, dtype=np.float64)
         T = np.asarray(durations, dtype=np.float64)
@@ -176,7 +177,8 @@ class TopSolver:
         if samples:
             cons = _Constraints(int(samples), _dptr(lo), _dptr(hi), float(vmax), float(amax))
         flags = WAYPOINT[mode] | (TOP_RD_NORMALISED if rd_normalised else 0) | \
-            (TOP_EPS_N_SCALED if eps_n_scaled else 0) | SYNC[sync] | (TOP_RHO_ADAPTIVE if adaptive_rho else 0)
+            (TOP_EPS_N_SCALED if eps_n_scaled else 0) | SYNC[sync] | (TOP_RHO_ADAPTIVE if adaptive_rho else 0) | \
+            (TOP_KERNEL_NO_MMA if no_mma else 0)
         opt = _Options(ctypes.sizeof(_Options), flags, int(check_every), int(device), int(max_iter),
                        ctypes.c_void_p(stream), int(segs_per_cta), int(lanes), float(adapt_mu), float(adapt_tau_incr),
                        float(adapt_tau_decr))
