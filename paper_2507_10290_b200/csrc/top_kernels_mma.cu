@@ -258,7 +258,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         }
         // a3: evaluate the new polynomial: consensus rows of B = M c (Eq. 20b), and the lane's two samples of E0 c, E1 c,
         // E2 c (Eq. 20d-g).  A operand = the lane's own coefficient rows; accumulator columns = the lane's own items.
-        double Bnd[2][3], Pv[2][3], Vv[2][3], Av[2][3];
+        double Bnd[2][3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             double e0 = 0, e1 = 0;
@@ -266,9 +266,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 0) * 32]);
             Bnd[0][d] = e0 * invTk[0]; Bnd[1][d] = e1 * invTk[1];
         }
-        // publish: shared memory for the neighbours in this CTA, mailbox for the neighbouring CTAs
-        bool need[2];
-        const unsigned char* rslot[2];
+        // publish: shared memory for the neighbours in this CTA (and for this lane's own phase B), mailbox for the
+        // neighbouring CTAs.  A lane needs at most ONE of its two rows from another CTA (a CTA with a neighbour on
+        // both sides owns >= 4 segments, so its left-edge and right-edge segments differ): one prefetch buffer.
+        bool need = false;
+        int need_h = 0;
+        const unsigned char* rslot = mbox;
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             if (isrow[h]) {
@@ -288,46 +291,43 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             }
             const bool need_l = active && isrow[h] && sl == 0 && !right[h] && cta > 0;
             const bool need_r = active && isrow[h] && sl == nact - 1 && right[h] && cta + 1 < nctas;
-            need[h] = need_l || need_r;
-            rslot[h] = mbox + par * mbox_par_stride +
-                (need_l ? ((size_t)(cta - 1) * 24 + 12 + korder[h] * 3) * 16 : ((size_t)(cta + 1) * 24 + korder[h] * 3) * 16);
+            if (need_l || need_r) {
+                need = true; need_h = h;
+                rslot = mbox + par * mbox_par_stride +
+                    (need_l ? ((size_t)(cta - 1) * 24 + 12 + korder[h] * 3) * 16 : ((size_t)(cta + 1) * 24 + korder[h] * 3) * 16);
+            }
         }
         // prefetch the rows of the neighbouring CTAs: the loads fly during the projections
-        LLRaw rr[2][3];
+        LLRaw rr[3];
+        if (need) {
 #pragma unroll
-        for (int h = 0; h < 2; ++h)
-            if (need[h]) {
-#pragma unroll
-                for (int d = 0; d < 3; ++d) ll_issue(rslot[h] + d * 16, rr[h][d]);
-            }
+            for (int d = 0; d < 3; ++d) ll_issue(rslot + d * 16, rr[d]);
+        }
         if (CONS) {
-            if (has_box) {
+            if (has_vel) {      // a4: Eq. 20f, 20g on the velocity samples
+                double Vv[2][3];
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + (0) * 4 + 1) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 1) * 32]); Pv[0][d] = e0; Pv[1][d] = e1; }
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 2) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 2) * 32]); Vv[0][d] = e0 * invT; Vv[1][d] = e1 * invT; }
+#pragma unroll
+                for (int h = 0; h < 2; ++h) ball_update(Vv[h], vmax, phv[h], wv[h]);
             }
-            if (has_vel) {
+            if (has_acc) {      //     and on the acceleration samples
+                double Av[2][3];
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + (0) * 4 + 2) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 2) * 32]); Vv[0][d] = e0 * invT; Vv[1][d] = e1 * invT; }
-            }
-            if (has_acc) {
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = e0 * invT2; Av[1][d] = e1 * invT2; }
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + (0) * 4 + 3) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 3) * 32]); Av[0][d] = e0 * invT2; Av[1][d] = e1 * invT2; }
-            }
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                if (has_vel) ball_update(Vv[h], vmax, phv[h], wv[h]);      // a4: Eq. 20f, 20g
-                if (has_acc) ball_update(Av[h], amax, pha[h], wa[h]);
+                for (int h = 0; h < 2; ++h) ball_update(Av[h], amax, pha[h], wa[h]);
             }
             if (has_box) {      // a7 + a8: Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q)
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
+                    double P0 = 0, P1 = 0;
+                    dmma884(P0, P1, c[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(P0, P1, c[1][d], ctab[(8 + 1 * 4 + 1) * 32]);
                     const double lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
-#pragma unroll
-                    for (int h = 0; h < 2; ++h) {
-                        const double vp = fmax(-qp[h][d], 0.0), vn = fmax(-qn[h][d], 0.0);
-                        qp[h][d] = (hi - Pv[h][d]) - vp;
-                        qn[h][d] = (Pv[h][d] - lo) - vn;
-                    }
+                    qp[0][d] = (hi - P0) - fmax(-qp[0][d], 0.0);
+                    qn[0][d] = (P0 - lo) - fmax(-qn[0][d], 0.0);
+                    qp[1][d] = (hi - P1) - fmax(-qp[1][d], 0.0);
+                    qn[1][d] = (P1 - lo) - fmax(-qn[1][d], 0.0);
                 }
             }
         }
@@ -335,24 +335,16 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         // ================= exchange of boundary rows =================
         int wait_failed = 0;
         {
-            bool okk = true;
-#pragma unroll
-            for (int h = 0; h < 2; ++h)
-                if (need[h]) okk = okk && ll_ok(rr[h][0], seq) && ll_ok(rr[h][1], seq) && ll_ok(rr[h][2], seq);
+            bool okk = !need || (ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq));
             if (pairwise && *(volatile int*)&abort_any) okk = true;
             if (!__all_sync(0xffffffffu, okk)) {
                 const long long t0 = global_ns();
                 unsigned spins = 0;
                 do {
                     if (!okk) {
-                        okk = true;
 #pragma unroll
-                        for (int h = 0; h < 2; ++h)
-                            if (need[h]) {
-#pragma unroll
-                                for (int d = 0; d < 3; ++d) ll_issue(rslot[h] + d * 16, rr[h][d]);
-                                okk = okk && ll_ok(rr[h][0], seq) && ll_ok(rr[h][1], seq) && ll_ok(rr[h][2], seq);
-                            }
+                        for (int d = 0; d < 3; ++d) ll_issue(rslot + d * 16, rr[d]);
+                        okk = ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq);
                     }
                     bool bail = false;
                     if ((++spins & 255u) == 0) bail = *(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS;
@@ -383,10 +375,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
             for (int d = 0; d < 3; ++d) dz[h][d] = 0.0;
             if (!isrow[h]) continue;
-            double nb[3];
-            if (need[h]) {
+            double nb[3], own[3];
 #pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] = ll_value(rr[h][d]);
+            for (int d = 0; d < 3; ++d) own[d] = Bcur[(sl + 1) * 24 + jj[h] * 3 + d];
+            if (need && need_h == h) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) nb[d] = ll_value(rr[d]);
             } else {
                 const double* e = right[h] ? Bcur + (sl + 2) * 24 + korder[h] * 3 : Bcur + sl * 24 + (korder[h] + S) * 3;
 #pragma unroll
@@ -400,15 +394,15 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                                (right[h] ? open_r : open_l);      // outer end of a halo: no neighbour in this launch
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                const double bl = right[h] ? Bnd[h][d] : nb[d], br = right[h] ? nb[d] : Bnd[h][d];
+                const double bl = right[h] ? own[d] : nb[d], br = right[h] ? nb[d] : own[d];
                 const double znew = fixed ? zt[h][d] : 0.5 * (bl + br);      // a5: Eq. 6b / 20b
                 dz[h][d] = znew - zt[h][d];
                 zt[h][d] = znew;
-                const double res = Bnd[h][d] - znew;
+                const double res = own[d] - znew;
                 u[h][d] += res;                                              // a8: Eq. 6c / 20c (scaled dual, A5)
                 if (last_sweep) {
                     rp2 += res * res;
-                    if (right[h] && !(sf & SEG_LAST)) { const double gp = Bnd[h][d] - nb[d]; gap2 += gp * gp; }   // Eq. 21
+                    if (right[h] && !(sf & SEG_LAST)) { const double gp = own[d] - nb[d]; gap2 += gp * gp; }   // Eq. 21
                 }
             }
         }
