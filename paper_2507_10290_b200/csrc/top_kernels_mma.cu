@@ -27,11 +27,35 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+// 1/sqrt(x) for x > 0, normal: the hardware seed (MUFU.RSQ64H, ~2^-22 relative) and ONE cubically convergent step
+// y (1 + e/2 + 3e^2/8), e = 1 - x y^2  =>  error ~ e^3: full double precision (a few ulp), 5 fp64 operations and no
+// branch.  The library rsqrt() adds special-case branches that keep ptxas from interleaving independent projections.
+__device__ __forceinline__ double rsqrt_pos(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x * y, y, 1.0);
+    return fma(y * e, fma(0.375, e, 0.5), y);
+}
+
+// max(-q, 0) on the integer pipe (the fp64 pipe is the bound of this kernel): -q where the sign bit of q is set, else +0
+__device__ __forceinline__ double neg_part(double q) {
+    const int hi = __double2hiint(q), lo = __double2loint(q);
+    const int m = hi >> 31;
+    return __hiloint2double((hi ^ 0x80000000) & m, lo & m);
+}
+
+// Eq. 20f without a branch: the factor min(1, bound/||y||) of the projection of y onto ||.|| <= bound (reading A15)
+__device__ __forceinline__ double ball_scale(const double (&y)[3], double bound) {
+    const double n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+    const double sc = bound * rsqrt_pos(n2);               // garbage (inf/NaN) when n2 == 0: not selected then
+    return n2 > bound * bound ? sc : 1.0;
+}
+
 // one instantiation: <= 288 threads (9 warps of 8 segments: 224 registers per thread)
 constexpr int MAXT_MMA = 288;
 
 struct SmemLayoutMma {
-    size_t pm, c0, ctab, lohi, xs, bs, zoff, total;
+    size_t pm, c0, zu, qs, ws, ctab, lohi, xs, bs, zoff, total;
 };
 __host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc) {
     SmemLayoutMma L;
@@ -39,6 +63,9 @@ __host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_all
     size_t off = 0;
     L.pm = off;   off = align16(off + (size_t)2 * 4 * T * sizeof(double2));            // rho*Pm^ rows, [h][b/2][thread] pairs
     L.c0 = off;   off = align16(off + (size_t)6 * T * sizeof(double));                 // c0^ rows, [h][d][thread]
+    L.zu = off;   off = align16(off + (size_t)6 * T * sizeof(double2));                // (z~, u) of the lane's two consensus rows, [h][d][thread]
+    L.qs = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // Moreau pair values (q+, q-) of the lane's two samples
+    L.ws = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // ball duals (w_v, w_a) of the lane's two samples
     L.ctab = off; off = align16(off + (size_t)16 * 32 * sizeof(double));               // constant MMA operands, [16][lane of warp]
     L.lohi = off; off = align16(off + (size_t)(cons ? 6 : 0) * segs_alloc * sizeof(double));
     L.xs = off;   off = align16(off + (size_t)segs_alloc * XSTRIDE * sizeof(double));  // rhs rows, all-gather
@@ -46,6 +73,32 @@ __host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_all
     L.zoff = off; off = align16(off + (size_t)6 * segs_alloc * sizeof(double));        // frame shift of the neighbours' position rows
     L.total = off;
     return L;
+}
+
+// Operator refresh of one coefficient row inside the solve kernel (Eq. 24 changed rho): row `row` of rho Pm^ and of c0^ from
+// the rho-independent spectral data, as refresh_operator_kernel does for the arrays.  Rare path: kept out of line so
+// that its registers do not count against the sweep loop.
+template <int N2, int TS>
+__device__ __noinline__ void refresh_operator_rows(const KParams& p, long long gseg, long long gt, int row, double rho_new,
+                                                   double2* pm_row /* [4 pairs] stride TS */, double* c0_row /* [3] stride TS */) {
+    double wd[MAXN];
+    for (int i = 0; i < MAXN; ++i) {
+        const double lam = i < p.q ? p.lam[i * p.nseg_pad + gseg] : 0.0;
+        wd[i] = i < p.q ? p.W[i * p.stride + gt] * (rho_new / (lam + rho_new)) : 0.0;
+    }
+    double c0n[3];
+    for (int d = 0; d < 3; ++d) c0n[d] = row == 1 ? p.dp[d * p.nseg_pad + gseg] : 0.0;
+    for (int b = 0; b < 8; b += 2) {
+        double v2[2];
+        for (int e = 0; e < 2; ++e) {
+            double v = 0.0;
+            if (b + e < N2) for (int i = 0; i < p.q; ++i) v += wd[i] * p.W[i * p.stride + gseg * LANES + b + e];
+            v2[e] = v;
+            for (int d = 0; d < 3; ++d) c0n[d] -= v * p.g0[d * p.stride + gseg * LANES + b + e];
+        }
+        pm_row[(b >> 1) * TS] = make_double2(v2[0], v2[1]);
+    }
+    for (int d = 0; d < 3; ++d) c0_row[d * TS] = c0n[d];
 }
 
 template <int S, bool CONS, int MAXT, bool SOLVE>
@@ -56,7 +109,11 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 
     const int T = blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
     const int grp = (tid >> 2) & 7;                // segment within the warp = row / column group of the MMA fragments
-    const int SA = T >> 2;                         // segment slots of this CTA (>= segs_per_cta; T is a multiple of 32)
+    // Shared-memory arrays are laid out for the LARGEST CTA of this instantiation whatever the launched size (one CTA
+    // per SM: the space is there), so every stride is a compile-time constant and every shared-memory address is one
+    // per-thread base register plus an immediate (with run-time strides ptxas re-derived the offsets inside the loop).
+    constexpr int TS = MAXT;                       // thread stride of the per-thread arrays
+    constexpr int SA = MAXT / 4;                   // segment slots
     const int SEGS = p.segs_per_cta;
     const int cta = blockIdx.x, nctas = gridDim.x;
     const uint32_t flags = p.flags;
@@ -65,8 +122,11 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     const bool nb_sync = flags & KF_NEIGHBOUR_SYNC;
 
     const SmemLayoutMma L = smem_layout_mma(CONS, SA);
-    double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + tid;          // [(h*4 + b/2) * T]
-    double* c0s = reinterpret_cast<double*>(smem_raw + L.c0) + tid;            // [(h*3 + d) * T]
+    double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + tid;          // [(h*4 + b/2) * TS]
+    double* c0s = reinterpret_cast<double*>(smem_raw + L.c0) + tid;            // [(h*3 + d) * TS]
+    double2* zus = reinterpret_cast<double2*>(smem_raw + L.zu) + tid;         // [(h*3 + d) * TS]: (z~, u); registers are short at 9 warps per SM
+    double2* qs = reinterpret_cast<double2*>(smem_raw + L.qs) + tid;          // [(h*3 + d) * TS]: (q+, q-)
+    double2* ws = reinterpret_cast<double2*>(smem_raw + L.ws) + tid;          // [(h*3 + d) * TS]: (w_v, w_a)
     double* ctab = reinterpret_cast<double*>(smem_raw + L.ctab) + (tid & 31);  // [k * 32]: a1 k-step operands at k = 0..7, a3 operands at k = 8 + kstep*4 + block
     double* lohi = reinterpret_cast<double*>(smem_raw + L.lohi);               // [6][SA]
     double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE;
@@ -132,9 +192,9 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     for (int h = 0; h < 2; ++h) {
 #pragma unroll
         for (int b = 0; b < 8; b += 2)
-            Pms[(h * 4 + (b >> 1)) * T] = make_double2(b < N2 ? p.Pm[b * stride + gt[h]] : 0.0, b + 1 < N2 ? p.Pm[(b + 1) * stride + gt[h]] : 0.0);
+            Pms[(h * 4 + (b >> 1)) * TS] = make_double2(b < N2 ? p.Pm[b * stride + gt[h]] : 0.0, b + 1 < N2 ? p.Pm[(b + 1) * stride + gt[h]] : 0.0);
 #pragma unroll
-        for (int d = 0; d < 3; ++d) c0s[(h * 3 + d) * T] = p.c0[d * stride + gt[h]];
+        for (int d = 0; d < 3; ++d) c0s[(h * 3 + d) * TS] = p.c0[d * stride + gt[h]];
         invTk[h] = static_cast<const double*>(p.invTk)[gt[h]];
     }
     const double invT = static_cast<const double*>(p.invT)[gseg], invT2 = static_cast<const double*>(p.invT)[p.nseg_pad + gseg];
@@ -148,21 +208,33 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     }
     const uint8_t sf = p.segflags[gseg];
     const bool open_l = (flags & KF_OPEN_LEFT) && gseg == p.seg_begin, open_r = (flags & KF_OPEN_RIGHT) && gseg == p.seg_end - 1;
-    // ---- state of iterate k
-    double zt[2][3], u[2][3], qp[2][3], qn[2][3], phv[2][3], wv[2][3], pha[2][3], wa[2][3];
+    // ---- state of iterate k.  Registers hold the a1 OPERANDS (the A fragments of the first contraction), each produced
+    // where its inputs are updated (phase B, projections) so that a1 itself is 24 back-to-back MMAs with no dependent
+    // arithmetic in front of them:
+    //   gM = (z~ - u)/T^k      A0 = (hi - s+ - v+) + (lo + s- + v-)      gv = (phi_v - w_v)/T      ga = (phi_a - w_a)/T^2
+    // The variables behind them live in shared memory as pairs, read and written once per sweep where they are updated:
+    // (z~, u), the Moreau pair values (q+, q-), and the ball duals (w_v, w_a).  phi is not kept at all: it is written to
+    // global memory on the sweeps whose iterate is observable (the last of the launch, and every test sweep of a solve).
+    double gM[2][3], A0[2][3], gv[2][3], ga[2][3];
 #pragma unroll
     for (int h = 0; h < 2; ++h)
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             const long long i = d * stride + gt[h];
-            zt[h][d] = static_cast<const double*>(p.zt)[i];
-            u[h][d] = static_cast<const double*>(p.u)[i];
-            qp[h][d] = has_box ? static_cast<const double*>(p.qp)[i] : 0.0;
-            qn[h][d] = has_box ? static_cast<const double*>(p.qn)[i] : 0.0;
-            phv[h][d] = has_vel ? static_cast<const double*>(p.phv)[i] : 0.0;
-            wv[h][d] = has_vel ? static_cast<const double*>(p.wv)[i] : 0.0;
-            pha[h][d] = has_acc ? static_cast<const double*>(p.pha)[i] : 0.0;
-            wa[h][d] = has_acc ? static_cast<const double*>(p.wa)[i] : 0.0;
+            const double z0 = static_cast<const double*>(p.zt)[i], u0 = static_cast<const double*>(p.u)[i];
+            zus[(h * 3 + d) * TS] = make_double2(z0, u0);
+            gM[h][d] = (z0 - u0) * invTk[h];
+            A0[h][d] = gv[h][d] = ga[h][d] = 0.0;
+            double w_v = 0.0, w_a = 0.0;
+            if (has_box) {
+                const double lo = static_cast<const double*>(p.lohi)[d * p.nseg_pad + gseg], hi = static_cast<const double*>(p.lohi)[(3 + d) * p.nseg_pad + gseg];
+                const double a = static_cast<const double*>(p.qp)[i], b = static_cast<const double*>(p.qn)[i];
+                qs[(h * 3 + d) * TS] = make_double2(a, b);
+                A0[h][d] = (hi - fabs(a)) + (lo + fabs(b));
+            }
+            if (has_vel) { w_v = static_cast<const double*>(p.wv)[i]; gv[h][d] = (static_cast<const double*>(p.phv)[i] - w_v) * invT; }
+            if (has_acc) { w_a = static_cast<const double*>(p.wa)[i]; ga[h][d] = (static_cast<const double*>(p.pha)[i] - w_a) * invT2; }
+            if (CONS) ws[(h * 3 + d) * TS] = make_double2(w_v, w_a);
         }
 
     const double vmax = p.vmax, amax = p.amax;
@@ -187,7 +259,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         const unsigned seq = p.seq_base + (unsigned)it + 1u;
         const int par = (int)(seq & 1u);
         const bool final_sweep = (it == p.k_sweeps - 1);
-        // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
+        // sweeps on which residuals (and the coefficients, and phi) are materialised: the last one, and every test sweep
         const bool last_sweep = final_sweep || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
         double* const Bcur = Bs + (size_t)par * (SA + 2) * 24;
 
@@ -200,28 +272,25 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
-                for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], (zt[h][d] - u[h][d]) * invTk[h], ctab[(h) * 32]);
+                for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gM[h][d], ctab[h * 32]);
             if (CONS) {
                 if (has_box) {      // Ao'(b - s - v), Ao = [E0; -E0], b = [hi; -lo];  s + v = |q| (Moreau pair)
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) {
-                        const double lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
+                    for (int h = 0; h < 2; ++h)
 #pragma unroll
-                        for (int h = 0; h < 2; ++h)
-                            dmma884(acc[d][0], acc[d][1], (hi - fabs(qp[h][d])) + (lo + fabs(qn[h][d])), ctab[(2 + h) * 32]);
-                    }
+                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], A0[h][d], ctab[(2 + h) * 32]);
                 }
                 if (has_vel) {
 #pragma unroll
                     for (int h = 0; h < 2; ++h)
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], (phv[h][d] - wv[h][d]) * invT, ctab[(4 + h) * 32]);
+                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gv[h][d], ctab[(4 + h) * 32]);
                 }
                 if (has_acc) {
 #pragma unroll
                     for (int h = 0; h < 2; ++h)
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], (pha[h][d] - wa[h][d]) * invT2, ctab[(6 + h) * 32]);
+                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], ga[h][d], ctab[(6 + h) * 32]);
                 }
             }
 #pragma unroll
@@ -235,12 +304,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             double pm[8];
 #pragma unroll
             for (int b = 0; b < N2; b += 2) {
-                const double2 t2 = Pms[(h * 4 + (b >> 1)) * T];
+                const double2 t2 = Pms[(h * 4 + (b >> 1)) * TS];
                 pm[b] = t2.x; pm[b + 1] = t2.y;
             }
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                double v = c0s[(h * 3 + d) * T];
+                double v = c0s[(h * 3 + d) * TS];
 #pragma unroll
                 for (int b = 0; b < N2; b += 2) {
                     const double2 t2 = *reinterpret_cast<const double2*>(Xs + d * 8 + b);
@@ -258,23 +327,20 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         }
         // a3: evaluate the new polynomial: consensus rows of B = M c (Eq. 20b), and the lane's two samples of E0 c, E1 c,
         // E2 c (Eq. 20d-g).  A operand = the lane's own coefficient rows; accumulator columns = the lane's own items.
-        double Bnd[2][3];
+        {
+            double Bnd[2][3];
 #pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            double e0 = 0, e1 = 0;
-            dmma884(e0, e1, c[0][d], ctab[(8 + (0) * 4 + 0) * 32]);
-            dmma884(e0, e1, c[1][d], ctab[(8 + (1) * 4 + 0) * 32]);
-            Bnd[0][d] = e0 * invTk[0]; Bnd[1][d] = e1 * invTk[1];
-        }
-        // publish: shared memory for the neighbours in this CTA (and for this lane's own phase B), mailbox for the
-        // neighbouring CTAs.  A lane needs at most ONE of its two rows from another CTA (a CTA with a neighbour on
-        // both sides owns >= 4 segments, so its left-edge and right-edge segments differ): one prefetch buffer.
-        bool need = false;
-        int need_h = 0;
-        const unsigned char* rslot = mbox;
+            for (int d = 0; d < 3; ++d) {
+                double e0 = 0, e1 = 0;
+                dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 0) * 32]);
+                dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 0) * 32]);
+                Bnd[0][d] = e0 * invTk[0]; Bnd[1][d] = e1 * invTk[1];
+            }
+            // publish: shared memory for the neighbours in this CTA (and for this lane's own phase B), mailbox for the
+            // neighbouring CTAs
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            if (isrow[h]) {
+            for (int h = 0; h < 2; ++h) {
+                if (!isrow[h]) continue;
 #pragma unroll
                 for (int d = 0; d < 3; ++d) Bcur[(sl + 1) * 24 + jj[h] * 3 + d] = Bnd[h][d];
                 if (nctas > 1 && active) {
@@ -289,6 +355,15 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     }
                 }
             }
+        }
+        // A lane needs at most ONE of its two rows from another CTA (a CTA with a neighbour on both sides owns >= 4
+        // segments, so its left-edge and right-edge segments differ): one prefetch buffer.  The loads fly during the
+        // projections.
+        bool need = false;
+        int need_h = 0;
+        const unsigned char* rslot = mbox;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
             const bool need_l = active && isrow[h] && sl == 0 && !right[h] && cta > 0;
             const bool need_r = active && isrow[h] && sl == nact - 1 && right[h] && cta + 1 < nctas;
             if (need_l || need_r) {
@@ -297,37 +372,70 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     (need_l ? ((size_t)(cta - 1) * 24 + 12 + korder[h] * 3) * 16 : ((size_t)(cta + 1) * 24 + korder[h] * 3) * 16);
             }
         }
-        // prefetch the rows of the neighbouring CTAs: the loads fly during the projections
         LLRaw rr[3];
         if (need) {
 #pragma unroll
             for (int d = 0; d < 3; ++d) ll_issue(rslot + d * 16, rr[d]);
         }
         if (CONS) {
-            if (has_vel) {      // a4: Eq. 20f, 20g on the velocity samples
-                double Vv[2][3];
+            // the three sample blocks of the evaluation back to back (the fp64 pipe stays busy), then the projections of
+            // all blocks side by side: independent dependency chains, no branch between them
+            double Pv[2][3], Vv[2][3], Av[2][3];
+            if (has_vel) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 2) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 2) * 32]); Vv[0][d] = e0 * invT; Vv[1][d] = e1 * invT; }
-#pragma unroll
-                for (int h = 0; h < 2; ++h) ball_update(Vv[h], vmax, phv[h], wv[h]);
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 2) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 2) * 32]); Vv[0][d] = e0; Vv[1][d] = e1; }
             }
-            if (has_acc) {      //     and on the acceleration samples
-                double Av[2][3];
+            if (has_acc) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = e0 * invT2; Av[1][d] = e1 * invT2; }
-#pragma unroll
-                for (int h = 0; h < 2; ++h) ball_update(Av[h], amax, pha[h], wa[h]);
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = e0; Av[1][d] = e1; }
             }
-            if (has_box) {      // a7 + a8: Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q)
+            if (has_box) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 1) * 32]); Pv[0][d] = e0; Pv[1][d] = e1; }
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                double2 w2[3];
+#pragma unroll
+                for (int d = 0; d < 3; ++d) w2[d] = ws[(h * 3 + d) * TS];
+                if (has_vel) {      // a4: Eq. 20f, 20g;  y = A c + w,  phi = proj(y),  w <- y - phi;  next operand (phi - w)/T
+                    double y[3], phi[3];
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) y[d] = Vv[h][d] * invT + w2[d].x;
+                    const double scale = ball_scale(y, vmax);
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) { phi[d] = scale * y[d]; w2[d].x = y[d] - phi[d]; gv[h][d] = (phi[d] - w2[d].x) * invT; }
+                    if (last_sweep && owned) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) static_cast<double*>(p.phv_out)[d * stride + gt[h]] = phi[d];
+                    }
+                }
+                if (has_acc) {
+                    double y[3], phi[3];
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) y[d] = Av[h][d] * invT2 + w2[d].y;
+                    const double scale = ball_scale(y, amax);
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) { phi[d] = scale * y[d]; w2[d].y = y[d] - phi[d]; ga[h][d] = (phi[d] - w2[d].y) * invT2; }
+                    if (last_sweep && owned) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) static_cast<double*>(p.pha_out)[d * stride + gt[h]] = phi[d];
+                    }
+                }
+#pragma unroll
+                for (int d = 0; d < 3; ++d) ws[(h * 3 + d) * TS] = w2[d];
+            }
+            if (has_box) {      // a7 + a8: Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q);  next operand
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
-                    double P0 = 0, P1 = 0;
-                    dmma884(P0, P1, c[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(P0, P1, c[1][d], ctab[(8 + 1 * 4 + 1) * 32]);
                     const double lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
-                    qp[0][d] = (hi - P0) - fmax(-qp[0][d], 0.0);
-                    qn[0][d] = (P0 - lo) - fmax(-qn[0][d], 0.0);
-                    qp[1][d] = (hi - P1) - fmax(-qp[1][d], 0.0);
-                    qn[1][d] = (P1 - lo) - fmax(-qn[1][d], 0.0);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const double2 q = qs[(h * 3 + d) * TS];
+                        const double qpn = (hi - Pv[h][d]) - neg_part(q.x), qnn = (Pv[h][d] - lo) - neg_part(q.y);
+                        qs[(h * 3 + d) * TS] = make_double2(qpn, qnn);
+                        A0[h][d] = (hi - fabs(qpn)) + (lo + fabs(qnn));
+                    }
                 }
             }
         }
@@ -395,11 +503,13 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const double bl = right[h] ? own[d] : nb[d], br = right[h] ? nb[d] : own[d];
-                const double znew = fixed ? zt[h][d] : 0.5 * (bl + br);      // a5: Eq. 6b / 20b
-                dz[h][d] = znew - zt[h][d];
-                zt[h][d] = znew;
+                const double2 zu = zus[(h * 3 + d) * TS];
+                const double znew = fixed ? zu.x : 0.5 * (bl + br);          // a5: Eq. 6b / 20b
+                dz[h][d] = znew - zu.x;
                 const double res = own[d] - znew;
-                u[h][d] += res;                                              // a8: Eq. 6c / 20c (scaled dual, A5)
+                const double unew = zu.y + res;                              // a8: Eq. 6c / 20c (scaled dual, A5)
+                zus[(h * 3 + d) * TS] = make_double2(znew, unew);
+                gM[h][d] = (znew - unew) * invTk[h];                         // operand of the next sweep's a1
                 if (last_sweep) {
                     rp2 += res * res;
                     if (right[h] && !(sf & SEG_LAST)) { const double gp = own[d] - nb[d]; gap2 += gp * gp; }   // Eq. 21
@@ -414,8 +524,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 double x0 = 0, x1 = 0;
-                dmma884(x0, x1, dz[0][d] * invTk[0], ctab[(0) * 32]);
-                dmma884(x0, x1, dz[1][d] * invTk[1], ctab[(1) * 32]);
+                dmma884(x0, x1, dz[0][d] * invTk[0], ctab[0 * 32]);
+                dmma884(x0, x1, dz[1][d] * invTk[1], ctab[1 * 32]);
                 const double xr0 = rho_cur * x0, xr1 = rho_cur * x1;
                 rdn2 += xr0 * xr0 + xr1 * xr1;
                 rd2 += (xr0 * Tp0) * (xr0 * Tp0) + (xr1 * Tp1) * (xr1 * Tp1);
@@ -477,37 +587,34 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     else if (rd > p.mu * rp) rho_new = rho_cur / p.tau_decr;
                     if (rho_new != rho_cur) {
                         const double ratio = rho_cur / rho_new;
+                        // u, w, v = max(0,-q) are scaled duals: times rho_old/rho_new; then the operands that depend on them
+                        // (phi of this test sweep was written to global memory above and is read back: exact)
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
 #pragma unroll
                             for (int d = 0; d < 3; ++d) {
-                                u[h][d] *= ratio; wv[h][d] *= ratio; wa[h][d] *= ratio;
-                                if (qp[h][d] < 0) qp[h][d] *= ratio;
-                                if (qn[h][d] < 0) qn[h][d] *= ratio;
-                            }
-                            // operator refresh from the spectral form (as refresh_operator_kernel): my rows of rho Pm^, c0^
-                            double wd[MAXN];
-                            for (int i = 0; i < MAXN; ++i) {
-                                const double lam = i < p.q ? p.lam[i * p.nseg_pad + gseg] : 0.0;
-                                wd[i] = i < p.q ? p.W[i * stride + gt[h]] * (rho_new / (lam + rho_new)) : 0.0;
-                            }
-#pragma unroll
-                            double c0n[3];
-#pragma unroll
-                            for (int d = 0; d < 3; ++d) c0n[d] = jj[h] == 1 ? p.dp[d * p.nseg_pad + gseg] : 0.0;
-                            for (int b = 0; b < 8; b += 2) {
-                                double v2[2];
-                                for (int e = 0; e < 2; ++e) {
-                                    double v = 0.0;
-                                    if (b + e < N2) for (int i = 0; i < p.q; ++i) v += wd[i] * p.W[i * stride + gseg * LANES + b + e];
-                                    v2[e] = v;
-#pragma unroll
-                                    for (int d = 0; d < 3; ++d) c0n[d] -= v * p.g0[d * stride + gseg * LANES + b + e];
+                                const long long i = d * stride + gt[h];
+                                double2 zu = zus[(h * 3 + d) * TS];
+                                zu.y *= ratio;
+                                zus[(h * 3 + d) * TS] = zu;
+                                gM[h][d] = (zu.x - zu.y) * invTk[h];
+                                if (has_box) {
+                                    const double lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
+                                    double2 q = qs[(h * 3 + d) * TS];
+                                    if (q.x < 0) q.x *= ratio;
+                                    if (q.y < 0) q.y *= ratio;
+                                    qs[(h * 3 + d) * TS] = q;
+                                    A0[h][d] = (hi - fabs(q.x)) + (lo + fabs(q.y));
                                 }
-                                Pms[(h * 4 + (b >> 1)) * T] = make_double2(v2[0], v2[1]);
+                                if (CONS) {
+                                    double2 w2 = ws[(h * 3 + d) * TS];
+                                    w2.x *= ratio; w2.y *= ratio;
+                                    ws[(h * 3 + d) * TS] = w2;
+                                    if (has_vel) gv[h][d] = ((owned ? static_cast<const double*>(p.phv_out)[i] : 0.0) - w2.x) * invT;
+                                    if (has_acc) ga[h][d] = ((owned ? static_cast<const double*>(p.pha_out)[i] : 0.0) - w2.y) * invT2;
+                                }
                             }
-#pragma unroll
-                            for (int d = 0; d < 3; ++d) c0s[(h * 3 + d) * T] = c0n[d];
+                            refresh_operator_rows<N2, TS>(p, gseg, gt[h], jj[h], rho_new, Pms + h * 4 * TS, c0s + h * 3 * TS);
                         }
                         rho_cur = rho_new;
                     }
@@ -521,18 +628,22 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         o[3] = sqrt(tot_sh[0]); o[4] = sqrt(tot_sh[1]); o[5] = sqrt(tot_sh[2]); o[6] = sqrt(tot_sh[3]);
     }
 
-    // ---- write iterate k + k_sweeps back
+    // ---- write iterate k + k_sweeps back (phi went out with the last sweep)
     if (owned) {
 #pragma unroll
         for (int h = 0; h < 2; ++h)
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const long long i = d * stride + gt[h];
-                static_cast<double*>(p.zt_out)[i] = zt[h][d];
-                static_cast<double*>(p.u_out)[i] = u[h][d];
-                if (has_box) { static_cast<double*>(p.qp_out)[i] = qp[h][d]; static_cast<double*>(p.qn_out)[i] = qn[h][d]; }
-                if (has_vel) { static_cast<double*>(p.phv_out)[i] = phv[h][d]; static_cast<double*>(p.wv_out)[i] = wv[h][d]; }
-                if (has_acc) { static_cast<double*>(p.pha_out)[i] = pha[h][d]; static_cast<double*>(p.wa_out)[i] = wa[h][d]; }
+                const double2 zu = zus[(h * 3 + d) * TS];
+                static_cast<double*>(p.zt_out)[i] = zu.x;
+                static_cast<double*>(p.u_out)[i] = zu.y;
+                if (has_box) { const double2 q = qs[(h * 3 + d) * TS]; static_cast<double*>(p.qp_out)[i] = q.x; static_cast<double*>(p.qn_out)[i] = q.y; }
+                if (CONS) {
+                    const double2 w2 = ws[(h * 3 + d) * TS];
+                    if (has_vel) static_cast<double*>(p.wv_out)[i] = w2.x;
+                    if (has_acc) static_cast<double*>(p.wa_out)[i] = w2.y;
+                }
             }
     }
 }
@@ -578,8 +689,8 @@ cudaError_t sweep_kernel_limits_mma(int s, bool constrained, int threads, size_t
     return cudaErrorInvalidValue;
 }
 
-size_t sweep_smem_bytes_mma(bool constrained, int segs_per_cta) {
-    return smem_layout_mma(constrained, (segs_per_cta * 4 + 31) / 32 * 8).total;
+size_t sweep_smem_bytes_mma(bool constrained, int /*segs_per_cta*/) {
+    return smem_layout_mma(constrained, MAXT_MMA / 4).total;      // laid out for the largest CTA (see the kernel)
 }
 
 }  // namespace top
