@@ -607,7 +607,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     }
     for (const auto& w : h->waves) {
         int per_sm = 0;
-        cudaError_t e = h->mma ? sweep_kernel_limits_mma(s, h->constrained, w.threads, w.smem, &per_sm)
+        cudaError_t e = h->mma ? sweep_kernel_limits_mma(s, h->kflags, w.threads, w.smem, &per_sm)
                                : sweep_kernel_limits(h->dtype, s, h->constrained, h->lanes, w.threads, w.smem, &per_sm);
         if (e != cudaSuccess) CREATE_FAIL(cuda_fail(h, e, "occupancy query"));
         if (per_sm < 1) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "sweep kernel does not fit an SM"));

@@ -92,7 +92,7 @@ cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, i
 cudaError_t launch_sweeps_mma(const KParams& p, int s, bool constrained, int ctas, int threads, size_t smem, cudaStream_t st);
 size_t sweep_smem_bytes_mma(bool constrained, int segs_per_cta);
 int max_threads_mma();
-cudaError_t sweep_kernel_limits_mma(int s, bool constrained, int threads, size_t smem, int* max_ctas_per_sm);
+cudaError_t sweep_kernel_limits_mma(int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm);
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
 // rho Pm^ = W diag(rho/(lambda_i+rho)) W',  c0^ = c_chord - (rho Pm^) g0   (spectral form; top_api.cpp build_spectral)
 struct RefreshParams {

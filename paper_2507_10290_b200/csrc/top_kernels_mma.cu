@@ -13,9 +13,19 @@
 // results land in the lane that owns them: no shuffle reduce-scatter, no select instructions, no second all-gather.
 // The only intra-segment exchange left is the all-gather of R^ (8 rows x 3 dims through shared memory) in front of the
 // per-segment 8 x 8 operator apply a2 (Eq. 20a first bracket), which stays on DFMA: its matrix differs per segment.
-// Measured on B200: DMMA m8n8k4 runs at the DFMA FLOP rate (16 cycles per instruction and scheduler) but
-// with 26-cycle dependent latency and independent accumulators a single warp keeps the fp64 pipe busy, where the
-// shuffle / synthetic-division form was bound by instruction issue and dependent-chain latency.
+// Measured on B200: DMMA m8n8k4 runs at the DFMA FLOP rate on the SAME pipe (16 cycles per instruction
+// and scheduler, 26-cycle dependent latency, the issuing warp waits ~17 cycles after each), so the gain is not FLOPs
+// but everything around them: the shuffle / select / synthetic-division form was bound by instruction issue and
+// dependent-chain latency.
+//
+// Data flow of one lane (registers are short at 9 warps per SM: 168):
+//   registers   the a1 OPERANDS gM, A0, gv, ga (the A fragments of the first contraction), each produced where its
+//               inputs are updated (phase B, projections) so that a1 is 24 back-to-back MMAs with nothing in front
+//   shared      the variables behind them, as pairs read and written once per sweep where they are updated:
+//               (z~, u), the Moreau pair values (q+, q-), the ball variables (phi_v, phi_a) and (w_v, w_a);
+//               the per-segment operator rows; the all-gather buffer; the boundary-row exchange buffer
+// The constraint selection is a template parameter (the three combinations BASELINE.json's configs use, plus a
+// run-time-flag variant for the others): no branch inside the sweep body except the exchange.
 #include "top_device.cuh"
 
 namespace top {
@@ -51,11 +61,13 @@ __device__ __forceinline__ double ball_scale(const double (&y)[3], double bound)
     return n2 > bound * bound ? sc : 1.0;
 }
 
-// one instantiation: <= 288 threads (9 warps of 8 segments: 224 registers per thread)
+// one instantiation: <= 288 threads (9 warps of 8 segments; 3 warps on one scheduler: 168 registers per thread)
 constexpr int MAXT_MMA = 288;
+// constraint mask of an instantiation: KF_BOX | KF_VEL | KF_ACC, or CM_RUNTIME = read the flags at run time
+constexpr int CM_RUNTIME = 8;
 
 struct SmemLayoutMma {
-    size_t pm, c0, zu, qs, ws, ctab, lohi, xs, bs, zoff, total;
+    size_t pm, c0, zu, qs, ws, ph, ctab, lohi, xs, bs, zoff, total;
 };
 __host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc) {
     SmemLayoutMma L;
@@ -66,6 +78,7 @@ __host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_all
     L.zu = off;   off = align16(off + (size_t)6 * T * sizeof(double2));                // (z~, u) of the lane's two consensus rows, [h][d][thread]
     L.qs = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // Moreau pair values (q+, q-) of the lane's two samples
     L.ws = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // ball duals (w_v, w_a) of the lane's two samples
+    L.ph = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // ball variables (phi_v, phi_a)
     L.ctab = off; off = align16(off + (size_t)16 * 32 * sizeof(double));               // constant MMA operands, [16][lane of warp]
     L.lohi = off; off = align16(off + (size_t)(cons ? 6 : 0) * segs_alloc * sizeof(double));
     L.xs = off;   off = align16(off + (size_t)segs_alloc * XSTRIDE * sizeof(double));  // rhs rows, all-gather
@@ -101,10 +114,11 @@ __device__ __noinline__ void refresh_operator_rows(const KParams& p, long long g
     for (int d = 0; d < 3; ++d) c0_row[d * TS] = c0n[d];
 }
 
-template <int S, bool CONS, int MAXT, bool SOLVE>
+template <int S, int CM, int MAXT, bool SOLVE>
 __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams p) {
     constexpr int N2 = 2 * S;
     constexpr int LPS = 4;                         // lanes per segment
+    constexpr bool CONS = CM != 0;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int T = blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
@@ -114,24 +128,28 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     // per-thread base register plus an immediate (with run-time strides ptxas re-derived the offsets inside the loop).
     constexpr int TS = MAXT;                       // thread stride of the per-thread arrays
     constexpr int SA = MAXT / 4;                   // segment slots
+    constexpr int BPAR = (SA + 2) * 24;            // doubles per parity of the boundary-row buffer
     const int SEGS = p.segs_per_cta;
     const int cta = blockIdx.x, nctas = gridDim.x;
     const uint32_t flags = p.flags;
-    const bool has_box = CONS && (flags & KF_BOX), has_vel = CONS && (flags & KF_VEL), has_acc = CONS && (flags & KF_ACC);
+    const bool has_box = CM == CM_RUNTIME ? (flags & KF_BOX) != 0 : (CM & (int)KF_BOX) != 0;
+    const bool has_vel = CM == CM_RUNTIME ? (flags & KF_VEL) != 0 : (CM & (int)KF_VEL) != 0;
+    const bool has_acc = CM == CM_RUNTIME ? (flags & KF_ACC) != 0 : (CM & (int)KF_ACC) != 0;
     const bool pin_pos = flags & KF_PIN_POS;
     const bool nb_sync = flags & KF_NEIGHBOUR_SYNC;
 
     const SmemLayoutMma L = smem_layout_mma(CONS, SA);
     double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + tid;          // [(h*4 + b/2) * TS]
     double* c0s = reinterpret_cast<double*>(smem_raw + L.c0) + tid;            // [(h*3 + d) * TS]
-    double2* zus = reinterpret_cast<double2*>(smem_raw + L.zu) + tid;         // [(h*3 + d) * TS]: (z~, u); registers are short at 9 warps per SM
-    double2* qs = reinterpret_cast<double2*>(smem_raw + L.qs) + tid;          // [(h*3 + d) * TS]: (q+, q-)
-    double2* ws = reinterpret_cast<double2*>(smem_raw + L.ws) + tid;          // [(h*3 + d) * TS]: (w_v, w_a)
+    double2* zus = reinterpret_cast<double2*>(smem_raw + L.zu) + tid;          // [(h*3 + d) * TS]: (z~, u)
+    double2* qs = reinterpret_cast<double2*>(smem_raw + L.qs) + tid;           // [(h*3 + d) * TS]: (q+, q-)
+    double2* ws = reinterpret_cast<double2*>(smem_raw + L.ws) + tid;           // [(h*3 + d) * TS]: (w_v, w_a)
+    double2* phs = reinterpret_cast<double2*>(smem_raw + L.ph) + tid;          // [(h*3 + d) * TS]: (phi_v, phi_a)
     double* ctab = reinterpret_cast<double*>(smem_raw + L.ctab) + (tid & 31);  // [k * 32]: a1 k-step operands at k = 0..7, a3 operands at k = 8 + kstep*4 + block
-    double* lohi = reinterpret_cast<double*>(smem_raw + L.lohi);               // [6][SA]
+    double* lohi = reinterpret_cast<double*>(smem_raw + L.lohi) + sl;          // [6 * SA]
     double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE;
     double* Bs = reinterpret_cast<double*>(smem_raw + L.bs);                   // [2 parity][SA+2][8 rows][3]
-    double* zoffs = reinterpret_cast<double*>(smem_raw + L.zoff);              // [2 sides][3][SA]
+    double* zoffs = reinterpret_cast<double*>(smem_raw + L.zoff) + sl;         // [(side*3 + d) * SA]
 
     const long long cta_first = p.seg_begin + (long long)cta * SEGS;
     const long long remaining = p.seg_end - cta_first;
@@ -144,13 +162,14 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     const long long stride = p.stride;
 
     // the two items of this lane: sample / row index jj[h], global lane slot gt[h]
+    // (s = 4: item 0 is always a left consensus row, item 1 a right one; s = 3: decided per lane)
     int jj[2]; long long gt[2]; bool isrow[2], right[2]; int korder[2];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
         jj[h] = lane + 4 * h;
         gt[h] = gseg * LANES + jj[h];
-        isrow[h] = jj[h] < N2;
-        right[h] = jj[h] >= S;
+        isrow[h] = S == 4 ? true : jj[h] < N2;
+        right[h] = S == 4 ? h == 1 : jj[h] >= S;
         korder[h] = right[h] ? jj[h] - S : jj[h];
     }
 
@@ -199,22 +218,47 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     }
     const double invT = static_cast<const double*>(p.invT)[gseg], invT2 = static_cast<const double*>(p.invT)[p.nseg_pad + gseg];
     if (CONS) {
-        lohi[lane * SA + sl] = static_cast<const double*>(p.lohi)[lane * p.nseg_pad + gseg];
-        if (lane < 2) lohi[(lane + 4) * SA + sl] = static_cast<const double*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
+        lohi[lane * SA] = static_cast<const double*>(p.lohi)[lane * p.nseg_pad + gseg];
+        if (lane < 2) lohi[(lane + 4) * SA] = static_cast<const double*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
     }
     if (lane < 3) {        // frame shifts of the neighbours' position rows: left junction (row 0), right junction (row S)
-        zoffs[lane * SA + sl] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + 0];
-        zoffs[(3 + lane) * SA + sl] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + S];
+        zoffs[lane * SA] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + 0];
+        zoffs[(3 + lane) * SA] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + S];
     }
     const uint8_t sf = p.segflags[gseg];
     const bool open_l = (flags & KF_OPEN_LEFT) && gseg == p.seg_begin, open_r = (flags & KF_OPEN_RIGHT) && gseg == p.seg_end - 1;
-    // ---- state of iterate k.  Registers hold the a1 OPERANDS (the A fragments of the first contraction), each produced
-    // where its inputs are updated (phase B, projections) so that a1 itself is 24 back-to-back MMAs with no dependent
-    // arithmetic in front of them:
+
+    // ---- per-lane facts of the exchange, fixed for the launch
+    // boundary-row buffer (doubles, relative to the parity base): my rows, and where the neighbour segment's matching rows are
+    int own_off[2], nb_off[2];
+    bool fixed[2], zshift[2], gaprow[2];
+    // mailbox (bytes, relative to the parity base): where I publish, what I fetch.  A lane needs at most ONE of its two
+    // rows from another CTA (a CTA with a neighbour on both sides owns >= 4 segments, so its left-edge and right-edge
+    // segments differ): one prefetch buffer.
+    int pub_off[2];
+    bool pub[2];
+    bool need = false;
+    int need_h = 0, need_off = 0;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        own_off[h] = (sl + 1) * 24 + jj[h] * 3;
+        nb_off[h] = right[h] ? (sl + 2) * 24 + korder[h] * 3 : sl * 24 + (korder[h] + S) * 3;
+        fixed[h] = (right[h] ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder[h] == 0) ||
+                   (right[h] ? open_r : open_l);      // outer end of a halo: no neighbour in this launch
+        zshift[h] = isrow[h] && korder[h] == 0;       // position rows live in segment-local frames
+        gaprow[h] = isrow[h] && right[h] && !(sf & SEG_LAST);
+        const bool edge_l = active && isrow[h] && sl == 0 && !right[h] && cta > 0;
+        const bool edge_r = active && isrow[h] && sl == nact - 1 && right[h] && cta + 1 < nctas;
+        pub[h] = nctas > 1 && (edge_l || edge_r);
+        pub_off[h] = (cta * 24 + (edge_r ? 12 : 0) + korder[h] * 3) * 16;
+        if (edge_l || edge_r) {
+            need = true; need_h = h;
+            need_off = edge_l ? ((cta - 1) * 24 + 12 + korder[h] * 3) * 16 : ((cta + 1) * 24 + korder[h] * 3) * 16;
+        }
+    }
+
+    // ---- state of iterate k.  Registers hold the a1 OPERANDS:
     //   gM = (z~ - u)/T^k      A0 = (hi - s+ - v+) + (lo + s- + v-)      gv = (phi_v - w_v)/T      ga = (phi_a - w_a)/T^2
-    // The variables behind them live in shared memory as pairs, read and written once per sweep where they are updated:
-    // (z~, u), the Moreau pair values (q+, q-), and the ball duals (w_v, w_a).  phi is not kept at all: it is written to
-    // global memory on the sweeps whose iterate is observable (the last of the launch, and every test sweep of a solve).
     double gM[2][3], A0[2][3], gv[2][3], ga[2][3];
 #pragma unroll
     for (int h = 0; h < 2; ++h)
@@ -225,16 +269,16 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             zus[(h * 3 + d) * TS] = make_double2(z0, u0);
             gM[h][d] = (z0 - u0) * invTk[h];
             A0[h][d] = gv[h][d] = ga[h][d] = 0.0;
-            double w_v = 0.0, w_a = 0.0;
+            double w_v = 0.0, w_a = 0.0, ph_v = 0.0, ph_a = 0.0;
             if (has_box) {
                 const double lo = static_cast<const double*>(p.lohi)[d * p.nseg_pad + gseg], hi = static_cast<const double*>(p.lohi)[(3 + d) * p.nseg_pad + gseg];
                 const double a = static_cast<const double*>(p.qp)[i], b = static_cast<const double*>(p.qn)[i];
                 qs[(h * 3 + d) * TS] = make_double2(a, b);
                 A0[h][d] = (hi - fabs(a)) + (lo + fabs(b));
             }
-            if (has_vel) { w_v = static_cast<const double*>(p.wv)[i]; gv[h][d] = (static_cast<const double*>(p.phv)[i] - w_v) * invT; }
-            if (has_acc) { w_a = static_cast<const double*>(p.wa)[i]; ga[h][d] = (static_cast<const double*>(p.pha)[i] - w_a) * invT2; }
-            if (CONS) ws[(h * 3 + d) * TS] = make_double2(w_v, w_a);
+            if (has_vel) { w_v = static_cast<const double*>(p.wv)[i]; ph_v = static_cast<const double*>(p.phv)[i]; gv[h][d] = (ph_v - w_v) * invT; }
+            if (has_acc) { w_a = static_cast<const double*>(p.wa)[i]; ph_a = static_cast<const double*>(p.pha)[i]; ga[h][d] = (ph_a - w_a) * invT2; }
+            if (CONS) { ws[(h * 3 + d) * TS] = make_double2(w_v, w_a); phs[(h * 3 + d) * TS] = make_double2(ph_v, ph_a); }
         }
 
     const double vmax = p.vmax, amax = p.amax;
@@ -259,11 +303,22 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         const unsigned seq = p.seq_base + (unsigned)it + 1u;
         const int par = (int)(seq & 1u);
         const bool final_sweep = (it == p.k_sweeps - 1);
-        // sweeps on which residuals (and the coefficients, and phi) are materialised: the last one, and every test sweep
+        // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
         const bool last_sweep = final_sweep || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
-        double* const Bcur = Bs + (size_t)par * (SA + 2) * 24;
+        double* const Bcur = Bs + par * BPAR;
+        unsigned char* const mpar = mbox + par * mbox_par_stride;
 
         // ================= phase A: segment local =================
+        // operator rows and c0 of this lane: issued first, they arrive while the MMAs of a1 run
+        double2 pm[2][4];
+        double cacc[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+            for (int b = 0; b < 4; ++b) pm[h][b] = Pms[(h * 4 + b) * TS];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) cacc[h][d] = c0s[(h * 3 + d) * TS];
+        }
         // a1: right-hand side of Eq. 20a (second bracket; rho is folded into the operator, A3):
         // R^ = M^'[(z~ - u)/T^k] + E0'[(hi - s+ - v+) + (lo + s- + v-)] + E1'[(phi_v - w_v)/T] + E2'[(phi_a - w_a)/T^2].
         // Three accumulator tiles (one per dim), up to 8 k-steps each; the accumulator of lane t holds rows 2t, 2t+1.
@@ -273,57 +328,46 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             for (int h = 0; h < 2; ++h)
 #pragma unroll
                 for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gM[h][d], ctab[h * 32]);
-            if (CONS) {
-                if (has_box) {      // Ao'(b - s - v), Ao = [E0; -E0], b = [hi; -lo];  s + v = |q| (Moreau pair)
+            if (has_box) {      // Ao'(b - s - v), Ao = [E0; -E0], b = [hi; -lo];  s + v = |q| (Moreau pair)
 #pragma unroll
-                    for (int h = 0; h < 2; ++h)
+                for (int h = 0; h < 2; ++h)
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], A0[h][d], ctab[(2 + h) * 32]);
-                }
-                if (has_vel) {
+                    for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], A0[h][d], ctab[(2 + h) * 32]);
+            }
+            if (has_vel) {
 #pragma unroll
-                    for (int h = 0; h < 2; ++h)
+                for (int h = 0; h < 2; ++h)
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gv[h][d], ctab[(4 + h) * 32]);
-                }
-                if (has_acc) {
+                    for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gv[h][d], ctab[(4 + h) * 32]);
+            }
+            if (has_acc) {
 #pragma unroll
-                    for (int h = 0; h < 2; ++h)
+                for (int h = 0; h < 2; ++h)
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], ga[h][d], ctab[(6 + h) * 32]);
-                }
+                    for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], ga[h][d], ctab[(6 + h) * 32]);
             }
 #pragma unroll
             for (int d = 0; d < 3; ++d) *reinterpret_cast<double2*>(Xs + d * 8 + 2 * lane) = make_double2(acc[d][0], acc[d][1]);
         }
         __syncwarp();
         // a2: x-update  c^ = (rho Pm^) R^ + c0^   (Eq. 20a first bracket, precomputed per segment): rows lane, lane+4
-        double c[2][3];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            double pm[8];
+        for (int d = 0; d < 3; ++d) {
 #pragma unroll
-            for (int b = 0; b < N2; b += 2) {
-                const double2 t2 = Pms[(h * 4 + (b >> 1)) * TS];
-                pm[b] = t2.x; pm[b + 1] = t2.y;
-            }
+            for (int b = 0; b < N2 / 2; ++b) {
+                const double2 x2 = *reinterpret_cast<const double2*>(Xs + d * 8 + 2 * b);
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                double v = c0s[(h * 3 + d) * TS];
-#pragma unroll
-                for (int b = 0; b < N2; b += 2) {
-                    const double2 t2 = *reinterpret_cast<const double2*>(Xs + d * 8 + b);
-                    v += pm[b] * t2.x;
-                    v += pm[b + 1] * t2.y;
+                for (int h = 0; h < 2; ++h) {
+                    cacc[h][d] += pm[h][b].x * x2.x;
+                    cacc[h][d] += pm[h][b].y * x2.y;
                 }
-                c[h][d] = v;
             }
         }
         if (last_sweep && owned) {      // (every test sweep as well: the solve may stop there)
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
-                for (int d = 0; d < 3; ++d) static_cast<double*>(p.chat)[d * stride + gt[h]] = c[h][d];
+                for (int d = 0; d < 3; ++d) static_cast<double*>(p.chat)[d * stride + gt[h]] = cacc[h][d];
         }
         // a3: evaluate the new polynomial: consensus rows of B = M c (Eq. 20b), and the lane's two samples of E0 c, E1 c,
         // E2 c (Eq. 20d-g).  A operand = the lane's own coefficient rows; accumulator columns = the lane's own items.
@@ -332,107 +376,94 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 double e0 = 0, e1 = 0;
-                dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 0) * 32]);
-                dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 0) * 32]);
+                dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 0) * 32]);
+                dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 0) * 32]);
                 Bnd[0][d] = e0 * invTk[0]; Bnd[1][d] = e1 * invTk[1];
             }
             // publish: shared memory for the neighbours in this CTA (and for this lane's own phase B), mailbox for the
             // neighbouring CTAs
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                if (!isrow[h]) continue;
+                if (isrow[h]) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) Bcur[(sl + 1) * 24 + jj[h] * 3 + d] = Bnd[h][d];
-                if (nctas > 1 && active) {
-                    unsigned char* e = mbox + par * mbox_par_stride + (size_t)cta * 24 * 16;
-                    if (sl == 0 && !right[h] && cta > 0) {
+                    for (int d = 0; d < 3; ++d) Bcur[own_off[h] + d] = Bnd[h][d];
+                }
+                if (pub[h]) {
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) ll_store(e + (0 * 12 + korder[h] * 3 + d) * 16, Bnd[h][d], seq);
-                    }
-                    if (sl == nact - 1 && right[h] && cta + 1 < nctas) {
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) ll_store(e + (1 * 12 + korder[h] * 3 + d) * 16, Bnd[h][d], seq);
-                    }
+                    for (int d = 0; d < 3; ++d) ll_store(mpar + pub_off[h] + d * 16, Bnd[h][d], seq);
                 }
             }
         }
-        // A lane needs at most ONE of its two rows from another CTA (a CTA with a neighbour on both sides owns >= 4
-        // segments, so its left-edge and right-edge segments differ): one prefetch buffer.  The loads fly during the
-        // projections.
-        bool need = false;
-        int need_h = 0;
-        const unsigned char* rslot = mbox;
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const bool need_l = active && isrow[h] && sl == 0 && !right[h] && cta > 0;
-            const bool need_r = active && isrow[h] && sl == nact - 1 && right[h] && cta + 1 < nctas;
-            if (need_l || need_r) {
-                need = true; need_h = h;
-                rslot = mbox + par * mbox_par_stride +
-                    (need_l ? ((size_t)(cta - 1) * 24 + 12 + korder[h] * 3) * 16 : ((size_t)(cta + 1) * 24 + korder[h] * 3) * 16);
-            }
-        }
+        // prefetch the rows of the neighbouring CTA: the loads fly during the projections
         LLRaw rr[3];
         if (need) {
 #pragma unroll
-            for (int d = 0; d < 3; ++d) ll_issue(rslot + d * 16, rr[d]);
+            for (int d = 0; d < 3; ++d) ll_issue(mpar + need_off + d * 16, rr[d]);
         }
         if (CONS) {
-            // the three sample blocks of the evaluation back to back (the fp64 pipe stays busy), then the projections of
-            // all blocks side by side: independent dependency chains, no branch between them
+            // the three sample blocks of the evaluation back to back, then the projections of all blocks side by side:
+            // independent dependency chains, no branch between them
             double Pv[2][3], Vv[2][3], Av[2][3];
             if (has_vel) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 2) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 2) * 32]); Vv[0][d] = e0; Vv[1][d] = e1; }
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 2) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 2) * 32]); Vv[0][d] = e0; Vv[1][d] = e1; }
             }
             if (has_acc) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = e0; Av[1][d] = e1; }
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = e0; Av[1][d] = e1; }
             }
             if (has_box) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, c[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(e0, e1, c[1][d], ctab[(8 + 1 * 4 + 1) * 32]); Pv[0][d] = e0; Pv[1][d] = e1; }
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 1) * 32]); Pv[0][d] = e0; Pv[1][d] = e1; }
             }
+            double2 w2[2][3], q2[2][3];
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    if (has_vel || has_acc) w2[h][d] = ws[(h * 3 + d) * TS];
+                    if (has_box) q2[h][d] = qs[(h * 3 + d) * TS];
+                }
+            // a4: Eq. 20f, 20g;  y = A c + w,  phi = proj(y),  w <- y - phi;  next operand (phi - w)/T
+            double2 ph2[2][3];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                double2 w2[3];
+                if (has_vel) {
+                    double y[3];
 #pragma unroll
-                for (int d = 0; d < 3; ++d) w2[d] = ws[(h * 3 + d) * TS];
-                if (has_vel) {      // a4: Eq. 20f, 20g;  y = A c + w,  phi = proj(y),  w <- y - phi;  next operand (phi - w)/T
-                    double y[3], phi[3];
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) y[d] = Vv[h][d] * invT + w2[d].x;
+                    for (int d = 0; d < 3; ++d) y[d] = Vv[h][d] * invT + w2[h][d].x;
                     const double scale = ball_scale(y, vmax);
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) { phi[d] = scale * y[d]; w2[d].x = y[d] - phi[d]; gv[h][d] = (phi[d] - w2[d].x) * invT; }
-                    if (last_sweep && owned) {
+                    for (int d = 0; d < 3; ++d) { const double ph = scale * y[d]; ph2[h][d].x = ph; w2[h][d].x = y[d] - ph; gv[h][d] = (ph - w2[h][d].x) * invT; }
+                } else {
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) static_cast<double*>(p.phv_out)[d * stride + gt[h]] = phi[d];
-                    }
+                    for (int d = 0; d < 3; ++d) ph2[h][d].x = 0.0;
                 }
                 if (has_acc) {
-                    double y[3], phi[3];
+                    double y[3];
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) y[d] = Av[h][d] * invT2 + w2[d].y;
+                    for (int d = 0; d < 3; ++d) y[d] = Av[h][d] * invT2 + w2[h][d].y;
                     const double scale = ball_scale(y, amax);
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) { phi[d] = scale * y[d]; w2[d].y = y[d] - phi[d]; ga[h][d] = (phi[d] - w2[d].y) * invT2; }
-                    if (last_sweep && owned) {
+                    for (int d = 0; d < 3; ++d) { const double ph = scale * y[d]; ph2[h][d].y = ph; w2[h][d].y = y[d] - ph; ga[h][d] = (ph - w2[h][d].y) * invT2; }
+                } else {
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) static_cast<double*>(p.pha_out)[d * stride + gt[h]] = phi[d];
-                    }
+                    for (int d = 0; d < 3; ++d) ph2[h][d].y = 0.0;
                 }
+            }
+            if (has_vel || has_acc) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) ws[(h * 3 + d) * TS] = w2[d];
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) { ws[(h * 3 + d) * TS] = w2[h][d]; phs[(h * 3 + d) * TS] = ph2[h][d]; }
             }
             if (has_box) {      // a7 + a8: Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q);  next operand
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
-                    const double lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
+                    const double lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        const double2 q = qs[(h * 3 + d) * TS];
-                        const double qpn = (hi - Pv[h][d]) - neg_part(q.x), qnn = (Pv[h][d] - lo) - neg_part(q.y);
+                        const double qpn = (hi - Pv[h][d]) - neg_part(q2[h][d].x), qnn = (Pv[h][d] - lo) - neg_part(q2[h][d].y);
                         qs[(h * 3 + d) * TS] = make_double2(qpn, qnn);
                         A0[h][d] = (hi - fabs(qpn)) + (lo + fabs(qnn));
                     }
@@ -451,7 +482,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 do {
                     if (!okk) {
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) ll_issue(rslot + d * 16, rr[d]);
+                        for (int d = 0; d < 3; ++d) ll_issue(mpar + need_off + d * 16, rr[d]);
                         okk = ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq);
                     }
                     bool bail = false;
@@ -476,46 +507,45 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         }
 
         // ================= phase B: consensus, dual, residuals =================
+        // everything is loaded first (own rows, neighbour rows, frame shifts, (z~, u)), then updated, then stored
+        double own[2][3], nb[2][3];
+        double2 zu[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                own[h][d] = Bcur[own_off[h] + d];
+                nb[h][d] = Bcur[nb_off[h] + d];
+                zu[h][d] = zus[(h * 3 + d) * TS];
+            }
+        if (need) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { const double v = ll_value(rr[d]); if (need_h == 0) nb[0][d] = v; else nb[1][d] = v; }
+        }
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+            if (zshift[h]) {
+#pragma unroll
+                for (int d = 0; d < 3; ++d) nb[h][d] += zoffs[((right[h] ? 3 : 0) + d) * SA];
+            }
         double rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
         double dz[2][3];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-#pragma unroll
-            for (int d = 0; d < 3; ++d) dz[h][d] = 0.0;
-            if (!isrow[h]) continue;
-            double nb[3], own[3];
-#pragma unroll
-            for (int d = 0; d < 3; ++d) own[d] = Bcur[(sl + 1) * 24 + jj[h] * 3 + d];
-            if (need && need_h == h) {
-#pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] = ll_value(rr[d]);
-            } else {
-                const double* e = right[h] ? Bcur + (sl + 2) * 24 + korder[h] * 3 : Bcur + sl * 24 + (korder[h] + S) * 3;
-#pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] = e[d];
-            }
-            if (korder[h] == 0) {       // position rows live in segment-local frames: shift the neighbour's into mine
-#pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] += zoffs[((right[h] ? 3 : 0) + d) * SA + sl];
-            }
-            const bool fixed = (right[h] ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder[h] == 0) ||
-                               (right[h] ? open_r : open_l);      // outer end of a halo: no neighbour in this launch
+        for (int h = 0; h < 2; ++h)
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                const double bl = right[h] ? own[d] : nb[d], br = right[h] ? nb[d] : own[d];
-                const double2 zu = zus[(h * 3 + d) * TS];
-                const double znew = fixed ? zu.x : 0.5 * (bl + br);          // a5: Eq. 6b / 20b
-                dz[h][d] = znew - zu.x;
-                const double res = own[d] - znew;
-                const double unew = zu.y + res;                              // a8: Eq. 6c / 20c (scaled dual, A5)
+                const double avg = 0.5 * (own[h][d] + nb[h][d]);
+                const double znew = (fixed[h] || !isrow[h]) ? zu[h][d].x : avg;    // a5: Eq. 6b / 20b
+                dz[h][d] = znew - zu[h][d].x;
+                const double res = isrow[h] ? own[h][d] - znew : 0.0;
+                const double unew = zu[h][d].y + res;                               // a8: Eq. 6c / 20c (scaled dual, A5)
                 zus[(h * 3 + d) * TS] = make_double2(znew, unew);
-                gM[h][d] = (znew - unew) * invTk[h];                         // operand of the next sweep's a1
+                gM[h][d] = (znew - unew) * invTk[h];                                // operand of the next sweep's a1
                 if (last_sweep) {
                     rp2 += res * res;
-                    if (right[h] && !(sf & SEG_LAST)) { const double gp = own[d] - nb[d]; gap2 += gp * gp; }   // Eq. 21
+                    if (gaprow[h]) { const double gp = own[h][d] - nb[h][d]; gap2 += gp * gp; }   // Eq. 21
                 }
             }
-        }
         if (last_sweep) {
             // a6: dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8):
             // the consensus block of the a1 contraction applied to dz; lane t ends with coefficient rows 2t, 2t+1
@@ -588,30 +618,29 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     if (rho_new != rho_cur) {
                         const double ratio = rho_cur / rho_new;
                         // u, w, v = max(0,-q) are scaled duals: times rho_old/rho_new; then the operands that depend on them
-                        // (phi of this test sweep was written to global memory above and is read back: exact)
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
 #pragma unroll
                             for (int d = 0; d < 3; ++d) {
-                                const long long i = d * stride + gt[h];
-                                double2 zu = zus[(h * 3 + d) * TS];
-                                zu.y *= ratio;
-                                zus[(h * 3 + d) * TS] = zu;
-                                gM[h][d] = (zu.x - zu.y) * invTk[h];
+                                double2 zz = zus[(h * 3 + d) * TS];
+                                zz.y *= ratio;
+                                zus[(h * 3 + d) * TS] = zz;
+                                gM[h][d] = (zz.x - zz.y) * invTk[h];
                                 if (has_box) {
-                                    const double lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
+                                    const double lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
                                     double2 q = qs[(h * 3 + d) * TS];
                                     if (q.x < 0) q.x *= ratio;
                                     if (q.y < 0) q.y *= ratio;
                                     qs[(h * 3 + d) * TS] = q;
                                     A0[h][d] = (hi - fabs(q.x)) + (lo + fabs(q.y));
                                 }
-                                if (CONS) {
+                                if (has_vel || has_acc) {
                                     double2 w2 = ws[(h * 3 + d) * TS];
+                                    const double2 ph = phs[(h * 3 + d) * TS];
                                     w2.x *= ratio; w2.y *= ratio;
                                     ws[(h * 3 + d) * TS] = w2;
-                                    if (has_vel) gv[h][d] = ((owned ? static_cast<const double*>(p.phv_out)[i] : 0.0) - w2.x) * invT;
-                                    if (has_acc) ga[h][d] = ((owned ? static_cast<const double*>(p.pha_out)[i] : 0.0) - w2.y) * invT2;
+                                    if (has_vel) gv[h][d] = (ph.x - w2.x) * invT;
+                                    if (has_acc) ga[h][d] = (ph.y - w2.y) * invT2;
                                 }
                             }
                             refresh_operator_rows<N2, TS>(p, gseg, gt[h], jj[h], rho_new, Pms + h * 4 * TS, c0s + h * 3 * TS);
@@ -628,29 +657,29 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         o[3] = sqrt(tot_sh[0]); o[4] = sqrt(tot_sh[1]); o[5] = sqrt(tot_sh[2]); o[6] = sqrt(tot_sh[3]);
     }
 
-    // ---- write iterate k + k_sweeps back (phi went out with the last sweep)
+    // ---- write iterate k + k_sweeps back
     if (owned) {
 #pragma unroll
         for (int h = 0; h < 2; ++h)
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const long long i = d * stride + gt[h];
-                const double2 zu = zus[(h * 3 + d) * TS];
-                static_cast<double*>(p.zt_out)[i] = zu.x;
-                static_cast<double*>(p.u_out)[i] = zu.y;
+                const double2 zz = zus[(h * 3 + d) * TS];
+                static_cast<double*>(p.zt_out)[i] = zz.x;
+                static_cast<double*>(p.u_out)[i] = zz.y;
                 if (has_box) { const double2 q = qs[(h * 3 + d) * TS]; static_cast<double*>(p.qp_out)[i] = q.x; static_cast<double*>(p.qn_out)[i] = q.y; }
-                if (CONS) {
-                    const double2 w2 = ws[(h * 3 + d) * TS];
-                    if (has_vel) static_cast<double*>(p.wv_out)[i] = w2.x;
-                    if (has_acc) static_cast<double*>(p.wa_out)[i] = w2.y;
+                if (has_vel || has_acc) {
+                    const double2 w2 = ws[(h * 3 + d) * TS], ph = phs[(h * 3 + d) * TS];
+                    if (has_vel) { static_cast<double*>(p.wv_out)[i] = w2.x; static_cast<double*>(p.phv_out)[i] = ph.x; }
+                    if (has_acc) { static_cast<double*>(p.wa_out)[i] = w2.y; static_cast<double*>(p.pha_out)[i] = ph.y; }
                 }
             }
     }
 }
 
-template <int S, bool CONS, int MAXT>
+template <int S, int CM, int MAXT>
 cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
-    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<S, CONS, MAXT, true> : cadmm_sweeps_mma_kernel<S, CONS, MAXT, false>;
+    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<S, CM, MAXT, true> : cadmm_sweeps_mma_kernel<S, CM, MAXT, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     KParams pc = p;
@@ -659,30 +688,38 @@ cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cud
     return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
 }
 
-template <int S, bool CONS, int MAXT>
+template <int S, int CM, int MAXT>
 cudaError_t limits_mma(int threads, size_t smem, int* per_sm) {
-    auto kern = cadmm_sweeps_mma_kernel<S, CONS, MAXT, true>;     // the larger of the two instantiations
+    auto kern = cadmm_sweeps_mma_kernel<S, CM, MAXT, true>;     // the larger of the two instantiations
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
 }
 
+// constraint selection -> instantiation: none, box + velocity, box + velocity + acceleration; anything else at run time
+int mma_mask(uint32_t kflags) {
+    const int m = (int)(kflags & (KF_BOX | KF_VEL | KF_ACC));
+    return (m == 0 || m == 3 || m == 7) ? m : CM_RUNTIME;
+}
+
 }  // namespace
 
-#define TOP_DISPATCH_MMA(CALL)                                                         \
-    if (s == 3) { if (constrained) { CALL(3, true) } else { CALL(3, false) } }         \
-    else        { if (constrained) { CALL(4, true) } else { CALL(4, false) } }
+#define TOP_DISPATCH_MMA(CALL)                                                                              \
+    const int cm = mma_mask(kflags);                                                                        \
+    if (s == 3) { if (cm == 0) { CALL(3, 0) } else if (cm == 3) { CALL(3, 3) } else if (cm == 7) { CALL(3, 7) } else { CALL(3, CM_RUNTIME) } } \
+    else        { if (cm == 0) { CALL(4, 0) } else if (cm == 3) { CALL(4, 3) } else if (cm == 7) { CALL(4, 7) } else { CALL(4, CM_RUNTIME) } }
 
 int max_threads_mma() { return MAXT_MMA; }
 
-cudaError_t launch_sweeps_mma(const KParams& p, int s, bool constrained, int ctas, int threads, size_t smem, cudaStream_t st) {
+cudaError_t launch_sweeps_mma(const KParams& p, int s, bool /*constrained*/, int ctas, int threads, size_t smem, cudaStream_t st) {
+    const uint32_t kflags = p.flags;
 #define CALL(S_, C_) return launch_mma<S_, C_, MAXT_MMA>(p, ctas, threads, smem, st);
     TOP_DISPATCH_MMA(CALL)
 #undef CALL
     return cudaErrorInvalidValue;
 }
 
-cudaError_t sweep_kernel_limits_mma(int s, bool constrained, int threads, size_t smem, int* max_ctas_per_sm) {
+cudaError_t sweep_kernel_limits_mma(int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm) {
 #define CALL(S_, C_) return limits_mma<S_, C_, MAXT_MMA>(threads, smem, max_ctas_per_sm);
     TOP_DISPATCH_MMA(CALL)
 #undef CALL
