@@ -557,11 +557,15 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     int coop = 0;
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
     if (!coop) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "device lacks cooperative launch"));
-    // 8 lanes per segment unless told otherwise; 4 lanes (twice the registers per thread, two samples per lane) win
-    // for fp32 once every SM is full of segments (measured on config 5: 4.1e9 vs 3.3e9 segment-iterations/s), and
-    // lose for fp64 (register spills) and for short chains (longer serial path per warp)
+    // fp32: 8 lanes per segment unless told otherwise; 4 lanes (twice the registers per thread, two samples per lane) win
+    // once every SM is full of segments (measured on config 5: 4.1e9 vs 3.3e9 segment-iterations/s)
     h->lanes = o.lanes_per_segment ? o.lanes_per_segment : 8;
     if (!o.lanes_per_segment && dtype == TOP_F32 && nseg >= (long long)h->num_sms * 96) h->lanes = 4;
+    // fp64: the 4-lane kernel runs its constant-matrix contractions on the tensor cores (top_kernels_mma.cu); it wins
+    // whenever there are inequality constraints (config 2: 1.55 vs 1.74 us per sweep, config 4: 3.0 vs 4.6) and for
+    // unconstrained chains once an SM holds more than a few warps (N = 10^4: 1.6 vs 2.1-2.3); short unconstrained chains
+    // (configs 1, 3) stay on the 8-lane kernel (0.64 vs 0.85, 1.42 vs 1.57)
+    if (!o.lanes_per_segment && dtype == TOP_F64 && ((has_box || has_vel || has_acc) || nseg >= (long long)h->num_sms * 32)) h->lanes = 4;
     h->mma = dtype == TOP_F64 && h->lanes == 4 && !(o.flags & TOP_KERNEL_NO_MMA);
     const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192);
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
