@@ -44,7 +44,9 @@
  * too (used by a test that bounds the fp64 oracle's own rounding error).
  *
  * Parity pins: tests/test_oracle_pins.py (closed forms, dense KKT, banded solve, SLSQP,
- * KKT certificate, per-iterate invariants).  Finite-iteration iterates themselves depend on
+ * KKT certificate, per-iterate invariants); tests/test_oracle_residual_pins.py (r_p, r_d, r_d_norm,
+ * r_p_gap recomputed from the iterates with numpy's polynomial calculus, Eq. 21-22, and shown to
+ * catch a dropped rho / M for M' / a wrong power of T).  Finite-iteration iterates themselves depend on
  * readings A2/A9: PARITY UNPINNED for those (GPU-vs-oracle only), as DESIGN.md states.
  */
 #include <math.h>
