@@ -7,7 +7,7 @@ import pytest
 from paper_2507_10290_b200 import build as top_build
 from paper_2507_10290_b200 import top
 from paper_2507_10290_b200 import workloads as W
-from tests.parity_util import field_errors, make_oracle
+from tests.parity_util import field_errors, make_oracle, sampled_positions
 
 pytestmark = pytest.mark.gpu
 
@@ -40,6 +40,14 @@ def test_random_option_sweep(seed):
             for o in oracles:
                 o.sweep(k, 1)
             for name, v in field_errors(sol, oracles, w).items():
-                tol = 1e-6 if name.startswith("res_") else 1e-9
+                tol = 1e-6 if name.startswith("resself_") else 1e-9
                 assert v < tol, (case, name, v, N, s, acc, batch, dims, cons, w.rho, mode, lanes, sync, segs, ks)
         sol.close()
+        if case % 4 == 0 and w.samples:      # the fp32 (mixed) variant on the same case: sampled positions, 1e-3 m
+            sol = top.from_workload(w, mode=mode, lanes=lanes, sync=sync, segs_per_cta=segs, dtype="f32")
+            sol.iterate(sum(ks))
+            for b, o in enumerate(oracles):
+                T = w.durations[b]
+                d = np.abs(sampled_positions(sol.coeffs()[b].astype(np.float64), T) - sampled_positions(o.get("coeffs"), T)).max()
+                assert d < 1e-3, (case, "fp32", d, N, s, acc, batch, dims, cons, w.rho, mode, lanes, sync, segs, ks)
+            sol.close()

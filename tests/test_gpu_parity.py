@@ -13,7 +13,8 @@ from tests.parity_util import field_errors, make_oracle, sampled_positions, scal
 pytestmark = pytest.mark.gpu
 
 TOL_ITER = 1e-9      # north_star: "GPU fp64 must match the oracle iterate-by-iterate to 1e-9 relative"
-TOL_RES = 1e-6       # residual norms: sums of squares of differences near the rounding floor are compared looser
+TOL_RES = 1e-9       # residual norms: r_p against itself, r_d against its natural scale (parity_util.field_errors)
+TOL_RES_SELF = 1e-6  # r_d against itself (a norm of differences of consecutive iterates: DESIGN.md "Residual parity")
 
 
 @pytest.fixture(scope="module", autouse=True)
@@ -23,7 +24,7 @@ def built():
 
 def check_fields(errs, where):
     for k, v in errs.items():
-        tol = TOL_RES if k.startswith("res_") else TOL_ITER
+        tol = TOL_RES_SELF if k.startswith("resself_") else (TOL_RES if k.startswith("res_") else TOL_ITER)
         assert v < tol, (where, k, v, errs)
 
 
