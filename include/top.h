@@ -91,7 +91,7 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
  * velocity and acceleration (quadratic sets, Eq. 11-14), all enforced at `samples` interior sample times
  * t_ij = T_i*j/(samples+1), j=1..samples (reading A10). */
 typedef struct {
-    int32_t samples;        /* Ms: 0 => no inequality constraints; otherwise must be 8 in this build */
+    int32_t samples;        /* Ms: 0 => no inequality constraints; otherwise 8 in this build (else TOP_E_UNSUPPORTED) */
     const double* box_lo;   /* host [batch][N][dims] or NULL => no box */
     const double* box_hi;   /* host [batch][N][dims]; lo < hi elementwise */
     double vmax;            /* > 0: ||sigma'(t_ij)||_2  <= vmax ; <= 0: off */
@@ -115,8 +115,9 @@ typedef struct {
 /*
  * top_create -- Init of Alg. 1 (PAPER.md:L270 line 1, L301): validates, precomputes per segment (host,
  * extended precision) the x-update operator of Eq. 20a from T_i, rho and the enabled constraint sets,
- * uploads it in segment-major SoA form, and sets iterate 0 (reading A9: chord at constant speed, z0 from
- * the chord, duals 0, slacks/phi = projections of the chord samples).
+ * uploads it (one device allocation, one host-to-device copy of the operator rows and of the caller's arrays as they
+ * are), and an init kernel derives every per-lane constant and iterate 0 (reading A9: chord at constant speed, z0 from
+ * the chord, duals 0, slacks/phi = projections of the chord samples).  The device work is asynchronous.
  *   batch        number of independent trajectories (>= 1), each with N segments
  *   N            segments per trajectory (>= 1);  s in {3,4};  dims in {1,2,3}
  *   waypoints    host [batch][N+1][dims] metres       (the path P of Alg. 1)
@@ -126,8 +127,9 @@ typedef struct {
  *   cons         NULL = unconstrained
  *   rho          > 0, penalty of Eq. 5; one rho for every penalty (A18)
  *   opt          NULL = defaults
- * Errors: TOP_E_INVALID (sizes, non-finite input, T<=0, lo>=hi, rho<=0, samples not in {0,8}),
- * TOP_E_NOMEM, TOP_E_CUDA, TOP_E_UNSUPPORTED.  A trajectory longer than the on-chip capacity of the persistent
+ * Errors: TOP_E_INVALID (sizes, non-finite input, T<=0, lo>=hi, rho<=0, samples < 0), TOP_E_UNSUPPORTED (samples other
+ * than 0 or 8: the paper's M is a parameter; this build evaluates at 8; more than 2^28 segments),
+ * TOP_E_NOMEM, TOP_E_CUDA.  A trajectory longer than the on-chip capacity of the persistent
  * kernel (top_capacity) is streamed in pieces with halo segments (temporal blocking: same results, state
  * round-trips through device memory every 64 sweeps).  On error *out is NULL; top_last_error(NULL) has the message.
  */
@@ -135,6 +137,18 @@ TOP_API top_status top_create(top_solver** out, int32_t batch, int32_t N, int32_
                       const double* waypoints, const double* durations,
                       const double* start_derivs, const double* end_derivs,
                       const top_constraints* cons, double rho, const top_options* opt);
+
+/*
+ * top_reset -- a NEW PROBLEM OF THE SAME SHAPE on an existing handle: Init of Alg. 1 again (PAPER.md:L270 line 1), as a
+ * re-planning loop calls it.  batch, N, s, dims, dtype, options and the constraint
+ * SELECTION (box present or not, vmax > 0 or not, amax > 0 or not) are those of top_create; waypoints, durations, end
+ * states, box bounds, vmax, amax and rho are new (same layouts as top_create; host pointers, copied).  Nothing is
+ * allocated: the per-segment operator is recomputed on the host, one host-to-device copy, one init kernel; the
+ * iterate is iterate 0 again and top_iteration() restarts at 0.  Asynchronous with respect to the host.
+ * Errors: TOP_E_INVALID (as top_create, or a different constraint selection), TOP_E_CUDA, TOP_E_NOMEM.
+ */
+TOP_API top_status top_reset(top_solver* h, const double* waypoints, const double* durations,
+                     const double* start_derivs, const double* end_derivs, const top_constraints* cons, double rho);
 
 /* top_iterate -- exactly k sweeps of Alg. 1 lines 3-13 (k >= 0; k == 0 is a no-op), enqueued on the
  * stream, no host synchronisation.  Afterwards the observable state is iterate (previous + k) and the
@@ -155,7 +169,8 @@ TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iters);
  * of every segment is re-evaluated on the device for the new rho (from the rho-independent spectral form that
  * top_create precomputes in extended precision), and the SCALED duals u, v, w are multiplied by rho_old/rho_new
  * so that the multipliers y = rho*u are unchanged (reading A16; the paper is silent; Boyd et al. 3.4.1).
- * Two small kernels on the stream; no host synchronisation.
+ * Two small kernels on the stream.  The FIRST change of rho on a handle (or TOP_RHO_ADAPTIVE at top_create) builds the
+ * spectral form on the host (per-segment eigen-solves in extended precision; synchronises once).
  * TOP_E_INVALID if rho <= 0 or not finite. */
 TOP_API top_status top_set_rho(top_solver* h, double rho);
 
@@ -186,7 +201,8 @@ TOP_API top_status top_get_state(top_solver* h, const char* field, double* out, 
 /* Checkpoint / resume (warm start).  top_snapshot_save copies the complete iterate (z~, u, slack / ball variables and
  * their duals, coefficients, residuals, sweep count, rho) into a caller-owned HOST buffer of top_snapshot_bytes(h)
  * bytes; top_snapshot_restore puts it back into a solver that was created with the same sizes, dtype and constraint
- * selection (checked: TOP_E_INVALID otherwise).  Sweeping on from a restored snapshot reproduces the uninterrupted
+ * selection, waypoint mode and N (checked: TOP_E_INVALID otherwise).  A restore also clears the barrier time-out flag
+ * of the handle.  Sweeping on from a restored snapshot reproduces the uninterrupted
  * run bit for bit.  Both synchronise the stream.  The buffer layout is private to this library version. */
 TOP_API size_t top_snapshot_bytes(const top_solver* h);
 TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, size_t bytes);

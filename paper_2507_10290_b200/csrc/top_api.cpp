@@ -5,11 +5,15 @@
 
 #include <algorithm>
 #include <atomic>
+#include <chrono>
+#include <cstdlib>
 #include <thread>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
 #include <limits>
+#include <memory>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -24,6 +28,19 @@ namespace {
 typedef long double xreal;   // precision of the one-off operator precompute (cond(H) reaches 1e13, R6)
 
 thread_local std::string g_create_error;
+
+// phase timer of top_create / top_reset (stderr, enabled by the environment variable TOP_TRACE_CREATE=1)
+struct PhaseTimer {
+    bool on;
+    std::chrono::steady_clock::time_point t0;
+    PhaseTimer() : on(std::getenv("TOP_TRACE_CREATE") != nullptr), t0(std::chrono::steady_clock::now()) {}
+    void mark(const char* what) {
+        if (!on) return;
+        const auto t1 = std::chrono::steady_clock::now();
+        std::fprintf(stderr, "[top_create] %-28s %8.3f ms\n", what, std::chrono::duration<double, std::milli>(t1 - t0).count());
+        t0 = t1;
+    }
+};
 
 }  // namespace
 
@@ -47,13 +64,21 @@ struct top_solver {
     int halo = 0;
     void* alt[8] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     std::vector<Wave> waves;
-    // device buffers
-    std::vector<void*> allocs;
+    // device buffers: ONE arena allocation carved into the arrays below (one cudaMalloc / cudaFree per solver)
+    unsigned char* arena = nullptr;
+    size_t arena_bytes = 0;
+    unsigned char* d_upload = nullptr;     // region that mirrors the host staging buffer: [rho Pm^ rows | the caller's arrays]
+    size_t upload_bytes = 0, off_wp = 0, off_T = 0, off_lo = 0, off_hi = 0, off_sd = 0, off_ed = 0;
+    bool have_sd = false, have_ed = false;
+    unsigned char* zero_begin = nullptr;   // arrays that top_reset sets to zero again (duals, partial sums)
+    size_t zero_bytes = 0;
+    std::unique_ptr<unsigned char[]> stage;   // host staging buffer (kept: top_reset re-uses it)
+    std::vector<double> h_wp, h_T;         // host copies of waypoints / durations (local-frame origins, lazy spectral form)
+    bool have_spectral = false;            // W, lambda on the device (built on first use: top_set_rho, Eq. 24)
     double *d_Pm = nullptr, *d_c0 = nullptr, *d_part = nullptr, *d_res = nullptr;
     double *d_W = nullptr, *d_lam = nullptr, *d_g0 = nullptr, *d_dp = nullptr;   // spectral operator data (rho-independent)
     void *d_invTk = nullptr, *d_Tpow = nullptr, *d_invT = nullptr, *d_lohi = nullptr, *d_zoff = nullptr;
     double* d_origin = nullptr;        // [3][nseg_pad] origin o_i = p_{i-1} of each segment's local frame
-    std::vector<double> origin;        // host copy (top_get_state)
     uint32_t wp_mode = 0;
     double adapt_mu = 10.0, adapt_incr = 1.1, adapt_decr = 1.1;
     uint8_t* d_segflags = nullptr;
@@ -61,11 +86,11 @@ struct top_solver {
          *d_pha = nullptr, *d_wa = nullptr, *d_chat = nullptr, *d_Bedge = nullptr, *d_coef = nullptr;
     unsigned char* d_sync = nullptr;   // u64 grid-barrier counter
     int* d_abort = nullptr;
-    double* h_res = nullptr;           // pinned [batch][4]
-    int* h_abort = nullptr;            // pinned
+    std::vector<double> h_res;         // [batch][4]   (small results come back into pageable memory: every fetch
+    int h_abort[4] = {0, 0, 0, 0};     //                synchronises the stream anyway, and pinned allocations cost ms)
     void* d_resbox = nullptr;          // in-kernel solve: LL slots of the per-CTA residual partial sums
     double* d_solve = nullptr;         // in-kernel solve result [8]
-    double* h_solve = nullptr;         // pinned
+    double h_solve[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     bool have_residuals = false;
     int64_t iter = 0, launches = 0;
     unsigned long long seq_counter = 0;   // sweeps launched so far over all waves (mailbox sequence space)
@@ -98,14 +123,14 @@ xreal beta_hat(int k, int a, xreal tau) {
 
 // In-place inverse of a symmetric positive definite q x q matrix: symmetric diagonal scaling, then
 // Gauss-Jordan elimination without pivoting (safe for SPD), in extended precision.  false if not SPD.
-bool spd_invert(int q, std::vector<xreal>& A) {
-    std::vector<xreal> sc(q);
+bool spd_invert(int q, xreal* A) {
+    xreal sc[MAXN], W[MAXN * 2 * MAXN];
     for (int i = 0; i < q; ++i) {
         if (!(A[i * q + i] > 0)) return false;
         sc[i] = 1 / std::sqrt(A[i * q + i]);
     }
-    std::vector<xreal> W(q * 2 * q, 0);
     for (int i = 0; i < q; ++i) {
+        for (int j = 0; j < 2 * q; ++j) W[i * 2 * q + j] = 0;
         for (int j = 0; j < q; ++j) W[i * 2 * q + j] = A[i * q + j] * sc[i] * sc[j];
         W[i * 2 * q + q + i] = 1;
     }
@@ -139,11 +164,7 @@ struct GramTables {
     xreal Gc[4][MAXN * MAXN];     // consensus rows of derivative order k: beta_k(0)beta_k(0)' + beta_k(1)beta_k(1)'
     xreal Ge[3][MAXN * MAXN];     // sample rows of E_0, E_1, E_2: sum_j beta_k(tau_j) beta_k(tau_j)'
 };
-const GramTables& gram_tables(int s) {
-    static GramTables tab[2];
-    static bool ready[2] = {false, false};
-    GramTables& G = tab[s - 3];
-    if (ready[s - 3]) return G;        // benign race: concurrent builders write identical values
+void build_gram_tables(int s, GramTables& G) {
     const int n = 2 * s;
     std::memset(&G, 0, sizeof G);
     for (int j = s; j < n; ++j)
@@ -160,8 +181,12 @@ const GramTables& gram_tables(int s) {
     for (int k = 0; k < s; ++k) { add(G.Gc[k], k, 0); add(G.Gc[k], k, 1); }
     for (int j = 1; j <= MS; ++j)
         for (int k = 0; k < 3; ++k) add(G.Ge[k], k, (xreal)j / (xreal)(MS + 1));     // reading A10
-    ready[s - 3] = true;
-    return G;
+}
+const GramTables& gram_tables(int s) {       // built once per s, whatever thread comes first (concurrent top_create calls)
+    static GramTables tab[2];
+    static std::once_flag once[2];
+    std::call_once(once[s - 3], [s] { build_gram_tables(s, tab[s - 3]); });
+    return tab[s - 3];
 }
 
 bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int mode,
@@ -174,7 +199,7 @@ bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int
     const xreal wq = 2 * T * iT[2 * s - 1] * iT[1];             // 2 T^(1-2s)
     const xreal wb = box ? 2 * rho : 0;                        // two sides of the box (A11)
     const xreal wv = vel ? rho * iT[2] : 0, wa = acc ? rho * iT[4] : 0;
-    std::vector<xreal> H(n * n, 0);
+    xreal H[MAXN * MAXN];
     for (int a = 0; a < n; ++a)
         for (int b = 0; b < n; ++b) {
             const int i = a * MAXN + b;
@@ -183,10 +208,10 @@ bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int
             H[a * n + b] = v;
         }
     for (int i = 0; i < MAXN * MAXN; ++i) Pm[i] = 0;
-    for (int i = 0; i < MAXN * 3; ++i) c0[i] = 0;
+    if (c0) for (int i = 0; i < MAXN * 3; ++i) c0[i] = 0;
     if (mode == (int)TOP_WAYPOINT_HARD) {
         const int q = n - 2;
-        std::vector<xreal> A(q * q);
+        xreal A[MAXN * MAXN];
         auto Hz = [&](int a, int b) { return H[a * n + b]; };
         for (int i = 0; i < q; ++i)
             for (int j = 0; j < q; ++j) {
@@ -203,7 +228,7 @@ bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int
                 Pm[(i + 2) * MAXN + 1] -= v;
                 Pm[1 * MAXN + 1] += v;
             }
-        for (int d = 0; d < 3; ++d) {
+        for (int d = 0; c0 && d < 3; ++d) {
             xreal cp[MAXN] = {0}, Hc[MAXN] = {0};
             cp[0] = p0[d]; cp[1] = p1[d] - p0[d];
             for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) Hc[a] += H[a * n + b] * cp[b];
@@ -214,7 +239,8 @@ bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int
             }
         }
     } else {
-        std::vector<xreal> A(H);
+        xreal A[MAXN * MAXN];
+        for (int i = 0; i < n * n; ++i) A[i] = H[i];
         if (!spd_invert(n, A)) return false;
         for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) Pm[a * MAXN + b] = A[a * n + b];
     }
@@ -372,31 +398,6 @@ void project_ball_host(const double* y, double bound, Real* phi) {
     for (int d = 0; d < 3; ++d) phi[d] = (Real)(sc * y[d]);
 }
 
-top_status dev_alloc(top_solver* h, void** out, size_t bytes, bool zero) {
-    void* p = nullptr;
-    cudaError_t e = cudaMalloc(&p, bytes ? bytes : 16);
-    if (e != cudaSuccess) { *out = nullptr; return fail(h, e == cudaErrorMemoryAllocation ? TOP_E_NOMEM : TOP_E_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e)); }
-    h->allocs.push_back(p);
-    if (zero) { e = cudaMemsetAsync(p, 0, bytes ? bytes : 16, h->stream); if (e != cudaSuccess) return cuda_fail(h, e, "cudaMemsetAsync"); }
-    *out = p;
-    return TOP_OK;
-}
-
-// host fp64 staging -> device array of the solver's Real type
-top_status upload_real(top_solver* h, void* dst, const std::vector<double>& src) {
-    if (src.empty()) return TOP_OK;
-    if (h->dtype == TOP_F64) {
-        CU(cudaMemcpyAsync(dst, src.data(), src.size() * 8, cudaMemcpyHostToDevice, h->stream), "H2D");
-        CU(cudaStreamSynchronize(h->stream), "sync");
-    } else {
-        std::vector<float> f(src.size());
-        for (size_t i = 0; i < src.size(); ++i) f[i] = (float)src[i];
-        CU(cudaMemcpyAsync(dst, f.data(), f.size() * 4, cudaMemcpyHostToDevice, h->stream), "H2D");
-        CU(cudaStreamSynchronize(h->stream), "sync");
-    }
-    return TOP_OK;
-}
-
 top_status download_real(top_solver* h, const void* src, std::vector<double>& dst, size_t count) {
     dst.resize(count);
     if (h->dtype == TOP_F64) {
@@ -440,37 +441,150 @@ cudaError_t refresh_operator(top_solver* h, double rho) {
     h->launches += 1;
     return launch_refresh_operator(r, h->stream);
 }
-// run fn(g0, g1) over [0, n) on the host cores (segments are independent)
+// run fn(g0, g1) over [0, n) on the host cores (segments are independent).  A chunk whose thread cannot be started runs
+// on the calling thread; fn must not throw (the callers catch inside).
 template <typename F> void parallel_segments(long long n, F fn) {
     unsigned nt = std::thread::hardware_concurrency();
     nt = std::max(1u, std::min(nt, 32u));
     if (n < 2048) nt = 1;
     std::vector<std::thread> pool;
     const long long chunk = (n + nt - 1) / nt;
-    for (unsigned t = 1; t < nt; ++t)
-        if ((long long)t * chunk < n) pool.emplace_back(fn, (long long)t * chunk, std::min(n, (long long)(t + 1) * chunk));
+    for (unsigned t = 1; t < nt; ++t) {
+        const long long lo = (long long)t * chunk, hi = std::min(n, (long long)(t + 1) * chunk);
+        if (lo >= n) break;
+        try { pool.emplace_back(fn, lo, hi); } catch (...) { fn(lo, hi); }
+    }
     fn(0, std::min(n, chunk));
     for (auto& th : pool) th.join();
 }
 }  // namespace
 
-// =================================================================================== top_create
+namespace {
 
-extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_t N, int32_t s, int32_t dims, top_dtype dtype,
-                                 const double* waypoints, const double* durations, const double* start_derivs,
-                                 const double* end_derivs, const top_constraints* cons, double rho,
-                                 const top_options* opt) {
-    top_solver* h = nullptr;   // errors before the handle exists go to the thread-local message
-    if (!out) return fail(h, TOP_E_INVALID, "out is NULL");
-    *out = nullptr;
-    if (batch < 1 || N < 1) return fail(h, TOP_E_INVALID, "batch and N must be >= 1");
-    if (s != 3 && s != 4) return fail(h, TOP_E_INVALID, "s must be 3 (jerk) or 4 (snap)");
-    if (dims < 1 || dims > 3) return fail(h, TOP_E_INVALID, "dims must be 1..3");
-    if (dtype != TOP_F64 && dtype != TOP_F32) return fail(h, TOP_E_INVALID, "unknown dtype");
+// The per-problem part of top_create, shared with top_reset: host precompute of the x-update operator (Eq. 20a first
+// bracket; per segment, extended precision, for the current rho), ONE host-to-device copy of the operator rows and of
+// the caller's arrays, then the init kernel (per-lane constants and iterate 0, reading A9).  Asynchronous.
+top_status fill_problem(top_solver* h, const double* waypoints, const double* durations, const double* start_derivs,
+                        const double* end_derivs, const top_constraints* cons, PhaseTimer* pt) {
+    const int N = h->N, s = h->s, dims = h->dims, batch = h->batch, n = 2 * s;
+    const long long nseg = h->nseg;
+    const size_t LS = (size_t)h->stride;
+    unsigned char* S = h->stage.get();
+    double* Pm_st = reinterpret_cast<double*>(S);
+    std::memcpy(S + h->off_wp, waypoints, (size_t)batch * (N + 1) * dims * 8);
+    std::memcpy(S + h->off_T, durations, (size_t)nseg * 8);
+    if (h->has_box) {
+        std::memcpy(S + h->off_lo, cons->box_lo, (size_t)nseg * dims * 8);
+        std::memcpy(S + h->off_hi, cons->box_hi, (size_t)nseg * dims * 8);
+    }
+    h->have_sd = start_derivs != nullptr; h->have_ed = end_derivs != nullptr;
+    if (start_derivs) std::memcpy(S + h->off_sd, start_derivs, (size_t)batch * (s - 1) * dims * 8);
+    if (end_derivs) std::memcpy(S + h->off_ed, end_derivs, (size_t)batch * (s - 1) * dims * 8);
+    h->h_wp.assign(waypoints, waypoints + (size_t)batch * (N + 1) * dims);
+    h->h_T.assign(durations, durations + nseg);
+    const GramTables& G = gram_tables(s);     // built before the worker threads start
+    if (pt) pt->mark("staging copies");
+
+    // rho Pm^ of every segment by the direct (null-space) inverse; segments of equal duration (config 3: all of them)
+    // share one factorisation.  The rho-independent spectral form is only built when rho is going to change.
+    std::atomic<int> bad_operator(0);
+    const bool box = h->has_box, vel = h->has_vel, acc = h->has_acc;
+    const int mode = (int)h->wp_mode;
+    const xreal rho = (xreal)h->rho;
+    auto do_segments = [&](long long g0, long long g1) {
+        try {
+            xreal Pm[MAXN * MAXN];
+            double cached_T = -1.0;
+            for (long long g = g0; g < g1; ++g) {
+                const double Td = durations[g];
+                if (Td != cached_T) {
+                    if (!build_operator(s, (xreal)Td, rho, box, vel, acc, mode, nullptr, nullptr, Pm, nullptr)) { bad_operator.store(1); return; }
+                    cached_T = Td;
+                }
+                for (int lane = 0; lane < n; ++lane)
+                    for (int b = 0; b < n; ++b) Pm_st[(size_t)b * LS + (size_t)g * LANES + lane] = (double)(rho * Pm[lane * MAXN + b]);
+            }
+        } catch (...) { bad_operator.store(2); }
+    };
+    parallel_segments(nseg, do_segments);
+    if (pt) pt->mark("host precompute");
+    if (bad_operator.load() == 2) return fail(h, TOP_E_NOMEM, "host precompute failed");
+    if (bad_operator.load()) return fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)");
+
+    CU(cudaMemcpyAsync(h->d_upload, S, h->upload_bytes, cudaMemcpyHostToDevice, h->stream), "H2D problem data");
+    InitParams ip;
+    std::memset(&ip, 0, sizeof ip);
+    unsigned char* D = h->d_upload;
+    ip.waypoints = (const double*)(D + h->off_wp); ip.durations = (const double*)(D + h->off_T);
+    ip.box_lo = h->has_box ? (const double*)(D + h->off_lo) : nullptr; ip.box_hi = h->has_box ? (const double*)(D + h->off_hi) : nullptr;
+    ip.start_derivs = start_derivs ? (const double*)(D + h->off_sd) : nullptr;
+    ip.end_derivs = end_derivs ? (const double*)(D + h->off_ed) : nullptr;
+    for (int a = 0; a < MAXN; ++a) {
+        for (int k = 0; k < 4; ++k) ip.gc1[k][a] = (double)G.Gc[k][a * MAXN + 1];
+        for (int k = 0; k < 3; ++k) ip.ge1[k][a] = (double)G.Ge[k][a * MAXN + 1];
+    }
+    ip.Pm = h->d_Pm; ip.c0 = h->d_c0; ip.g0 = h->d_g0; ip.dp = h->d_dp; ip.origin = h->d_origin;
+    ip.invTk = h->d_invTk; ip.Tpow = h->d_Tpow; ip.invT = h->d_invT; ip.lohi = h->d_lohi; ip.zoff = h->d_zoff;
+    ip.zt = h->d_zt; ip.chat = h->d_chat; ip.qp = h->d_qp; ip.qn = h->d_qn; ip.phv = h->d_phv; ip.segflags = h->d_segflags;
+    ip.stride = h->stride; ip.nseg_pad = h->nseg_pad; ip.nseg = nseg; ip.N = N; ip.batch = batch; ip.s = s; ip.dims = dims;
+    ip.hard = h->wp_mode == TOP_WAYPOINT_HARD; ip.has_box = h->has_box; ip.has_vel = h->has_vel; ip.has_acc = h->has_acc;
+    ip.vmax = h->vmax;
+    CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
+    h->launches += 1;
+    h->have_spectral = false;
+    h->have_residuals = false;
+    std::fill(h->h_res.begin(), h->h_res.end(), std::numeric_limits<double>::quiet_NaN());
+    h->iter = 0;
+    if (pt) pt->mark("upload + init kernel");
+    return TOP_OK;
+}
+
+// W, lambda of the rho-independent spectral form (build_spectral) on the device: needed only when rho changes
+// (top_set_rho, Eq. 24, a snapshot with another rho).  Host eigen-solves in extended precision; synchronises.
+top_status ensure_spectral(top_solver* h) {
+    if (h->have_spectral) return TOP_OK;
+    const int s = h->s, n = 2 * s;
+    const size_t LS = (size_t)h->stride, NP = (size_t)h->nseg_pad;
+    std::vector<double> Wv, lamv;
+    try { Wv.assign(MAXN * LS, 0.0); lamv.assign(MAXN * NP, 0.0); } catch (...) { return fail(h, TOP_E_NOMEM, "host allocation failed"); }
+    gram_tables(s);
+    std::atomic<int> bad(0);
+    const double* durations = h->h_T.data();
+    auto work = [&](long long g0, long long g1) {
+        try {
+            Spectral SP;
+            double cached_T = -1.0;
+            const xreal zero3[3] = {0, 0, 0};
+            for (long long g = g0; g < g1; ++g) {
+                if (durations[g] != cached_T) {
+                    if (!build_spectral(s, (xreal)durations[g], h->has_box, h->has_vel, h->has_acc, (int)h->wp_mode, zero3, SP)) { bad.store(1); return; }
+                    cached_T = durations[g];
+                }
+                for (int i = 0; i < MAXN; ++i) lamv[(size_t)i * NP + g] = i < SP.q ? (double)SP.lam[i] : 0.0;
+                for (int lane = 0; lane < n; ++lane)
+                    for (int i = 0; i < MAXN; ++i) Wv[(size_t)i * LS + (size_t)g * LANES + lane] = (double)SP.W[lane * MAXN + i];
+            }
+        } catch (...) { bad.store(2); }
+    };
+    parallel_segments(h->nseg, work);
+    if (bad.load()) return fail(h, bad.load() == 2 ? TOP_E_NOMEM : TOP_E_INVALID, "spectral form of the x-update operator failed");
+    CU(cudaMemcpyAsync(h->d_W, Wv.data(), MAXN * LS * 8, cudaMemcpyHostToDevice, h->stream), "H2D spectral form");
+    CU(cudaMemcpyAsync(h->d_lam, lamv.data(), MAXN * NP * 8, cudaMemcpyHostToDevice, h->stream), "H2D spectral form");
+    CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+    h->have_spectral = true;
+    return TOP_OK;
+}
+
+}  // namespace
+
+namespace {
+// argument checks common to top_create and top_reset (messages go to the handle, or to the thread-local slot)
+top_status validate_problem(top_solver* h, int batch, int N, int s, int dims, const double* waypoints, const double* durations,
+                            const double* start_derivs, const double* end_derivs, const top_constraints* cons, double rho,
+                            bool* has_box, bool* has_vel, bool* has_acc) {
     if (!waypoints || !durations) return fail(h, TOP_E_INVALID, "waypoints and durations are required");
     if (!(rho > 0) || !std::isfinite(rho)) return fail(h, TOP_E_INVALID, "rho must be finite and > 0");
     const long long nseg = (long long)batch * N;
-    if (nseg > (1ll << 28)) return fail(h, TOP_E_UNSUPPORTED, "more than 2^28 segments");
     for (long long i = 0; i < (long long)batch * (N + 1) * dims; ++i)
         if (!std::isfinite(waypoints[i])) return fail(h, TOP_E_INVALID, "non-finite waypoint");
     for (long long i = 0; i < nseg; ++i)
@@ -480,19 +594,52 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
         if (dv) for (long long i = 0; i < (long long)batch * (s - 1) * dims; ++i)
             if (!std::isfinite(dv[i])) return fail(h, TOP_E_INVALID, "non-finite end state");
     }
-    bool has_box = false, has_vel = false, has_acc = false;
+    *has_box = *has_vel = *has_acc = false;
     if (cons && cons->samples != 0) {
-        if (cons->samples != MS) return fail(h, TOP_E_INVALID, "constraints.samples must be 0 or 8");
+        if (cons->samples < 0) return fail(h, TOP_E_INVALID, "constraints.samples must be >= 0");
+        if (cons->samples != MS) return fail(h, TOP_E_UNSUPPORTED, "constraints.samples: this build evaluates the inequality sets at 8 samples per segment");
         if ((cons->box_lo == nullptr) != (cons->box_hi == nullptr)) return fail(h, TOP_E_INVALID, "box_lo and box_hi go together");
-        has_box = cons->box_lo != nullptr;
-        if (has_box) for (long long i = 0; i < nseg * dims; ++i) {
+        *has_box = cons->box_lo != nullptr;
+        if (*has_box) for (long long i = 0; i < nseg * dims; ++i) {
             if (!std::isfinite(cons->box_lo[i]) || !std::isfinite(cons->box_hi[i]) || !(cons->box_lo[i] < cons->box_hi[i]))
                 return fail(h, TOP_E_INVALID, "box needs finite lo < hi");
         }
         if (std::isnan(cons->vmax) || std::isnan(cons->amax) || std::isinf(cons->vmax) || std::isinf(cons->amax))
             return fail(h, TOP_E_INVALID, "vmax/amax must be finite");
-        has_vel = cons->vmax > 0;
-        has_acc = cons->amax > 0;
+        *has_vel = cons->vmax > 0;
+        *has_acc = cons->amax > 0;
+    }
+    return TOP_OK;
+}
+}  // namespace
+
+// =================================================================================== top_create
+
+namespace {
+struct HandleGuard {        // destroys a half-built solver on every early return / exception of top_create
+    top_solver* h = nullptr;
+    ~HandleGuard() { if (h) top_destroy(h); }
+};
+
+top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, int32_t dims, top_dtype dtype,
+                       const double* waypoints, const double* durations, const double* start_derivs,
+                       const double* end_derivs, const top_constraints* cons, double rho, const top_options* opt) {
+    top_solver* h = nullptr;   // errors before the handle exists go to the thread-local message
+    HandleGuard guard;
+    PhaseTimer pt;
+    if (!out) return fail(h, TOP_E_INVALID, "out is NULL");
+    *out = nullptr;
+    if (batch < 1 || N < 1) return fail(h, TOP_E_INVALID, "batch and N must be >= 1");
+    if (s != 3 && s != 4) return fail(h, TOP_E_INVALID, "s must be 3 (jerk) or 4 (snap)");
+    if (dims < 1 || dims > 3) return fail(h, TOP_E_INVALID, "dims must be 1..3");
+    if (dtype != TOP_F64 && dtype != TOP_F32) return fail(h, TOP_E_INVALID, "unknown dtype");
+    const long long nseg = (long long)batch * N;
+    if (nseg > (1ll << 28)) return fail(h, TOP_E_UNSUPPORTED, "more than 2^28 segments");
+    bool has_box = false, has_vel = false, has_acc = false;
+    {
+        top_status vs = validate_problem(nullptr, batch, N, s, dims, waypoints, durations, start_derivs, end_derivs, cons, rho,
+                                         &has_box, &has_vel, &has_acc);
+        if (vs != TOP_OK) return vs;
     }
     top_options o;
     std::memset(&o, 0, sizeof o);
@@ -521,6 +668,7 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
     for (double v : {o.adapt_mu, o.adapt_tau_incr, o.adapt_tau_decr})
         if (v != 0 && !(v > 1 && std::isfinite(v))) return fail(h, TOP_E_INVALID, "adapt_mu / adapt_tau_* must be > 1 (or 0 = default)");
 
+    pt.mark("validation");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         cudaGetLastError();
@@ -533,8 +681,9 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
 
     h = new (std::nothrow) top_solver();
     if (!h) return fail(nullptr, TOP_E_NOMEM, "host allocation failed");
-    // from here on errors are reported through the thread-local message and the handle is destroyed
-#define CREATE_FAIL(st_) do { top_status s__ = (st_); g_create_error = h->err; top_destroy(h); return s__; } while (0)
+    guard.h = h;
+    // from here on errors are reported through the thread-local message and the guard destroys the handle
+#define CREATE_FAIL(st_) do { top_status s__ = (st_); g_create_error = h->err; return s__; } while (0)
     h->batch = batch; h->N = N; h->s = s; h->n = 2 * s; h->dims = dims; h->dtype = (int)dtype;
     h->opt_flags = o.flags; h->rho = rho; h->check_every = o.check_every; h->max_iter = o.max_iter;
     h->device = dev; h->stream = (cudaStream_t)o.cuda_stream; h->user_segs = o.segs_per_cta;
@@ -617,163 +766,125 @@ extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_
         if (per_sm < 1) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "sweep kernel does not fit an SM"));
     }
 
-    // ---- host precompute (extended precision) and iterate 0 (reading A9), packed per lane
+    pt.mark("launch plan");
+
+    // ---- memory: one device arena, one host staging buffer
     const size_t LS = (size_t)h->stride, NP = (size_t)h->nseg_pad;
-    std::vector<double> Wv(MAXN * LS, 0.0), g0v(3 * LS, 0.0), lamv(MAXN * NP, 0.0), dpv(3 * NP, 0.0), invTk(LS, 0.0), Tpow(LS, 0.0), invT(2 * NP, 0.0),
-        lohi(6 * NP, 0.0), zt(3 * LS, 0.0), chat(3 * LS, 0.0), zoff(3 * LS, 0.0), origin(3 * NP, 0.0), qp, qn, phv, pha;
-    std::vector<uint8_t> segflags(NP, 0);
-    if (has_box) { qp.assign(3 * LS, 0.0); qn.assign(3 * LS, 0.0); }
-    if (has_vel) phv.assign(3 * LS, 0.0);
-    const int n = 2 * s;
-    auto wp = [&](long long b, long long j, int d) -> double { return d < dims ? waypoints[((size_t)b * (N + 1) + j) * dims + d] : 0.0; };
-    gram_tables(s);                       // build the shared tables before the worker threads start
-
-    std::atomic<int> bad_operator(0);
-    auto do_segments = [&](long long g0, long long g1) {
-        Spectral SP;
-        bool have_cached = false;
-        double cached_T = 0.0;
-        for (long long gg = g0; gg < g1; ++gg) {
-            const long long b = gg / N, i = gg % N;
-            const size_t g = (size_t)gg;
-            const double Td = durations[g];
-            const xreal T = (xreal)Td;
-            // Segment-local frame: every position-like quantity of segment i (coefficient c_0, position rows of
-            // z~, box bounds) is stored relative to the origin o_i = p_{i-1}.  An exact change of variable (the
-            // sweep only ever uses position differences) that keeps the operator free of the cancellation of
-            // |p| ~ 100 m against segment-sized quantities; top_get_coeffs / top_get_state add o_i back.
-            xreal p0[3], p1[3];
-            double org3[3];
-            for (int d = 0; d < 3; ++d) {
-                org3[d] = wp(b, i, d);
-                p0[d] = 0; p1[d] = (xreal)wp(b, i + 1, d) - (xreal)wp(b, i, d);
-                origin[(size_t)d * NP + g] = org3[d];
-            }
-            // W, lambda and G depend on the duration only: segments of equal duration (config 3: all of them) share
-            // one factorisation; only g0 = (G e_1) dp is per segment
-            if (!(have_cached && Td == cached_T)) {
-                if (!build_spectral(s, T, has_box, has_vel, has_acc, (int)mode, p1, SP)) {
-                    bad_operator.store(1);
-                    return;
-                }
-                have_cached = true; cached_T = Td;
-            } else if (mode == TOP_WAYPOINT_HARD) {
-                for (int a = 0; a < n; ++a) for (int d = 0; d < 3; ++d) SP.g0[a * 3 + d] = SP.gcol1[a] * p1[d];
-            }
-            for (int ii = 0; ii < MAXN; ++ii) lamv[(size_t)ii * NP + g] = ii < SP.q ? (double)SP.lam[ii] : 0.0;
-            for (int d = 0; d < 3; ++d) dpv[(size_t)d * NP + g] = (mode == TOP_WAYPOINT_HARD && d < dims) ? (double)p1[d] : 0.0;
-            segflags[g] = (uint8_t)((i == 0 ? SEG_FIRST : 0) | (i == N - 1 ? SEG_LAST : 0));
-            invT[g] = (double)(1 / T); invT[NP + g] = (double)(1 / (T * T));
-            for (int d = 0; d < 3; ++d) {
-                lohi[(size_t)d * NP + g] = (has_box && d < dims) ? cons->box_lo[g * dims + d] - org3[d] : -1.0;
-                lohi[(size_t)(3 + d) * NP + g] = (has_box && d < dims) ? cons->box_hi[g * dims + d] - org3[d] : 1.0;
-            }
-            for (int lane = 0; lane < LANES; ++lane) {
-                const size_t gt = g * LANES + lane;
-                for (int ii = 0; ii < MAXN; ++ii) Wv[(size_t)ii * LS + gt] = (double)SP.W[lane * MAXN + ii];
-                for (int d = 0; d < 3; ++d) g0v[(size_t)d * LS + gt] = d < dims ? (double)SP.g0[lane * 3 + d] : 0.0;
-                Tpow[gt] = (double)std::pow(T, (xreal)lane);
-                // a neighbour's position row arrives in the neighbour's frame: shift it into this segment's frame
-                for (int d = 0; d < dims; ++d) {
-                    if (lane == 0 && i > 0) zoff[(size_t)d * LS + gt] = wp(b, i - 1, d) - wp(b, i, d);   // o_{i-1} - o_i
-                    if (lane == s && i < N - 1) zoff[(size_t)d * LS + gt] = (double)p1[d];               // o_{i+1} - o_i
-                }
-                if (lane < n) {
-                    const int k = lane % s;
-                    invTk[gt] = (double)(1 / std::pow(T, (xreal)k));
-                    // z0: position = waypoint; velocity = mean of the adjacent chord velocities; higher orders 0;
-                    // z_0 and z_N carry the given end states (Eq. 2c)
-                    const long long j = lane < s ? i : i + 1;
-                    for (int d = 0; d < dims; ++d) {
-                        double v = 0;
-                        if (k == 0) v = wp(b, j, d) - org3[d];
-                        else if (j == 0) v = start_derivs ? start_derivs[((size_t)b * (s - 1) + (k - 1)) * dims + d] : 0.0;
-                        else if (j == N) v = end_derivs ? end_derivs[((size_t)b * (s - 1) + (k - 1)) * dims + d] : 0.0;
-                        else if (k == 1) {
-                            const double vl = (wp(b, j, d) - wp(b, j - 1, d)) / durations[b * N + j - 1];
-                            const double vr = (wp(b, j + 1, d) - wp(b, j, d)) / durations[b * N + j];
-                            v = 0.5 * (vl + vr);
-                        }
-                        zt[(size_t)d * LS + gt] = v;
-                    }
-                }
-                // C0 = chord at constant speed: c^_0 = p_{i-1}, c^_1 = p_i - p_{i-1}
-                for (int d = 0; d < dims; ++d)
-                    chat[(size_t)d * LS + gt] = lane == 0 ? (double)p0[d] : (lane == 1 ? (double)(p1[d] - p0[d]) : 0.0);
-                // samples of the chord: slack = max(0, .), phi = projection of the chord velocity, duals 0
-                const double tau = (double)(lane + 1) / (double)(MS + 1);
-                double V0[3] = {0, 0, 0};
-                for (int d = 0; d < dims; ++d) {
-                    const double P0 = tau * (double)p1[d];         // local frame
-                    V0[d] = (double)(p1[d] - p0[d]) / Td;
-                    if (has_box) {
-                        qp[(size_t)d * LS + gt] = std::max(0.0, (cons->box_hi[g * dims + d] - org3[d]) - P0);
-                        qn[(size_t)d * LS + gt] = std::max(0.0, P0 - (cons->box_lo[g * dims + d] - org3[d]));
-                    }
-                }
-                if (has_box) for (int d = dims; d < 3; ++d) { qp[(size_t)d * LS + gt] = 1.0; qn[(size_t)d * LS + gt] = 1.0; }
-                if (has_vel) {
-                    double phi[3];
-                    project_ball_host<double>(V0, h->vmax, phi);
-                    for (int d = 0; d < 3; ++d) phv[(size_t)d * LS + gt] = phi[d];
-                }
-            }
-        }
-    };
-    parallel_segments(nseg, do_segments);
-    if (bad_operator.load())
-        CREATE_FAIL(fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)"));
-
-    // ---- device memory
     const size_t rb = real_bytes(h);
-    top_status st;
-#define ALLOC(ptr, bytes, zero) do { void* p__ = nullptr; st = dev_alloc(h, &p__, (bytes), (zero)); if (st != TOP_OK) CREATE_FAIL(st); ptr = static_cast<decltype(ptr)>(p__); } while (0)
-    ALLOC(h->d_Pm, MAXN * LS * 8, false); ALLOC(h->d_c0, 3 * LS * 8, false);
-    ALLOC(h->d_W, MAXN * LS * 8, false); ALLOC(h->d_g0, 3 * LS * 8, false);
-    ALLOC(h->d_lam, MAXN * NP * 8, false); ALLOC(h->d_dp, 3 * NP * 8, false);
-    ALLOC(h->d_invTk, LS * rb, false); ALLOC(h->d_Tpow, LS * rb, false); ALLOC(h->d_invT, 2 * NP * rb, false);
-    ALLOC(h->d_lohi, 6 * NP * rb, false); ALLOC(h->d_segflags, NP, false);
-    ALLOC(h->d_zoff, 3 * LS * rb, false); ALLOC(h->d_origin, 3 * NP * 8, false);
-    ALLOC(h->d_zt, 3 * LS * rb, false); ALLOC(h->d_u, 3 * LS * rb, true); ALLOC(h->d_chat, 3 * LS * rb, false);
-    if (has_box) { ALLOC(h->d_qp, 3 * LS * rb, false); ALLOC(h->d_qn, 3 * LS * rb, false); }
-    if (has_vel) { ALLOC(h->d_phv, 3 * LS * rb, false); ALLOC(h->d_wv, 3 * LS * rb, true); }
-    if (has_acc) { ALLOC(h->d_pha, 3 * LS * rb, true); ALLOC(h->d_wa, 3 * LS * rb, true); }
+    const int n = 2 * s;
+    struct Carve { size_t off = 0; size_t take(size_t bytes) { const size_t o = off; off = (off + bytes + 255) & ~(size_t)255; return o; } } cv;
+    // (a) the region that mirrors the staging buffer: operator rows, then the caller's arrays as they are
+    const size_t o_Pm = cv.take(MAXN * LS * 8);
+    h->off_wp = cv.take((size_t)batch * (N + 1) * dims * 8);
+    h->off_T = cv.take((size_t)nseg * 8);
+    h->off_lo = cv.take(has_box ? (size_t)nseg * dims * 8 : 0);
+    h->off_hi = cv.take(has_box ? (size_t)nseg * dims * 8 : 0);
+    h->off_sd = cv.take((size_t)batch * (s - 1) * dims * 8);
+    h->off_ed = cv.take((size_t)batch * (s - 1) * dims * 8);
+    h->upload_bytes = cv.off;
+    // (b) constants written by the init kernel
+    const size_t o_c0 = cv.take(3 * LS * 8), o_W = cv.take(MAXN * LS * 8), o_g0 = cv.take(3 * LS * 8), o_lam = cv.take(MAXN * NP * 8),
+                 o_dp = cv.take(3 * NP * 8), o_invTk = cv.take(LS * rb), o_Tpow = cv.take(LS * rb), o_invT = cv.take(2 * NP * rb),
+                 o_lohi = cv.take(6 * NP * rb), o_segf = cv.take(NP), o_zoff = cv.take(3 * LS * rb), o_origin = cv.take(3 * NP * 8),
+                 o_coef = cv.take((size_t)nseg * dims * n * rb);
+    // (c) iterate: written by the init kernel ...
+    const size_t o_zt = cv.take(3 * LS * rb), o_chat = cv.take(3 * LS * rb), o_qp = cv.take(has_box ? 3 * LS * rb : 0),
+                 o_qn = cv.take(has_box ? 3 * LS * rb : 0), o_phv = cv.take(has_vel ? 3 * LS * rb : 0);
+    // ... or zero at iterate 0 (duals), together with the reduction buffers: one memset, repeated by top_reset
+    const size_t o_zero = cv.off;
+    const size_t o_u = cv.take(3 * LS * rb), o_wv = cv.take(has_vel ? 3 * LS * rb : 0), o_pha = cv.take(has_acc ? 3 * LS * rb : 0),
+                 o_wa = cv.take(has_acc ? 3 * LS * rb : 0), o_part = cv.take(NP * 4 * 8), o_res = cv.take((size_t)batch * 4 * 8),
+                 o_solve = cv.take(64);
+    size_t o_alt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+    if (h->streaming) {
+        const bool on[8] = {true, true, has_box, has_box, has_vel, has_vel, has_acc, has_acc};
+        for (int i = 0; i < 8; ++i) o_alt[i] = cv.take(on[i] ? 3 * LS * rb : 0);
+    }
+    h->zero_bytes = cv.off - o_zero;
+    // (d) exchange buffers (zero once; sequence numbers keep growing over the life of the solver)
+    const size_t o_Bedge = cv.take((size_t)2 * h->max_ctas * 24 * 16), o_resbox = cv.take((size_t)2 * h->max_ctas * 4 * 16),
+                 o_sync = cv.take(16), o_abort = cv.take(16);
+    h->arena_bytes = cv.off;
+    {
+        void* pa = nullptr;
+        cudaError_t e = cudaMalloc(&pa, h->arena_bytes);
+        if (e != cudaSuccess) CREATE_FAIL(fail(h, e == cudaErrorMemoryAllocation ? TOP_E_NOMEM : TOP_E_CUDA, std::string("cudaMalloc: ") + cudaGetErrorString(e)));
+        h->arena = static_cast<unsigned char*>(pa);
+        if ((e = cudaMemsetAsync(h->arena, 0, h->arena_bytes, h->stream)) != cudaSuccess) CREATE_FAIL(cuda_fail(h, e, "cudaMemsetAsync"));
+    }
+    unsigned char* A = h->arena;
+    h->d_upload = A; h->zero_begin = A + o_zero;
+    h->d_Pm = (double*)(A + o_Pm); h->d_c0 = (double*)(A + o_c0); h->d_W = (double*)(A + o_W); h->d_g0 = (double*)(A + o_g0);
+    h->d_lam = (double*)(A + o_lam); h->d_dp = (double*)(A + o_dp); h->d_invTk = A + o_invTk; h->d_Tpow = A + o_Tpow;
+    h->d_invT = A + o_invT; h->d_lohi = A + o_lohi; h->d_segflags = A + o_segf; h->d_zoff = A + o_zoff;
+    h->d_origin = (double*)(A + o_origin); h->d_coef = A + o_coef; h->d_zt = A + o_zt; h->d_chat = A + o_chat;
+    h->d_u = A + o_u; h->d_part = (double*)(A + o_part); h->d_res = (double*)(A + o_res); h->d_solve = (double*)(A + o_solve);
+    if (has_box) { h->d_qp = A + o_qp; h->d_qn = A + o_qn; }
+    if (has_vel) { h->d_phv = A + o_phv; h->d_wv = A + o_wv; }
+    if (has_acc) { h->d_pha = A + o_pha; h->d_wa = A + o_wa; }
     if (h->streaming) {
         void* cur[8] = {h->d_zt, h->d_u, h->d_qp, h->d_qn, h->d_phv, h->d_wv, h->d_pha, h->d_wa};
-        for (int i = 0; i < 8; ++i) if (cur[i]) ALLOC(h->alt[i], 3 * LS * rb, true);
+        for (int i = 0; i < 8; ++i) if (cur[i]) h->alt[i] = A + o_alt[i];
     }
-    ALLOC(h->d_Bedge, (size_t)2 * h->max_ctas * 24 * 16, true);
-    ALLOC(h->d_part, NP * 4 * 8, true); ALLOC(h->d_res, (size_t)batch * 4 * 8, true);
-    ALLOC(h->d_sync, 16, true); ALLOC(h->d_abort, 16, true);
-    ALLOC(h->d_coef, (size_t)nseg * dims * n * rb, false);
-    ALLOC(h->d_resbox, (size_t)2 * h->max_ctas * 4 * 16, true); ALLOC(h->d_solve, 64, true);
-#undef ALLOC
-    if (cudaMallocHost((void**)&h->h_res, (size_t)batch * 4 * 8) != cudaSuccess ||
-        cudaMallocHost((void**)&h->h_abort, 16) != cudaSuccess || cudaMallocHost((void**)&h->h_solve, 64) != cudaSuccess)
-        CREATE_FAIL(fail(h, TOP_E_NOMEM, "pinned host allocation failed"));
-    for (long long i = 0; i < (long long)batch * 4; ++i) h->h_res[i] = std::numeric_limits<double>::quiet_NaN();
-    h->h_abort[0] = 0;
+    h->d_Bedge = A + o_Bedge; h->d_resbox = A + o_resbox; h->d_sync = A + o_sync; h->d_abort = (int*)(A + o_abort);
+    h->stage.reset(new (std::nothrow) unsigned char[h->upload_bytes]);
+    if (!h->stage) CREATE_FAIL(fail(h, TOP_E_NOMEM, "host allocation failed"));
+    std::memset(h->stage.get(), 0, MAXN * LS * 8);        // padded operator rows stay zero
+    h->h_res.assign((size_t)batch * 4, std::numeric_limits<double>::quiet_NaN());
+    pt.mark("memory (1 cudaMalloc)");
 
-    cudaError_t ce;
-    if ((ce = cudaMemcpyAsync(h->d_W, Wv.data(), MAXN * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
-        (ce = cudaMemcpyAsync(h->d_g0, g0v.data(), 3 * LS * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
-        (ce = cudaMemcpyAsync(h->d_lam, lamv.data(), MAXN * NP * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
-        (ce = cudaMemcpyAsync(h->d_dp, dpv.data(), 3 * NP * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
-        (ce = refresh_operator(h, rho)) != cudaSuccess ||
-        (ce = cudaMemcpyAsync(h->d_segflags, segflags.data(), NP, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
-        (ce = cudaMemcpyAsync(h->d_origin, origin.data(), 3 * NP * 8, cudaMemcpyHostToDevice, h->stream)) != cudaSuccess ||
-        (ce = cudaStreamSynchronize(h->stream)) != cudaSuccess)
-        CREATE_FAIL(cuda_fail(h, ce, "upload"));
-#define UP(dst, src) do { st = upload_real(h, dst, src); if (st != TOP_OK) CREATE_FAIL(st); } while (0)
-    UP(h->d_invTk, invTk); UP(h->d_Tpow, Tpow); UP(h->d_invT, invT); UP(h->d_lohi, lohi); UP(h->d_zoff, zoff);
-    h->origin = origin;
-    UP(h->d_zt, zt); UP(h->d_chat, chat);
-    if (has_box) { UP(h->d_qp, qp); UP(h->d_qn, qn); }
-    if (has_vel) UP(h->d_phv, phv);
-#undef UP
+    top_status st = fill_problem(h, waypoints, durations, start_derivs, end_derivs, cons, &pt);
+    if (st != TOP_OK) CREATE_FAIL(st);
+    if (o.flags & TOP_RHO_ADAPTIVE) {        // Eq. 24 will change rho: have the rho-independent form ready
+        st = ensure_spectral(h);
+        if (st != TOP_OK) CREATE_FAIL(st);
+        pt.mark("spectral form");
+    }
 #undef CREATE_FAIL
+    guard.h = nullptr;
     *out = h;
     return TOP_OK;
+}
+}  // namespace
+
+// Nothing throws across the ABI: allocation failures and anything unexpected come back as a status.
+#define TOP_GUARDED(handle, ...)                                                                          \
+    try { __VA_ARGS__ }                                                                                   \
+    catch (const std::bad_alloc&) { return fail(handle, TOP_E_NOMEM, "out of host memory"); }             \
+    catch (const std::exception& e) { return fail(handle, TOP_E_INVALID, std::string("internal error: ") + e.what()); } \
+    catch (...) { return fail(handle, TOP_E_INVALID, "internal error"); }
+
+extern "C" TOP_API top_status top_create(top_solver** out, int32_t batch, int32_t N, int32_t s, int32_t dims, top_dtype dtype,
+                                 const double* waypoints, const double* durations, const double* start_derivs,
+                                 const double* end_derivs, const top_constraints* cons, double rho,
+                                 const top_options* opt) {
+    if (out) *out = nullptr;
+    TOP_GUARDED(nullptr, return create_impl(out, batch, N, s, dims, dtype, waypoints, durations, start_derivs, end_derivs, cons, rho, opt);)
+}
+
+// top_reset: a new problem of the same shape on an existing handle (re-planning): same batch,
+// N, s, dims, dtype, options and constraint SELECTION; new waypoints, durations, end states, bounds and rho.  No
+// allocation, one host-to-device copy, iterate 0 again.
+extern "C" TOP_API top_status top_reset(top_solver* h, const double* waypoints, const double* durations, const double* start_derivs,
+                                const double* end_derivs, const top_constraints* cons, double rho) {
+    if (!h) return TOP_E_INVALID;
+    TOP_GUARDED(h,
+        bool hb, hv, ha;
+        top_status st = validate_problem(h, h->batch, h->N, h->s, h->dims, waypoints, durations, start_derivs, end_derivs, cons, rho, &hb, &hv, &ha);
+        if (st != TOP_OK) return st;
+        if (hb != h->has_box || hv != h->has_vel || ha != h->has_acc)
+            return fail(h, TOP_E_INVALID, "top_reset: the constraint selection (box / velocity / acceleration) must be the one the solver was created with");
+        if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
+        PhaseTimer pt;
+        h->rho = rho;
+        h->vmax = hv ? cons->vmax : 0; h->amax = ha ? cons->amax : 0;
+        CU(cudaMemsetAsync(h->zero_begin, 0, h->zero_bytes, h->stream), "cudaMemsetAsync");
+        CU(cudaMemsetAsync(h->d_abort, 0, sizeof(int), h->stream), "cudaMemsetAsync");
+        st = fill_problem(h, waypoints, durations, start_derivs, end_derivs, cons, &pt);
+        if (st != TOP_OK) return st;
+        if (h->opt_flags & TOP_RHO_ADAPTIVE) st = ensure_spectral(h);
+        return st;
+    )
 }
 
 // =================================================================================== sweeps
@@ -854,7 +965,7 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
             h->iter += done;
             if (h->h_solve[2] != h->rho) {      // the kernel refreshed its on-chip operator only: bring the arrays along
                 h->rho = h->h_solve[2];
-                CU(refresh_operator(h, h->rho), "operator refresh launch");
+                CU(refresh_operator(h, h->rho), "operator refresh launch");      // (Eq. 24 ran: the spectral form is there)
             }
             if (h->h_solve[1] != 0.0 || done < kk) break;
         } else {
@@ -869,7 +980,7 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
 
 top_status fetch_residuals(top_solver* h) {
     if (!h->have_residuals) return TOP_OK;
-    CU(cudaMemcpyAsync(h->h_res, h->d_res, (size_t)h->batch * 4 * 8, cudaMemcpyDeviceToHost, h->stream), "D2H residuals");
+    CU(cudaMemcpyAsync(h->h_res.data(), h->d_res, (size_t)h->batch * 4 * 8, cudaMemcpyDeviceToHost, h->stream), "D2H residuals");
     return check_abort(h);   // synchronises
 }
 
@@ -895,6 +1006,7 @@ extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iter
         InKernelSolve iks;
         iks.check_every = h->check_every; iks.rd_sel = rd_idx; iks.adaptive = (h->opt_flags & TOP_RHO_ADAPTIVE) ? 1 : 0;
         iks.tol = tol;
+        if (iks.adaptive) { top_status se = ensure_spectral(h); if (se != TOP_OK) return se; }
         const int64_t it0 = h->iter;
         top_status st = run_sweeps(h, h->max_iter, &iks);
         if (st != TOP_OK) return st;
@@ -947,7 +1059,8 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
     if (rho == h->rho) return TOP_OK;
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     const size_t LS = (size_t)h->stride;
-    CU(refresh_operator(h, rho), "operator refresh launch");      // on the device, from the spectral data: no host work
+    { top_status se = ensure_spectral(h); if (se != TOP_OK) return se; }      // first change of rho: build W, lambda (host, once)
+    CU(refresh_operator(h, rho), "operator refresh launch");      // on the device, from the spectral data
     RescaleParams r;
     r.u = h->d_u; r.qp = h->d_qp; r.qn = h->d_qn; r.wv = h->d_wv; r.wa = h->d_wa;
     r.count = 3 * (long long)LS; r.ratio = h->rho / rho;
@@ -1008,7 +1121,7 @@ extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, do
                 for (int r = 0; r < 2 * s; ++r)
                     for (int d = 0; d < dims; ++d) {
                         double v = buf[(size_t)d * LS + g * LANES + r];
-                        if (f == "z" && r % s == 0) v += h->origin[(size_t)d * h->nseg_pad + g];   // local frame -> global
+                        if (f == "z" && r % s == 0) v += h->h_wp[((size_t)b * (N + 1) + i) * dims + d];   // local frame (origin p_{i-1}) -> global
                         if (f == "u") out[((g * 2 * s) + r) * dims + d] = v;
                         else if (r < s) out[(((size_t)b * (N + 1) + i) * s + r) * dims + d] = v;
                         else if (i == N - 1) out[(((size_t)b * (N + 1) + N) * s + (r - s)) * dims + d] = v;
@@ -1045,9 +1158,10 @@ struct SnapshotHeader {
     int64_t nseg, stride, iter;
     int32_t s, dims, dtype, batch;
     uint32_t kflags, have_residuals;
+    uint32_t wp_mode, N;
     double rho;
 };
-constexpr uint64_t SNAP_MAGIC = 0x544f50534e415031ull;     // "TOPSNAP1"
+constexpr uint64_t SNAP_MAGIC = 0x544f50534e415032ull;     // "TOPSNAP2"
 // the device arrays that make up an iterate, in snapshot order (null ones are skipped)
 int snapshot_fields(top_solver* h, void** out) {
     void* all[] = {h->d_zt, h->d_u, h->d_qp, h->d_qn, h->d_phv, h->d_wv, h->d_pha, h->d_wa, h->d_chat};
@@ -1073,6 +1187,7 @@ extern "C" TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, s
     std::memset(&hd, 0, sizeof hd);
     hd.magic = SNAP_MAGIC; hd.nseg = h->nseg; hd.stride = h->stride; hd.iter = h->iter; hd.s = h->s; hd.dims = h->dims;
     hd.dtype = h->dtype; hd.batch = h->batch; hd.kflags = h->kflags; hd.have_residuals = h->have_residuals ? 1u : 0u; hd.rho = h->rho;
+    hd.wp_mode = h->wp_mode; hd.N = (uint32_t)h->N;
     unsigned char* o = static_cast<unsigned char*>(host_buf);
     std::memcpy(o, &hd, sizeof hd); o += sizeof hd;
     void* f[9];
@@ -1089,7 +1204,8 @@ extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* ho
     SnapshotHeader hd;
     std::memcpy(&hd, host_buf, sizeof hd);
     if (hd.magic != SNAP_MAGIC || hd.nseg != h->nseg || hd.stride != h->stride || hd.s != h->s || hd.dims != h->dims ||
-        hd.dtype != h->dtype || hd.batch != h->batch || hd.kflags != h->kflags || !(hd.rho > 0))
+        hd.dtype != h->dtype || hd.batch != h->batch || hd.kflags != h->kflags || hd.wp_mode != h->wp_mode ||
+        hd.N != (uint32_t)h->N || !(hd.rho > 0))
         return fail(h, TOP_E_INVALID, "top_snapshot_restore: the snapshot belongs to a different problem");
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     const unsigned char* o = static_cast<const unsigned char*>(host_buf) + sizeof hd;
@@ -1098,11 +1214,17 @@ extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* ho
     const size_t fb = 3 * (size_t)h->stride * real_bytes(h);
     for (int i = 0; i < n; ++i) { CU(cudaMemcpyAsync(f[i], o, fb, cudaMemcpyHostToDevice, h->stream), "H2D snapshot"); o += fb; }
     CU(cudaMemcpyAsync(h->d_res, o, (size_t)h->batch * 4 * 8, cudaMemcpyHostToDevice, h->stream), "H2D snapshot");
-    if (hd.rho != h->rho) { CU(refresh_operator(h, hd.rho), "operator refresh launch"); h->rho = hd.rho; }
+    if (hd.rho != h->rho) {
+        top_status se = ensure_spectral(h);
+        if (se != TOP_OK) return se;
+        CU(refresh_operator(h, hd.rho), "operator refresh launch");
+        h->rho = hd.rho;
+    }
+    CU(cudaMemsetAsync(h->d_abort, 0, sizeof(int), h->stream), "cudaMemsetAsync");      // a restored iterate starts with a clean abort flag
     CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
     h->iter = hd.iter;
     h->have_residuals = hd.have_residuals != 0;
-    if (!h->have_residuals) for (int i = 0; i < h->batch * 4; ++i) h->h_res[i] = std::numeric_limits<double>::quiet_NaN();
+    if (!h->have_residuals) std::fill(h->h_res.begin(), h->h_res.end(), std::numeric_limits<double>::quiet_NaN());
     return TOP_OK;
 }
 
@@ -1128,10 +1250,10 @@ extern "C" TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dty
     int sms = 0, smem = 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
         cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) { cudaGetLastError(); return -1; }
-    const uint32_t kf = constrained ? (KF_BOX | KF_VEL | KF_ACC) : 0;
-    (void)kf;
-    return (int64_t)sms * std::max(max_segs_per_cta((int)dtype, s, constrained != 0, 8, false, (size_t)smem - 1024),
-                                   max_segs_per_cta((int)dtype, s, constrained != 0, 4, false, (size_t)smem - 1024));
+    // the same rule top_create applies (kernel family of a long chain, shared-memory reserve)
+    const int lanes = 4;
+    const bool mma = dtype == TOP_F64;
+    return (int64_t)sms * max_segs_per_cta((int)dtype, s, constrained != 0, lanes, mma, (size_t)smem - 8192);
 }
 
 extern "C" TOP_API double top_fma_peak(int32_t device, top_dtype dtype, int32_t reps, void* cuda_stream) {
@@ -1202,10 +1324,7 @@ extern "C" TOP_API top_status top_destroy(top_solver* h) {
     if (!h) return TOP_OK;
     cudaSetDevice(h->device);
     cudaStreamSynchronize(h->stream);
-    for (void* p : h->allocs) cudaFree(p);
-    if (h->h_res) cudaFreeHost(h->h_res);
-    if (h->h_abort) cudaFreeHost(h->h_abort);
-    if (h->h_solve) cudaFreeHost(h->h_solve);
+    if (h->arena) cudaFree(h->arena);
     cudaGetLastError();
     delete h;
     return TOP_OK;

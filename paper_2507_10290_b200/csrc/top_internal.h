@@ -107,6 +107,29 @@ struct RefreshParams {
     double rho;
 };
 cudaError_t launch_refresh_operator(const RefreshParams& p, cudaStream_t st);
+// Init of Alg. 1 (PAPER.md:L270 line 1, L301; reading A9) on the device: from the caller's arrays (uploaded as they are)
+// and the per-segment operator rows, every per-lane constant and iterate 0.
+struct InitParams {
+    // the caller's arrays (device copies)
+    const double* waypoints;      // [batch][N+1][dims]
+    const double* durations;      // [batch][N]
+    const double* box_lo;         // [batch][N][dims] or null
+    const double* box_hi;
+    const double* start_derivs;   // [batch][s-1][dims] or null = rest
+    const double* end_derivs;
+    // column 1 of the Gram matrix G of the penalty rows (G e_1 = sum_k T^-2k gc1[k] + 2 ge1[0] + T^-2 ge1[1] + T^-4 ge1[2],
+    // the enabled blocks only): constants per s, the T weights are applied per segment
+    double gc1[4][MAXN], ge1[3][MAXN];
+    const double* Pm;             // [MAXN][stride] rho Pm^ rows (host precompute)
+    // outputs
+    double *c0, *g0, *dp, *origin;
+    void *invTk, *Tpow, *invT, *lohi, *zoff, *zt, *chat, *qp, *qn, *phv;
+    uint8_t* segflags;
+    long long stride, nseg_pad, nseg;
+    int N, batch, s, dims, hard, has_box, has_vel, has_acc;
+    double vmax;
+};
+cudaError_t launch_init(const InitParams& p, int dtype, cudaStream_t st);
 // duals *= ratio after a change of rho: u, w (both balls), and the negative part of the Moreau values q (= -v)
 struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; };
 cudaError_t launch_rescale_duals(const RescaleParams& p, int dtype, cudaStream_t st);

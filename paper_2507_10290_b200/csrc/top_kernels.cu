@@ -1017,6 +1017,117 @@ __global__ void refresh_operator_kernel(const RefreshParams p) {
     }
 }
 
+// Init of Alg. 1 (PAPER.md:L270 line 1; reading A9), one thread per (segment, lane): the per-lane constants of the sweep
+// (powers of T, segment-local frame, box in the local frame, c0^ from the operator rows) and iterate 0: C0 = chord at
+// constant speed, z0_j = (p_j, mean of the adjacent chord velocities, 0..), z_0 and z_N = the given end states
+// (Eq. 2c), duals 0, slacks = max(0, .) of the chord samples, phi = projection of the chord velocity.
+template <typename Real>
+__global__ void init_problem_kernel(const InitParams p) {
+    const long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= p.nseg * LANES) return;
+    const long long g = idx / LANES;
+    const int lane = (int)(idx % LANES);
+    const int N = p.N, s = p.s, n = 2 * s, dims = p.dims;
+    const long long b = g / N, i = g % N;
+    auto wp = [&](long long j, int d) -> double { return d < dims ? p.waypoints[((size_t)b * (N + 1) + j) * dims + d] : 0.0; };
+    const double T = p.durations[g];
+    // segment-local frame: origin o_i = p_{i-1}; every position-like quantity of segment i is stored relative to it
+    double org[3], dp[3];
+    for (int d = 0; d < 3; ++d) { org[d] = wp(i, d); dp[d] = wp(i + 1, d) - org[d]; }
+    const long long NP = p.nseg_pad, LS = p.stride;
+    if (lane == 0) {
+        p.segflags[g] = (uint8_t)((i == 0 ? SEG_FIRST : 0) | (i == N - 1 ? SEG_LAST : 0));
+        static_cast<Real*>(p.invT)[g] = (Real)(1.0 / T);
+        static_cast<Real*>(p.invT)[NP + g] = (Real)(1.0 / (T * T));
+        for (int d = 0; d < 3; ++d) {
+            p.origin[d * NP + g] = org[d];
+            p.dp[d * NP + g] = (p.hard && d < dims) ? dp[d] : 0.0;
+            static_cast<Real*>(p.lohi)[d * NP + g] = (Real)((p.has_box && d < dims) ? p.box_lo[g * dims + d] - org[d] : -1.0);
+            static_cast<Real*>(p.lohi)[(3 + d) * NP + g] = (Real)((p.has_box && d < dims) ? p.box_hi[g * dims + d] - org[d] : 1.0);
+        }
+    }
+    // G e_1 of this segment, then c0^ = c_chord - (rho Pm^)(G c_chord) with c_chord = e_1 dp in the local frame (HARD mode)
+    const double iT2 = 1.0 / (T * T);
+    double gcol1[MAXN];
+    {
+        double w = 1.0;
+        for (int a = 0; a < MAXN; ++a) gcol1[a] = 0.0;
+        for (int k = 0; k < s; ++k) { for (int a = 0; a < n; ++a) gcol1[a] += w * p.gc1[k][a]; w *= iT2; }
+        for (int a = 0; a < n; ++a) {
+            if (p.has_box) gcol1[a] += 2.0 * p.ge1[0][a];
+            if (p.has_vel) gcol1[a] += iT2 * p.ge1[1][a];
+            if (p.has_acc) gcol1[a] += iT2 * iT2 * p.ge1[2][a];
+        }
+    }
+    double pg = 0.0;
+    for (int bb = 0; bb < MAXN; ++bb) pg += p.Pm[bb * LS + idx] * gcol1[bb];
+    for (int d = 0; d < 3; ++d) {
+        p.g0[d * LS + idx] = (p.hard && d < dims) ? gcol1[lane] * dp[d] : 0.0;
+        p.c0[d * LS + idx] = (p.hard && d < dims) ? ((lane == 1 ? dp[d] : 0.0) - pg * dp[d]) : 0.0;
+    }
+    double Tp = 1.0;
+    for (int q = 0; q < lane; ++q) Tp *= T;
+    static_cast<Real*>(p.Tpow)[idx] = (Real)Tp;
+    // a neighbour's position row arrives in the neighbour's frame: shift it into this segment's frame
+    for (int d = 0; d < 3; ++d) {
+        double zo = 0.0;
+        if (d < dims) {
+            if (lane == 0 && i > 0) zo = wp(i - 1, d) - wp(i, d);       // o_{i-1} - o_i
+            if (lane == s && i < N - 1) zo = dp[d];                     // o_{i+1} - o_i
+        }
+        static_cast<Real*>(p.zoff)[d * LS + idx] = (Real)zo;
+    }
+    double itk = 0.0;
+    if (lane < n) {
+        const int k = lane % s;
+        double tk = 1.0;
+        for (int q = 0; q < k; ++q) tk *= T;
+        itk = 1.0 / tk;
+    }
+    static_cast<Real*>(p.invTk)[idx] = (Real)itk;
+    for (int d = 0; d < 3; ++d) {
+        // z0: position = waypoint; velocity = mean of the adjacent chord velocities; higher orders 0; z_0, z_N given
+        double z = 0.0;
+        if (lane < n && d < dims) {
+            const int k = lane % s;
+            const long long j = lane < s ? i : i + 1;
+            if (k == 0) z = wp(j, d) - org[d];
+            else if (j == 0) z = p.start_derivs ? p.start_derivs[((size_t)b * (s - 1) + (k - 1)) * dims + d] : 0.0;
+            else if (j == N) z = p.end_derivs ? p.end_derivs[((size_t)b * (s - 1) + (k - 1)) * dims + d] : 0.0;
+            else if (k == 1) {
+                const double vl = (wp(j, d) - wp(j - 1, d)) / p.durations[b * N + j - 1];
+                const double vr = (wp(j + 1, d) - wp(j, d)) / p.durations[b * N + j];
+                z = 0.5 * (vl + vr);
+            }
+        }
+        static_cast<Real*>(p.zt)[d * LS + idx] = (Real)z;
+        // C0 = chord at constant speed: c^_0 = 0 (local frame), c^_1 = p_i - p_{i-1}
+        static_cast<Real*>(p.chat)[d * LS + idx] = (Real)((d < dims && lane == 1) ? dp[d] : 0.0);
+    }
+    // samples of the chord: slack = max(0, .), phi = projection of the chord velocity, duals 0
+    const double tau = (double)(lane + 1) / (double)(MS + 1);
+    double V0[3] = {0, 0, 0};
+    for (int d = 0; d < 3; ++d) {
+        if (d < dims) V0[d] = dp[d] / T;
+        if (p.has_box) {
+            double a = 1.0, c = 1.0;
+            if (d < dims) {
+                const double P0 = tau * dp[d];
+                a = fmax(0.0, (p.box_hi[g * dims + d] - org[d]) - P0);
+                c = fmax(0.0, P0 - (p.box_lo[g * dims + d] - org[d]));
+            }
+            static_cast<Real*>(p.qp)[d * LS + idx] = (Real)a;
+            static_cast<Real*>(p.qn)[d * LS + idx] = (Real)c;
+        }
+    }
+    if (p.has_vel) {
+        const double n2 = V0[0] * V0[0] + V0[1] * V0[1] + V0[2] * V0[2];
+        double sc = 1.0;
+        if (n2 > p.vmax * p.vmax) sc = p.vmax / sqrt(n2);
+        for (int d = 0; d < 3; ++d) static_cast<Real*>(p.phv)[d * LS + idx] = (Real)(sc * V0[d]);
+    }
+}
+
 // scaled duals after rho_old -> rho_new (reading A16): u, w_v, w_a *= ratio; box: v = max(0,-q) *= ratio, s unchanged
 template <typename Real>
 __global__ void rescale_duals_kernel(const RescaleParams p) {
@@ -1172,6 +1283,15 @@ cudaError_t launch_refresh_operator(const RefreshParams& p, cudaStream_t st) {
     const long long n = p.nseg * LANES;
     if (n == 0) return cudaSuccess;
     refresh_operator_kernel<<<(int)((n + 127) / 128), 128, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_init(const InitParams& p, int dtype, cudaStream_t st) {
+    const long long n = p.nseg * LANES;
+    if (n == 0) return cudaSuccess;
+    const int blocks = (int)((n + 127) / 128);
+    if (dtype == 0) init_problem_kernel<double><<<blocks, 128, 0, st>>>(p);
+    else init_problem_kernel<float><<<blocks, 128, 0, st>>>(p);
     return cudaGetLastError();
 }
 

@@ -24,7 +24,7 @@ TOP_RHO_ADAPTIVE = 64
 TOP_KERNEL_NO_MMA = 128
 SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
-EXPORTS = ["top_create", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
+EXPORTS = ["top_create", "top_reset", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
            "top_snapshot_bytes", "top_snapshot_save", "top_snapshot_restore", "top_iteration", "top_set_rho", "top_get_rho", "top_launch_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
            "top_destroy", "top_last_error"]
 
@@ -66,6 +66,8 @@ def lib():
     L.top_create.argtypes = [ctypes.POINTER(vp), ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
                              ctypes.c_int, dp, dp, dp, dp, ctypes.POINTER(_Constraints), ctypes.c_double,
                              ctypes.POINTER(_Options)]
+    L.top_reset.restype = ctypes.c_int
+    L.top_reset.argtypes = [vp, dp, dp, dp, dp, ctypes.POINTER(_Constraints), ctypes.c_double]
     L.top_iterate.restype = ctypes.c_int
     L.top_iterate.argtypes = [vp, ctypes.c_int64]
     L.top_solve.restype = ctypes.c_int
@@ -206,6 +208,25 @@ class TopSolver:
             self.close()
         except Exception:
             pass
+
+    def reset(self, waypoints, durations, rho, box_lo=None, box_hi=None, vmax=0.0, amax=0.0, start_derivs=None,
+              end_derivs=None):
+        """top_reset: a new problem of the same shape on this handle (no allocation)."""
+        wp = np.asarray(waypoints, dtype=np.float64)
+        T = np.asarray(durations, dtype=np.float64)
+        if wp.ndim == 2:
+            wp, T = wp[None], T[None]
+            box_lo = None if box_lo is None else np.asarray(box_lo)[None]
+            box_hi = None if box_hi is None else np.asarray(box_hi)[None]
+            start_derivs = None if start_derivs is None else np.asarray(start_derivs)[None]
+            end_derivs = None if end_derivs is None else np.asarray(end_derivs)[None]
+        wp, T = _f64(wp, (self.batch, self.N + 1, self.dims)), _f64(T, (self.batch, self.N))
+        lo = _f64(box_lo, (self.batch, self.N, self.dims)); hi = _f64(box_hi, (self.batch, self.N, self.dims))
+        sd = _f64(start_derivs, (self.batch, self.s - 1, self.dims)); ed = _f64(end_derivs, (self.batch, self.s - 1, self.dims))
+        cons = _Constraints(self.Ms, _dptr(lo), _dptr(hi), float(vmax), float(amax)) if self.Ms else None
+        self._check(self._L.top_reset(self._h, _dptr(wp), _dptr(T), _dptr(sd), _dptr(ed),
+                                      ctypes.byref(cons) if cons is not None else None, float(rho)))
+        self.durations = T
 
     def iterate(self, k: int):
         self._check(self._L.top_iterate(self._h, int(k)))

@@ -472,3 +472,31 @@ def test_snapshot_restore_resumes_bit_for_bit():
     with pytest.raises(top.TopError) as e:
         other.restore(snap)
     assert e.value.status == top.TOP_E_INVALID
+
+
+def test_reset_reuses_the_handle_for_a_new_problem():
+    """top_reset: a new problem of the same shape on an existing handle (re-planning): iterates equal those of a fresh
+    solver bit for bit, the constraint selection is checked, an adaptive solve after a reset works."""
+    w1 = W.small_constrained(N=53, s=4, acc=True, seed=11)
+    w2 = W.small_constrained(N=53, s=4, acc=True, seed=12)
+    sol = top.from_workload(w1, segs_per_cta=8)
+    sol.iterate(40)
+    sol.reset(w2.waypoints, w2.durations, 7.0, box_lo=w2.box_lo, box_hi=w2.box_hi, vmax=2.5, amax=4.0)
+    assert sol.iteration == 0 and sol.rho == 7.0
+    w2.rho, w2.vmax, w2.amax = 7.0, 2.5, 4.0
+    fresh = top.from_workload(w2, segs_per_cta=8)
+    o = make_oracle(w2)
+    for k in (0, 1, 30):
+        sol.iterate(k); fresh.iterate(k); o.sweep(k, 1)
+        for f in ("z", "u", "s_pos", "v_neg", "phi_v", "w_a"):
+            assert np.array_equal(sol.state(f), fresh.state(f)), (k, f)
+        assert np.array_equal(sol.coeffs(), fresh.coeffs())
+        check_fields(field_errors(sol, [o], w2), "after reset, sweep %d" % k)
+    with pytest.raises(top.TopError) as e:      # another constraint selection needs another solver
+        sol.reset(w2.waypoints, w2.durations, 7.0, box_lo=w2.box_lo, box_hi=w2.box_hi, vmax=2.5, amax=0.0)
+    assert e.value.status == top.TOP_E_INVALID
+    # rho changes after a reset go through the (lazily built) spectral form of the NEW problem
+    sol.set_rho(3.0); o.set_rho(3.0)
+    sol.iterate(5); o.sweep(5, 1)
+    check_fields(field_errors(sol, [o], w2), "after reset and set_rho")
+    sol.close(); fresh.close()

@@ -50,7 +50,7 @@ def test_validation_happens_before_the_device_is_needed():
         dict(waypoints=wp, durations=T, s=3, rho=0.0),                       # rho
         dict(waypoints=wp, durations=np.array([1.0, -1.0]), s=3, rho=1.0),   # T <= 0
         dict(waypoints=wp * np.nan, durations=T, s=3, rho=1.0),              # non-finite
-        dict(waypoints=wp, durations=T, s=3, rho=1.0, samples=4, vmax=1.0),  # samples
+        dict(waypoints=wp, durations=T, s=3, rho=1.0, samples=-2, vmax=1.0), # samples < 0
         dict(waypoints=wp, durations=T, s=3, rho=1.0, samples=8, box_lo=np.ones((2, 3)), box_hi=np.zeros((2, 3))),
         dict(waypoints=wp, durations=T, s=3, rho=1.0, segs_per_cta=6),
         dict(waypoints=wp, durations=T, s=3, rho=1.0, lanes=3),
@@ -62,6 +62,10 @@ def test_validation_happens_before_the_device_is_needed():
         with pytest.raises(top.TopError) as e:
             top.TopSolver(**kw)
         assert e.value.status == top.TOP_E_INVALID, kw
+    # a valid request this build does not run (the paper's M is a parameter; the kernels evaluate at 8)
+    with pytest.raises(top.TopError) as e:
+        top.TopSolver(waypoints=wp, durations=T, s=3, rho=1.0, samples=4, vmax=1.0)
+    assert e.value.status == top.TOP_E_UNSUPPORTED
 
 
 def test_no_cpu_fallback_without_a_device():
