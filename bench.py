@@ -35,6 +35,9 @@ UNIT = "segment-iterations/s"
 # rhs assembly + operator apply + evaluation + projections + consensus/dual updates (residuals excluded: they
 # are computed on the last sweep of a launch only).
 FLOPS_PER_SEG_SWEEP = {"cfg4": 4260.0, "cfg2": 3330.0, "cfg5": 3330.0, "cfg3": 740.0, "cfg1": 740.0}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the sweep kernel on config 4 with the default plan
+PROFILED_TRAFFIC_CFG4 = 27850240
+PROFILED_TRAFFIC_SOURCE = "profiles/r2_final_cfg4_ncu_summary.md (ncu --set full, one launch)"
 
 
 def make_workload(name: str, rank: int = 0):
@@ -98,20 +101,59 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def cpu_model() -> str:
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+ORACLE_FLAGS = "gcc -O2 -fPIC -shared -fopenmp (oracle/top_oracle.py build())"
+
+
 def oracle_rate(w, seconds: float, threads: int):
     """Oracle (as it stands) on the host cores: a bounded number of sweeps of trajectory 0 of the workload."""
     from oracle.top_oracle import Oracle
     o = Oracle(w.waypoints[0], w.durations[0], w.s, w.rho, samples=w.samples,
                box_lo=None if w.box_lo is None else w.box_lo[0], box_hi=None if w.box_hi is None else w.box_hi[0],
                vmax=w.vmax, amax=w.amax)
-    if threads <= 0:
-        threads = min(o.max_threads(), os.cpu_count() or 1)
+    if threads <= 0:       # all host cores (not the OpenMP runtime's current setting: an earlier 1-thread run lowers that)
+        threads = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
     o.sweep(2, threads)                                            # thread start-up, page faults
     t0 = time.perf_counter(); o.sweep(10, threads); probe = (time.perf_counter() - t0) / 10
     sweeps = int(max(3, min(2000000, seconds / max(probe, 1e-9))))
     t0 = time.perf_counter(); o.sweep(sweeps, threads); dt = time.perf_counter() - t0
     return {"value": w.N * sweeps / dt, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": "%d sweeps of trajectory 0 (N=%d) of %s, %.1f s, gcc -O2 -fopenmp" % (sweeps, w.N, w.name, dt)}, sweeps, dt
+            "sample": "%d sweeps of trajectory 0 (N=%d) of %s, %.1f s" % (sweeps, w.N, w.name, dt),
+            "cpu_model": cpu_model(), "flags": ORACLE_FLAGS}, sweeps, dt
+
+
+def cpu_baseline_both(w, seconds: float, threads: int):
+    """the oracle single-threaded and on all host cores (OpenMP over segments), side by side."""
+    allc, _, _ = oracle_rate(w, seconds * 0.6, threads)
+    one, _, _ = oracle_rate(w, seconds * 0.4, 1)
+    allc["single_thread"] = {"value": one["value"], "unit": UNIT, "cores": 1, "sample": one["sample"]}
+    return allc
+
+
+def roofline_entry(top, name, w, waves, ms_per_call, sweeps, peaks, sms, sm_mhz, traffic=None, traffic_source=None):
+    """ALU roofline of one timed top_iterate call: achieved = algorithmic FLOPs per launch / launch time,
+    peak = the FMA rate of the arithmetic type measured in this run (top_fma_peak)."""
+    fl = FLOPS_PER_SEG_SWEEP.get(name.replace("f32", ""))
+    if fl is None:
+        return None
+    dt_name = "f64" if w.dtype == "f64" else "f32"
+    peak = peaks[dt_name]
+    ach = fl * w.batch * w.N * sweeps / waves / (ms_per_call * 1e-3 / waves)
+    return {"bound": "alu", "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s", "frac": ach / peak,
+            "traffic": traffic, "traffic_source": traffic_source,
+            "peak_source": "measured in this run: top_fma_peak (%s FMA loop, all SMs)" % dt_name,
+            "flops_per_segment_sweep": fl,
+            # unit count x clock (DESIGN.md 5.4): SMs x 64 fp64 (128 fp32) FMA/clk x 2 x SM clock
+            "peak_derived": sms * (64 if dt_name == "f64" else 128) * 2 * sm_mhz * 1e6 / 1e12}
 
 
 def aggregate_over_ranks(total_ms: float, units: float, world: int, device="cpu"):
@@ -190,6 +232,72 @@ def run_fig5(args, local_rank):
                       "s": 3, "rho": 10.0, "tolerance": "N*0.05 (PAPER.md:L288)", "check_every": 8, "M": M, "rows": rows}))
 
 
+def run_latency(args, local_rank):
+    """Per-sweep latency of the small configs (the paper's regime: tens to a thousand segments) and where it goes:
+    the same chain cut into fewer / more CTAs, the three synchronisation modes, both kernel families, and -- as the
+    exchange-free reference -- ONE CTA running a chain of the per-CTA size with the same constraint sets
+    (north_star: "launch and sync overhead per iteration")."""
+    import torch
+    from paper_2507_10290_b200 import build as top_build
+    from paper_2507_10290_b200 import top
+    top_build.build()
+    torch.cuda.set_device(local_rank)
+    stream = torch.cuda.current_stream()
+
+    def time_us(w, k=2000, **kw):
+        sol = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, dtype="f64", **kw)
+        sol.iterate(k); torch.cuda.synchronize()
+        best = 1e30
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); sol.iterate(k); e1.record(stream); torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1))
+        li = sol.launch_info()
+        sol.close()
+        return 1e3 * best / k, li
+
+    rows = []
+    makers = {"cfg1": lambda N=None: W.config1(), "cfg2": lambda N=None: W.config2(N=N or 100), "cfg3": lambda N=None: W.config3(N=N or 1000)}
+    for name in ("cfg1", "cfg2", "cfg3"):
+        w = makers[name]()
+        for lanes in (8, 4):
+            for segs in (0, 4, 8, 16, 32, 64):
+                if segs and (segs * 148 < w.N or (lanes == 8 and segs > 64)):
+                    continue
+                for sync in (("auto", "neighbour", "grid") if segs == 0 else ("auto",)):
+                    try:
+                        us, li = time_us(w, lanes=lanes, segs_per_cta=segs, sync=sync)
+                    except top.TopError:
+                        continue
+                    rows.append({"config": name, "N": w.N, "lanes": lanes, "kernel": "mma" if lanes == 4 else "8-lane", "sync": sync,
+                                 "segs_per_cta": li["segs_per_cta"], "ctas": li["ctas"], "threads": li["threads"], "us_per_sweep": us})
+            # exchange-free reference: one CTA, a chain as long as one CTA's share of the default plan
+            if name != "cfg1":
+                for per in (8, 16, 32, 64):
+                    wr = makers[name](per)
+                    try:
+                        us, li = time_us(wr, lanes=lanes, segs_per_cta=per)
+                    except top.TopError:
+                        continue
+                    if li["ctas"] == 1:
+                        rows.append({"config": name + "_single_cta_reference", "N": per, "lanes": lanes, "kernel": "mma" if lanes == 4 else "8-lane",
+                                     "sync": "none (one CTA)", "segs_per_cta": li["segs_per_cta"], "ctas": 1, "threads": li["threads"], "us_per_sweep": us})
+    # launch overhead: an empty-ish launch (1 sweep) against the per-sweep time inside a long launch
+    w = W.config2()
+    sol = top.from_workload(w, device=local_rank, stream=stream.cuda_stream)
+    sol.iterate(10); torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(200):
+        sol.iterate(1)
+    e1.record(stream); torch.cuda.synchronize()
+    per_launch = 1e3 * e0.elapsed_time(e1) / 200
+    sol.close()
+    print(json.dumps({"experiment": "small_config_latency", "unit": "us per sweep", "rows": rows,
+                      "launch_overhead": {"config": "cfg2", "us_per_top_iterate_1": per_launch,
+                                          "note": "one cooperative launch + the residual-reduction launch per call; inside a long launch this cost is paid once"}}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -206,6 +314,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fig5", action="store_true", help="run the Fig. 5 stand-in (time and similarity vs N) instead")
     ap.add_argument("--no-extras", action="store_true", help="skip time-to-eps and the e2e leg")
+    ap.add_argument("--latency", action="store_true", help="per-sweep latency breakdown of the small configs instead")
+    ap.add_argument("--cfg2-eps-cap", type=int, default=60000000, help="sweep cap of the config-2 run to its own 1e-6 (0 = skip)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -217,6 +327,10 @@ def main():
     if args.fig5:
         if rank == 0:
             run_fig5(args, local_rank)
+        return
+    if args.latency:
+        if rank == 0:
+            run_latency(args, local_rank)
         return
 
     import torch
@@ -285,47 +399,57 @@ def main():
            "residuals_after": {k: float(v[0]) for k, v in res.items()}}
 
     if rank == 0:
-        # ---- roofline of the dominant kernel (cadmm_sweeps_kernel): plain FP64/FP32 ALU bound, state on chip
-        fl = FLOPS_PER_SEG_SWEEP.get(args.workload.replace("f32", ""), None)
-        dt_name = "f64" if w.dtype == "f64" else "f32"
-        peak = top.fma_peak(dt_name, reps=5, device=local_rank, stream=stream.cuda_stream)
-        if fl is not None:
-            waves = info["waves"]
-            per_launch_flops = fl * w.batch * w.N * sweeps / waves
-            per_launch_s = (sum(ms) / args.steps) * 1e-3 / waves
-            ach = per_launch_flops / per_launch_s
-            out["roofline"] = {"bound": "alu", "achieved": ach / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
-                               "frac": ach / peak,
-                               # DRAM bytes per launch (read + write) from the committed ncu capture of this command
-                               # (profiles/r1_final_cfg4_ncu_summary.md); independent of the sweep count: state is on chip
-                               "traffic": 27850240 if args.workload == "cfg4" else None,
-                               "peak_source": "measured in this run: top_fma_peak (%s FMA loop, all SMs)" % dt_name,
-                               "flops_per_segment_sweep": fl,
-                               # unit count x clock: 148 SMs x 64 fp64 (128 fp32) FMA/clk x 2 x SM clock
-                               "peak_derived": 148 * (64 if dt_name == "f64" else 128) * 2 * (clocks.get("sm_mhz") or 1965.0) * 1e6 / 1e12}
+        # ---- roofline of the dominant kernel (the persistent sweep kernel): plain FP64/FP32 ALU bound, state on chip
+        props = torch.cuda.get_device_properties(local_rank)
+        sms = props.multi_processor_count
+        sm_mhz = clocks.get("sm_mhz") or clocks.get("sm_max_mhz") or 1965.0
+        peaks = {"f64": top.fma_peak("f64", reps=5, device=local_rank, stream=stream.cuda_stream),
+                 "f32": top.fma_peak("f32", reps=5, device=local_rank, stream=stream.cuda_stream)}
+        # DRAM bytes per launch (read + write) of the committed ncu capture, valid for the library's default plan of
+        # config 4 only (state is on chip: independent of the sweep count)
+        default_plan = args.workload == "cfg4" and args.lanes == 0 and args.segs_per_cta == 0 and args.sync == "auto"
+        rf = roofline_entry(top, args.workload, w, info["waves"], sum(ms) / args.steps, sweeps, peaks, sms, sm_mhz,
+                            traffic=PROFILED_TRAFFIC_CFG4 if default_plan else None,
+                            traffic_source=PROFILED_TRAFFIC_SOURCE if default_plan else None)
+        if rf:
+            out["roofline"] = rf
         peaks_path = os.path.join(ROOT, "MEASURED_PEAKS.json")
         if os.path.exists(peaks_path):
             out["measured_peaks"] = {k: v for k, v in json.load(open(peaks_path)).items() if k in ("hbm_gbs", "sm_max_mhz")}
 
         if not args.no_extras:
-            # ---- e2e: the user's calls with HOST buffers: top_create (H2D) + top_iterate + top_get_coeffs (D2H)
+            # ---- e2e: the user's calls with HOST buffers: top_create (H2D) + top_iterate + top_get_coeffs (D2H) + top_destroy
             torch.cuda.synchronize()
             e2e_t, nrep = 0.0, 3
             h2d = d2h = 0
             for rep in range(nrep + 1):          # rep 0 is an untimed warm-up of the same calls
                 t0 = time.perf_counter()
                 s2 = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync,
-                                       segs_per_cta=args.segs_per_cta)
+                                       segs_per_cta=args.segs_per_cta, lanes=args.lanes)
                 s2.iterate(sweeps)
                 c = s2.coeffs()
-                if rep > 0:
-                    e2e_t += time.perf_counter() - t0
-                h2d = w.waypoints.nbytes + w.durations.nbytes + (0 if w.box_lo is None else w.box_lo.nbytes + w.box_hi.nbytes)
+                h2d = s2.memory_info()["h2d_bytes_per_problem"]      # operator rows + the caller's arrays, as the library copies them
                 d2h = c.nbytes
                 s2.close()
+                if rep > 0:
+                    e2e_t += time.perf_counter() - t0
             out["e2e"] = {"value": float(w.batch * w.N) * sweeps * nrep / e2e_t, "unit": UNIT,
-                          "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                          "what": "top_create(host arrays: validate, fp80 operator precompute, upload) + top_iterate(%d) + top_get_coeffs(host), wall clock" % sweeps}
+                          "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e2e_t / nrep,
+                          "what": "top_create(host arrays: validate, fp80 operator precompute, one H2D copy, init kernel) + top_iterate(%d) + top_get_coeffs(host) + top_destroy, wall clock" % sweeps}
+            # the re-planning form of the same thing: top_reset on a live handle instead of create / destroy
+            s2 = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync,
+                                   segs_per_cta=args.segs_per_cta, lanes=args.lanes)
+            kwr = dict(box_lo=w.box_lo, box_hi=w.box_hi, vmax=w.vmax, amax=w.amax)
+            s2.reset(w.waypoints, w.durations, w.rho, **kwr); s2.iterate(sweeps); s2.coeffs()
+            t0 = time.perf_counter()
+            for rep in range(nrep):
+                s2.reset(w.waypoints, w.durations, w.rho, **kwr)
+                s2.iterate(sweeps)
+                s2.coeffs()
+            e2e_r = time.perf_counter() - t0
+            s2.close()
+            out["e2e_reset"] = {"value": float(w.batch * w.N) * sweeps * nrep / e2e_r, "unit": UNIT, "ms_per_step": 1e3 * e2e_r / nrep,
+                                "what": "top_reset(host arrays) + top_iterate(%d) + top_get_coeffs(host) on a live handle" % sweeps}
             # ---- time-to-eps (BASELINE.json's second figure)
             s3 = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync, check_every=64,
                                    max_iter=200000, segs_per_cta=args.segs_per_cta)
@@ -366,8 +490,11 @@ def main():
                 e0.record(stream); so.iterate(k); so.iterate(k); so.iterate(k); e1.record(stream)
                 torch.cuda.synchronize()
                 msk = e0.elapsed_time(e1) / 3
+                li = so.launch_info()
                 others[wo.name] = {"segment_iterations_per_s": wo.batch * wo.N * k / (msk * 1e-3), "sweeps": k,
-                                   "us_per_sweep_per_wave": 1e3 * msk / k / so.launch_info()["waves"], "dtype": wo.dtype}
+                                   "us_per_sweep_per_wave": 1e3 * msk / k / li["waves"], "dtype": wo.dtype,
+                                   "ctas": li["ctas"], "threads": li["threads"], "waves": li["waves"],
+                                   "roofline": roofline_entry(top, name, wo, li["waves"], msk, k, peaks, sms, sm_mhz)}
                 so.close()
             # a chain three times the on-chip capacity: streamed in pieces with halos (temporal blocking)
             wl = W.config4(seed=1004 + rank, N=30000)
@@ -395,8 +522,25 @@ def main():
                               "r_p": float(ra["r_p"][0]), "r_d": float(ra["r_d"][0])}
                 sa.close()
             out["paper_tolerance_cfg2"] = {"eps": "N*0.05", "check_every": 1, **reg}
+            # ---- config 2 to ITS OWN stopping figure (BASELINE.json configs[1]: "until primal and dual residuals < 1e-6";
+            # Eq. 23): one launch, the stop rule runs inside the kernel every 64 sweeps
+            if args.cfg2_eps_cap > 0:
+                s5 = top.from_workload(w2, device=local_rank, stream=stream.cuda_stream, check_every=64, max_iter=args.cfg2_eps_cap)
+                torch.cuda.synchronize(); t0 = time.perf_counter()
+                ok5, it5 = s5.solve(1e-6)
+                torch.cuda.synchronize(); dt5 = time.perf_counter() - t0
+                r5 = s5.residuals()
+                s5.close()
+                entry = {"eps": 1e-6, "rho": w2.rho, "check_every": 64, "converged": bool(ok5), "sweeps": int(it5.max()), "seconds": dt5,
+                         "r_p": float(r5["r_p"][0]), "r_d": float(r5["r_d"][0]),
+                         "note": "ok" if ok5 else "cap reached (--cfg2-eps-cap %d)" % args.cfg2_eps_cap}
+                if not args.no_cpu_baseline:
+                    o1, _, _ = oracle_rate(w2, 3.0, 1)
+                    entry["oracle_single_thread_seconds_extrapolated"] = int(it5.max()) * w2.N / o1["value"]
+                    entry["oracle_note"] = "extrapolated: the GPU's sweep count x the oracle's measured seconds per sweep (1 thread, %s)" % o1["sample"]
+                out["time_to_eps_cfg2"] = entry
         if not args.no_cpu_baseline and world == 1:
-            out["cpu_baseline"], _, _ = oracle_rate(w, args.oracle_seconds, args.oracle_threads)
+            out["cpu_baseline"] = cpu_baseline_both(w, args.oracle_seconds, args.oracle_threads)
         print(json.dumps(out))
     sol.close()
     if world > 1:

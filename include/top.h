@@ -217,9 +217,14 @@ TOP_API int64_t top_iteration(const top_solver* h);
 TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas, int32_t* threads, int32_t* segs_per_cta,
                            int32_t* smem_bytes, int32_t* waves, int64_t* launches);
 
+/* Memory facts of this solver; any pointer may be NULL: bytes of its (single) device allocation, and the bytes that
+ * top_create / top_reset copy host-to-device per problem (the x-update operator rows + the caller's arrays). */
+TOP_API top_status top_memory_info(const top_solver* h, int64_t* device_bytes, int64_t* h2d_bytes_per_problem);
+
 /* Largest N (segments of ONE trajectory) the persistent kernel can hold ON CHIP on the given device (longer
  * trajectories are streamed)
- * (-1 = current) for this s / dtype / constraint selection; < 0 on error. */
+ * (-1 = current) for this s / dtype / constraint selection -- computed by the rule top_create applies to a long chain
+ * (4 lanes per segment, same shared-memory reserve); < 0 on error. */
 TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dtype, int32_t constrained);
 
 /* top_fma_peak -- measured plain-ALU FMA throughput of the device in FLOP/s (2 per FMA) for the given

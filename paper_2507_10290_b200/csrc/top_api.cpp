@@ -1243,6 +1243,13 @@ extern "C" TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas
     return TOP_OK;
 }
 
+extern "C" TOP_API top_status top_memory_info(const top_solver* h, int64_t* device_bytes, int64_t* h2d_bytes_per_problem) {
+    if (!h) return TOP_E_INVALID;
+    if (device_bytes) *device_bytes = (int64_t)h->arena_bytes;
+    if (h2d_bytes_per_problem) *h2d_bytes_per_problem = (int64_t)h->upload_bytes;
+    return TOP_OK;
+}
+
 extern "C" TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dtype, int32_t constrained) {
     if ((s != 3 && s != 4) || (dtype != TOP_F64 && dtype != TOP_F32)) return -1;
     int dev = device;

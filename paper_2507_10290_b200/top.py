@@ -25,7 +25,7 @@ TOP_KERNEL_NO_MMA = 128
 SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
 EXPORTS = ["top_create", "top_reset", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
-           "top_snapshot_bytes", "top_snapshot_save", "top_snapshot_restore", "top_iteration", "top_set_rho", "top_get_rho", "top_launch_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
+           "top_snapshot_bytes", "top_snapshot_save", "top_snapshot_restore", "top_iteration", "top_set_rho", "top_get_rho", "top_launch_info", "top_memory_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
            "top_destroy", "top_last_error"]
 
 
@@ -92,6 +92,8 @@ def lib():
     L.top_iteration.argtypes = [vp]
     L.top_launch_info.restype = ctypes.c_int
     L.top_launch_info.argtypes = [vp, i32p, i32p, i32p, i32p, i32p, ctypes.POINTER(ctypes.c_int64)]
+    L.top_memory_info.restype = ctypes.c_int
+    L.top_memory_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
     L.top_capacity.restype = ctypes.c_int64
     L.top_capacity.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int, ctypes.c_int32]
     L.top_fma_peak.restype = ctypes.c_double
@@ -290,6 +292,11 @@ class TopSolver:
         d = {k: x.value for k, x in zip(keys, v)}
         d["launches"] = n.value
         return d
+
+    def memory_info(self):
+        a, b = ctypes.c_int64(), ctypes.c_int64()
+        self._check(self._L.top_memory_info(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return {"device_bytes": a.value, "h2d_bytes_per_problem": b.value}
 
 
 def from_workload(w, b0: int = 0, b1: Optional[int] = None, **kw) -> TopSolver:
