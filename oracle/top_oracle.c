@@ -33,6 +33,11 @@
  *       duals 0; S = max(0,.) of the chord samples; Phi = projection of the chord velocity.
  *   A10 sample times t_ij = T_i * j/(Ms+1), j = 1..Ms.
  *   A11 box corridor: Ao = [E0; -E0] per axis, b = [hi; -lo].
+ *   A11p general polytope corridor (Eq. 7-10): K half-spaces a_k'p <= b_k per
+ *       segment, applied to the position at each of the Ms sample times: row (j,k) of Ao is
+ *       kron(beta_0(t_ij)', a_k') (Ao is MK x m(d+1) as printed), one slack and one scaled dual per (sample, plane).
+ *       The flat dimensions are then coupled: H is (n m) x (n m) and is formed and inverted as such (no
+ *       per-dimension shortcut in the oracle).
  *   A15 ball projection scale = min(1, bound/||y||), ||y|| = 0 -> scale 1.
  *   A18 a single rho for every penalty.   A19 cost c'Qc without 1/2  =>  2Q in H.
  *
@@ -90,6 +95,12 @@ typedef struct {
     real_t *u;      /* [N][2s][m]  */
     real_t *Sp, *Sn, *Vp, *Vn;   /* [N][Ms][m] slack / dual of the box, + and - side */
     real_t *PhiV, *WV, *PhiA, *WA; /* [N][Ms][m] */
+    /* general polytope corridor (reading A11p): K planes per segment, coupled (n m) x (n m) operator */
+    int K, has_poly;
+    real_t *planes; /* [N][K][m+1]: normal a_k (m), offset b_k */
+    real_t *PmF;    /* [N][nm][nm]  coupled operator, coefficient index a*m + d */
+    real_t *c0F;    /* [N][nm]      */
+    real_t *Spl, *Vpl; /* [N][Ms][K] slack / scaled dual per (sample, plane) */
     real_t *part;   /* [N][4] residual partial sums */
     double rp, rd, rd_norm, rp_gap;
     int64_t iter;
@@ -156,6 +167,39 @@ static int spd_inverse(int n, const pre_t *A, pre_t *Ainv) {
     return 0;
 }
 
+#define FMAX 24  /* n*m <= 8*3 */
+/* inverse of an SPD q x q matrix, q <= FMAX: Jacobi equilibration + Cholesky in pre_t. returns 0 on success */
+static int spd_inverse_big(int q, const pre_t *A, pre_t *Ainv) {
+    static __thread pre_t d[FMAX], L[FMAX * FMAX], X[FMAX * FMAX], y[FMAX];
+    for (int i = 0; i < q; ++i) {
+        if (!(A[i * q + i] > 0)) return -1;
+        d[i] = 1 / sqrtl(A[i * q + i]);
+    }
+    memset(L, 0, sizeof L);
+    for (int i = 0; i < q; ++i)
+        for (int j = 0; j <= i; ++j) {
+            pre_t acc = A[i * q + j] * d[i] * d[j];
+            for (int k = 0; k < j; ++k) acc -= L[i * q + k] * L[j * q + k];
+            if (i == j) { if (!(acc > 0)) return -1; L[i * q + i] = sqrtl(acc); }
+            else L[i * q + j] = acc / L[j * q + j];
+        }
+    for (int c = 0; c < q; ++c) {
+        for (int i = 0; i < q; ++i) {
+            pre_t acc = (i == c) ? 1 : 0;
+            for (int k = 0; k < i; ++k) acc -= L[i * q + k] * y[k];
+            y[i] = acc / L[i * q + i];
+        }
+        for (int i = q - 1; i >= 0; --i) {
+            pre_t acc = y[i];
+            for (int k = i + 1; k < q; ++k) acc -= L[k * q + i] * X[k * q + c];
+            X[i * q + c] = acc / L[i * q + i];
+        }
+    }
+    for (int i = 0; i < q; ++i)
+        for (int j = 0; j < q; ++j) Ainv[i * q + j] = X[i * q + j] * d[i] * d[j];
+    return 0;
+}
+
 /* ------------------------------------------------------------------ create */
 
 #define ALLOC(ptr, count) do { (ptr) = (real_t *)calloc((size_t)(count) > 0 ? (size_t)(count) : 1, sizeof(real_t)); \
@@ -168,6 +212,7 @@ void oracle_destroy(oracle_t *o) {
     free(o->C); free(o->z); free(o->zprev); free(o->u);
     free(o->Sp); free(o->Sn); free(o->Vp); free(o->Vn);
     free(o->PhiV); free(o->WV); free(o->PhiA); free(o->WA); free(o->part);
+    free(o->planes); free(o->PmF); free(o->c0F); free(o->Spl); free(o->Vpl);
     free(o);
 }
 
@@ -238,15 +283,92 @@ static int build_operator(oracle_t *o, int i) {
     return 0;
 }
 
+/* Coupled operator of segment i with a polytope corridor (reading A11p), coefficient index a*m + d:
+ *   H = kron(2Q + rho(M'M + E1'E1 + E2'E2), I_m) + rho sum_j sum_k kron(e0_j, a_k) kron(e0_j, a_k)'     (Eq. 20a)
+ * HARD mode: the 2m waypoint equalities Ew (x) I_m are imposed inside the QP exactly as in build_operator. */
+static int build_operator_poly(oracle_t *o, int i) {
+    const int n = o->n, s = o->s, Ms = o->Ms, m = o->m, K = o->K, q = n * m;
+    const pre_t T = (pre_t)o->T[i], rho = (pre_t)o->rho;
+    static __thread pre_t H[FMAX * FMAX], Hinv[FMAX * FMAX], Pm[FMAX * FMAX], HE[FMAX * 6], Kg[FMAX * 6];
+    pre_t Q[NMAX * NMAX], D[NMAX * NMAX], row[NMAX];
+    build_Q(n, s, T, Q);
+    for (int a = 0; a < n * n; ++a) { o->Q[(size_t)i * n * n + a] = (real_t)Q[a]; D[a] = 2 * Q[a]; }
+    for (int r = 0; r < 2 * s; ++r) {
+        beta_row(n, r % s, r < s ? (pre_t)0 : T, row);
+        for (int j = 0; j < n; ++j) o->M[((size_t)i * 2 * s + r) * n + j] = (real_t)row[j];
+        for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) D[a * n + b] += rho * row[a] * row[b];
+    }
+    memset(H, 0, sizeof(pre_t) * q * q);
+    for (int j = 0; j < Ms; ++j) {
+        pre_t t = T * (pre_t)(j + 1) / (pre_t)(Ms + 1);
+        for (int k = 0; k < 3; ++k) {
+            real_t *E = k == 0 ? o->E0 : (k == 1 ? o->E1 : o->E2);
+            beta_row(n, k, t, row);
+            for (int a = 0; a < n; ++a) E[((size_t)i * Ms + j) * n + a] = (real_t)row[a];
+            if (k == 0) {
+                /* rows kron(e0_j, a_k), k = 1..K */
+                for (int kk = 0; kk < K; ++kk) {
+                    const real_t *pl = o->planes + ((size_t)i * K + kk) * (m + 1);
+                    for (int a = 0; a < n; ++a) for (int d = 0; d < m; ++d)
+                        for (int b = 0; b < n; ++b) for (int e = 0; e < m; ++e)
+                            H[(a * m + d) * q + (b * m + e)] += rho * (row[a] * (pre_t)pl[d]) * (row[b] * (pre_t)pl[e]);
+                }
+            } else if (k == 1 ? o->has_vel : o->has_acc) {
+                for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) D[a * n + b] += rho * row[a] * row[b];
+            }
+        }
+    }
+    for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) for (int d = 0; d < m; ++d) H[(a * m + d) * q + (b * m + d)] += D[a * n + b];
+    if (spd_inverse_big(q, H, Hinv)) return -1;
+    real_t *PmF = o->PmF + (size_t)i * q * q, *c0F = o->c0F + (size_t)i * q;
+    for (int a = 0; a < q; ++a) c0F[a] = 0;
+    if (o->mode == MODE_HARD) {
+        /* Ewf rows: (beta_0(0) (x) e_d), (beta_0(T) (x) e_d); 2m of them */
+        pre_t Ew[2 * NMAX], S[36], Si[36];
+        const int w = 2 * m;
+        beta_row(n, 0, 0, Ew); beta_row(n, 0, T, Ew + n);
+        /* HE = Hinv Ewf'  (q x 2m);  column c = (end e, dim d): Ewf row has Ew[e][b] at index b*m + d */
+        for (int a = 0; a < q; ++a) for (int e = 0; e < 2; ++e) for (int d = 0; d < m; ++d) {
+            pre_t acc = 0; for (int b = 0; b < n; ++b) acc += Hinv[a * q + b * m + d] * Ew[e * n + b];
+            HE[a * w + e * m + d] = acc;
+        }
+        for (int e = 0; e < 2; ++e) for (int d = 0; d < m; ++d) for (int c = 0; c < w; ++c) {
+            pre_t acc = 0; for (int b = 0; b < n; ++b) acc += Ew[e * n + b] * HE[(b * m + d) * w + c];
+            S[(e * m + d) * w + c] = acc;
+        }
+        if (spd_inverse_big(w, S, Si)) return -1;
+        for (int a = 0; a < q; ++a) for (int c = 0; c < w; ++c) {
+            pre_t acc = 0; for (int r = 0; r < w; ++r) acc += HE[a * w + r] * Si[r * w + c];
+            Kg[a * w + c] = acc;
+        }
+        for (int a = 0; a < q; ++a) for (int b = 0; b < q; ++b) {
+            pre_t acc = Hinv[a * q + b];
+            for (int c = 0; c < w; ++c) acc -= Kg[a * w + c] * HE[b * w + c];
+            Pm[a * q + b] = acc;
+        }
+        for (int a = 0; a < q; ++a) {
+            pre_t acc = 0;
+            for (int d = 0; d < m; ++d)
+                acc += Kg[a * w + 0 * m + d] * (pre_t)o->p[(size_t)i * m + d] + Kg[a * w + 1 * m + d] * (pre_t)o->p[(size_t)(i + 1) * m + d];
+            c0F[a] = (real_t)acc;
+        }
+    } else {
+        memcpy(Pm, Hinv, sizeof(pre_t) * q * q);
+    }
+    for (int a = 0; a < q * q; ++a) PmF[a] = (real_t)Pm[a];
+    return 0;
+}
+
 /*
  * All inputs are host fp64.  waypoints [N+1][m]; durations [N]; start/end_derivs [s-1][m] (orders
  * 1..s-1) or NULL = rest; box_lo/hi [N][m] or NULL; vmax/amax <= 0 => off; Ms = samples per segment.
  */
-oracle_t *oracle_create(int N, int s, int m, const double *waypoints, const double *durations,
+static oracle_t *oracle_create_impl(int N, int s, int m, const double *waypoints, const double *durations,
                         const double *start_derivs, const double *end_derivs, int Ms,
                         const double *box_lo, const double *box_hi, double vmax, double amax,
-                        double rho, int mode) {
+                        double rho, int mode, int K, const double *planes) {
     if (N < 1 || (s != 3 && s != 4) || m < 1 || m > 3 || Ms < 0 || !(rho > 0) || mode < 0 || mode > 2) return NULL;
+    if (K < 0 || (K > 0 && (!planes || Ms <= 0 || box_lo || box_hi))) return NULL;   /* a polytope replaces the box */
     oracle_t *o = (oracle_t *)calloc(1, sizeof(oracle_t));
     if (!o) return NULL;
     const int n = 2 * s;
@@ -255,6 +377,11 @@ oracle_t *oracle_create(int N, int s, int m, const double *waypoints, const doub
     o->has_box = (Ms > 0 && box_lo && box_hi);
     o->has_vel = (Ms > 0 && vmax > 0);
     o->has_acc = (Ms > 0 && amax > 0);
+    o->K = K; o->has_poly = K > 0;
+    ALLOC(o->planes, (size_t)N * K * (m + 1)); ALLOC(o->PmF, o->has_poly ? (size_t)N * n * m * n * m : 0);
+    ALLOC(o->c0F, o->has_poly ? (size_t)N * n * m : 0);
+    ALLOC(o->Spl, (size_t)N * Ms * K); ALLOC(o->Vpl, (size_t)N * Ms * K);
+    for (size_t a = 0; a < (size_t)N * K * (m + 1); ++a) o->planes[a] = (real_t)planes[a];
     ALLOC(o->T, N); ALLOC(o->p, (N + 1) * m); ALLOC(o->lo, N * m); ALLOC(o->hi, N * m);
     ALLOC(o->Q, (size_t)N * n * n); ALLOC(o->M, (size_t)N * 2 * s * n);
     ALLOC(o->E0, (size_t)N * Ms * n); ALLOC(o->E1, (size_t)N * Ms * n); ALLOC(o->E2, (size_t)N * Ms * n);
@@ -269,7 +396,7 @@ oracle_t *oracle_create(int N, int s, int m, const double *waypoints, const doub
     for (int i = 0; i < N; ++i) { if (!(durations[i] > 0)) { oracle_destroy(o); return NULL; } o->T[i] = (real_t)durations[i]; }
     for (int a = 0; a < (N + 1) * m; ++a) o->p[a] = (real_t)waypoints[a];
     if (o->has_box) for (int a = 0; a < N * m; ++a) { o->lo[a] = (real_t)box_lo[a]; o->hi[a] = (real_t)box_hi[a]; }
-    for (int i = 0; i < N; ++i) if (build_operator(o, i)) { oracle_destroy(o); return NULL; }
+    for (int i = 0; i < N; ++i) if (o->has_poly ? build_operator_poly(o, i) : build_operator(o, i)) { oracle_destroy(o); return NULL; }
 
     /* ---- Init (Alg. 1 line 1; reading A9) ---- */
     for (int i = 0; i < N; ++i) {          /* C0 = chord at constant speed */
@@ -307,9 +434,30 @@ oracle_t *oracle_create(int N, int s, int m, const double *waypoints, const doub
             }
             if (o->has_vel) proj_ball(m, V, o->vmax, o->PhiV + q);
             if (o->has_acc) proj_ball(m, A, o->amax, o->PhiA + q);
+            for (int k = 0; k < K; ++k) {          /* polytope slacks of the chord samples: s = max(0, b - a'p) */
+                const real_t *pl = o->planes + ((size_t)i * K + k) * (m + 1);
+                real_t val = 0;
+                for (int d = 0; d < m; ++d) val += pl[d] * P[d];
+                real_t sl = pl[m] - val;
+                o->Spl[((size_t)i * Ms + j) * K + k] = sl > 0 ? sl : 0;
+            }
         }
     o->iter = 0; o->rp = o->rd = o->rd_norm = o->rp_gap = NAN;
     return o;
+}
+
+oracle_t *oracle_create(int N, int s, int m, const double *waypoints, const double *durations,
+                        const double *start_derivs, const double *end_derivs, int Ms,
+                        const double *box_lo, const double *box_hi, double vmax, double amax,
+                        double rho, int mode) {
+    return oracle_create_impl(N, s, m, waypoints, durations, start_derivs, end_derivs, Ms, box_lo, box_hi, vmax, amax, rho, mode, 0, NULL);
+}
+
+/* the same with a general polytope corridor: planes [N][K][m+1] = (normal a_k, offset b_k), a_k'p <= b_k (A11p) */
+oracle_t *oracle_create_poly(int N, int s, int m, const double *waypoints, const double *durations,
+                             const double *start_derivs, const double *end_derivs, int Ms, int K, const double *planes,
+                             double vmax, double amax, double rho, int mode) {
+    return oracle_create_impl(N, s, m, waypoints, durations, start_derivs, end_derivs, Ms, NULL, NULL, vmax, amax, rho, mode, K, planes);
 }
 
 /* ------------------------------------------------------------------ one sweep (Alg. 1 lines 3-13) */
@@ -346,6 +494,22 @@ static void sweep_once(oracle_t *o) {
                 if (o->has_vel) { real_t g = o->PhiV[q + d] - o->WV[q + d]; for (int a = 0; a < n; ++a) R[a * m + d] += e1[a] * g; }
                 if (o->has_acc) { real_t g = o->PhiA[q + d] - o->WA[q + d]; for (int a = 0; a < n; ++a) R[a * m + d] += e2[a] * g; }
             }
+            for (int k = 0; k < o->K; ++k) {       /* Ao'(b - s - v), row (j,k) of Ao = kron(e0_j, a_k)   (A11p) */
+                const real_t *pl = o->planes + ((size_t)i * o->K + k) * (m + 1);
+                size_t qk = ((size_t)i * Ms + j) * o->K + k;
+                real_t g = pl[m] - o->Spl[qk] - o->Vpl[qk];
+                for (int a = 0; a < n; ++a) for (int d = 0; d < m; ++d) R[a * m + d] += e0[a] * pl[d] * g;
+            }
+        }
+        if (o->has_poly) {                         /* coupled dims: c = PmF (rho R) + c0F over the (n m)-vector */
+            const int qd = n * m;
+            const real_t *PmF = o->PmF + (size_t)i * qd * qd;
+            for (int a = 0; a < qd; ++a) {
+                real_t acc = 0;
+                for (int b = 0; b < qd; ++b) acc += PmF[a * qd + b] * (rho * R[b]);
+                o->C[(size_t)i * qd + a] = acc + o->c0F[(size_t)i * qd + a];
+            }
+            continue;
         }
         const real_t *Pm = o->Pm + (size_t)i * n * n;
         for (int a = 0; a < n; ++a)
@@ -448,6 +612,24 @@ static void sweep_once(oracle_t *o) {
                 }
             }
     }
+    if (o->has_poly) {                           /* Eq. 20d, 20e per (sample, plane): A = kron(e0_j, a_k), b = b_k */
+#pragma omp parallel for schedule(static)
+        for (int i = 0; i < N; ++i)
+            for (int j = 0; j < Ms; ++j) {
+                const real_t *e0 = o->E0 + ((size_t)i * Ms + j) * n;
+                real_t P[3] = {0, 0, 0};
+                for (int d = 0; d < m; ++d) for (int a = 0; a < n; ++a) P[d] += e0[a] * o->C[((size_t)i * n + a) * m + d];
+                for (int k = 0; k < o->K; ++k) {
+                    const real_t *pl = o->planes + ((size_t)i * o->K + k) * (m + 1);
+                    size_t qk = ((size_t)i * Ms + j) * o->K + k;
+                    real_t val = 0;
+                    for (int d = 0; d < m; ++d) val += pl[d] * P[d];
+                    real_t sl = -(val - pl[m] + o->Vpl[qk]);
+                    o->Spl[qk] = sl > 0 ? sl : 0;
+                    o->Vpl[qk] += val + o->Spl[qk] - pl[m];
+                }
+            }
+    }
     real_t a0 = 0, a1 = 0, a2 = 0, a3 = 0;       /* fixed-order (serial) reduction */
     for (int i = 0; i < N; ++i) { a0 += o->part[(size_t)i * 4]; a1 += o->part[(size_t)i * 4 + 1];
                                   a2 += o->part[(size_t)i * 4 + 2]; a3 += o->part[(size_t)i * 4 + 3]; }
@@ -501,8 +683,9 @@ int oracle_set_rho(oracle_t *o, double rho_new) {
     const real_t r = o->rho / (real_t)rho_new;
     for (size_t a = 0; a < (size_t)N * 2 * s * m; ++a) o->u[a] *= r;
     for (size_t a = 0; a < (size_t)N * Ms * m; ++a) { o->Vp[a] *= r; o->Vn[a] *= r; o->WV[a] *= r; o->WA[a] *= r; }
+    for (size_t a = 0; a < (size_t)N * Ms * o->K; ++a) o->Vpl[a] *= r;
     o->rho = (real_t)rho_new;
-    for (int i = 0; i < N; ++i) if (build_operator(o, i)) return -1;
+    for (int i = 0; i < N; ++i) if (o->has_poly ? build_operator_poly(o, i) : build_operator(o, i)) return -1;
     return 0;
 }
 
@@ -567,6 +750,7 @@ int64_t oracle_get(const oracle_t *o, const char *name, double *out) {
     FIELD("v_pos", o->Vp, (size_t)N * Ms * m) FIELD("v_neg", o->Vn, (size_t)N * Ms * m)
     FIELD("phi_v", o->PhiV, (size_t)N * Ms * m) FIELD("w_v", o->WV, (size_t)N * Ms * m)
     FIELD("phi_a", o->PhiA, (size_t)N * Ms * m) FIELD("w_a", o->WA, (size_t)N * Ms * m)
+    FIELD("s_poly", o->Spl, (size_t)N * Ms * o->K) FIELD("v_poly", o->Vpl, (size_t)N * Ms * o->K)
     FIELD("Pm", o->Pm, (size_t)N * n * n) FIELD("c0", o->c0, (size_t)N * n * m) FIELD("Q", o->Q, (size_t)N * n * n)
     FIELD("M", o->M, (size_t)N * 2 * s * n) FIELD("E0", o->E0, (size_t)N * Ms * n) FIELD("E1", o->E1, (size_t)N * Ms * n)
     FIELD("E2", o->E2, (size_t)N * Ms * n)

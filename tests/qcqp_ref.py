@@ -26,8 +26,19 @@ def tiny_instance():
 
 
 
-def slsqp_optimum(unc, lo, hi, vmax):
-    """Optimum of min sum c'Q c s.t. waypoints, C^(s-1) continuity, rest ends, box and speed bound at the samples."""
+def box_as_planes(lo, hi):
+    """The axis-aligned box lo <= p <= hi as 6 half-spaces a'p <= b per segment: [N][6][4]."""
+    N = lo.shape[0]
+    pl = np.zeros((N, 6, 4))
+    for d in range(3):
+        pl[:, d, d] = 1.0; pl[:, d, 3] = hi[:, d]
+        pl[:, 3 + d, d] = -1.0; pl[:, 3 + d, 3] = -lo[:, d]
+    return pl
+
+
+def slsqp_optimum(unc, lo, hi, vmax, planes=None):
+    """Optimum of min sum c'Q c s.t. waypoints, C^(s-1) continuity, rest ends, box (or polytope planes [N][K][4]:
+    a'p <= b) and speed bound at the samples."""
     n = 2 * S_
     nv = N_ * M_ * n                                     # x = coeffs [N][m][n] flattened, physical time
     Qs = [direct.Q_unit(S_) * (TT[i] ** (1 - 2 * S_)) for i in range(N_)]
@@ -66,9 +77,13 @@ def slsqp_optimum(unc, lo, hi, vmax):
     for i in range(N_):
         for tau in TAUS:
             b0 = direct.beta(n, 0, tau * TT[i])
-            for d in range(M_):
-                Abox.append(row(i, d, b0)); bbox.append(hi[i, d])
-                Abox.append(-row(i, d, b0)); bbox.append(-lo[i, d])
+            if planes is None:
+                for d in range(M_):
+                    Abox.append(row(i, d, b0)); bbox.append(hi[i, d])
+                    Abox.append(-row(i, d, b0)); bbox.append(-lo[i, d])
+            else:
+                for k in range(planes.shape[1]):
+                    Abox.append(sum(planes[i, k, d] * row(i, d, b0) for d in range(M_))); bbox.append(planes[i, k, 3])
     Abox, bbox = np.array(Abox), np.array(bbox)
     B1 = [[direct.beta(n, 1, tau * TT[i]) for tau in TAUS] for i in range(N_)]
 
