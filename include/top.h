@@ -96,6 +96,15 @@ typedef struct {
     const double* box_hi;   /* host [batch][N][dims]; lo < hi elementwise */
     double vmax;            /* > 0: ||sigma'(t_ij)||_2  <= vmax ; <= 0: off */
     double amax;            /* > 0: ||sigma''(t_ij)||_2 <= amax ; <= 0: off */
+    /* General convex-polytope corridor (Eq. 7-10 "FIRI ... multiple linear inequality
+     * constraints", L231 A_i^o in R^{MK x m(d+1)}): num_planes = K half-spaces a_k'p <= b_k per segment, enforced on the
+     * position at the `samples` sample times, one slack and one scaled dual per (sample, plane) (Eq. 20d, 20e).
+     * planes: host [batch][N][K][dims+1] = (a_k (dims), b_k); normals need not be unit but must be non-zero.
+     * Replaces the box (box_lo/box_hi must be NULL).  1 <= K <= 16; TOP_F64 with the tensor-core kernel only
+     * (lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA), N up to top_capacity_polytope; else TOP_E_UNSUPPORTED.
+     * num_planes == 0: no polytope. */
+    int32_t num_planes;
+    const double* planes;
 } top_constraints;
 
 typedef struct {
@@ -195,6 +204,7 @@ TOP_API top_status top_get_coeffs(top_solver* h, void* out, int32_t out_is_devic
 /* top_get_state -- one field of the current iterate as host fp64 (parity tests, warm-start snapshots).
  * field / layout:  "z" [batch][N+1][s][dims]   "u" [batch][N][2s][dims]
  *                  "s_pos","s_neg","v_pos","v_neg","phi_v","w_v","phi_a","w_a" [batch][N][Ms][dims]
+ *                  "s_poly","v_poly" [batch][N][Ms][K]   (polytope corridor: slack / scaled dual per (sample, plane))
  * count = number of doubles `out` holds; TOP_E_INVALID if it does not match or the field is unknown. */
 TOP_API top_status top_get_state(top_solver* h, const char* field, double* out, size_t count);
 

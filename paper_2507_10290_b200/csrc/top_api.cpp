@@ -75,6 +75,13 @@ struct top_solver {
     std::unique_ptr<unsigned char[]> stage;   // host staging buffer (kept: top_reset re-uses it)
     std::vector<double> h_wp, h_T;         // host copies of waypoints / durations (local-frame origins, lazy spectral form)
     bool have_spectral = false;            // W, lambda on the device (built on first use: top_set_rho, Eq. 24)
+    // general polytope corridor (reading A11p): K planes per segment; per-segment rotated frame
+    bool has_poly = false;
+    int K = 0;
+    double *d_rot = nullptr, *d_planes = nullptr, *d_lam3 = nullptr, *d_qpl = nullptr;
+    size_t off_rot = 0, off_planes = 0, off_lam3 = 0, pm_dims = 1;
+    std::vector<double> h_rot;             // [9][nseg_pad] host copy of the rotations (top_get_state)
+    std::vector<double> h_planes;          // host copy of the caller's planes (a new rho rebuilds the operators)
     double *d_Pm = nullptr, *d_c0 = nullptr, *d_part = nullptr, *d_res = nullptr;
     double *d_W = nullptr, *d_lam = nullptr, *d_g0 = nullptr, *d_dp = nullptr;   // spectral operator data (rho-independent)
     void *d_invTk = nullptr, *d_Tpow = nullptr, *d_invT = nullptr, *d_lohi = nullptr, *d_zoff = nullptr;
@@ -190,14 +197,14 @@ const GramTables& gram_tables(int s) {       // built once per s, whatever threa
 }
 
 bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int mode,
-                    const xreal* p0, const xreal* p1, xreal* Pm /*[8][8]*/, xreal* c0 /*[8][3]*/) {
+                    const xreal* p0, const xreal* p1, xreal* Pm /*[8][8]*/, xreal* c0 /*[8][3]*/, xreal box_weight = 2) {
     const int n = 2 * s;
     const GramTables& G = gram_tables(s);
     xreal iT[8];                       // T^-k
     iT[0] = 1;
     for (int k = 1; k < 8; ++k) iT[k] = iT[k - 1] / T;
     const xreal wq = 2 * T * iT[2 * s - 1] * iT[1];             // 2 T^(1-2s)
-    const xreal wb = box ? 2 * rho : 0;                        // two sides of the box (A11)
+    const xreal wb = box ? box_weight * rho : 0;               // box: its two sides (A11); polytope: eigenvalue of sum_k a_k a_k' (A11p)
     const xreal wv = vel ? rho * iT[2] : 0, wa = acc ? rho * iT[4] : 0;
     xreal H[MAXN * MAXN];
     for (int a = 0; a < n; ++a)
@@ -415,16 +422,16 @@ top_status download_real(top_solver* h, const void* src, std::vector<double>& ds
 int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 // the sweep kernel family of a solver: 8 lanes, 4 lanes (shuffle form), or 4 lanes with fp64 tensor-core contractions
-size_t kernel_smem(int dtype, int s, bool constrained, int lanes, bool mma, int segs) {
-    return mma ? sweep_smem_bytes_mma(constrained, segs) : sweep_smem_bytes(dtype, s, constrained, lanes, segs);
+size_t kernel_smem(int dtype, int s, bool constrained, int lanes, bool mma, int segs, bool poly = false) {
+    return mma ? sweep_smem_bytes_mma(constrained, poly) : sweep_smem_bytes(dtype, s, constrained, lanes, segs);
 }
-int kernel_max_threads(int dtype, int lanes, bool mma) { return mma ? max_threads_mma() : max_threads_for(dtype, lanes); }
+int kernel_max_threads(int dtype, int lanes, bool mma, bool poly = false) { return mma ? max_threads_mma(poly) : max_threads_for(dtype, lanes); }
 
 // largest segments-per-CTA (multiple of 4) whose threads and shared memory fit one CTA
-int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, bool mma, size_t smem_limit) {
+int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, bool mma, size_t smem_limit, bool poly = false) {
     int best = 0;
-    for (int segs = 4; (segs * lanes + 31) / 32 * 32 <= kernel_max_threads(dtype, lanes, mma); segs += 4)
-        if (kernel_smem(dtype, s, constrained, lanes, mma, segs) <= smem_limit) best = segs;
+    for (int segs = 4; (segs * lanes + 31) / 32 * 32 <= kernel_max_threads(dtype, lanes, mma, poly); segs += 4)
+        if (kernel_smem(dtype, s, constrained, lanes, mma, segs, poly) <= smem_limit) best = segs;
     return best;
 }
 
@@ -461,6 +468,117 @@ template <typename F> void parallel_segments(long long n, F fn) {
 
 namespace {
 
+// symmetric 3x3 eigen-decomposition A = V diag(lam) V' (cyclic Jacobi, extended precision); V row-major, columns = axes
+void eigen3(const xreal* A, xreal* V, xreal* lam) {
+    xreal C[9];
+    for (int i = 0; i < 9; ++i) { C[i] = A[i]; V[i] = (i % 4 == 0) ? 1 : 0; }
+    for (int sweep = 0; sweep < 60; ++sweep) {
+        const xreal off = C[1] * C[1] + C[2] * C[2] + C[5] * C[5], diag = C[0] * C[0] + C[4] * C[4] + C[8] * C[8];
+        if (off <= diag * (xreal)1e-40 || off == 0) break;
+        for (int pp = 0; pp < 3; ++pp)
+            for (int r = pp + 1; r < 3; ++r) {
+                const xreal apq = C[pp * 3 + r];
+                if (apq == 0) continue;
+                const xreal theta = (C[r * 3 + r] - C[pp * 3 + pp]) / (2 * apq);
+                const xreal tt = (theta >= 0 ? 1 : -1) / (std::fabs(theta) + std::sqrt(theta * theta + 1));
+                const xreal c = 1 / std::sqrt(tt * tt + 1), sn = tt * c;
+                for (int k = 0; k < 3; ++k) { const xreal x = C[k * 3 + pp], y = C[k * 3 + r]; C[k * 3 + pp] = c * x - sn * y; C[k * 3 + r] = sn * x + c * y; }
+                for (int k = 0; k < 3; ++k) { const xreal x = C[pp * 3 + k], y = C[r * 3 + k]; C[pp * 3 + k] = c * x - sn * y; C[r * 3 + k] = sn * x + c * y; }
+                for (int k = 0; k < 3; ++k) { const xreal x = V[k * 3 + pp], y = V[k * 3 + r]; V[k * 3 + pp] = c * x - sn * y; V[k * 3 + r] = sn * x + c * y; }
+            }
+    }
+    for (int d = 0; d < 3; ++d) lam[d] = C[d * 3 + d] > 0 ? C[d * 3 + d] : 0;
+}
+void fill_init_params(top_solver* h, InitParams& ip) {
+    const GramTables& G = gram_tables(h->s);
+    unsigned char* D = h->d_upload;
+    ip.waypoints = (const double*)(D + h->off_wp); ip.durations = (const double*)(D + h->off_T);
+    ip.box_lo = h->has_box ? (const double*)(D + h->off_lo) : nullptr; ip.box_hi = h->has_box ? (const double*)(D + h->off_hi) : nullptr;
+    ip.start_derivs = h->have_sd ? (const double*)(D + h->off_sd) : nullptr;
+    ip.end_derivs = h->have_ed ? (const double*)(D + h->off_ed) : nullptr;
+    for (int a = 0; a < MAXN; ++a) {
+        for (int k = 0; k < 4; ++k) ip.gc1[k][a] = (double)G.Gc[k][a * MAXN + 1];
+        for (int k = 0; k < 3; ++k) ip.ge1[k][a] = (double)G.Ge[k][a * MAXN + 1];
+    }
+    ip.Pm = h->d_Pm; ip.c0 = h->d_c0; ip.g0 = h->d_g0; ip.dp = h->d_dp; ip.origin = h->d_origin;
+    ip.invTk = h->d_invTk; ip.Tpow = h->d_Tpow; ip.invT = h->d_invT; ip.lohi = h->d_lohi; ip.zoff = h->d_zoff;
+    ip.zt = h->d_zt; ip.chat = h->d_chat; ip.qp = h->d_qp; ip.qn = h->d_qn; ip.phv = h->d_phv; ip.segflags = h->d_segflags;
+    ip.stride = h->stride; ip.nseg_pad = h->nseg_pad; ip.nseg = h->nseg; ip.N = h->N; ip.batch = h->batch; ip.s = h->s; ip.dims = h->dims;
+    ip.hard = h->wp_mode == TOP_WAYPOINT_HARD; ip.has_box = h->has_box; ip.has_vel = h->has_vel; ip.has_acc = h->has_acc;
+    ip.vmax = h->vmax;
+    ip.rot = h->d_rot; ip.planes = h->d_planes; ip.lam3 = h->d_lam3; ip.qpl = h->d_qpl; ip.K = h->K; ip.has_poly = h->has_poly;
+}
+
+// rho Pm^ of every segment for the current rho into the staging buffer, by the direct (null-space) inverse in extended
+// precision; segments of equal duration (config 3: all of them) share one factorisation.  The rho-independent spectral
+// form is only built when rho is going to change.  Polytope corridor (reading A11p): with N_i = sum_k a_k a_k' = V L V'
+// the coupled (n m)^2 operator of Eq. 20a splits, in the rotated frame y = V'(p - o_i), into one n x n operator per
+// rotated dim with box weight L_d; also staged: V, L and the planes in that frame.
+top_status stage_operators(top_solver* h) {
+    const int N = h->N, s = h->s, dims = h->dims, n = 2 * s, K = h->K;
+    const long long nseg = h->nseg;
+    const size_t LS = (size_t)h->stride, NP = (size_t)h->nseg_pad;
+    unsigned char* S = h->stage.get();
+    double* Pm_st = reinterpret_cast<double*>(S);
+    double* rot_st = reinterpret_cast<double*>(S + h->off_rot);
+    double* pl_st = reinterpret_cast<double*>(S + h->off_planes);
+    double* lam_st = reinterpret_cast<double*>(S + h->off_lam3);
+    const double* durations = h->h_T.data();
+    gram_tables(s);     // built before the worker threads start
+    std::atomic<int> bad_operator(0);
+    const bool box = h->has_box, vel = h->has_vel, acc = h->has_acc, poly = h->has_poly;
+    const int mode = (int)h->wp_mode;
+    const xreal rho = (xreal)h->rho;
+    auto do_segments = [&](long long g0, long long g1) {
+        try {
+            xreal Pm[MAXN * MAXN];
+            double cached_T = -1.0;
+            for (long long g = g0; g < g1; ++g) {
+                const double Td = durations[g];
+                if (!poly) {
+                    if (Td != cached_T) {
+                        if (!build_operator(s, (xreal)Td, rho, box, vel, acc, mode, nullptr, nullptr, Pm, nullptr)) { bad_operator.store(1); return; }
+                        cached_T = Td;
+                    }
+                    for (int lane = 0; lane < n; ++lane)
+                        for (int b = 0; b < n; ++b) Pm_st[(size_t)b * LS + (size_t)g * LANES + lane] = (double)(rho * Pm[lane * MAXN + b]);
+                    continue;
+                }
+                const double* pl = h->h_planes.data() + (size_t)g * K * (dims + 1);
+                xreal Nm[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, V[9], lam[3];
+                for (int k = 0; k < K; ++k)
+                    for (int d = 0; d < dims; ++d) for (int e = 0; e < dims; ++e) Nm[d * 3 + e] += (xreal)pl[k * (dims + 1) + d] * (xreal)pl[k * (dims + 1) + e];
+                eigen3(Nm, V, lam);
+                const long long b_ = g / N, i_ = g % N;
+                const double* o = h->h_wp.data() + ((size_t)b_ * (N + 1) + i_) * dims;      // origin of the local frame
+                for (int q = 0; q < 9; ++q) rot_st[(size_t)q * NP + g] = (double)V[q];
+                for (int d = 0; d < 3; ++d) {
+                    lam_st[(size_t)d * NP + g] = (double)lam[d];
+                    if (!build_operator(s, (xreal)Td, rho, true, vel, acc, mode, nullptr, nullptr, Pm, nullptr, lam[d])) { bad_operator.store(1); return; }
+                    for (int lane = 0; lane < n; ++lane)
+                        for (int b = 0; b < n; ++b)
+                            Pm_st[((size_t)d * MAXN + b) * LS + (size_t)g * LANES + lane] = (double)(rho * Pm[lane * MAXN + b]);
+                }
+                for (int k = 0; k < K; ++k) {
+                    xreal ao = 0;
+                    for (int d = 0; d < dims; ++d) ao += (xreal)pl[k * (dims + 1) + d] * (xreal)o[d];
+                    for (int e = 0; e < 3; ++e) {
+                        xreal v = 0;
+                        for (int d = 0; d < dims; ++d) v += V[d * 3 + e] * (xreal)pl[k * (dims + 1) + d];
+                        pl_st[((size_t)k * 4 + e) * NP + g] = (double)v;                    // a'_k = V'a_k
+                    }
+                    pl_st[((size_t)k * 4 + 3) * NP + g] = (double)((xreal)pl[k * (dims + 1) + dims] - ao);   // b'_k = b_k - a_k'o_i
+                }
+            }
+        } catch (...) { bad_operator.store(2); }
+    };
+    parallel_segments(nseg, do_segments);
+    if (bad_operator.load() == 2) return fail(h, TOP_E_NOMEM, "host precompute failed");
+    if (bad_operator.load()) return fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)");
+    if (poly) h->h_rot.assign(rot_st, rot_st + 9 * NP);
+    return TOP_OK;
+}
+
 // The per-problem part of top_create, shared with top_reset: host precompute of the x-update operator (Eq. 20a first
 // bracket; per segment, extended precision, for the current rho), ONE host-to-device copy of the operator rows and of
 // the caller's arrays, then the init kernel (per-lane constants and iterate 0, reading A9).  Asynchronous.
@@ -470,7 +588,6 @@ top_status fill_problem(top_solver* h, const double* waypoints, const double* du
     const long long nseg = h->nseg;
     const size_t LS = (size_t)h->stride;
     unsigned char* S = h->stage.get();
-    double* Pm_st = reinterpret_cast<double*>(S);
     std::memcpy(S + h->off_wp, waypoints, (size_t)batch * (N + 1) * dims * 8);
     std::memcpy(S + h->off_T, durations, (size_t)nseg * 8);
     if (h->has_box) {
@@ -482,53 +599,20 @@ top_status fill_problem(top_solver* h, const double* waypoints, const double* du
     if (end_derivs) std::memcpy(S + h->off_ed, end_derivs, (size_t)batch * (s - 1) * dims * 8);
     h->h_wp.assign(waypoints, waypoints + (size_t)batch * (N + 1) * dims);
     h->h_T.assign(durations, durations + nseg);
-    const GramTables& G = gram_tables(s);     // built before the worker threads start
+    if (h->has_poly) h->h_planes.assign(cons->planes, cons->planes + (size_t)nseg * h->K * (dims + 1));
+    const GramTables& G = gram_tables(s);
     if (pt) pt->mark("staging copies");
 
-    // rho Pm^ of every segment by the direct (null-space) inverse; segments of equal duration (config 3: all of them)
-    // share one factorisation.  The rho-independent spectral form is only built when rho is going to change.
-    std::atomic<int> bad_operator(0);
-    const bool box = h->has_box, vel = h->has_vel, acc = h->has_acc;
-    const int mode = (int)h->wp_mode;
-    const xreal rho = (xreal)h->rho;
-    auto do_segments = [&](long long g0, long long g1) {
-        try {
-            xreal Pm[MAXN * MAXN];
-            double cached_T = -1.0;
-            for (long long g = g0; g < g1; ++g) {
-                const double Td = durations[g];
-                if (Td != cached_T) {
-                    if (!build_operator(s, (xreal)Td, rho, box, vel, acc, mode, nullptr, nullptr, Pm, nullptr)) { bad_operator.store(1); return; }
-                    cached_T = Td;
-                }
-                for (int lane = 0; lane < n; ++lane)
-                    for (int b = 0; b < n; ++b) Pm_st[(size_t)b * LS + (size_t)g * LANES + lane] = (double)(rho * Pm[lane * MAXN + b]);
-            }
-        } catch (...) { bad_operator.store(2); }
-    };
-    parallel_segments(nseg, do_segments);
-    if (pt) pt->mark("host precompute");
-    if (bad_operator.load() == 2) return fail(h, TOP_E_NOMEM, "host precompute failed");
-    if (bad_operator.load()) return fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)");
+    {
+        top_status so = stage_operators(h);
+        if (pt) pt->mark("host precompute");
+        if (so != TOP_OK) return so;
+    }
 
     CU(cudaMemcpyAsync(h->d_upload, S, h->upload_bytes, cudaMemcpyHostToDevice, h->stream), "H2D problem data");
     InitParams ip;
     std::memset(&ip, 0, sizeof ip);
-    unsigned char* D = h->d_upload;
-    ip.waypoints = (const double*)(D + h->off_wp); ip.durations = (const double*)(D + h->off_T);
-    ip.box_lo = h->has_box ? (const double*)(D + h->off_lo) : nullptr; ip.box_hi = h->has_box ? (const double*)(D + h->off_hi) : nullptr;
-    ip.start_derivs = start_derivs ? (const double*)(D + h->off_sd) : nullptr;
-    ip.end_derivs = end_derivs ? (const double*)(D + h->off_ed) : nullptr;
-    for (int a = 0; a < MAXN; ++a) {
-        for (int k = 0; k < 4; ++k) ip.gc1[k][a] = (double)G.Gc[k][a * MAXN + 1];
-        for (int k = 0; k < 3; ++k) ip.ge1[k][a] = (double)G.Ge[k][a * MAXN + 1];
-    }
-    ip.Pm = h->d_Pm; ip.c0 = h->d_c0; ip.g0 = h->d_g0; ip.dp = h->d_dp; ip.origin = h->d_origin;
-    ip.invTk = h->d_invTk; ip.Tpow = h->d_Tpow; ip.invT = h->d_invT; ip.lohi = h->d_lohi; ip.zoff = h->d_zoff;
-    ip.zt = h->d_zt; ip.chat = h->d_chat; ip.qp = h->d_qp; ip.qn = h->d_qn; ip.phv = h->d_phv; ip.segflags = h->d_segflags;
-    ip.stride = h->stride; ip.nseg_pad = h->nseg_pad; ip.nseg = nseg; ip.N = N; ip.batch = batch; ip.s = s; ip.dims = dims;
-    ip.hard = h->wp_mode == TOP_WAYPOINT_HARD; ip.has_box = h->has_box; ip.has_vel = h->has_vel; ip.has_acc = h->has_acc;
-    ip.vmax = h->vmax;
+    fill_init_params(h, ip);
     CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
     h->launches += 1;
     h->have_spectral = false;
@@ -581,7 +665,8 @@ namespace {
 // argument checks common to top_create and top_reset (messages go to the handle, or to the thread-local slot)
 top_status validate_problem(top_solver* h, int batch, int N, int s, int dims, const double* waypoints, const double* durations,
                             const double* start_derivs, const double* end_derivs, const top_constraints* cons, double rho,
-                            bool* has_box, bool* has_vel, bool* has_acc) {
+                            bool* has_box, bool* has_vel, bool* has_acc, int* num_planes = nullptr) {
+    if (num_planes) *num_planes = 0;
     if (!waypoints || !durations) return fail(h, TOP_E_INVALID, "waypoints and durations are required");
     if (!(rho > 0) || !std::isfinite(rho)) return fail(h, TOP_E_INVALID, "rho must be finite and > 0");
     const long long nseg = (long long)batch * N;
@@ -608,9 +693,24 @@ top_status validate_problem(top_solver* h, int batch, int N, int s, int dims, co
             return fail(h, TOP_E_INVALID, "vmax/amax must be finite");
         *has_vel = cons->vmax > 0;
         *has_acc = cons->amax > 0;
+        if (cons->num_planes != 0) {       // general polytope corridor (reading A11p)
+            if (cons->num_planes < 0 || !cons->planes) return fail(h, TOP_E_INVALID, "num_planes must be >= 0 and planes non-NULL");
+            if (*has_box) return fail(h, TOP_E_INVALID, "a polytope corridor replaces the box: box_lo / box_hi must be NULL");
+            if (cons->num_planes > KMAX) return fail(h, TOP_E_UNSUPPORTED, "more than 16 planes per segment");
+            const long long cnt = nseg * cons->num_planes;
+            for (long long i = 0; i < cnt; ++i) {
+                const double* pl = cons->planes + i * (dims + 1);
+                double n2 = 0;
+                for (int d = 0; d <= dims; ++d) { if (!std::isfinite(pl[d])) return fail(h, TOP_E_INVALID, "non-finite plane"); if (d < dims) n2 += pl[d] * pl[d]; }
+                if (!(n2 > 0)) return fail(h, TOP_E_INVALID, "a plane normal is zero");
+            }
+            if (num_planes) *num_planes = cons->num_planes;
+            else return fail(h, TOP_E_INVALID, "polytope corridor not expected here");
+        }
     }
     return TOP_OK;
 }
+
 }  // namespace
 
 // =================================================================================== top_create
@@ -636,9 +736,10 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     const long long nseg = (long long)batch * N;
     if (nseg > (1ll << 28)) return fail(h, TOP_E_UNSUPPORTED, "more than 2^28 segments");
     bool has_box = false, has_vel = false, has_acc = false;
+    int num_planes = 0;
     {
         top_status vs = validate_problem(nullptr, batch, N, s, dims, waypoints, durations, start_derivs, end_derivs, cons, rho,
-                                         &has_box, &has_vel, &has_acc);
+                                         &has_box, &has_vel, &has_acc, &num_planes);
         if (vs != TOP_OK) return vs;
     }
     top_options o;
@@ -688,14 +789,15 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->opt_flags = o.flags; h->rho = rho; h->check_every = o.check_every; h->max_iter = o.max_iter;
     h->device = dev; h->stream = (cudaStream_t)o.cuda_stream; h->user_segs = o.segs_per_cta;
     h->has_box = has_box; h->has_vel = has_vel; h->has_acc = has_acc;
-    h->constrained = has_box || has_vel || has_acc;
+    h->has_poly = num_planes > 0; h->K = num_planes; h->pm_dims = h->has_poly ? 3 : 1;
+    h->constrained = has_box || has_vel || has_acc || h->has_poly;
     h->vmax = has_vel ? cons->vmax : 0; h->amax = has_acc ? cons->amax : 0;
     h->wp_mode = mode;
     if (o.adapt_mu > 0) h->adapt_mu = o.adapt_mu;
     if (o.adapt_tau_incr > 0) h->adapt_incr = o.adapt_tau_incr;
     if (o.adapt_tau_decr > 0) h->adapt_decr = o.adapt_tau_decr;
     h->kflags = (has_box ? KF_BOX : 0) | (has_vel ? KF_VEL : 0) | (has_acc ? KF_ACC : 0) |
-                (mode == TOP_WAYPOINT_PINNED_Z ? KF_PIN_POS : 0);
+                (mode == TOP_WAYPOINT_PINNED_Z ? KF_PIN_POS : 0) | (h->has_poly ? KF_POLY : 0);
     h->nseg = nseg; h->nseg_pad = (nseg + 31) / 32 * 32; h->stride = h->nseg_pad * LANES;
 
     // ---- launch plan: waves of whole trajectories, each wave resident on chip for all its sweeps
@@ -715,8 +817,11 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     // unconstrained chains once an SM holds more than a few warps (N = 10^4: 1.6 vs 2.1-2.3); short unconstrained chains
     // (configs 1, 3) stay on the 8-lane kernel (0.64 vs 0.85, 1.42 vs 1.57)
     if (!o.lanes_per_segment && dtype == TOP_F64 && ((has_box || has_vel || has_acc) || nseg >= (long long)h->num_sms * 32)) h->lanes = 4;
+    if (!o.lanes_per_segment && h->has_poly) h->lanes = 4;
     h->mma = dtype == TOP_F64 && h->lanes == 4 && !(o.flags & TOP_KERNEL_NO_MMA);
-    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192);
+    if (h->has_poly && !h->mma)
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "polytope corridors run on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA)"));
+    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192, h->has_poly);
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
     h->max_ctas = h->num_sms;
     const long long capacity = (long long)h->max_ctas * std::min(segs_max, h->user_segs ? h->user_segs : segs_max);
@@ -729,11 +834,13 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
         w.segs_per_cta = segs;
         w.ctas = (int)((cnt + segs - 1) / segs);
         w.threads = (segs * h->lanes + 31) / 32 * 32;
-        w.smem = kernel_smem(h->dtype, s, h->constrained, h->lanes, h->mma, segs);
+        w.smem = kernel_smem(h->dtype, s, h->constrained, h->lanes, h->mma, segs, h->has_poly);
         if (w.ctas > h->max_ctas) return false;
         h->waves.push_back(w);
         return true;
     };
+    if ((long long)N > capacity && h->has_poly)
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "a trajectory with a polytope corridor must fit on chip (streaming is not built for it)"));
     if ((long long)N > capacity) {
         // one trajectory does not fit on chip: stream the whole segment index space in pieces with halos
         h->streaming = true;
@@ -774,7 +881,10 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     const int n = 2 * s;
     struct Carve { size_t off = 0; size_t take(size_t bytes) { const size_t o = off; off = (off + bytes + 255) & ~(size_t)255; return o; } } cv;
     // (a) the region that mirrors the staging buffer: operator rows, then the caller's arrays as they are
-    const size_t o_Pm = cv.take(MAXN * LS * 8);
+    const size_t o_Pm = cv.take(h->pm_dims * MAXN * LS * 8);
+    h->off_rot = cv.take(h->has_poly ? 9 * NP * 8 : 0);
+    h->off_planes = cv.take(h->has_poly ? (size_t)h->K * 4 * NP * 8 : 0);
+    h->off_lam3 = cv.take(h->has_poly ? 3 * NP * 8 : 0);
     h->off_wp = cv.take((size_t)batch * (N + 1) * dims * 8);
     h->off_T = cv.take((size_t)nseg * 8);
     h->off_lo = cv.take(has_box ? (size_t)nseg * dims * 8 : 0);
@@ -789,7 +899,8 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
                  o_coef = cv.take((size_t)nseg * dims * n * rb);
     // (c) iterate: written by the init kernel ...
     const size_t o_zt = cv.take(3 * LS * rb), o_chat = cv.take(3 * LS * rb), o_qp = cv.take(has_box ? 3 * LS * rb : 0),
-                 o_qn = cv.take(has_box ? 3 * LS * rb : 0), o_phv = cv.take(has_vel ? 3 * LS * rb : 0);
+                 o_qn = cv.take(has_box ? 3 * LS * rb : 0), o_phv = cv.take(has_vel ? 3 * LS * rb : 0),
+                 o_qpl = cv.take(h->has_poly ? (size_t)h->K * LS * 8 : 0);
     // ... or zero at iterate 0 (duals), together with the reduction buffers: one memset, repeated by top_reset
     const size_t o_zero = cv.off;
     const size_t o_u = cv.take(3 * LS * rb), o_wv = cv.take(has_vel ? 3 * LS * rb : 0), o_pha = cv.take(has_acc ? 3 * LS * rb : 0),
@@ -820,6 +931,10 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->d_origin = (double*)(A + o_origin); h->d_coef = A + o_coef; h->d_zt = A + o_zt; h->d_chat = A + o_chat;
     h->d_u = A + o_u; h->d_part = (double*)(A + o_part); h->d_res = (double*)(A + o_res); h->d_solve = (double*)(A + o_solve);
     if (has_box) { h->d_qp = A + o_qp; h->d_qn = A + o_qn; }
+    if (h->has_poly) {
+        h->d_rot = (double*)(A + h->off_rot); h->d_planes = (double*)(A + h->off_planes); h->d_lam3 = (double*)(A + h->off_lam3);
+        h->d_qpl = (double*)(A + o_qpl);
+    }
     if (has_vel) { h->d_phv = A + o_phv; h->d_wv = A + o_wv; }
     if (has_acc) { h->d_pha = A + o_pha; h->d_wa = A + o_wa; }
     if (h->streaming) {
@@ -829,7 +944,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->d_Bedge = A + o_Bedge; h->d_resbox = A + o_resbox; h->d_sync = A + o_sync; h->d_abort = (int*)(A + o_abort);
     h->stage.reset(new (std::nothrow) unsigned char[h->upload_bytes]);
     if (!h->stage) CREATE_FAIL(fail(h, TOP_E_NOMEM, "host allocation failed"));
-    std::memset(h->stage.get(), 0, MAXN * LS * 8);        // padded operator rows stay zero
+    std::memset(h->stage.get(), 0, h->off_wp);             // padded operator rows (and rotation / plane tables) stay zero
     h->h_res.assign((size_t)batch * 4, std::numeric_limits<double>::quiet_NaN());
     pt.mark("memory (1 cudaMalloc)");
 
@@ -870,9 +985,10 @@ extern "C" TOP_API top_status top_reset(top_solver* h, const double* waypoints, 
     if (!h) return TOP_E_INVALID;
     TOP_GUARDED(h,
         bool hb, hv, ha;
-        top_status st = validate_problem(h, h->batch, h->N, h->s, h->dims, waypoints, durations, start_derivs, end_derivs, cons, rho, &hb, &hv, &ha);
+        int kp = 0;
+        top_status st = validate_problem(h, h->batch, h->N, h->s, h->dims, waypoints, durations, start_derivs, end_derivs, cons, rho, &hb, &hv, &ha, &kp);
         if (st != TOP_OK) return st;
-        if (hb != h->has_box || hv != h->has_vel || ha != h->has_acc)
+        if (hb != h->has_box || hv != h->has_vel || ha != h->has_acc || kp != h->K)
             return fail(h, TOP_E_INVALID, "top_reset: the constraint selection (box / velocity / acceleration) must be the one the solver was created with");
         if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
         PhaseTimer pt;
@@ -943,6 +1059,7 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
                 p.W = h->d_W; p.lam = h->d_lam; p.g0 = h->d_g0; p.dp = h->d_dp;
             }
             p.max_ctas = h->max_ctas; p.rho = h->rho; p.vmax = h->vmax; p.amax = h->amax;
+            p.rot = h->d_rot; p.planes = h->d_planes; p.qpl = h->d_qpl; p.qpl_out = h->d_qpl; p.K = h->K;
             p.seq_base = (unsigned int)(h->seq_counter & 0xffffffffull);
             h->seq_counter += (unsigned long long)kk;
             if (w.ctas > 1 && !(p.flags & KF_NEIGHBOUR_SYNC))
@@ -1000,7 +1117,7 @@ extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iter
     const int rd_idx = (h->opt_flags & TOP_RD_NORMALISED) ? 2 : 1;
     // (large CTAs run the plain kernel faster than the solve instantiation -- 96-register cap -- so with a sparse
     // test cadence they keep the host loop below)
-    if (h->batch == 1 && h->waves.size() == 1 && !h->streaming && (h->lanes == 8 || h->mma) && h->waves[0].ctas <= 160 &&
+    if (h->batch == 1 && h->waves.size() == 1 && !h->streaming && !h->has_poly && (h->lanes == 8 || h->mma) && h->waves[0].ctas <= 160 &&
         (h->waves[0].threads <= 256 || h->check_every < 16)) {
         // one resident trajectory: the stop rule (and Eq. 24) runs inside the kernel, one launch for the whole solve
         InKernelSolve iks;
@@ -1059,11 +1176,31 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
     if (rho == h->rho) return TOP_OK;
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     const size_t LS = (size_t)h->stride;
+    if (h->has_poly) {
+        // polytope corridor: three operators per segment; they are rebuilt on the host for the new rho (no spectral form),
+        // uploaded, c0^ follows on the device, and the scaled duals (u, w, and v = max(0,-q) of every plane) are rescaled
+        const double old = h->rho;
+        h->rho = rho;
+        top_status so = stage_operators(h);
+        if (so != TOP_OK) { h->rho = old; return so; }
+        CU(cudaMemcpyAsync(h->d_upload, h->stage.get(), h->off_wp, cudaMemcpyHostToDevice, h->stream), "H2D operators");
+        InitParams ip;
+        std::memset(&ip, 0, sizeof ip);
+        fill_init_params(h, ip);
+        ip.c0_only = 1;
+        CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
+        RescaleParams r;
+        r.u = h->d_u; r.qp = nullptr; r.qn = nullptr; r.wv = h->d_wv; r.wa = h->d_wa;
+        r.count = 3 * (long long)LS; r.ratio = old / rho; r.qpl = h->d_qpl; r.qpl_count = (long long)h->K * (long long)LS;
+        CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
+        h->launches += 2;
+        return TOP_OK;
+    }
     { top_status se = ensure_spectral(h); if (se != TOP_OK) return se; }      // first change of rho: build W, lambda (host, once)
     CU(refresh_operator(h, rho), "operator refresh launch");      // on the device, from the spectral data
     RescaleParams r;
     r.u = h->d_u; r.qp = h->d_qp; r.qn = h->d_qn; r.wv = h->d_wv; r.wa = h->d_wa;
-    r.count = 3 * (long long)LS; r.ratio = h->rho / rho;
+    r.count = 3 * (long long)LS; r.ratio = h->rho / rho; r.qpl = nullptr; r.qpl_count = 0;
     CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
     h->launches += 1;
     h->rho = rho;
@@ -1091,6 +1228,7 @@ extern "C" TOP_API top_status top_get_coeffs(top_solver* h, void* out, int32_t o
     if (!out) return fail(h, TOP_E_INVALID, "out is NULL");
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     ConvParams p;
+    p.rot = h->d_rot;
     p.chat = h->d_chat; p.invT = h->d_invT; p.origin = h->d_origin; p.out = out_is_device ? out : h->d_coef;
     p.nseg_pad = h->nseg_pad;
     p.stride = h->stride; p.nseg = h->nseg; p.s = h->s; p.dims = h->dims;
@@ -1129,6 +1267,20 @@ extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, do
             }
         return check_abort(h);
     }
+    if (f == "s_poly" || f == "v_poly") {
+        const size_t want = (size_t)batch * N * MS * (size_t)h->K;
+        if (!h->has_poly || count != want) return fail(h, TOP_E_INVALID, "top_get_state: count does not match the field (or no polytope corridor)");
+        buf.resize((size_t)h->K * LS);
+        CU(cudaMemcpyAsync(buf.data(), h->d_qpl, buf.size() * 8, cudaMemcpyDeviceToHost, h->stream), "D2H");
+        CU(cudaStreamSynchronize(h->stream), "sync");
+        for (size_t g = 0; g < (size_t)batch * N; ++g)
+            for (int j = 0; j < MS; ++j)
+                for (int k = 0; k < h->K; ++k) {
+                    const double v = buf[(size_t)k * LS + g * LANES + j];      // Moreau pair: s = max(0,q), v = max(0,-q)
+                    out[(g * MS + j) * h->K + k] = f == "s_poly" ? std::max(0.0, v) : std::max(0.0, -v);
+                }
+        return check_abort(h);
+    }
     struct { const char* name; void* ptr; int how; bool on; } tab[] = {
         {"s_pos", h->d_qp, 1, h->has_box}, {"v_pos", h->d_qp, 2, h->has_box},
         {"s_neg", h->d_qn, 1, h->has_box}, {"v_neg", h->d_qn, 2, h->has_box},
@@ -1141,12 +1293,21 @@ extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, do
         if (!t.on) { std::fill(out, out + count, 0.0); return TOP_OK; }
         if ((st = download_real(h, t.ptr, buf, 3 * LS)) != TOP_OK) return st;
         for (size_t g = 0; g < (size_t)batch * N; ++g)
-            for (int j = 0; j < MS; ++j)
+            for (int j = 0; j < MS; ++j) {
+                double v3[3];
+                for (int d = 0; d < 3; ++d) v3[d] = buf[(size_t)d * LS + g * LANES + j];
+                if (h->has_poly) {      // ball variables live in the segment's rotated frame: x = V y
+                    const double a0 = v3[0], a1 = v3[1], a2 = v3[2];
+                    const double* R = h->h_rot.data();
+                    const size_t NPp = (size_t)h->nseg_pad;
+                    for (int d = 0; d < 3; ++d) v3[d] = R[(d * 3 + 0) * NPp + g] * a0 + R[(d * 3 + 1) * NPp + g] * a1 + R[(d * 3 + 2) * NPp + g] * a2;
+                }
                 for (int d = 0; d < dims; ++d) {
-                    const double v = buf[(size_t)d * LS + g * LANES + j];
+                    const double v = v3[d];
                     // Moreau pair of the slack projection (Eq. 10 / 20d-e): s = max(0,q), v = max(0,-q)
                     out[(g * MS + j) * dims + d] = t.how == 0 ? v : (t.how == 1 ? std::max(0.0, v) : std::max(0.0, -v));
                 }
+            }
         return check_abort(h);
     }
     return fail(h, TOP_E_INVALID, "top_get_state: unknown field '" + f + "'");
@@ -1176,7 +1337,8 @@ extern "C" TOP_API size_t top_snapshot_bytes(const top_solver* hc) {
     top_solver* h = const_cast<top_solver*>(hc);
     void* f[9];
     const int n = snapshot_fields(h, f);
-    return sizeof(SnapshotHeader) + (size_t)n * 3 * (size_t)h->stride * real_bytes(h) + (size_t)h->batch * 4 * 8;
+    return sizeof(SnapshotHeader) + (size_t)n * 3 * (size_t)h->stride * real_bytes(h) + (size_t)h->batch * 4 * 8 +
+           (h->has_poly ? (size_t)h->K * (size_t)h->stride * 8 : 0);
 }
 
 extern "C" TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, size_t bytes) {
@@ -1195,6 +1357,8 @@ extern "C" TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, s
     const size_t fb = 3 * (size_t)h->stride * real_bytes(h);
     for (int i = 0; i < n; ++i) { CU(cudaMemcpyAsync(o, f[i], fb, cudaMemcpyDeviceToHost, h->stream), "D2H snapshot"); o += fb; }
     CU(cudaMemcpyAsync(o, h->d_res, (size_t)h->batch * 4 * 8, cudaMemcpyDeviceToHost, h->stream), "D2H snapshot");
+    o += (size_t)h->batch * 4 * 8;
+    if (h->has_poly) CU(cudaMemcpyAsync(o, h->d_qpl, (size_t)h->K * (size_t)h->stride * 8, cudaMemcpyDeviceToHost, h->stream), "D2H snapshot");
     return check_abort(h);
 }
 
@@ -1214,7 +1378,19 @@ extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* ho
     const size_t fb = 3 * (size_t)h->stride * real_bytes(h);
     for (int i = 0; i < n; ++i) { CU(cudaMemcpyAsync(f[i], o, fb, cudaMemcpyHostToDevice, h->stream), "H2D snapshot"); o += fb; }
     CU(cudaMemcpyAsync(h->d_res, o, (size_t)h->batch * 4 * 8, cudaMemcpyHostToDevice, h->stream), "H2D snapshot");
-    if (hd.rho != h->rho) {
+    o += (size_t)h->batch * 4 * 8;
+    if (h->has_poly) CU(cudaMemcpyAsync(h->d_qpl, o, (size_t)h->K * (size_t)h->stride * 8, cudaMemcpyHostToDevice, h->stream), "H2D snapshot");
+    if (hd.rho != h->rho && h->has_poly) {
+        h->rho = hd.rho;
+        top_status so = stage_operators(h);
+        if (so != TOP_OK) return so;
+        CU(cudaMemcpyAsync(h->d_upload, h->stage.get(), h->off_wp, cudaMemcpyHostToDevice, h->stream), "H2D operators");
+        InitParams ip;
+        std::memset(&ip, 0, sizeof ip);
+        fill_init_params(h, ip);
+        ip.c0_only = 1;
+        CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
+    } else if (hd.rho != h->rho) {
         top_status se = ensure_spectral(h);
         if (se != TOP_OK) return se;
         CU(refresh_operator(h, hd.rho), "operator refresh launch");

@@ -10,6 +10,7 @@ constexpr int LANES = 8;        // threads per segment: lane j <-> sample j, lan
 constexpr int MS = 8;           // samples per segment (Ms)
 constexpr int MAXN = 8;         // n = 2s <= 8
 constexpr int DIMS = 3;         // flat dimensions are padded to 3 (unused ones carry zeros)
+constexpr int KMAX = 16;        // general polytope corridor: at most this many half-spaces per segment
 
 // segment flags
 constexpr uint8_t SEG_FIRST = 1;  // first segment of its trajectory: left junction (z_0) is fixed
@@ -18,7 +19,8 @@ constexpr uint8_t SEG_LAST = 2;   // last segment: right junction (z_N) is fixed
 // kernel flags
 constexpr uint32_t KF_BOX = 1, KF_VEL = 2, KF_ACC = 4, KF_PIN_POS = 8 /* PINNED_Z: position row of z held */,
                    KF_NEIGHBOUR_SYNC = 16, KF_PAIRWISE = 32 /* warp-pair named barriers instead of the CTA barrier */,
-                   KF_OPEN_LEFT = 64, KF_OPEN_RIGHT = 128 /* streaming: the launch range starts / ends inside a chain (halo) */;
+                   KF_OPEN_LEFT = 64, KF_OPEN_RIGHT = 128 /* streaming: the launch range starts / ends inside a chain (halo) */,
+                   KF_POLY = 256 /* general polytope corridor (K planes per segment, rotated per-segment frame) */;
 
 // Per-lane field arrays: element [f * stride + gseg * LANES + lane]; stride = padded lane count.
 // "Real" is double (TOP_F64) or float (TOP_F32); the x-update operator is always double.
@@ -69,9 +71,18 @@ struct KParams {
     void* resbox;           // [2][max_ctas][4] LL slots: per-CTA residual partial sums, all-gathered by every CTA
     double* solve_out;      // [8]: sweeps done, stopped (0/1), rho, r_p, r_d, r_d_norm, r_p_gap, unused
     const double *W, *lam, *g0, *dp;   // spectral operator data (RefreshParams)
+    // ---- general polytope corridor (KF_POLY; fp64 tensor-core kernel only).  Every segment works in its own rotated frame
+    // y = V'(p - o_i), V = eigenvectors of sum_k a_k a_k': there the dims decouple again (one operator per dim, Pm is
+    // [DIMS][MAXN][stride]); consensus rows are rotated in and out, the planes are stored rotated.
+    const double* rot;      // [9][nseg_pad]          V row-major: V[d][e] = component d (global) of axis e (rotated)
+    const double* planes;   // [K][4][nseg_pad]       a'_k = V'a_k (3), b'_k = b_k - a_k'o_i
+    void* qpl;              // double [K][stride]     Moreau value of (sample `lane`, plane k): s = max(0,q), v = max(0,-q)
+    void* qpl_out;
+    int K;
 };
 
 struct ConvParams {       // coefficient conversion to the paper's basis (Eq. 18)
+    const double* rot;    // [9][nseg_pad] or null: rotate the dims back to the global frame first (polytope corridor)
     const void* chat;     // Real [DIMS][stride]
     const void* invT;     // Real [2][nseg_pad]
     const double* origin; // [3][nseg_pad]  origin of each segment's local frame (added to c_0)
@@ -90,8 +101,8 @@ int max_threads_for(int dtype, int lanes);
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, int threads, size_t smem, int* max_ctas_per_sm);
 // fp64 tensor-core variant of the 4-lane kernel (top_kernels_mma.cu: cadmm_sweeps_mma_kernel)
 cudaError_t launch_sweeps_mma(const KParams& p, int s, bool constrained, int ctas, int threads, size_t smem, cudaStream_t st);
-size_t sweep_smem_bytes_mma(bool constrained, int segs_per_cta);
-int max_threads_mma();
+size_t sweep_smem_bytes_mma(bool constrained, bool poly);
+int max_threads_mma(bool poly);
 cudaError_t sweep_kernel_limits_mma(int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm);
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
 // rho Pm^ = W diag(rho/(lambda_i+rho)) W',  c0^ = c_chord - (rho Pm^) g0   (spectral form; top_api.cpp build_spectral)
@@ -124,6 +135,11 @@ struct InitParams {
     // outputs
     double *c0, *g0, *dp, *origin;
     void *invTk, *Tpow, *invT, *lohi, *zoff, *zt, *chat, *qp, *qn, *phv;
+    // polytope corridor: rotation and rotated planes (host precompute), per-dim box weight lambda_d (eigenvalues of sum a a'),
+    // and the Moreau values of the chord samples (output)
+    const double *rot, *planes, *lam3;   // [9][nseg_pad], [K][4][nseg_pad], [3][nseg_pad]
+    double* qpl;                          // [K][stride]
+    int K, has_poly, c0_only;
     uint8_t* segflags;
     long long stride, nseg_pad, nseg;
     int N, batch, s, dims, hard, has_box, has_vel, has_acc;
@@ -131,7 +147,7 @@ struct InitParams {
 };
 cudaError_t launch_init(const InitParams& p, int dtype, cudaStream_t st);
 // duals *= ratio after a change of rho: u, w (both balls), and the negative part of the Moreau values q (= -v)
-struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; };
+struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; void* qpl; long long qpl_count; };
 cudaError_t launch_rescale_duals(const RescaleParams& p, int dtype, cudaStream_t st);
 cudaError_t launch_residual_reduce(const double* part, double* res, long long N, int batch, cudaStream_t st);
 cudaError_t launch_fma_peak(int dtype, int blocks, int threads, long long iters, float* sink, cudaStream_t st);

@@ -966,8 +966,15 @@ __global__ void convert_coeffs_kernel(const ConvParams p) {
     Real sc = 1;
     for (int q = 0; q < a; ++q) sc *= invT;
     Real* out = static_cast<Real*>(p.out);
+    double c3[3];
+    for (int d = 0; d < 3; ++d) c3[d] = (double)(static_cast<const Real*>(p.chat)[d * p.stride + idx] * sc);
+    if (p.rot) {                                                  // rotated frame of the segment -> global axes
+        const double a0 = c3[0], a1 = c3[1], a2 = c3[2];
+        for (int d = 0; d < 3; ++d)
+            c3[d] = p.rot[(d * 3 + 0) * p.nseg_pad + seg] * a0 + p.rot[(d * 3 + 1) * p.nseg_pad + seg] * a1 + p.rot[(d * 3 + 2) * p.nseg_pad + seg] * a2;
+    }
     for (int d = 0; d < p.dims; ++d) {
-        double v = (double)(static_cast<const Real*>(p.chat)[d * p.stride + idx] * sc);
+        double v = c3[d];
         if (a == 0) v += p.origin[d * p.nseg_pad + seg];          // segment-local frame -> global frame
         out[(seg * p.dims + d) * (2 * p.s) + a] = (Real)v;
     }
@@ -1046,6 +1053,13 @@ __global__ void init_problem_kernel(const InitParams p) {
             static_cast<Real*>(p.lohi)[(3 + d) * NP + g] = (Real)((p.has_box && d < dims) ? p.box_hi[g * dims + d] - org[d] : 1.0);
         }
     }
+    // polytope corridor: the segment works in the rotated frame y = V'(p - o_i); the chord goes there too
+    double dpr[3] = {dp[0], dp[1], dp[2]};
+    if (p.has_poly) {
+        double V[9];
+        for (int q = 0; q < 9; ++q) V[q] = p.rot[q * NP + g];
+        for (int e = 0; e < 3; ++e) dpr[e] = V[0 * 3 + e] * dp[0] + V[1 * 3 + e] * dp[1] + V[2 * 3 + e] * dp[2];
+    }
     // G e_1 of this segment, then c0^ = c_chord - (rho Pm^)(G c_chord) with c_chord = e_1 dp in the local frame (HARD mode)
     const double iT2 = 1.0 / (T * T);
     double gcol1[MAXN];
@@ -1059,12 +1073,23 @@ __global__ void init_problem_kernel(const InitParams p) {
             if (p.has_acc) gcol1[a] += iT2 * iT2 * p.ge1[2][a];
         }
     }
-    double pg = 0.0;
-    for (int bb = 0; bb < MAXN; ++bb) pg += p.Pm[bb * LS + idx] * gcol1[bb];
-    for (int d = 0; d < 3; ++d) {
-        p.g0[d * LS + idx] = (p.hard && d < dims) ? gcol1[lane] * dp[d] : 0.0;
-        p.c0[d * LS + idx] = (p.hard && d < dims) ? ((lane == 1 ? dp[d] : 0.0) - pg * dp[d]) : 0.0;
+    if (p.has_poly) {       // one operator per rotated dim: box weight lambda_d (eigenvalue of sum_k a_k a_k') instead of 2
+        for (int d = 0; d < 3; ++d) {
+            const double lam = p.lam3[d * NP + g];
+            double pg = 0.0;
+            for (int bb = 0; bb < MAXN; ++bb) pg += p.Pm[((long long)d * MAXN + bb) * LS + idx] * (gcol1[bb] + lam * p.ge1[0][bb]);
+            p.g0[d * LS + idx] = p.hard ? (gcol1[lane] + lam * p.ge1[0][lane]) * dpr[d] : 0.0;
+            p.c0[d * LS + idx] = p.hard ? ((lane == 1 ? dpr[d] : 0.0) - pg * dpr[d]) : 0.0;
+        }
+    } else {
+        double pg = 0.0;
+        for (int bb = 0; bb < MAXN; ++bb) pg += p.Pm[bb * LS + idx] * gcol1[bb];
+        for (int d = 0; d < 3; ++d) {
+            p.g0[d * LS + idx] = (p.hard && d < dims) ? gcol1[lane] * dp[d] : 0.0;
+            p.c0[d * LS + idx] = (p.hard && d < dims) ? ((lane == 1 ? dp[d] : 0.0) - pg * dp[d]) : 0.0;
+        }
     }
+    if (p.c0_only) return;      // a new rho on a polytope solver: only c0^ follows the new operator rows
     double Tp = 1.0;
     for (int q = 0; q < lane; ++q) Tp *= T;
     static_cast<Real*>(p.Tpow)[idx] = (Real)Tp;
@@ -1102,13 +1127,13 @@ __global__ void init_problem_kernel(const InitParams p) {
         }
         static_cast<Real*>(p.zt)[d * LS + idx] = (Real)z;
         // C0 = chord at constant speed: c^_0 = 0 (local frame), c^_1 = p_i - p_{i-1}
-        static_cast<Real*>(p.chat)[d * LS + idx] = (Real)((d < dims && lane == 1) ? dp[d] : 0.0);
+        static_cast<Real*>(p.chat)[d * LS + idx] = (Real)(lane == 1 ? (p.has_poly ? dpr[d] : (d < dims ? dp[d] : 0.0)) : 0.0);
     }
     // samples of the chord: slack = max(0, .), phi = projection of the chord velocity, duals 0
     const double tau = (double)(lane + 1) / (double)(MS + 1);
     double V0[3] = {0, 0, 0};
     for (int d = 0; d < 3; ++d) {
-        if (d < dims) V0[d] = dp[d] / T;
+        if (p.has_poly) V0[d] = dpr[d] / T; else if (d < dims) V0[d] = dp[d] / T;
         if (p.has_box) {
             double a = 1.0, c = 1.0;
             if (d < dims) {
@@ -1126,12 +1151,20 @@ __global__ void init_problem_kernel(const InitParams p) {
         if (n2 > p.vmax * p.vmax) sc = p.vmax / sqrt(n2);
         for (int d = 0; d < 3; ++d) static_cast<Real*>(p.phv)[d * LS + idx] = (Real)(sc * V0[d]);
     }
+    if (p.has_poly) {       // slack of the chord sample against every plane: q = b'_k - a'_k . y_j  (s = max(0, q), v = 0)
+        for (int k = 0; k < p.K; ++k) {
+            const double a0 = p.planes[(k * 4 + 0) * NP + g], a1 = p.planes[(k * 4 + 1) * NP + g], a2 = p.planes[(k * 4 + 2) * NP + g];
+            const double q = p.planes[(k * 4 + 3) * NP + g] - tau * (a0 * dpr[0] + a1 * dpr[1] + a2 * dpr[2]);
+            p.qpl[k * LS + idx] = fmax(0.0, q);
+        }
+    }
 }
 
 // scaled duals after rho_old -> rho_new (reading A16): u, w_v, w_a *= ratio; box: v = max(0,-q) *= ratio, s unchanged
 template <typename Real>
 __global__ void rescale_duals_kernel(const RescaleParams p) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p.qpl && i < p.qpl_count) { double* q = static_cast<double*>(p.qpl); if (q[i] < 0) q[i] *= p.ratio; }
     if (i >= p.count) return;
     const Real r = (Real)p.ratio;
     static_cast<Real*>(p.u)[i] *= r;
@@ -1297,7 +1330,8 @@ cudaError_t launch_init(const InitParams& p, int dtype, cudaStream_t st) {
 
 cudaError_t launch_rescale_duals(const RescaleParams& p, int dtype, cudaStream_t st) {
     if (p.count == 0) return cudaSuccess;
-    const int blocks = (int)((p.count + 255) / 256);
+    const long long nthr = (p.qpl && p.qpl_count > p.count) ? p.qpl_count : p.count;
+    const int blocks = (int)((nthr + 255) / 256);
     if (dtype == 0) rescale_duals_kernel<double><<<blocks, 256, 0, st>>>(p);
     else rescale_duals_kernel<float><<<blocks, 256, 0, st>>>(p);
     return cudaGetLastError();

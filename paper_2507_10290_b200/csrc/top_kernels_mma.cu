@@ -61,29 +61,49 @@ __device__ __forceinline__ double ball_scale(const double (&y)[3], double bound)
     return n2 > bound * bound ? sc : 1.0;
 }
 
+// y = V'x (global -> rotated frame of the segment) and x = V y (back); V row-major 3x3 in shared memory
+__device__ __forceinline__ void rot_in(const double* V, double (&x)[3]) {
+    const double a = x[0], b = x[1], c = x[2];
+#pragma unroll
+    for (int e = 0; e < 3; ++e) x[e] = V[0 * 3 + e] * a + V[1 * 3 + e] * b + V[2 * 3 + e] * c;
+}
+__device__ __forceinline__ void rot_out(const double* V, double (&y)[3]) {
+    const double a = y[0], b = y[1], c = y[2];
+#pragma unroll
+    for (int d = 0; d < 3; ++d) y[d] = V[d * 3 + 0] * a + V[d * 3 + 1] * b + V[d * 3 + 2] * c;
+}
+
 // one instantiation: <= 288 threads (9 warps of 8 segments; 3 warps on one scheduler: 168 registers per thread)
 constexpr int MAXT_MMA = 288;
 // constraint mask of an instantiation: KF_BOX | KF_VEL | KF_ACC, or CM_RUNTIME = read the flags at run time
 constexpr int CM_RUNTIME = 8;
 
+// polytope corridor instantiations: <= 160 threads (5 warps: 40 segments; the per-plane state needs the shared memory)
+constexpr int MAXT_MMA_POLY = 160;
+constexpr int PSTR = KMAX * 4 + 2;      // doubles per segment of the plane table (padded: the 8 segments of a warp hit distinct banks)
+constexpr int VSTR = 10;                // doubles per segment of the rotation table
+
 struct SmemLayoutMma {
-    size_t pm, c0, zu, qs, ws, ph, ctab, lohi, xs, bs, zoff, total;
+    size_t pm, c0, zu, qs, ws, ph, ctab, lohi, xs, bs, zoff, qpl, pls, vs, total;
 };
-__host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc) {
+__host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc, bool poly = false) {
     SmemLayoutMma L;
     const int T = segs_alloc * 4;
     size_t off = 0;
-    L.pm = off;   off = align16(off + (size_t)2 * 4 * T * sizeof(double2));            // rho*Pm^ rows, [h][b/2][thread] pairs
+    L.pm = off;   off = align16(off + (size_t)(poly ? 3 : 1) * 2 * 4 * T * sizeof(double2));   // rho*Pm^ rows, [d (poly)][h][b/2][thread] pairs
     L.c0 = off;   off = align16(off + (size_t)6 * T * sizeof(double));                 // c0^ rows, [h][d][thread]
     L.zu = off;   off = align16(off + (size_t)6 * T * sizeof(double2));                // (z~, u) of the lane's two consensus rows, [h][d][thread]
-    L.qs = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // Moreau pair values (q+, q-) of the lane's two samples
+    L.qs = off;   off = align16(off + (size_t)(cons && !poly ? 6 : 0) * T * sizeof(double2));   // Moreau pair values (q+, q-) of the lane's two samples (box)
     L.ws = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // ball duals (w_v, w_a) of the lane's two samples
     L.ph = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // ball variables (phi_v, phi_a)
     L.ctab = off; off = align16(off + (size_t)16 * 32 * sizeof(double));               // constant MMA operands, [16][lane of warp]
-    L.lohi = off; off = align16(off + (size_t)(cons ? 6 : 0) * segs_alloc * sizeof(double));
+    L.lohi = off; off = align16(off + (size_t)(cons && !poly ? 6 : 0) * segs_alloc * sizeof(double));
     L.xs = off;   off = align16(off + (size_t)segs_alloc * XSTRIDE * sizeof(double));  // rhs rows, all-gather
     L.bs = off;   off = align16(off + (size_t)2 * (segs_alloc + 2) * 24 * sizeof(double));   // boundary rows, double buffered
     L.zoff = off; off = align16(off + (size_t)6 * segs_alloc * sizeof(double));        // frame shift of the neighbours' position rows
+    L.qpl = off;  off = align16(off + (size_t)(poly ? KMAX * 2 : 0) * T * sizeof(double));          // Moreau values per (plane, sample of the lane)
+    L.pls = off;  off = align16(off + (size_t)(poly ? segs_alloc : 0) * PSTR * sizeof(double));     // rotated planes (a'_k, b'_k) per segment
+    L.vs = off;   off = align16(off + (size_t)(poly ? segs_alloc : 0) * VSTR * sizeof(double));     // rotation V per segment
     L.total = off;
     return L;
 }
@@ -114,11 +134,12 @@ __device__ __noinline__ void refresh_operator_rows(const KParams& p, long long g
     for (int d = 0; d < 3; ++d) c0_row[d * TS] = c0n[d];
 }
 
-template <int S, int CM, int MAXT, bool SOLVE>
+template <int S, int CM, int MAXT, bool SOLVE, bool POLY = false>
 __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams p) {
     constexpr int N2 = 2 * S;
     constexpr int LPS = 4;                         // lanes per segment
-    constexpr bool CONS = CM != 0;
+    constexpr bool CONS = CM != 0 || POLY;
+    static_assert(!(SOLVE && POLY), "the in-kernel stop rule is not instantiated for polytope corridors (host loop)");
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int T = blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
@@ -132,14 +153,14 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     const int SEGS = p.segs_per_cta;
     const int cta = blockIdx.x, nctas = gridDim.x;
     const uint32_t flags = p.flags;
-    const bool has_box = CM == CM_RUNTIME ? (flags & KF_BOX) != 0 : (CM & (int)KF_BOX) != 0;
+    const bool has_box = POLY ? false : (CM == CM_RUNTIME ? (flags & KF_BOX) != 0 : (CM & (int)KF_BOX) != 0);
     const bool has_vel = CM == CM_RUNTIME ? (flags & KF_VEL) != 0 : (CM & (int)KF_VEL) != 0;
     const bool has_acc = CM == CM_RUNTIME ? (flags & KF_ACC) != 0 : (CM & (int)KF_ACC) != 0;
     const bool pin_pos = flags & KF_PIN_POS;
     const bool nb_sync = flags & KF_NEIGHBOUR_SYNC;
 
-    const SmemLayoutMma L = smem_layout_mma(CONS, SA);
-    double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + tid;          // [(h*4 + b/2) * TS]
+    const SmemLayoutMma L = smem_layout_mma(CONS, SA, POLY);
+    double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + tid;          // [((d*2 +) h*4 + b/2) * TS]   (d only with POLY)
     double* c0s = reinterpret_cast<double*>(smem_raw + L.c0) + tid;            // [(h*3 + d) * TS]
     double2* zus = reinterpret_cast<double2*>(smem_raw + L.zu) + tid;          // [(h*3 + d) * TS]: (z~, u)
     double2* qs = reinterpret_cast<double2*>(smem_raw + L.qs) + tid;           // [(h*3 + d) * TS]: (q+, q-)
@@ -150,6 +171,10 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE;
     double* Bs = reinterpret_cast<double*>(smem_raw + L.bs);                   // [2 parity][SA+2][8 rows][3]
     double* zoffs = reinterpret_cast<double*>(smem_raw + L.zoff) + sl;         // [(side*3 + d) * SA]
+    double* qpls = reinterpret_cast<double*>(smem_raw + L.qpl) + tid;          // [(k*2 + h) * TS]
+    double* pls = reinterpret_cast<double*>(smem_raw + L.pls) + (size_t)sl * PSTR;   // [k*4 + c]
+    double* vs = reinterpret_cast<double*>(smem_raw + L.vs) + (size_t)sl * VSTR;     // V[d][e] at d*3 + e
+    const int KP = POLY ? p.K : 0;
 
     const long long cta_first = p.seg_begin + (long long)cta * SEGS;
     const long long remaining = p.seg_end - cta_first;
@@ -210,14 +235,17 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
 #pragma unroll
-        for (int b = 0; b < 8; b += 2)
-            Pms[(h * 4 + (b >> 1)) * TS] = make_double2(b < N2 ? p.Pm[b * stride + gt[h]] : 0.0, b + 1 < N2 ? p.Pm[(b + 1) * stride + gt[h]] : 0.0);
+        for (int dd = 0; dd < (POLY ? 3 : 1); ++dd)
+#pragma unroll
+            for (int b = 0; b < 8; b += 2)
+                Pms[((dd * 2 + h) * 4 + (b >> 1)) * TS] = make_double2(b < N2 ? p.Pm[((long long)dd * MAXN + b) * stride + gt[h]] : 0.0,
+                                                                   b + 1 < N2 ? p.Pm[((long long)dd * MAXN + b + 1) * stride + gt[h]] : 0.0);
 #pragma unroll
         for (int d = 0; d < 3; ++d) c0s[(h * 3 + d) * TS] = p.c0[d * stride + gt[h]];
         invTk[h] = static_cast<const double*>(p.invTk)[gt[h]];
     }
     const double invT = static_cast<const double*>(p.invT)[gseg], invT2 = static_cast<const double*>(p.invT)[p.nseg_pad + gseg];
-    if (CONS) {
+    if (CONS && !POLY) {
         lohi[lane * SA] = static_cast<const double*>(p.lohi)[lane * p.nseg_pad + gseg];
         if (lane < 2) lohi[(lane + 4) * SA] = static_cast<const double*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
     }
@@ -225,6 +253,14 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         zoffs[lane * SA] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + 0];
         zoffs[(3 + lane) * SA] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + S];
     }
+    if (POLY) {
+        for (int i = lane; i < 9; i += LPS) vs[i] = p.rot[i * p.nseg_pad + gseg];
+        for (int i = lane; i < KP * 4; i += LPS) pls[i] = p.planes[i * p.nseg_pad + gseg];
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+            for (int k = 0; k < KP; ++k) qpls[(k * 2 + h) * TS] = static_cast<const double*>(p.qpl)[k * stride + gt[h]];
+    }
+    __syncwarp();
     const uint8_t sf = p.segflags[gseg];
     const bool open_l = (flags & KF_OPEN_LEFT) && gseg == p.seg_begin, open_r = (flags & KF_OPEN_RIGHT) && gseg == p.seg_end - 1;
 
@@ -280,6 +316,17 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             if (has_acc) { w_a = static_cast<const double*>(p.wa)[i]; ph_a = static_cast<const double*>(p.pha)[i]; ga[h][d] = (ph_a - w_a) * invT2; }
             if (CONS) { ws[(h * 3 + d) * TS] = make_double2(w_v, w_a); phs[(h * 3 + d) * TS] = make_double2(ph_v, ph_a); }
         }
+    if (POLY) {      // consensus rows enter the segment's rotated frame; the E0 operand is sum_k (b_k - s_k - v_k) a_k
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            rot_in(vs, gM[h]);
+            for (int k = 0; k < KP; ++k) {
+                const double2 a01 = *reinterpret_cast<const double2*>(pls + k * 4), a2b = *reinterpret_cast<const double2*>(pls + k * 4 + 2);
+                const double g = a2b.y - fabs(qpls[(k * 2 + h) * TS]);
+                A0[h][0] += g * a01.x; A0[h][1] += g * a01.y; A0[h][2] += g * a2b.x;
+            }
+        }
+    }
 
     const double vmax = p.vmax, amax = p.amax;
     unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
@@ -310,12 +357,15 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 
         // ================= phase A: segment local =================
         // operator rows and c0 of this lane: issued first, they arrive while the MMAs of a1 run
+        // (polytope corridor: one operator per rotated dim, read inside the dim loop of a2)
         double2 pm[2][4];
         double cacc[2][3];
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
+            if (!POLY) {
 #pragma unroll
-            for (int b = 0; b < 4; ++b) pm[h][b] = Pms[(h * 4 + b) * TS];
+                for (int b = 0; b < 4; ++b) pm[h][b] = Pms[(h * 4 + b) * TS];
+            }
 #pragma unroll
             for (int d = 0; d < 3; ++d) cacc[h][d] = c0s[(h * 3 + d) * TS];
         }
@@ -328,7 +378,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             for (int h = 0; h < 2; ++h)
 #pragma unroll
                 for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gM[h][d], ctab[h * 32]);
-            if (has_box) {      // Ao'(b - s - v), Ao = [E0; -E0], b = [hi; -lo];  s + v = |q| (Moreau pair)
+            if (has_box || POLY) {      // Ao'(b - s - v): box Ao = [E0; -E0], b = [hi; -lo], s + v = |q| (Moreau pair); polytope: kron(E0, a_k')
 #pragma unroll
                 for (int h = 0; h < 2; ++h)
 #pragma unroll
@@ -353,6 +403,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         // a2: x-update  c^ = (rho Pm^) R^ + c0^   (Eq. 20a first bracket, precomputed per segment): rows lane, lane+4
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
+            if (POLY) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int b = 0; b < 4; ++b) pm[h][b] = Pms[((d * 2 + h) * 4 + b) * TS];
+            }
 #pragma unroll
             for (int b = 0; b < N2 / 2; ++b) {
                 const double2 x2 = *reinterpret_cast<const double2*>(Xs + d * 8 + 2 * b);
@@ -380,6 +436,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 0) * 32]);
                 Bnd[0][d] = e0 * invTk[0]; Bnd[1][d] = e1 * invTk[1];
             }
+            if (POLY) { rot_out(vs, Bnd[0]); rot_out(vs, Bnd[1]); }      // consensus lives in the global frame
             // publish: shared memory for the neighbours in this CTA (and for this lane's own phase B), mailbox for the
             // neighbouring CTAs
 #pragma unroll
@@ -412,7 +469,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
                 for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = e0; Av[1][d] = e1; }
             }
-            if (has_box) {
+            if (has_box || POLY) {
 #pragma unroll
                 for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 1) * 32]); Pv[0][d] = e0; Pv[1][d] = e1; }
             }
@@ -456,6 +513,21 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 for (int h = 0; h < 2; ++h)
 #pragma unroll
                     for (int d = 0; d < 3; ++d) { ws[(h * 3 + d) * TS] = w2[h][d]; phs[(h * 3 + d) * TS] = ph2[h][d]; }
+            }
+            if (POLY) {         // a7 + a8 per (sample, plane): q = -(a_k'p - b_k + v);  next operand sum_k (b_k - |q_k|) a_k
+#pragma unroll
+                for (int h = 0; h < 2; ++h) A0[h][0] = A0[h][1] = A0[h][2] = 0.0;
+                for (int k = 0; k < KP; ++k) {
+                    const double2 a01 = *reinterpret_cast<const double2*>(pls + k * 4), a2b = *reinterpret_cast<const double2*>(pls + k * 4 + 2);
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const double val = a01.x * Pv[h][0] + a01.y * Pv[h][1] + a2b.x * Pv[h][2];
+                        const double qn_ = (a2b.y - val) - neg_part(qpls[(k * 2 + h) * TS]);
+                        qpls[(k * 2 + h) * TS] = qn_;
+                        const double g = a2b.y - fabs(qn_);
+                        A0[h][0] += g * a01.x; A0[h][1] += g * a01.y; A0[h][2] += g * a2b.x;
+                    }
+                }
             }
             if (has_box) {      // a7 + a8: Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q);  next operand
 #pragma unroll
@@ -546,6 +618,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     if (gaprow[h]) { const double gp = own[h][d] - nb[h][d]; gap2 += gp * gp; }   // Eq. 21
                 }
             }
+        if (POLY) { rot_in(vs, gM[0]); rot_in(vs, gM[1]); }
         if (last_sweep) {
             // a6: dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8):
             // the consensus block of the a1 contraction applied to dz; lane t ends with coefficient rows 2t, 2t+1
@@ -668,6 +741,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 static_cast<double*>(p.zt_out)[i] = zz.x;
                 static_cast<double*>(p.u_out)[i] = zz.y;
                 if (has_box) { const double2 q = qs[(h * 3 + d) * TS]; static_cast<double*>(p.qp_out)[i] = q.x; static_cast<double*>(p.qn_out)[i] = q.y; }
+                if (POLY && d == 0) for (int k = 0; k < KP; ++k) static_cast<double*>(p.qpl_out)[k * stride + gt[h]] = qpls[(k * 2 + h) * TS];
                 if (has_vel || has_acc) {
                     const double2 w2 = ws[(h * 3 + d) * TS], ph = phs[(h * 3 + d) * TS];
                     if (has_vel) { static_cast<double*>(p.wv_out)[i] = w2.x; static_cast<double*>(p.phv_out)[i] = ph.x; }
@@ -696,6 +770,24 @@ cudaError_t limits_mma(int threads, size_t smem, int* per_sm) {
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
 }
 
+template <int S>
+cudaError_t launch_mma_poly(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
+    auto kern = cadmm_sweeps_mma_kernel<S, CM_RUNTIME, MAXT_MMA_POLY, false, true>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    KParams pc = p;
+    void* args[] = {&pc};
+    if (ctas > 1) return cudaLaunchCooperativeKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+    return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+}
+template <int S>
+cudaError_t limits_mma_poly(int threads, size_t smem, int* per_sm) {
+    auto kern = cadmm_sweeps_mma_kernel<S, CM_RUNTIME, MAXT_MMA_POLY, false, true>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
+}
+
 // constraint selection -> instantiation: none, box + velocity, box + velocity + acceleration; anything else at run time
 int mma_mask(uint32_t kflags) {
     const int m = (int)(kflags & (KF_BOX | KF_VEL | KF_ACC));
@@ -709,10 +801,14 @@ int mma_mask(uint32_t kflags) {
     if (s == 3) { if (cm == 0) { CALL(3, 0) } else if (cm == 3) { CALL(3, 3) } else if (cm == 7) { CALL(3, 7) } else { CALL(3, CM_RUNTIME) } } \
     else        { if (cm == 0) { CALL(4, 0) } else if (cm == 3) { CALL(4, 3) } else if (cm == 7) { CALL(4, 7) } else { CALL(4, CM_RUNTIME) } }
 
-int max_threads_mma() { return MAXT_MMA; }
+int max_threads_mma(bool poly) { return poly ? MAXT_MMA_POLY : MAXT_MMA; }
 
 cudaError_t launch_sweeps_mma(const KParams& p, int s, bool /*constrained*/, int ctas, int threads, size_t smem, cudaStream_t st) {
     const uint32_t kflags = p.flags;
+    if (kflags & KF_POLY) {
+        if (p.check_every > 0) return cudaErrorInvalidValue;      // host loop only
+        return s == 3 ? launch_mma_poly<3>(p, ctas, threads, smem, st) : launch_mma_poly<4>(p, ctas, threads, smem, st);
+    }
 #define CALL(S_, C_) return launch_mma<S_, C_, MAXT_MMA>(p, ctas, threads, smem, st);
     TOP_DISPATCH_MMA(CALL)
 #undef CALL
@@ -720,14 +816,15 @@ cudaError_t launch_sweeps_mma(const KParams& p, int s, bool /*constrained*/, int
 }
 
 cudaError_t sweep_kernel_limits_mma(int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm) {
+    if (kflags & KF_POLY) return s == 3 ? limits_mma_poly<3>(threads, smem, max_ctas_per_sm) : limits_mma_poly<4>(threads, smem, max_ctas_per_sm);
 #define CALL(S_, C_) return limits_mma<S_, C_, MAXT_MMA>(threads, smem, max_ctas_per_sm);
     TOP_DISPATCH_MMA(CALL)
 #undef CALL
     return cudaErrorInvalidValue;
 }
 
-size_t sweep_smem_bytes_mma(bool constrained, int /*segs_per_cta*/) {
-    return smem_layout_mma(constrained, MAXT_MMA / 4).total;      // laid out for the largest CTA (see the kernel)
+size_t sweep_smem_bytes_mma(bool constrained, bool poly) {      // laid out for the largest CTA of the instantiation (see the kernel)
+    return poly ? smem_layout_mma(true, MAXT_MMA_POLY / 4, true).total : smem_layout_mma(constrained, MAXT_MMA / 4).total;
 }
 
 }  // namespace top

@@ -37,7 +37,8 @@ class TopError(RuntimeError):
 
 class _Constraints(ctypes.Structure):
     _fields_ = [("samples", ctypes.c_int32), ("box_lo", ctypes.POINTER(ctypes.c_double)),
-                ("box_hi", ctypes.POINTER(ctypes.c_double)), ("vmax", ctypes.c_double), ("amax", ctypes.c_double)]
+                ("box_hi", ctypes.POINTER(ctypes.c_double)), ("vmax", ctypes.c_double), ("amax", ctypes.c_double),
+                ("num_planes", ctypes.c_int32), ("planes", ctypes.POINTER(ctypes.c_double))]
 
 
 class _Options(ctypes.Structure):
@@ -156,7 +157,7 @@ class TopSolver:
     def __init__(self, waypoints, durations, s, rho, dtype="f64", samples=0, box_lo=None, box_hi=None, vmax=0.0,
                  amax=0.0, start_derivs=None, end_derivs=None, mode="hard", rd_normalised=False, eps_n_scaled=False,
                  sync="auto", check_every=0, max_iter=0, device=-1, stream=0, segs_per_cta=0, lanes=0, adaptive_rho=False,
-                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0, no_mma=False):
+                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0, no_mma=False, planes=None):
         L = lib()
         wp = np.asarray(waypoints, dtype=np.float64)
         T = np.asarray(durations, dtype=np.float64)
@@ -166,6 +167,7 @@ class TopSolver:
             box_hi = None if box_hi is None else np.asarray(box_hi)[None]
             start_derivs = None if start_derivs is None else np.asarray(start_derivs)[None]
             end_derivs = None if end_derivs is None else np.asarray(end_derivs)[None]
+            planes = None if planes is None else np.asarray(planes)[None]
         if wp.ndim != 3 or T.ndim != 2 or wp.shape[0] != T.shape[0] or wp.shape[1] != T.shape[1] + 1:
             raise ValueError("waypoints [batch,N+1,dims] and durations [batch,N] do not match")
         wp, T = _f64(wp), _f64(T)
@@ -178,8 +180,12 @@ class TopSolver:
         sd = _f64(start_derivs, (self.batch, self.s - 1, self.dims))
         ed = _f64(end_derivs, (self.batch, self.s - 1, self.dims))
         cons = None
+        pl = None if planes is None else _f64(planes)
+        if pl is not None and (pl.ndim != 4 or pl.shape[:2] != (self.batch, self.N) or pl.shape[3] != self.dims + 1):
+            raise ValueError("planes must be [batch, N, K, dims+1]")
+        self.K = 0 if pl is None else pl.shape[2]
         if samples:
-            cons = _Constraints(int(samples), _dptr(lo), _dptr(hi), float(vmax), float(amax))
+            cons = _Constraints(int(samples), _dptr(lo), _dptr(hi), float(vmax), float(amax), self.K, _dptr(pl))
         flags = WAYPOINT[mode] | (TOP_RD_NORMALISED if rd_normalised else 0) | \
             (TOP_EPS_N_SCALED if eps_n_scaled else 0) | SYNC[sync] | (TOP_RHO_ADAPTIVE if adaptive_rho else 0) | \
             (TOP_KERNEL_NO_MMA if no_mma else 0)
@@ -212,7 +218,7 @@ class TopSolver:
             pass
 
     def reset(self, waypoints, durations, rho, box_lo=None, box_hi=None, vmax=0.0, amax=0.0, start_derivs=None,
-              end_derivs=None):
+              end_derivs=None, planes=None):
         """top_reset: a new problem of the same shape on this handle (no allocation)."""
         wp = np.asarray(waypoints, dtype=np.float64)
         T = np.asarray(durations, dtype=np.float64)
@@ -222,10 +228,12 @@ class TopSolver:
             box_hi = None if box_hi is None else np.asarray(box_hi)[None]
             start_derivs = None if start_derivs is None else np.asarray(start_derivs)[None]
             end_derivs = None if end_derivs is None else np.asarray(end_derivs)[None]
+            planes = None if planes is None else np.asarray(planes)[None]
+        pl = _f64(planes, (self.batch, self.N, self.K, self.dims + 1)) if planes is not None else None
         wp, T = _f64(wp, (self.batch, self.N + 1, self.dims)), _f64(T, (self.batch, self.N))
         lo = _f64(box_lo, (self.batch, self.N, self.dims)); hi = _f64(box_hi, (self.batch, self.N, self.dims))
         sd = _f64(start_derivs, (self.batch, self.s - 1, self.dims)); ed = _f64(end_derivs, (self.batch, self.s - 1, self.dims))
-        cons = _Constraints(self.Ms, _dptr(lo), _dptr(hi), float(vmax), float(amax)) if self.Ms else None
+        cons = _Constraints(self.Ms, _dptr(lo), _dptr(hi), float(vmax), float(amax), 0 if pl is None else self.K, _dptr(pl)) if self.Ms else None
         self._check(self._L.top_reset(self._h, _dptr(wp), _dptr(T), _dptr(sd), _dptr(ed),
                                       ctypes.byref(cons) if cons is not None else None, float(rho)))
         self.durations = T
@@ -275,7 +283,10 @@ class TopSolver:
     _STATE_SHAPES = {"z": lambda o: (o.batch, o.N + 1, o.s, o.dims), "u": lambda o: (o.batch, o.N, 2 * o.s, o.dims)}
 
     def state(self, field: str):
-        shape = self._STATE_SHAPES.get(field, lambda o: (o.batch, o.N, 8, o.dims))(self)
+        if field in ("s_poly", "v_poly"):
+            shape = (self.batch, self.N, 8, self.K)
+        else:
+            shape = self._STATE_SHAPES.get(field, lambda o: (o.batch, o.N, 8, o.dims))(self)
         out = np.zeros(shape)
         self._check(self._L.top_get_state(self._h, field.encode(), _dptr(out), out.size))
         return out
@@ -305,4 +316,5 @@ def from_workload(w, b0: int = 0, b1: Optional[int] = None, **kw) -> TopSolver:
     sl = slice(b0, b1)
     return TopSolver(w.waypoints[sl], w.durations[sl], w.s, w.rho, dtype=kw.pop("dtype", w.dtype), samples=w.samples,
                      box_lo=None if w.box_lo is None else w.box_lo[sl],
-                     box_hi=None if w.box_hi is None else w.box_hi[sl], vmax=w.vmax, amax=w.amax, **kw)
+                     box_hi=None if w.box_hi is None else w.box_hi[sl], vmax=w.vmax, amax=w.amax,
+                     planes=None if getattr(w, "planes", None) is None else w.planes[sl], **kw)

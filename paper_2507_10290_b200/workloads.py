@@ -42,6 +42,7 @@ class Workload:
     box_hi: Optional[np.ndarray] = None
     vmax: float = 0.0
     amax: float = 0.0
+    planes: Optional[np.ndarray] = None   # general polytope corridor [batch, N, K, dims+1]: a_k'p <= b_k (replaces the box)
     sweeps: int = 0            # fixed sweep count of the config (0 = run to eps)
     eps: float = 0.0           # tolerance of the config (0 = fixed sweeps)
     notes: dict = field(default_factory=dict)
@@ -161,6 +162,24 @@ def small_constrained(seed: int = 7, N: int = 37, s: int = 4, acc: bool = True, 
         LO[b], HI[b] = _chord_box(pts, h)
     return Workload("small_N%d_s%d" % (N, s), batch, N, s, dims, "f64", P, T, rho=10.0, samples=8,
                     box_lo=LO, box_hi=HI, vmax=3.0, amax=5.0 if acc else 0.0)
+
+
+def polytope_corridor(w: Workload, K: int = 8, seed: int = 3, margin=(0.3, 1.5)) -> Workload:
+    """Replace the box corridor of `w` by K oblique half-spaces per segment (a convex cell around the chord, as the cells
+    of a FIRI flight corridor are): random unit normals, offset = the larger of a'p over the segment's two
+    waypoints + a margin.  Holds no method arithmetic: only draws the sets."""
+    rng = np.random.default_rng(seed)
+    pl = np.zeros((w.batch, w.N, K, w.dims + 1))
+    for b in range(w.batch):
+        for i in range(w.N):
+            a = rng.standard_normal((K, w.dims))
+            a /= np.sqrt((a * a).sum(axis=1, keepdims=True))
+            p0, p1 = w.waypoints[b, i], w.waypoints[b, i + 1]
+            pl[b, i, :, :w.dims] = a
+            pl[b, i, :, w.dims] = np.maximum(a @ p0, a @ p1) + rng.uniform(margin[0], margin[1], size=K)
+    w.planes, w.box_lo, w.box_hi = pl, None, None
+    w.name += "_poly%d" % K
+    return w
 
 
 def fig5_curve(theta: np.ndarray) -> np.ndarray:
