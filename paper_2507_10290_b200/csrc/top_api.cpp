@@ -423,9 +423,9 @@ int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 // the sweep kernel family of a solver: 8 lanes, 4 lanes (shuffle form), or 4 lanes with fp64 tensor-core contractions
 size_t kernel_smem(int dtype, int s, bool constrained, int lanes, bool mma, int segs, bool poly = false) {
-    return mma ? sweep_smem_bytes_mma(constrained, poly) : sweep_smem_bytes(dtype, s, constrained, lanes, segs);
+    return mma ? sweep_smem_bytes_mma(dtype, constrained, poly) : sweep_smem_bytes(dtype, s, constrained, lanes, segs);
 }
-int kernel_max_threads(int dtype, int lanes, bool mma, bool poly = false) { return mma ? max_threads_mma(poly) : max_threads_for(dtype, lanes); }
+int kernel_max_threads(int dtype, int lanes, bool mma, bool poly = false) { return mma ? max_threads_mma(dtype, poly) : max_threads_for(dtype, lanes); }
 
 // largest segments-per-CTA (multiple of 4) whose threads and shared memory fit one CTA
 int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, bool mma, size_t smem_limit, bool poly = false) {
@@ -818,8 +818,8 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     // (configs 1, 3) stay on the 8-lane kernel (0.64 vs 0.85, 1.42 vs 1.57)
     if (!o.lanes_per_segment && dtype == TOP_F64 && ((has_box || has_vel || has_acc) || nseg >= (long long)h->num_sms * 32)) h->lanes = 4;
     if (!o.lanes_per_segment && h->has_poly) h->lanes = 4;
-    h->mma = dtype == TOP_F64 && h->lanes == 4 && !(o.flags & TOP_KERNEL_NO_MMA);
-    if (h->has_poly && !h->mma)
+    h->mma = h->lanes == 4 && !(o.flags & TOP_KERNEL_NO_MMA);
+    if (h->has_poly && !(h->mma && dtype == TOP_F64))
         CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "polytope corridors run on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA)"));
     const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192, h->has_poly);
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
@@ -867,7 +867,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     }
     for (const auto& w : h->waves) {
         int per_sm = 0;
-        cudaError_t e = h->mma ? sweep_kernel_limits_mma(s, h->kflags, w.threads, w.smem, &per_sm)
+        cudaError_t e = h->mma ? sweep_kernel_limits_mma(h->dtype, s, h->kflags, w.threads, w.smem, &per_sm)
                                : sweep_kernel_limits(h->dtype, s, h->constrained, h->lanes, w.threads, w.smem, &per_sm);
         if (e != cudaSuccess) CREATE_FAIL(cuda_fail(h, e, "occupancy query"));
         if (per_sm < 1) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "sweep kernel does not fit an SM"));
@@ -1064,7 +1064,7 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
             h->seq_counter += (unsigned long long)kk;
             if (w.ctas > 1 && !(p.flags & KF_NEIGHBOUR_SYNC))
                 CU(cudaMemsetAsync(h->d_sync, 0, 8, h->stream), "cudaMemsetAsync");
-            CU(h->mma ? launch_sweeps_mma(p, h->s, h->constrained, w.ctas, w.threads, w.smem, h->stream)
+            CU(h->mma ? launch_sweeps_mma(p, h->dtype, h->s, w.ctas, w.threads, w.smem, h->stream)
                       : launch_sweeps(p, h->dtype, h->s, h->constrained, h->lanes, w.ctas, w.threads, w.smem, h->stream), "sweep kernel launch");
             h->launches += 1;
         }
@@ -1435,7 +1435,7 @@ extern "C" TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dty
         cudaDeviceGetAttribute(&smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev) != cudaSuccess) { cudaGetLastError(); return -1; }
     // the same rule top_create applies (kernel family of a long chain, shared-memory reserve)
     const int lanes = 4;
-    const bool mma = dtype == TOP_F64;
+    const bool mma = true;
     return (int64_t)sms * max_segs_per_cta((int)dtype, s, constrained != 0, lanes, mma, (size_t)smem - 8192);
 }
 

@@ -100,10 +100,10 @@ size_t sweep_smem_bytes(int dtype, int s, bool constrained, int lanes, int segs_
 int max_threads_for(int dtype, int lanes);
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, int threads, size_t smem, int* max_ctas_per_sm);
 // fp64 tensor-core variant of the 4-lane kernel (top_kernels_mma.cu: cadmm_sweeps_mma_kernel)
-cudaError_t launch_sweeps_mma(const KParams& p, int s, bool constrained, int ctas, int threads, size_t smem, cudaStream_t st);
-size_t sweep_smem_bytes_mma(bool constrained, bool poly);
-int max_threads_mma(bool poly);
-cudaError_t sweep_kernel_limits_mma(int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm);
+cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st);
+size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly);
+int max_threads_mma(int dtype, bool poly);
+cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm);
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
 // rho Pm^ = W diag(rho/(lambda_i+rho)) W',  c0^ = c_chord - (rho Pm^) g0   (spectral form; top_api.cpp build_spectral)
 struct RefreshParams {

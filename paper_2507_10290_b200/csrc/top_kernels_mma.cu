@@ -54,12 +54,26 @@ __device__ __forceinline__ double neg_part(double q) {
     return __hiloint2double((hi ^ 0x80000000) & m, lo & m);
 }
 
-// Eq. 20f without a branch: the factor min(1, bound/||y||) of the projection of y onto ||.|| <= bound (reading A15)
-__device__ __forceinline__ double ball_scale(const double (&y)[3], double bound) {
-    const double n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
-    const double sc = bound * rsqrt_pos(n2);               // garbage (inf/NaN) when n2 == 0: not selected then
-    return n2 > bound * bound ? sc : 1.0;
+__device__ __forceinline__ float rsqrt_pos(float x) { return rsqrtf(x); }
+__device__ __forceinline__ float neg_part(float q) {
+    const int b = __float_as_int(q);
+    return __int_as_float((b ^ 0x80000000) & (b >> 31));
 }
+
+// Eq. 20f without a branch: the factor min(1, bound/||y||) of the projection of y onto ||.|| <= bound (reading A15)
+template <typename Real>
+__device__ __forceinline__ Real ball_scale(const Real (&y)[3], Real bound) {
+    const Real n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+    const Real sc = bound * rsqrt_pos(n2);                 // garbage (inf/NaN) when n2 == 0: not selected then
+    return n2 > bound * bound ? sc : (Real)1;
+}
+
+// the state of a lane lives in shared memory as pairs
+template <typename Real> struct Pair;
+template <> struct Pair<double> { typedef double2 type; };
+template <> struct Pair<float> { typedef float2 type; };
+__device__ __forceinline__ double2 make2(double a, double b) { return make_double2(a, b); }
+__device__ __forceinline__ float2 make2(float a, float b) { return make_float2(a, b); }
 
 // y = V'x (global -> rotated frame of the segment) and x = V y (back); V row-major 3x3 in shared memory
 __device__ __forceinline__ void rot_in(const double* V, double (&x)[3]) {
@@ -75,6 +89,7 @@ __device__ __forceinline__ void rot_out(const double* V, double (&y)[3]) {
 
 // one instantiation: <= 288 threads (9 warps of 8 segments; 3 warps on one scheduler: 168 registers per thread)
 constexpr int MAXT_MMA = 288;
+constexpr int MAXT_MMA_F32 = 384;
 // constraint mask of an instantiation: KF_BOX | KF_VEL | KF_ACC, or CM_RUNTIME = read the flags at run time
 constexpr int CM_RUNTIME = 8;
 
@@ -86,21 +101,21 @@ constexpr int VSTR = 10;                // doubles per segment of the rotation t
 struct SmemLayoutMma {
     size_t pm, c0, zu, qs, ws, ph, ctab, lohi, xs, bs, zoff, qpl, pls, vs, total;
 };
-__host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc, bool poly = false) {
+__host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc, bool poly = false, int rb = 8) {
     SmemLayoutMma L;
     const int T = segs_alloc * 4;
     size_t off = 0;
     L.pm = off;   off = align16(off + (size_t)(poly ? 3 : 1) * 2 * 4 * T * sizeof(double2));   // rho*Pm^ rows, [d (poly)][h][b/2][thread] pairs
     L.c0 = off;   off = align16(off + (size_t)6 * T * sizeof(double));                 // c0^ rows, [h][d][thread]
-    L.zu = off;   off = align16(off + (size_t)6 * T * sizeof(double2));                // (z~, u) of the lane's two consensus rows, [h][d][thread]
-    L.qs = off;   off = align16(off + (size_t)(cons && !poly ? 6 : 0) * T * sizeof(double2));   // Moreau pair values (q+, q-) of the lane's two samples (box)
-    L.ws = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // ball duals (w_v, w_a) of the lane's two samples
-    L.ph = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * sizeof(double2));   // ball variables (phi_v, phi_a)
+    L.zu = off;   off = align16(off + (size_t)6 * T * 2 * rb);                // (z~, u) of the lane's two consensus rows, [h][d][thread]
+    L.qs = off;   off = align16(off + (size_t)(cons && !poly ? 6 : 0) * T * 2 * rb);   // Moreau pair values (q+, q-) of the lane's two samples (box)
+    L.ws = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * 2 * rb);   // ball duals (w_v, w_a) of the lane's two samples
+    L.ph = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * 2 * rb);   // ball variables (phi_v, phi_a)
     L.ctab = off; off = align16(off + (size_t)16 * 32 * sizeof(double));               // constant MMA operands, [16][lane of warp]
-    L.lohi = off; off = align16(off + (size_t)(cons && !poly ? 6 : 0) * segs_alloc * sizeof(double));
+    L.lohi = off; off = align16(off + (size_t)(cons && !poly ? 6 : 0) * segs_alloc * rb);
     L.xs = off;   off = align16(off + (size_t)segs_alloc * XSTRIDE * sizeof(double));  // rhs rows, all-gather
-    L.bs = off;   off = align16(off + (size_t)2 * (segs_alloc + 2) * 24 * sizeof(double));   // boundary rows, double buffered
-    L.zoff = off; off = align16(off + (size_t)6 * segs_alloc * sizeof(double));        // frame shift of the neighbours' position rows
+    L.bs = off;   off = align16(off + (size_t)2 * (segs_alloc + 2) * 24 * rb);   // boundary rows, double buffered
+    L.zoff = off; off = align16(off + (size_t)6 * segs_alloc * rb);        // frame shift of the neighbours' position rows
     L.qpl = off;  off = align16(off + (size_t)(poly ? KMAX * 2 : 0) * T * sizeof(double));          // Moreau values per (plane, sample of the lane)
     L.pls = off;  off = align16(off + (size_t)(poly ? segs_alloc : 0) * PSTR * sizeof(double));     // rotated planes (a'_k, b'_k) per segment
     L.vs = off;   off = align16(off + (size_t)(poly ? segs_alloc : 0) * VSTR * sizeof(double));     // rotation V per segment
@@ -134,12 +149,17 @@ __device__ __noinline__ void refresh_operator_rows(const KParams& p, long long g
     for (int d = 0; d < 3; ++d) c0_row[d * TS] = c0n[d];
 }
 
-template <int S, int CM, int MAXT, bool SOLVE, bool POLY = false>
+template <typename Real, int S, int CM, int MAXT, bool SOLVE, bool POLY = false>
 __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams p) {
     constexpr int N2 = 2 * S;
     constexpr int LPS = 4;                         // lanes per segment
     constexpr bool CONS = CM != 0 || POLY;
     static_assert(!(SOLVE && POLY), "the in-kernel stop rule is not instantiated for polytope corridors (host loop)");
+    static_assert(!POLY || sizeof(Real) == 8, "polytope corridors are fp64 only");
+    // Real = double: everything in fp64.  Real = float (TOP_F32, mixed): state, projections, consensus and duals in fp32; the
+    // two contractions stay on the fp64 tensor pipe (products of fp32-rounded operands, fp64 accumulation) and the operator
+    // apply a2 stays fp64 (an fp32 operator loses Q against rho G): the fp64 pipe then carries the MMAs only.
+    using R2 = typename Pair<Real>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
 
     const int T = blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
@@ -159,18 +179,18 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     const bool pin_pos = flags & KF_PIN_POS;
     const bool nb_sync = flags & KF_NEIGHBOUR_SYNC;
 
-    const SmemLayoutMma L = smem_layout_mma(CONS, SA, POLY);
+    const SmemLayoutMma L = smem_layout_mma(CONS, SA, POLY, (int)sizeof(Real));
     double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + tid;          // [((d*2 +) h*4 + b/2) * TS]   (d only with POLY)
     double* c0s = reinterpret_cast<double*>(smem_raw + L.c0) + tid;            // [(h*3 + d) * TS]
-    double2* zus = reinterpret_cast<double2*>(smem_raw + L.zu) + tid;          // [(h*3 + d) * TS]: (z~, u)
-    double2* qs = reinterpret_cast<double2*>(smem_raw + L.qs) + tid;           // [(h*3 + d) * TS]: (q+, q-)
-    double2* ws = reinterpret_cast<double2*>(smem_raw + L.ws) + tid;           // [(h*3 + d) * TS]: (w_v, w_a)
-    double2* phs = reinterpret_cast<double2*>(smem_raw + L.ph) + tid;          // [(h*3 + d) * TS]: (phi_v, phi_a)
+    R2* zus = reinterpret_cast<R2*>(smem_raw + L.zu) + tid;          // [(h*3 + d) * TS]: (z~, u)
+    R2* qs = reinterpret_cast<R2*>(smem_raw + L.qs) + tid;           // [(h*3 + d) * TS]: (q+, q-)
+    R2* ws = reinterpret_cast<R2*>(smem_raw + L.ws) + tid;           // [(h*3 + d) * TS]: (w_v, w_a)
+    R2* phs = reinterpret_cast<R2*>(smem_raw + L.ph) + tid;          // [(h*3 + d) * TS]: (phi_v, phi_a)
     double* ctab = reinterpret_cast<double*>(smem_raw + L.ctab) + (tid & 31);  // [k * 32]: a1 k-step operands at k = 0..7, a3 operands at k = 8 + kstep*4 + block
-    double* lohi = reinterpret_cast<double*>(smem_raw + L.lohi) + sl;          // [6 * SA]
+    Real* lohi = reinterpret_cast<Real*>(smem_raw + L.lohi) + sl;          // [6 * SA]
     double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE;
-    double* Bs = reinterpret_cast<double*>(smem_raw + L.bs);                   // [2 parity][SA+2][8 rows][3]
-    double* zoffs = reinterpret_cast<double*>(smem_raw + L.zoff) + sl;         // [(side*3 + d) * SA]
+    Real* Bs = reinterpret_cast<Real*>(smem_raw + L.bs);                   // [2 parity][SA+2][8 rows][3]
+    Real* zoffs = reinterpret_cast<Real*>(smem_raw + L.zoff) + sl;         // [(side*3 + d) * SA]
     double* qpls = reinterpret_cast<double*>(smem_raw + L.qpl) + tid;          // [(k*2 + h) * TS]
     double* pls = reinterpret_cast<double*>(smem_raw + L.pls) + (size_t)sl * PSTR;   // [k*4 + c]
     double* vs = reinterpret_cast<double*>(smem_raw + L.vs) + (size_t)sl * VSTR;     // V[d][e] at d*3 + e
@@ -231,7 +251,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             }
         }
     }
-    double invTk[2];
+    Real invTk[2];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
 #pragma unroll
@@ -242,16 +262,16 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                                                                    b + 1 < N2 ? p.Pm[((long long)dd * MAXN + b + 1) * stride + gt[h]] : 0.0);
 #pragma unroll
         for (int d = 0; d < 3; ++d) c0s[(h * 3 + d) * TS] = p.c0[d * stride + gt[h]];
-        invTk[h] = static_cast<const double*>(p.invTk)[gt[h]];
+        invTk[h] = static_cast<const Real*>(p.invTk)[gt[h]];
     }
-    const double invT = static_cast<const double*>(p.invT)[gseg], invT2 = static_cast<const double*>(p.invT)[p.nseg_pad + gseg];
+    const Real invT = static_cast<const Real*>(p.invT)[gseg], invT2 = static_cast<const Real*>(p.invT)[p.nseg_pad + gseg];
     if (CONS && !POLY) {
-        lohi[lane * SA] = static_cast<const double*>(p.lohi)[lane * p.nseg_pad + gseg];
-        if (lane < 2) lohi[(lane + 4) * SA] = static_cast<const double*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
+        lohi[lane * SA] = static_cast<const Real*>(p.lohi)[lane * p.nseg_pad + gseg];
+        if (lane < 2) lohi[(lane + 4) * SA] = static_cast<const Real*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
     }
     if (lane < 3) {        // frame shifts of the neighbours' position rows: left junction (row 0), right junction (row S)
-        zoffs[lane * SA] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + 0];
-        zoffs[(3 + lane) * SA] = static_cast<const double*>(p.zoff)[lane * stride + gseg * LANES + S];
+        zoffs[lane * SA] = static_cast<const Real*>(p.zoff)[lane * stride + gseg * LANES + 0];
+        zoffs[(3 + lane) * SA] = static_cast<const Real*>(p.zoff)[lane * stride + gseg * LANES + S];
     }
     if (POLY) {
         for (int i = lane; i < 9; i += LPS) vs[i] = p.rot[i * p.nseg_pad + gseg];
@@ -301,22 +321,22 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
             const long long i = d * stride + gt[h];
-            const double z0 = static_cast<const double*>(p.zt)[i], u0 = static_cast<const double*>(p.u)[i];
-            zus[(h * 3 + d) * TS] = make_double2(z0, u0);
-            gM[h][d] = (z0 - u0) * invTk[h];
+            const Real z0 = static_cast<const Real*>(p.zt)[i], u0 = static_cast<const Real*>(p.u)[i];
+            zus[(h * 3 + d) * TS] = make2(z0, u0);
+            gM[h][d] = (double)((z0 - u0) * invTk[h]);
             A0[h][d] = gv[h][d] = ga[h][d] = 0.0;
-            double w_v = 0.0, w_a = 0.0, ph_v = 0.0, ph_a = 0.0;
+            Real w_v = 0, w_a = 0, ph_v = 0, ph_a = 0;
             if (has_box) {
-                const double lo = static_cast<const double*>(p.lohi)[d * p.nseg_pad + gseg], hi = static_cast<const double*>(p.lohi)[(3 + d) * p.nseg_pad + gseg];
-                const double a = static_cast<const double*>(p.qp)[i], b = static_cast<const double*>(p.qn)[i];
-                qs[(h * 3 + d) * TS] = make_double2(a, b);
-                A0[h][d] = (hi - fabs(a)) + (lo + fabs(b));
+                const Real lo = static_cast<const Real*>(p.lohi)[d * p.nseg_pad + gseg], hi = static_cast<const Real*>(p.lohi)[(3 + d) * p.nseg_pad + gseg];
+                const Real a = static_cast<const Real*>(p.qp)[i], b = static_cast<const Real*>(p.qn)[i];
+                qs[(h * 3 + d) * TS] = make2(a, b);
+                A0[h][d] = (double)((hi - fabs(a)) + (lo + fabs(b)));
             }
-            if (has_vel) { w_v = static_cast<const double*>(p.wv)[i]; ph_v = static_cast<const double*>(p.phv)[i]; gv[h][d] = (ph_v - w_v) * invT; }
-            if (has_acc) { w_a = static_cast<const double*>(p.wa)[i]; ph_a = static_cast<const double*>(p.pha)[i]; ga[h][d] = (ph_a - w_a) * invT2; }
-            if (CONS) { ws[(h * 3 + d) * TS] = make_double2(w_v, w_a); phs[(h * 3 + d) * TS] = make_double2(ph_v, ph_a); }
+            if (has_vel) { w_v = static_cast<const Real*>(p.wv)[i]; ph_v = static_cast<const Real*>(p.phv)[i]; gv[h][d] = (double)((ph_v - w_v) * invT); }
+            if (has_acc) { w_a = static_cast<const Real*>(p.wa)[i]; ph_a = static_cast<const Real*>(p.pha)[i]; ga[h][d] = (double)((ph_a - w_a) * invT2); }
+            if (CONS) { ws[(h * 3 + d) * TS] = make2(w_v, w_a); phs[(h * 3 + d) * TS] = make2(ph_v, ph_a); }
         }
-    if (POLY) {      // consensus rows enter the segment's rotated frame; the E0 operand is sum_k (b_k - s_k - v_k) a_k
+    if constexpr (POLY) {      // consensus rows enter the segment's rotated frame; the E0 operand is sum_k (b_k - s_k - v_k) a_k
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             rot_in(vs, gM[h]);
@@ -328,7 +348,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         }
     }
 
-    const double vmax = p.vmax, amax = p.amax;
+    const Real vmax = (Real)p.vmax, amax = (Real)p.amax;
     unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
     const size_t mbox_par_stride = (size_t)p.max_ctas * 24 * 16;
     __shared__ int abort_sh[2];
@@ -352,7 +372,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         const bool final_sweep = (it == p.k_sweeps - 1);
         // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
         const bool last_sweep = final_sweep || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
-        double* const Bcur = Bs + par * BPAR;
+        Real* const Bcur = Bs + par * BPAR;
         unsigned char* const mpar = mbox + par * mbox_par_stride;
 
         // ================= phase A: segment local =================
@@ -423,20 +443,20 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
-                for (int d = 0; d < 3; ++d) static_cast<double*>(p.chat)[d * stride + gt[h]] = cacc[h][d];
+                for (int d = 0; d < 3; ++d) static_cast<Real*>(p.chat)[d * stride + gt[h]] = (Real)cacc[h][d];
         }
         // a3: evaluate the new polynomial: consensus rows of B = M c (Eq. 20b), and the lane's two samples of E0 c, E1 c,
         // E2 c (Eq. 20d-g).  A operand = the lane's own coefficient rows; accumulator columns = the lane's own items.
         {
-            double Bnd[2][3];
+            Real Bnd[2][3];
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 double e0 = 0, e1 = 0;
                 dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 0) * 32]);
                 dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 0) * 32]);
-                Bnd[0][d] = e0 * invTk[0]; Bnd[1][d] = e1 * invTk[1];
+                Bnd[0][d] = (Real)e0 * invTk[0]; Bnd[1][d] = (Real)e1 * invTk[1];
             }
-            if (POLY) { rot_out(vs, Bnd[0]); rot_out(vs, Bnd[1]); }      // consensus lives in the global frame
+            if constexpr (POLY) { rot_out(vs, Bnd[0]); rot_out(vs, Bnd[1]); }      // consensus lives in the global frame
             // publish: shared memory for the neighbours in this CTA (and for this lane's own phase B), mailbox for the
             // neighbouring CTAs
 #pragma unroll
@@ -447,7 +467,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 }
                 if (pub[h]) {
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) ll_store(mpar + pub_off[h] + d * 16, Bnd[h][d], seq);
+                    for (int d = 0; d < 3; ++d) ll_store(mpar + pub_off[h] + d * 16, (double)Bnd[h][d], seq);
                 }
             }
         }
@@ -460,20 +480,20 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         if (CONS) {
             // the three sample blocks of the evaluation back to back, then the projections of all blocks side by side:
             // independent dependency chains, no branch between them
-            double Pv[2][3], Vv[2][3], Av[2][3];
+            Real Pv[2][3], Vv[2][3], Av[2][3];
             if (has_vel) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 2) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 2) * 32]); Vv[0][d] = e0; Vv[1][d] = e1; }
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 2) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 2) * 32]); Vv[0][d] = (Real)e0; Vv[1][d] = (Real)e1; }
             }
             if (has_acc) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = e0; Av[1][d] = e1; }
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = (Real)e0; Av[1][d] = (Real)e1; }
             }
             if (has_box || POLY) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 1) * 32]); Pv[0][d] = e0; Pv[1][d] = e1; }
+                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 1) * 32]); Pv[0][d] = (Real)e0; Pv[1][d] = (Real)e1; }
             }
-            double2 w2[2][3], q2[2][3];
+            R2 w2[2][3], q2[2][3];
 #pragma unroll
             for (int h = 0; h < 2; ++h)
 #pragma unroll
@@ -482,30 +502,30 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     if (has_box) q2[h][d] = qs[(h * 3 + d) * TS];
                 }
             // a4: Eq. 20f, 20g;  y = A c + w,  phi = proj(y),  w <- y - phi;  next operand (phi - w)/T
-            double2 ph2[2][3];
+            R2 ph2[2][3];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 if (has_vel) {
-                    double y[3];
+                    Real y[3];
 #pragma unroll
                     for (int d = 0; d < 3; ++d) y[d] = Vv[h][d] * invT + w2[h][d].x;
-                    const double scale = ball_scale(y, vmax);
+                    const Real scale = ball_scale(y, vmax);
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) { const double ph = scale * y[d]; ph2[h][d].x = ph; w2[h][d].x = y[d] - ph; gv[h][d] = (ph - w2[h][d].x) * invT; }
+                    for (int d = 0; d < 3; ++d) { const Real ph = scale * y[d]; ph2[h][d].x = ph; w2[h][d].x = y[d] - ph; gv[h][d] = (double)((ph - w2[h][d].x) * invT); }
                 } else {
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) ph2[h][d].x = 0.0;
+                    for (int d = 0; d < 3; ++d) ph2[h][d].x = 0;
                 }
                 if (has_acc) {
-                    double y[3];
+                    Real y[3];
 #pragma unroll
                     for (int d = 0; d < 3; ++d) y[d] = Av[h][d] * invT2 + w2[h][d].y;
-                    const double scale = ball_scale(y, amax);
+                    const Real scale = ball_scale(y, amax);
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) { const double ph = scale * y[d]; ph2[h][d].y = ph; w2[h][d].y = y[d] - ph; ga[h][d] = (ph - w2[h][d].y) * invT2; }
+                    for (int d = 0; d < 3; ++d) { const Real ph = scale * y[d]; ph2[h][d].y = ph; w2[h][d].y = y[d] - ph; ga[h][d] = (double)((ph - w2[h][d].y) * invT2); }
                 } else {
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) ph2[h][d].y = 0.0;
+                    for (int d = 0; d < 3; ++d) ph2[h][d].y = 0;
                 }
             }
             if (has_vel || has_acc) {
@@ -514,7 +534,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
                     for (int d = 0; d < 3; ++d) { ws[(h * 3 + d) * TS] = w2[h][d]; phs[(h * 3 + d) * TS] = ph2[h][d]; }
             }
-            if (POLY) {         // a7 + a8 per (sample, plane): q = -(a_k'p - b_k + v);  next operand sum_k (b_k - |q_k|) a_k
+            if constexpr (POLY) {         // a7 + a8 per (sample, plane): q = -(a_k'p - b_k + v);  next operand sum_k (b_k - |q_k|) a_k
 #pragma unroll
                 for (int h = 0; h < 2; ++h) A0[h][0] = A0[h][1] = A0[h][2] = 0.0;
                 for (int k = 0; k < KP; ++k) {
@@ -532,12 +552,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             if (has_box) {      // a7 + a8: Eq. 20d, 20e with q = -(A c - b + v):  s = max(0,q),  v <- max(0,-q);  next operand
 #pragma unroll
                 for (int d = 0; d < 3; ++d) {
-                    const double lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
+                    const Real lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
 #pragma unroll
                     for (int h = 0; h < 2; ++h) {
-                        const double qpn = (hi - Pv[h][d]) - neg_part(q2[h][d].x), qnn = (Pv[h][d] - lo) - neg_part(q2[h][d].y);
-                        qs[(h * 3 + d) * TS] = make_double2(qpn, qnn);
-                        A0[h][d] = (hi - fabs(qpn)) + (lo + fabs(qnn));
+                        const Real qpn = (hi - Pv[h][d]) - neg_part(q2[h][d].x), qnn = (Pv[h][d] - lo) - neg_part(q2[h][d].y);
+                        qs[(h * 3 + d) * TS] = make2(qpn, qnn);
+                        A0[h][d] = (double)((hi - fabs(qpn)) + (lo + fabs(qnn)));
                     }
                 }
             }
@@ -580,8 +600,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 
         // ================= phase B: consensus, dual, residuals =================
         // everything is loaded first (own rows, neighbour rows, frame shifts, (z~, u)), then updated, then stored
-        double own[2][3], nb[2][3];
-        double2 zu[2][3];
+        Real own[2][3], nb[2][3];
+        R2 zu[2][3];
 #pragma unroll
         for (int h = 0; h < 2; ++h)
 #pragma unroll
@@ -592,7 +612,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             }
         if (need) {
 #pragma unroll
-            for (int d = 0; d < 3; ++d) { const double v = ll_value(rr[d]); if (need_h == 0) nb[0][d] = v; else nb[1][d] = v; }
+            for (int d = 0; d < 3; ++d) { const Real v = (Real)ll_value(rr[d]); if (need_h == 0) nb[0][d] = v; else nb[1][d] = v; }
         }
 #pragma unroll
         for (int h = 0; h < 2; ++h)
@@ -601,34 +621,34 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 for (int d = 0; d < 3; ++d) nb[h][d] += zoffs[((right[h] ? 3 : 0) + d) * SA];
             }
         double rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
-        double dz[2][3];
+        Real dz[2][3];
 #pragma unroll
         for (int h = 0; h < 2; ++h)
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
-                const double avg = 0.5 * (own[h][d] + nb[h][d]);
-                const double znew = (fixed[h] || !isrow[h]) ? zu[h][d].x : avg;    // a5: Eq. 6b / 20b
+                const Real avg = (Real)0.5 * (own[h][d] + nb[h][d]);
+                const Real znew = (fixed[h] || !isrow[h]) ? zu[h][d].x : avg;    // a5: Eq. 6b / 20b
                 dz[h][d] = znew - zu[h][d].x;
-                const double res = isrow[h] ? own[h][d] - znew : 0.0;
-                const double unew = zu[h][d].y + res;                               // a8: Eq. 6c / 20c (scaled dual, A5)
-                zus[(h * 3 + d) * TS] = make_double2(znew, unew);
-                gM[h][d] = (znew - unew) * invTk[h];                                // operand of the next sweep's a1
+                const Real res = isrow[h] ? own[h][d] - znew : (Real)0;
+                const Real unew = zu[h][d].y + res;                               // a8: Eq. 6c / 20c (scaled dual, A5)
+                zus[(h * 3 + d) * TS] = make2(znew, unew);
+                gM[h][d] = (double)((znew - unew) * invTk[h]);                                // operand of the next sweep's a1
                 if (last_sweep) {
-                    rp2 += res * res;
-                    if (gaprow[h]) { const double gp = own[h][d] - nb[h][d]; gap2 += gp * gp; }   // Eq. 21
+                    rp2 += (double)res * (double)res;
+                    if (gaprow[h]) { const double gp = (double)own[h][d] - (double)nb[h][d]; gap2 += gp * gp; }   // Eq. 21
                 }
             }
-        if (POLY) { rot_in(vs, gM[0]); rot_in(vs, gM[1]); }
+        if constexpr (POLY) { rot_in(vs, gM[0]); rot_in(vs, gM[1]); }
         if (last_sweep) {
             // a6: dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8):
             // the consensus block of the a1 contraction applied to dz; lane t ends with coefficient rows 2t, 2t+1
-            const double Tp0 = static_cast<const double*>(p.Tpow)[gseg * LANES + 2 * lane];
-            const double Tp1 = static_cast<const double*>(p.Tpow)[gseg * LANES + 2 * lane + 1];
+            const double Tp0 = (double)static_cast<const Real*>(p.Tpow)[gseg * LANES + 2 * lane];
+            const double Tp1 = (double)static_cast<const Real*>(p.Tpow)[gseg * LANES + 2 * lane + 1];
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 double x0 = 0, x1 = 0;
-                dmma884(x0, x1, dz[0][d] * invTk[0], ctab[0 * 32]);
-                dmma884(x0, x1, dz[1][d] * invTk[1], ctab[1 * 32]);
+                dmma884(x0, x1, (double)(dz[0][d] * invTk[0]), ctab[0 * 32]);
+                dmma884(x0, x1, (double)(dz[1][d] * invTk[1]), ctab[1 * 32]);
                 const double xr0 = rho_cur * x0, xr1 = rho_cur * x1;
                 rdn2 += xr0 * xr0 + xr1 * xr1;
                 rd2 += (xr0 * Tp0) * (xr0 * Tp0) + (xr1 * Tp1) * (xr1 * Tp1);
@@ -689,31 +709,31 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     if (rp > p.mu * rd) rho_new = rho_cur * p.tau_incr;
                     else if (rd > p.mu * rp) rho_new = rho_cur / p.tau_decr;
                     if (rho_new != rho_cur) {
-                        const double ratio = rho_cur / rho_new;
+                        const Real ratio = (Real)(rho_cur / rho_new);
                         // u, w, v = max(0,-q) are scaled duals: times rho_old/rho_new; then the operands that depend on them
 #pragma unroll
                         for (int h = 0; h < 2; ++h) {
 #pragma unroll
                             for (int d = 0; d < 3; ++d) {
-                                double2 zz = zus[(h * 3 + d) * TS];
+                                R2 zz = zus[(h * 3 + d) * TS];
                                 zz.y *= ratio;
                                 zus[(h * 3 + d) * TS] = zz;
-                                gM[h][d] = (zz.x - zz.y) * invTk[h];
+                                gM[h][d] = (double)((zz.x - zz.y) * invTk[h]);
                                 if (has_box) {
-                                    const double lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
-                                    double2 q = qs[(h * 3 + d) * TS];
+                                    const Real lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
+                                    R2 q = qs[(h * 3 + d) * TS];
                                     if (q.x < 0) q.x *= ratio;
                                     if (q.y < 0) q.y *= ratio;
                                     qs[(h * 3 + d) * TS] = q;
-                                    A0[h][d] = (hi - fabs(q.x)) + (lo + fabs(q.y));
+                                    A0[h][d] = (double)((hi - fabs(q.x)) + (lo + fabs(q.y)));
                                 }
                                 if (has_vel || has_acc) {
-                                    double2 w2 = ws[(h * 3 + d) * TS];
-                                    const double2 ph = phs[(h * 3 + d) * TS];
+                                    R2 w2 = ws[(h * 3 + d) * TS];
+                                    const R2 ph = phs[(h * 3 + d) * TS];
                                     w2.x *= ratio; w2.y *= ratio;
                                     ws[(h * 3 + d) * TS] = w2;
-                                    if (has_vel) gv[h][d] = (ph.x - w2.x) * invT;
-                                    if (has_acc) ga[h][d] = (ph.y - w2.y) * invT2;
+                                    if (has_vel) gv[h][d] = (double)((ph.x - w2.x) * invT);
+                                    if (has_acc) ga[h][d] = (double)((ph.y - w2.y) * invT2);
                                 }
                             }
                             refresh_operator_rows<N2, TS>(p, gseg, gt[h], jj[h], rho_new, Pms + h * 4 * TS, c0s + h * 3 * TS);
@@ -737,23 +757,23 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
             for (int d = 0; d < 3; ++d) {
                 const long long i = d * stride + gt[h];
-                const double2 zz = zus[(h * 3 + d) * TS];
-                static_cast<double*>(p.zt_out)[i] = zz.x;
-                static_cast<double*>(p.u_out)[i] = zz.y;
-                if (has_box) { const double2 q = qs[(h * 3 + d) * TS]; static_cast<double*>(p.qp_out)[i] = q.x; static_cast<double*>(p.qn_out)[i] = q.y; }
+                const R2 zz = zus[(h * 3 + d) * TS];
+                static_cast<Real*>(p.zt_out)[i] = zz.x;
+                static_cast<Real*>(p.u_out)[i] = zz.y;
+                if (has_box) { const R2 q = qs[(h * 3 + d) * TS]; static_cast<Real*>(p.qp_out)[i] = q.x; static_cast<Real*>(p.qn_out)[i] = q.y; }
                 if (POLY && d == 0) for (int k = 0; k < KP; ++k) static_cast<double*>(p.qpl_out)[k * stride + gt[h]] = qpls[(k * 2 + h) * TS];
                 if (has_vel || has_acc) {
-                    const double2 w2 = ws[(h * 3 + d) * TS], ph = phs[(h * 3 + d) * TS];
-                    if (has_vel) { static_cast<double*>(p.wv_out)[i] = w2.x; static_cast<double*>(p.phv_out)[i] = ph.x; }
-                    if (has_acc) { static_cast<double*>(p.wa_out)[i] = w2.y; static_cast<double*>(p.pha_out)[i] = ph.y; }
+                    const R2 w2 = ws[(h * 3 + d) * TS], ph = phs[(h * 3 + d) * TS];
+                    if (has_vel) { static_cast<Real*>(p.wv_out)[i] = w2.x; static_cast<Real*>(p.phv_out)[i] = ph.x; }
+                    if (has_acc) { static_cast<Real*>(p.wa_out)[i] = w2.y; static_cast<Real*>(p.pha_out)[i] = ph.y; }
                 }
             }
     }
 }
 
-template <int S, int CM, int MAXT>
+template <typename Real, int S, int CM, int MAXT>
 cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
-    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<S, CM, MAXT, true> : cadmm_sweeps_mma_kernel<S, CM, MAXT, false>;
+    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, true> : cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     KParams pc = p;
@@ -762,9 +782,9 @@ cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cud
     return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
 }
 
-template <int S, int CM, int MAXT>
+template <typename Real, int S, int CM, int MAXT>
 cudaError_t limits_mma(int threads, size_t smem, int* per_sm) {
-    auto kern = cadmm_sweeps_mma_kernel<S, CM, MAXT, true>;     // the larger of the two instantiations
+    auto kern = cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, true>;     // the larger of the two instantiations
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
@@ -772,7 +792,7 @@ cudaError_t limits_mma(int threads, size_t smem, int* per_sm) {
 
 template <int S>
 cudaError_t launch_mma_poly(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
-    auto kern = cadmm_sweeps_mma_kernel<S, CM_RUNTIME, MAXT_MMA_POLY, false, true>;
+    auto kern = cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_POLY, false, true>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     KParams pc = p;
@@ -782,7 +802,7 @@ cudaError_t launch_mma_poly(const KParams& p, int ctas, int threads, size_t smem
 }
 template <int S>
 cudaError_t limits_mma_poly(int threads, size_t smem, int* per_sm) {
-    auto kern = cadmm_sweeps_mma_kernel<S, CM_RUNTIME, MAXT_MMA_POLY, false, true>;
+    auto kern = cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_POLY, false, true>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
@@ -796,35 +816,43 @@ int mma_mask(uint32_t kflags) {
 
 }  // namespace
 
+// fp64: one instantiation of <= 288 threads.  fp32 (mixed): the state is half the size, <= 384 threads (12 warps of 8 segments:
+// three warps on every scheduler, 168 registers)
 #define TOP_DISPATCH_MMA(CALL)                                                                              \
     const int cm = mma_mask(kflags);                                                                        \
-    if (s == 3) { if (cm == 0) { CALL(3, 0) } else if (cm == 3) { CALL(3, 3) } else if (cm == 7) { CALL(3, 7) } else { CALL(3, CM_RUNTIME) } } \
-    else        { if (cm == 0) { CALL(4, 0) } else if (cm == 3) { CALL(4, 3) } else if (cm == 7) { CALL(4, 7) } else { CALL(4, CM_RUNTIME) } }
+    if (dtype == 0) {                                                                                       \
+        if (s == 3) { if (cm == 0) { CALL(double, 3, 0, MAXT_MMA) } else if (cm == 3) { CALL(double, 3, 3, MAXT_MMA) } else if (cm == 7) { CALL(double, 3, 7, MAXT_MMA) } else { CALL(double, 3, CM_RUNTIME, MAXT_MMA) } } \
+        else        { if (cm == 0) { CALL(double, 4, 0, MAXT_MMA) } else if (cm == 3) { CALL(double, 4, 3, MAXT_MMA) } else if (cm == 7) { CALL(double, 4, 7, MAXT_MMA) } else { CALL(double, 4, CM_RUNTIME, MAXT_MMA) } } \
+    } else {                                                                                                \
+        if (s == 3) { if (cm == 0) { CALL(float, 3, 0, MAXT_MMA_F32) } else if (cm == 3) { CALL(float, 3, 3, MAXT_MMA_F32) } else if (cm == 7) { CALL(float, 3, 7, MAXT_MMA_F32) } else { CALL(float, 3, CM_RUNTIME, MAXT_MMA_F32) } } \
+        else        { if (cm == 0) { CALL(float, 4, 0, MAXT_MMA_F32) } else if (cm == 3) { CALL(float, 4, 3, MAXT_MMA_F32) } else if (cm == 7) { CALL(float, 4, 7, MAXT_MMA_F32) } else { CALL(float, 4, CM_RUNTIME, MAXT_MMA_F32) } } \
+    }
 
-int max_threads_mma(bool poly) { return poly ? MAXT_MMA_POLY : MAXT_MMA; }
+int max_threads_mma(int dtype, bool poly) { return poly ? MAXT_MMA_POLY : (dtype == 0 ? MAXT_MMA : MAXT_MMA_F32); }
 
-cudaError_t launch_sweeps_mma(const KParams& p, int s, bool /*constrained*/, int ctas, int threads, size_t smem, cudaStream_t st) {
+cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st) {
     const uint32_t kflags = p.flags;
     if (kflags & KF_POLY) {
-        if (p.check_every > 0) return cudaErrorInvalidValue;      // host loop only
+        if (p.check_every > 0 || dtype != 0) return cudaErrorInvalidValue;      // host loop only, fp64 only
         return s == 3 ? launch_mma_poly<3>(p, ctas, threads, smem, st) : launch_mma_poly<4>(p, ctas, threads, smem, st);
     }
-#define CALL(S_, C_) return launch_mma<S_, C_, MAXT_MMA>(p, ctas, threads, smem, st);
+#define CALL(R_, S_, C_, M_) return launch_mma<R_, S_, C_, M_>(p, ctas, threads, smem, st);
     TOP_DISPATCH_MMA(CALL)
 #undef CALL
     return cudaErrorInvalidValue;
 }
 
-cudaError_t sweep_kernel_limits_mma(int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm) {
+cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm) {
     if (kflags & KF_POLY) return s == 3 ? limits_mma_poly<3>(threads, smem, max_ctas_per_sm) : limits_mma_poly<4>(threads, smem, max_ctas_per_sm);
-#define CALL(S_, C_) return limits_mma<S_, C_, MAXT_MMA>(threads, smem, max_ctas_per_sm);
+#define CALL(R_, S_, C_, M_) return limits_mma<R_, S_, C_, M_>(threads, smem, max_ctas_per_sm);
     TOP_DISPATCH_MMA(CALL)
 #undef CALL
     return cudaErrorInvalidValue;
 }
 
-size_t sweep_smem_bytes_mma(bool constrained, bool poly) {      // laid out for the largest CTA of the instantiation (see the kernel)
-    return poly ? smem_layout_mma(true, MAXT_MMA_POLY / 4, true).total : smem_layout_mma(constrained, MAXT_MMA / 4).total;
+size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly) {      // laid out for the largest CTA of the instantiation (see the kernel)
+    if (poly) return smem_layout_mma(true, MAXT_MMA_POLY / 4, true).total;
+    return dtype == 0 ? smem_layout_mma(constrained, MAXT_MMA / 4).total : smem_layout_mma(constrained, MAXT_MMA_F32 / 4, false, 4).total;
 }
 
 }  // namespace top
