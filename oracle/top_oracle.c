@@ -19,7 +19,13 @@
  *   u,v   <- scaled dual updates                     (Eq. 6c/20c/20e)
  *
  * Readings of the paper taken here:
- *   A1  consensus carries derivative orders 0..s-1 (n_c = s), so M is 2s x 2s.
+ *   A1  consensus carries derivative orders 0..n_c-1 at each boundary.  Default n_c = s (M is 2s x 2s).  The paper's
+ *       literal choice (M(t) has rows beta^0..beta^(d-1), d = 2p-1; L257 "overdetermined", m x 2d
+ *       continuity constraints on m(d+1) unknowns) is n_c = 2s-1 ("wide" consensus): M is 2(2s-1) x 2s.  z_0 and z_N
+ *       are "initialized by sigma_0 and sigma_N" (L141), which carry orders 0..s-1 only (Eq. 2c: the boundary
+ *       conditions go to order p-1, L261), so with n_c = 2s-1 the rows of orders s..2s-2 at the two trajectory ENDS do
+ *       not exist: they are left out of M for the first / last segment (rowmask), nothing is fixed there.  Fixing them
+ *       (e.g. at 0) would be a different problem from the one the paper's Optimality Conditions (L259-264) describe.
  *   A2  waypoint mode: HARD (default; sigma_i(0)=p_{i-1}, sigma_i(T_i)=p_i imposed as
  *       equalities inside each segment QP: Pm = H^-1 - K Ew H^-1, c0 = K [p_{i-1};p_i],
  *       K = H^-1 Ew'(Ew H^-1 Ew')^-1), PINNED_Z (Eq. 20a verbatim, position row of z_j held
@@ -72,12 +78,14 @@ typedef double real_t;
 typedef long double pre_t; /* precision of the one-off operator precompute */
 
 #define NMAX 8   /* n = 2s <= 8 */
+#define RMAX 14  /* consensus rows per segment 2 n_c <= 2(2s-1) = 14 */
 #define MODE_HARD 0
 #define MODE_PINNED_Z 1
 #define MODE_FREE 2
 
 typedef struct {
     int N, s, n, m, Ms, mode;
+    int nc;         /* consensus derivative orders per boundary: s (default) or 2s-1 (reading A1) */
     int has_box, has_vel, has_acc;
     real_t rho, vmax, amax;
     real_t *T;      /* [N] */
@@ -85,14 +93,15 @@ typedef struct {
     real_t *lo, *hi;/* [N][m] */
     /* per-segment matrices (Eq. 19 / L231) */
     real_t *Q;      /* [N][n][n]   */
-    real_t *M;      /* [N][2s][n]  */
+    real_t *M;      /* [N][2nc][n]: rows beta_0(0)..beta_{nc-1}(0), beta_0(T)..beta_{nc-1}(T) */
+    real_t *rowmask;/* [N][2nc]: 1 = the row takes part in the consensus, 0 = it does not exist (A1: ends, orders >= s) */
     real_t *E0, *E1, *E2; /* [N][Ms][n] : rows beta_k(t_ij) */
     real_t *Pm;     /* [N][n][n]   */
     real_t *c0;     /* [N][n][m]   */
     /* state */
     real_t *C;      /* [N][n][m]   */
-    real_t *z, *zprev; /* [N+1][s][m] */
-    real_t *u;      /* [N][2s][m]  */
+    real_t *z, *zprev; /* [N+1][nc][m] */
+    real_t *u;      /* [N][2nc][m]  */
     real_t *Sp, *Sn, *Vp, *Vn;   /* [N][Ms][m] slack / dual of the box, + and - side */
     real_t *PhiV, *WV, *PhiA, *WA; /* [N][Ms][m] */
     /* general polytope corridor (reading A11p): K planes per segment, coupled (n m) x (n m) operator */
@@ -208,7 +217,7 @@ static int spd_inverse_big(int q, const pre_t *A, pre_t *Ainv) {
 void oracle_destroy(oracle_t *o) {
     if (!o) return;
     free(o->T); free(o->p); free(o->lo); free(o->hi);
-    free(o->Q); free(o->M); free(o->E0); free(o->E1); free(o->E2); free(o->Pm); free(o->c0);
+    free(o->Q); free(o->M); free(o->rowmask); free(o->E0); free(o->E1); free(o->E2); free(o->Pm); free(o->c0);
     free(o->C); free(o->z); free(o->zprev); free(o->u);
     free(o->Sp); free(o->Sn); free(o->Vp); free(o->Vn);
     free(o->PhiV); free(o->WV); free(o->PhiA); free(o->WA); free(o->part);
@@ -232,10 +241,13 @@ static int build_operator(oracle_t *o, int i) {
     pre_t Q[NMAX * NMAX], H[NMAX * NMAX], Hinv[NMAX * NMAX], row[NMAX];
     build_Q(n, s, T, Q);
     for (int a = 0; a < n * n; ++a) { o->Q[(size_t)i * n * n + a] = (real_t)Q[a]; H[a] = 2 * Q[a]; }
-    /* M(T): rows beta_0(0)..beta_{s-1}(0), beta_0(T)..beta_{s-1}(T) */
-    for (int r = 0; r < 2 * s; ++r) {
-        beta_row(n, r % s, r < s ? (pre_t)0 : T, row);
-        for (int j = 0; j < n; ++j) o->M[((size_t)i * 2 * s + r) * n + j] = (real_t)row[j];
+    /* M(T): rows beta_0(0)..beta_{nc-1}(0), beta_0(T)..beta_{nc-1}(T); rows that do not exist
+     * (rowmask 0, reading A1) are stored but take no part in H */
+    const int nc = o->nc;
+    for (int r = 0; r < 2 * nc; ++r) {
+        beta_row(n, r % nc, r < nc ? (pre_t)0 : T, row);
+        for (int j = 0; j < n; ++j) o->M[((size_t)i * 2 * nc + r) * n + j] = (real_t)row[j];
+        if (o->rowmask[(size_t)i * 2 * nc + r] == 0) continue;
         for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) H[a * n + b] += rho * row[a] * row[b];
     }
     /* sample rows (A10) and their Gram terms: 2 E0'E0 (two box sides, A11), E1'E1, E2'E2 */
@@ -293,9 +305,11 @@ static int build_operator_poly(oracle_t *o, int i) {
     pre_t Q[NMAX * NMAX], D[NMAX * NMAX], row[NMAX];
     build_Q(n, s, T, Q);
     for (int a = 0; a < n * n; ++a) { o->Q[(size_t)i * n * n + a] = (real_t)Q[a]; D[a] = 2 * Q[a]; }
-    for (int r = 0; r < 2 * s; ++r) {
-        beta_row(n, r % s, r < s ? (pre_t)0 : T, row);
-        for (int j = 0; j < n; ++j) o->M[((size_t)i * 2 * s + r) * n + j] = (real_t)row[j];
+    const int nc = o->nc;
+    for (int r = 0; r < 2 * nc; ++r) {
+        beta_row(n, r % nc, r < nc ? (pre_t)0 : T, row);
+        for (int j = 0; j < n; ++j) o->M[((size_t)i * 2 * nc + r) * n + j] = (real_t)row[j];
+        if (o->rowmask[(size_t)i * 2 * nc + r] == 0) continue;
         for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) D[a * n + b] += rho * row[a] * row[b];
     }
     memset(H, 0, sizeof(pre_t) * q * q);
@@ -366,13 +380,14 @@ static int build_operator_poly(oracle_t *o, int i) {
 static oracle_t *oracle_create_impl(int N, int s, int m, const double *waypoints, const double *durations,
                         const double *start_derivs, const double *end_derivs, int Ms,
                         const double *box_lo, const double *box_hi, double vmax, double amax,
-                        double rho, int mode, int K, const double *planes) {
+                        double rho, int mode, int K, const double *planes, int nc) {
     if (N < 1 || (s != 3 && s != 4) || m < 1 || m > 3 || Ms < 0 || !(rho > 0) || mode < 0 || mode > 2) return NULL;
+    if (nc != s && nc != 2 * s - 1) return NULL;
     if (K < 0 || (K > 0 && (!planes || Ms <= 0 || box_lo || box_hi))) return NULL;   /* a polytope replaces the box */
     oracle_t *o = (oracle_t *)calloc(1, sizeof(oracle_t));
     if (!o) return NULL;
     const int n = 2 * s;
-    o->N = N; o->s = s; o->n = n; o->m = m; o->Ms = Ms; o->mode = mode;
+    o->N = N; o->s = s; o->n = n; o->m = m; o->Ms = Ms; o->mode = mode; o->nc = nc;
     o->rho = (real_t)rho; o->vmax = (real_t)vmax; o->amax = (real_t)amax;
     o->has_box = (Ms > 0 && box_lo && box_hi);
     o->has_vel = (Ms > 0 && vmax > 0);
@@ -383,11 +398,11 @@ static oracle_t *oracle_create_impl(int N, int s, int m, const double *waypoints
     ALLOC(o->Spl, (size_t)N * Ms * K); ALLOC(o->Vpl, (size_t)N * Ms * K);
     for (size_t a = 0; a < (size_t)N * K * (m + 1); ++a) o->planes[a] = (real_t)planes[a];
     ALLOC(o->T, N); ALLOC(o->p, (N + 1) * m); ALLOC(o->lo, N * m); ALLOC(o->hi, N * m);
-    ALLOC(o->Q, (size_t)N * n * n); ALLOC(o->M, (size_t)N * 2 * s * n);
+    ALLOC(o->Q, (size_t)N * n * n); ALLOC(o->M, (size_t)N * 2 * nc * n); ALLOC(o->rowmask, (size_t)N * 2 * nc);
     ALLOC(o->E0, (size_t)N * Ms * n); ALLOC(o->E1, (size_t)N * Ms * n); ALLOC(o->E2, (size_t)N * Ms * n);
     ALLOC(o->Pm, (size_t)N * n * n); ALLOC(o->c0, (size_t)N * n * m);
-    ALLOC(o->C, (size_t)N * n * m); ALLOC(o->z, (size_t)(N + 1) * s * m); ALLOC(o->zprev, (size_t)(N + 1) * s * m);
-    ALLOC(o->u, (size_t)N * 2 * s * m);
+    ALLOC(o->C, (size_t)N * n * m); ALLOC(o->z, (size_t)(N + 1) * nc * m); ALLOC(o->zprev, (size_t)(N + 1) * nc * m);
+    ALLOC(o->u, (size_t)N * 2 * nc * m);
     ALLOC(o->Sp, (size_t)N * Ms * m); ALLOC(o->Sn, (size_t)N * Ms * m);
     ALLOC(o->Vp, (size_t)N * Ms * m); ALLOC(o->Vn, (size_t)N * Ms * m);
     ALLOC(o->PhiV, (size_t)N * Ms * m); ALLOC(o->WV, (size_t)N * Ms * m);
@@ -396,6 +411,14 @@ static oracle_t *oracle_create_impl(int N, int s, int m, const double *waypoints
     for (int i = 0; i < N; ++i) { if (!(durations[i] > 0)) { oracle_destroy(o); return NULL; } o->T[i] = (real_t)durations[i]; }
     for (int a = 0; a < (N + 1) * m; ++a) o->p[a] = (real_t)waypoints[a];
     if (o->has_box) for (int a = 0; a < N * m; ++a) { o->lo[a] = (real_t)box_lo[a]; o->hi[a] = (real_t)box_hi[a]; }
+    /* rows of M that exist (reading A1): all of them, except orders s..nc-1 at the start of the first segment and at the
+     * end of the last one (z_0, z_N carry the given end state, orders 0..s-1, L141 / Eq. 2c) */
+    for (int i = 0; i < N; ++i)
+        for (int r = 0; r < 2 * nc; ++r) {
+            const int k = r % nc, at_end = r >= nc;
+            const int missing = k >= s && ((i == 0 && !at_end) || (i == N - 1 && at_end));
+            o->rowmask[(size_t)i * 2 * nc + r] = missing ? 0 : 1;
+        }
     for (int i = 0; i < N; ++i) if (o->has_poly ? build_operator_poly(o, i) : build_operator(o, i)) { oracle_destroy(o); return NULL; }
 
     /* ---- Init (Alg. 1 line 1; reading A9) ---- */
@@ -407,16 +430,16 @@ static oracle_t *oracle_create_impl(int N, int s, int m, const double *waypoints
     }
     for (int j = 0; j <= N; ++j)           /* z0_j: position p_j, mean chord velocity, higher orders 0 */
         for (int d = 0; d < m; ++d) {
-            o->z[((size_t)j * s + 0) * m + d] = o->p[(size_t)j * m + d];
+            o->z[((size_t)j * nc + 0) * m + d] = o->p[(size_t)j * m + d];
             if (j >= 1 && j <= N - 1)
-                o->z[((size_t)j * s + 1) * m + d] = (real_t)0.5 * (o->C[((size_t)(j - 1) * n + 1) * m + d] + o->C[((size_t)j * n + 1) * m + d]);
+                o->z[((size_t)j * nc + 1) * m + d] = (real_t)0.5 * (o->C[((size_t)(j - 1) * n + 1) * m + d] + o->C[((size_t)j * n + 1) * m + d]);
         }
     for (int k = 1; k < s; ++k)            /* z_0, z_N = given end states (Eq. 2c); rest if NULL */
         for (int d = 0; d < m; ++d) {
-            o->z[((size_t)0 * s + k) * m + d] = start_derivs ? (real_t)start_derivs[(k - 1) * m + d] : 0;
-            o->z[((size_t)N * s + k) * m + d] = end_derivs ? (real_t)end_derivs[(k - 1) * m + d] : 0;
+            o->z[((size_t)0 * nc + k) * m + d] = start_derivs ? (real_t)start_derivs[(k - 1) * m + d] : 0;
+            o->z[((size_t)N * nc + k) * m + d] = end_derivs ? (real_t)end_derivs[(k - 1) * m + d] : 0;
         }
-    memcpy(o->zprev, o->z, sizeof(real_t) * (size_t)(N + 1) * s * m);
+    memcpy(o->zprev, o->z, sizeof(real_t) * (size_t)(N + 1) * nc * m);
     for (int i = 0; i < N; ++i)            /* slacks / phi of the chord samples; all duals 0 */
         for (int j = 0; j < Ms; ++j) {
             real_t P[3] = {0, 0, 0}, V[3] = {0, 0, 0}, A[3] = {0, 0, 0};
@@ -450,20 +473,29 @@ oracle_t *oracle_create(int N, int s, int m, const double *waypoints, const doub
                         const double *start_derivs, const double *end_derivs, int Ms,
                         const double *box_lo, const double *box_hi, double vmax, double amax,
                         double rho, int mode) {
-    return oracle_create_impl(N, s, m, waypoints, durations, start_derivs, end_derivs, Ms, box_lo, box_hi, vmax, amax, rho, mode, 0, NULL);
+    return oracle_create_impl(N, s, m, waypoints, durations, start_derivs, end_derivs, Ms, box_lo, box_hi, vmax, amax, rho, mode, 0, NULL, s);
+}
+
+/* the general entry: box (K = 0) or polytope corridor (K > 0, box_lo = box_hi = NULL), and the number n_c of consensus
+ * derivative orders per boundary: s, or the paper-literal 2s-1 (reading A1) */
+oracle_t *oracle_create_ex(int N, int s, int m, const double *waypoints, const double *durations,
+                           const double *start_derivs, const double *end_derivs, int Ms,
+                           const double *box_lo, const double *box_hi, int K, const double *planes,
+                           double vmax, double amax, double rho, int mode, int nc) {
+    return oracle_create_impl(N, s, m, waypoints, durations, start_derivs, end_derivs, Ms, box_lo, box_hi, vmax, amax, rho, mode, K, planes, nc);
 }
 
 /* the same with a general polytope corridor: planes [N][K][m+1] = (normal a_k, offset b_k), a_k'p <= b_k (A11p) */
 oracle_t *oracle_create_poly(int N, int s, int m, const double *waypoints, const double *durations,
                              const double *start_derivs, const double *end_derivs, int Ms, int K, const double *planes,
                              double vmax, double amax, double rho, int mode) {
-    return oracle_create_impl(N, s, m, waypoints, durations, start_derivs, end_derivs, Ms, NULL, NULL, vmax, amax, rho, mode, K, planes);
+    return oracle_create_impl(N, s, m, waypoints, durations, start_derivs, end_derivs, Ms, NULL, NULL, vmax, amax, rho, mode, K, planes, s);
 }
 
 /* ------------------------------------------------------------------ one sweep (Alg. 1 lines 3-13) */
 
 static void sweep_once(oracle_t *o) {
-    const int N = o->N, s = o->s, n = o->n, m = o->m, Ms = o->Ms;
+    const int N = o->N, n = o->n, m = o->m, Ms = o->Ms, nc = o->nc;
     const real_t rho = o->rho;
 
     /* ClosedFormSolve: Eq. 20a with rho on the right-hand side (A3) */
@@ -471,10 +503,11 @@ static void sweep_once(oracle_t *o) {
     for (int i = 0; i < N; ++i) {
         real_t R[NMAX * 3];
         for (int a = 0; a < n * m; ++a) R[a] = 0;
-        const real_t *M = o->M + (size_t)i * 2 * s * n;
-        for (int r = 0; r < 2 * s; ++r) {          /* M'(z~_i - u_i), z~_i = (z_{i-1}; z_i) */
-            const real_t *zr = o->z + ((size_t)(i + (r >= s)) * s + (r % s)) * m;
-            const real_t *ur = o->u + ((size_t)i * 2 * s + r) * m;
+        const real_t *M = o->M + (size_t)i * 2 * nc * n;
+        for (int r = 0; r < 2 * nc; ++r) {         /* M'(z~_i - u_i), z~_i = (z_{i-1}; z_i) */
+            if (o->rowmask[(size_t)i * 2 * nc + r] == 0) continue;
+            const real_t *zr = o->z + ((size_t)(i + (r >= nc)) * nc + (r % nc)) * m;
+            const real_t *ur = o->u + ((size_t)i * 2 * nc + r) * m;
             for (int d = 0; d < m; ++d) {
                 real_t g = zr[d] - ur[d];
                 for (int a = 0; a < n; ++a) R[a * m + d] += M[r * n + a] * g;
@@ -541,19 +574,19 @@ static void sweep_once(oracle_t *o) {
         }
 
     /* UpdateConsensus: Eq. 6b / 20b. z_0, z_N fixed (L141). */
-    memcpy(o->zprev, o->z, sizeof(real_t) * (size_t)(N + 1) * s * m);
+    memcpy(o->zprev, o->z, sizeof(real_t) * (size_t)(N + 1) * nc * m);
 #pragma omp parallel for schedule(static)
     for (int j = 1; j <= N - 1; ++j) {
-        const real_t *Ml = o->M + (size_t)(j - 1) * 2 * s * n, *Mr = o->M + (size_t)j * 2 * s * n;
-        for (int k = 0; k < s; ++k) {
+        const real_t *Ml = o->M + (size_t)(j - 1) * 2 * nc * n, *Mr = o->M + (size_t)j * 2 * nc * n;
+        for (int k = 0; k < nc; ++k) {
             if (k == 0 && o->mode == MODE_PINNED_Z) continue;   /* position row held at p_j */
             for (int d = 0; d < m; ++d) {
                 real_t bl = 0, br = 0;
                 for (int a = 0; a < n; ++a) {
-                    bl += Ml[(s + k) * n + a] * o->C[((size_t)(j - 1) * n + a) * m + d];
+                    bl += Ml[(nc + k) * n + a] * o->C[((size_t)(j - 1) * n + a) * m + d];
                     br += Mr[k * n + a] * o->C[((size_t)j * n + a) * m + d];
                 }
-                o->z[((size_t)j * s + k) * m + d] = (real_t)0.5 * (bl + br);
+                o->z[((size_t)j * nc + k) * m + d] = (real_t)0.5 * (bl + br);
             }
         }
     }
@@ -561,22 +594,24 @@ static void sweep_once(oracle_t *o) {
     /* UpdateResidual (Eq. 21, 22; A7, A8), ProjectNonNeg (20d), UpdateDual (20c, 20e) */
 #pragma omp parallel for schedule(static)
     for (int i = 0; i < N; ++i) {
-        const real_t *M = o->M + (size_t)i * 2 * s * n;
+        const real_t *M = o->M + (size_t)i * 2 * nc * n;
         real_t rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
-        real_t dz[NMAX * 3];
-        for (int r = 0; r < 2 * s; ++r) {
-            size_t zi = ((size_t)(i + (r >= s)) * s + (r % s)) * m;
+        real_t dz[RMAX * 3];
+        for (int r = 0; r < 2 * nc; ++r) {
+            size_t zi = ((size_t)(i + (r >= nc)) * nc + (r % nc)) * m;
             for (int d = 0; d < m; ++d) {
+                dz[r * m + d] = 0;
+                if (o->rowmask[(size_t)i * 2 * nc + r] == 0) continue;  /* no such row (A1) */
                 real_t b = 0;
                 for (int a = 0; a < n; ++a) b += M[r * n + a] * o->C[((size_t)i * n + a) * m + d];
                 real_t res = b - o->z[zi + d];
                 rp2 += res * res;
-                o->u[((size_t)i * 2 * s + r) * m + d] += res;           /* Eq. 20c */
+                o->u[((size_t)i * 2 * nc + r) * m + d] += res;          /* Eq. 20c */
                 dz[r * m + d] = o->z[zi + d] - o->zprev[zi + d];
-                if (r >= s && i < N - 1) {                              /* Eq. 21 verbatim: junction gap */
+                if (r >= nc && i < N - 1) {                             /* Eq. 21 verbatim: junction gap */
                     real_t br = 0;
-                    const real_t *Mn = o->M + (size_t)(i + 1) * 2 * s * n;
-                    for (int a = 0; a < n; ++a) br += Mn[(r - s) * n + a] * o->C[((size_t)(i + 1) * n + a) * m + d];
+                    const real_t *Mn = o->M + (size_t)(i + 1) * 2 * nc * n;
+                    for (int a = 0; a < n; ++a) br += Mn[(r - nc) * n + a] * o->C[((size_t)(i + 1) * n + a) * m + d];
                     gap2 += (b - br) * (b - br);
                 }
             }
@@ -585,7 +620,7 @@ static void sweep_once(oracle_t *o) {
         for (int a = 0; a < n; ++a) {                                   /* rho M'(dz~): Eq. 22 */
             for (int d = 0; d < m; ++d) {
                 real_t acc = 0;
-                for (int r = 0; r < 2 * s; ++r) acc += M[r * n + a] * dz[r * m + d];
+                for (int r = 0; r < 2 * nc; ++r) acc += M[r * n + a] * dz[r * m + d];
                 acc *= rho;
                 rd2 += acc * acc;
                 rdn2 += (acc / Tp) * (acc / Tp);
@@ -679,9 +714,9 @@ int64_t oracle_solve(oracle_t *o, double eps, int64_t max_iter, int use_rd_norm,
  */
 int oracle_set_rho(oracle_t *o, double rho_new) {
     if (!(rho_new > 0)) return -1;
-    const int N = o->N, s = o->s, m = o->m, Ms = o->Ms;
+    const int N = o->N, m = o->m, Ms = o->Ms;
     const real_t r = o->rho / (real_t)rho_new;
-    for (size_t a = 0; a < (size_t)N * 2 * s * m; ++a) o->u[a] *= r;
+    for (size_t a = 0; a < (size_t)N * 2 * o->nc * m; ++a) o->u[a] *= r;
     for (size_t a = 0; a < (size_t)N * Ms * m; ++a) { o->Vp[a] *= r; o->Vn[a] *= r; o->WV[a] *= r; o->WA[a] *= r; }
     for (size_t a = 0; a < (size_t)N * Ms * o->K; ++a) o->Vpl[a] *= r;
     o->rho = (real_t)rho_new;
@@ -734,9 +769,9 @@ int64_t oracle_iter(const oracle_t *o) { return o->iter; }
 
 /* copy a field as doubles. returns the element count, or -1 for an unknown name.
  * "coeffs" is [N][m][n] (dim-major per segment, the paper's squeezed c_i); every other field is in its
- * native layout: C [N][n][m], z [N+1][s][m], u [N][2s][m], sample fields [N][Ms][m], Pm [N][n][n] ... */
+ * native layout: C [N][n][m], z [N+1][nc][m], u [N][2nc][m], sample fields [N][Ms][m], Pm [N][n][n] ... */
 int64_t oracle_get(const oracle_t *o, const char *name, double *out) {
-    const int N = o->N, s = o->s, n = o->n, m = o->m, Ms = o->Ms;
+    const int N = o->N, n = o->n, m = o->m, Ms = o->Ms, nc = o->nc;
     const real_t *src = NULL; size_t cnt = 0;
     if (!strcmp(name, "coeffs")) {
         for (int i = 0; i < N; ++i) for (int d = 0; d < m; ++d) for (int a = 0; a < n; ++a)
@@ -745,14 +780,14 @@ int64_t oracle_get(const oracle_t *o, const char *name, double *out) {
     }
 #define FIELD(nm, ptr, count) else if (!strcmp(name, nm)) { src = (ptr); cnt = (size_t)(count); }
     if (0) {}
-    FIELD("C", o->C, (size_t)N * n * m) FIELD("z", o->z, (size_t)(N + 1) * s * m) FIELD("u", o->u, (size_t)N * 2 * s * m)
+    FIELD("C", o->C, (size_t)N * n * m) FIELD("z", o->z, (size_t)(N + 1) * nc * m) FIELD("u", o->u, (size_t)N * 2 * nc * m)
     FIELD("s_pos", o->Sp, (size_t)N * Ms * m) FIELD("s_neg", o->Sn, (size_t)N * Ms * m)
     FIELD("v_pos", o->Vp, (size_t)N * Ms * m) FIELD("v_neg", o->Vn, (size_t)N * Ms * m)
     FIELD("phi_v", o->PhiV, (size_t)N * Ms * m) FIELD("w_v", o->WV, (size_t)N * Ms * m)
     FIELD("phi_a", o->PhiA, (size_t)N * Ms * m) FIELD("w_a", o->WA, (size_t)N * Ms * m)
     FIELD("s_poly", o->Spl, (size_t)N * Ms * o->K) FIELD("v_poly", o->Vpl, (size_t)N * Ms * o->K)
     FIELD("Pm", o->Pm, (size_t)N * n * n) FIELD("c0", o->c0, (size_t)N * n * m) FIELD("Q", o->Q, (size_t)N * n * n)
-    FIELD("M", o->M, (size_t)N * 2 * s * n) FIELD("E0", o->E0, (size_t)N * Ms * n) FIELD("E1", o->E1, (size_t)N * Ms * n)
+    FIELD("M", o->M, (size_t)N * 2 * nc * n) FIELD("rowmask", o->rowmask, (size_t)N * 2 * nc) FIELD("E0", o->E0, (size_t)N * Ms * n) FIELD("E1", o->E1, (size_t)N * Ms * n)
     FIELD("E2", o->E2, (size_t)N * Ms * n)
     else return -1;
 #undef FIELD

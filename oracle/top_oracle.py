@@ -43,6 +43,9 @@ def _lib(long_double: bool):
         L.oracle_create_poly.restype = ctypes.c_void_p
         L.oracle_create_poly.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, dp, ctypes.c_int, ctypes.c_int, dp,
                                          ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int]
+        L.oracle_create_ex.restype = ctypes.c_void_p
+        L.oracle_create_ex.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, dp, ctypes.c_int, dp, dp, ctypes.c_int, dp,
+                                       ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int]
         L.oracle_destroy.argtypes = [ctypes.c_void_p]
         L.oracle_sweep.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int]
         L.oracle_solve.restype = ctypes.c_int64
@@ -74,11 +77,14 @@ class Oracle:
     """One trajectory (the oracle has no batch dimension; loop over it)."""
 
     def __init__(self, waypoints, durations, s, rho, samples=0, box_lo=None, box_hi=None, vmax=0.0, amax=0.0,
-                 start_derivs=None, end_derivs=None, mode="hard", long_double=False, planes=None):
+                 start_derivs=None, end_derivs=None, mode="hard", long_double=False, planes=None, consensus="s"):
+        """consensus: "s" = derivative orders 0..s-1 at every boundary (default, reading A1); "wide" = the paper-literal
+        orders 0..2s-2, the orders >= s left out at the two trajectory ends."""
         wp = np.ascontiguousarray(waypoints, dtype=np.float64)
         T = np.ascontiguousarray(durations, dtype=np.float64)
         assert wp.ndim == 2 and T.ndim == 1 and wp.shape[0] == T.shape[0] + 1
         self.N, self.m, self.s, self.n, self.Ms = T.shape[0], wp.shape[1], int(s), 2 * int(s), int(samples)
+        self.nc = {"s": int(s), "wide": 2 * int(s) - 1}[consensus]
         self.T = T
         keep = [wp, T]
         def opt(a, shape):
@@ -92,16 +98,15 @@ class Oracle:
         sd = opt(start_derivs, (self.s - 1, self.m)); ed = opt(end_derivs, (self.s - 1, self.m))
         self._L = _lib(long_double)
         self.K = 0
+        pl = None
         if planes is not None:            # general polytope corridor: [N][K][m+1] = (normal, offset), normal'p <= offset
             pl = np.ascontiguousarray(planes, dtype=np.float64)
             assert pl.ndim == 3 and pl.shape[0] == self.N and pl.shape[2] == self.m + 1 and lo is None and hi is None
             keep.append(pl)
             self.K = pl.shape[1]
-            self._h = self._L.oracle_create_poly(self.N, self.s, self.m, _dptr(wp), _dptr(T), _dptr(sd), _dptr(ed), self.Ms,
-                                                 self.K, _dptr(pl), float(vmax), float(amax), float(rho), MODES[mode])
-        else:
-            self._h = self._L.oracle_create(self.N, self.s, self.m, _dptr(wp), _dptr(T), _dptr(sd), _dptr(ed), self.Ms,
-                                            _dptr(lo), _dptr(hi), float(vmax), float(amax), float(rho), MODES[mode])
+        self._h = self._L.oracle_create_ex(self.N, self.s, self.m, _dptr(wp), _dptr(T), _dptr(sd), _dptr(ed), self.Ms,
+                                           _dptr(lo), _dptr(hi), self.K, _dptr(pl), float(vmax), float(amax), float(rho),
+                                           MODES[mode], self.nc)
         if not self._h:
             raise ValueError("oracle_create rejected the inputs")
 
@@ -144,9 +149,9 @@ class Oracle:
         return int(self._L.oracle_threads())
 
     _SHAPES = {
-        "coeffs": lambda o: (o.N, o.m, o.n), "C": lambda o: (o.N, o.n, o.m), "z": lambda o: (o.N + 1, o.s, o.m),
-        "u": lambda o: (o.N, 2 * o.s, o.m), "Pm": lambda o: (o.N, o.n, o.n), "c0": lambda o: (o.N, o.n, o.m),
-        "Q": lambda o: (o.N, o.n, o.n), "M": lambda o: (o.N, 2 * o.s, o.n),
+        "coeffs": lambda o: (o.N, o.m, o.n), "C": lambda o: (o.N, o.n, o.m), "z": lambda o: (o.N + 1, o.nc, o.m),
+        "u": lambda o: (o.N, 2 * o.nc, o.m), "rowmask": lambda o: (o.N, 2 * o.nc), "Pm": lambda o: (o.N, o.n, o.n), "c0": lambda o: (o.N, o.n, o.m),
+        "Q": lambda o: (o.N, o.n, o.n), "M": lambda o: (o.N, 2 * o.nc, o.n),
         "E0": lambda o: (o.N, o.Ms, o.n), "E1": lambda o: (o.N, o.Ms, o.n), "E2": lambda o: (o.N, o.Ms, o.n),
         "s_poly": lambda o: (o.N, o.Ms, o.K), "v_poly": lambda o: (o.N, o.Ms, o.K),
     }
