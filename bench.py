@@ -505,6 +505,23 @@ def main():
             others[wl.name + "_streamed"] = {"segment_iterations_per_s": wl.N * 1280 / (e0.elapsed_time(e1) * 1e-3), "sweeps": 1280,
                                              "pieces": sl_.launch_info()["waves"], "dtype": wl.dtype}
             sl_.close()
+            # the paper-literal consensus (n_c = 2s-1 derivative orders per boundary, waypoints free: Alg. 1 verbatim) on a
+            # cfg4-shaped chain that fits its on-chip capacity (148 x 56 segments)
+            ww = W.config4(seed=1004 + rank, N=8192)
+            sw = top.from_workload(ww, device=local_rank, stream=stream.cuda_stream, sync=args.sync, consensus="wide", mode="free")
+            sw.iterate(500); torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); sw.iterate(2000); e1.record(stream); torch.cuda.synchronize()
+            msw = e0.elapsed_time(e1)
+            liw = sw.launch_info()
+            fl_w = FLOPS_PER_SEG_SWEEP["cfg4"] + 612.0      # + 2(s-1) consensus rows in a1, a3, a5, a8
+            others["cfg4shape_N8192_snap_f64_wide_consensus_free"] = {
+                "segment_iterations_per_s": ww.N * 2000 / (msw * 1e-3), "sweeps": 2000, "us_per_sweep_per_wave": 1e3 * msw / 2000,
+                "dtype": "f64", "ctas": liw["ctas"], "threads": liw["threads"], "waves": liw["waves"],
+                "roofline": {"bound": "alu", "achieved": fl_w * ww.N * 2000 / (msw * 1e-3) / 1e12, "peak": peaks["f64"] / 1e12,
+                             "unit": "TFLOP/s", "frac": fl_w * ww.N * 2000 / (msw * 1e-3) / peaks["f64"],
+                             "flops_per_segment_sweep": fl_w}}
+            sw.close()
             out["other_workloads"] = others
             # ---- the paper's own regime (Tables I-II): tolerance ||r|| < N*0.05 on config 2, fixed rho
             # vs adaptive rho (Eq. 24, rho0 = 1, updated every sweep as in Alg. 1 line 14)

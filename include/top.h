@@ -85,6 +85,14 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
  * constant-matrix contractions (Eq. 20a second bracket; evaluation of Eq. 20b, 20d-g) on the tensor cores
  * (mma.sync m8n8k4 f64).  This flag keeps the shuffle / synthetic-division form of the 4-lane kernel instead. */
 #define TOP_KERNEL_NO_MMA     128u
+/* Consensus width (reading A1 of DESIGN.md).  Default: every junction carries the derivative orders 0..s-1 (M is 2s x 2s).
+ * TOP_CONSENSUS_WIDE: the paper's literal choice (M(t) stacks beta^0..beta^(d-1) with d = 2p-1; L257: each
+ * x-update is over-determined; L259-264): orders 0..2s-2, i.e. n_c = 2s-1 rows per boundary; z_0 and z_N carry the given
+ * end state (orders 0..s-1, Eq. 2c), so the orders s..2s-2 do not exist at the two trajectory ends.
+ * top_get_state "z" is then [batch][N+1][2s-1][dims] and "u" [batch][N][2(2s-1)][dims] (rows that do not exist read 0).
+ * TOP_F64 on the tensor-core kernel only, no polytope corridor, the trajectory must fit on chip (N <= 148 x 56);
+ * else TOP_E_UNSUPPORTED. */
+#define TOP_CONSENSUS_WIDE    256u
 
 /* The paper's convex sets, specialised as BASELINE.json's configs use them:
  * an axis-aligned box corridor per segment (K=6 half-spaces, linear set, Eq. 7-10) and Euclidean balls on

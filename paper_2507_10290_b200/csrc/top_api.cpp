@@ -56,6 +56,9 @@ struct top_solver {
     long long nseg = 0, nseg_pad = 0, stride = 0;
     int num_sms = 0, max_ctas = 0, user_segs = 0, lanes = 8;
     bool mma = false;                  // fp64, 4 lanes per segment: the tensor-core (DMMA) kernel of top_kernels_mma.cu
+    bool wide = false;                 // paper-literal consensus n_c = 2s-1 (reading A1): second block of consensus rows
+    int nc = 0;                        // consensus derivative orders per boundary: s, or 2s-1
+    void *d_zt2 = nullptr, *d_u2 = nullptr, *d_invTk2 = nullptr;
     struct Wave { long long seg_begin, seg_end, own_begin, own_end; uint32_t kflags; int segs_per_cta, ctas, threads; size_t smem; };
     // streaming (temporal blocking) for chains longer than the on-chip capacity: pieces with `halo` extra segments on
     // each open side run `halo` sweeps per launch (the dependency radius of a sweep is one segment), reading iterate
@@ -170,6 +173,7 @@ struct GramTables {
     xreal Q1[MAXN * MAXN];        // int_0^1 beta^(s) beta^(s)'
     xreal Gc[4][MAXN * MAXN];     // consensus rows of derivative order k: beta_k(0)beta_k(0)' + beta_k(1)beta_k(1)'
     xreal Ge[3][MAXN * MAXN];     // sample rows of E_0, E_1, E_2: sum_j beta_k(tau_j) beta_k(tau_j)'
+    xreal Gw[2][3][MAXN * MAXN];  // wide consensus (n_c = 2s-1): order s + j at tau = 0 ([0][j]) and at tau = 1 ([1][j]), j <= s-2
 };
 void build_gram_tables(int s, GramTables& G) {
     const int n = 2 * s;
@@ -186,6 +190,7 @@ void build_gram_tables(int s, GramTables& G) {
         for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) M[a * MAXN + b] += row[a] * row[b];
     };
     for (int k = 0; k < s; ++k) { add(G.Gc[k], k, 0); add(G.Gc[k], k, 1); }
+    for (int j = 0; j <= s - 2; ++j) { add(G.Gw[0][j], s + j, 0); add(G.Gw[1][j], s + j, 1); }
     for (int j = 1; j <= MS; ++j)
         for (int k = 0; k < 3; ++k) add(G.Ge[k], k, (xreal)j / (xreal)(MS + 1));     // reading A10
 }
@@ -197,12 +202,13 @@ const GramTables& gram_tables(int s) {       // built once per s, whatever threa
 }
 
 bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int mode,
-                    const xreal* p0, const xreal* p1, xreal* Pm /*[8][8]*/, xreal* c0 /*[8][3]*/, xreal box_weight = 2) {
+                    const xreal* p0, const xreal* p1, xreal* Pm /*[8][8]*/, xreal* c0 /*[8][3]*/, xreal box_weight = 2,
+                    int wide_mask = 0 /* bit 0 / 1: the consensus rows of orders s..2s-2 exist at the start / end boundary */) {
     const int n = 2 * s;
     const GramTables& G = gram_tables(s);
-    xreal iT[8];                       // T^-k
+    xreal iT[14];                      // T^-k
     iT[0] = 1;
-    for (int k = 1; k < 8; ++k) iT[k] = iT[k - 1] / T;
+    for (int k = 1; k < 14; ++k) iT[k] = iT[k - 1] / T;
     const xreal wq = 2 * T * iT[2 * s - 1] * iT[1];             // 2 T^(1-2s)
     const xreal wb = box ? box_weight * rho : 0;               // box: its two sides (A11); polytope: eigenvalue of sum_k a_k a_k' (A11p)
     const xreal wv = vel ? rho * iT[2] : 0, wa = acc ? rho * iT[4] : 0;
@@ -212,6 +218,8 @@ bool build_operator(int s, xreal T, xreal rho, bool box, bool vel, bool acc, int
             const int i = a * MAXN + b;
             xreal v = wq * G.Q1[i] + wb * G.Ge[0][i] + wv * G.Ge[1][i] + wa * G.Ge[2][i];
             for (int k = 0; k < s; ++k) v += rho * iT[2 * k] * G.Gc[k][i];
+            for (int side = 0; side < 2; ++side)
+                if (wide_mask & (1 << side)) for (int j = 0; j <= s - 2; ++j) v += rho * iT[2 * (s + j)] * G.Gw[side][j][i];
             H[a * n + b] = v;
         }
     for (int i = 0; i < MAXN * MAXN; ++i) Pm[i] = 0;
@@ -302,12 +310,12 @@ bool jacobi_eigen(int q, std::vector<xreal>& C, std::vector<xreal>& U) {       /
     return true;
 }
 
-bool build_spectral(int s, xreal T, bool box, bool vel, bool acc, int mode, const xreal* dp, Spectral& S) {
+bool build_spectral(int s, xreal T, bool box, bool vel, bool acc, int mode, const xreal* dp, Spectral& S, int wide_mask = 0) {
     const int n = 2 * s;
     const GramTables& G = gram_tables(s);
-    xreal iT[8];
+    xreal iT[14];
     iT[0] = 1;
-    for (int k = 1; k < 8; ++k) iT[k] = iT[k - 1] / T;
+    for (int k = 1; k < 14; ++k) iT[k] = iT[k - 1] / T;
     const xreal wq = 2 * T * iT[2 * s - 1] * iT[1];             // 2 T^(1-2s)
     std::vector<xreal> Q2(n * n), Gm(n * n);
     for (int a = 0; a < n; ++a)
@@ -316,6 +324,8 @@ bool build_spectral(int s, xreal T, bool box, bool vel, bool acc, int mode, cons
             Q2[a * n + b] = wq * G.Q1[i];
             xreal v = (box ? 2 * G.Ge[0][i] : 0) + (vel ? iT[2] * G.Ge[1][i] : 0) + (acc ? iT[4] * G.Ge[2][i] : 0);
             for (int k = 0; k < s; ++k) v += iT[2 * k] * G.Gc[k][i];
+            for (int side = 0; side < 2; ++side)
+                if (wide_mask & (1 << side)) for (int j = 0; j <= s - 2; ++j) v += iT[2 * (s + j)] * G.Gw[side][j][i];
             Gm[a * n + b] = v;
         }
     const bool hard = mode == (int)TOP_WAYPOINT_HARD;
@@ -422,16 +432,18 @@ top_status download_real(top_solver* h, const void* src, std::vector<double>& ds
 int round_up(int x, int m) { return (x + m - 1) / m * m; }
 
 // the sweep kernel family of a solver: 8 lanes, 4 lanes (shuffle form), or 4 lanes with fp64 tensor-core contractions
-size_t kernel_smem(int dtype, int s, bool constrained, int lanes, bool mma, int segs, bool poly = false) {
-    return mma ? sweep_smem_bytes_mma(dtype, constrained, poly) : sweep_smem_bytes(dtype, s, constrained, lanes, segs);
+size_t kernel_smem(int dtype, int s, bool constrained, int lanes, bool mma, int segs, bool poly = false, bool wide = false) {
+    return mma ? sweep_smem_bytes_mma(dtype, constrained, poly, wide) : sweep_smem_bytes(dtype, s, constrained, lanes, segs);
 }
-int kernel_max_threads(int dtype, int lanes, bool mma, bool poly = false) { return mma ? max_threads_mma(dtype, poly) : max_threads_for(dtype, lanes); }
+int kernel_max_threads(int dtype, int lanes, bool mma, bool poly = false, bool wide = false) {
+    return mma ? max_threads_mma(dtype, poly, wide) : max_threads_for(dtype, lanes);
+}
 
 // largest segments-per-CTA (multiple of 4) whose threads and shared memory fit one CTA
-int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, bool mma, size_t smem_limit, bool poly = false) {
+int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, bool mma, size_t smem_limit, bool poly = false, bool wide = false) {
     int best = 0;
-    for (int segs = 4; (segs * lanes + 31) / 32 * 32 <= kernel_max_threads(dtype, lanes, mma, poly); segs += 4)
-        if (kernel_smem(dtype, s, constrained, lanes, mma, segs, poly) <= smem_limit) best = segs;
+    for (int segs = 4; (segs * lanes + 31) / 32 * 32 <= kernel_max_threads(dtype, lanes, mma, poly, wide); segs += 4)
+        if (kernel_smem(dtype, s, constrained, lanes, mma, segs, poly, wide) <= smem_limit) best = segs;
     return best;
 }
 
@@ -502,6 +514,7 @@ void fill_init_params(top_solver* h, InitParams& ip) {
     }
     ip.Pm = h->d_Pm; ip.c0 = h->d_c0; ip.g0 = h->d_g0; ip.dp = h->d_dp; ip.origin = h->d_origin;
     ip.invTk = h->d_invTk; ip.Tpow = h->d_Tpow; ip.invT = h->d_invT; ip.lohi = h->d_lohi; ip.zoff = h->d_zoff;
+    ip.invTk2 = h->d_invTk2;
     ip.zt = h->d_zt; ip.chat = h->d_chat; ip.qp = h->d_qp; ip.qn = h->d_qn; ip.phv = h->d_phv; ip.segflags = h->d_segflags;
     ip.stride = h->stride; ip.nseg_pad = h->nseg_pad; ip.nseg = h->nseg; ip.N = h->N; ip.batch = h->batch; ip.s = h->s; ip.dims = h->dims;
     ip.hard = h->wp_mode == TOP_WAYPOINT_HARD; ip.has_box = h->has_box; ip.has_vel = h->has_vel; ip.has_acc = h->has_acc;
@@ -533,12 +546,15 @@ top_status stage_operators(top_solver* h) {
         try {
             xreal Pm[MAXN * MAXN];
             double cached_T = -1.0;
+            int cached_mask = -1;
             for (long long g = g0; g < g1; ++g) {
                 const double Td = durations[g];
+                // wide consensus: the rows of orders >= s exist at every boundary except the two trajectory ends (A1)
+                const int wmask = h->wide ? ((g % N != 0 ? 1 : 0) | (g % N != N - 1 ? 2 : 0)) : 0;
                 if (!poly) {
-                    if (Td != cached_T) {
-                        if (!build_operator(s, (xreal)Td, rho, box, vel, acc, mode, nullptr, nullptr, Pm, nullptr)) { bad_operator.store(1); return; }
-                        cached_T = Td;
+                    if (Td != cached_T || wmask != cached_mask) {
+                        if (!build_operator(s, (xreal)Td, rho, box, vel, acc, mode, nullptr, nullptr, Pm, nullptr, 2, wmask)) { bad_operator.store(1); return; }
+                        cached_T = Td; cached_mask = wmask;
                     }
                     for (int lane = 0; lane < n; ++lane)
                         for (int b = 0; b < n; ++b) Pm_st[(size_t)b * LS + (size_t)g * LANES + lane] = (double)(rho * Pm[lane * MAXN + b]);
@@ -638,11 +654,13 @@ top_status ensure_spectral(top_solver* h) {
         try {
             Spectral SP;
             double cached_T = -1.0;
+            int cached_mask = -1;
             const xreal zero3[3] = {0, 0, 0};
             for (long long g = g0; g < g1; ++g) {
-                if (durations[g] != cached_T) {
-                    if (!build_spectral(s, (xreal)durations[g], h->has_box, h->has_vel, h->has_acc, (int)h->wp_mode, zero3, SP)) { bad.store(1); return; }
-                    cached_T = durations[g];
+                const int wmask = h->wide ? ((g % h->N != 0 ? 1 : 0) | (g % h->N != h->N - 1 ? 2 : 0)) : 0;
+                if (durations[g] != cached_T || wmask != cached_mask) {
+                    if (!build_spectral(s, (xreal)durations[g], h->has_box, h->has_vel, h->has_acc, (int)h->wp_mode, zero3, SP, wmask)) { bad.store(1); return; }
+                    cached_T = durations[g]; cached_mask = wmask;
                 }
                 for (int i = 0; i < MAXN; ++i) lamv[(size_t)i * NP + g] = i < SP.q ? (double)SP.lam[i] : 0.0;
                 for (int lane = 0; lane < n; ++lane)
@@ -793,11 +811,13 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->constrained = has_box || has_vel || has_acc || h->has_poly;
     h->vmax = has_vel ? cons->vmax : 0; h->amax = has_acc ? cons->amax : 0;
     h->wp_mode = mode;
+    h->wide = (o.flags & TOP_CONSENSUS_WIDE) != 0;
+    h->nc = h->wide ? 2 * s - 1 : s;
     if (o.adapt_mu > 0) h->adapt_mu = o.adapt_mu;
     if (o.adapt_tau_incr > 0) h->adapt_incr = o.adapt_tau_incr;
     if (o.adapt_tau_decr > 0) h->adapt_decr = o.adapt_tau_decr;
     h->kflags = (has_box ? KF_BOX : 0) | (has_vel ? KF_VEL : 0) | (has_acc ? KF_ACC : 0) |
-                (mode == TOP_WAYPOINT_PINNED_Z ? KF_PIN_POS : 0) | (h->has_poly ? KF_POLY : 0);
+                (mode == TOP_WAYPOINT_PINNED_Z ? KF_PIN_POS : 0) | (h->has_poly ? KF_POLY : 0) | (h->wide ? KF_WIDE : 0);
     h->nseg = nseg; h->nseg_pad = (nseg + 31) / 32 * 32; h->stride = h->nseg_pad * LANES;
 
     // ---- launch plan: waves of whole trajectories, each wave resident on chip for all its sweeps
@@ -817,11 +837,13 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     // unconstrained chains once an SM holds more than a few warps (N = 10^4: 1.6 vs 2.1-2.3); short unconstrained chains
     // (configs 1, 3) stay on the 8-lane kernel (0.64 vs 0.85, 1.42 vs 1.57)
     if (!o.lanes_per_segment && dtype == TOP_F64 && ((has_box || has_vel || has_acc) || nseg >= (long long)h->num_sms * 32)) h->lanes = 4;
-    if (!o.lanes_per_segment && h->has_poly) h->lanes = 4;
+    if (!o.lanes_per_segment && (h->has_poly || h->wide)) h->lanes = 4;
     h->mma = h->lanes == 4 && !(o.flags & TOP_KERNEL_NO_MMA);
+    if (h->wide && (!(h->mma && dtype == TOP_F64) || h->has_poly))
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_CONSENSUS_WIDE runs on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA, no polytope corridor)"));
     if (h->has_poly && !(h->mma && dtype == TOP_F64))
         CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "polytope corridors run on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA)"));
-    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192, h->has_poly);
+    const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192, h->has_poly, h->wide);
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
     h->max_ctas = h->num_sms;
     const long long capacity = (long long)h->max_ctas * std::min(segs_max, h->user_segs ? h->user_segs : segs_max);
@@ -834,13 +856,13 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
         w.segs_per_cta = segs;
         w.ctas = (int)((cnt + segs - 1) / segs);
         w.threads = (segs * h->lanes + 31) / 32 * 32;
-        w.smem = kernel_smem(h->dtype, s, h->constrained, h->lanes, h->mma, segs, h->has_poly);
+        w.smem = kernel_smem(h->dtype, s, h->constrained, h->lanes, h->mma, segs, h->has_poly, h->wide);
         if (w.ctas > h->max_ctas) return false;
         h->waves.push_back(w);
         return true;
     };
-    if ((long long)N > capacity && h->has_poly)
-        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "a trajectory with a polytope corridor must fit on chip (streaming is not built for it)"));
+    if ((long long)N > capacity && (h->has_poly || h->wide))
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "a trajectory with a polytope corridor or with TOP_CONSENSUS_WIDE must fit on chip (streaming is not built for it)"));
     if ((long long)N > capacity) {
         // one trajectory does not fit on chip: stream the whole segment index space in pieces with halos
         h->streaming = true;
@@ -896,7 +918,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     const size_t o_c0 = cv.take(3 * LS * 8), o_W = cv.take(MAXN * LS * 8), o_g0 = cv.take(3 * LS * 8), o_lam = cv.take(MAXN * NP * 8),
                  o_dp = cv.take(3 * NP * 8), o_invTk = cv.take(LS * rb), o_Tpow = cv.take(LS * rb), o_invT = cv.take(2 * NP * rb),
                  o_lohi = cv.take(6 * NP * rb), o_segf = cv.take(NP), o_zoff = cv.take(3 * LS * rb), o_origin = cv.take(3 * NP * 8),
-                 o_coef = cv.take((size_t)nseg * dims * n * rb);
+                 o_coef = cv.take((size_t)nseg * dims * n * rb), o_invTk2 = cv.take(h->wide ? LS * rb : 0);
     // (c) iterate: written by the init kernel ...
     const size_t o_zt = cv.take(3 * LS * rb), o_chat = cv.take(3 * LS * rb), o_qp = cv.take(has_box ? 3 * LS * rb : 0),
                  o_qn = cv.take(has_box ? 3 * LS * rb : 0), o_phv = cv.take(has_vel ? 3 * LS * rb : 0),
@@ -905,7 +927,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     const size_t o_zero = cv.off;
     const size_t o_u = cv.take(3 * LS * rb), o_wv = cv.take(has_vel ? 3 * LS * rb : 0), o_pha = cv.take(has_acc ? 3 * LS * rb : 0),
                  o_wa = cv.take(has_acc ? 3 * LS * rb : 0), o_part = cv.take(NP * 4 * 8), o_res = cv.take((size_t)batch * 4 * 8),
-                 o_solve = cv.take(64);
+                 o_solve = cv.take(64), o_zt2 = cv.take(h->wide ? 3 * LS * rb : 0), o_u2 = cv.take(h->wide ? 3 * LS * rb : 0);
     size_t o_alt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     if (h->streaming) {
         const bool on[8] = {true, true, has_box, has_box, has_vel, has_vel, has_acc, has_acc};
@@ -913,7 +935,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     }
     h->zero_bytes = cv.off - o_zero;
     // (d) exchange buffers (zero once; sequence numbers keep growing over the life of the solver)
-    const size_t o_Bedge = cv.take((size_t)2 * h->max_ctas * 24 * 16), o_resbox = cv.take((size_t)2 * h->max_ctas * 4 * 16),
+    const size_t o_Bedge = cv.take((size_t)2 * h->max_ctas * (h->wide ? 48 : 24) * 16), o_resbox = cv.take((size_t)2 * h->max_ctas * 4 * 16),
                  o_sync = cv.take(16), o_abort = cv.take(16);
     h->arena_bytes = cv.off;
     {
@@ -931,6 +953,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->d_origin = (double*)(A + o_origin); h->d_coef = A + o_coef; h->d_zt = A + o_zt; h->d_chat = A + o_chat;
     h->d_u = A + o_u; h->d_part = (double*)(A + o_part); h->d_res = (double*)(A + o_res); h->d_solve = (double*)(A + o_solve);
     if (has_box) { h->d_qp = A + o_qp; h->d_qn = A + o_qn; }
+    if (h->wide) { h->d_invTk2 = A + o_invTk2; h->d_zt2 = A + o_zt2; h->d_u2 = A + o_u2; }
     if (h->has_poly) {
         h->d_rot = (double*)(A + h->off_rot); h->d_planes = (double*)(A + h->off_planes); h->d_lam3 = (double*)(A + h->off_lam3);
         h->d_qpl = (double*)(A + o_qpl);
@@ -1060,6 +1083,7 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
             }
             p.max_ctas = h->max_ctas; p.rho = h->rho; p.vmax = h->vmax; p.amax = h->amax;
             p.rot = h->d_rot; p.planes = h->d_planes; p.qpl = h->d_qpl; p.qpl_out = h->d_qpl; p.K = h->K;
+            p.invTk2 = h->d_invTk2; p.zt2 = h->d_zt2; p.u2 = h->d_u2;
             p.seq_base = (unsigned int)(h->seq_counter & 0xffffffffull);
             h->seq_counter += (unsigned long long)kk;
             if (w.ctas > 1 && !(p.flags & KF_NEIGHBOUR_SYNC))
@@ -1191,7 +1215,7 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
         CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
         RescaleParams r;
         r.u = h->d_u; r.qp = nullptr; r.qn = nullptr; r.wv = h->d_wv; r.wa = h->d_wa;
-        r.count = 3 * (long long)LS; r.ratio = old / rho; r.qpl = h->d_qpl; r.qpl_count = (long long)h->K * (long long)LS;
+        r.count = 3 * (long long)LS; r.ratio = old / rho; r.qpl = h->d_qpl; r.qpl_count = (long long)h->K * (long long)LS; r.u2 = nullptr;
         CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
         h->launches += 2;
         return TOP_OK;
@@ -1200,7 +1224,7 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
     CU(refresh_operator(h, rho), "operator refresh launch");      // on the device, from the spectral data
     RescaleParams r;
     r.u = h->d_u; r.qp = h->d_qp; r.qn = h->d_qn; r.wv = h->d_wv; r.wa = h->d_wa;
-    r.count = 3 * (long long)LS; r.ratio = h->rho / rho; r.qpl = nullptr; r.qpl_count = 0;
+    r.count = 3 * (long long)LS; r.ratio = h->rho / rho; r.qpl = nullptr; r.qpl_count = 0; r.u2 = h->d_u2;
     CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
     h->launches += 1;
     h->rho = rho;
@@ -1250,20 +1274,27 @@ extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, do
     std::vector<double> buf;
     top_status st;
     if (f == "z" || f == "u") {
-        const size_t want = f == "z" ? (size_t)batch * (N + 1) * s * dims : (size_t)batch * N * 2 * s * dims;
+        // consensus rows per boundary: nc = s, or 2s-1 with TOP_CONSENSUS_WIDE (the orders >= s live in the second row block:
+        // slot t = start-boundary row of order s + t, slot 4 + t = end-boundary row; rows that do not exist read 0)
+        const int nc = h->nc;
+        const size_t want = f == "z" ? (size_t)batch * (N + 1) * nc * dims : (size_t)batch * N * 2 * nc * dims;
         if (count != want) return fail(h, TOP_E_INVALID, "top_get_state: count does not match the field");
         if ((st = download_real(h, f == "z" ? h->d_zt : h->d_u, buf, 3 * LS)) != TOP_OK) return st;
+        std::vector<double> buf2;
+        if (h->wide && (st = download_real(h, f == "z" ? h->d_zt2 : h->d_u2, buf2, 3 * LS)) != TOP_OK) return st;
         for (int b = 0; b < batch; ++b)
             for (int i = 0; i < N; ++i) {
                 const size_t g = (size_t)b * N + i;
-                for (int r = 0; r < 2 * s; ++r)
-                    for (int d = 0; d < dims; ++d) {
-                        double v = buf[(size_t)d * LS + g * LANES + r];
-                        if (f == "z" && r % s == 0) v += h->h_wp[((size_t)b * (N + 1) + i) * dims + d];   // local frame (origin p_{i-1}) -> global
-                        if (f == "u") out[((g * 2 * s) + r) * dims + d] = v;
-                        else if (r < s) out[(((size_t)b * (N + 1) + i) * s + r) * dims + d] = v;
-                        else if (i == N - 1) out[(((size_t)b * (N + 1) + N) * s + (r - s)) * dims + d] = v;
-                    }
+                for (int side = 0; side < 2; ++side)
+                    for (int k = 0; k < nc; ++k)
+                        for (int d = 0; d < dims; ++d) {
+                            double v = k < s ? buf[(size_t)d * LS + g * LANES + side * s + k]
+                                             : buf2[(size_t)d * LS + g * LANES + side * 4 + (k - s)];
+                            if (f == "z" && k == 0) v += h->h_wp[((size_t)b * (N + 1) + i) * dims + d];   // local frame (origin p_{i-1}) -> global
+                            if (f == "u") out[((g * 2 * nc) + side * nc + k) * dims + d] = v;
+                            else if (side == 0) out[(((size_t)b * (N + 1) + i) * nc + k) * dims + d] = v;
+                            else if (i == N - 1) out[(((size_t)b * (N + 1) + N) * nc + k) * dims + d] = v;
+                        }
             }
         return check_abort(h);
     }
@@ -1325,7 +1356,7 @@ struct SnapshotHeader {
 constexpr uint64_t SNAP_MAGIC = 0x544f50534e415032ull;     // "TOPSNAP2"
 // the device arrays that make up an iterate, in snapshot order (null ones are skipped)
 int snapshot_fields(top_solver* h, void** out) {
-    void* all[] = {h->d_zt, h->d_u, h->d_qp, h->d_qn, h->d_phv, h->d_wv, h->d_pha, h->d_wa, h->d_chat};
+    void* all[] = {h->d_zt, h->d_u, h->d_qp, h->d_qn, h->d_phv, h->d_wv, h->d_pha, h->d_wa, h->d_chat, h->d_zt2, h->d_u2};
     int n = 0;
     for (void* p : all) if (p) out[n++] = p;
     return n;
@@ -1335,7 +1366,7 @@ int snapshot_fields(top_solver* h, void** out) {
 extern "C" TOP_API size_t top_snapshot_bytes(const top_solver* hc) {
     if (!hc) return 0;
     top_solver* h = const_cast<top_solver*>(hc);
-    void* f[9];
+    void* f[11];
     const int n = snapshot_fields(h, f);
     return sizeof(SnapshotHeader) + (size_t)n * 3 * (size_t)h->stride * real_bytes(h) + (size_t)h->batch * 4 * 8 +
            (h->has_poly ? (size_t)h->K * (size_t)h->stride * 8 : 0);
@@ -1352,7 +1383,7 @@ extern "C" TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, s
     hd.wp_mode = h->wp_mode; hd.N = (uint32_t)h->N;
     unsigned char* o = static_cast<unsigned char*>(host_buf);
     std::memcpy(o, &hd, sizeof hd); o += sizeof hd;
-    void* f[9];
+    void* f[11];
     const int n = snapshot_fields(h, f);
     const size_t fb = 3 * (size_t)h->stride * real_bytes(h);
     for (int i = 0; i < n; ++i) { CU(cudaMemcpyAsync(o, f[i], fb, cudaMemcpyDeviceToHost, h->stream), "D2H snapshot"); o += fb; }
@@ -1373,7 +1404,7 @@ extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* ho
         return fail(h, TOP_E_INVALID, "top_snapshot_restore: the snapshot belongs to a different problem");
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     const unsigned char* o = static_cast<const unsigned char*>(host_buf) + sizeof hd;
-    void* f[9];
+    void* f[11];
     const int n = snapshot_fields(h, f);
     const size_t fb = 3 * (size_t)h->stride * real_bytes(h);
     for (int i = 0; i < n; ++i) { CU(cudaMemcpyAsync(f[i], o, fb, cudaMemcpyHostToDevice, h->stream), "H2D snapshot"); o += fb; }

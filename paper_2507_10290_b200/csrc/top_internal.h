@@ -20,7 +20,8 @@ constexpr uint8_t SEG_LAST = 2;   // last segment: right junction (z_N) is fixed
 constexpr uint32_t KF_BOX = 1, KF_VEL = 2, KF_ACC = 4, KF_PIN_POS = 8 /* PINNED_Z: position row of z held */,
                    KF_NEIGHBOUR_SYNC = 16, KF_PAIRWISE = 32 /* warp-pair named barriers instead of the CTA barrier */,
                    KF_OPEN_LEFT = 64, KF_OPEN_RIGHT = 128 /* streaming: the launch range starts / ends inside a chain (halo) */,
-                   KF_POLY = 256 /* general polytope corridor (K planes per segment, rotated per-segment frame) */;
+                   KF_POLY = 256 /* general polytope corridor (K planes per segment, rotated per-segment frame) */,
+                   KF_WIDE = 512 /* paper-literal consensus n_c = 2s-1: a second block of consensus rows (orders s..2s-2) */;
 
 // Per-lane field arrays: element [f * stride + gseg * LANES + lane]; stride = padded lane count.
 // "Real" is double (TOP_F64) or float (TOP_F32); the x-update operator is always double.
@@ -79,6 +80,12 @@ struct KParams {
     void* qpl;              // double [K][stride]     Moreau value of (sample `lane`, plane k): s = max(0,q), v = max(0,-q)
     void* qpl_out;
     int K;
+    // ---- paper-literal consensus n_c = 2s-1 (KF_WIDE; fp64 tensor-core kernel only): the second block of consensus rows.
+    // Slot t < 4 of a segment = start-boundary row of derivative order s + t, slot 4 + t = end-boundary row of that order
+    // (t <= s-2); invTk2 = 1/T^(s+t), and 0 for slots / rows that do not exist (reading A1).  Read and written in place.
+    const void* invTk2;     // Real [stride]
+    void* zt2;              // Real [DIMS][stride]
+    void* u2;               // Real [DIMS][stride]
 };
 
 struct ConvParams {       // coefficient conversion to the paper's basis (Eq. 18)
@@ -101,8 +108,8 @@ int max_threads_for(int dtype, int lanes);
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, int threads, size_t smem, int* max_ctas_per_sm);
 // fp64 tensor-core variant of the 4-lane kernel (top_kernels_mma.cu: cadmm_sweeps_mma_kernel)
 cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st);
-size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly);
-int max_threads_mma(int dtype, bool poly);
+size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly, bool wide = false);
+int max_threads_mma(int dtype, bool poly, bool wide = false);
 cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm);
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
 // rho Pm^ = W diag(rho/(lambda_i+rho)) W',  c0^ = c_chord - (rho Pm^) g0   (spectral form; top_api.cpp build_spectral)
@@ -135,6 +142,7 @@ struct InitParams {
     // outputs
     double *c0, *g0, *dp, *origin;
     void *invTk, *Tpow, *invT, *lohi, *zoff, *zt, *chat, *qp, *qn, *phv;
+    void* invTk2;                 // wide consensus (n_c = 2s-1): 1/T^(s+t) per slot of the second row block, 0 where no row exists; or null
     // polytope corridor: rotation and rotated planes (host precompute), per-dim box weight lambda_d (eigenvalues of sum a a'),
     // and the Moreau values of the chord samples (output)
     const double *rot, *planes, *lam3;   // [9][nseg_pad], [K][4][nseg_pad], [3][nseg_pad]
@@ -147,7 +155,7 @@ struct InitParams {
 };
 cudaError_t launch_init(const InitParams& p, int dtype, cudaStream_t st);
 // duals *= ratio after a change of rho: u, w (both balls), and the negative part of the Moreau values q (= -v)
-struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; void* qpl; long long qpl_count; };
+struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; void* qpl; long long qpl_count; void* u2; };
 cudaError_t launch_rescale_duals(const RescaleParams& p, int dtype, cudaStream_t st);
 cudaError_t launch_residual_reduce(const double* part, double* res, long long N, int batch, cudaStream_t st);
 cudaError_t launch_fma_peak(int dtype, int blocks, int threads, long long iters, float* sink, cudaStream_t st);

@@ -1110,6 +1110,18 @@ __global__ void init_problem_kernel(const InitParams p) {
         itk = 1.0 / tk;
     }
     static_cast<Real*>(p.invTk)[idx] = (Real)itk;
+    if (p.invTk2) {
+        // wide consensus (reading A1): slot t < 4 = start-boundary row of order s + t, slot 4 + t = end-boundary row; the
+        // orders >= s do not exist at the two trajectory ends (z_0, z_N carry the given end state, orders < s) nor for t = s-1
+        const int t = lane & 3, at_end = lane >> 2;
+        double v = 0.0;
+        if (t <= s - 2 && !(at_end ? i == N - 1 : i == 0)) {
+            double tk = 1.0;
+            for (int q = 0; q < s + t; ++q) tk *= T;
+            v = 1.0 / tk;
+        }
+        static_cast<Real*>(p.invTk2)[idx] = (Real)v;
+    }
     for (int d = 0; d < 3; ++d) {
         // z0: position = waypoint; velocity = mean of the adjacent chord velocities; higher orders 0; z_0, z_N given
         double z = 0.0;
@@ -1168,6 +1180,7 @@ __global__ void rescale_duals_kernel(const RescaleParams p) {
     if (i >= p.count) return;
     const Real r = (Real)p.ratio;
     static_cast<Real*>(p.u)[i] *= r;
+    if (p.u2) static_cast<Real*>(p.u2)[i] *= r;
     if (p.wv) static_cast<Real*>(p.wv)[i] *= r;
     if (p.wa) static_cast<Real*>(p.wa)[i] *= r;
     if (p.qp) {

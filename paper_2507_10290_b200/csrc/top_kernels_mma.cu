@@ -95,13 +95,16 @@ constexpr int CM_RUNTIME = 8;
 
 // polytope corridor instantiations: <= 160 threads (5 warps: 40 segments; the per-plane state needs the shared memory)
 constexpr int MAXT_MMA_POLY = 160;
+// paper-literal consensus n_c = 2s-1 (reading A1): a second block of consensus rows per segment (orders s..2s-2 at both
+// boundaries: (z~, u) pairs, boundary-row buffer, mailbox slots); <= 224 threads (7 warps: 56 segments)
+constexpr int MAXT_MMA_WIDE = 224;
 constexpr int PSTR = KMAX * 4 + 2;      // doubles per segment of the plane table (padded: the 8 segments of a warp hit distinct banks)
 constexpr int VSTR = 10;                // doubles per segment of the rotation table
 
 struct SmemLayoutMma {
-    size_t pm, c0, zu, qs, ws, ph, ctab, lohi, xs, bs, zoff, qpl, pls, vs, total;
+    size_t pm, c0, zu, qs, ws, ph, ctab, lohi, xs, bs, zoff, qpl, pls, vs, zu2, bs2, total;
 };
-__host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc, bool poly = false, int rb = 8) {
+__host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_alloc, bool poly = false, int rb = 8, bool wide = false) {
     SmemLayoutMma L;
     const int T = segs_alloc * 4;
     size_t off = 0;
@@ -111,7 +114,7 @@ __host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_all
     L.qs = off;   off = align16(off + (size_t)(cons && !poly ? 6 : 0) * T * 2 * rb);   // Moreau pair values (q+, q-) of the lane's two samples (box)
     L.ws = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * 2 * rb);   // ball duals (w_v, w_a) of the lane's two samples
     L.ph = off;   off = align16(off + (size_t)(cons ? 6 : 0) * T * 2 * rb);   // ball variables (phi_v, phi_a)
-    L.ctab = off; off = align16(off + (size_t)16 * 32 * sizeof(double));               // constant MMA operands, [16][lane of warp]
+    L.ctab = off; off = align16(off + (size_t)20 * 32 * sizeof(double));               // constant MMA operands, [16 (+4: wide consensus)][lane of warp]
     L.lohi = off; off = align16(off + (size_t)(cons && !poly ? 6 : 0) * segs_alloc * rb);
     L.xs = off;   off = align16(off + (size_t)segs_alloc * XSTRIDE * sizeof(double));  // rhs rows, all-gather
     L.bs = off;   off = align16(off + (size_t)2 * (segs_alloc + 2) * 24 * rb);   // boundary rows, double buffered
@@ -119,6 +122,8 @@ __host__ __device__ inline SmemLayoutMma smem_layout_mma(bool cons, int segs_all
     L.qpl = off;  off = align16(off + (size_t)(poly ? KMAX * 2 : 0) * T * sizeof(double));          // Moreau values per (plane, sample of the lane)
     L.pls = off;  off = align16(off + (size_t)(poly ? segs_alloc : 0) * PSTR * sizeof(double));     // rotated planes (a'_k, b'_k) per segment
     L.vs = off;   off = align16(off + (size_t)(poly ? segs_alloc : 0) * VSTR * sizeof(double));     // rotation V per segment
+    L.zu2 = off;  off = align16(off + (size_t)(wide ? 6 : 0) * T * 2 * rb);                         // (z~, u) of the lane's two rows of the second consensus block
+    L.bs2 = off;  off = align16(off + (size_t)(wide ? 2 : 0) * (segs_alloc + 2) * 24 * rb);         // boundary rows of the second block, double buffered
     L.total = off;
     return L;
 }
@@ -149,9 +154,16 @@ __device__ __noinline__ void refresh_operator_rows(const KParams& p, long long g
     for (int d = 0; d < 3; ++d) c0_row[d * TS] = c0n[d];
 }
 
-template <typename Real, int S, int CM, int MAXT, bool SOLVE, bool POLY = false>
+template <typename Real, int S, int CM, int MAXT, bool SOLVE, bool POLY = false, bool WIDE = false>
 __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams p) {
     constexpr int N2 = 2 * S;
+    // WIDE: the paper-literal consensus (reading A1): derivative orders 0..2s-2 at both boundaries.
+    // Orders 0..s-1 are the first block (as always); orders s..2s-2 form a SECOND block of consensus rows with the same
+    // lane <-> row map: lane t owns order s+t at the start boundary (item h = 0) and at the end boundary (h = 1), t <= s-2.
+    // Rows that do not exist (t = s-1; the trajectory ends, where z_0 / z_N carry orders < s only) have 1/T^k = 0 in
+    // invTk2: their operand, boundary value, residual and dual are identically 0.
+    static_assert(!(WIDE && POLY), "wide consensus is not instantiated for polytope corridors");
+    constexpr int MBS = WIDE ? 48 : 24;              // mailbox slots per CTA and parity: [2 sides][4 or 8 orders][3 dims]
     constexpr int LPS = 4;                         // lanes per segment
     constexpr bool CONS = CM != 0 || POLY;
     static_assert(!(SOLVE && POLY), "the in-kernel stop rule is not instantiated for polytope corridors (host loop)");
@@ -179,7 +191,9 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     const bool pin_pos = flags & KF_PIN_POS;
     const bool nb_sync = flags & KF_NEIGHBOUR_SYNC;
 
-    const SmemLayoutMma L = smem_layout_mma(CONS, SA, POLY, (int)sizeof(Real));
+    const SmemLayoutMma L = smem_layout_mma(CONS, SA, POLY, (int)sizeof(Real), WIDE);
+    R2* zus2 = reinterpret_cast<R2*>(smem_raw + L.zu2) + tid;        // [(h*3 + d) * TS]: (z~, u) of the second block
+    Real* Bs2 = reinterpret_cast<Real*>(smem_raw + L.bs2);           // [2 parity][SA+2][2 sides][4][3]
     double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + tid;          // [((d*2 +) h*4 + b/2) * TS]   (d only with POLY)
     double* c0s = reinterpret_cast<double*>(smem_raw + L.c0) + tid;            // [(h*3 + d) * TS]
     R2* zus = reinterpret_cast<R2*>(smem_raw + L.zu) + tid;          // [(h*3 + d) * TS]: (z~, u)
@@ -250,6 +264,20 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 ctab[(8 + kk * 4 + nt) * 32] = v;
             }
         }
+        if (WIDE) {
+            // second consensus block.  a1 operand of k-step h (h = 0 start, 1 end boundary): row k = lane <-> order S + lane,
+            // column n = grp = coefficient row.  a3 operand of k-step kk: row k = coefficient row 4 kk + lane, column n = grp
+            // <-> item (grp >> 1, side grp & 1), so that accumulator columns 2t, 2t+1 are the lane's own two rows.
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+                ctab[(16 + h) * 32] = (a < N2 && lane <= S - 2) ? beta_entry(S + lane, a, h ? 1.0 : 0.0) : 0.0;
+            const int t2 = grp >> 1, h2 = grp & 1;
+#pragma unroll
+            for (int kk = 0; kk < 2; ++kk) {
+                const int ar = 4 * kk + lane;
+                ctab[(18 + kk) * 32] = (ar < N2 && t2 <= S - 2) ? beta_entry(S + t2, ar, h2 ? 1.0 : 0.0) : 0.0;
+            }
+        }
     }
     Real invTk[2];
 #pragma unroll
@@ -264,6 +292,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         for (int d = 0; d < 3; ++d) c0s[(h * 3 + d) * TS] = p.c0[d * stride + gt[h]];
         invTk[h] = static_cast<const Real*>(p.invTk)[gt[h]];
     }
+    Real invTk2[2] = {0, 0};
+    if (WIDE) { invTk2[0] = static_cast<const Real*>(p.invTk2)[gt[0]]; invTk2[1] = static_cast<const Real*>(p.invTk2)[gt[1]]; }
     const Real invT = static_cast<const Real*>(p.invT)[gseg], invT2 = static_cast<const Real*>(p.invT)[p.nseg_pad + gseg];
     if (CONS && !POLY) {
         lohi[lane * SA] = static_cast<const Real*>(p.lohi)[lane * p.nseg_pad + gseg];
@@ -306,16 +336,51 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         const bool edge_l = active && isrow[h] && sl == 0 && !right[h] && cta > 0;
         const bool edge_r = active && isrow[h] && sl == nact - 1 && right[h] && cta + 1 < nctas;
         pub[h] = nctas > 1 && (edge_l || edge_r);
-        pub_off[h] = (cta * 24 + (edge_r ? 12 : 0) + korder[h] * 3) * 16;
+        pub_off[h] = (cta * MBS + (edge_r ? MBS / 2 : 0) + korder[h] * 3) * 16;
         if (edge_l || edge_r) {
             need = true; need_h = h;
-            need_off = edge_l ? ((cta - 1) * 24 + 12 + korder[h] * 3) * 16 : ((cta + 1) * 24 + korder[h] * 3) * 16;
+            need_off = edge_l ? ((cta - 1) * MBS + MBS / 2 + korder[h] * 3) * 16 : ((cta + 1) * MBS + korder[h] * 3) * 16;
+        }
+    }
+    // second consensus block (WIDE): item h = 0 is the start-boundary row of order S + lane, h = 1 the end-boundary row
+    const bool isrow2 = WIDE && lane <= S - 2;
+    int own2_off[2] = {0, 0}, nb2_off[2] = {0, 0}, pub2_off[2] = {0, 0};
+    bool fixed2[2] = {true, true}, gaprow2[2] = {false, false}, pub2[2] = {false, false};
+    bool need2 = false;
+    int need2_h = 0, need2_off = 0;
+    if (WIDE) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            own2_off[h] = (sl + 1) * 24 + (h * 4 + lane) * 3;
+            nb2_off[h] = h ? (sl + 2) * 24 + lane * 3 : sl * 24 + (4 + lane) * 3;
+            fixed2[h] = (h ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (h ? open_r : open_l);
+            gaprow2[h] = isrow2 && h == 1 && !(sf & SEG_LAST);
+            const bool edge_l = active && isrow2 && sl == 0 && h == 0 && cta > 0;
+            const bool edge_r = active && isrow2 && sl == nact - 1 && h == 1 && cta + 1 < nctas;
+            pub2[h] = nctas > 1 && (edge_l || edge_r);
+            pub2_off[h] = (cta * MBS + (edge_r ? MBS / 2 : 0) + (S + lane) * 3) * 16;
+            if (edge_l || edge_r) {
+                need2 = true; need2_h = h;
+                need2_off = edge_l ? ((cta - 1) * MBS + MBS / 2 + (S + lane) * 3) * 16 : ((cta + 1) * MBS + (S + lane) * 3) * 16;
+            }
         }
     }
 
     // ---- state of iterate k.  Registers hold the a1 OPERANDS:
     //   gM = (z~ - u)/T^k      A0 = (hi - s+ - v+) + (lo + s- + v-)      gv = (phi_v - w_v)/T      ga = (phi_a - w_a)/T^2
     double gM[2][3], A0[2][3], gv[2][3], ga[2][3];
+    double gM2[2][3] = {{0, 0, 0}, {0, 0, 0}};      // WIDE: operand of the second consensus block, (z~ - u)/T^k
+    if (WIDE) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                const long long i = d * stride + gt[h];
+                const Real z0 = static_cast<const Real*>(p.zt2)[i], u0 = static_cast<const Real*>(p.u2)[i];
+                zus2[(h * 3 + d) * TS] = make2(z0, u0);
+                gM2[h][d] = (double)((z0 - u0) * invTk2[h]);
+            }
+    }
 #pragma unroll
     for (int h = 0; h < 2; ++h)
 #pragma unroll
@@ -350,7 +415,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 
     const Real vmax = (Real)p.vmax, amax = (Real)p.amax;
     unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
-    const size_t mbox_par_stride = (size_t)p.max_ctas * 24 * 16;
+    const size_t mbox_par_stride = (size_t)p.max_ctas * MBS * 16;
     __shared__ int abort_sh[2];
     __shared__ int abort_any;
     if (tid < 2) abort_sh[tid] = 0;
@@ -373,6 +438,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
         const bool last_sweep = final_sweep || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
         Real* const Bcur = Bs + par * BPAR;
+        Real* const Bcur2 = Bs2 + par * BPAR;
         unsigned char* const mpar = mbox + par * mbox_par_stride;
 
         // ================= phase A: segment local =================
@@ -398,6 +464,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             for (int h = 0; h < 2; ++h)
 #pragma unroll
                 for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gM[h][d], ctab[h * 32]);
+            if (WIDE) {
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gM2[h][d], ctab[(16 + h) * 32]);
+            }
             if (has_box || POLY) {      // Ao'(b - s - v): box Ao = [E0; -E0], b = [hi; -lo], s + v = |q| (Moreau pair); polytope: kron(E0, a_k')
 #pragma unroll
                 for (int h = 0; h < 2; ++h)
@@ -471,11 +543,36 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 }
             }
         }
+        if (WIDE) {     // boundary derivatives of orders s..2s-2 (second block of B = M c)
+            Real Bnd2[2][3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                double e0 = 0, e1 = 0;
+                dmma884(e0, e1, cacc[0][d], ctab[18 * 32]);
+                dmma884(e0, e1, cacc[1][d], ctab[19 * 32]);
+                Bnd2[0][d] = (Real)e0 * invTk2[0]; Bnd2[1][d] = (Real)e1 * invTk2[1];
+            }
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (isrow2) {
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) Bcur2[own2_off[h] + d] = Bnd2[h][d];
+                }
+                if (pub2[h]) {
+#pragma unroll
+                    for (int d = 0; d < 3; ++d) ll_store(mpar + pub2_off[h] + d * 16, (double)Bnd2[h][d], seq);
+                }
+            }
+        }
         // prefetch the rows of the neighbouring CTA: the loads fly during the projections
-        LLRaw rr[3];
+        LLRaw rr[3], rr2[3];
         if (need) {
 #pragma unroll
             for (int d = 0; d < 3; ++d) ll_issue(mpar + need_off + d * 16, rr[d]);
+        }
+        if (WIDE && need2) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) ll_issue(mpar + need2_off + d * 16, rr2[d]);
         }
         if (CONS) {
             // the three sample blocks of the evaluation back to back, then the projections of all blocks side by side:
@@ -567,8 +664,9 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         int wait_failed = 0;
         {
             bool okk = !need || (ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq));
-            if (pairwise && *(volatile int*)&abort_any) okk = true;
-            if (!__all_sync(0xffffffffu, okk)) {
+            bool okk2 = !(WIDE && need2) || (ll_ok(rr2[0], seq) && ll_ok(rr2[1], seq) && ll_ok(rr2[2], seq));
+            if (pairwise && *(volatile int*)&abort_any) okk = okk2 = true;
+            if (!__all_sync(0xffffffffu, okk && okk2)) {
                 const long long t0 = global_ns();
                 unsigned spins = 0;
                 do {
@@ -577,10 +675,15 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                         for (int d = 0; d < 3; ++d) ll_issue(mpar + need_off + d * 16, rr[d]);
                         okk = ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq);
                     }
+                    if (WIDE && !okk2) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) ll_issue(mpar + need2_off + d * 16, rr2[d]);
+                        okk2 = ll_ok(rr2[0], seq) && ll_ok(rr2[1], seq) && ll_ok(rr2[2], seq);
+                    }
                     bool bail = false;
                     if ((++spins & 255u) == 0) bail = *(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS;
-                    if (__any_sync(0xffffffffu, bail)) { if (!okk) { atomicExch(p.abort_flag, 1); wait_failed = 1; } break; }
-                } while (!__all_sync(0xffffffffu, okk));
+                    if (__any_sync(0xffffffffu, bail)) { if (!(okk && okk2)) { atomicExch(p.abort_flag, 1); wait_failed = 1; } break; }
+                } while (!__all_sync(0xffffffffu, okk && okk2));
             }
         }
         if (wait_failed) { abort_sh[it & 1] = 1; *(volatile int*)&abort_any = 1; }
@@ -639,6 +742,29 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 }
             }
         if constexpr (POLY) { rot_in(vs, gM[0]); rot_in(vs, gM[1]); }
+        Real dz2[2][3] = {{0, 0, 0}, {0, 0, 0}};
+        if (WIDE) {     // the same consensus / dual step on the rows of orders s..2s-2 (never position rows: no frame shift)
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+#pragma unroll
+                for (int d = 0; d < 3; ++d) {
+                    const Real own2 = Bcur2[own2_off[h] + d];
+                    Real nb2 = Bcur2[nb2_off[h] + d];
+                    if (need2 && need2_h == h) nb2 = (Real)ll_value(rr2[d]);
+                    const R2 zu2 = zus2[(h * 3 + d) * TS];
+                    const Real avg = (Real)0.5 * (own2 + nb2);
+                    const Real znew = (fixed2[h] || !isrow2) ? zu2.x : avg;             // a5: Eq. 6b / 20b
+                    dz2[h][d] = znew - zu2.x;
+                    const Real res = (isrow2 && !fixed2[h]) ? own2 - znew : (Real)0;    // rows at the trajectory ends do not exist (A1)
+                    const Real unew = zu2.y + res;                                      // a8: Eq. 6c / 20c
+                    zus2[(h * 3 + d) * TS] = make2(znew, unew);
+                    gM2[h][d] = (double)((znew - unew) * invTk2[h]);
+                    if (last_sweep) {
+                        rp2 += (double)res * (double)res;
+                        if (gaprow2[h]) { const double gp = (double)own2 - (double)nb2; gap2 += gp * gp; }   // Eq. 21
+                    }
+                }
+        }
         if (last_sweep) {
             // a6: dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8):
             // the consensus block of the a1 contraction applied to dz; lane t ends with coefficient rows 2t, 2t+1
@@ -649,6 +775,10 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 double x0 = 0, x1 = 0;
                 dmma884(x0, x1, (double)(dz[0][d] * invTk[0]), ctab[0 * 32]);
                 dmma884(x0, x1, (double)(dz[1][d] * invTk[1]), ctab[1 * 32]);
+                if (WIDE) {
+                    dmma884(x0, x1, (double)(dz2[0][d] * invTk2[0]), ctab[16 * 32]);
+                    dmma884(x0, x1, (double)(dz2[1][d] * invTk2[1]), ctab[17 * 32]);
+                }
                 const double xr0 = rho_cur * x0, xr1 = rho_cur * x1;
                 rdn2 += xr0 * xr0 + xr1 * xr1;
                 rd2 += (xr0 * Tp0) * (xr0 * Tp0) + (xr1 * Tp1) * (xr1 * Tp1);
@@ -719,6 +849,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                                 zz.y *= ratio;
                                 zus[(h * 3 + d) * TS] = zz;
                                 gM[h][d] = (double)((zz.x - zz.y) * invTk[h]);
+                                if (WIDE) {
+                                    R2 z2 = zus2[(h * 3 + d) * TS];
+                                    z2.y *= ratio;
+                                    zus2[(h * 3 + d) * TS] = z2;
+                                    gM2[h][d] = (double)((z2.x - z2.y) * invTk2[h]);
+                                }
                                 if (has_box) {
                                     const Real lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
                                     R2 q = qs[(h * 3 + d) * TS];
@@ -760,6 +896,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 const R2 zz = zus[(h * 3 + d) * TS];
                 static_cast<Real*>(p.zt_out)[i] = zz.x;
                 static_cast<Real*>(p.u_out)[i] = zz.y;
+                if (WIDE) { const R2 z2 = zus2[(h * 3 + d) * TS]; static_cast<Real*>(p.zt2)[i] = z2.x; static_cast<Real*>(p.u2)[i] = z2.y; }
                 if (has_box) { const R2 q = qs[(h * 3 + d) * TS]; static_cast<Real*>(p.qp_out)[i] = q.x; static_cast<Real*>(p.qn_out)[i] = q.y; }
                 if (POLY && d == 0) for (int k = 0; k < KP; ++k) static_cast<double*>(p.qpl_out)[k * stride + gt[h]] = qpls[(k * 2 + h) * TS];
                 if (has_vel || has_acc) {
@@ -785,6 +922,25 @@ cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cud
 template <typename Real, int S, int CM, int MAXT>
 cudaError_t limits_mma(int threads, size_t smem, int* per_sm) {
     auto kern = cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, true>;     // the larger of the two instantiations
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
+}
+
+template <int S>
+cudaError_t launch_mma_wide(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
+    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_WIDE, true, false, true>
+                                  : cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_WIDE, false, false, true>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    KParams pc = p;
+    void* args[] = {&pc};
+    if (ctas > 1) return cudaLaunchCooperativeKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+    return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+}
+template <int S>
+cudaError_t limits_mma_wide(int threads, size_t smem, int* per_sm) {
+    auto kern = cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_WIDE, true, false, true>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
@@ -828,13 +984,17 @@ int mma_mask(uint32_t kflags) {
         else        { if (cm == 0) { CALL(float, 4, 0, MAXT_MMA_F32) } else if (cm == 3) { CALL(float, 4, 3, MAXT_MMA_F32) } else if (cm == 7) { CALL(float, 4, 7, MAXT_MMA_F32) } else { CALL(float, 4, CM_RUNTIME, MAXT_MMA_F32) } } \
     }
 
-int max_threads_mma(int dtype, bool poly) { return poly ? MAXT_MMA_POLY : (dtype == 0 ? MAXT_MMA : MAXT_MMA_F32); }
+int max_threads_mma(int dtype, bool poly, bool wide) { return wide ? MAXT_MMA_WIDE : poly ? MAXT_MMA_POLY : (dtype == 0 ? MAXT_MMA : MAXT_MMA_F32); }
 
 cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st) {
     const uint32_t kflags = p.flags;
     if (kflags & KF_POLY) {
         if (p.check_every > 0 || dtype != 0) return cudaErrorInvalidValue;      // host loop only, fp64 only
         return s == 3 ? launch_mma_poly<3>(p, ctas, threads, smem, st) : launch_mma_poly<4>(p, ctas, threads, smem, st);
+    }
+    if (kflags & KF_WIDE) {
+        if (dtype != 0) return cudaErrorInvalidValue;      // fp64 only
+        return s == 3 ? launch_mma_wide<3>(p, ctas, threads, smem, st) : launch_mma_wide<4>(p, ctas, threads, smem, st);
     }
 #define CALL(R_, S_, C_, M_) return launch_mma<R_, S_, C_, M_>(p, ctas, threads, smem, st);
     TOP_DISPATCH_MMA(CALL)
@@ -844,13 +1004,15 @@ cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int 
 
 cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm) {
     if (kflags & KF_POLY) return s == 3 ? limits_mma_poly<3>(threads, smem, max_ctas_per_sm) : limits_mma_poly<4>(threads, smem, max_ctas_per_sm);
+    if (kflags & KF_WIDE) return s == 3 ? limits_mma_wide<3>(threads, smem, max_ctas_per_sm) : limits_mma_wide<4>(threads, smem, max_ctas_per_sm);
 #define CALL(R_, S_, C_, M_) return limits_mma<R_, S_, C_, M_>(threads, smem, max_ctas_per_sm);
     TOP_DISPATCH_MMA(CALL)
 #undef CALL
     return cudaErrorInvalidValue;
 }
 
-size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly) {      // laid out for the largest CTA of the instantiation (see the kernel)
+size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly, bool wide) {      // laid out for the largest CTA of the instantiation (see the kernel)
+    if (wide) return smem_layout_mma(true, MAXT_MMA_WIDE / 4, false, 8, true).total;      // (run-time constraint mask: laid out with the constraint arrays)
     if (poly) return smem_layout_mma(true, MAXT_MMA_POLY / 4, true).total;
     return dtype == 0 ? smem_layout_mma(constrained, MAXT_MMA / 4).total : smem_layout_mma(constrained, MAXT_MMA_F32 / 4, false, 4).total;
 }

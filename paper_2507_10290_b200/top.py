@@ -22,6 +22,7 @@ TOP_RD_NORMALISED = 4
 TOP_EPS_N_SCALED = 8
 TOP_RHO_ADAPTIVE = 64
 TOP_KERNEL_NO_MMA = 128
+TOP_CONSENSUS_WIDE = 256
 SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
 EXPORTS = ["top_create", "top_reset", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
@@ -157,7 +158,7 @@ class TopSolver:
     def __init__(self, waypoints, durations, s, rho, dtype="f64", samples=0, box_lo=None, box_hi=None, vmax=0.0,
                  amax=0.0, start_derivs=None, end_derivs=None, mode="hard", rd_normalised=False, eps_n_scaled=False,
                  sync="auto", check_every=0, max_iter=0, device=-1, stream=0, segs_per_cta=0, lanes=0, adaptive_rho=False,
-                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0, no_mma=False, planes=None):
+                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0, no_mma=False, planes=None, consensus="s"):
         L = lib()
         wp = np.asarray(waypoints, dtype=np.float64)
         T = np.asarray(durations, dtype=np.float64)
@@ -174,6 +175,7 @@ class TopSolver:
         self.batch, self.N, self.dims = T.shape[0], T.shape[1], wp.shape[2]
         self.s, self.n, self.dtype = int(s), 2 * int(s), dtype
         self.Ms = int(samples)
+        self.nc = {"s": self.s, "wide": 2 * self.s - 1}[consensus]     # consensus derivative orders per boundary
         self.durations = T
         lo = _f64(box_lo, (self.batch, self.N, self.dims))
         hi = _f64(box_hi, (self.batch, self.N, self.dims))
@@ -188,7 +190,7 @@ class TopSolver:
             cons = _Constraints(int(samples), _dptr(lo), _dptr(hi), float(vmax), float(amax), self.K, _dptr(pl))
         flags = WAYPOINT[mode] | (TOP_RD_NORMALISED if rd_normalised else 0) | \
             (TOP_EPS_N_SCALED if eps_n_scaled else 0) | SYNC[sync] | (TOP_RHO_ADAPTIVE if adaptive_rho else 0) | \
-            (TOP_KERNEL_NO_MMA if no_mma else 0)
+            (TOP_KERNEL_NO_MMA if no_mma else 0) | (TOP_CONSENSUS_WIDE if consensus == "wide" else 0)
         opt = _Options(ctypes.sizeof(_Options), flags, int(check_every), int(device), int(max_iter),
                        ctypes.c_void_p(stream), int(segs_per_cta), int(lanes), float(adapt_mu), float(adapt_tau_incr),
                        float(adapt_tau_decr))
@@ -280,7 +282,7 @@ class TopSolver:
         """top_get_coeffs into a device buffer (no host synchronisation)."""
         self._check(self._L.top_get_coeffs(self._h, ctypes.c_void_p(device_ptr), 1))
 
-    _STATE_SHAPES = {"z": lambda o: (o.batch, o.N + 1, o.s, o.dims), "u": lambda o: (o.batch, o.N, 2 * o.s, o.dims)}
+    _STATE_SHAPES = {"z": lambda o: (o.batch, o.N + 1, o.nc, o.dims), "u": lambda o: (o.batch, o.N, 2 * o.nc, o.dims)}
 
     def state(self, field: str):
         if field in ("s_poly", "v_poly"):
