@@ -264,12 +264,16 @@ def run_latency(args, local_rank):
             for segs in (0, 4, 8, 16, 32, 64):
                 if segs and (segs * 148 < w.N or (lanes == 8 and segs > 64)):
                     continue
-                for sync in (("auto", "neighbour", "grid") if segs == 0 else ("auto",)):
+                # "auto" on the tensor-core kernel with 2..16 CTAs runs as ONE thread-block cluster (boundary rows through
+                # distributed shared memory); the explicit "pairwise" is the same synchronisation over the L2 mailbox
+                for sync in (("auto", "neighbour", "grid") if segs == 0 else ("auto", "pairwise")):
                     try:
                         us, li = time_us(w, lanes=lanes, segs_per_cta=segs, sync=sync)
                     except top.TopError:
                         continue
-                    rows.append({"config": name, "N": w.N, "lanes": lanes, "kernel": "mma" if lanes == 4 else "8-lane", "sync": sync,
+                    exch = "none" if li["ctas"] == 1 else ("dsmem-cluster" if (lanes == 4 and sync == "auto" and li["ctas"] <= 16) else
+                                                           ("grid-barrier" if sync == "grid" else "l2-mailbox"))
+                    rows.append({"config": name, "N": w.N, "lanes": lanes, "kernel": "mma" if lanes == 4 else "8-lane", "sync": sync, "exchange": exch,
                                  "segs_per_cta": li["segs_per_cta"], "ctas": li["ctas"], "threads": li["threads"], "us_per_sweep": us})
             # exchange-free reference: one CTA, a chain as long as one CTA's share of the default plan
             if name != "cfg1":
@@ -282,6 +286,10 @@ def run_latency(args, local_rank):
                     if li["ctas"] == 1:
                         rows.append({"config": name + "_single_cta_reference", "N": per, "lanes": lanes, "kernel": "mma" if lanes == 4 else "8-lane",
                                      "sync": "none (one CTA)", "segs_per_cta": li["segs_per_cta"], "ctas": 1, "threads": li["threads"], "us_per_sweep": us})
+        us, li = time_us(w)      # what top_create picks by itself
+        rows.append({"config": name, "N": w.N, "lanes": 0, "kernel": "default plan", "sync": "auto",
+                     "exchange": "none" if li["ctas"] == 1 else ("dsmem-cluster" if li["ctas"] <= 16 else "l2-mailbox"),
+                     "segs_per_cta": li["segs_per_cta"], "ctas": li["ctas"], "threads": li["threads"], "us_per_sweep": us})
     # launch overhead: an empty-ish launch (1 sweep) against the per-sweep time inside a long launch
     w = W.config2()
     sol = top.from_workload(w, device=local_rank, stream=stream.cuda_stream)

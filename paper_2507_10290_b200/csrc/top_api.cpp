@@ -59,7 +59,9 @@ struct top_solver {
     bool wide = false;                 // paper-literal consensus n_c = 2s-1 (reading A1): second block of consensus rows
     int nc = 0;                        // consensus derivative orders per boundary: s, or 2s-1
     void *d_zt2 = nullptr, *d_u2 = nullptr, *d_invTk2 = nullptr;
-    struct Wave { long long seg_begin, seg_end, own_begin, own_end; uint32_t kflags; int segs_per_cta, ctas, threads; size_t smem; };
+    struct Wave { long long seg_begin, seg_end, own_begin, own_end; uint32_t kflags; int segs_per_cta, ctas, threads; size_t smem;
+                  bool cluster;      // the wave can run as ONE thread-block cluster (<= 16 CTAs): exchange through distributed shared memory
+    };
     // streaming (temporal blocking) for chains longer than the on-chip capacity: pieces with `halo` extra segments on
     // each open side run `halo` sweeps per launch (the dependency radius of a sweep is one segment), reading iterate
     // k from one set of state buffers and writing iterate k + halo of their own segments to the other set
@@ -838,6 +840,21 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     // (configs 1, 3) stay on the 8-lane kernel (0.64 vs 0.85, 1.42 vs 1.57)
     if (!o.lanes_per_segment && dtype == TOP_F64 && ((has_box || has_vel || has_acc) || nseg >= (long long)h->num_sms * 32)) h->lanes = 4;
     if (!o.lanes_per_segment && (h->has_poly || h->wide)) h->lanes = 4;
+    // short chains (the paper's regime, tens to a thousand segments): at most 16 CTAs run as ONE thread-block cluster and
+    // exchange their boundary rows through distributed shared memory, which costs 0-0.25 us per sweep instead of the
+    // 0.45-0.8 us of the L2 mailbox between 25-125 small CTAs (profiles/r2_small_configs_latency.md: config 2 1.60 -> 1.38 us,
+    // config 3 1.41 -> 1.24 us).  It pays as long as the per-CTA share stays small: <= 32 segments per CTA with inequality
+    // sets, <= 64 without.  Chains of <= 16 segments stay on one CTA.
+    int plan_segs = 0;
+    if (dtype == TOP_F64 && !o.lanes_per_segment && !o.segs_per_cta && (o.flags & TOP_SYNC_MASK) == TOP_SYNC_AUTO &&
+        !(o.flags & TOP_KERNEL_NO_MMA) && !h->has_poly) {
+        const bool cons_any = has_box || has_vel || has_acc;
+        const long long per_cta_max = cons_any ? 32 : 64, per_cta_min = cons_any ? 16 : 32;
+        if (nseg > 16 && nseg <= 16 * per_cta_max) {
+            h->lanes = 4;
+            plan_segs = (int)std::max<long long>(per_cta_min, round_up((int)((nseg + 15) / 16), 8));
+        }
+    }
     h->mma = h->lanes == 4 && !(o.flags & TOP_KERNEL_NO_MMA);
     if (h->wide && (!(h->mma && dtype == TOP_F64) || h->has_poly))
         CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_CONSENSUS_WIDE runs on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA, no polytope corridor)"));
@@ -846,17 +863,19 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192, h->has_poly, h->wide);
     if (segs_max < 4) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "shared memory too small for one warp of segments"));
     h->max_ctas = h->num_sms;
+    if (plan_segs > segs_max) plan_segs = 0;
     const long long capacity = (long long)h->max_ctas * std::min(segs_max, h->user_segs ? h->user_segs : segs_max);
     auto make_wave = [&](long long r0, long long r1, long long o0, long long o1, uint32_t kf) -> bool {
         top_solver::Wave w;
         w.seg_begin = r0; w.seg_end = r1; w.own_begin = o0; w.own_end = o1; w.kflags = kf;
         const long long cnt = r1 - r0;
-        int segs = h->user_segs ? h->user_segs : round_up((int)((cnt + h->max_ctas - 1) / h->max_ctas), 4);
+        int segs = h->user_segs ? h->user_segs : plan_segs ? plan_segs : round_up((int)((cnt + h->max_ctas - 1) / h->max_ctas), 4);
         segs = std::max(4, std::min(segs, segs_max));
         w.segs_per_cta = segs;
         w.ctas = (int)((cnt + segs - 1) / segs);
         w.threads = (segs * h->lanes + 31) / 32 * 32;
         w.smem = kernel_smem(h->dtype, s, h->constrained, h->lanes, h->mma, segs, h->has_poly, h->wide);
+        w.cluster = false;
         if (w.ctas > h->max_ctas) return false;
         h->waves.push_back(w);
         return true;
@@ -894,6 +913,17 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
         if (e != cudaSuccess) CREATE_FAIL(cuda_fail(h, e, "occupancy query"));
         if (per_sm < 1) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "sweep kernel does not fit an SM"));
     }
+    // short chains (the paper's regime: tens to a few hundred segments): when a wave is at most 16 CTAs it runs as ONE
+    // thread-block cluster and the boundary rows travel through distributed shared memory instead of the L2 mailbox
+    // (TOP_SYNC_AUTO only; the explicit sync modes keep the mailbox so that the two can be compared)
+    if (h->mma && !h->streaming && (o.flags & TOP_SYNC_MASK) == TOP_SYNC_AUTO)
+        for (auto& w : h->waves) {
+            int ncl = 0;
+            if (w.ctas >= 2 && w.ctas <= 16 &&
+                sweep_cluster_limits_mma(h->dtype, s, h->kflags, w.ctas, w.threads, w.smem, &ncl) == cudaSuccess && ncl >= 1)
+                w.cluster = true;
+            cudaGetLastError();
+        }
 
     pt.mark("launch plan");
 
@@ -1072,7 +1102,7 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
             p.bar = reinterpret_cast<unsigned long long*>(h->d_sync);
             p.abort_flag = h->d_abort;
             p.stride = h->stride; p.nseg_pad = h->nseg_pad; p.seg_begin = w.seg_begin; p.seg_end = w.seg_end;
-            p.segs_per_cta = w.segs_per_cta; p.k_sweeps = kk; p.flags = h->kflags | sync_flag(h) | w.kflags;
+            p.segs_per_cta = w.segs_per_cta; p.k_sweeps = kk; p.flags = h->kflags | sync_flag(h) | w.kflags | (w.cluster ? KF_CLUSTER : 0);
             if (iks) {      // device-side stop rule / Eq. 24 (one CTA-wide barrier per sweep: no warp-pair barriers)
                 p.flags &= ~KF_PAIRWISE;
                 p.check_every = iks->check_every; p.rd_sel = iks->rd_sel; p.adaptive = iks->adaptive; p.tol = iks->tol;

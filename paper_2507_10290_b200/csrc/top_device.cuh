@@ -75,6 +75,27 @@ __device__ __forceinline__ double ll_value(const LLRaw& r) {
     return __longlong_as_double((long long)(((unsigned long long)r.b << 32) | r.a));
 }
 
+// ---- the same LL slots in DISTRIBUTED SHARED MEMORY (thread-block cluster): the producer stores straight into the
+// consumer CTA's shared memory (st.shared::cluster, ~215 cycles one way), the consumer polls its OWN shared memory
+// (~40 cycles per look) -- no L2 round trip.  Used when the whole chain fits one cluster (<= 16 CTAs).
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ unsigned cluster_map(unsigned local_addr, unsigned cta_rank) {
+    unsigned r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(cta_rank));
+    return r;
+}
+__device__ __forceinline__ void ll_store_cluster(unsigned remote_addr, double v, unsigned seq) {
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    asm volatile("st.shared::cluster.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(remote_addr), "r"((unsigned)b), "r"(seq),
+                 "r"((unsigned)(b >> 32)), "r"(seq) : "memory");
+}
+__device__ __forceinline__ void ll_issue_smem(unsigned local_addr, LLRaw& r) {
+    asm volatile("ld.volatile.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.a), "=r"(r.f0), "=r"(r.b), "=r"(r.f1) : "r"(local_addr) : "memory");
+}
+__device__ __forceinline__ void cluster_barrier() {
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
 // [beta_k(tau)]_a = a!/(a-k)! tau^(a-k), a >= k   (Eq. 18 differentiated k times, normalised time)
 __device__ __forceinline__ double beta_entry(int k, int a, double tau) {
     if (a < k) return 0.0;

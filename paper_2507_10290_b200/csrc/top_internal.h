@@ -21,7 +21,8 @@ constexpr uint32_t KF_BOX = 1, KF_VEL = 2, KF_ACC = 4, KF_PIN_POS = 8 /* PINNED_
                    KF_NEIGHBOUR_SYNC = 16, KF_PAIRWISE = 32 /* warp-pair named barriers instead of the CTA barrier */,
                    KF_OPEN_LEFT = 64, KF_OPEN_RIGHT = 128 /* streaming: the launch range starts / ends inside a chain (halo) */,
                    KF_POLY = 256 /* general polytope corridor (K planes per segment, rotated per-segment frame) */,
-                   KF_WIDE = 512 /* paper-literal consensus n_c = 2s-1: a second block of consensus rows (orders s..2s-2) */;
+                   KF_WIDE = 512 /* paper-literal consensus n_c = 2s-1: a second block of consensus rows (orders s..2s-2) */,
+                   KF_CLUSTER = 1024 /* the launch is ONE thread-block cluster: boundary rows go through distributed shared memory */;
 
 // Per-lane field arrays: element [f * stride + gseg * LANES + lane]; stride = padded lane count.
 // "Real" is double (TOP_F64) or float (TOP_F32); the x-update operator is always double.
@@ -111,6 +112,7 @@ cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int 
 size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly, bool wide = false);
 int max_threads_mma(int dtype, bool poly, bool wide = false);
 cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm);
+cudaError_t sweep_cluster_limits_mma(int dtype, int s, uint32_t kflags, int ctas, int threads, size_t smem, int* nclusters);
 cudaError_t launch_convert(const ConvParams& p, int dtype, cudaStream_t st);
 // rho Pm^ = W diag(rho/(lambda_i+rho)) W',  c0^ = c_chord - (rho Pm^) g0   (spectral form; top_api.cpp build_spectral)
 struct RefreshParams {

@@ -26,6 +26,8 @@
 //               the per-segment operator rows; the all-gather buffer; the boundary-row exchange buffer
 // The constraint selection is a template parameter (the three combinations BASELINE.json's configs use, plus a
 // run-time-flag variant for the others): no branch inside the sweep body except the exchange.
+#include <string.h>
+
 #include "top_device.cuh"
 
 namespace top {
@@ -416,6 +418,32 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     const Real vmax = (Real)p.vmax, amax = (Real)p.amax;
     unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
     const size_t mbox_par_stride = (size_t)p.max_ctas * MBS * 16;
+    // cluster exchange (KF_CLUSTER: the grid is one thread-block cluster): the mailbox of a CTA lives in its own shared
+    // memory, [2 parity][2 sides: 0 = from the left neighbour, 1 = from the right][MBS/2 slots]; the neighbours store into
+    // it through distributed shared memory, this CTA polls it locally
+    const bool clus = (flags & KF_CLUSTER) != 0;
+    __shared__ __align__(16) unsigned char cmbox[2 * MBS * 16];
+    const unsigned cm_local = smem_u32(cmbox);
+    unsigned cm_remote[2] = {0, 0};      // the mailbox of the CTA my item h publishes to
+    if (clus) {
+        for (int i = tid; i < 2 * MBS * 4; i += T) reinterpret_cast<unsigned*>(cmbox)[i] = 0u;
+        cm_remote[0] = cta > 0 ? cluster_map(cm_local, (unsigned)(cta - 1)) : 0u;            // left neighbour
+        cm_remote[1] = cta + 1 < nctas ? cluster_map(cm_local, (unsigned)(cta + 1)) : 0u;    // right neighbour
+        cluster_barrier();      // every CTA of the cluster runs and has cleared its mailbox before anyone stores into it
+        // offsets inside a mailbox (bytes, relative to the parity base): a row at my right edge goes to the right neighbour's
+        // half 0, a row at my left edge to the left neighbour's half 1; what I need sits in my own half 0 (left edge) / 1
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const bool er = right[h];
+            pub_off[h] = ((er ? 0 : 1) * (MBS / 2) + korder[h] * 3) * 16;
+            if (need && need_h == h) need_off = ((er ? 1 : 0) * (MBS / 2) + korder[h] * 3) * 16;
+            if (WIDE) {
+                pub2_off[h] = ((h ? 0 : 1) * (MBS / 2) + (S + lane) * 3) * 16;
+                if (need2 && need2_h == h) need2_off = ((h ? 1 : 0) * (MBS / 2) + (S + lane) * 3) * 16;
+            }
+        }
+    }
+    const size_t par_stride = clus ? (size_t)MBS * 16 : mbox_par_stride;
     __shared__ int abort_sh[2];
     __shared__ int abort_any;
     if (tid < 2) abort_sh[tid] = 0;
@@ -439,7 +467,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         const bool last_sweep = final_sweep || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
         Real* const Bcur = Bs + par * BPAR;
         Real* const Bcur2 = Bs2 + par * BPAR;
-        unsigned char* const mpar = mbox + par * mbox_par_stride;
+        unsigned char* const mpar = mbox + par * par_stride;     // (cluster exchange: only the offset part is used)
+        const unsigned cpar = (unsigned)(par * MBS * 16);
 
         // ================= phase A: segment local =================
         // operator rows and c0 of this lane: issued first, they arrive while the MMAs of a1 run
@@ -538,8 +567,13 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     for (int d = 0; d < 3; ++d) Bcur[own_off[h] + d] = Bnd[h][d];
                 }
                 if (pub[h]) {
+                    if (clus) {
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) ll_store(mpar + pub_off[h] + d * 16, (double)Bnd[h][d], seq);
+                        for (int d = 0; d < 3; ++d) ll_store_cluster(cm_remote[right[h] ? 1 : 0] + cpar + pub_off[h] + d * 16, (double)Bnd[h][d], seq);
+                    } else {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) ll_store(mpar + pub_off[h] + d * 16, (double)Bnd[h][d], seq);
+                    }
                 }
             }
         }
@@ -559,8 +593,13 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     for (int d = 0; d < 3; ++d) Bcur2[own2_off[h] + d] = Bnd2[h][d];
                 }
                 if (pub2[h]) {
+                    if (clus) {
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) ll_store(mpar + pub2_off[h] + d * 16, (double)Bnd2[h][d], seq);
+                        for (int d = 0; d < 3; ++d) ll_store_cluster(cm_remote[h] + cpar + pub2_off[h] + d * 16, (double)Bnd2[h][d], seq);
+                    } else {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) ll_store(mpar + pub2_off[h] + d * 16, (double)Bnd2[h][d], seq);
+                    }
                 }
             }
         }
@@ -568,11 +607,11 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         LLRaw rr[3], rr2[3];
         if (need) {
 #pragma unroll
-            for (int d = 0; d < 3; ++d) ll_issue(mpar + need_off + d * 16, rr[d]);
+            for (int d = 0; d < 3; ++d) { if (clus) ll_issue_smem(cm_local + cpar + need_off + d * 16, rr[d]); else ll_issue(mpar + need_off + d * 16, rr[d]); }
         }
         if (WIDE && need2) {
 #pragma unroll
-            for (int d = 0; d < 3; ++d) ll_issue(mpar + need2_off + d * 16, rr2[d]);
+            for (int d = 0; d < 3; ++d) { if (clus) ll_issue_smem(cm_local + cpar + need2_off + d * 16, rr2[d]); else ll_issue(mpar + need2_off + d * 16, rr2[d]); }
         }
         if (CONS) {
             // the three sample blocks of the evaluation back to back, then the projections of all blocks side by side:
@@ -672,12 +711,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 do {
                     if (!okk) {
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) ll_issue(mpar + need_off + d * 16, rr[d]);
+                        for (int d = 0; d < 3; ++d) { if (clus) ll_issue_smem(cm_local + cpar + need_off + d * 16, rr[d]); else ll_issue(mpar + need_off + d * 16, rr[d]); }
                         okk = ll_ok(rr[0], seq) && ll_ok(rr[1], seq) && ll_ok(rr[2], seq);
                     }
                     if (WIDE && !okk2) {
 #pragma unroll
-                        for (int d = 0; d < 3; ++d) ll_issue(mpar + need2_off + d * 16, rr2[d]);
+                        for (int d = 0; d < 3; ++d) { if (clus) ll_issue_smem(cm_local + cpar + need2_off + d * 16, rr2[d]); else ll_issue(mpar + need2_off + d * 16, rr2[d]); }
                         okk2 = ll_ok(rr2[0], seq) && ll_ok(rr2[1], seq) && ll_ok(rr2[2], seq);
                     }
                     bool bail = false;
@@ -886,6 +925,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         o[3] = sqrt(tot_sh[0]); o[4] = sqrt(tot_sh[1]); o[5] = sqrt(tot_sh[2]); o[6] = sqrt(tot_sh[3]);
     }
 
+    if (clus) cluster_barrier();      // nobody leaves while a neighbour may still store into its mailbox
     // ---- write iterate k + k_sweeps back
     if (owned) {
 #pragma unroll
@@ -908,15 +948,59 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     }
 }
 
-template <typename Real, int S, int CM, int MAXT>
-cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
-    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, true> : cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, false>;
+// one launch: a single CTA plainly; KF_CLUSTER: the whole grid as ONE thread-block cluster (<= 16 CTAs, co-scheduled by
+// the hardware); otherwise cooperatively (all CTAs co-resident: they wait for one another through the L2 mailbox)
+template <typename K>
+cudaError_t launch_any(K kern, const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     KParams pc = p;
     void* args[] = {&pc};
+    if (ctas > 1 && (p.flags & KF_CLUSTER)) {
+        if (ctas > 8 && (e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1)) != cudaSuccess) return e;
+        cudaLaunchConfig_t cfg;
+        memset(&cfg, 0, sizeof cfg);
+        cfg.gridDim = dim3(ctas); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)ctas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        return cudaLaunchKernelExC(&cfg, (const void*)kern, args);
+    }
     if (ctas > 1) return cudaLaunchCooperativeKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
     return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+}
+
+template <typename Real, int S, int CM, int MAXT>
+cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
+    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, true> : cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, false>;
+    return launch_any(kern, p, ctas, threads, smem, st);
+}
+
+// can `ctas` CTAs of this size run as ONE thread-block cluster?  *nclusters = co-resident clusters (0: no)
+template <typename K>
+cudaError_t cluster_query(K kern, int ctas, int threads, size_t smem, int* nclusters) {
+    *nclusters = 0;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    if (ctas > 8 && (e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1)) != cudaSuccess) return e;
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3(ctas); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = (unsigned)ctas; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaOccupancyMaxActiveClusters(nclusters, (const void*)kern, &cfg);
+}
+template <typename Real, int S, int CM, int MAXT>
+cudaError_t cluster_mma(int ctas, int threads, size_t smem, int* nclusters) {
+    int a = 0, b = 0;
+    cudaError_t e = cluster_query(cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, true>, ctas, threads, smem, &a);
+    if (e != cudaSuccess) return e;
+    e = cluster_query(cadmm_sweeps_mma_kernel<Real, S, CM, MAXT, false>, ctas, threads, smem, &b);
+    *nclusters = a < b ? a : b;
+    return e;
 }
 
 template <typename Real, int S, int CM, int MAXT>
@@ -931,12 +1015,7 @@ template <int S>
 cudaError_t launch_mma_wide(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
     auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_WIDE, true, false, true>
                                   : cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_WIDE, false, false, true>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    KParams pc = p;
-    void* args[] = {&pc};
-    if (ctas > 1) return cudaLaunchCooperativeKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
-    return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+    return launch_any(kern, p, ctas, threads, smem, st);
 }
 template <int S>
 cudaError_t limits_mma_wide(int threads, size_t smem, int* per_sm) {
@@ -949,12 +1028,7 @@ cudaError_t limits_mma_wide(int threads, size_t smem, int* per_sm) {
 template <int S>
 cudaError_t launch_mma_poly(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
     auto kern = cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_POLY, false, true>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    KParams pc = p;
-    void* args[] = {&pc};
-    if (ctas > 1) return cudaLaunchCooperativeKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
-    return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
+    return launch_any(kern, p, ctas, threads, smem, st);
 }
 template <int S>
 cudaError_t limits_mma_poly(int threads, size_t smem, int* per_sm) {
@@ -1006,6 +1080,29 @@ cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threa
     if (kflags & KF_POLY) return s == 3 ? limits_mma_poly<3>(threads, smem, max_ctas_per_sm) : limits_mma_poly<4>(threads, smem, max_ctas_per_sm);
     if (kflags & KF_WIDE) return s == 3 ? limits_mma_wide<3>(threads, smem, max_ctas_per_sm) : limits_mma_wide<4>(threads, smem, max_ctas_per_sm);
 #define CALL(R_, S_, C_, M_) return limits_mma<R_, S_, C_, M_>(threads, smem, max_ctas_per_sm);
+    TOP_DISPATCH_MMA(CALL)
+#undef CALL
+    return cudaErrorInvalidValue;
+}
+
+// 0 in *nclusters: the launch cannot run as one cluster (too many CTAs for a GPC at this shared-memory size): L2 mailbox then
+cudaError_t sweep_cluster_limits_mma(int dtype, int s, uint32_t kflags, int ctas, int threads, size_t smem, int* nclusters) {
+    *nclusters = 0;
+    if (ctas < 2 || ctas > 16) return cudaSuccess;
+    if (kflags & KF_POLY)
+        return s == 3 ? cluster_query(cadmm_sweeps_mma_kernel<double, 3, CM_RUNTIME, MAXT_MMA_POLY, false, true>, ctas, threads, smem, nclusters)
+                      : cluster_query(cadmm_sweeps_mma_kernel<double, 4, CM_RUNTIME, MAXT_MMA_POLY, false, true>, ctas, threads, smem, nclusters);
+    if (kflags & KF_WIDE) {
+        int a = 0, b = 0;
+        cudaError_t e = s == 3 ? cluster_query(cadmm_sweeps_mma_kernel<double, 3, CM_RUNTIME, MAXT_MMA_WIDE, true, false, true>, ctas, threads, smem, &a)
+                               : cluster_query(cadmm_sweeps_mma_kernel<double, 4, CM_RUNTIME, MAXT_MMA_WIDE, true, false, true>, ctas, threads, smem, &a);
+        if (e != cudaSuccess) return e;
+        e = s == 3 ? cluster_query(cadmm_sweeps_mma_kernel<double, 3, CM_RUNTIME, MAXT_MMA_WIDE, false, false, true>, ctas, threads, smem, &b)
+                   : cluster_query(cadmm_sweeps_mma_kernel<double, 4, CM_RUNTIME, MAXT_MMA_WIDE, false, false, true>, ctas, threads, smem, &b);
+        *nclusters = a < b ? a : b;
+        return e;
+    }
+#define CALL(R_, S_, C_, M_) return cluster_mma<R_, S_, C_, M_>(ctas, threads, smem, nclusters);
     TOP_DISPATCH_MMA(CALL)
 #undef CALL
     return cudaErrorInvalidValue;
