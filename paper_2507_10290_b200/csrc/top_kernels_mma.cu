@@ -39,6 +39,35 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
 }
 
+// A operand of one k-block of a contraction (the lane's two items x three dims), B operand (the two k-steps of the constant
+// matrix that go with them), and the accumulator tiles of one contraction output: value (dim d, column 2t + j).
+// TOP_F32 feeds fp32-rounded operands to the same fp64 tensor instructions (fp64 accumulation).  [Tried and dropped for
+// TOP_F32: mma.sync m16n8k8 tf32 with the 3-term split a_hi b_hi + a_lo b_hi + a_hi b_lo on the regular tensor pipe -- 8 cycles
+// per instruction and scheduler against 16 for DMMA, measured, and it frees the fp64 pipe; parity green, but config 5 ran at
+// 5.9e9 instead of 6.5e9 segment-iterations/s: that kernel is bound by shared-memory wavefronts (73 % of peak, ncu) and
+// issue slots, not by the fp64 pipe, and the split adds ~90 instructions per lane and sweep.]
+struct AOp { double v[2][3]; };
+struct BOp { double b0, b1; };
+template <typename Real>
+__device__ __forceinline__ AOp make_aop(const Real (&op)[2][3]) {
+    AOp a;
+#pragma unroll
+    for (int h = 0; h < 2; ++h)
+#pragma unroll
+        for (int d = 0; d < 3; ++d) a.v[h][d] = (double)op[h][d];
+    return a;
+}
+struct Acc {
+    double v[3][2] = {{0, 0}, {0, 0}, {0, 0}};
+    __device__ __forceinline__ void blk(const AOp& a, const BOp& b) {
+#pragma unroll
+        for (int d = 0; d < 3; ++d) dmma884(v[d][0], v[d][1], a.v[0][d], b.b0);
+#pragma unroll
+        for (int d = 0; d < 3; ++d) dmma884(v[d][0], v[d][1], a.v[1][d], b.b1);
+    }
+    __device__ __forceinline__ double get(int d, int j) const { return v[d][j]; }
+};
+
 // 1/sqrt(x) for x > 0, normal: the hardware seed (MUFU.RSQ64H, ~2^-22 relative) and ONE cubically convergent step
 // y (1 + e/2 + 3e^2/8), e = 1 - x y^2  =>  error ~ e^3: full double precision (a few ulp), 5 fp64 operations and no
 // branch.  The library rsqrt() adds special-case branches that keep ptxas from interleaving independent projections.
@@ -281,6 +310,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             }
         }
     }
+    // B operand of a k-block: entries i0 (k-step of the lane's first item) and i1 (second item) of the constant table
+    auto ldb = [&](int i0, int i1) {
+        BOp b;
+        b.b0 = ctab[i0 * 32]; b.b1 = ctab[i1 * 32];
+        return b;
+    };
     Real invTk[2];
 #pragma unroll
     for (int h = 0; h < 2; ++h) {
@@ -370,8 +405,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 
     // ---- state of iterate k.  Registers hold the a1 OPERANDS:
     //   gM = (z~ - u)/T^k      A0 = (hi - s+ - v+) + (lo + s- + v-)      gv = (phi_v - w_v)/T      ga = (phi_a - w_a)/T^2
-    double gM[2][3], A0[2][3], gv[2][3], ga[2][3];
-    double gM2[2][3] = {{0, 0, 0}, {0, 0, 0}};      // WIDE: operand of the second consensus block, (z~ - u)/T^k
+    Real gM[2][3], A0[2][3], gv[2][3], ga[2][3];
+    Real gM2[2][3] = {{0, 0, 0}, {0, 0, 0}};        // WIDE: operand of the second consensus block, (z~ - u)/T^k
     if (WIDE) {
 #pragma unroll
         for (int h = 0; h < 2; ++h)
@@ -380,7 +415,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 const long long i = d * stride + gt[h];
                 const Real z0 = static_cast<const Real*>(p.zt2)[i], u0 = static_cast<const Real*>(p.u2)[i];
                 zus2[(h * 3 + d) * TS] = make2(z0, u0);
-                gM2[h][d] = (double)((z0 - u0) * invTk2[h]);
+                gM2[h][d] = (z0 - u0) * invTk2[h];
             }
     }
 #pragma unroll
@@ -390,17 +425,17 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             const long long i = d * stride + gt[h];
             const Real z0 = static_cast<const Real*>(p.zt)[i], u0 = static_cast<const Real*>(p.u)[i];
             zus[(h * 3 + d) * TS] = make2(z0, u0);
-            gM[h][d] = (double)((z0 - u0) * invTk[h]);
-            A0[h][d] = gv[h][d] = ga[h][d] = 0.0;
+            gM[h][d] = (z0 - u0) * invTk[h];
+            A0[h][d] = gv[h][d] = ga[h][d] = 0;
             Real w_v = 0, w_a = 0, ph_v = 0, ph_a = 0;
             if (has_box) {
                 const Real lo = static_cast<const Real*>(p.lohi)[d * p.nseg_pad + gseg], hi = static_cast<const Real*>(p.lohi)[(3 + d) * p.nseg_pad + gseg];
                 const Real a = static_cast<const Real*>(p.qp)[i], b = static_cast<const Real*>(p.qn)[i];
                 qs[(h * 3 + d) * TS] = make2(a, b);
-                A0[h][d] = (double)((hi - fabs(a)) + (lo + fabs(b)));
+                A0[h][d] = (hi - fabs(a)) + (lo + fabs(b));
             }
-            if (has_vel) { w_v = static_cast<const Real*>(p.wv)[i]; ph_v = static_cast<const Real*>(p.phv)[i]; gv[h][d] = (double)((ph_v - w_v) * invT); }
-            if (has_acc) { w_a = static_cast<const Real*>(p.wa)[i]; ph_a = static_cast<const Real*>(p.pha)[i]; ga[h][d] = (double)((ph_a - w_a) * invT2); }
+            if (has_vel) { w_v = static_cast<const Real*>(p.wv)[i]; ph_v = static_cast<const Real*>(p.phv)[i]; gv[h][d] = (ph_v - w_v) * invT; }
+            if (has_acc) { w_a = static_cast<const Real*>(p.wa)[i]; ph_a = static_cast<const Real*>(p.pha)[i]; ga[h][d] = (ph_a - w_a) * invT2; }
             if (CONS) { ws[(h * 3 + d) * TS] = make2(w_v, w_a); phs[(h * 3 + d) * TS] = make2(ph_v, ph_a); }
         }
     if constexpr (POLY) {      // consensus rows enter the segment's rotated frame; the E0 operand is sum_k (b_k - s_k - v_k) a_k
@@ -488,37 +523,14 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         // R^ = M^'[(z~ - u)/T^k] + E0'[(hi - s+ - v+) + (lo + s- + v-)] + E1'[(phi_v - w_v)/T] + E2'[(phi_a - w_a)/T^2].
         // Three accumulator tiles (one per dim), up to 8 k-steps each; the accumulator of lane t holds rows 2t, 2t+1.
         {
-            double acc[3][2] = {{0, 0}, {0, 0}, {0, 0}};
+            Acc acc;
+            acc.blk(make_aop(gM), ldb(0, 1));
+            if (WIDE) acc.blk(make_aop(gM2), ldb(16, 17));
+            if (has_box || POLY) acc.blk(make_aop(A0), ldb(2, 3));      // Ao'(b - s - v): box Ao = [E0; -E0], b = [hi; -lo], s + v = |q| (Moreau pair); polytope: kron(E0, a_k')
+            if (has_vel) acc.blk(make_aop(gv), ldb(4, 5));
+            if (has_acc) acc.blk(make_aop(ga), ldb(6, 7));
 #pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-                for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gM[h][d], ctab[h * 32]);
-            if (WIDE) {
-#pragma unroll
-                for (int h = 0; h < 2; ++h)
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gM2[h][d], ctab[(16 + h) * 32]);
-            }
-            if (has_box || POLY) {      // Ao'(b - s - v): box Ao = [E0; -E0], b = [hi; -lo], s + v = |q| (Moreau pair); polytope: kron(E0, a_k')
-#pragma unroll
-                for (int h = 0; h < 2; ++h)
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], A0[h][d], ctab[(2 + h) * 32]);
-            }
-            if (has_vel) {
-#pragma unroll
-                for (int h = 0; h < 2; ++h)
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], gv[h][d], ctab[(4 + h) * 32]);
-            }
-            if (has_acc) {
-#pragma unroll
-                for (int h = 0; h < 2; ++h)
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) dmma884(acc[d][0], acc[d][1], ga[h][d], ctab[(6 + h) * 32]);
-            }
-#pragma unroll
-            for (int d = 0; d < 3; ++d) *reinterpret_cast<double2*>(Xs + d * 8 + 2 * lane) = make_double2(acc[d][0], acc[d][1]);
+            for (int d = 0; d < 3; ++d) *reinterpret_cast<double2*>(Xs + d * 8 + 2 * lane) = make_double2((double)acc.get(d, 0), (double)acc.get(d, 1));
         }
         __syncwarp();
         // a2: x-update  c^ = (rho Pm^) R^ + c0^   (Eq. 20a first bracket, precomputed per segment): rows lane, lane+4
@@ -548,14 +560,19 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         }
         // a3: evaluate the new polynomial: consensus rows of B = M c (Eq. 20b), and the lane's two samples of E0 c, E1 c,
         // E2 c (Eq. 20d-g).  A operand = the lane's own coefficient rows; accumulator columns = the lane's own items.
+        Real cf[2][3];
+#pragma unroll
+        for (int h = 0; h < 2; ++h)
+#pragma unroll
+            for (int d = 0; d < 3; ++d) cf[h][d] = (Real)cacc[h][d];
+        const AOp cop = make_aop(cf);
         {
             Real Bnd[2][3];
+            {
+                Acc e;
+                e.blk(cop, ldb(8, 12));
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                double e0 = 0, e1 = 0;
-                dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 0) * 32]);
-                dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 0) * 32]);
-                Bnd[0][d] = (Real)e0 * invTk[0]; Bnd[1][d] = (Real)e1 * invTk[1];
+                for (int d = 0; d < 3; ++d) { Bnd[0][d] = (Real)e.get(d, 0) * invTk[0]; Bnd[1][d] = (Real)e.get(d, 1) * invTk[1]; }
             }
             if constexpr (POLY) { rot_out(vs, Bnd[0]); rot_out(vs, Bnd[1]); }      // consensus lives in the global frame
             // publish: shared memory for the neighbours in this CTA (and for this lane's own phase B), mailbox for the
@@ -579,12 +596,11 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         }
         if (WIDE) {     // boundary derivatives of orders s..2s-2 (second block of B = M c)
             Real Bnd2[2][3];
+            {
+                Acc e;
+                e.blk(cop, ldb(18, 19));
 #pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                double e0 = 0, e1 = 0;
-                dmma884(e0, e1, cacc[0][d], ctab[18 * 32]);
-                dmma884(e0, e1, cacc[1][d], ctab[19 * 32]);
-                Bnd2[0][d] = (Real)e0 * invTk2[0]; Bnd2[1][d] = (Real)e1 * invTk2[1];
+                for (int d = 0; d < 3; ++d) { Bnd2[0][d] = (Real)e.get(d, 0) * invTk2[0]; Bnd2[1][d] = (Real)e.get(d, 1) * invTk2[1]; }
             }
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
@@ -617,17 +633,21 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
             // the three sample blocks of the evaluation back to back, then the projections of all blocks side by side:
             // independent dependency chains, no branch between them
             Real Pv[2][3], Vv[2][3], Av[2][3];
+            Acc ev, ea, ep;
+            if (has_vel) ev.blk(cop, ldb(10, 14));
+            if (has_acc) ea.blk(cop, ldb(11, 15));
+            if (has_box || POLY) ep.blk(cop, ldb(9, 13));
             if (has_vel) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 2) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 2) * 32]); Vv[0][d] = (Real)e0; Vv[1][d] = (Real)e1; }
+                for (int d = 0; d < 3; ++d) { Vv[0][d] = (Real)ev.get(d, 0); Vv[1][d] = (Real)ev.get(d, 1); }
             }
             if (has_acc) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 3) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 3) * 32]); Av[0][d] = (Real)e0; Av[1][d] = (Real)e1; }
+                for (int d = 0; d < 3; ++d) { Av[0][d] = (Real)ea.get(d, 0); Av[1][d] = (Real)ea.get(d, 1); }
             }
             if (has_box || POLY) {
 #pragma unroll
-                for (int d = 0; d < 3; ++d) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0][d], ctab[(8 + 0 * 4 + 1) * 32]); dmma884(e0, e1, cacc[1][d], ctab[(8 + 1 * 4 + 1) * 32]); Pv[0][d] = (Real)e0; Pv[1][d] = (Real)e1; }
+                for (int d = 0; d < 3; ++d) { Pv[0][d] = (Real)ep.get(d, 0); Pv[1][d] = (Real)ep.get(d, 1); }
             }
             R2 w2[2][3], q2[2][3];
 #pragma unroll
@@ -647,7 +667,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     for (int d = 0; d < 3; ++d) y[d] = Vv[h][d] * invT + w2[h][d].x;
                     const Real scale = ball_scale(y, vmax);
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) { const Real ph = scale * y[d]; ph2[h][d].x = ph; w2[h][d].x = y[d] - ph; gv[h][d] = (double)((ph - w2[h][d].x) * invT); }
+                    for (int d = 0; d < 3; ++d) { const Real ph = scale * y[d]; ph2[h][d].x = ph; w2[h][d].x = y[d] - ph; gv[h][d] = ((ph - w2[h][d].x) * invT); }
                 } else {
 #pragma unroll
                     for (int d = 0; d < 3; ++d) ph2[h][d].x = 0;
@@ -658,7 +678,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     for (int d = 0; d < 3; ++d) y[d] = Av[h][d] * invT2 + w2[h][d].y;
                     const Real scale = ball_scale(y, amax);
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) { const Real ph = scale * y[d]; ph2[h][d].y = ph; w2[h][d].y = y[d] - ph; ga[h][d] = (double)((ph - w2[h][d].y) * invT2); }
+                    for (int d = 0; d < 3; ++d) { const Real ph = scale * y[d]; ph2[h][d].y = ph; w2[h][d].y = y[d] - ph; ga[h][d] = ((ph - w2[h][d].y) * invT2); }
                 } else {
 #pragma unroll
                     for (int d = 0; d < 3; ++d) ph2[h][d].y = 0;
@@ -668,7 +688,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
                 for (int h = 0; h < 2; ++h)
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) { ws[(h * 3 + d) * TS] = w2[h][d]; phs[(h * 3 + d) * TS] = ph2[h][d]; }
+                    for (int d = 0; d < 3; ++d) {
+                        ws[(h * 3 + d) * TS] = w2[h][d];
+                        // phi itself is only read back at the end of the launch and by the rho change of a test sweep (its
+                        // effect on the next sweep is already in the operands gv, ga)
+                        if (last_sweep) phs[(h * 3 + d) * TS] = ph2[h][d];
+                    }
             }
             if constexpr (POLY) {         // a7 + a8 per (sample, plane): q = -(a_k'p - b_k + v);  next operand sum_k (b_k - |q_k|) a_k
 #pragma unroll
@@ -693,7 +718,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     for (int h = 0; h < 2; ++h) {
                         const Real qpn = (hi - Pv[h][d]) - neg_part(q2[h][d].x), qnn = (Pv[h][d] - lo) - neg_part(q2[h][d].y);
                         qs[(h * 3 + d) * TS] = make2(qpn, qnn);
-                        A0[h][d] = (double)((hi - fabs(qpn)) + (lo + fabs(qnn)));
+                        A0[h][d] = ((hi - fabs(qpn)) + (lo + fabs(qnn)));
                     }
                 }
             }
@@ -774,7 +799,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 const Real res = isrow[h] ? own[h][d] - znew : (Real)0;
                 const Real unew = zu[h][d].y + res;                               // a8: Eq. 6c / 20c (scaled dual, A5)
                 zus[(h * 3 + d) * TS] = make2(znew, unew);
-                gM[h][d] = (double)((znew - unew) * invTk[h]);                                // operand of the next sweep's a1
+                gM[h][d] = ((znew - unew) * invTk[h]);                                // operand of the next sweep's a1
                 if (last_sweep) {
                     rp2 += (double)res * (double)res;
                     if (gaprow[h]) { const double gp = (double)own[h][d] - (double)nb[h][d]; gap2 += gp * gp; }   // Eq. 21
@@ -797,7 +822,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     const Real res = (isrow2 && !fixed2[h]) ? own2 - znew : (Real)0;    // rows at the trajectory ends do not exist (A1)
                     const Real unew = zu2.y + res;                                      // a8: Eq. 6c / 20c
                     zus2[(h * 3 + d) * TS] = make2(znew, unew);
-                    gM2[h][d] = (double)((znew - unew) * invTk2[h]);
+                    gM2[h][d] = ((znew - unew) * invTk2[h]);
                     if (last_sweep) {
                         rp2 += (double)res * (double)res;
                         if (gaprow2[h]) { const double gp = (double)own2 - (double)nb2; gap2 += gp * gp; }   // Eq. 21
@@ -887,12 +912,12 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                                 R2 zz = zus[(h * 3 + d) * TS];
                                 zz.y *= ratio;
                                 zus[(h * 3 + d) * TS] = zz;
-                                gM[h][d] = (double)((zz.x - zz.y) * invTk[h]);
+                                gM[h][d] = ((zz.x - zz.y) * invTk[h]);
                                 if (WIDE) {
                                     R2 z2 = zus2[(h * 3 + d) * TS];
                                     z2.y *= ratio;
                                     zus2[(h * 3 + d) * TS] = z2;
-                                    gM2[h][d] = (double)((z2.x - z2.y) * invTk2[h]);
+                                    gM2[h][d] = ((z2.x - z2.y) * invTk2[h]);
                                 }
                                 if (has_box) {
                                     const Real lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
@@ -900,15 +925,15 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                                     if (q.x < 0) q.x *= ratio;
                                     if (q.y < 0) q.y *= ratio;
                                     qs[(h * 3 + d) * TS] = q;
-                                    A0[h][d] = (double)((hi - fabs(q.x)) + (lo + fabs(q.y)));
+                                    A0[h][d] = ((hi - fabs(q.x)) + (lo + fabs(q.y)));
                                 }
                                 if (has_vel || has_acc) {
                                     R2 w2 = ws[(h * 3 + d) * TS];
                                     const R2 ph = phs[(h * 3 + d) * TS];
                                     w2.x *= ratio; w2.y *= ratio;
                                     ws[(h * 3 + d) * TS] = w2;
-                                    if (has_vel) gv[h][d] = (double)((ph.x - w2.x) * invT);
-                                    if (has_acc) ga[h][d] = (double)((ph.y - w2.y) * invT2);
+                                    if (has_vel) gv[h][d] = ((ph.x - w2.x) * invT);
+                                    if (has_acc) ga[h][d] = ((ph.y - w2.y) * invT2);
                                 }
                             }
                             refresh_operator_rows<N2, TS>(p, gseg, gt[h], jj[h], rho_new, Pms + h * 4 * TS, c0s + h * 3 * TS);
