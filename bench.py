@@ -443,7 +443,7 @@ def main():
                     e2e_t += time.perf_counter() - t0
             out["e2e"] = {"value": float(w.batch * w.N) * sweeps * nrep / e2e_t, "unit": UNIT,
                           "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "ms_per_step": 1e3 * e2e_t / nrep,
-                          "what": "top_create(host arrays: validate, fp80 operator precompute, one H2D copy, init kernel) + top_iterate(%d) + top_get_coeffs(host) + top_destroy, wall clock" % sweeps}
+                          "what": "top_create(host arrays: validate, one H2D copy, operator precompute kernel (double-double), init kernel) + top_iterate(%d) + top_get_coeffs(host) + top_destroy, wall clock" % sweeps}
             # the re-planning form of the same thing: top_reset on a live handle instead of create / destroy
             s2 = top.from_workload(w, device=local_rank, stream=stream.cuda_stream, sync=args.sync,
                                    segs_per_cta=args.segs_per_cta, lanes=args.lanes)

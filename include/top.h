@@ -130,11 +130,13 @@ typedef struct {
 } top_options;
 
 /*
- * top_create -- Init of Alg. 1 (PAPER.md:L270 line 1, L301): validates, precomputes per segment (host,
- * extended precision) the x-update operator of Eq. 20a from T_i, rho and the enabled constraint sets,
- * uploads it (one device allocation, one host-to-device copy of the operator rows and of the caller's arrays as they
- * are), and an init kernel derives every per-lane constant and iterate 0 (reading A9: chord at constant speed, z0 from
- * the chord, duals 0, slacks/phi = projections of the chord samples).  The device work is asynchronous.
+ * top_create -- Init of Alg. 1 (PAPER.md:L270 line 1, L301): validates, uploads the caller's arrays as they are (one
+ * device allocation, one host-to-device copy), precomputes per segment the x-update operator of Eq. 20a from T_i, rho and the
+ * enabled constraint sets in a kernel (double-double arithmetic; with a polytope corridor: on the host in extended precision,
+ * three operators per segment), and an init kernel derives every per-lane constant and iterate 0 (reading A9: chord at
+ * constant speed, z0 from the chord, duals 0, slacks/phi = projections of the chord samples).  The device work is
+ * asynchronous; an operator that is not positive definite (extreme durations / rho) is reported as TOP_E_INVALID by the next
+ * call that synchronises.
  *   batch        number of independent trajectories (>= 1), each with N segments
  *   N            segments per trajectory (>= 1);  s in {3,4};  dims in {1,2,3}
  *   waypoints    host [batch][N+1][dims] metres       (the path P of Alg. 1)

@@ -73,6 +73,7 @@ struct top_solver {
     unsigned char* arena = nullptr;
     size_t arena_bytes = 0;
     unsigned char* d_upload = nullptr;     // region that mirrors the host staging buffer: [rho Pm^ rows | the caller's arrays]
+    size_t off_gram = 0;                   // double-double Gram tables for the device-side operator precompute (first byte of what is uploaded then)
     size_t upload_bytes = 0, off_wp = 0, off_T = 0, off_lo = 0, off_hi = 0, off_sd = 0, off_ed = 0;
     bool have_sd = false, have_ed = false;
     unsigned char* zero_begin = nullptr;   // arrays that top_reset sets to zero again (duals, partial sums)
@@ -621,13 +622,34 @@ top_status fill_problem(top_solver* h, const double* waypoints, const double* du
     const GramTables& G = gram_tables(s);
     if (pt) pt->mark("staging copies");
 
-    {
+    if (h->has_poly) {       // three operators per segment in a rotated frame: host precompute (stage_operators)
         top_status so = stage_operators(h);
         if (pt) pt->mark("host precompute");
         if (so != TOP_OK) return so;
+        CU(cudaMemcpyAsync(h->d_upload, S, h->upload_bytes, cudaMemcpyHostToDevice, h->stream), "H2D problem data");
+    } else {
+        // the operator is computed on the device (precompute_operator_kernel, double-double): what goes up is the caller's
+        // arrays and 14 KB of Gram tables -- not 8 operator rows per lane
+        GramDD* gd = reinterpret_cast<GramDD*>(S + h->off_gram);
+        const xreal* tabs[GRAM_TABLES] = {G.Q1, G.Gc[0], G.Gc[1], G.Gc[2], G.Gc[3], G.Ge[0], G.Ge[1], G.Ge[2],
+                                          G.Gw[0][0], G.Gw[0][1], G.Gw[0][2], G.Gw[1][0], G.Gw[1][1], G.Gw[1][2]};
+        for (int t = 0; t < GRAM_TABLES; ++t)
+            for (int i = 0; i < MAXN * MAXN; ++i) {
+                const double hi = (double)tabs[t][i];
+                gd->hi[t][i] = hi; gd->lo[t][i] = (double)(tabs[t][i] - (xreal)hi);
+            }
+        CU(cudaMemcpyAsync(h->d_upload + h->off_gram, S + h->off_gram, h->upload_bytes - h->off_gram, cudaMemcpyHostToDevice, h->stream), "H2D problem data");
+        PrecompParams pp;
+        std::memset(&pp, 0, sizeof pp);
+        pp.gram = reinterpret_cast<const GramDD*>(h->d_upload + h->off_gram);
+        pp.durations = reinterpret_cast<const double*>(h->d_upload + h->off_T);
+        pp.Pm = h->d_Pm; pp.stride = h->stride; pp.nseg = h->nseg; pp.N = h->N; pp.s = h->s;
+        pp.hard = h->wp_mode == TOP_WAYPOINT_HARD; pp.box = h->has_box; pp.vel = h->has_vel; pp.acc = h->has_acc; pp.wide = h->wide;
+        pp.rho = h->rho; pp.bad = h->d_abort + 1;
+        CU(launch_precompute_operator(pp, h->stream), "operator precompute launch");
+        h->launches += 1;
+        if (pt) pt->mark("operator kernel launch");
     }
-
-    CU(cudaMemcpyAsync(h->d_upload, S, h->upload_bytes, cudaMemcpyHostToDevice, h->stream), "H2D problem data");
     InitParams ip;
     std::memset(&ip, 0, sizeof ip);
     fill_init_params(h, ip);
@@ -937,6 +959,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->off_rot = cv.take(h->has_poly ? 9 * NP * 8 : 0);
     h->off_planes = cv.take(h->has_poly ? (size_t)h->K * 4 * NP * 8 : 0);
     h->off_lam3 = cv.take(h->has_poly ? 3 * NP * 8 : 0);
+    h->off_gram = cv.take(h->has_poly ? 0 : sizeof(GramDD));
     h->off_wp = cv.take((size_t)batch * (N + 1) * dims * 8);
     h->off_T = cv.take((size_t)nseg * 8);
     h->off_lo = cv.take(has_box ? (size_t)nseg * dims * 8 : 0);
@@ -997,7 +1020,8 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->d_Bedge = A + o_Bedge; h->d_resbox = A + o_resbox; h->d_sync = A + o_sync; h->d_abort = (int*)(A + o_abort);
     h->stage.reset(new (std::nothrow) unsigned char[h->upload_bytes]);
     if (!h->stage) CREATE_FAIL(fail(h, TOP_E_NOMEM, "host allocation failed"));
-    std::memset(h->stage.get(), 0, h->off_wp);             // padded operator rows (and rotation / plane tables) stay zero
+    if (h->has_poly) std::memset(h->stage.get(), 0, h->off_wp);      // padded operator rows (and rotation / plane tables) stay zero
+    // (without a polytope corridor the operator rows are computed on the device and that part of the buffer is never touched)
     h->h_res.assign((size_t)batch * 4, std::numeric_limits<double>::quiet_NaN());
     pt.mark("memory (1 cudaMalloc)");
 
@@ -1048,7 +1072,7 @@ extern "C" TOP_API top_status top_reset(top_solver* h, const double* waypoints, 
         h->rho = rho;
         h->vmax = hv ? cons->vmax : 0; h->amax = ha ? cons->amax : 0;
         CU(cudaMemsetAsync(h->zero_begin, 0, h->zero_bytes, h->stream), "cudaMemsetAsync");
-        CU(cudaMemsetAsync(h->d_abort, 0, sizeof(int), h->stream), "cudaMemsetAsync");
+        CU(cudaMemsetAsync(h->d_abort, 0, 2 * sizeof(int), h->stream), "cudaMemsetAsync");
         st = fill_problem(h, waypoints, durations, start_derivs, end_derivs, cons, &pt);
         if (st != TOP_OK) return st;
         if (h->opt_flags & TOP_RHO_ADAPTIVE) st = ensure_spectral(h);
@@ -1061,8 +1085,9 @@ extern "C" TOP_API top_status top_reset(top_solver* h, const double* waypoints, 
 namespace {
 
 top_status check_abort(top_solver* h) {
-    CU(cudaMemcpyAsync(h->h_abort, h->d_abort, sizeof(int), cudaMemcpyDeviceToHost, h->stream), "D2H abort flag");
+    CU(cudaMemcpyAsync(h->h_abort, h->d_abort, 2 * sizeof(int), cudaMemcpyDeviceToHost, h->stream), "D2H abort flag");
     CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+    if (h->h_abort[1]) return fail(h, TOP_E_INVALID, "x-update operator is not positive definite (check durations / rho)");
     if (h->h_abort[0]) return fail(h, TOP_E_CUDA, "inter-CTA barrier timed out inside the sweep kernel");
     return TOP_OK;
 }
@@ -1483,7 +1508,7 @@ extern "C" TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas
 extern "C" TOP_API top_status top_memory_info(const top_solver* h, int64_t* device_bytes, int64_t* h2d_bytes_per_problem) {
     if (!h) return TOP_E_INVALID;
     if (device_bytes) *device_bytes = (int64_t)h->arena_bytes;
-    if (h2d_bytes_per_problem) *h2d_bytes_per_problem = (int64_t)h->upload_bytes;
+    if (h2d_bytes_per_problem) *h2d_bytes_per_problem = (int64_t)(h->has_poly ? h->upload_bytes : h->upload_bytes - h->off_gram);
     return TOP_OK;
 }
 

@@ -127,6 +127,22 @@ struct RefreshParams {
     double rho;
 };
 cudaError_t launch_refresh_operator(const RefreshParams& p, cudaStream_t st);
+// The x-update operator of Eq. 20a (first bracket) on the device, one thread per segment, in double-double
+// arithmetic (106-bit significand: the host path uses the 64-bit significand of long double): H^ from the Gram tables
+// of the constant normalised-time rows weighted by powers of 1/T_i, the waypoint equalities eliminated with the null-space
+// basis (HARD), symmetric scaling by powers of two, Gauss-Jordan, rho * Pm^ rounded to fp64 into the per-lane layout.
+constexpr int GRAM_TABLES = 14;      // Q1 | Gc[0..3] | Ge[0..2] | Gw[start][0..2] | Gw[end][0..2]
+struct GramDD { double hi[GRAM_TABLES][MAXN * MAXN], lo[GRAM_TABLES][MAXN * MAXN]; };
+struct PrecompParams {
+    const GramDD* gram;           // device
+    const double* durations;      // [nseg] (device copy of the caller's array)
+    double* Pm;                   // out [MAXN b][stride]: element b of row `lane` of rho * Pm^
+    long long stride, nseg;
+    int N, s, hard, box, vel, acc, wide;
+    double rho;
+    int* bad;                     // set to 1 when a segment's operator is not positive definite
+};
+cudaError_t launch_precompute_operator(const PrecompParams& p, cudaStream_t st);
 // Init of Alg. 1 (PAPER.md:L270 line 1, L301; reading A9) on the device: from the caller's arrays (uploaded as they are)
 // and the per-segment operator rows, every per-lane constant and iterate 0.
 struct InitParams {

@@ -1024,6 +1024,121 @@ __global__ void refresh_operator_kernel(const RefreshParams p) {
     }
 }
 
+// ---- double-double arithmetic (error-free transformations; Dekker / Knuth with FMA) for the one-off operator precompute
+struct dd { double hi, lo; };
+__device__ __forceinline__ dd dd_quick(double a, double b) { const double s = a + b; return {s, b - (s - a)}; }
+__device__ __forceinline__ dd dd_two_sum(double a, double b) { const double s = a + b, bb = s - a; return {s, (a - (s - bb)) + (b - bb)}; }
+__device__ __forceinline__ dd dd_add(dd a, dd b) {
+    dd s = dd_two_sum(a.hi, b.hi);
+    const dd t = dd_two_sum(a.lo, b.lo);
+    s.lo += t.hi;
+    s = dd_quick(s.hi, s.lo);
+    s.lo += t.lo;
+    return dd_quick(s.hi, s.lo);
+}
+__device__ __forceinline__ dd dd_neg(dd a) { return {-a.hi, -a.lo}; }
+__device__ __forceinline__ dd dd_mul(dd a, dd b) {
+    const double p = a.hi * b.hi;
+    double e = fma(a.hi, b.hi, -p);
+    e = fma(a.hi, b.lo, e);
+    e = fma(a.lo, b.hi, e);
+    return dd_quick(p, e);
+}
+__device__ __forceinline__ dd dd_muld(dd a, double b) {
+    const double p = a.hi * b;
+    double e = fma(a.hi, b, -p);
+    e = fma(a.lo, b, e);
+    return dd_quick(p, e);
+}
+__device__ __forceinline__ dd dd_div(dd a, dd b) {
+    const double q1 = a.hi / b.hi;
+    dd r = dd_add(a, dd_neg(dd_muld(b, q1)));
+    const double q2 = r.hi / b.hi;
+    r = dd_add(r, dd_neg(dd_muld(b, q2)));
+    const double q3 = r.hi / b.hi;
+    return dd_add(dd_quick(q1, q2), dd{q3, 0.0});
+}
+
+// rho * Pm^ of every segment (see PrecompParams).  H^ = 2 T^(1-2s) Q(1) + rho [ sum_k T^-2k Gc_k + 2 Ge_0 + T^-2 Ge_1 + T^-4 Ge_2 ]
+// (+ the consensus rows of orders s..2s-2 that exist, wide consensus); HARD: Pm^ = Z (Z'H^Z)^-1 Z' with Z = {e_a - e_1, a >= 2}.
+__global__ void precompute_operator_kernel(const PrecompParams p) {
+    const long long g = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= p.nseg) return;
+    const int s = p.s, n = 2 * s;
+    const GramDD& G = *p.gram;
+    auto tab = [&](int t, int i) -> dd { return dd{G.hi[t][i], G.lo[t][i]}; };
+    const double T = p.durations[g];
+    dd iT[14];
+    iT[0] = dd{1.0, 0.0};
+    for (int k = 1; k < 14; ++k) iT[k] = dd_div(iT[k - 1], dd{T, 0.0});
+    const dd wq = dd_muld(dd_mul(dd_muld(iT[2 * s - 1], T), iT[1]), 2.0);      // 2 T^(1-2s)
+    const long long i_in = g % p.N;
+    const int wmask = p.wide ? ((i_in != 0 ? 1 : 0) | (i_in != p.N - 1 ? 2 : 0)) : 0;
+    dd H[MAXN * MAXN];
+    for (int a = 0; a < n; ++a)
+        for (int b = 0; b < n; ++b) {
+            const int i = a * MAXN + b;
+            dd v = dd_mul(wq, tab(0, i));
+            for (int k = 0; k < s; ++k) v = dd_add(v, dd_muld(dd_mul(iT[2 * k], tab(1 + k, i)), p.rho));
+            if (p.box) v = dd_add(v, dd_muld(tab(5, i), 2.0 * p.rho));
+            if (p.vel) v = dd_add(v, dd_muld(dd_mul(iT[2], tab(6, i)), p.rho));
+            if (p.acc) v = dd_add(v, dd_muld(dd_mul(iT[4], tab(7, i)), p.rho));
+            for (int side = 0; side < 2; ++side)
+                if (wmask & (1 << side))
+                    for (int j = 0; j <= s - 2; ++j) v = dd_add(v, dd_muld(dd_mul(iT[2 * (s + j)], tab(8 + side * 3 + j, i)), p.rho));
+            H[a * MAXN + b] = v;
+        }
+    // reduced matrix A (q x q) and its inverse by Gauss-Jordan on [A | I] after a symmetric power-of-two scaling
+    const int q = p.hard ? n - 2 : n;
+    dd W[MAXN][2 * MAXN];
+    double sc[MAXN];
+    bool ok = true;
+    for (int i = 0; i < q; ++i)
+        for (int j = 0; j < q; ++j) {
+            dd v;
+            if (p.hard) {
+                const int a = i + 2, b = j + 2;
+                v = dd_add(dd_add(H[a * MAXN + b], dd_neg(H[a * MAXN + 1])), dd_add(H[1 * MAXN + 1], dd_neg(H[1 * MAXN + b])));
+            } else v = H[i * MAXN + j];
+            W[i][j] = v;
+        }
+    for (int i = 0; i < q; ++i) {
+        if (!(W[i][i].hi > 0)) { ok = false; sc[i] = 1.0; continue; }
+        int e;
+        frexp(W[i][i].hi, &e);
+        sc[i] = ldexp(1.0, -(e / 2));
+    }
+    for (int i = 0; i < q; ++i)
+        for (int j = 0; j < q; ++j) { W[i][j] = dd_muld(W[i][j], sc[i] * sc[j]); W[i][q + j] = dd{i == j ? 1.0 : 0.0, 0.0}; }
+    for (int c = 0; c < q && ok; ++c) {
+        const dd piv = W[c][c];
+        if (!(piv.hi > 0)) { ok = false; break; }
+        for (int j = 0; j < 2 * q; ++j) W[c][j] = dd_div(W[c][j], piv);
+        for (int r = 0; r < q; ++r) {
+            if (r == c) continue;
+            const dd f = W[r][c];
+            if (f.hi == 0.0 && f.lo == 0.0) continue;
+            for (int j = 0; j < 2 * q; ++j) W[r][j] = dd_add(W[r][j], dd_neg(dd_mul(f, W[c][j])));
+        }
+    }
+    if (!ok) { atomicExch(p.bad, 1); return; }
+    // A^-1 (symmetrised), back to Pm^ = Z A^-1 Z' (HARD) and out as rho * Pm^
+    dd Pm[MAXN * MAXN];
+    for (int i = 0; i < MAXN * MAXN; ++i) Pm[i] = dd{0.0, 0.0};
+    for (int i = 0; i < q; ++i)
+        for (int j = 0; j < q; ++j) {
+            dd v = dd_muld(dd_add(dd_muld(W[i][q + j], sc[i] * sc[j]), dd_muld(W[j][q + i], sc[i] * sc[j])), 0.5);
+            if (p.hard) {
+                Pm[(i + 2) * MAXN + (j + 2)] = dd_add(Pm[(i + 2) * MAXN + (j + 2)], v);
+                Pm[1 * MAXN + (j + 2)] = dd_add(Pm[1 * MAXN + (j + 2)], dd_neg(v));
+                Pm[(i + 2) * MAXN + 1] = dd_add(Pm[(i + 2) * MAXN + 1], dd_neg(v));
+                Pm[1 * MAXN + 1] = dd_add(Pm[1 * MAXN + 1], v);
+            } else Pm[i * MAXN + j] = v;
+        }
+    for (int lane = 0; lane < n; ++lane)
+        for (int b = 0; b < n; ++b) p.Pm[(long long)b * p.stride + g * LANES + lane] = dd_muld(Pm[lane * MAXN + b], p.rho).hi;
+}
+
 // Init of Alg. 1 (PAPER.md:L270 line 1; reading A9), one thread per (segment, lane): the per-lane constants of the sweep
 // (powers of T, segment-local frame, box in the local frame, c0^ from the operator rows) and iterate 0: C0 = chord at
 // constant speed, z0_j = (p_j, mean of the adjacent chord velocities, 0..), z_0 and z_N = the given end states
@@ -1329,6 +1444,12 @@ cudaError_t launch_refresh_operator(const RefreshParams& p, cudaStream_t st) {
     const long long n = p.nseg * LANES;
     if (n == 0) return cudaSuccess;
     refresh_operator_kernel<<<(int)((n + 127) / 128), 128, 0, st>>>(p);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_precompute_operator(const PrecompParams& p, cudaStream_t st) {
+    if (p.nseg == 0) return cudaSuccess;
+    precompute_operator_kernel<<<(int)((p.nseg + 63) / 64), 64, 0, st>>>(p);
     return cudaGetLastError();
 }
 
