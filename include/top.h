@@ -81,9 +81,10 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
  * check_every sweeps; the paper: every sweep) rho <- tau_incr*rho if r_p > mu*r_d, rho <- rho/tau_decr if
  * r_d > mu*r_p.  The change goes through top_set_rho. */
 #define TOP_RHO_ADAPTIVE      64u
-/* Kernel selection (a tuning knob; results agree to rounding): with 4 lanes per segment the fp64 sweep runs its two
- * constant-matrix contractions (Eq. 20a second bracket; evaluation of Eq. 20b, 20d-g) on the tensor cores
- * (mma.sync m8n8k4 f64).  This flag keeps the shuffle / synthetic-division form of the 4-lane kernel instead. */
+/* Kernel selection.  With 4 lanes per segment the sweep runs its two constant-matrix contractions (Eq. 20a second
+ * bracket; evaluation of Eq. 20b, 20d-g) on the tensor cores (mma.sync m8n8k4 f64); with 8 lanes per segment
+ * (lanes_per_segment = 8) it uses warp shuffles and synthetic division, no tensor cores.  The shuffle form of the 4-lane
+ * kernel that this flag used to select was removed: together with 4 lanes it now returns TOP_E_UNSUPPORTED. */
 #define TOP_KERNEL_NO_MMA     128u
 /* Consensus width (reading A1 of DESIGN.md).  Default: every junction carries the derivative orders 0..s-1 (M is 2s x 2s).
  * TOP_CONSENSUS_WIDE: the paper's literal choice (M(t) stacks beta^0..beta^(d-1) with d = 2p-1; L257: each

@@ -877,7 +877,9 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
             plan_segs = (int)std::max<long long>(per_cta_min, round_up((int)((nseg + 15) / 16), 8));
         }
     }
-    h->mma = h->lanes == 4 && !(o.flags & TOP_KERNEL_NO_MMA);
+    if (h->lanes == 4 && (o.flags & TOP_KERNEL_NO_MMA))
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_KERNEL_NO_MMA: the shuffle form of the 4-lane kernel was removed (use lanes_per_segment = 8 for a kernel without tensor-core contractions)"));
+    h->mma = h->lanes == 4;
     if (h->wide && (!(h->mma && dtype == TOP_F64) || h->has_poly))
         CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_CONSENSUS_WIDE runs on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA, no polytope corridor)"));
     if (h->has_poly && !(h->mma && dtype == TOP_F64))

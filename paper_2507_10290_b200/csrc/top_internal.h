@@ -101,7 +101,7 @@ struct ConvParams {       // coefficient conversion to the paper's basis (Eq. 18
 };
 
 // launchers (top_kernels.cu).  dtype: 0 = f64, 1 = f32.  Return cudaError_t.
-// `lanes` = threads per segment of the sweep kernel: 8 (cadmm_sweeps_kernel) or 4 (cadmm_sweeps_kernel4)
+// 8 lanes per segment (cadmm_sweeps_kernel); the 4-lane kernel is cadmm_sweeps_mma_kernel below
 cudaError_t launch_sweeps(const KParams& p, int dtype, int s, bool constrained, int lanes, int ctas, int threads,
                           size_t smem, cudaStream_t st);
 size_t sweep_smem_bytes(int dtype, int s, bool constrained, int lanes, int segs_per_cta);

@@ -513,443 +513,6 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel(const KParams p) 
 
 }  // namespace
 
-// ------------------------------------------------------------------------------------------------ 4-lane variant
-//
-// Same sweep, same global-memory layout, same exchange protocol as cadmm_sweeps_kernel, but FOUR lanes per segment:
-// lane l owns samples {l, l+4} and coefficient / consensus rows {l, l+4}.  Half the threads per segment means twice
-// the registers per thread (17 warps x 96 registers -> 9 warps x up to 224: the fp64 state fits without spills) and two
-// independent samples / rows per lane for instruction-level parallelism; the reduce-scatter needs two shuffle
-// stages (4 + 2) instead of three.
-
-namespace {
-
-__host__ __device__ inline SmemLayout smem_layout4(int real_bytes, int S, bool cons, int segs_alloc) {
-    SmemLayout L;
-    const int CSTRIDE = real_bytes == 8 ? 26 : 28;
-    const int T = segs_alloc * 4;
-    size_t off = 0;
-    L.pm = off;   off = align16(off + (size_t)2 * 2 * S * T * sizeof(double));          // rho*Pm^ rows, [h][b][thread]
-    L.bco = off;  off = align16(off + (size_t)8 * 8 * real_bytes);                      // consensus-row coefficients [a][row]
-    L.lohi = off; off = align16(off + (size_t)(cons ? 6 : 0) * segs_alloc * real_bytes);
-    L.xs = off;   off = align16(off + (size_t)segs_alloc * XSTRIDE * sizeof(double));
-    L.cs = off;   off = align16(off + (size_t)segs_alloc * CSTRIDE * real_bytes);
-    L.bs = off;   off = align16(off + (size_t)2 * (segs_alloc + 2) * 24 * real_bytes);
-    L.zoff = off;
-    L.total = off;
-    return L;
-}
-
-// Reduce-scatter of v[0..7] over the 4 lanes of a segment: afterwards lane l holds rows l (out0) and l+4 (out1).
-template <typename Real>
-__device__ __forceinline__ void reduce_scatter4(const Real (&v)[8], int lane, Real& out0, Real& out1) {
-    const bool b1 = lane & 2, b0 = lane & 1;
-    Real w[4];
-    // stage 1 (partner lane^2): keep the rows whose bit 1 equals mine
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
-        const int lo = (i & 1) + 4 * (i >> 1), hi = lo + 2;          // row pairs (0,2) (1,3) (4,6) (5,7)
-        const Real send = sel(b1, v[lo], v[hi]), keep = sel(b1, v[hi], v[lo]);
-        w[i] = keep + shfl_xor(send, 2);
-    }
-    // stage 2 (partner lane^1): keep the rows whose bit 0 equals mine
-    {
-        const Real send = sel(b0, w[0], w[1]), keep = sel(b0, w[1], w[0]);
-        out0 = keep + shfl_xor(send, 1);
-    }
-    {
-        const Real send = sel(b0, w[2], w[3]), keep = sel(b0, w[3], w[2]);
-        out1 = keep + shfl_xor(send, 1);
-    }
-}
-
-template <typename Real, int S, bool CONS, int MAXT>
-__global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_kernel4(const KParams p) {
-    constexpr int N2 = 2 * S;
-    constexpr int LPS = 4;                         // lanes per segment
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-
-    const int T = blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
-    const int SA = T >> 2;                         // segment slots of this CTA (>= segs_per_cta; T is a multiple of 32)
-    const int SEGS = p.segs_per_cta;
-    const int cta = blockIdx.x, nctas = gridDim.x;
-    const uint32_t flags = p.flags;
-    const bool has_box = CONS && (flags & KF_BOX), has_vel = CONS && (flags & KF_VEL), has_acc = CONS && (flags & KF_ACC);
-    const bool pin_pos = flags & KF_PIN_POS;
-    const bool nb_sync = flags & KF_NEIGHBOUR_SYNC;
-
-    const SmemLayout L = smem_layout4((int)sizeof(Real), S, CONS, SA);
-    double* Pms = reinterpret_cast<double*>(smem_raw + L.pm) + tid;            // [(h*N2 + b)*T]
-    Real* bco = reinterpret_cast<Real*>(smem_raw + L.bco);                     // [a][row]
-    Real* lohi = reinterpret_cast<Real*>(smem_raw + L.lohi);                   // [6][SA]
-    double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE;
-    Real* Cs = reinterpret_cast<Real*>(smem_raw + L.cs) + (size_t)sl * (sizeof(Real) == 8 ? 26 : 28);
-    Real* Bs = reinterpret_cast<Real*>(smem_raw + L.bs);                       // [2 parity][SA+2][8 rows][3]
-
-    const long long cta_first = p.seg_begin + (long long)cta * SEGS;
-    const long long remaining = p.seg_end - cta_first;
-    const int nact = remaining < SEGS ? (int)remaining : SEGS;
-    const bool active = sl < nact;
-    const long long gseg = active ? cta_first + sl : cta_first;
-    const bool owned = active && gseg >= p.own_begin && gseg < p.own_end;
-    const long long stride = p.stride;
-
-    // the two items of this lane: sample / row index jj[h], global lane slot gt[h]
-    int jj[2]; long long gt[2]; bool isrow[2], right[2]; int korder[2];
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-        jj[h] = lane + 4 * h;
-        gt[h] = gseg * LANES + jj[h];
-        isrow[h] = jj[h] < N2;
-        right[h] = jj[h] >= S;
-        korder[h] = right[h] ? jj[h] - S : jj[h];
-    }
-
-    // ---- constants
-    for (int idx = tid; idx < 64; idx += T) {
-        const int a = idx >> 3, r = idx & 7;
-        double v = 0.0;
-        if (r < N2 && a < N2) v = beta_entry(r % S, a, r < S ? 0.0 : 1.0);
-        bco[a * 8 + r] = (Real)v;
-    }
-    double c0[2][3];
-    Real invTk[2], tau[2], itau2[2], zoff[2][3];
-#pragma unroll
-    for (int h = 0; h < 2; ++h) {
-#pragma unroll
-        for (int b = 0; b < N2; ++b) Pms[(h * N2 + b) * T] = p.Pm[b * stride + gt[h]];
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            c0[h][d] = p.c0[d * stride + gt[h]];
-            zoff[h][d] = static_cast<const Real*>(p.zoff)[d * stride + gt[h]];
-        }
-        invTk[h] = static_cast<const Real*>(p.invTk)[gt[h]];
-        const double t = (double)(jj[h] + 1) / (double)(MS + 1);       // sample time (reading A10)
-        tau[h] = (Real)t; itau2[h] = (Real)(1.0 / (t * t));
-    }
-    const Real invT = static_cast<const Real*>(p.invT)[gseg], invT2 = static_cast<const Real*>(p.invT)[p.nseg_pad + gseg];
-    if (CONS) {
-        lohi[lane * SA + sl] = static_cast<const Real*>(p.lohi)[lane * p.nseg_pad + gseg];
-        if (lane < 2) lohi[(lane + 4) * SA + sl] = static_cast<const Real*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
-    }
-    const uint8_t sf = p.segflags[gseg];
-    const bool open_l = (flags & KF_OPEN_LEFT) && gseg == p.seg_begin, open_r = (flags & KF_OPEN_RIGHT) && gseg == p.seg_end - 1;
-    // ---- state of iterate k
-    Real zt[2][3], u[2][3], qp[2][3], qn[2][3], phv[2][3], wv[2][3], pha[2][3], wa[2][3];
-#pragma unroll
-    for (int h = 0; h < 2; ++h)
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            const long long i = d * stride + gt[h];
-            zt[h][d] = static_cast<const Real*>(p.zt)[i];
-            u[h][d] = static_cast<const Real*>(p.u)[i];
-            qp[h][d] = has_box ? static_cast<const Real*>(p.qp)[i] : (Real)0;
-            qn[h][d] = has_box ? static_cast<const Real*>(p.qn)[i] : (Real)0;
-            phv[h][d] = has_vel ? static_cast<const Real*>(p.phv)[i] : (Real)0;
-            wv[h][d] = has_vel ? static_cast<const Real*>(p.wv)[i] : (Real)0;
-            pha[h][d] = has_acc ? static_cast<const Real*>(p.pha)[i] : (Real)0;
-            wa[h][d] = has_acc ? static_cast<const Real*>(p.wa)[i] : (Real)0;
-        }
-    __syncthreads();
-
-    const Real vmax = (Real)p.vmax, amax = (Real)p.amax;
-    unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
-    const size_t mbox_par_stride = (size_t)p.max_ctas * 24 * 16;
-    __shared__ int abort_sh[2];
-    __shared__ int abort_any;
-    if (tid < 2) abort_sh[tid] = 0;
-    if (tid == 0) abort_any = 0;
-    const int warp = tid >> 5, nwarps = T >> 5;
-    const bool pairwise = nb_sync && nctas > 1 && nwarps <= 17 && (flags & KF_PAIRWISE);
-    __syncthreads();
-    for (int it = 0; it < p.k_sweeps; ++it) {
-        const unsigned seq = p.seq_base + (unsigned)it + 1u;
-        const int par = (int)(seq & 1u);
-        const bool last_sweep = (it == p.k_sweeps - 1);
-        Real* const Bcur = Bs + (size_t)par * (SA + 2) * 24;
-
-        // ================= phase A =================
-        // a1: right-hand side of Eq. 20a: both samples and both consensus rows of this lane go into all n rows,
-        // then the 4 lanes reduce-scatter (lane l ends with rows l and l+4)
-        Real R[2][3];
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            Real v[8];
-#pragma unroll
-            for (int a = 0; a < 8; ++a) v[a] = (Real)0;
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const Real gM = isrow[h] ? (zt[h][d] - u[h][d]) * invTk[h] : (Real)0;     // M'(z~ - u)
-                const Real* bc = bco + jj[h];
-                if (CONS) {
-                    Real A0 = 0, A1 = 0, A2 = 0;
-                    if (has_box) {      // Ao'(b - s - v); s + v = |q| (Moreau pair)
-                        const Real lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
-                        A0 = ((hi - fabs(qp[h][d])) + (lo + fabs(qn[h][d]))) * (tau[h] * tau[h]);
-                    }
-                    if (has_vel) A1 = (phv[h][d] - wv[h][d]) * (invT * tau[h]);
-                    if (has_acc) A2 = (pha[h][d] - wa[h][d]) * invT2;
-                    Real tp = itau2[h];                                       // tau^(a-2)
-#pragma unroll
-                    for (int a = 0; a < N2; ++a) {
-                        const Real inner = A0 + (Real)a * A1 + (Real)(a * (a - 1)) * A2;
-                        v[a] += tp * inner + bc[8 * a] * gM;
-                        tp *= tau[h];
-                    }
-                } else {
-#pragma unroll
-                    for (int a = 0; a < N2; ++a) v[a] += bc[8 * a] * gM;
-                }
-            }
-            reduce_scatter4(v, lane, R[0][d], R[1][d]);
-        }
-#pragma unroll
-        for (int h = 0; h < 2; ++h)
-#pragma unroll
-            for (int d = 0; d < 3; ++d) Xs[d * 8 + jj[h]] = (double)R[h][d];
-        __syncwarp();
-        // a2: x-update  c^ = (rho Pm^) R^ + c0^   (fp64 always)
-        Real crow[2][3];
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            double x[N2];
-#pragma unroll
-            for (int b = 0; b < N2; b += 2) {
-                const double2 t = *reinterpret_cast<const double2*>(Xs + d * 8 + b);
-                x[b] = t.x; x[b + 1] = t.y;
-            }
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                double c = c0[h][d];
-#pragma unroll
-                for (int b = 0; b < N2; ++b) c += Pms[(h * N2 + b) * T] * x[b];
-                crow[h][d] = (Real)c;
-                Cs[d * 8 + jj[h]] = (Real)c;
-            }
-        }
-        if (last_sweep && owned) {
-#pragma unroll
-            for (int h = 0; h < 2; ++h)
-#pragma unroll
-                for (int d = 0; d < 3; ++d) static_cast<Real*>(p.chat)[d * stride + gt[h]] = crow[h][d];
-        }
-        __syncwarp();
-        // a3: evaluate: consensus rows of B = M c, and the two samples of E0 c, E1 c, E2 c (synthetic division)
-        Real Bnd[2][3], Vv[2][3], Av[2][3];
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {
-            Real C[8];
-            if (sizeof(Real) == 8) {
-#pragma unroll
-                for (int b = 0; b < N2; b += 2) {
-                    const double2 t = *reinterpret_cast<const double2*>(Cs + d * 8 + b);
-                    C[b] = (Real)t.x; C[b + 1] = (Real)t.y;
-                }
-            } else {
-#pragma unroll
-                for (int b = 0; b < N2; b += 2) {
-                    const float2 t = *reinterpret_cast<const float2*>(Cs + d * 8 + b);
-                    C[b] = (Real)t.x; C[b + 1] = (Real)t.y;
-                }
-            }
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const Real* bc = bco + jj[h];
-                Real acc = 0;
-#pragma unroll
-                for (int b = 0; b < N2; ++b) acc += bc[8 * b] * C[b];
-                Bnd[h][d] = acc * invTk[h];
-                if (CONS) {
-                    Real D[8];
-#pragma unroll
-                    for (int b = 0; b < N2; ++b) D[b] = C[b];
-#pragma unroll
-                    for (int b = N2 - 2; b >= 0; --b) D[b] += tau[h] * D[b + 1];
-#pragma unroll
-                    for (int b = N2 - 2; b >= 1; --b) D[b] += tau[h] * D[b + 1];
-#pragma unroll
-                    for (int b = N2 - 2; b >= 2; --b) D[b] += tau[h] * D[b + 1];
-                    Vv[h][d] = D[1] * invT; Av[h][d] = (D[2] + D[2]) * invT2;
-                    if (has_box) {  // a7 + a8: q = -(A c - b + v): s = max(0,q), v <- max(0,-q)
-                        const Real lo = lohi[d * SA + sl], hi = lohi[(3 + d) * SA + sl];
-                        const Real vp = qp[h][d] < 0 ? -qp[h][d] : (Real)0, vn = qn[h][d] < 0 ? -qn[h][d] : (Real)0;
-                        qp[h][d] = (hi - D[0]) - vp;
-                        qn[h][d] = (D[0] - lo) - vn;
-                    }
-                }
-            }
-        }
-        // publish: shared memory for the neighbours in this CTA, mailbox for the neighbouring CTAs
-        bool need[2];
-        const unsigned char* rslot[2];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            if (isrow[h]) {
-#pragma unroll
-                for (int d = 0; d < 3; ++d) Bcur[(sl + 1) * 24 + jj[h] * 3 + d] = Bnd[h][d];
-                if (nctas > 1 && active) {
-                    unsigned char* e = mbox + par * mbox_par_stride + (size_t)cta * 24 * 16;
-                    if (sl == 0 && !right[h] && cta > 0) {
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) ll_store(e + (0 * 12 + korder[h] * 3 + d) * 16, (double)Bnd[h][d], seq);
-                    }
-                    if (sl == nact - 1 && right[h] && cta + 1 < nctas) {
-#pragma unroll
-                        for (int d = 0; d < 3; ++d) ll_store(e + (1 * 12 + korder[h] * 3 + d) * 16, (double)Bnd[h][d], seq);
-                    }
-                }
-            }
-            const bool need_l = active && isrow[h] && sl == 0 && !right[h] && cta > 0;
-            const bool need_r = active && isrow[h] && sl == nact - 1 && right[h] && cta + 1 < nctas;
-            need[h] = need_l || need_r;
-            rslot[h] = mbox + par * mbox_par_stride +
-                (need_l ? ((size_t)(cta - 1) * 24 + 12 + korder[h] * 3) * 16 : ((size_t)(cta + 1) * 24 + korder[h] * 3) * 16);
-        }
-        LLRaw rr[2][3];
-#pragma unroll
-        for (int h = 0; h < 2; ++h)
-            if (need[h]) {
-#pragma unroll
-                for (int d = 0; d < 3; ++d) ll_issue(rslot[h] + d * 16, rr[h][d]);
-            }
-        if (CONS) {
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                if (has_vel) ball_update(Vv[h], vmax, phv[h], wv[h]);      // a4: Eq. 20f, 20g
-                if (has_acc) ball_update(Av[h], amax, pha[h], wa[h]);
-            }
-        }
-
-        // ================= exchange of boundary rows =================
-        int wait_failed = 0;
-        {
-            bool okk = true;
-#pragma unroll
-            for (int h = 0; h < 2; ++h)
-                if (need[h]) okk = okk && ll_ok(rr[h][0], seq) && ll_ok(rr[h][1], seq) && ll_ok(rr[h][2], seq);
-            if (pairwise && *(volatile int*)&abort_any) okk = true;
-            if (!__all_sync(0xffffffffu, okk)) {
-                const long long t0 = global_ns();
-                unsigned spins = 0;
-                do {
-                    if (!okk) {
-                        okk = true;
-#pragma unroll
-                        for (int h = 0; h < 2; ++h)
-                            if (need[h]) {
-#pragma unroll
-                                for (int d = 0; d < 3; ++d) ll_issue(rslot[h] + d * 16, rr[h][d]);
-                                okk = okk && ll_ok(rr[h][0], seq) && ll_ok(rr[h][1], seq) && ll_ok(rr[h][2], seq);
-                            }
-                    }
-                    bool bail = false;
-                    if ((++spins & 255u) == 0) bail = *(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS;
-                    if (__any_sync(0xffffffffu, bail)) { if (!okk) { atomicExch(p.abort_flag, 1); wait_failed = 1; } break; }
-                } while (!__all_sync(0xffffffffu, okk));
-            }
-        }
-        if (wait_failed) { abort_sh[it & 1] = 1; *(volatile int*)&abort_any = 1; }
-        if (pairwise) {
-            const int first = (warp & 1) ? warp - 1 : warp, second = (warp & 1) ? warp : warp - 1;
-            if (first >= 0 && first + 1 < nwarps) asm volatile("bar.sync %0, 64;" ::"r"(first) : "memory");
-            if (second >= 0 && second + 1 < nwarps) asm volatile("bar.sync %0, 64;" ::"r"(second) : "memory");
-        } else if (nctas == 1) {
-            __syncthreads();
-        } else if (!nb_sync) {
-            if (!grid_barrier(p.bar, (unsigned long long)(it + 1) * nctas, p.abort_flag)) break;
-            if (abort_sh[it & 1]) break;
-        } else {
-            __syncthreads();
-            if (abort_sh[it & 1]) break;
-        }
-
-        // ================= phase B: consensus, dual, residuals =================
-        double rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
-        Real dz[2][3];
-#pragma unroll
-        for (int h = 0; h < 2; ++h) {
-#pragma unroll
-            for (int d = 0; d < 3; ++d) dz[h][d] = (Real)0;
-            if (!isrow[h]) continue;
-            Real nb[3];
-            if (need[h]) {
-#pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] = (Real)ll_value(rr[h][d]);
-            } else {
-                const Real* e = right[h] ? Bcur + (sl + 2) * 24 + korder[h] * 3 : Bcur + sl * 24 + (korder[h] + S) * 3;
-#pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] = e[d];
-            }
-            if (korder[h] == 0) {       // position rows live in segment-local frames
-#pragma unroll
-                for (int d = 0; d < 3; ++d) nb[d] += zoff[h][d];
-            }
-            const bool fixed = (right[h] ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder[h] == 0) ||
-                               (right[h] ? open_r : open_l);
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                const Real bl = right[h] ? Bnd[h][d] : nb[d], br = right[h] ? nb[d] : Bnd[h][d];
-                const Real znew = fixed ? zt[h][d] : (Real)0.5 * (bl + br);      // a5: Eq. 6b / 20b
-                dz[h][d] = znew - zt[h][d];
-                zt[h][d] = znew;
-                const Real res = Bnd[h][d] - znew;
-                u[h][d] += res;                                                  // a8: Eq. 6c / 20c
-                if (last_sweep) {
-                    rp2 += (double)res * (double)res;
-                    if (right[h] && !(sf & SEG_LAST)) { const double gp = (double)Bnd[h][d] - (double)nb[d]; gap2 += gp * gp; }
-                }
-            }
-        }
-        if (last_sweep) {
-            // a6: dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8)
-            double Tp[2];
-#pragma unroll
-            for (int h = 0; h < 2; ++h) Tp[h] = (double)static_cast<const Real*>(p.Tpow)[gt[h]];
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                Real v[8];
-#pragma unroll
-                for (int a = 0; a < 8; ++a) v[a] = (Real)0;
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    const Real gd = isrow[h] ? dz[h][d] * invTk[h] : (Real)0;
-#pragma unroll
-                    for (int a = 0; a < N2; ++a) v[a] += bco[8 * a + jj[h]] * gd;
-                }
-                Real x0, x1;
-                reduce_scatter4(v, lane, x0, x1);
-                const double xr0 = p.rho * (double)x0, xr1 = p.rho * (double)x1;
-                rdn2 += xr0 * xr0 + xr1 * xr1;
-                rd2 += (xr0 * Tp[0]) * (xr0 * Tp[0]) + (xr1 * Tp[1]) * (xr1 * Tp[1]);
-            }
-#pragma unroll
-            for (int m = 1; m < LPS; m <<= 1) {     // fixed-order tree over the 4 lanes of the segment
-                rp2 += shfl_xor(rp2, m); rd2 += shfl_xor(rd2, m); rdn2 += shfl_xor(rdn2, m); gap2 += shfl_xor(gap2, m);
-            }
-            if (owned && lane == 0) {
-                double* o = p.part + gseg * 4;
-                o[0] = rp2; o[1] = rd2; o[2] = rdn2; o[3] = gap2;
-            }
-        }
-    }
-
-    // ---- write iterate k + k_sweeps back
-    if (owned) {
-#pragma unroll
-        for (int h = 0; h < 2; ++h)
-#pragma unroll
-            for (int d = 0; d < 3; ++d) {
-                const long long i = d * stride + gt[h];
-                static_cast<Real*>(p.zt_out)[i] = zt[h][d];
-                static_cast<Real*>(p.u_out)[i] = u[h][d];
-                if (has_box) { static_cast<Real*>(p.qp_out)[i] = qp[h][d]; static_cast<Real*>(p.qn_out)[i] = qn[h][d]; }
-                if (has_vel) { static_cast<Real*>(p.phv_out)[i] = phv[h][d]; static_cast<Real*>(p.wv_out)[i] = wv[h][d]; }
-                if (has_acc) { static_cast<Real*>(p.pha_out)[i] = pha[h][d]; static_cast<Real*>(p.wa_out)[i] = wa[h][d]; }
-            }
-    }
-}
-
-}  // namespace
-
 // ------------------------------------------------------------------------------------------------ small kernels
 
 namespace {
@@ -1336,25 +899,6 @@ cudaError_t launch_one(const KParams& p, int ctas, int threads, size_t smem, cud
 }
 
 template <typename Real, int S, bool CONS, int MAXT>
-cudaError_t launch_one4(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
-    auto kern = cadmm_sweeps_kernel4<Real, S, CONS, MAXT>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    KParams pc = p;
-    void* args[] = {&pc};
-    if (ctas > 1) return cudaLaunchCooperativeKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
-    return cudaLaunchKernel((const void*)kern, dim3(ctas), dim3(threads), args, smem, st);
-}
-
-template <typename Real, int S, bool CONS, int MAXT>
-cudaError_t limits_one4(int threads, size_t smem, int* per_sm) {
-    auto kern = cadmm_sweeps_kernel4<Real, S, CONS, MAXT>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
-}
-
-template <typename Real, int S, bool CONS, int MAXT>
 cudaError_t limits_one(int threads, size_t smem, int* per_sm) {
     auto kern = cadmm_sweeps_kernel<Real, S, CONS, MAXT, true>;     // the larger of the two instantiations
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -1365,9 +909,6 @@ cudaError_t limits_one(int threads, size_t smem, int* per_sm) {
 // f64 kernels are compiled for <= 576 threads (112 registers per thread); f32 for <= 1024 (64 registers)
 // plus a variant for small CTAs (<= 256 threads: up to 255 registers, no spills, more ILP across dims)
 constexpr int MAXT_F64 = 576, MAXT_F32 = 1024, MAXT_SMALL = 256;
-// 4-lane kernels: fp64 <= 320 threads (3 warps per scheduler: 168 registers), fp32 <= 512 (128 registers),
-// and a small-CTA variant (<= 128 threads: 255 registers)
-constexpr int MAXT4_F64 = 320, MAXT4_F32 = 512, MAXT4_SMALL = 128;
 
 }  // namespace
 
@@ -1381,21 +922,13 @@ constexpr int MAXT4_F64 = 320, MAXT4_F32 = 512, MAXT4_SMALL = 128;
     }
 
 int max_threads_for(int dtype, int lanes) {
-    if (lanes == 4) return dtype == 0 ? MAXT4_F64 : MAXT4_F32;
+    (void)lanes;      // 8 lanes per segment; the 4-lane kernel is the tensor-core one (top_kernels_mma.cu)
     return dtype == 0 ? MAXT_F64 : MAXT_F32;
 }
 
 cudaError_t launch_sweeps(const KParams& p, int dtype, int s, bool constrained, int lanes, int ctas, int threads,
                           size_t smem, cudaStream_t st) {
-    if (lanes == 4) {
-#define F64(S_, C_) return threads <= MAXT4_SMALL ? launch_one4<double, S_, C_, MAXT4_SMALL>(p, ctas, threads, smem, st) \
-                                                  : launch_one4<double, S_, C_, MAXT4_F64>(p, ctas, threads, smem, st);
-#define F32(S_, C_) return threads <= MAXT4_SMALL ? launch_one4<float, S_, C_, MAXT4_SMALL>(p, ctas, threads, smem, st) \
-                                                  : launch_one4<float, S_, C_, MAXT4_F32>(p, ctas, threads, smem, st);
-        TOP_DISPATCH(F64, F32)
-#undef F64
-#undef F32
-    }
+    if (lanes != 8) return cudaErrorInvalidValue;
 #define F64(S_, C_) return threads <= MAXT_SMALL ? launch_one<double, S_, C_, MAXT_SMALL>(p, ctas, threads, smem, st) \
                                                  : launch_one<double, S_, C_, MAXT_F64>(p, ctas, threads, smem, st);
 #define F32(S_, C_) return threads <= MAXT_SMALL ? launch_one<float, S_, C_, MAXT_SMALL>(p, ctas, threads, smem, st) \
@@ -1407,15 +940,7 @@ cudaError_t launch_sweeps(const KParams& p, int dtype, int s, bool constrained, 
 }
 
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, int threads, size_t smem, int* max_ctas_per_sm) {
-    if (lanes == 4) {
-#define F64(S_, C_) return threads <= MAXT4_SMALL ? limits_one4<double, S_, C_, MAXT4_SMALL>(threads, smem, max_ctas_per_sm) \
-                                                  : limits_one4<double, S_, C_, MAXT4_F64>(threads, smem, max_ctas_per_sm);
-#define F32(S_, C_) return threads <= MAXT4_SMALL ? limits_one4<float, S_, C_, MAXT4_SMALL>(threads, smem, max_ctas_per_sm) \
-                                                  : limits_one4<float, S_, C_, MAXT4_F32>(threads, smem, max_ctas_per_sm);
-        TOP_DISPATCH(F64, F32)
-#undef F64
-#undef F32
-    }
+    if (lanes != 8) return cudaErrorInvalidValue;
 #define F64(S_, C_) return threads <= MAXT_SMALL ? limits_one<double, S_, C_, MAXT_SMALL>(threads, smem, max_ctas_per_sm) \
                                                  : limits_one<double, S_, C_, MAXT_F64>(threads, smem, max_ctas_per_sm);
 #define F32(S_, C_) return threads <= MAXT_SMALL ? limits_one<float, S_, C_, MAXT_SMALL>(threads, smem, max_ctas_per_sm) \
@@ -1427,7 +952,7 @@ cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, i
 }
 
 size_t sweep_smem_bytes(int dtype, int s, bool constrained, int lanes, int segs_per_cta) {
-    if (lanes == 4) return smem_layout4(dtype == 0 ? 8 : 4, s, constrained, (segs_per_cta * 4 + 31) / 32 * 8).total;
+    (void)lanes;
     return smem_layout(dtype == 0 ? 8 : 4, s, constrained, segs_per_cta).total;
 }
 

@@ -1,6 +1,6 @@
 // top_kernels_mma.cu -- the fp64 CADMM sweep with its constant-matrix contractions on the tensor cores.
 //
-// Same sweep, same global-memory layout, same exchange protocol as cadmm_sweeps_kernel4 (top_kernels.cu): FOUR lanes
+// Same sweep, same global-memory layout, same exchange protocol as cadmm_sweeps_kernel (top_kernels.cu), but FOUR lanes
 // per segment, lane t owns inequality samples {t, t+4} and coefficient / consensus rows {t, t+4}; 8 segments per
 // warp.  What differs is how the two contractions with CONSTANT matrices are done.  In the normalised-time basis
 // (c^_a = c_a T^a) the evaluation matrices of Eq. 19 are the same for every segment:
