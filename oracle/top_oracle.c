@@ -44,6 +44,22 @@
  *       kron(beta_0(t_ij)', a_k') (Ao is MK x m(d+1) as printed), one slack and one scaled dual per (sample, plane).
  *       The flat dimensions are then coupled: H is (n m) x (n m) and is formed and inverted as such (no
  *       per-dimension shortcut in the oracle).
+ *   A20 NumericSolve (Eq. 15-17; Alg. 1 lines 6-7 "c, w <- NumericSolve(c, z, u, s, v, w)"; L303): the
+ *       alternative x-update for "general convex inequality constraints".  Taken here: the LINEAR sets (box corridor) keep
+ *       their slack form -- s and v are still arguments of NumericSolve and ProjectNonNeg / UpdateDual follow unchanged --
+ *       and the QUADRATIC sets (velocity / acceleration balls) are the general constraints g0_j(c) = ||A(T_ij) c||^2 - bound^2
+ *       <= 0, one per sample and ball, replaced by the equality g_j(c) = max{0, g0_j(c)}^2 = 0 (Eq. 15) with one multiplier
+ *       each.  The x-update minimises the augmented Lagrangian (Eq. 17 on top of Eq. 5 and the slack penalty, scaled
+ *       multiplier w_j = y_j / rho):
+ *           F(c) = c'Q~c + rho/2 ||M~c - z~ + u||^2 + rho/2 ||Ao c + s - b + v||^2 + rho/2 sum_j (g_j(c) + w_j)^2   (+ const)
+ *       with L-BFGS [21] started at c^k, and the multiplier follows "similarly to Eq. 6c": w_j <- w_j + g_j(c^{k+1}).
+ *       The paper gives no L-BFGS parameters; taken: memory 6; initial inverse Hessian H0 = the closed-form operator of the
+ *       quadratic part of F (Pm of reading A2 built WITHOUT the ball terms: exact when no ball is violated, and it keeps
+ *       the iterates on the waypoint equalities in HARD mode, where the gradient is also projected onto the null space of
+ *       the two waypoint rows so that the whole iteration lives in that subspace); Armijo backtracking (1e-4, halving from
+ *       step 1); curvature pairs with s'y <= 1e-10 |s||y| are skipped; stop when the step is below tol (default 1e-10)
+ *       relative to the coefficients (in metres: component a times T^a), when the line search cannot decrease F any more,
+ *       or after max_inner (default 50) iterations.  Pins: tests/test_oracle_numeric.py.
  *   A15 ball projection scale = min(1, bound/||y||), ||y|| = 0 -> scale 1.
  *   A18 a single rho for every penalty.   A19 cost c'Qc without 1/2  =>  2Q in H.
  *
@@ -111,6 +127,11 @@ typedef struct {
     real_t *c0F;    /* [N][nm]      */
     real_t *Spl, *Vpl; /* [N][Ms][K] slack / scaled dual per (sample, plane) */
     real_t *part;   /* [N][4] residual partial sums */
+    /* NumericSolve branch (reading A20) */
+    int numeric, lbfgs_m, lbfgs_maxit;
+    double lbfgs_tol;
+    real_t *Yv, *Ya;   /* [N][Ms] scaled multipliers w_j of Eq. 17, velocity / acceleration ball */
+    int64_t inner_iters;   /* L-BFGS iterations so far, all segments */
     double rp, rd, rd_norm, rp_gap;
     int64_t iter;
 } oracle_t;
@@ -221,7 +242,7 @@ void oracle_destroy(oracle_t *o) {
     free(o->C); free(o->z); free(o->zprev); free(o->u);
     free(o->Sp); free(o->Sn); free(o->Vp); free(o->Vn);
     free(o->PhiV); free(o->WV); free(o->PhiA); free(o->WA); free(o->part);
-    free(o->planes); free(o->PmF); free(o->c0F); free(o->Spl); free(o->Vpl);
+    free(o->planes); free(o->PmF); free(o->c0F); free(o->Spl); free(o->Vpl); free(o->Yv); free(o->Ya);
     free(o);
 }
 
@@ -256,6 +277,7 @@ static int build_operator(oracle_t *o, int i) {
         for (int k = 0; k < 3; ++k) {
             real_t *E = k == 0 ? o->E0 : (k == 1 ? o->E1 : o->E2);
             int on = k == 0 ? o->has_box : (k == 1 ? o->has_vel : o->has_acc);
+            if (o->numeric && k > 0) on = 0;      /* A20: the balls are not part of the quadratic model */
             pre_t w = k == 0 ? 2 : 1;
             beta_row(n, k, t, row);
             for (int a = 0; a < n; ++a) E[((size_t)i * Ms + j) * n + a] = (real_t)row[a];
@@ -408,6 +430,7 @@ static oracle_t *oracle_create_impl(int N, int s, int m, const double *waypoints
     ALLOC(o->PhiV, (size_t)N * Ms * m); ALLOC(o->WV, (size_t)N * Ms * m);
     ALLOC(o->PhiA, (size_t)N * Ms * m); ALLOC(o->WA, (size_t)N * Ms * m);
     ALLOC(o->part, (size_t)N * 4);
+    ALLOC(o->Yv, (size_t)N * Ms); ALLOC(o->Ya, (size_t)N * Ms);
     for (int i = 0; i < N; ++i) { if (!(durations[i] > 0)) { oracle_destroy(o); return NULL; } o->T[i] = (real_t)durations[i]; }
     for (int a = 0; a < (N + 1) * m; ++a) o->p[a] = (real_t)waypoints[a];
     if (o->has_box) for (int a = 0; a < N * m; ++a) { o->lo[a] = (real_t)box_lo[a]; o->hi[a] = (real_t)box_hi[a]; }
@@ -492,15 +515,187 @@ oracle_t *oracle_create_poly(int N, int s, int m, const double *waypoints, const
     return oracle_create_impl(N, s, m, waypoints, durations, start_derivs, end_derivs, Ms, NULL, NULL, vmax, amax, rho, mode, K, planes, s);
 }
 
+/* ------------------------------------------------------------------ NumericSolve (reading A20; Eq. 15-17) */
+
+#define NVAR (NMAX * 3)   /* unknowns of one segment: c[a*m + d] */
+#define LBFGS_MMAX 8
+
+/* F(c) of segment i (see A20) and, if grad != NULL, its gradient, straight from the definition:
+ *   F = sum_d c_d'Q c_d + rho/2 ||M c - z~ + u||^2 (rows that exist) + rho/2 ||Ao c + s - b + v||^2 (box, both sides)
+ *       + rho/2 sum_j [ (g^v_j + w^v_j)^2 + (g^a_j + w^a_j)^2 ],   g_j = max(0, ||A_j c||^2 - bound^2)^2        (Eq. 15, 17) */
+static real_t numeric_eval(const oracle_t *o, int i, const real_t *c, real_t *grad) {
+    const int n = o->n, m = o->m, Ms = o->Ms, nc = o->nc;
+    const real_t rho = o->rho;
+    real_t F = 0;
+    if (grad) for (int a = 0; a < n * m; ++a) grad[a] = 0;
+    const real_t *Q = o->Q + (size_t)i * n * n;
+    for (int d = 0; d < m; ++d)                       /* c'Q~c (no 1/2: A19) */
+        for (int a = 0; a < n; ++a) {
+            real_t qc = 0;
+            for (int b = 0; b < n; ++b) qc += Q[a * n + b] * c[b * m + d];
+            F += c[a * m + d] * qc;
+            if (grad) grad[a * m + d] += 2 * qc;
+        }
+    const real_t *M = o->M + (size_t)i * 2 * nc * n;
+    for (int r = 0; r < 2 * nc; ++r) {                /* consensus penalty of Eq. 5 */
+        if (o->rowmask[(size_t)i * 2 * nc + r] == 0) continue;
+        const real_t *zr = o->z + ((size_t)(i + (r >= nc)) * nc + (r % nc)) * m;
+        const real_t *ur = o->u + ((size_t)i * 2 * nc + r) * m;
+        for (int d = 0; d < m; ++d) {
+            real_t e = -zr[d] + ur[d];
+            for (int a = 0; a < n; ++a) e += M[r * n + a] * c[a * m + d];
+            F += (rho / 2) * e * e;
+            if (grad) for (int a = 0; a < n; ++a) grad[a * m + d] += rho * M[r * n + a] * e;
+        }
+    }
+    for (int j = 0; j < Ms; ++j) {
+        const real_t *e0 = o->E0 + ((size_t)i * Ms + j) * n, *e1 = o->E1 + ((size_t)i * Ms + j) * n, *e2 = o->E2 + ((size_t)i * Ms + j) * n;
+        size_t q = ((size_t)i * Ms + j) * m;
+        if (o->has_box)                                /* slack penalty of the linear set (Eq. 8), + and - side */
+            for (int d = 0; d < m; ++d) {
+                real_t P = 0;
+                for (int a = 0; a < n; ++a) P += e0[a] * c[a * m + d];
+                real_t ep = P + o->Sp[q + d] - o->hi[(size_t)i * m + d] + o->Vp[q + d];
+                real_t en = -P + o->Sn[q + d] + o->lo[(size_t)i * m + d] + o->Vn[q + d];
+                F += (rho / 2) * (ep * ep + en * en);
+                if (grad) for (int a = 0; a < n; ++a) grad[a * m + d] += rho * e0[a] * (ep - en);
+            }
+        for (int kind = 1; kind <= 2; ++kind) {        /* general constraints: Eq. 15 inside Eq. 17 */
+            if (kind == 1 ? !o->has_vel : !o->has_acc) continue;
+            const real_t *e = kind == 1 ? e1 : e2;
+            const real_t bound = kind == 1 ? o->vmax : o->amax;
+            const real_t w = (kind == 1 ? o->Yv : o->Ya)[(size_t)i * Ms + j];
+            real_t val[3] = {0, 0, 0}, n2 = 0;
+            for (int d = 0; d < m; ++d) { for (int a = 0; a < n; ++a) val[d] += e[a] * c[a * m + d]; n2 += val[d] * val[d]; }
+            const real_t g0 = n2 - bound * bound, gp = g0 > 0 ? g0 : 0, g = gp * gp;
+            F += (rho / 2) * (g + w) * (g + w);
+            if (grad && gp > 0) {                      /* d/dc: rho (g + w) * 2 gp * 2 A_j'(A_j c) */
+                const real_t k = rho * (g + w) * 2 * gp * 2;
+                for (int d = 0; d < m; ++d) for (int a = 0; a < n; ++a) grad[a * m + d] += k * e[a] * val[d];
+            }
+        }
+    }
+    return F;
+}
+
+/* g_j(c) = max(0, ||A_j c||^2 - bound^2)^2 of sample j (Eq. 15) */
+static real_t numeric_g(const oracle_t *o, int i, int j, int kind, const real_t *c) {
+    const int n = o->n, m = o->m, Ms = o->Ms;
+    const real_t *e = (kind == 1 ? o->E1 : o->E2) + ((size_t)i * Ms + j) * n;
+    const real_t bound = kind == 1 ? o->vmax : o->amax;
+    real_t n2 = 0;
+    for (int d = 0; d < m; ++d) { real_t v = 0; for (int a = 0; a < n; ++a) v += e[a] * c[a * m + d]; n2 += v * v; }
+    const real_t g0 = n2 - bound * bound, gp = g0 > 0 ? g0 : 0;
+    return gp * gp;
+}
+
+/* HARD waypoints: orthogonal projection of a gradient onto the null space of the two waypoint rows Ew = [beta_0(0); beta_0(T)]
+ * of every dimension.  The L-BFGS iteration then lives in that subspace: H0 = Pm maps into it, and no rounding residue of
+ * the steps can pick up the (large) constraint-normal part of the gradient. */
+static void project_tangent(const oracle_t *o, int i, real_t *g) {
+    if (o->mode != MODE_HARD) return;
+    const int n = o->n, m = o->m;
+    real_t r1[NMAX], g11 = 0;
+    r1[0] = 1;
+    for (int a = 1; a < n; ++a) r1[a] = r1[a - 1] * o->T[i];
+    for (int a = 0; a < n; ++a) g11 += r1[a] * r1[a];
+    /* Gram of (e_0, r1) = [[1, 1], [1, g11]] */
+    const real_t det = g11 - 1;
+    for (int d = 0; d < m; ++d) {
+        real_t b0 = g[0 * m + d], b1 = 0;
+        for (int a = 0; a < n; ++a) b1 += r1[a] * g[a * m + d];
+        const real_t l0 = (g11 * b0 - b1) / det, l1 = (b1 - b0) / det;
+        g[0 * m + d] -= l0;
+        for (int a = 0; a < n; ++a) g[a * m + d] -= l1 * r1[a];
+    }
+}
+
+/* x-update of segment i by L-BFGS (Nocedal & Wright, Numerical Optimization, Alg. 7.4 / 7.5) from c^k, in place.
+ * H0 = Pm per dimension (A20).  Returns the iterations used. */
+static int numeric_solve_segment(oracle_t *o, int i) {
+    const int n = o->n, m = o->m, nv = n * m, mem = o->lbfgs_m;
+    real_t *x = o->C + (size_t)i * nv;
+    const real_t *Pm = o->Pm + (size_t)i * n * n;
+    real_t g[NVAR], gn[NVAR], xn[NVAR], dir[NVAR], qv[NVAR];
+    real_t S[LBFGS_MMAX][NVAR], Y[LBFGS_MMAX][NVAR], rhoi[LBFGS_MMAX], alpha[LBFGS_MMAX];
+    int hist = 0, it = 0;
+    real_t F = numeric_eval(o, i, x, g);
+    project_tangent(o, i, g);
+    real_t Tp[NMAX];
+    Tp[0] = 1;
+    for (int a = 1; a < n; ++a) Tp[a] = Tp[a - 1] * o->T[i];
+    for (; it < o->lbfgs_maxit; ++it) {
+        for (int a = 0; a < nv; ++a) qv[a] = g[a];                       /* two-loop recursion */
+        for (int h = hist - 1; h >= 0; --h) {
+            real_t sq = 0;
+            for (int a = 0; a < nv; ++a) sq += S[h][a] * qv[a];
+            alpha[h] = rhoi[h] * sq;
+            for (int a = 0; a < nv; ++a) qv[a] -= alpha[h] * Y[h][a];
+        }
+        for (int a = 0; a < n; ++a) for (int d = 0; d < m; ++d) {        /* r = H0 q */
+            real_t acc = 0;
+            for (int b = 0; b < n; ++b) acc += Pm[a * n + b] * qv[b * m + d];
+            dir[a * m + d] = acc;
+        }
+        for (int h = 0; h < hist; ++h) {
+            real_t yr = 0;
+            for (int a = 0; a < nv; ++a) yr += Y[h][a] * dir[a];
+            const real_t beta = rhoi[h] * yr;
+            for (int a = 0; a < nv; ++a) dir[a] += S[h][a] * (alpha[h] - beta);
+        }
+        real_t slope = 0, dmax = 0, xmax = 0;
+        for (int a = 0; a < n; ++a) for (int d = 0; d < m; ++d) {
+            dir[a * m + d] = -dir[a * m + d];
+            slope += g[a * m + d] * dir[a * m + d];
+            real_t da = fabsl((long double)(dir[a * m + d] * Tp[a])), xa = fabsl((long double)(x[a * m + d] * Tp[a]));
+            if (da > dmax) dmax = da;
+            if (xa > xmax) xmax = xa;
+        }
+        if (!(dmax > (real_t)o->lbfgs_tol * xmax) || !(slope < 0)) break;     /* converged (step below tolerance) */
+        real_t t = 1, Fn = F;
+        int ok = 0;
+        for (int ls = 0; ls < 40; ++ls) {                                   /* Armijo backtracking */
+            for (int a = 0; a < nv; ++a) xn[a] = x[a] + t * dir[a];
+            Fn = numeric_eval(o, i, xn, NULL);
+            if (Fn <= F + (real_t)1e-4 * t * slope) { ok = 1; break; }
+            t *= (real_t)0.5;
+        }
+        if (!ok) break;                                                     /* no decrease possible: rounding floor */
+        numeric_eval(o, i, xn, gn);
+        project_tangent(o, i, gn);
+        real_t sy = 0, ss = 0, yy = 0;
+        real_t sv[NVAR], yv[NVAR];
+        for (int a = 0; a < nv; ++a) { sv[a] = t * dir[a]; yv[a] = gn[a] - g[a]; sy += sv[a] * yv[a]; ss += sv[a] * sv[a]; yy += yv[a] * yv[a]; }
+        if (sy > (real_t)1e-10 * R_SQRT(ss * yy)) {      /* curvature pair (skipped when it carries no curvature information) */
+            if (hist == mem) {
+                for (int h = 1; h < mem; ++h) { memcpy(S[h - 1], S[h], sizeof(real_t) * nv); memcpy(Y[h - 1], Y[h], sizeof(real_t) * nv); rhoi[h - 1] = rhoi[h]; }
+                hist = mem - 1;
+            }
+            memcpy(S[hist], sv, sizeof(real_t) * nv); memcpy(Y[hist], yv, sizeof(real_t) * nv); rhoi[hist] = 1 / sy;
+            ++hist;
+        }
+        for (int a = 0; a < nv; ++a) { x[a] = xn[a]; g[a] = gn[a]; }
+        F = Fn;
+    }
+    return it;
+}
+
 /* ------------------------------------------------------------------ one sweep (Alg. 1 lines 3-13) */
 
 static void sweep_once(oracle_t *o) {
     const int N = o->N, n = o->n, m = o->m, Ms = o->Ms, nc = o->nc;
     const real_t rho = o->rho;
 
+    if (o->numeric) {      /* NumericSolve (Alg. 1 lines 6-7; reading A20) instead of ClosedFormSolve */
+        int64_t inner = 0;
+#pragma omp parallel for schedule(static) reduction(+ : inner)
+        for (int i = 0; i < N; ++i) inner += numeric_solve_segment(o, i);
+        o->inner_iters += inner;
+    }
     /* ClosedFormSolve: Eq. 20a with rho on the right-hand side (A3) */
 #pragma omp parallel for schedule(static)
     for (int i = 0; i < N; ++i) {
+        if (o->numeric) continue;
         real_t R[NMAX * 3];
         for (int a = 0; a < n * m; ++a) R[a] = 0;
         const real_t *M = o->M + (size_t)i * 2 * nc * n;
@@ -559,6 +754,7 @@ static void sweep_once(oracle_t *o) {
         for (int j = 0; j < Ms; ++j) {
             size_t q = ((size_t)i * Ms + j) * m;
             for (int kind = 1; kind <= 2; ++kind) {
+                if (o->numeric) continue;                   /* A20: the balls are handled inside NumericSolve */
                 if (kind == 1 ? !o->has_vel : !o->has_acc) continue;
                 const real_t *e = (kind == 1 ? o->E1 : o->E2) + ((size_t)i * Ms + j) * n;
                 real_t *Phi = (kind == 1 ? o->PhiV : o->PhiA) + q, *W = (kind == 1 ? o->WV : o->WA) + q;
@@ -629,6 +825,12 @@ static void sweep_once(oracle_t *o) {
         }
         o->part[(size_t)i * 4 + 0] = rp2; o->part[(size_t)i * 4 + 1] = rd2;
         o->part[(size_t)i * 4 + 2] = rdn2; o->part[(size_t)i * 4 + 3] = gap2;
+
+        if (o->numeric)                                  /* multiplier of Eq. 17, scaled: w_j <- w_j + g_j(c^{k+1})  (A20) */
+            for (int j = 0; j < Ms; ++j) {
+                if (o->has_vel) o->Yv[(size_t)i * Ms + j] += numeric_g(o, i, j, 1, o->C + (size_t)i * n * m);
+                if (o->has_acc) o->Ya[(size_t)i * Ms + j] += numeric_g(o, i, j, 2, o->C + (size_t)i * n * m);
+            }
 
         if (o->has_box)
             for (int j = 0; j < Ms; ++j) {
@@ -719,12 +921,30 @@ int oracle_set_rho(oracle_t *o, double rho_new) {
     for (size_t a = 0; a < (size_t)N * 2 * o->nc * m; ++a) o->u[a] *= r;
     for (size_t a = 0; a < (size_t)N * Ms * m; ++a) { o->Vp[a] *= r; o->Vn[a] *= r; o->WV[a] *= r; o->WA[a] *= r; }
     for (size_t a = 0; a < (size_t)N * Ms * o->K; ++a) o->Vpl[a] *= r;
+    for (size_t a = 0; a < (size_t)N * Ms; ++a) { o->Yv[a] *= r; o->Ya[a] *= r; }
     o->rho = (real_t)rho_new;
     for (int i = 0; i < N; ++i) if (o->has_poly ? build_operator_poly(o, i) : build_operator(o, i)) return -1;
     return 0;
 }
 
 double oracle_rho(const oracle_t *o) { return (double)o->rho; }
+
+/* switch the solver to the NumericSolve branch (reading A20); call right after create (iterate 0).  Returns 0 on success. */
+int oracle_set_numeric(oracle_t *o, int memory, int max_inner, double tol) {
+    if (o->has_poly || o->iter != 0 || memory < 1 || memory > LBFGS_MMAX || max_inner < 1 || !(tol >= 0)) return -1;
+    o->numeric = 1; o->lbfgs_m = memory; o->lbfgs_maxit = max_inner; o->lbfgs_tol = tol;
+    for (int i = 0; i < o->N; ++i) if (build_operator(o, i)) return -1;      /* H0: the quadratic part only */
+    return 0;
+}
+int64_t oracle_inner_iters(const oracle_t *o) { return o->inner_iters; }
+/* F and its gradient for segment i at coefficients c [n][m] (the current z, u, s, v, w): exposed for the pins */
+double oracle_numeric_eval(const oracle_t *o, int i, const double *c, double *grad) {
+    real_t cc[NVAR], gg[NVAR];
+    for (int a = 0; a < o->n * o->m; ++a) cc[a] = (real_t)c[a];
+    real_t F = numeric_eval(o, i, cc, grad ? gg : NULL);
+    if (grad) for (int a = 0; a < o->n * o->m; ++a) grad[a] = (double)gg[a];
+    return (double)F;
+}
 
 /* Alg. 1 with line 14: sweep; test the stop rule (Eq. 23); every `every` sweeps apply Eq. 24 with the residuals of
  * that sweep:  rho <- tau_incr*rho if r_p > mu r_d;  rho <- rho/tau_decr if r_d > mu r_p.  Returns sweeps done. */
@@ -785,6 +1005,7 @@ int64_t oracle_get(const oracle_t *o, const char *name, double *out) {
     FIELD("v_pos", o->Vp, (size_t)N * Ms * m) FIELD("v_neg", o->Vn, (size_t)N * Ms * m)
     FIELD("phi_v", o->PhiV, (size_t)N * Ms * m) FIELD("w_v", o->WV, (size_t)N * Ms * m)
     FIELD("phi_a", o->PhiA, (size_t)N * Ms * m) FIELD("w_a", o->WA, (size_t)N * Ms * m)
+    FIELD("y_v", o->Yv, (size_t)N * Ms) FIELD("y_a", o->Ya, (size_t)N * Ms)
     FIELD("s_poly", o->Spl, (size_t)N * Ms * o->K) FIELD("v_poly", o->Vpl, (size_t)N * Ms * o->K)
     FIELD("Pm", o->Pm, (size_t)N * n * n) FIELD("c0", o->c0, (size_t)N * n * m) FIELD("Q", o->Q, (size_t)N * n * n)
     FIELD("M", o->M, (size_t)N * 2 * nc * n) FIELD("rowmask", o->rowmask, (size_t)N * 2 * nc) FIELD("E0", o->E0, (size_t)N * Ms * n) FIELD("E1", o->E1, (size_t)N * Ms * n)

@@ -46,6 +46,12 @@ def _lib(long_double: bool):
         L.oracle_create_ex.restype = ctypes.c_void_p
         L.oracle_create_ex.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp, dp, ctypes.c_int, dp, dp, ctypes.c_int, dp,
                                        ctypes.c_double, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int]
+        L.oracle_set_numeric.restype = ctypes.c_int
+        L.oracle_set_numeric.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_double]
+        L.oracle_inner_iters.restype = ctypes.c_int64
+        L.oracle_inner_iters.argtypes = [ctypes.c_void_p]
+        L.oracle_numeric_eval.restype = ctypes.c_double
+        L.oracle_numeric_eval.argtypes = [ctypes.c_void_p, ctypes.c_int, dp, dp]
         L.oracle_destroy.argtypes = [ctypes.c_void_p]
         L.oracle_sweep.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int]
         L.oracle_solve.restype = ctypes.c_int64
@@ -77,7 +83,8 @@ class Oracle:
     """One trajectory (the oracle has no batch dimension; loop over it)."""
 
     def __init__(self, waypoints, durations, s, rho, samples=0, box_lo=None, box_hi=None, vmax=0.0, amax=0.0,
-                 start_derivs=None, end_derivs=None, mode="hard", long_double=False, planes=None, consensus="s"):
+                 start_derivs=None, end_derivs=None, mode="hard", long_double=False, planes=None, consensus="s",
+                 numeric=False, lbfgs_memory=6, max_inner=50, inner_tol=1e-10):
         """consensus: "s" = derivative orders 0..s-1 at every boundary (default, reading A1); "wide" = the paper-literal
         orders 0..2s-2, the orders >= s left out at the two trajectory ends."""
         wp = np.ascontiguousarray(waypoints, dtype=np.float64)
@@ -109,6 +116,9 @@ class Oracle:
                                            MODES[mode], self.nc)
         if not self._h:
             raise ValueError("oracle_create rejected the inputs")
+        if numeric:       # NumericSolve branch (reading A20): L-BFGS x-update for the ball sets
+            if self._L.oracle_set_numeric(self._h, int(lbfgs_memory), int(max_inner), float(inner_tol)) != 0:
+                raise ValueError("oracle_set_numeric rejected the inputs")
 
     def __del__(self):
         if getattr(self, "_h", None):
@@ -133,6 +143,17 @@ class Oracle:
         return int(self._L.oracle_solve_adaptive(self._h, float(eps), int(max_iter), int(use_rd_norm), float(mu),
                                                  float(tau_incr), float(tau_decr), int(every), int(threads)))
 
+    @property
+    def inner_iters(self):
+        return int(self._L.oracle_inner_iters(self._h))
+
+    def numeric_eval(self, i, c, want_grad=True):
+        """F (A20) and its gradient for segment i at coefficients c [n][m], with the solver's current z, u, s, v, w."""
+        c = np.ascontiguousarray(c, dtype=np.float64)
+        g = np.zeros_like(c) if want_grad else None
+        F = float(self._L.oracle_numeric_eval(self._h, int(i), _dptr(c), _dptr(g)))
+        return (F, g) if want_grad else F
+
     def residuals(self):
         out = np.zeros(4)
         self._L.oracle_residuals(self._h, _dptr(out))
@@ -153,7 +174,7 @@ class Oracle:
         "u": lambda o: (o.N, 2 * o.nc, o.m), "rowmask": lambda o: (o.N, 2 * o.nc), "Pm": lambda o: (o.N, o.n, o.n), "c0": lambda o: (o.N, o.n, o.m),
         "Q": lambda o: (o.N, o.n, o.n), "M": lambda o: (o.N, 2 * o.nc, o.n),
         "E0": lambda o: (o.N, o.Ms, o.n), "E1": lambda o: (o.N, o.Ms, o.n), "E2": lambda o: (o.N, o.Ms, o.n),
-        "s_poly": lambda o: (o.N, o.Ms, o.K), "v_poly": lambda o: (o.N, o.Ms, o.K),
+        "y_v": lambda o: (o.N, o.Ms), "y_a": lambda o: (o.N, o.Ms), "s_poly": lambda o: (o.N, o.Ms, o.K), "v_poly": lambda o: (o.N, o.Ms, o.K),
     }
 
     def get(self, name):
