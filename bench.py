@@ -530,6 +530,23 @@ def main():
                              "unit": "TFLOP/s", "frac": fl_w * ww.N * 2000 / (msw * 1e-3) / peaks["f64"],
                              "flops_per_segment_sweep": fl_w}}
             sw.close()
+            # the NumericSolve branch of Alg. 1 (Eq. 15-17: L-BFGS x-update) on config 4's input
+            wn = make_workload("cfg4", rank)
+            sn = top.from_workload(wn, device=local_rank, stream=stream.cuda_stream, numeric=True)
+            sn.iterate(10); torch.cuda.synchronize()
+            in0 = sn.inner_iterations()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream); sn.iterate(100); e1.record(stream); torch.cuda.synchronize()
+            msn = e0.elapsed_time(e1)
+            inner = (sn.inner_iterations() - in0) / (100.0 * wn.N)
+            fl_it = 7800.0       # per L-BFGS iteration: ray map + gradient + two-loop recursion + >= 1 line-search trial
+            others[wn.name + "_numeric_solve"] = {
+                "segment_iterations_per_s": wn.N * 100 / (msn * 1e-3), "sweeps": 100, "us_per_sweep_per_wave": 1e3 * msn / 100, "dtype": "f64",
+                "lbfgs_iterations_per_segment_sweep": inner, "launches_per_sweep": 2,
+                "roofline": {"bound": "alu", "achieved": fl_it * inner * wn.N * 100 / (msn * 1e-3) / 1e12, "peak": peaks["f64"] / 1e12, "unit": "TFLOP/s",
+                             "frac": fl_it * inner * wn.N * 100 / (msn * 1e-3) / peaks["f64"], "flops_per_lbfgs_iteration": fl_it,
+                             "note": "latency bound: the sweep waits for the segments with the longest inner iteration"}}
+            sn.close()
             out["other_workloads"] = others
             # ---- the paper's own regime (Tables I-II): tolerance ||r|| < N*0.05 on config 2, fixed rho
             # vs adaptive rho (Eq. 24, rho0 = 1, updated every sweep as in Alg. 1 line 14)

@@ -94,6 +94,16 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
  * TOP_F64 on the tensor-core kernel only, no polytope corridor, the trajectory must fit on chip (N <= 148 x 56);
  * else TOP_E_UNSUPPORTED. */
 #define TOP_CONSENSUS_WIDE    256u
+/* x-update branch of Alg. 1 (PAPER.md:L266-270 lines 4-8).  Default: ClosedFormSolve (Eq. 20a, 20f, 20g).
+ * TOP_XUPDATE_NUMERIC: NumericSolve (Eq. 15-17; L303) -- the ball sets ||sigma'|| <= vmax, ||sigma''|| <= amax
+ * are treated as general convex inequality constraints g0_j(c) <= 0, replaced by g_j(c) = max{0, g0_j(c)}^2 = 0 (Eq. 15) with
+ * one scaled multiplier per sample and ball, w_j <- w_j + g_j(c^{k+1}); the x-update minimises the augmented Lagrangian
+ * (Eq. 17 added to Eq. 5 and to the slack penalty of the box, which keeps its slack form) with L-BFGS: memory 6, initial
+ * inverse Hessian = the closed-form operator of the quadratic part, Armijo backtracking, stop when the step (proposed or taken) is below 1e-10
+ * of the coefficients or after 50 iterations (the paper gives no parameters; reading A20 of DESIGN.md).
+ * top_get_state "y_v" / "y_a" [batch][N][8] are the multipliers; "phi_*" / "w_*" read 0.  TOP_F64 only; no polytope
+ * corridor, TOP_CONSENSUS_WIDE, TOP_RHO_ADAPTIVE, top_set_rho or snapshots (TOP_E_UNSUPPORTED / TOP_E_INVALID). */
+#define TOP_XUPDATE_NUMERIC   512u
 
 /* The paper's convex sets, specialised as BASELINE.json's configs use them:
  * an axis-aligned box corridor per segment (K=6 half-spaces, linear set, Eq. 7-10) and Euclidean balls on
@@ -231,6 +241,10 @@ TOP_API top_status top_snapshot_restore(top_solver* h, const void* host_buf, siz
 
 /* Sweeps done since top_create. */
 TOP_API int64_t top_iteration(const top_solver* h);
+
+/* top_numeric_info -- TOP_XUPDATE_NUMERIC solvers: the number of L-BFGS iterations spent so far, summed over segments and
+ * sweeps (out may be NULL).  Synchronises the stream.  TOP_E_INVALID for a closed-form solver. */
+TOP_API top_status top_numeric_info(top_solver* h, int64_t* inner_iterations);
 
 /* Launch facts of this solver (for the bench's roofline arithmetic); any pointer may be NULL:
  * CTAs per launch, threads per CTA, segments per CTA, dynamic shared memory bytes per CTA,

@@ -57,7 +57,7 @@
  *       quadratic part of F (Pm of reading A2 built WITHOUT the ball terms: exact when no ball is violated, and it keeps
  *       the iterates on the waypoint equalities in HARD mode, where the gradient is also projected onto the null space of
  *       the two waypoint rows so that the whole iteration lives in that subspace); Armijo backtracking (1e-4, halving from
- *       step 1); curvature pairs with s'y <= 1e-10 |s||y| are skipped; stop when the step is below tol (default 1e-10)
+ *       step 1); curvature pairs with s'y <= 0 are skipped; stop when the step (proposed, or taken after back-tracking) is below tol (default 1e-10)
  *       relative to the coefficients (in metres: component a times T^a), when the line search cannot decrease F any more,
  *       or after max_inner (default 50) iterations.  Pins: tests/test_oracle_numeric.py.
  *   A15 ball projection scale = min(1, bound/||y||), ||y|| = 0 -> scale 1.
@@ -663,10 +663,10 @@ static int numeric_solve_segment(oracle_t *o, int i) {
         if (!ok) break;                                                     /* no decrease possible: rounding floor */
         numeric_eval(o, i, xn, gn);
         project_tangent(o, i, gn);
-        real_t sy = 0, ss = 0, yy = 0;
+        real_t sy = 0;
         real_t sv[NVAR], yv[NVAR];
-        for (int a = 0; a < nv; ++a) { sv[a] = t * dir[a]; yv[a] = gn[a] - g[a]; sy += sv[a] * yv[a]; ss += sv[a] * sv[a]; yy += yv[a] * yv[a]; }
-        if (sy > (real_t)1e-10 * R_SQRT(ss * yy)) {      /* curvature pair (skipped when it carries no curvature information) */
+        for (int a = 0; a < nv; ++a) { sv[a] = t * dir[a]; yv[a] = gn[a] - g[a]; sy += sv[a] * yv[a]; }
+        if (sy > 0) {                                    /* curvature pair (F is convex: s'y >= 0; = 0 only at the rounding floor) */
             if (hist == mem) {
                 for (int h = 1; h < mem; ++h) { memcpy(S[h - 1], S[h], sizeof(real_t) * nv); memcpy(Y[h - 1], Y[h], sizeof(real_t) * nv); rhoi[h - 1] = rhoi[h]; }
                 hist = mem - 1;
@@ -676,6 +676,7 @@ static int numeric_solve_segment(oracle_t *o, int i) {
         }
         for (int a = 0; a < nv; ++a) { x[a] = xn[a]; g[a] = gn[a]; }
         F = Fn;
+        if (!(t * dmax > (real_t)o->lbfgs_tol * xmax)) { ++it; break; }      /* the step TAKEN is below tolerance: converged */
     }
     return it;
 }

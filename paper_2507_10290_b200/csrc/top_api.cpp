@@ -59,6 +59,10 @@ struct top_solver {
     bool wide = false;                 // paper-literal consensus n_c = 2s-1 (reading A1): second block of consensus rows
     int nc = 0;                        // consensus derivative orders per boundary: s, or 2s-1
     void *d_zt2 = nullptr, *d_u2 = nullptr, *d_invTk2 = nullptr;
+    // NumericSolve branch (TOP_XUPDATE_NUMERIC; top_kernels_numeric.cu): state in device memory, two launches per sweep
+    bool numeric = false;
+    double *d_yv = nullptr, *d_ya = nullptr, *d_bnd = nullptr;
+    unsigned long long* d_inner = nullptr;
     struct Wave { long long seg_begin, seg_end, own_begin, own_end; uint32_t kflags; int segs_per_cta, ctas, threads; size_t smem;
                   bool cluster;      // the wave can run as ONE thread-block cluster (<= 16 CTAs): exchange through distributed shared memory
     };
@@ -520,7 +524,8 @@ void fill_init_params(top_solver* h, InitParams& ip) {
     ip.invTk2 = h->d_invTk2;
     ip.zt = h->d_zt; ip.chat = h->d_chat; ip.qp = h->d_qp; ip.qn = h->d_qn; ip.phv = h->d_phv; ip.segflags = h->d_segflags;
     ip.stride = h->stride; ip.nseg_pad = h->nseg_pad; ip.nseg = h->nseg; ip.N = h->N; ip.batch = h->batch; ip.s = h->s; ip.dims = h->dims;
-    ip.hard = h->wp_mode == TOP_WAYPOINT_HARD; ip.has_box = h->has_box; ip.has_vel = h->has_vel; ip.has_acc = h->has_acc;
+    ip.hard = h->wp_mode == TOP_WAYPOINT_HARD; ip.has_box = h->has_box;
+    ip.has_vel = h->has_vel && !h->numeric; ip.has_acc = h->has_acc && !h->numeric;
     ip.vmax = h->vmax;
     ip.rot = h->d_rot; ip.planes = h->d_planes; ip.lam3 = h->d_lam3; ip.qpl = h->d_qpl; ip.K = h->K; ip.has_poly = h->has_poly;
 }
@@ -644,7 +649,8 @@ top_status fill_problem(top_solver* h, const double* waypoints, const double* du
         pp.gram = reinterpret_cast<const GramDD*>(h->d_upload + h->off_gram);
         pp.durations = reinterpret_cast<const double*>(h->d_upload + h->off_T);
         pp.Pm = h->d_Pm; pp.stride = h->stride; pp.nseg = h->nseg; pp.N = h->N; pp.s = h->s;
-        pp.hard = h->wp_mode == TOP_WAYPOINT_HARD; pp.box = h->has_box; pp.vel = h->has_vel; pp.acc = h->has_acc; pp.wide = h->wide;
+        pp.hard = h->wp_mode == TOP_WAYPOINT_HARD; pp.box = h->has_box; pp.wide = h->wide;
+        pp.vel = h->has_vel && !h->numeric; pp.acc = h->has_acc && !h->numeric;      // NumericSolve: H0 is the quadratic part only
         pp.rho = h->rho; pp.bad = h->d_abort + 1;
         CU(launch_precompute_operator(pp, h->stream), "operator precompute launch");
         h->launches += 1;
@@ -836,6 +842,9 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->vmax = has_vel ? cons->vmax : 0; h->amax = has_acc ? cons->amax : 0;
     h->wp_mode = mode;
     h->wide = (o.flags & TOP_CONSENSUS_WIDE) != 0;
+    h->numeric = (o.flags & TOP_XUPDATE_NUMERIC) != 0;
+    if (h->numeric && (dtype != TOP_F64 || h->has_poly || h->wide || (o.flags & TOP_RHO_ADAPTIVE)))
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_XUPDATE_NUMERIC: TOP_F64 only, no polytope corridor, no TOP_CONSENSUS_WIDE, no TOP_RHO_ADAPTIVE"));
     h->nc = h->wide ? 2 * s - 1 : s;
     if (o.adapt_mu > 0) h->adapt_mu = o.adapt_mu;
     if (o.adapt_tau_incr > 0) h->adapt_incr = o.adapt_tau_incr;
@@ -852,6 +861,15 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     int coop = 0;
     cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
     if (!coop) CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "device lacks cooperative launch"));
+    if (h->numeric) {
+        // NumericSolve branch: the state lives in device memory and a sweep is two plain launches (no on-chip capacity,
+        // no cooperative grid): one "wave" that only describes the x-update launch for top_launch_info
+        top_solver::Wave w;
+        w.seg_begin = 0; w.seg_end = nseg; w.own_begin = 0; w.own_end = nseg; w.kflags = 0;
+        w.segs_per_cta = 64; w.ctas = (int)((nseg + 63) / 64); w.threads = 64; w.smem = 0; w.cluster = false;
+        h->waves.push_back(w);
+        h->lanes = 8; h->mma = false; h->max_ctas = h->num_sms;
+    } else {
     // fp32: 8 lanes per segment unless told otherwise; 4 lanes (twice the registers per thread, two samples per lane) win
     // once every SM is full of segments (measured on config 5: 4.1e9 vs 3.3e9 segment-iterations/s)
     h->lanes = o.lanes_per_segment ? o.lanes_per_segment : 8;
@@ -949,6 +967,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
             cudaGetLastError();
         }
 
+    }
     pt.mark("launch plan");
 
     // ---- memory: one device arena, one host staging buffer
@@ -982,7 +1001,9 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     const size_t o_zero = cv.off;
     const size_t o_u = cv.take(3 * LS * rb), o_wv = cv.take(has_vel ? 3 * LS * rb : 0), o_pha = cv.take(has_acc ? 3 * LS * rb : 0),
                  o_wa = cv.take(has_acc ? 3 * LS * rb : 0), o_part = cv.take(NP * 4 * 8), o_res = cv.take((size_t)batch * 4 * 8),
-                 o_solve = cv.take(64), o_zt2 = cv.take(h->wide ? 3 * LS * rb : 0), o_u2 = cv.take(h->wide ? 3 * LS * rb : 0);
+                 o_solve = cv.take(64), o_zt2 = cv.take(h->wide ? 3 * LS * rb : 0), o_u2 = cv.take(h->wide ? 3 * LS * rb : 0),
+                 o_yv = cv.take(h->numeric ? LS * 8 : 0), o_ya = cv.take(h->numeric ? LS * 8 : 0), o_bnd = cv.take(h->numeric ? 3 * LS * 8 : 0),
+                 o_inner = cv.take(h->numeric ? 16 : 0);      // u64 iteration count + u32 work-queue counter
     size_t o_alt[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     if (h->streaming) {
         const bool on[8] = {true, true, has_box, has_box, has_vel, has_vel, has_acc, has_acc};
@@ -1009,6 +1030,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->d_u = A + o_u; h->d_part = (double*)(A + o_part); h->d_res = (double*)(A + o_res); h->d_solve = (double*)(A + o_solve);
     if (has_box) { h->d_qp = A + o_qp; h->d_qn = A + o_qn; }
     if (h->wide) { h->d_invTk2 = A + o_invTk2; h->d_zt2 = A + o_zt2; h->d_u2 = A + o_u2; }
+    if (h->numeric) { h->d_yv = (double*)(A + o_yv); h->d_ya = (double*)(A + o_ya); h->d_bnd = (double*)(A + o_bnd); h->d_inner = (unsigned long long*)(A + o_inner); }
     if (h->has_poly) {
         h->d_rot = (double*)(A + h->off_rot); h->d_planes = (double*)(A + h->off_planes); h->d_lam3 = (double*)(A + h->off_lam3);
         h->d_qpl = (double*)(A + o_qpl);
@@ -1106,6 +1128,24 @@ struct InKernelSolve { int check_every; int rd_sel; int adaptive; double tol; };
 
 top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullptr) {
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
+    if (h->numeric) {      // NumericSolve branch: x-update kernel + consensus kernel per sweep, state in device memory
+        NumParams np;
+        std::memset(&np, 0, sizeof np);
+        np.Pm = h->d_Pm; np.invT = (const double*)h->d_invT; np.lohi = (const double*)h->d_lohi; np.origin = h->d_origin;
+        np.segflags = h->d_segflags; np.zoff = (const double*)h->d_zoff; np.Tpow = (const double*)h->d_Tpow;
+        np.zt = (double*)h->d_zt; np.u = (double*)h->d_u; np.qp = (double*)h->d_qp; np.qn = (double*)h->d_qn; np.chat = (double*)h->d_chat;
+        np.yv = h->d_yv; np.ya = h->d_ya; np.bnd = h->d_bnd; np.part = h->d_part; np.inner_iters = h->d_inner;
+        np.work_counter = reinterpret_cast<unsigned int*>(h->d_inner + 1); np.max_blocks = 3 * h->num_sms;
+        np.stride = h->stride; np.nseg_pad = h->nseg_pad; np.nseg = h->nseg; np.s = h->s; np.hard = h->wp_mode == TOP_WAYPOINT_HARD;
+        np.flags = h->kflags & (KF_BOX | KF_VEL | KF_ACC | KF_PIN_POS); np.rho = h->rho; np.vmax = h->vmax; np.amax = h->amax;
+        for (int64_t i = 0; i < k; ++i) CU(launch_numeric_sweep(np, h->stream), "numeric sweep launch");
+        h->launches += 2 * k;
+        h->iter += k;
+        CU(launch_residual_reduce(h->d_part, h->d_res, h->N, h->batch, h->stream), "residual reduction launch");
+        h->launches += 1;
+        h->have_residuals = true;
+        return TOP_OK;
+    }
     while (k > 0) {
         // streaming: at most `halo` sweeps per launch (that is how far a piece can run before the staleness of
         // its halo reaches the segments it owns)
@@ -1198,7 +1238,7 @@ extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iter
     const int rd_idx = (h->opt_flags & TOP_RD_NORMALISED) ? 2 : 1;
     // (large CTAs run the plain kernel faster than the solve instantiation -- 96-register cap -- so with a sparse
     // test cadence they keep the host loop below)
-    if (h->batch == 1 && h->waves.size() == 1 && !h->streaming && !h->has_poly && (h->lanes == 8 || h->mma) && h->waves[0].ctas <= 160 &&
+    if (h->batch == 1 && h->waves.size() == 1 && !h->streaming && !h->has_poly && !h->numeric && (h->lanes == 8 || h->mma) && h->waves[0].ctas <= 160 &&
         (h->waves[0].threads <= 256 || h->check_every < 16)) {
         // one resident trajectory: the stop rule (and Eq. 24) runs inside the kernel, one launch for the whole solve
         InKernelSolve iks;
@@ -1255,6 +1295,7 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
     if (!h) return TOP_E_INVALID;
     if (!(rho > 0) || !std::isfinite(rho)) return fail(h, TOP_E_INVALID, "rho must be finite and > 0");
     if (rho == h->rho) return TOP_OK;
+    if (h->numeric) return fail(h, TOP_E_UNSUPPORTED, "top_set_rho is not built for TOP_XUPDATE_NUMERIC");
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     const size_t LS = (size_t)h->stride;
     if (h->has_poly) {
@@ -1355,6 +1396,15 @@ extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, do
             }
         return check_abort(h);
     }
+    if (f == "y_v" || f == "y_a") {       // scaled multipliers of Eq. 17 (NumericSolve branch), [batch][N][Ms]
+        const size_t want = (size_t)batch * N * MS;
+        if (!h->numeric || count != want) return fail(h, TOP_E_INVALID, "top_get_state: count does not match the field (or not a TOP_XUPDATE_NUMERIC solver)");
+        buf.resize(LS);
+        CU(cudaMemcpyAsync(buf.data(), f == "y_v" ? h->d_yv : h->d_ya, LS * 8, cudaMemcpyDeviceToHost, h->stream), "D2H");
+        CU(cudaStreamSynchronize(h->stream), "sync");
+        for (size_t g = 0; g < (size_t)batch * N; ++g) for (int j = 0; j < MS; ++j) out[g * MS + j] = buf[g * LANES + j];
+        return check_abort(h);
+    }
     if (f == "s_poly" || f == "v_poly") {
         const size_t want = (size_t)batch * N * MS * (size_t)h->K;
         if (!h->has_poly || count != want) return fail(h, TOP_E_INVALID, "top_get_state: count does not match the field (or no polytope corridor)");
@@ -1421,7 +1471,7 @@ int snapshot_fields(top_solver* h, void** out) {
 }  // namespace
 
 extern "C" TOP_API size_t top_snapshot_bytes(const top_solver* hc) {
-    if (!hc) return 0;
+    if (!hc || hc->numeric) return 0;      // (snapshots are not built for TOP_XUPDATE_NUMERIC: save / restore then reject every size)
     top_solver* h = const_cast<top_solver*>(hc);
     void* f[11];
     const int n = snapshot_fields(h, f);
@@ -1493,6 +1543,16 @@ extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* ho
 }
 
 extern "C" TOP_API int64_t top_iteration(const top_solver* h) { return h ? h->iter : -1; }
+
+extern "C" TOP_API top_status top_numeric_info(top_solver* h, int64_t* inner_iterations) {
+    if (!h) return TOP_E_INVALID;
+    if (!h->numeric) return fail(h, TOP_E_INVALID, "top_numeric_info: not a TOP_XUPDATE_NUMERIC solver");
+    unsigned long long v = 0;
+    CU(cudaMemcpyAsync(&v, h->d_inner, 8, cudaMemcpyDeviceToHost, h->stream), "D2H");
+    CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
+    if (inner_iterations) *inner_iterations = (int64_t)v;
+    return TOP_OK;
+}
 
 extern "C" TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas, int32_t* threads, int32_t* segs_per_cta,
                                       int32_t* smem_bytes, int32_t* waves, int64_t* launches) {

@@ -143,6 +143,28 @@ struct PrecompParams {
     int* bad;                     // set to 1 when a segment's operator is not positive definite
 };
 cudaError_t launch_precompute_operator(const PrecompParams& p, cudaStream_t st);
+// NumericSolve branch (top_kernels_numeric.cu): one sweep = x-update kernel + consensus kernel.  fp64 only.
+struct NumParams {
+    const double* Pm;         // [MAXN][stride] rho * Pm^ rows of the QUADRATIC part (no ball terms)
+    const double* invT;       // [2][nseg_pad]
+    const double* lohi;       // [6][nseg_pad]
+    const double* origin;     // [3][nseg_pad]
+    const uint8_t* segflags;
+    const double* zoff;       // [3][stride]
+    const double* Tpow;       // [stride]
+    double *zt, *u, *qp, *qn, *chat;   // [3][stride] each (qp, qn: box only)
+    double *yv, *ya;          // [stride] scaled multipliers of Eq. 17 (lane j = sample j)
+    double* bnd;              // [3][stride] boundary rows B = M c of the newest coefficients
+    double* part;             // [nseg_pad][4]
+    unsigned long long* inner_iters;   // L-BFGS iterations, summed over segments and sweeps
+    unsigned int* work_counter;        // work queue of the x-update kernel (next segment to fetch; reset by the consensus kernel)
+    int max_blocks;                    // persistent grid of the x-update kernel: CTAs that are co-resident (3 per SM)
+    long long stride, nseg_pad, nseg;
+    int s, hard;
+    uint32_t flags;           // KF_BOX | KF_VEL | KF_ACC | KF_PIN_POS
+    double rho, vmax, amax;
+};
+cudaError_t launch_numeric_sweep(const NumParams& p, cudaStream_t st);
 // Init of Alg. 1 (PAPER.md:L270 line 1, L301; reading A9) on the device: from the caller's arrays (uploaded as they are)
 // and the per-segment operator rows, every per-lane constant and iterate 0.
 struct InitParams {

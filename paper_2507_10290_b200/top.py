@@ -23,10 +23,11 @@ TOP_EPS_N_SCALED = 8
 TOP_RHO_ADAPTIVE = 64
 TOP_KERNEL_NO_MMA = 128
 TOP_CONSENSUS_WIDE = 256
+TOP_XUPDATE_NUMERIC = 512
 SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
 EXPORTS = ["top_create", "top_reset", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
-           "top_snapshot_bytes", "top_snapshot_save", "top_snapshot_restore", "top_iteration", "top_set_rho", "top_get_rho", "top_launch_info", "top_memory_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
+           "top_snapshot_bytes", "top_snapshot_save", "top_snapshot_restore", "top_iteration", "top_numeric_info", "top_set_rho", "top_get_rho", "top_launch_info", "top_memory_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
            "top_destroy", "top_last_error"]
 
 
@@ -90,6 +91,8 @@ def lib():
     L.top_snapshot_save.argtypes = [vp, vp, ctypes.c_size_t]
     L.top_snapshot_restore.restype = ctypes.c_int
     L.top_snapshot_restore.argtypes = [vp, vp, ctypes.c_size_t]
+    L.top_numeric_info.restype = ctypes.c_int
+    L.top_numeric_info.argtypes = [vp, ctypes.POINTER(ctypes.c_int64)]
     L.top_iteration.restype = ctypes.c_int64
     L.top_iteration.argtypes = [vp]
     L.top_launch_info.restype = ctypes.c_int
@@ -158,7 +161,7 @@ class TopSolver:
     def __init__(self, waypoints, durations, s, rho, dtype="f64", samples=0, box_lo=None, box_hi=None, vmax=0.0,
                  amax=0.0, start_derivs=None, end_derivs=None, mode="hard", rd_normalised=False, eps_n_scaled=False,
                  sync="auto", check_every=0, max_iter=0, device=-1, stream=0, segs_per_cta=0, lanes=0, adaptive_rho=False,
-                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0, no_mma=False, planes=None, consensus="s"):
+                 adapt_mu=0.0, adapt_tau_incr=0.0, adapt_tau_decr=0.0, no_mma=False, planes=None, consensus="s", numeric=False):
         L = lib()
         wp = np.asarray(waypoints, dtype=np.float64)
         T = np.asarray(durations, dtype=np.float64)
@@ -190,7 +193,8 @@ class TopSolver:
             cons = _Constraints(int(samples), _dptr(lo), _dptr(hi), float(vmax), float(amax), self.K, _dptr(pl))
         flags = WAYPOINT[mode] | (TOP_RD_NORMALISED if rd_normalised else 0) | \
             (TOP_EPS_N_SCALED if eps_n_scaled else 0) | SYNC[sync] | (TOP_RHO_ADAPTIVE if adaptive_rho else 0) | \
-            (TOP_KERNEL_NO_MMA if no_mma else 0) | (TOP_CONSENSUS_WIDE if consensus == "wide" else 0)
+            (TOP_KERNEL_NO_MMA if no_mma else 0) | (TOP_CONSENSUS_WIDE if consensus == "wide" else 0) | \
+            (TOP_XUPDATE_NUMERIC if numeric else 0)
         opt = _Options(ctypes.sizeof(_Options), flags, int(check_every), int(device), int(max_iter),
                        ctypes.c_void_p(stream), int(segs_per_cta), int(lanes), float(adapt_mu), float(adapt_tau_incr),
                        float(adapt_tau_decr))
@@ -287,11 +291,19 @@ class TopSolver:
     def state(self, field: str):
         if field in ("s_poly", "v_poly"):
             shape = (self.batch, self.N, 8, self.K)
+        elif field in ("y_v", "y_a"):
+            shape = (self.batch, self.N, 8)
         else:
             shape = self._STATE_SHAPES.get(field, lambda o: (o.batch, o.N, 8, o.dims))(self)
         out = np.zeros(shape)
         self._check(self._L.top_get_state(self._h, field.encode(), _dptr(out), out.size))
         return out
+
+    def inner_iterations(self) -> int:
+        """top_numeric_info: L-BFGS iterations so far (NumericSolve branch)."""
+        v = ctypes.c_int64()
+        self._check(self._L.top_numeric_info(self._h, ctypes.byref(v)))
+        return v.value
 
     @property
     def iteration(self) -> int:
