@@ -883,10 +883,10 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     // short chains (the paper's regime, tens to a thousand segments): at most 16 CTAs run as ONE thread-block cluster and
     // exchange their boundary rows through distributed shared memory, which costs 0-0.25 us per sweep instead of the
     // 0.45-0.8 us of the L2 mailbox between 25-125 small CTAs (profiles/r2_small_configs_latency.md: config 2 1.60 -> 1.38 us,
-    // config 3 1.41 -> 1.24 us).  It pays as long as the per-CTA share stays small: <= 32 segments per CTA with inequality
+    // config 3 1.41 -> 1.24 us; fp32: config 3 1.30 -> 1.16 us).  It pays as long as the per-CTA share stays small: <= 32 segments per CTA with inequality
     // sets, <= 64 without.  Chains of <= 16 segments stay on one CTA.
     int plan_segs = 0;
-    if (dtype == TOP_F64 && !o.lanes_per_segment && !o.segs_per_cta && (o.flags & TOP_SYNC_MASK) == TOP_SYNC_AUTO &&
+    if (!o.lanes_per_segment && !o.segs_per_cta && (o.flags & TOP_SYNC_MASK) == TOP_SYNC_AUTO &&
         !(o.flags & TOP_KERNEL_NO_MMA) && !h->has_poly) {
         const bool cons_any = has_box || has_vel || has_acc;
         const long long per_cta_max = cons_any ? 32 : 64, per_cta_min = cons_any ? 16 : 32;
