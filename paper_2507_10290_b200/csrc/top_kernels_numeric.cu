@@ -174,7 +174,7 @@ __device__ __forceinline__ void lane_grad(const NumTables& t, const LaneCtx& k, 
     }
 }
 
-__global__ void __launch_bounds__(128, 4) numeric_xupdate_kernel(const NumParams p) {
+__global__ void __launch_bounds__(128, 3) numeric_xupdate_kernel(const NumParams p) {
     __shared__ NumTables tab;
     build_tables(tab, p.s);
     __syncthreads();
