@@ -1,5 +1,6 @@
 """`-m gpu`: seeded random sweep over the options of the CUDA path (sizes 1..300 incl. ragged CTAs, s, constraint subsets,
-dims, batch, rho, waypoint mode, lanes per segment, inter-CTA sync mode, segments per CTA, launch chunking) against the
+dims, batch, rho, waypoint mode, lanes per segment (or the planner's own choice), inter-CTA sync mode ("auto": one
+thread-block cluster when the launch is <= 16 CTAs), segments per CTA, launch chunking, consensus width) against the
 oracle run in long double; every state field of every compared iterate within 1e-9 norm-relative."""
 import numpy as np
 import pytest
@@ -12,7 +13,7 @@ from tests.parity_util import field_errors, make_oracle, sampled_positions
 pytestmark = pytest.mark.gpu
 
 
-@pytest.mark.parametrize("seed", [2, 3])
+@pytest.mark.parametrize("seed", [2, 3, 4])
 def test_random_option_sweep(seed):
     top_build.build()
     rng = np.random.default_rng(seed)
@@ -32,18 +33,23 @@ def test_random_option_sweep(seed):
         mode = str(rng.choice(["hard", "hard", "pinned_z", "free"]))
         lanes = int(rng.choice([8, 4])); sync = str(rng.choice(["pairwise", "neighbour", "grid"]))
         segs = int(rng.choice([0, 4, 8, 16]))
+        extra = {}
+        if seed >= 4:      # the later additions: planner's own lane choice, cluster exchange, paper-literal consensus
+            lanes = int(rng.choice([0, 4])); sync = str(rng.choice(["auto", "auto", "pairwise"]))
+            if rng.integers(3) == 0:
+                lanes = int(rng.choice([0, 4])); extra = {"consensus": "wide"}
         ks = [int(k) for k in rng.integers(1, 40, size=3)]
-        sol = top.from_workload(w, mode=mode, lanes=lanes, sync=sync, segs_per_cta=segs, dtype="f64")
-        oracles = [make_oracle(w, b, mode=mode, long_double=True) for b in range(batch)]
+        sol = top.from_workload(w, mode=mode, lanes=lanes, sync=sync, segs_per_cta=segs, dtype="f64", **extra)
+        oracles = [make_oracle(w, b, mode=mode, long_double=True, **extra) for b in range(batch)]
         for k in ks:
             sol.iterate(k)
             for o in oracles:
                 o.sweep(k, 1)
             for name, v in field_errors(sol, oracles, w).items():
                 tol = 1e-6 if name.startswith("resself_") else 1e-9
-                assert v < tol, (case, name, v, N, s, acc, batch, dims, cons, w.rho, mode, lanes, sync, segs, ks)
+                assert v < tol, (case, name, v, N, s, acc, batch, dims, cons, w.rho, mode, lanes, sync, segs, ks, extra)
         sol.close()
-        if case % 4 == 0 and w.samples:      # the fp32 (mixed) variant on the same case: sampled positions, 1e-3 m
+        if case % 4 == 0 and w.samples and not extra:      # the fp32 (mixed) variant on the same case: sampled positions, 1e-3 m
             sol = top.from_workload(w, mode=mode, lanes=lanes, sync=sync, segs_per_cta=segs, dtype="f32")
             sol.iterate(sum(ks))
             for b, o in enumerate(oracles):
