@@ -223,9 +223,10 @@ TOP_API top_status top_get_residuals(top_solver* h, double* r_primal, double* r_
 TOP_API top_status top_get_coeffs(top_solver* h, void* out, int32_t out_is_device);
 
 /* top_get_state -- one field of the current iterate as host fp64 (parity tests, warm-start snapshots).
- * field / layout:  "z" [batch][N+1][s][dims]   "u" [batch][N][2s][dims]
+ * field / layout:  "z" [batch][N+1][n_c][dims]   "u" [batch][N][2 n_c][dims]      (n_c = s, or 2s-1 with TOP_CONSENSUS_WIDE)
  *                  "s_pos","s_neg","v_pos","v_neg","phi_v","w_v","phi_a","w_a" [batch][N][Ms][dims]
  *                  "s_poly","v_poly" [batch][N][Ms][K]   (polytope corridor: slack / scaled dual per (sample, plane))
+ *                  "y_v","y_a" [batch][N][Ms]            (TOP_XUPDATE_NUMERIC: scaled multipliers of Eq. 17)
  * count = number of doubles `out` holds; TOP_E_INVALID if it does not match or the field is unknown. */
 TOP_API top_status top_get_state(top_solver* h, const char* field, double* out, size_t count);
 
@@ -253,7 +254,8 @@ TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas, int32_t* 
                            int32_t* smem_bytes, int32_t* waves, int64_t* launches);
 
 /* Memory facts of this solver; any pointer may be NULL: bytes of its (single) device allocation, and the bytes that
- * top_create / top_reset copy host-to-device per problem (the x-update operator rows + the caller's arrays). */
+ * top_create / top_reset copy host-to-device per problem (the caller's arrays and 14 KB of Gram tables; with a polytope
+ * corridor also the operator rows, which are then computed on the host). */
 TOP_API top_status top_memory_info(const top_solver* h, int64_t* device_bytes, int64_t* h2d_bytes_per_problem);
 
 /* Largest N (segments of ONE trajectory) the persistent kernel can hold ON CHIP on the given device (longer
@@ -267,8 +269,9 @@ TOP_API int64_t top_capacity(int32_t device, int32_t s, top_dtype dtype, int32_t
  * Runs `reps` launches on `stream` and returns the best.  < 0 on error. */
 TOP_API double top_fma_peak(int32_t device, top_dtype dtype, int32_t reps, void* cuda_stream);
 
-/* top_precompute_operator -- the host-side precompute top_create runs per segment, exposed so that it can
- * be checked without a device (it launches nothing): the x-update operator of Eq. 20a in the
+/* top_precompute_operator -- the host twin (extended precision) of the per-segment operator precompute that top_create
+ * runs in a kernel (and on the host for polytope corridors and for the spectral form behind top_set_rho), exposed so that
+ * it can be checked without a device (it launches nothing): the x-update operator of Eq. 20a in the
  * library's internal normalised-time basis c^_a = c_a T^a, for one segment of duration T between waypoints
  * p0, p1 (host [3]):  c^ = Pm_hat (rho R^) + c0_hat.   Pm_hat host [8][8] row-major (zero padded beyond 2s),
  * c0_hat host [8][3].  flags: TOP_WAYPOINT_*.  box/vel/acc != 0 enable the constraint blocks (8 samples). */
