@@ -530,6 +530,23 @@ def main():
                              "unit": "TFLOP/s", "frac": fl_w * ww.N * 2000 / (msw * 1e-3) / peaks["f64"],
                              "flops_per_segment_sweep": fl_w}}
             sw.close()
+            # polytope corridors (K = 8 half-spaces per segment) and the paper's literal configuration: polytope
+            # corridor + 2s-1 consensus orders + free waypoints, each at its on-chip capacity
+            for tag, Np, kwp in (("polytopeK8", 5920, {}), ("polytopeK8_wide_consensus_free", 4736, {"consensus": "wide", "mode": "free"})):
+                wp_ = W.polytope_corridor(W.config4(seed=1004 + rank, N=Np), K=8, seed=3)
+                sp_ = top.from_workload(wp_, device=local_rank, stream=stream.cuda_stream, sync=args.sync, **kwp)
+                sp_.iterate(500); torch.cuda.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record(stream); sp_.iterate(2000); e1.record(stream); torch.cuda.synchronize()
+                msp = e0.elapsed_time(e1)
+                lip = sp_.launch_info()
+                fl_p = 3970.0 + 128.0 * 8 + 240.0 + (612.0 if kwp else 0.0)
+                others["cfg4shape_N%d_snap_f64_%s" % (Np, tag)] = {
+                    "segment_iterations_per_s": Np * 2000 / (msp * 1e-3), "sweeps": 2000, "us_per_sweep_per_wave": 1e3 * msp / 2000,
+                    "dtype": "f64", "ctas": lip["ctas"], "threads": lip["threads"], "waves": lip["waves"],
+                    "roofline": {"bound": "alu", "achieved": fl_p * Np * 2000 / (msp * 1e-3) / 1e12, "peak": peaks["f64"] / 1e12,
+                                 "unit": "TFLOP/s", "frac": fl_p * Np * 2000 / (msp * 1e-3) / peaks["f64"], "flops_per_segment_sweep": fl_p}}
+                sp_.close()
             # the NumericSolve branch of Alg. 1 (Eq. 15-17: L-BFGS x-update) on config 4's input
             wn = make_workload("cfg4", rank)
             sn = top.from_workload(wn, device=local_rank, stream=stream.cuda_stream, numeric=True)

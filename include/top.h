@@ -91,8 +91,8 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
  * x-update is over-determined; L259-264): orders 0..2s-2, i.e. n_c = 2s-1 rows per boundary; z_0 and z_N carry the given
  * end state (orders 0..s-1, Eq. 2c), so the orders s..2s-2 do not exist at the two trajectory ends.
  * top_get_state "z" is then [batch][N+1][2s-1][dims] and "u" [batch][N][2(2s-1)][dims] (rows that do not exist read 0).
- * TOP_F64 on the tensor-core kernel only, no polytope corridor, the trajectory must fit on chip (N <= 148 x 56);
- * else TOP_E_UNSUPPORTED. */
+ * TOP_F64 on the tensor-core kernel only; the trajectory must fit on chip (N <= 148 x 56; together with a polytope corridor
+ * N <= 148 x 32); else TOP_E_UNSUPPORTED. */
 #define TOP_CONSENSUS_WIDE    256u
 /* x-update branch of Alg. 1 (PAPER.md:L266-270 lines 4-8).  Default: ClosedFormSolve (Eq. 20a, 20f, 20g).
  * TOP_XUPDATE_NUMERIC: NumericSolve (Eq. 15-17; L303) -- the ball sets ||sigma'|| <= vmax, ||sigma''|| <= amax

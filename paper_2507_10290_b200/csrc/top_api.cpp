@@ -578,7 +578,7 @@ top_status stage_operators(top_solver* h) {
                 for (int q = 0; q < 9; ++q) rot_st[(size_t)q * NP + g] = (double)V[q];
                 for (int d = 0; d < 3; ++d) {
                     lam_st[(size_t)d * NP + g] = (double)lam[d];
-                    if (!build_operator(s, (xreal)Td, rho, true, vel, acc, mode, nullptr, nullptr, Pm, nullptr, lam[d])) { bad_operator.store(1); return; }
+                    if (!build_operator(s, (xreal)Td, rho, true, vel, acc, mode, nullptr, nullptr, Pm, nullptr, lam[d], wmask)) { bad_operator.store(1); return; }
                     for (int lane = 0; lane < n; ++lane)
                         for (int b = 0; b < n; ++b)
                             Pm_st[((size_t)d * MAXN + b) * LS + (size_t)g * LANES + lane] = (double)(rho * Pm[lane * MAXN + b]);
@@ -898,8 +898,8 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     if (h->lanes == 4 && (o.flags & TOP_KERNEL_NO_MMA))
         CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_KERNEL_NO_MMA: the shuffle form of the 4-lane kernel was removed (use lanes_per_segment = 8 for a kernel without tensor-core contractions)"));
     h->mma = h->lanes == 4;
-    if (h->wide && (!(h->mma && dtype == TOP_F64) || h->has_poly))
-        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_CONSENSUS_WIDE runs on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA, no polytope corridor)"));
+    if (h->wide && !(h->mma && dtype == TOP_F64))
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_CONSENSUS_WIDE runs on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA)"));
     if (h->has_poly && !(h->mma && dtype == TOP_F64))
         CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "polytope corridors run on the fp64 tensor-core kernel only (TOP_F64, lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA)"));
     const int segs_max = max_segs_per_cta(h->dtype, s, h->constrained, h->lanes, h->mma, (size_t)smem_optin - 8192, h->has_poly, h->wide);

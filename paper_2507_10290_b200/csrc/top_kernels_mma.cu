@@ -129,6 +129,8 @@ constexpr int MAXT_MMA_POLY = 160;
 // paper-literal consensus n_c = 2s-1 (reading A1): a second block of consensus rows per segment (orders s..2s-2 at both
 // boundaries: (z~, u) pairs, boundary-row buffer, mailbox slots); <= 224 threads (7 warps: 56 segments)
 constexpr int MAXT_MMA_WIDE = 224;
+// both at once (the paper's literal configuration: FIRI polytope corridor + 2s-1 consensus orders): <= 128 threads (32 segments)
+constexpr int MAXT_MMA_POLY_WIDE = 128;
 constexpr int PSTR = KMAX * 4 + 2;      // doubles per segment of the plane table (padded: the 8 segments of a warp hit distinct banks)
 constexpr int VSTR = 10;                // doubles per segment of the rotation table
 
@@ -193,7 +195,6 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     // lane <-> row map: lane t owns order s+t at the start boundary (item h = 0) and at the end boundary (h = 1), t <= s-2.
     // Rows that do not exist (t = s-1; the trajectory ends, where z_0 / z_N carry orders < s only) have 1/T^k = 0 in
     // invTk2: their operand, boundary value, residual and dual are identically 0.
-    static_assert(!(WIDE && POLY), "wide consensus is not instantiated for polytope corridors");
     constexpr int MBS = WIDE ? 48 : 24;              // mailbox slots per CTA and parity: [2 sides][4 or 8 orders][3 dims]
     constexpr int LPS = 4;                         // lanes per segment
     constexpr bool CONS = CM != 0 || POLY;
@@ -442,6 +443,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             rot_in(vs, gM[h]);
+            if (WIDE) rot_in(vs, gM2[h]);
             for (int k = 0; k < KP; ++k) {
                 const double2 a01 = *reinterpret_cast<const double2*>(pls + k * 4), a2b = *reinterpret_cast<const double2*>(pls + k * 4 + 2);
                 const double g = a2b.y - fabs(qpls[(k * 2 + h) * TS]);
@@ -602,6 +604,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
 #pragma unroll
                 for (int d = 0; d < 3; ++d) { Bnd2[0][d] = (Real)e.get(d, 0) * invTk2[0]; Bnd2[1][d] = (Real)e.get(d, 1) * invTk2[1]; }
             }
+            if constexpr (POLY) { rot_out(vs, Bnd2[0]); rot_out(vs, Bnd2[1]); }      // consensus lives in the global frame
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 if (isrow2) {
@@ -828,6 +831,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                         if (gaprow2[h]) { const double gp = (double)own2 - (double)nb2; gap2 += gp * gp; }   // Eq. 21
                     }
                 }
+            if constexpr (POLY) { rot_in(vs, gM2[0]); rot_in(vs, gM2[1]); }
         }
         if (last_sweep) {
             // a6: dual residual rho M(T)'(z~^{k+1} - z~^k) in monomial physical-time coefficient space (Eq. 22, A8):
@@ -1056,6 +1060,18 @@ cudaError_t launch_mma_poly(const KParams& p, int ctas, int threads, size_t smem
     return launch_any(kern, p, ctas, threads, smem, st);
 }
 template <int S>
+cudaError_t launch_mma_poly_wide(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
+    auto kern = cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_POLY_WIDE, false, true, true>;
+    return launch_any(kern, p, ctas, threads, smem, st);
+}
+template <int S>
+cudaError_t limits_mma_poly_wide(int threads, size_t smem, int* per_sm) {
+    auto kern = cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_POLY_WIDE, false, true, true>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads, smem);
+}
+template <int S>
 cudaError_t limits_mma_poly(int threads, size_t smem, int* per_sm) {
     auto kern = cadmm_sweeps_mma_kernel<double, S, CM_RUNTIME, MAXT_MMA_POLY, false, true>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -1083,12 +1099,15 @@ int mma_mask(uint32_t kflags) {
         else        { if (cm == 0) { CALL(float, 4, 0, MAXT_MMA_F32) } else if (cm == 3) { CALL(float, 4, 3, MAXT_MMA_F32) } else if (cm == 7) { CALL(float, 4, 7, MAXT_MMA_F32) } else { CALL(float, 4, CM_RUNTIME, MAXT_MMA_F32) } } \
     }
 
-int max_threads_mma(int dtype, bool poly, bool wide) { return wide ? MAXT_MMA_WIDE : poly ? MAXT_MMA_POLY : (dtype == 0 ? MAXT_MMA : MAXT_MMA_F32); }
+int max_threads_mma(int dtype, bool poly, bool wide) {
+    return poly && wide ? MAXT_MMA_POLY_WIDE : wide ? MAXT_MMA_WIDE : poly ? MAXT_MMA_POLY : (dtype == 0 ? MAXT_MMA : MAXT_MMA_F32);
+}
 
 cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st) {
     const uint32_t kflags = p.flags;
     if (kflags & KF_POLY) {
         if (p.check_every > 0 || dtype != 0) return cudaErrorInvalidValue;      // host loop only, fp64 only
+        if (kflags & KF_WIDE) return s == 3 ? launch_mma_poly_wide<3>(p, ctas, threads, smem, st) : launch_mma_poly_wide<4>(p, ctas, threads, smem, st);
         return s == 3 ? launch_mma_poly<3>(p, ctas, threads, smem, st) : launch_mma_poly<4>(p, ctas, threads, smem, st);
     }
     if (kflags & KF_WIDE) {
@@ -1102,6 +1121,7 @@ cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int 
 }
 
 cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm) {
+    if ((kflags & KF_POLY) && (kflags & KF_WIDE)) return s == 3 ? limits_mma_poly_wide<3>(threads, smem, max_ctas_per_sm) : limits_mma_poly_wide<4>(threads, smem, max_ctas_per_sm);
     if (kflags & KF_POLY) return s == 3 ? limits_mma_poly<3>(threads, smem, max_ctas_per_sm) : limits_mma_poly<4>(threads, smem, max_ctas_per_sm);
     if (kflags & KF_WIDE) return s == 3 ? limits_mma_wide<3>(threads, smem, max_ctas_per_sm) : limits_mma_wide<4>(threads, smem, max_ctas_per_sm);
 #define CALL(R_, S_, C_, M_) return limits_mma<R_, S_, C_, M_>(threads, smem, max_ctas_per_sm);
@@ -1114,6 +1134,9 @@ cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threa
 cudaError_t sweep_cluster_limits_mma(int dtype, int s, uint32_t kflags, int ctas, int threads, size_t smem, int* nclusters) {
     *nclusters = 0;
     if (ctas < 2 || ctas > 16) return cudaSuccess;
+    if ((kflags & KF_POLY) && (kflags & KF_WIDE))
+        return s == 3 ? cluster_query(cadmm_sweeps_mma_kernel<double, 3, CM_RUNTIME, MAXT_MMA_POLY_WIDE, false, true, true>, ctas, threads, smem, nclusters)
+                      : cluster_query(cadmm_sweeps_mma_kernel<double, 4, CM_RUNTIME, MAXT_MMA_POLY_WIDE, false, true, true>, ctas, threads, smem, nclusters);
     if (kflags & KF_POLY)
         return s == 3 ? cluster_query(cadmm_sweeps_mma_kernel<double, 3, CM_RUNTIME, MAXT_MMA_POLY, false, true>, ctas, threads, smem, nclusters)
                       : cluster_query(cadmm_sweeps_mma_kernel<double, 4, CM_RUNTIME, MAXT_MMA_POLY, false, true>, ctas, threads, smem, nclusters);
@@ -1134,6 +1157,7 @@ cudaError_t sweep_cluster_limits_mma(int dtype, int s, uint32_t kflags, int ctas
 }
 
 size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly, bool wide) {      // laid out for the largest CTA of the instantiation (see the kernel)
+    if (wide && poly) return smem_layout_mma(true, MAXT_MMA_POLY_WIDE / 4, true, 8, true).total;
     if (wide) return smem_layout_mma(true, MAXT_MMA_WIDE / 4, false, 8, true).total;      // (run-time constraint mask: laid out with the constraint arrays)
     if (poly) return smem_layout_mma(true, MAXT_MMA_POLY / 4, true).total;
     return dtype == 0 ? smem_layout_mma(constrained, MAXT_MMA / 4).total : smem_layout_mma(constrained, MAXT_MMA_F32 / 4, false, 4).total;

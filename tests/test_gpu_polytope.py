@@ -131,3 +131,18 @@ def test_polytope_unsupported_combinations():
     with pytest.raises(top.TopError) as e:
         top.from_workload(w17)
     assert e.value.status == top.TOP_E_UNSUPPORTED
+
+
+@pytest.mark.parametrize("s,acc,K,segs,mode", [(4, True, 7, 8, "free"), (3, False, 5, 0, "hard"), (4, True, 12, 16, "pinned_z")])
+def test_polytope_with_paper_literal_consensus(s, acc, K, segs, mode):
+    """The paper's literal configuration: polytope corridor cells (L222) + 2s-1 consensus orders (L231) + free waypoints
+    (Alg. 1 verbatim): the POLY + WIDE instantiation against the oracle's coupled operator with its wide consensus."""
+    w = W.polytope_corridor(W.small_constrained(N=45, s=s, acc=acc, seed=23), K=K, seed=6)
+    sol = top.from_workload(w, segs_per_cta=segs, mode=mode, consensus="wide")
+    o = poly_oracle(w, mode=mode, long_double=True, consensus="wide")
+    assert sol.state("z").shape[2] == 2 * s - 1
+    compare(sol, [o], w, "iterate 0")
+    done = 0
+    for cp in (1, 2, 3, 10, 50, 200):
+        sol.iterate(cp - done); o.sweep(cp - done); done = cp
+        compare(sol, [o], w, "sweep %d" % cp)
