@@ -120,7 +120,7 @@ typedef struct {
      * position at the `samples` sample times, one slack and one scaled dual per (sample, plane) (Eq. 20d, 20e).
      * planes: host [batch][N][K][dims+1] = (a_k (dims), b_k); normals need not be unit but must be non-zero.
      * Replaces the box (box_lo/box_hi must be NULL).  1 <= K <= 16; TOP_F64 with the tensor-core kernel only
-     * (lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA), N up to top_capacity_polytope; else TOP_E_UNSUPPORTED.
+     * (lanes_per_segment 0 or 4, no TOP_KERNEL_NO_MMA), N up to 40 segments per SM (5 920 on a B200); else TOP_E_UNSUPPORTED.
      * num_planes == 0: no polytope. */
     int32_t num_planes;
     const double* planes;
