@@ -101,8 +101,9 @@ typedef enum { TOP_F64 = 0, TOP_F32 = 1 } top_dtype;
  * (Eq. 17 added to Eq. 5 and to the slack penalty of the box, which keeps its slack form) with L-BFGS: memory 6, initial
  * inverse Hessian = the closed-form operator of the quadratic part, Armijo backtracking, stop when the step (proposed or taken) is below 1e-10
  * of the coefficients or after 50 iterations (the paper gives no parameters; reading A20 of DESIGN.md).
- * top_get_state "y_v" / "y_a" [batch][N][8] are the multipliers; "phi_*" / "w_*" read 0.  TOP_F64 only; no polytope
- * corridor, TOP_CONSENSUS_WIDE, TOP_RHO_ADAPTIVE, top_set_rho or snapshots (TOP_E_UNSUPPORTED / TOP_E_INVALID). */
+ * top_get_state "y_v" / "y_a" [batch][N][8] are the multipliers; "phi_*" / "w_*" read 0.  top_set_rho and TOP_RHO_ADAPTIVE
+ * work as in the closed-form branch (the multipliers are scaled duals: times rho_old / rho_new).  TOP_F64 only; no polytope
+ * corridor, TOP_CONSENSUS_WIDE or snapshots (TOP_E_UNSUPPORTED / TOP_E_INVALID). */
 #define TOP_XUPDATE_NUMERIC   512u
 
 /* The paper's convex sets, specialised as BASELINE.json's configs use them:

@@ -689,7 +689,8 @@ top_status ensure_spectral(top_solver* h) {
             for (long long g = g0; g < g1; ++g) {
                 const int wmask = h->wide ? ((g % h->N != 0 ? 1 : 0) | (g % h->N != h->N - 1 ? 2 : 0)) : 0;
                 if (durations[g] != cached_T || wmask != cached_mask) {
-                    if (!build_spectral(s, (xreal)durations[g], h->has_box, h->has_vel, h->has_acc, (int)h->wp_mode, zero3, SP, wmask)) { bad.store(1); return; }
+                    // (NumericSolve branch: the operator is the quadratic part only, the balls are not in it)
+                    if (!build_spectral(s, (xreal)durations[g], h->has_box, h->has_vel && !h->numeric, h->has_acc && !h->numeric, (int)h->wp_mode, zero3, SP, wmask)) { bad.store(1); return; }
                     cached_T = durations[g]; cached_mask = wmask;
                 }
                 for (int i = 0; i < MAXN; ++i) lamv[(size_t)i * NP + g] = i < SP.q ? (double)SP.lam[i] : 0.0;
@@ -843,8 +844,8 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->wp_mode = mode;
     h->wide = (o.flags & TOP_CONSENSUS_WIDE) != 0;
     h->numeric = (o.flags & TOP_XUPDATE_NUMERIC) != 0;
-    if (h->numeric && (dtype != TOP_F64 || h->has_poly || h->wide || (o.flags & TOP_RHO_ADAPTIVE)))
-        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_XUPDATE_NUMERIC: TOP_F64 only, no polytope corridor, no TOP_CONSENSUS_WIDE, no TOP_RHO_ADAPTIVE"));
+    if (h->numeric && (dtype != TOP_F64 || h->has_poly || h->wide))
+        CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_XUPDATE_NUMERIC: TOP_F64 only, no polytope corridor, no TOP_CONSENSUS_WIDE"));
     h->nc = h->wide ? 2 * s - 1 : s;
     if (o.adapt_mu > 0) h->adapt_mu = o.adapt_mu;
     if (o.adapt_tau_incr > 0) h->adapt_incr = o.adapt_tau_incr;
@@ -1295,7 +1296,6 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
     if (!h) return TOP_E_INVALID;
     if (!(rho > 0) || !std::isfinite(rho)) return fail(h, TOP_E_INVALID, "rho must be finite and > 0");
     if (rho == h->rho) return TOP_OK;
-    if (h->numeric) return fail(h, TOP_E_UNSUPPORTED, "top_set_rho is not built for TOP_XUPDATE_NUMERIC");
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     const size_t LS = (size_t)h->stride;
     if (h->has_poly) {
@@ -1314,6 +1314,7 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
         RescaleParams r;
         r.u = h->d_u; r.qp = nullptr; r.qn = nullptr; r.wv = h->d_wv; r.wa = h->d_wa;
         r.count = 3 * (long long)LS; r.ratio = old / rho; r.qpl = h->d_qpl; r.qpl_count = (long long)h->K * (long long)LS; r.u2 = nullptr;
+        r.yv = r.ya = nullptr; r.y_count = 0;
         CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
         h->launches += 2;
         return TOP_OK;
@@ -1321,8 +1322,10 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
     { top_status se = ensure_spectral(h); if (se != TOP_OK) return se; }      // first change of rho: build W, lambda (host, once)
     CU(refresh_operator(h, rho), "operator refresh launch");      // on the device, from the spectral data
     RescaleParams r;
+    r.yv = r.ya = nullptr; r.y_count = 0;
     r.u = h->d_u; r.qp = h->d_qp; r.qn = h->d_qn; r.wv = h->d_wv; r.wa = h->d_wa;
     r.count = 3 * (long long)LS; r.ratio = h->rho / rho; r.qpl = nullptr; r.qpl_count = 0; r.u2 = h->d_u2;
+    if (h->numeric) { r.wv = nullptr; r.wa = nullptr; r.yv = h->d_yv; r.ya = h->d_ya; r.y_count = (long long)LS; }      // multipliers of Eq. 17 are scaled duals too
     CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
     h->launches += 1;
     h->rho = rho;
@@ -1481,6 +1484,7 @@ extern "C" TOP_API size_t top_snapshot_bytes(const top_solver* hc) {
 
 extern "C" TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, size_t bytes) {
     if (!h) return TOP_E_INVALID;
+    if (h->numeric) return fail(h, TOP_E_UNSUPPORTED, "snapshots are not built for TOP_XUPDATE_NUMERIC");
     if (!host_buf || bytes != top_snapshot_bytes(h)) return fail(h, TOP_E_INVALID, "top_snapshot_save: buffer size must be top_snapshot_bytes()");
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(h, TOP_E_CUDA, "cudaSetDevice failed");
     SnapshotHeader hd;
@@ -1502,6 +1506,7 @@ extern "C" TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, s
 
 extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* host_buf, size_t bytes) {
     if (!h) return TOP_E_INVALID;
+    if (h->numeric) return fail(h, TOP_E_UNSUPPORTED, "snapshots are not built for TOP_XUPDATE_NUMERIC");
     if (!host_buf || bytes != top_snapshot_bytes(h)) return fail(h, TOP_E_INVALID, "top_snapshot_restore: buffer size does not match this solver");
     SnapshotHeader hd;
     std::memcpy(&hd, host_buf, sizeof hd);

@@ -195,7 +195,8 @@ struct InitParams {
 };
 cudaError_t launch_init(const InitParams& p, int dtype, cudaStream_t st);
 // duals *= ratio after a change of rho: u, w (both balls), and the negative part of the Moreau values q (= -v)
-struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; void* qpl; long long qpl_count; void* u2; };
+struct RescaleParams { void *u, *qp, *qn, *wv, *wa; long long count; double ratio; void* qpl; long long qpl_count; void* u2;
+                       double *yv, *ya; long long y_count; /* NumericSolve: multipliers of Eq. 17, [stride] each */ };
 cudaError_t launch_rescale_duals(const RescaleParams& p, int dtype, cudaStream_t st);
 cudaError_t launch_residual_reduce(const double* part, double* res, long long N, int batch, cudaStream_t st);
 cudaError_t launch_fma_peak(int dtype, int blocks, int threads, long long iters, float* sink, cudaStream_t st);

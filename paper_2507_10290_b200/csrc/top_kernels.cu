@@ -855,6 +855,7 @@ template <typename Real>
 __global__ void rescale_duals_kernel(const RescaleParams p) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (p.qpl && i < p.qpl_count) { double* q = static_cast<double*>(p.qpl); if (q[i] < 0) q[i] *= p.ratio; }
+    if (i < p.y_count) { if (p.yv) p.yv[i] *= p.ratio; if (p.ya) p.ya[i] *= p.ratio; }
     if (i >= p.count) return;
     const Real r = (Real)p.ratio;
     static_cast<Real*>(p.u)[i] *= r;

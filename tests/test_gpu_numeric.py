@@ -119,14 +119,32 @@ def test_numeric_solve_and_full_size_sampled():
     assert r["r_p"][0] < 0.15 and r["r_d"][0] < 0.15
 
 
+def test_numeric_set_rho_and_adaptive_rho():
+    """Eq. 24 / top_set_rho in the numeric branch: the multipliers of Eq. 17 are scaled duals too (times rho_old / rho_new),
+    the initial inverse Hessian is rebuilt for the new rho."""
+    w = tiny(0.9, 2.5)
+    o = make_oracle(w, 0, numeric=True)
+    sol = top.from_workload(w, dtype="f64", numeric=True)
+    sol.iterate(15); o.sweep(15)
+    sol.set_rho(3.5); o.set_rho(3.5)
+    sol.iterate(25); o.sweep(25)
+    compare(sol, [o], w, "after set_rho")
+    # Alg. 1 line 14 every sweep, the paper's parameters, N-scaled tolerance
+    o2 = make_oracle(w, 0, numeric=True)
+    s2 = top.from_workload(w, dtype="f64", numeric=True, adaptive_rho=True, check_every=1, max_iter=120, eps_n_scaled=True)
+    it_o = o2.solve_adaptive(0.05 * w.N, 120)
+    ok, it = s2.solve(0.05)
+    assert it[0] == it_o and abs(s2.rho - o2.rho) <= 1e-12 * o2.rho, (it, it_o, s2.rho, o2.rho)
+    compare(s2, [o2], w, "after adaptive solve")
+
+
 def test_numeric_unsupported():
     w = W.small_constrained(N=9, s=4, acc=False)
-    for kw in ({"dtype": "f32"}, {"dtype": "f64", "consensus": "wide"}, {"dtype": "f64", "adaptive_rho": True}):
+    for kw in ({"dtype": "f32"}, {"dtype": "f64", "consensus": "wide"}):
         with pytest.raises(top.TopError) as e:
             top.from_workload(w, numeric=True, **kw)
         assert e.value.status == top.TOP_E_UNSUPPORTED
-    sol = top.from_workload(w, dtype="f64", numeric=True)
     with pytest.raises(top.TopError):
-        sol.set_rho(3.0)
+        top.from_workload(w, dtype="f64", numeric=True).snapshot()
     with pytest.raises(top.TopError):
         top.from_workload(w, dtype="f64").inner_iterations()
