@@ -185,140 +185,140 @@ __global__ void __launch_bounds__(128, 3) numeric_xupdate_kernel(const NumParams
     k.lane = threadIdx.x & 7; k.base_lane = (threadIdx.x & 31) & ~7; k.mask = 0xffu << k.base_lane;
     const int l = k.lane;
     const long long LS = p.stride, NP = p.nseg_pad;
-  for (;;) {
-    unsigned int gq = 0;
-    if (l == 0) gq = atomicAdd(p.work_counter, 1u);
-    const long long g = (long long)__shfl_sync(k.mask, gq, k.base_lane);
-    if (g >= p.nseg) break;
-    const long long base = g * LANES;
-    k.s = p.s; k.n = 2 * p.s; k.rho = p.rho; k.hard = p.hard != 0;
-    k.has_box = (p.flags & KF_BOX) != 0; k.has_vel = (p.flags & KF_VEL) != 0; k.has_acc = (p.flags & KF_ACC) != 0;
-    k.invT = p.invT[g]; k.invT2 = p.invT[NP + g];
-    const double invTk[4] = {1.0, k.invT, k.invT2, k.invT2 * k.invT};
-    k.is_row = l < 2 * p.s; k.it_row = invTk[l % p.s];
-    k.wq = 1.0;
-    for (int q = 0; q < 2 * p.s - 1; ++q) k.wq *= k.invT;
-    k.vmax2 = p.vmax * p.vmax; k.amax2 = p.amax * p.amax;
-    const int n = k.n;
-    double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0}, x[3], org[3];
-#pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        k.zmu[d] = p.zt[d * LS + base + l] - p.u[d * LS + base + l];
-        k.bhi[d] = k.blo[d] = 0.0;
-        if (k.has_box) {
-            lo[d] = p.lohi[d * NP + g]; hi[d] = p.lohi[(3 + d) * NP + g];
-            k.bhi[d] = hi[d] - fabs(p.qp[d * LS + base + l]); k.blo[d] = lo[d] + fabs(p.qn[d * LS + base + l]);
-        }
-        x[d] = l < n ? p.chat[d * LS + base + l] : 0.0;
-        org[d] = p.origin[d * NP + g];
-    }
-    k.wv = k.has_vel ? p.yv[base + l] : 0.0; k.wa = k.has_acc ? p.ya[base + l] : 0.0;
-    double Pm_row[MAXN];                                   // row l of H0 = Pm^ (the array holds rho * Pm^)
-#pragma unroll
-    for (int b = 0; b < MAXN; ++b) Pm_row[b] = p.Pm[b * LS + base + l] / p.rho;
-
-    double S[LB_MEM][3], Y[LB_MEM][3], rhoi[LB_MEM], alpha[LB_MEM];
-    double gr[3], gn[3], xn[3], dir[3];
-    int hist = 0, it = 0;
-    LaneVals vx = lane_map(tab, k, x);
-    double F = lane_F(k, vx, x);
-    lane_grad(tab, k, vx, gr);
-    for (; it < LB_MAXIT; ++it) {
-        double qv[3] = {gr[0], gr[1], gr[2]};                                // two-loop recursion
-#pragma unroll
-        for (int h = LB_MEM - 1; h >= 0; --h)
-            if (h < hist) {
-                alpha[h] = rhoi[h] * grp_dot(k, S[h], qv);
-#pragma unroll
-                for (int d = 0; d < 3; ++d) qv[d] -= alpha[h] * Y[h][d];
-            }
-#pragma unroll
-        for (int d = 0; d < 3; ++d) {                                        // r = H0 q: row l needs every row of q
-            double acc = 0.0;
-#pragma unroll
-            for (int b = 0; b < MAXN; ++b) acc += Pm_row[b] * __shfl_sync(k.mask, qv[d], k.base_lane + b);
-            dir[d] = acc;
-        }
-#pragma unroll
-        for (int h = 0; h < LB_MEM; ++h)
-            if (h < hist) {
-                const double beta = rhoi[h] * grp_dot(k, Y[h], dir);
-#pragma unroll
-                for (int d = 0; d < 3; ++d) dir[d] += S[h][d] * (alpha[h] - beta);
-            }
-        double dm = 0.0, xm = 0.0;
+    for (;;) {
+        unsigned int gq = 0;
+        if (l == 0) gq = atomicAdd(p.work_counter, 1u);
+        const long long g = (long long)__shfl_sync(k.mask, gq, k.base_lane);
+        if (g >= p.nseg) break;
+        const long long base = g * LANES;
+        k.s = p.s; k.n = 2 * p.s; k.rho = p.rho; k.hard = p.hard != 0;
+        k.has_box = (p.flags & KF_BOX) != 0; k.has_vel = (p.flags & KF_VEL) != 0; k.has_acc = (p.flags & KF_ACC) != 0;
+        k.invT = p.invT[g]; k.invT2 = p.invT[NP + g];
+        const double invTk[4] = {1.0, k.invT, k.invT2, k.invT2 * k.invT};
+        k.is_row = l < 2 * p.s; k.it_row = invTk[l % p.s];
+        k.wq = 1.0;
+        for (int q = 0; q < 2 * p.s - 1; ++q) k.wq *= k.invT;
+        k.vmax2 = p.vmax * p.vmax; k.amax2 = p.amax * p.amax;
+        const int n = k.n;
+        double lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0}, x[3], org[3];
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
-            dir[d] = -dir[d];
-            dm = fmax(dm, fabs(dir[d]));                                     // normalised-time coefficients are metres already
-            xm = fmax(xm, fabs(x[d] + (l == 0 ? org[d] : 0.0)));             // (the tolerance is relative to the global-frame size)
+            k.zmu[d] = p.zt[d * LS + base + l] - p.u[d * LS + base + l];
+            k.bhi[d] = k.blo[d] = 0.0;
+            if (k.has_box) {
+                lo[d] = p.lohi[d * NP + g]; hi[d] = p.lohi[(3 + d) * NP + g];
+                k.bhi[d] = hi[d] - fabs(p.qp[d * LS + base + l]); k.blo[d] = lo[d] + fabs(p.qn[d * LS + base + l]);
+            }
+            x[d] = l < n ? p.chat[d * LS + base + l] : 0.0;
+            org[d] = p.origin[d * NP + g];
         }
-        const double slope = grp_dot(k, gr, dir);
+        k.wv = k.has_vel ? p.yv[base + l] : 0.0; k.wa = k.has_acc ? p.ya[base + l] : 0.0;
+        double Pm_row[MAXN];                                   // row l of H0 = Pm^ (the array holds rho * Pm^)
 #pragma unroll
-        for (int m = 1; m < 8; m <<= 1) { dm = fmax(dm, __shfl_xor_sync(k.mask, dm, m)); xm = fmax(xm, __shfl_xor_sync(k.mask, xm, m)); }
-        if (!(dm > LB_TOL * xm) || !(slope < 0.0)) break;
-        const LaneVals vd = lane_map(tab, k, dir);
-        LaneVals vn = vx;
-        double t = 1.0, Fn = F;
-        bool ok = false;
-        for (int ls = 0; ls < 40; ++ls) {                                    // Armijo backtracking along the ray
+        for (int b = 0; b < MAXN; ++b) Pm_row[b] = p.Pm[b * LS + base + l] / p.rho;
+
+        double S[LB_MEM][3], Y[LB_MEM][3], rhoi[LB_MEM], alpha[LB_MEM];
+        double gr[3], gn[3], xn[3], dir[3];
+        int hist = 0, it = 0;
+        LaneVals vx = lane_map(tab, k, x);
+        double F = lane_F(k, vx, x);
+        lane_grad(tab, k, vx, gr);
+        for (; it < LB_MAXIT; ++it) {
+            double qv[3] = {gr[0], gr[1], gr[2]};                                // two-loop recursion
 #pragma unroll
-            for (int d = 0; d < 3; ++d) xn[d] = x[d] + t * dir[d];
-            vn = vals_axpy(vx, t, vd);
-            Fn = lane_F(k, vn, xn);
-            if (Fn <= F + LB_C1 * t * slope) { ok = true; break; }
-            t *= 0.5;
-        }
-        if (!ok) break;
-        vx = vn;
-        lane_grad(tab, k, vx, gn);
-        double sv[3], yv[3];
+            for (int h = LB_MEM - 1; h >= 0; --h)
+                if (h < hist) {
+                    alpha[h] = rhoi[h] * grp_dot(k, S[h], qv);
 #pragma unroll
-        for (int d = 0; d < 3; ++d) { sv[d] = t * dir[d]; yv[d] = gn[d] - gr[d]; }
-        const double sy = grp_dot(k, sv, yv);
-        if (sy > 0.0) {
-            if (hist == LB_MEM) {
-#pragma unroll
-                for (int h = 1; h < LB_MEM; ++h) {
-#pragma unroll
-                    for (int d = 0; d < 3; ++d) { S[h - 1][d] = S[h][d]; Y[h - 1][d] = Y[h][d]; }
-                    rhoi[h - 1] = rhoi[h];
+                    for (int d = 0; d < 3; ++d) qv[d] -= alpha[h] * Y[h][d];
                 }
-                hist = LB_MEM - 1;
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {                                        // r = H0 q: row l needs every row of q
+                double acc = 0.0;
+#pragma unroll
+                for (int b = 0; b < MAXN; ++b) acc += Pm_row[b] * __shfl_sync(k.mask, qv[d], k.base_lane + b);
+                dir[d] = acc;
             }
 #pragma unroll
             for (int h = 0; h < LB_MEM; ++h)
-                if (h == hist) {
+                if (h < hist) {
+                    const double beta = rhoi[h] * grp_dot(k, Y[h], dir);
 #pragma unroll
-                    for (int d = 0; d < 3; ++d) { S[h][d] = sv[d]; Y[h][d] = yv[d]; }
-                    rhoi[h] = 1.0 / sy;
+                    for (int d = 0; d < 3; ++d) dir[d] += S[h][d] * (alpha[h] - beta);
                 }
-            ++hist;
-        }
+            double dm = 0.0, xm = 0.0;
 #pragma unroll
-        for (int d = 0; d < 3; ++d) { x[d] = xn[d]; gr[d] = gn[d]; }
-        F = Fn;
-        if (!(t * dm > LB_TOL * xm)) { ++it; break; }                        // the step TAKEN is below tolerance: converged
-    }
-    if (l == 0) atomicAdd(p.inner_iters, (unsigned long long)it);
+            for (int d = 0; d < 3; ++d) {
+                dir[d] = -dir[d];
+                dm = fmax(dm, fabs(dir[d]));                                     // normalised-time coefficients are metres already
+                xm = fmax(xm, fabs(x[d] + (l == 0 ? org[d] : 0.0)));             // (the tolerance is relative to the global-frame size)
+            }
+            const double slope = grp_dot(k, gr, dir);
+#pragma unroll
+            for (int m = 1; m < 8; m <<= 1) { dm = fmax(dm, __shfl_xor_sync(k.mask, dm, m)); xm = fmax(xm, __shfl_xor_sync(k.mask, xm, m)); }
+            if (!(dm > LB_TOL * xm) || !(slope < 0.0)) break;
+            const LaneVals vd = lane_map(tab, k, dir);
+            LaneVals vn = vx;
+            double t = 1.0, Fn = F;
+            bool ok = false;
+            for (int ls = 0; ls < 40; ++ls) {                                    // Armijo backtracking along the ray
+#pragma unroll
+                for (int d = 0; d < 3; ++d) xn[d] = x[d] + t * dir[d];
+                vn = vals_axpy(vx, t, vd);
+                Fn = lane_F(k, vn, xn);
+                if (Fn <= F + LB_C1 * t * slope) { ok = true; break; }
+                t *= 0.5;
+            }
+            if (!ok) break;
+            vx = vn;
+            lane_grad(tab, k, vx, gn);
+            double sv[3], yv[3];
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { sv[d] = t * dir[d]; yv[d] = gn[d] - gr[d]; }
+            const double sy = grp_dot(k, sv, yv);
+            if (sy > 0.0) {
+                if (hist == LB_MEM) {
+#pragma unroll
+                    for (int h = 1; h < LB_MEM; ++h) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) { S[h - 1][d] = S[h][d]; Y[h - 1][d] = Y[h][d]; }
+                        rhoi[h - 1] = rhoi[h];
+                    }
+                    hist = LB_MEM - 1;
+                }
+#pragma unroll
+                for (int h = 0; h < LB_MEM; ++h)
+                    if (h == hist) {
+#pragma unroll
+                        for (int d = 0; d < 3; ++d) { S[h][d] = sv[d]; Y[h][d] = yv[d]; }
+                        rhoi[h] = 1.0 / sy;
+                    }
+                ++hist;
+            }
+#pragma unroll
+            for (int d = 0; d < 3; ++d) { x[d] = xn[d]; gr[d] = gn[d]; }
+            F = Fn;
+            if (!(t * dm > LB_TOL * xm)) { ++it; break; }                        // the step TAKEN is below tolerance: converged
+        }
+        if (l == 0) atomicAdd(p.inner_iters, (unsigned long long)it);
 
-    // ---- c^{k+1}: coefficients, boundary rows, slack projection of the box (Eq. 10 / 20d-e as a Moreau pair), multipliers
-    vx = lane_map(tab, k, x);                              // (recomputed from the final coefficients: no accumulated ray arithmetic in the state)
-    double n2v = 0.0, n2a = 0.0;
+        // ---- c^{k+1}: coefficients, boundary rows, slack projection of the box (Eq. 10 / 20d-e as a Moreau pair), multipliers
+        vx = lane_map(tab, k, x);                              // (recomputed from the final coefficients: no accumulated ray arithmetic in the state)
+        double n2v = 0.0, n2a = 0.0;
 #pragma unroll
-    for (int d = 0; d < 3; ++d) {
-        if (l < n) p.chat[d * LS + base + l] = x[d];
-        if (k.is_row) p.bnd[d * LS + base + l] = vx.b[d];
-        if (k.has_box) {                                  // q = -(A c - b + v_old): s = max(0,q), v_new = max(0,-q)
-            const double qp0 = p.qp[d * LS + base + l], qn0 = p.qn[d * LS + base + l];
-            p.qp[d * LS + base + l] = (hi[d] - vx.P[d]) - fmax(-qp0, 0.0);
-            p.qn[d * LS + base + l] = (vx.P[d] - lo[d]) - fmax(-qn0, 0.0);
+        for (int d = 0; d < 3; ++d) {
+            if (l < n) p.chat[d * LS + base + l] = x[d];
+            if (k.is_row) p.bnd[d * LS + base + l] = vx.b[d];
+            if (k.has_box) {                                  // q = -(A c - b + v_old): s = max(0,q), v_new = max(0,-q)
+                const double qp0 = p.qp[d * LS + base + l], qn0 = p.qn[d * LS + base + l];
+                p.qp[d * LS + base + l] = (hi[d] - vx.P[d]) - fmax(-qp0, 0.0);
+                p.qn[d * LS + base + l] = (vx.P[d] - lo[d]) - fmax(-qn0, 0.0);
+            }
+            n2v += vx.V[d] * vx.V[d]; n2a += vx.A[d] * vx.A[d];
         }
-        n2v += vx.V[d] * vx.V[d]; n2a += vx.A[d] * vx.A[d];
+        if (k.has_vel) { const double g0 = n2v - k.vmax2, gp = g0 > 0.0 ? g0 : 0.0; p.yv[base + l] = k.wv + gp * gp; }
+        if (k.has_acc) { const double g0 = n2a - k.amax2, gp = g0 > 0.0 ? g0 : 0.0; p.ya[base + l] = k.wa + gp * gp; }
     }
-    if (k.has_vel) { const double g0 = n2v - k.vmax2, gp = g0 > 0.0 ? g0 : 0.0; p.yv[base + l] = k.wv + gp * gp; }
-    if (k.has_acc) { const double g0 = n2a - k.amax2, gp = g0 > 0.0 ? g0 : 0.0; p.ya[base + l] = k.wa + gp * gp; }
-  }
 }
 
 // ---- consensus z-update (Eq. 6b / 20b), scaled dual (Eq. 6c / 20c), residual partial sums (Eq. 21-22; readings A7, A8):
