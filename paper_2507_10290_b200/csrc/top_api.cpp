@@ -1564,7 +1564,10 @@ extern "C" TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas
     if (!h || h->waves.empty()) return TOP_E_INVALID;
     const auto& w = h->waves[0];
     if (ctas) *ctas = w.ctas;
-    if (threads) *threads = w.threads;
+    if (threads) {      // as top_iterate launches it (the fp64 tensor-core kernel may run its last octet on three warps)
+        const uint32_t f = h->kflags | sync_flag(h) | w.kflags | (w.cluster ? KF_CLUSTER : 0);
+        *threads = w.threads + (h->mma && !h->numeric && split_tail_applies(f, 0, h->dtype, w.ctas, w.threads) ? 64 : 0);
+    }
     if (segs_per_cta) *segs_per_cta = w.segs_per_cta;
     if (smem_bytes) *smem_bytes = (int32_t)w.smem;
     if (waves) *waves = (int32_t)h->waves.size();

@@ -109,6 +109,8 @@ int max_threads_for(int dtype, int lanes);
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, int threads, size_t smem, int* max_ctas_per_sm);
 // fp64 tensor-core variant of the 4-lane kernel (top_kernels_mma.cu: cadmm_sweeps_mma_kernel)
 cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st);
+// does a launch with these flags run its last octet on three warps (threads + 64 per CTA; top_kernels_mma.cu, "split tail")?
+bool split_tail_applies(uint32_t kparam_flags, int check_every, int dtype, int ctas, int threads);
 size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly, bool wide = false);
 int max_threads_mma(int dtype, bool poly, bool wide = false);
 cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm);

@@ -26,6 +26,7 @@
 //               the per-segment operator rows; the all-gather buffer; the boundary-row exchange buffer
 // The constraint selection is a template parameter (the three combinations BASELINE.json's configs use, plus a
 // run-time-flag variant for the others): no branch inside the sweep body except the exchange.
+#include <stdlib.h>
 #include <string.h>
 
 #include "top_device.cuh"
@@ -94,9 +95,20 @@ __device__ __forceinline__ float neg_part(float q) {
 // Eq. 20f without a branch: the factor min(1, bound/||y||) of the projection of y onto ||.|| <= bound (reading A15)
 template <typename Real>
 __device__ __forceinline__ Real ball_scale(const Real (&y)[3], Real bound) {
-    const Real n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
+    const Real n2 = fma(y[2], y[2], fma(y[1], y[1], y[0] * y[0]));      // (spelled out: the split-tail warps must round the same way)
     const Real sc = bound * rsqrt_pos(n2);                 // garbage (inf/NaN) when n2 == 0: not selected then
     return n2 > bound * bound ? sc : (Real)1;
+}
+
+// residual partial sums of one (row, dim) / one dim, spelled out with fma so that every path adds them in the same order
+__device__ __forceinline__ void rp_accum(double& rp2, double& gap2, double res, bool gaprow, double own, double nb) {
+    rp2 = fma(res, res, rp2);
+    if (gaprow) { const double gp = own - nb; gap2 = fma(gp, gp, gap2); }      // Eq. 21
+}
+__device__ __forceinline__ void rd_accum(double& rd2, double& rdn2, double xr0, double xr1, double Tp0, double Tp1) {
+    rdn2 = rdn2 + fma(xr1, xr1, xr0 * xr0);
+    const double a = xr0 * Tp0, b = xr1 * Tp1;
+    rd2 = rd2 + fma(b, b, a * a);
 }
 
 // the state of a lane lives in shared memory as pairs
@@ -187,9 +199,346 @@ __device__ __noinline__ void refresh_operator_rows(const KParams& p, long long g
     for (int d = 0; d < 3; ++d) c0_row[d * TS] = c0n[d];
 }
 
-template <typename Real, int S, int CM, int MAXT, bool SOLVE, bool POLY = false, bool WIDE = false>
-__global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams p) {
+// ================================================================================================ split tail
+// Load balance of the fp64 kernel when a CTA holds 4k+1 octets (config 4: 68 segments = 8 octets + 4 segments): as 4k+1 warps
+// one scheduler carries k+1 warps, and all the others wait for it at the pair barriers.  In the SPLIT instantiation the LAST
+// octet is run by THREE warps, one flat dimension each (4k+3 warps: the extra work is spread over three schedulers).  Everything
+// in the sweep is independent per dimension -- both contractions (one accumulator tile instead of three), the operator apply,
+// the box, the consensus, the duals -- except the ball projections, which need ||y||^2 over the three dims: the three warps
+// exchange their y_d through shared memory around one named barrier.  The arithmetic of a (row, dim) is the one of the unsplit
+// lane, operation for operation: results are bit-identical.  Towards the octet in front the three warps join that warp's pair
+// barrier (128 threads); towards the next CTA each publishes and fetches its own dim's mailbox slots.
+// (A kernel made of such warps ONLY was tried: 864 threads leave 72 registers and every operator row is read three times --
+// shared-memory bound, slower.  Here only one octet pays that.)
+constexpr int SPLIT_BALL_BAR = 15;      // named barrier of the three tail warps (the pair barriers use ids 0..8)
+
+template <int S, int CM, int MAXT>
+__device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned char* smem_raw, volatile int* abort_any, double2 (*nbuf)[2][3][32]) {
     constexpr int N2 = 2 * S;
+    constexpr int TS = MAXT, SA = MAXT / 4, BPAR = (SA + 2) * 24;
+    const int tmain = (int)blockDim.x - 96;                       // threads of the unsplit warps in front
+    const int oct = tmain >> 5, d = ((int)threadIdx.x - tmain) >> 5, lane32 = threadIdx.x & 31;
+    const int lane = lane32 & 3, grp = lane32 >> 2, sl = oct * 8 + grp, vt = sl * 4 + lane;      // vt: the thread an unsplit warp would be
+    const int SEGS = p.segs_per_cta, cta = blockIdx.x, nctas = gridDim.x;
+    const uint32_t flags = p.flags;
+    constexpr bool has_box = (CM & (int)KF_BOX) != 0, has_vel = (CM & (int)KF_VEL) != 0, has_acc = (CM & (int)KF_ACC) != 0;
+    static_assert(CM != CM_RUNTIME && CM != 0, "split tail: compile-time constraint sets only");
+    const bool pin_pos = flags & KF_PIN_POS;
+
+    const SmemLayoutMma L = smem_layout_mma(true, SA);
+    double2* Pms = reinterpret_cast<double2*>(smem_raw + L.pm) + vt;                          // [(h*4 + b/2) * TS]  (shared by the three dims)
+    double* c0s = reinterpret_cast<double*>(smem_raw + L.c0) + vt + (size_t)d * TS;           // [h*3 * TS]
+    double2* zus = reinterpret_cast<double2*>(smem_raw + L.zu) + vt + (size_t)d * TS;         // [h*3 * TS]: (z~, u)
+    double2* qs = reinterpret_cast<double2*>(smem_raw + L.qs) + vt + (size_t)d * TS;          // (q+, q-)
+    double2* ws = reinterpret_cast<double2*>(smem_raw + L.ws) + vt + (size_t)d * TS;          // (w_v, w_a)
+    double* ctab = reinterpret_cast<double*>(smem_raw + L.ctab) + lane32;                     // (filled by warp 0)
+    double* lohi = reinterpret_cast<double*>(smem_raw + L.lohi) + sl;                         // [6 * SA]
+    double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE + d * 8;
+    double* Bs = reinterpret_cast<double*>(smem_raw + L.bs);                                  // [2 parity][SA+2][8 rows][3]
+    double* zoffs = reinterpret_cast<double*>(smem_raw + L.zoff) + sl;                        // [(side*3 + dim) * SA]
+
+    const long long cta_first = p.seg_begin + (long long)cta * SEGS;
+    const long long remaining = p.seg_end - cta_first;
+    const int nact = remaining < SEGS ? (int)remaining : SEGS;
+    const bool active = sl < nact;
+    const long long gseg = active ? cta_first + sl : cta_first;
+    const bool owned = active && gseg >= p.own_begin && gseg < p.own_end;
+    const long long stride = p.stride;
+
+    int jj[2]; long long gt[2]; bool isrow[2], right[2]; int korder[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        jj[h] = lane + 4 * h;
+        gt[h] = gseg * LANES + jj[h];
+        isrow[h] = S == 4 ? true : jj[h] < N2;
+        right[h] = S == 4 ? h == 1 : jj[h] >= S;
+        korder[h] = right[h] ? jj[h] - S : jj[h];
+    }
+    double invTk[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        if (d == 0) {
+#pragma unroll
+            for (int b = 0; b < 8; b += 2)
+                Pms[(h * 4 + (b >> 1)) * TS] = make_double2(b < N2 ? p.Pm[(long long)b * stride + gt[h]] : 0.0,
+                                                            b + 1 < N2 ? p.Pm[(long long)(b + 1) * stride + gt[h]] : 0.0);
+        }
+        c0s[h * 3 * TS] = p.c0[d * stride + gt[h]];
+        invTk[h] = static_cast<const double*>(p.invTk)[gt[h]];
+    }
+    const double invT = static_cast<const double*>(p.invT)[gseg], invT2 = static_cast<const double*>(p.invT)[p.nseg_pad + gseg];
+    if (d == 0) {
+        lohi[lane * SA] = static_cast<const double*>(p.lohi)[lane * p.nseg_pad + gseg];
+        if (lane < 2) lohi[(lane + 4) * SA] = static_cast<const double*>(p.lohi)[(lane + 4) * p.nseg_pad + gseg];
+    }
+    if (lane == 0) {      // frame shifts of the neighbours' position rows of this dim: left junction (row 0), right junction (row S)
+        zoffs[d * SA] = static_cast<const double*>(p.zoff)[d * stride + gseg * LANES + 0];
+        zoffs[(3 + d) * SA] = static_cast<const double*>(p.zoff)[d * stride + gseg * LANES + S];
+    }
+    const uint8_t sf = p.segflags[gseg];
+    const bool open_l = (flags & KF_OPEN_LEFT) && gseg == p.seg_begin, open_r = (flags & KF_OPEN_RIGHT) && gseg == p.seg_end - 1;
+
+    // ---- per-lane facts of the exchange (one dim per lane: one value per row)
+    int own_off[2], nb_off[2], pub_off[2];
+    bool fixed[2], zshift[2], gaprow[2], pub[2];
+    bool need = false;
+    int need_h = 0, need_off = 0;
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        own_off[h] = (sl + 1) * 24 + jj[h] * 3 + d;
+        nb_off[h] = (right[h] ? (sl + 2) * 24 + korder[h] * 3 : sl * 24 + (korder[h] + S) * 3) + d;
+        fixed[h] = (right[h] ? (sf & SEG_LAST) : (sf & SEG_FIRST)) || (pin_pos && korder[h] == 0) || (right[h] ? open_r : open_l);
+        zshift[h] = isrow[h] && korder[h] == 0;
+        gaprow[h] = isrow[h] && right[h] && !(sf & SEG_LAST);
+        const bool edge_l = active && isrow[h] && sl == 0 && !right[h] && cta > 0;
+        const bool edge_r = active && isrow[h] && sl == nact - 1 && right[h] && cta + 1 < nctas;
+        pub[h] = nctas > 1 && (edge_l || edge_r);
+        pub_off[h] = (cta * 24 + (edge_r ? 12 : 0) + korder[h] * 3 + d) * 16;
+        if (edge_l || edge_r) {
+            need = true; need_h = h;
+            need_off = (edge_l ? ((cta - 1) * 24 + 12 + korder[h] * 3) : ((cta + 1) * 24 + korder[h] * 3)) * 16 + d * 16;
+        }
+    }
+
+    // ---- state of iterate k: the a1 operands in registers, the variables behind them in shared memory
+    double gM[2], A0[2], gv[2], ga[2];
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+        const long long i = d * stride + gt[h];
+        const double z0 = static_cast<const double*>(p.zt)[i], u0 = static_cast<const double*>(p.u)[i];
+        zus[h * 3 * TS] = make_double2(z0, u0);
+        gM[h] = (z0 - u0) * invTk[h];
+        A0[h] = gv[h] = ga[h] = 0.0;
+        double w_v = 0, w_a = 0;
+        if (has_box) {
+            const double lo = static_cast<const double*>(p.lohi)[d * p.nseg_pad + gseg], hi = static_cast<const double*>(p.lohi)[(3 + d) * p.nseg_pad + gseg];
+            const double a = static_cast<const double*>(p.qp)[i], b = static_cast<const double*>(p.qn)[i];
+            qs[h * 3 * TS] = make_double2(a, b);
+            A0[h] = (hi - fabs(a)) + (lo + fabs(b));
+        }
+        if (has_vel) { w_v = static_cast<const double*>(p.wv)[i]; gv[h] = (static_cast<const double*>(p.phv)[i] - w_v) * invT; }
+        if (has_acc) { w_a = static_cast<const double*>(p.wa)[i]; ga[h] = (static_cast<const double*>(p.pha)[i] - w_a) * invT2; }
+        ws[h * 3 * TS] = make_double2(w_v, w_a);
+    }
+    // (phi of iterate k is not kept: it only enters through gv, ga; phi of the final iterate is written on the last sweep -- a
+    // launch of zero sweeps writes nothing back at all)
+    const double vmax = p.vmax, amax = p.amax;
+    unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
+    const size_t mbox_par_stride = (size_t)p.max_ctas * 24 * 16;
+    __syncthreads();      // (the one CTA barrier of the launch: the unsplit warps arrive from cadmm_sweeps_mma_kernel)
+
+    for (int it = 0; it < p.k_sweeps; ++it) {
+        const unsigned seq = p.seq_base + (unsigned)it + 1u;
+        const int par = (int)(seq & 1u);
+        const bool last_sweep = (it == p.k_sweeps - 1);
+        double* const Bcur = Bs + par * BPAR;
+        unsigned char* const mpar = mbox + par * mbox_par_stride;
+
+        // ================= phase A: segment local, this dim =================
+        double2 pm[2][4];
+        double cacc[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+#pragma unroll
+            for (int b = 0; b < 4; ++b) pm[h][b] = Pms[(h * 4 + b) * TS];
+            cacc[h] = c0s[h * 3 * TS];
+        }
+        // a1 (Eq. 20a second bracket): one accumulator tile; lane t ends with rows 2t, 2t+1 of R^ of its segment and dim
+        {
+            double a0 = 0.0, a1 = 0.0;
+            dmma884(a0, a1, gM[0], ctab[0 * 32]); dmma884(a0, a1, gM[1], ctab[1 * 32]);
+            if (has_box) { dmma884(a0, a1, A0[0], ctab[2 * 32]); dmma884(a0, a1, A0[1], ctab[3 * 32]); }
+            if (has_vel) { dmma884(a0, a1, gv[0], ctab[4 * 32]); dmma884(a0, a1, gv[1], ctab[5 * 32]); }
+            if (has_acc) { dmma884(a0, a1, ga[0], ctab[6 * 32]); dmma884(a0, a1, ga[1], ctab[7 * 32]); }
+            *reinterpret_cast<double2*>(Xs + 2 * lane) = make_double2(a0, a1);
+        }
+        __syncwarp();
+        // a2 (Eq. 20a first bracket): c^ = (rho Pm^) R^ + c0^, rows lane, lane+4
+#pragma unroll
+        for (int b = 0; b < N2 / 2; ++b) {
+            const double2 x2 = *reinterpret_cast<const double2*>(Xs + 2 * b);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) { cacc[h] += pm[h][b].x * x2.x; cacc[h] += pm[h][b].y * x2.y; }
+        }
+        if (last_sweep && owned) {
+#pragma unroll
+            for (int h = 0; h < 2; ++h) static_cast<double*>(p.chat)[d * stride + gt[h]] = cacc[h];
+        }
+        __syncwarp();       // (Xs is read by every lane of the segment before the next sweep overwrites it)
+        // a3: the lane's consensus rows of B = M c and its two samples of E0 c, E1 c, E2 c, this dim
+        double Bnd[2];
+        {
+            double e0 = 0.0, e1 = 0.0;
+            dmma884(e0, e1, cacc[0], ctab[8 * 32]); dmma884(e0, e1, cacc[1], ctab[12 * 32]);
+            Bnd[0] = e0 * invTk[0]; Bnd[1] = e1 * invTk[1];
+        }
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            if (isrow[h]) Bcur[own_off[h]] = Bnd[h];
+            if (pub[h]) ll_store(mpar + pub_off[h], Bnd[h], seq);
+        }
+        LLRaw rr;
+        if (need) ll_issue(mpar + need_off, rr);
+        {
+            double Pv[2] = {0, 0}, Vv[2] = {0, 0}, Av[2] = {0, 0};
+            if (has_vel) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0], ctab[10 * 32]); dmma884(e0, e1, cacc[1], ctab[14 * 32]); Vv[0] = e0; Vv[1] = e1; }
+            if (has_acc) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0], ctab[11 * 32]); dmma884(e0, e1, cacc[1], ctab[15 * 32]); Av[0] = e0; Av[1] = e1; }
+            if (has_box) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0], ctab[9 * 32]); dmma884(e0, e1, cacc[1], ctab[13 * 32]); Pv[0] = e0; Pv[1] = e1; }
+            double2 w2[2], q2[2];
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+                if (has_vel || has_acc) w2[h] = ws[h * 3 * TS];
+                if (has_box) q2[h] = qs[h * 3 * TS];
+            }
+            // a4 (Eq. 20f, 20g): y = A c + w; ||y|| runs over the three dims: the three warps exchange y_d (buffer of this
+            // sweep's parity: the next sweep writes the other one, and nobody passes that sweep's barrier before everybody has
+            // read this one)
+            if (has_vel || has_acc) {
+                double yv[2] = {0, 0}, ya[2] = {0, 0};
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    if (has_vel) yv[h] = Vv[h] * invT + w2[h].x;
+                    if (has_acc) ya[h] = Av[h] * invT2 + w2[h].y;
+                    nbuf[par][h][d][lane32] = make_double2(yv[h], ya[h]);
+                }
+                asm volatile("bar.sync %0, 96;" ::"n"(SPLIT_BALL_BAR) : "memory");
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const double2 s0 = nbuf[par][h][0][lane32], s1 = nbuf[par][h][1][lane32], s2 = nbuf[par][h][2][lane32];
+                    if (has_vel) {
+                        const double y[3] = {s0.x, s1.x, s2.x};
+                        const double scale = ball_scale(y, vmax);
+                        const double ph = scale * yv[h];
+                        w2[h].x = yv[h] - ph; gv[h] = (ph - w2[h].x) * invT;
+                        if (last_sweep && owned) static_cast<double*>(p.phv_out)[d * stride + gt[h]] = ph;
+                    }
+                    if (has_acc) {
+                        const double y[3] = {s0.y, s1.y, s2.y};
+                        const double scale = ball_scale(y, amax);
+                        const double ph = scale * ya[h];
+                        w2[h].y = ya[h] - ph; ga[h] = (ph - w2[h].y) * invT2;
+                        if (last_sweep && owned) static_cast<double*>(p.pha_out)[d * stride + gt[h]] = ph;
+                    }
+                    ws[h * 3 * TS] = w2[h];
+                }
+            }
+            if (has_box) {      // a7 + a8 (Eq. 20d, 20e) as a Moreau pair
+                const double lo = lohi[d * SA], hi = lohi[(3 + d) * SA];
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const double qpn = (hi - Pv[h]) - neg_part(q2[h].x), qnn = (Pv[h] - lo) - neg_part(q2[h].y);
+                    qs[h * 3 * TS] = make_double2(qpn, qnn);
+                    A0[h] = (hi - fabs(qpn)) + (lo + fabs(qnn));
+                }
+            }
+        }
+
+        // ================= exchange: the next CTA's rows (mailbox), then the pair barrier with the octet in front
+        {
+            bool okk = !need || ll_ok(rr, seq);
+            if (*abort_any) okk = true;
+            if (!__all_sync(0xffffffffu, okk)) {
+                const long long t0 = global_ns();
+                unsigned spins = 0;
+                bool failed = false;
+                do {
+                    if (!okk) { ll_issue(mpar + need_off, rr); okk = ll_ok(rr, seq); }
+                    bool bail = false;
+                    if ((++spins & 255u) == 0) bail = *(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS;
+                    if (__any_sync(0xffffffffu, bail)) { if (!okk) { atomicExch(p.abort_flag, 1); failed = true; } break; }
+                } while (!__all_sync(0xffffffffu, okk));
+                if (failed) *abort_any = 1;
+            }
+        }
+        asm volatile("bar.sync %0, 128;" ::"r"(oct - 1) : "memory");
+
+        // ================= phase B: consensus, dual, residuals (this dim)
+        double res_[2], own_[2], nb_[2], dz[2];
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const double own = Bnd[h];
+            double nb = Bcur[nb_off[h]];
+            if (need && need_h == h) nb = ll_value(rr);
+            if (zshift[h]) nb += zoffs[((right[h] ? 3 : 0) + d) * SA];
+            const double2 zu = zus[h * 3 * TS];
+            const double avg = 0.5 * (own + nb);
+            const double znew = (fixed[h] || !isrow[h]) ? zu.x : avg;            // a5: Eq. 6b / 20b
+            dz[h] = znew - zu.x;
+            const double res = isrow[h] ? own - znew : 0.0;
+            const double unew = zu.y + res;                                        // a8: Eq. 6c / 20c
+            zus[h * 3 * TS] = make_double2(znew, unew);
+            gM[h] = (znew - unew) * invTk[h];
+            res_[h] = res; own_[h] = own; nb_[h] = nb;
+        }
+        if (last_sweep) {
+            // a6 (Eq. 21, 22; A7, A8): the three warps hand their terms to the dim-0 warp, which adds them in the order of the
+            // unsplit lane (rows, then dims; then the 4 lanes)
+            double x0 = 0, x1 = 0;
+            dmma884(x0, x1, dz[0] * invTk[0], ctab[0 * 32]);
+            dmma884(x0, x1, dz[1] * invTk[1], ctab[1 * 32]);
+            double2 (*rb)[3][32] = nbuf[par ^ 1];      // (free: everybody is past this sweep's ball barrier, and the launch ends here)
+            rb[0][d][lane32] = make_double2(res_[0], res_[1]);
+            rb[1][d][lane32] = make_double2(p.rho * x0, p.rho * x1);
+            asm volatile("bar.sync %0, 96;" ::"n"(SPLIT_BALL_BAR) : "memory");
+            double2 (*gb)[3][32] = nbuf[par];          // own - nb of the gap rows (the ball exchange of this sweep is over)
+            gb[0][d][lane32] = make_double2(own_[0] - nb_[0], own_[1] - nb_[1]);
+            asm volatile("bar.sync %0, 96;" ::"n"(SPLIT_BALL_BAR) : "memory");
+            if (d == 0) {
+                const double Tp0 = static_cast<const double*>(p.Tpow)[gseg * LANES + 2 * lane], Tp1 = static_cast<const double*>(p.Tpow)[gseg * LANES + 2 * lane + 1];
+                double rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
+#pragma unroll
+                for (int h = 0; h < 2; ++h)
+#pragma unroll
+                    for (int dd = 0; dd < 3; ++dd) {
+                        const double2 r2 = rb[0][dd][lane32], g2 = gb[0][dd][lane32];
+                        const double r = h ? r2.y : r2.x, g = h ? g2.y : g2.x;
+                        rp2 = fma(r, r, rp2);
+                        if (gaprow[h]) gap2 = fma(g, g, gap2);
+                    }
+#pragma unroll
+                for (int dd = 0; dd < 3; ++dd) { const double2 x2 = rb[1][dd][lane32]; rd_accum(rd2, rdn2, x2.x, x2.y, Tp0, Tp1); }
+#pragma unroll
+                for (int m = 1; m < 4; m <<= 1) { rp2 += shfl_xor(rp2, m); rd2 += shfl_xor(rd2, m); rdn2 += shfl_xor(rdn2, m); gap2 += shfl_xor(gap2, m); }
+                if (owned && lane == 0) { double* o = p.part + gseg * 4; o[0] = rp2; o[1] = rd2; o[2] = rdn2; o[3] = gap2; }
+            }
+        }
+    }
+
+    // ---- write iterate k + k_sweeps back (phi went out on the last sweep)
+    if (owned) {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const long long i = d * stride + gt[h];
+            const double2 zz = zus[h * 3 * TS];
+            static_cast<double*>(p.zt_out)[i] = zz.x;
+            static_cast<double*>(p.u_out)[i] = zz.y;
+            if (has_box) { const double2 q = qs[h * 3 * TS]; static_cast<double*>(p.qp_out)[i] = q.x; static_cast<double*>(p.qn_out)[i] = q.y; }
+            if (has_vel || has_acc) {
+                const double2 w2 = ws[h * 3 * TS];
+                if (has_vel) static_cast<double*>(p.wv_out)[i] = w2.x;
+                if (has_acc) static_cast<double*>(p.wa_out)[i] = w2.y;
+            }
+            if (p.k_sweeps == 0) {
+                if (has_vel) static_cast<double*>(p.phv_out)[i] = static_cast<const double*>(p.phv)[i];
+                if (has_acc) static_cast<double*>(p.pha_out)[i] = static_cast<const double*>(p.pha)[i];
+            }
+        }
+    }
+}
+
+template <typename Real, int S, int CM, int MAXT, bool SOLVE, bool POLY = false, bool WIDE = false, bool SPLIT = false>
+__global__ void __launch_bounds__(MAXT + (SPLIT ? 64 : 0), 1) cadmm_sweeps_mma_kernel(const KParams p) {
+    constexpr int N2 = 2 * S;
+    static_assert(!SPLIT || (sizeof(Real) == 8 && !SOLVE && !POLY && !WIDE), "split tail: plain fp64 sweeps only");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int abort_any;
+    __shared__ double2 nbuf_sh[SPLIT ? 2 : 1][2][3][SPLIT ? 32 : 1];
+    if constexpr (SPLIT) {      // the last three warps run the last octet, one dim each
+        if ((int)threadIdx.x >= (int)blockDim.x - 96) {
+            split_tail_sweeps<S, (CM == 0 || CM == CM_RUNTIME) ? 7 : CM, MAXT>(p, smem_raw, &abort_any, reinterpret_cast<double2 (*)[2][3][32]>(&nbuf_sh[0][0][0][0]));
+            return;
+        }
+    }
     // WIDE: the paper-literal consensus (reading A1): derivative orders 0..2s-2 at both boundaries.
     // Orders 0..s-1 are the first block (as always); orders s..2s-2 form a SECOND block of consensus rows with the same
     // lane <-> row map: lane t owns order s+t at the start boundary (item h = 0) and at the end boundary (h = 1), t <= s-2.
@@ -204,9 +553,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     // two contractions stay on the fp64 tensor pipe (products of fp32-rounded operands, fp64 accumulation) and the operator
     // apply a2 stays fp64 (an fp32 operator loses Q against rho G): the fp64 pipe then carries the MMAs only.
     using R2 = typename Pair<Real>::type;
-    extern __shared__ __align__(16) unsigned char smem_raw[];
 
-    const int T = blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
+    const int T = SPLIT ? blockDim.x - 96 : blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
     const int grp = (tid >> 2) & 7;                // segment within the warp = row / column group of the MMA fragments
     // Shared-memory arrays are laid out for the LARGEST CTA of this instantiation whatever the launched size (one CTA
     // per SM: the space is there), so every stride is a compile-time constant and every shared-memory address is one
@@ -458,7 +806,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     // cluster exchange (KF_CLUSTER: the grid is one thread-block cluster): the mailbox of a CTA lives in its own shared
     // memory, [2 parity][2 sides: 0 = from the left neighbour, 1 = from the right][MBS/2 slots]; the neighbours store into
     // it through distributed shared memory, this CTA polls it locally
-    const bool clus = (flags & KF_CLUSTER) != 0;
+    const bool clus = !SPLIT && (flags & KF_CLUSTER) != 0;
     __shared__ __align__(16) unsigned char cmbox[2 * MBS * 16];
     const unsigned cm_local = smem_u32(cmbox);
     unsigned cm_remote[2] = {0, 0};      // the mailbox of the CTA my item h publishes to
@@ -482,11 +830,11 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
     }
     const size_t par_stride = clus ? (size_t)MBS * 16 : mbox_par_stride;
     __shared__ int abort_sh[2];
-    __shared__ int abort_any;
     if (tid < 2) abort_sh[tid] = 0;
     if (tid == 0) abort_any = 0;
     const int warp = tid >> 5, nwarps = T >> 5;
-    const bool pairwise = nb_sync && nctas > 1 && nwarps <= 17 && (flags & KF_PAIRWISE);
+    const bool pairwise = SPLIT || (nb_sync && nctas > 1 && nwarps <= 17 && (flags & KF_PAIRWISE));
+    const int npair = nwarps + (SPLIT ? 1 : 0);      // octets of the CTA (SPLIT: the last one is run by the three tail warps)
     // in-kernel solve: stop rule and Eq. 24 evaluated on the device (all CTAs all-gather their residual partial
     // sums through LL slots and take the same decision from the same numbers)
     const int ce = SOLVE ? p.check_every : 0;
@@ -756,8 +1104,8 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
         if (wait_failed) { abort_sh[it & 1] = 1; *(volatile int*)&abort_any = 1; }
         if (pairwise) {
             const int first = (warp & 1) ? warp - 1 : warp, second = (warp & 1) ? warp : warp - 1;
-            if (first >= 0 && first + 1 < nwarps) asm volatile("bar.sync %0, 64;" ::"r"(first) : "memory");
-            if (second >= 0 && second + 1 < nwarps) asm volatile("bar.sync %0, 64;" ::"r"(second) : "memory");
+            if (first >= 0 && first + 1 < npair) asm volatile("bar.sync %0, %1;" ::"r"(first), "r"(SPLIT && first == nwarps - 1 ? 128 : 64) : "memory");
+            if (second >= 0 && second + 1 < npair) asm volatile("bar.sync %0, %1;" ::"r"(second), "r"(SPLIT && second == nwarps - 1 ? 128 : 64) : "memory");
         } else if (nctas == 1) {
             __syncthreads();
         } else if (!nb_sync) {
@@ -803,10 +1151,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                 const Real unew = zu[h][d].y + res;                               // a8: Eq. 6c / 20c (scaled dual, A5)
                 zus[(h * 3 + d) * TS] = make2(znew, unew);
                 gM[h][d] = ((znew - unew) * invTk[h]);                                // operand of the next sweep's a1
-                if (last_sweep) {
-                    rp2 += (double)res * (double)res;
-                    if (gaprow[h]) { const double gp = (double)own[h][d] - (double)nb[h][d]; gap2 += gp * gp; }   // Eq. 21
-                }
+                if (last_sweep) rp_accum(rp2, gap2, (double)res, gaprow[h], (double)own[h][d], (double)nb[h][d]);
             }
         if constexpr (POLY) { rot_in(vs, gM[0]); rot_in(vs, gM[1]); }
         Real dz2[2][3] = {{0, 0, 0}, {0, 0, 0}};
@@ -826,10 +1171,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     const Real unew = zu2.y + res;                                      // a8: Eq. 6c / 20c
                     zus2[(h * 3 + d) * TS] = make2(znew, unew);
                     gM2[h][d] = ((znew - unew) * invTk2[h]);
-                    if (last_sweep) {
-                        rp2 += (double)res * (double)res;
-                        if (gaprow2[h]) { const double gp = (double)own2 - (double)nb2; gap2 += gp * gp; }   // Eq. 21
-                    }
+                    if (last_sweep) rp_accum(rp2, gap2, (double)res, gaprow2[h], (double)own2, (double)nb2);
                 }
             if constexpr (POLY) { rot_in(vs, gM2[0]); rot_in(vs, gM2[1]); }
         }
@@ -847,9 +1189,7 @@ __global__ void __launch_bounds__(MAXT, 1) cadmm_sweeps_mma_kernel(const KParams
                     dmma884(x0, x1, (double)(dz2[0][d] * invTk2[0]), ctab[16 * 32]);
                     dmma884(x0, x1, (double)(dz2[1][d] * invTk2[1]), ctab[17 * 32]);
                 }
-                const double xr0 = rho_cur * x0, xr1 = rho_cur * x1;
-                rdn2 += xr0 * xr0 + xr1 * xr1;
-                rd2 += (xr0 * Tp0) * (xr0 * Tp0) + (xr1 * Tp1) * (xr1 * Tp1);
+                rd_accum(rd2, rdn2, rho_cur * x0, rho_cur * x1, Tp0, Tp1);
             }
 #pragma unroll
             for (int m = 1; m < LPS; m <<= 1) {     // fixed-order tree over the 4 lanes of the segment
@@ -1006,6 +1346,21 @@ cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cud
     return launch_any(kern, p, ctas, threads, smem, st);
 }
 
+// split-tail instantiations (fp64, box + velocity [+ acceleration], plain sweeps): `threads` counts the unsplit warps as planned
+// (4k+1 of them); the launch replaces the last one by three
+template <int S, int CM>
+cudaError_t launch_mma_split(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
+    auto kern = cadmm_sweeps_mma_kernel<double, S, CM, MAXT_MMA, false, false, false, true>;
+    return launch_any(kern, p, ctas, threads + 64, smem, st);
+}
+template <int S, int CM>
+cudaError_t limits_mma_split(int threads, size_t smem, int* per_sm) {
+    auto kern = cadmm_sweeps_mma_kernel<double, S, CM, MAXT_MMA, false, false, false, true>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads + 64, smem);
+}
+
 // can `ctas` CTAs of this size run as ONE thread-block cluster?  *nclusters = co-resident clusters (0: no)
 template <typename K>
 cudaError_t cluster_query(K kern, int ctas, int threads, size_t smem, int* nclusters) {
@@ -1103,6 +1458,16 @@ int max_threads_mma(int dtype, bool poly, bool wide) {
     return poly && wide ? MAXT_MMA_POLY_WIDE : wide ? MAXT_MMA_WIDE : poly ? MAXT_MMA_POLY : (dtype == 0 ? MAXT_MMA : MAXT_MMA_F32);
 }
 
+// Split tail (see split_tail_sweeps): a plain fp64 launch of several CTAs with warp-pair synchronisation over the L2 mailbox whose
+// CTAs hold 4k+1 octets (5 or 9 warps) runs its last octet on three warps.  TOP_SPLIT_TAIL=0 in the environment keeps the
+// unsplit launch (A/B measurements; the results are bit-identical).
+bool split_tail_applies(uint32_t f, int check_every, int dtype, int ctas, int threads) {
+    static const bool enabled = [] { const char* e = getenv("TOP_SPLIT_TAIL"); return !(e && e[0] == '0'); }();
+    const int cm = mma_mask(f), warps = threads / 32;
+    return enabled && dtype == 0 && !(f & (KF_POLY | KF_WIDE | KF_CLUSTER)) && check_every == 0 && ctas > 1 &&
+           (f & KF_NEIGHBOUR_SYNC) && (f & KF_PAIRWISE) && (cm == 3 || cm == 7) && threads % 32 == 0 && (warps == 5 || warps == 9);
+}
+
 cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st) {
     const uint32_t kflags = p.flags;
     if (kflags & KF_POLY) {
@@ -1113,6 +1478,11 @@ cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int 
     if (kflags & KF_WIDE) {
         if (dtype != 0) return cudaErrorInvalidValue;      // fp64 only
         return s == 3 ? launch_mma_wide<3>(p, ctas, threads, smem, st) : launch_mma_wide<4>(p, ctas, threads, smem, st);
+    }
+    if (split_tail_applies(p.flags, p.check_every, dtype, ctas, threads)) {
+        const int cm = mma_mask(kflags);
+        if (s == 3) return cm == 3 ? launch_mma_split<3, 3>(p, ctas, threads, smem, st) : launch_mma_split<3, 7>(p, ctas, threads, smem, st);
+        return cm == 3 ? launch_mma_split<4, 3>(p, ctas, threads, smem, st) : launch_mma_split<4, 7>(p, ctas, threads, smem, st);
     }
 #define CALL(R_, S_, C_, M_) return launch_mma<R_, S_, C_, M_>(p, ctas, threads, smem, st);
     TOP_DISPATCH_MMA(CALL)
