@@ -36,8 +36,8 @@ UNIT = "segment-iterations/s"
 # are computed on the last sweep of a launch only).
 FLOPS_PER_SEG_SWEEP = {"cfg4": 4260.0, "cfg2": 3330.0, "cfg5": 3330.0, "cfg3": 740.0, "cfg1": 740.0}
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the sweep kernel on config 4 with the default plan
-PROFILED_TRAFFIC_CFG4 = 26386176
-PROFILED_TRAFFIC_SOURCE = "profiles/r2_final2_cfg4_ncu_summary.md (ncu --set full, one launch)"
+PROFILED_TRAFFIC_CFG4 = 26378240
+PROFILED_TRAFFIC_SOURCE = "profiles/r2_final3_cfg4_ncu_summary.md (ncu --set full, one launch)"
 
 
 def make_workload(name: str, rank: int = 0):

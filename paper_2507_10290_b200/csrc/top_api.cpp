@@ -608,9 +608,8 @@ top_status stage_operators(top_solver* h) {
 // the caller's arrays, then the init kernel (per-lane constants and iterate 0, reading A9).  Asynchronous.
 top_status fill_problem(top_solver* h, const double* waypoints, const double* durations, const double* start_derivs,
                         const double* end_derivs, const top_constraints* cons, PhaseTimer* pt) {
-    const int N = h->N, s = h->s, dims = h->dims, batch = h->batch, n = 2 * s;
+    const int N = h->N, s = h->s, dims = h->dims, batch = h->batch;
     const long long nseg = h->nseg;
-    const size_t LS = (size_t)h->stride;
     unsigned char* S = h->stage.get();
     std::memcpy(S + h->off_wp, waypoints, (size_t)batch * (N + 1) * dims * 8);
     std::memcpy(S + h->off_T, durations, (size_t)nseg * 8);

@@ -527,7 +527,9 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
 }
 
 template <typename Real, int S, int CM, int MAXT, bool SOLVE, bool POLY = false, bool WIDE = false, bool SPLIT = false>
-__global__ void __launch_bounds__(MAXT + (SPLIT ? 64 : 0), 1) cadmm_sweeps_mma_kernel(const KParams p) {
+// (SPLIT: MAXT + 64 threads are launched; the bound is rounded up to 12 warps so that ptxas sees what the hardware enforces -- three
+// warps on a scheduler share its 16 K registers)
+__global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 1) cadmm_sweeps_mma_kernel(const KParams p) {
     constexpr int N2 = 2 * S;
     static_assert(!SPLIT || (sizeof(Real) == 8 && !SOLVE && !POLY && !WIDE), "split tail: plain fp64 sweeps only");
     extern __shared__ __align__(16) unsigned char smem_raw[];
