@@ -20,7 +20,10 @@
  *    (the caller may free them as soon as top_create returns).
  *  - Output buffers are caller-owned.  Where an argument says "host or device" a flag tells
  *    which; device pointers must belong to the solver's device.
- *  - The handle owns all other host and device memory; top_destroy frees it.
+ *  - The handle owns all other host and device memory; top_destroy frees it.  The device memory of a
+ *    solver is ONE allocation taken from a library-private stream-ordered memory pool of its device
+ *    (cudaMallocFromPoolAsync); top_destroy returns it to that pool, which keeps up to 1 GiB for the
+ *    next top_create (re-planning loops) and hands everything back to the driver at process exit.
  *  - Every call returns a top_status; nothing throws or aborts across the ABI.  A negative
  *    status leaves a message in top_last_error().  A handle is not thread-safe.
  *  - Kernels are enqueued on top_options.cuda_stream (a cudaStream_t passed as void*;
