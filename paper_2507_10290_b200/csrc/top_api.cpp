@@ -923,7 +923,8 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     if (!o.lanes_per_segment && !o.segs_per_cta && (o.flags & TOP_SYNC_MASK) == TOP_SYNC_AUTO &&
         !(o.flags & TOP_KERNEL_NO_MMA) && !h->has_poly) {
         const bool cons_any = has_box || has_vel || has_acc;
-        const long long per_cta_max = cons_any ? 32 : 64, per_cta_min = cons_any ? 16 : 32;
+        // (chains that the SPLIT instantiation can take run best at ONE octet per CTA, three warps each: config 2 1.35 -> 1.02 us)
+        const long long per_cta_max = cons_any ? 32 : 64, per_cta_min = cons_any ? (split_supported(h->kflags, dtype) ? 8 : 16) : 32;
         if (nseg > 16 && nseg <= 16 * per_cta_max) {
             h->lanes = 4;
             plan_segs = (int)std::max<long long>(per_cta_min, round_up((int)((nseg + 15) / 16), 8));
@@ -1606,7 +1607,7 @@ extern "C" TOP_API top_status top_launch_info(const top_solver* h, int32_t* ctas
     if (ctas) *ctas = w.ctas;
     if (threads) {      // as top_iterate launches it (the fp64 tensor-core kernel may run its last octet on three warps)
         const uint32_t f = h->kflags | sync_flag(h) | w.kflags | (w.cluster ? KF_CLUSTER : 0);
-        *threads = w.threads + (h->mma && !h->numeric && split_tail_applies(f, 0, h->dtype, w.ctas, w.threads) ? 64 : 0);
+        *threads = w.threads + (h->mma && !h->numeric ? 64 * split_octets_for(f, 0, h->dtype, w.ctas, w.threads) : 0);
     }
     if (segs_per_cta) *segs_per_cta = w.segs_per_cta;
     if (smem_bytes) *smem_bytes = (int32_t)w.smem;

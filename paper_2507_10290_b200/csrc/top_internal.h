@@ -60,6 +60,7 @@ struct KParams {
     long long own_begin, own_end;   // segments whose results are written back (streaming: range minus its halos)
     int segs_per_cta;
     int k_sweeps;
+    int split_octets;       // tensor-core kernel, SPLIT instantiation: the last this-many octets of a CTA run on three warps each
     uint32_t flags;
     int max_ctas;
     unsigned int seq_base;  // sweeps launched before this launch (mod 2^32): mailbox sequence numbers never repeat
@@ -109,8 +110,11 @@ int max_threads_for(int dtype, int lanes);
 cudaError_t sweep_kernel_limits(int dtype, int s, bool constrained, int lanes, int threads, size_t smem, int* max_ctas_per_sm);
 // fp64 tensor-core variant of the 4-lane kernel (top_kernels_mma.cu: cadmm_sweeps_mma_kernel)
 cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st);
-// does a launch with these flags run its last octet on three warps (threads + 64 per CTA; top_kernels_mma.cu, "split tail")?
-bool split_tail_applies(uint32_t kparam_flags, int check_every, int dtype, int ctas, int threads);
+// how many trailing octets of a CTA does a launch with these flags run on three warps each (top_kernels_mma.cu, "split
+// octets")?  0 = none; the launch then has threads + 64 * that many threads per CTA
+int split_octets_for(uint32_t kparam_flags, int check_every, int dtype, int ctas, int threads);
+// can this problem use the SPLIT instantiation at all (fp64, box + velocity [+ acceleration], no polytope / wide consensus)?
+bool split_supported(uint32_t kflags, int dtype);
 size_t sweep_smem_bytes_mma(int dtype, bool constrained, bool poly, bool wide = false);
 int max_threads_mma(int dtype, bool poly, bool wide = false);
 cudaError_t sweep_kernel_limits_mma(int dtype, int s, uint32_t kflags, int threads, size_t smem, int* max_ctas_per_sm);

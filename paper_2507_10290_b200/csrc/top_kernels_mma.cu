@@ -199,6 +199,112 @@ __device__ __noinline__ void refresh_operator_rows(const KParams& p, long long g
     for (int d = 0; d < 3; ++d) c0_row[d * TS] = c0n[d];
 }
 
+// In-kernel stop rule, the CTA-wide part (every thread of the CTA calls it on a test sweep, after the per-octet partial sums are in
+// wsum_sh): CTA partial in a fixed order, all-gather of the per-CTA partials through LL slots (every CTA reads all of them and
+// adds them in the same order, so all CTAs take the same decision from the same numbers), Eq. 23, Eq. 24.
+// Returns true when the launch ends here (converged: stopped = 1; or a failed gather / non-finite residual); otherwise rho_new is
+// the penalty of the next sweep (== rho_cur unless Eq. 24 moved it).
+__device__ __forceinline__ bool solve_decide(const KParams& p, unsigned seq, int noct, double (*wsum_sh)[4], double (*allp_sh)[4], double* tot_sh,
+                                             int& ncheck, double rho_cur, double& rho_new, int& stopped) {
+    const int tid = threadIdx.x, T = blockDim.x, cta = blockIdx.x, nctas = gridDim.x;
+    __syncthreads();
+    unsigned char* const rb = static_cast<unsigned char*>(p.resbox) + (size_t)(ncheck & 1) * p.max_ctas * 4 * 16;
+    if (tid == 0) {
+        for (int k = 0; k < 4; ++k) {
+            double acc = 0.0;
+            for (int w = 0; w < noct; ++w) acc += wsum_sh[w][k];
+            ll_store(rb + ((size_t)cta * 4 + k) * 16, acc, seq);
+        }
+    }
+    int gather_failed = 0;
+    for (int tt = tid; tt < nctas; tt += T) {
+        const long long t0 = global_ns();
+        unsigned spins = 0;
+        for (int k = 0; k < 4; ++k) {
+            LLRaw r;
+            ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
+            while (!ll_ok(r, seq)) {
+                if ((++spins & 255u) == 0 && (*(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS)) {
+                    atomicExch(p.abort_flag, 1); gather_failed = 1; break;
+                }
+                ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
+            }
+            allp_sh[tt][k] = ll_value(r);
+        }
+    }
+    gather_failed = __syncthreads_or(gather_failed);
+    if (tid < 4) {
+        double acc = 0.0;
+        for (int tt = 0; tt < nctas; ++tt) acc += allp_sh[tt][tid];
+        tot_sh[tid] = acc;
+    }
+    __syncthreads();
+    ++ncheck;
+    const double rp = sqrt(tot_sh[0]), rd = sqrt(tot_sh[p.rd_sel]);
+    const bool conv = rp < p.tol && rd < p.tol;
+    if (conv || gather_failed || !(rp == rp) || !(rd == rd)) { stopped = conv ? 1 : 0; return true; }
+    rho_new = rho_cur;
+    if (p.adaptive) {      // Eq. 24
+        if (rp > p.mu * rd) rho_new = rho_cur * p.tau_incr;
+        else if (rd > p.mu * rp) rho_new = rho_cur / p.tau_decr;
+    }
+    return false;
+}
+
+// Constant operands of the two contractions, written once per launch by the first warp of the CTA (ctab = table base + lane of warp).
+template <int S, bool WIDE>
+__device__ __forceinline__ void fill_ctab(double* ctab, int lane32) {
+    constexpr int N2 = 2 * S;
+    const int lane = lane32 & 3, grp = lane32 >> 2;
+    // ---- constant operands of the two contractions (B fragments: row k = 4*kstep + lane, column n = grp)
+    // a1: k runs over the 32 items [consensus rows | E0 samples | E1 samples | E2 samples], n = coefficient row
+    // a3: k = coefficient row, n runs over the items of one block, permuted so that the accumulator columns
+    //     2*lane, 2*lane+1 are the lane's own items lane, lane+4
+    {
+        const int a = grp;
+#pragma unroll
+        for (int kk = 0; kk < 8; ++kk) {
+            const int b = kk >> 1, item = lane + 4 * (kk & 1);
+            const double tau = (double)(item + 1) / (double)(MS + 1);       // sample time (reading A10)
+            double v = 0.0;
+            if (a < N2) {
+                if (b == 0) { if (item < N2) v = beta_entry(item % S, a, item < S ? 0.0 : 1.0); }
+                else v = beta_entry(b - 1, a, tau);
+            }
+            ctab[kk * 32] = v;
+        }
+        const int item = (grp >> 1) + 4 * (grp & 1);
+        const double tau = (double)(item + 1) / (double)(MS + 1);
+#pragma unroll
+        for (int kk = 0; kk < 2; ++kk) {
+            const int ar = 4 * kk + lane;
+#pragma unroll
+            for (int nt = 0; nt < 4; ++nt) {
+                double v = 0.0;
+                if (ar < N2) {
+                    if (nt == 0) { if (item < N2) v = beta_entry(item % S, ar, item < S ? 0.0 : 1.0); }
+                    else v = beta_entry(nt - 1, ar, tau);
+                }
+                ctab[(8 + kk * 4 + nt) * 32] = v;
+            }
+        }
+        if (WIDE) {
+            // second consensus block.  a1 operand of k-step h (h = 0 start, 1 end boundary): row k = lane <-> order S + lane,
+            // column n = grp = coefficient row.  a3 operand of k-step kk: row k = coefficient row 4 kk + lane, column n = grp
+            // <-> item (grp >> 1, side grp & 1), so that accumulator columns 2t, 2t+1 are the lane's own two rows.
+#pragma unroll
+            for (int h = 0; h < 2; ++h)
+                ctab[(16 + h) * 32] = (a < N2 && lane <= S - 2) ? beta_entry(S + lane, a, h ? 1.0 : 0.0) : 0.0;
+            const int t2 = grp >> 1, h2 = grp & 1;
+#pragma unroll
+            for (int kk = 0; kk < 2; ++kk) {
+                const int ar = 4 * kk + lane;
+                ctab[(18 + kk) * 32] = (ar < N2 && t2 <= S - 2) ? beta_entry(S + t2, ar, h2 ? 1.0 : 0.0) : 0.0;
+            }
+        }
+    }
+}
+
 // ================================================================================================ split tail
 // Load balance of the fp64 kernel when a CTA holds 4k+1 octets (config 4: 68 segments = 8 octets + 4 segments): as 4k+1 warps
 // one scheduler carries k+1 warps, and all the others wait for it at the pair barriers.  In the SPLIT instantiation the LAST
@@ -210,14 +316,26 @@ __device__ __noinline__ void refresh_operator_rows(const KParams& p, long long g
 // barrier (128 threads); towards the next CTA each publishes and fetches its own dim's mailbox slots.
 // (A kernel made of such warps ONLY was tried: 864 threads leave 72 registers and every operator row is read three times --
 // shared-memory bound, slower.  Here only one octet pays that.)
-constexpr int SPLIT_BALL_BAR = 15;      // named barrier of the three tail warps (the pair barriers use ids 0..8)
+// The same split applied to EVERY octet of a small CTA (<= 4 octets, 12 warps) shortens the dependent chain of a sweep and puts
+// three light warps on every scheduler instead of one heavy one: the latency-bound short and mid-size chains gain most
+// (p.split_octets = how many trailing octets are split; 1 for the tail case above).
+constexpr int SPLIT_BALL_BAR = 15;      // named barrier of split octet j: 15 - j (the pair barriers use ids 0..8)
+constexpr int SPLIT_MAX_ALL = 3;        // cluster CTAs of at most this many octets are split entirely
 
-template <int S, int CM, int MAXT>
-__device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned char* smem_raw, volatile int* abort_any, double2 (*nbuf)[2][3][32]) {
+// octets [0, W) run on one warp each, octets [W, noct) on three: threads of the pair barrier that joins octets b and b + 1
+__device__ __forceinline__ int pair_threads(int b, int W) { return (b >= W ? 96 : 32) + (b + 1 >= W ? 96 : 32); }
+
+// SOLVE (in-kernel stop rule and Eq. 24, as in cadmm_sweeps_mma_kernel): only for CTAs that are split entirely; one CTA barrier
+// per sweep instead of the pair barriers.
+struct SolveShared { int* abort_sh; double (*wsum)[4]; double (*allp)[4]; double* tot; };
+
+template <int S, int CM, int MAXT, bool SOLVE>
+__device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned char* smem_raw, volatile int* abort_any, unsigned char* cmbox, const SolveShared sv) {
     constexpr int N2 = 2 * S;
-    constexpr int TS = MAXT, SA = MAXT / 4, BPAR = (SA + 2) * 24;
-    const int tmain = (int)blockDim.x - 96;                       // threads of the unsplit warps in front
-    const int oct = tmain >> 5, d = ((int)threadIdx.x - tmain) >> 5, lane32 = threadIdx.x & 31;
+    constexpr int TS = MAXT, SA = MAXT / 4, BPAR = (SA + 2) * 24, MBS = 24;
+    const int nsplit = p.split_octets, tmain = (int)blockDim.x - 96 * nsplit;      // threads of the unsplit warps in front
+    const int W = tmain >> 5, noct = W + nsplit, rel = (int)threadIdx.x - tmain, jsp = rel / 96;
+    const int oct = W + jsp, d = (rel - 96 * jsp) >> 5, lane32 = threadIdx.x & 31;
     const int lane = lane32 & 3, grp = lane32 >> 2, sl = oct * 8 + grp, vt = sl * 4 + lane;      // vt: the thread an unsplit warp would be
     const int SEGS = p.segs_per_cta, cta = blockIdx.x, nctas = gridDim.x;
     const uint32_t flags = p.flags;
@@ -236,6 +354,10 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
     double* Xs = reinterpret_cast<double*>(smem_raw + L.xs) + (size_t)sl * XSTRIDE + d * 8;
     double* Bs = reinterpret_cast<double*>(smem_raw + L.bs);                                  // [2 parity][SA+2][8 rows][3]
     double* zoffs = reinterpret_cast<double*>(smem_raw + L.zoff) + sl;                        // [(side*3 + dim) * SA]
+    // ball exchange buffer of this octet, [parity][item h][dim][lane of warp] (y_v, y_a): in the slot of the (phi_v, phi_a)
+    // pairs, which the SPLIT instantiation does not keep in shared memory
+    double2* nbuf = reinterpret_cast<double2*>(smem_raw + L.ph) + (size_t)jsp * (2 * 2 * 3 * 32) + lane32;
+    const int ball_bar = SPLIT_BALL_BAR - jsp;
 
     const long long cta_first = p.seg_begin + (long long)cta * SEGS;
     const long long remaining = p.seg_end - cta_first;
@@ -324,15 +446,40 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
     // launch of zero sweeps writes nothing back at all)
     const double vmax = p.vmax, amax = p.amax;
     unsigned char* const mbox = static_cast<unsigned char*>(p.Bedge);
-    const size_t mbox_par_stride = (size_t)p.max_ctas * 24 * 16;
+    // cluster exchange (KF_CLUSTER; see cadmm_sweeps_mma_kernel): the mailbox is the CTA's own shared memory
+    const bool clus = (flags & KF_CLUSTER) != 0;
+    const unsigned cm_local = smem_u32(cmbox);
+    unsigned cm_remote[2] = {0, 0};
+    if (clus) {
+        cm_remote[0] = cta > 0 ? cluster_map(cm_local, (unsigned)(cta - 1)) : 0u;
+        cm_remote[1] = cta + 1 < nctas ? cluster_map(cm_local, (unsigned)(cta + 1)) : 0u;
+        cluster_barrier();
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const bool er = right[h];
+            pub_off[h] = ((er ? 0 : 1) * (MBS / 2) + korder[h] * 3 + d) * 16;
+            if (need && need_h == h) need_off = ((er ? 1 : 0) * (MBS / 2) + korder[h] * 3 + d) * 16;
+        }
+    }
+    const size_t par_stride = clus ? (size_t)MBS * 16 : (size_t)p.max_ctas * MBS * 16;
+    const int bfirst = (oct & 1) ? oct - 1 : oct, bsecond = (oct & 1) ? oct : oct - 1;      // pair barriers: the even id first, as every octet does
+    const bool use_first = bfirst >= 0 && bfirst + 1 < noct, use_second = bsecond >= 0 && bsecond + 1 < noct;
+    const int n_first = use_first ? pair_threads(bfirst, W) : 0, n_second = use_second ? pair_threads(bsecond, W) : 0;
+    const int ce = SOLVE ? p.check_every : 0;
+    double rho_cur = p.rho;
+    int ncheck = 0, sweeps_done = p.k_sweeps, stopped = 0;
+    double phv_[2] = {0, 0}, pha_[2] = {0, 0};      // SOLVE: phi of the newest iterate (Eq. 24 rebuilds the operands gv, ga from it)
     __syncthreads();      // (the one CTA barrier of the launch: the unsplit warps arrive from cadmm_sweeps_mma_kernel)
 
     for (int it = 0; it < p.k_sweeps; ++it) {
         const unsigned seq = p.seq_base + (unsigned)it + 1u;
         const int par = (int)(seq & 1u);
-        const bool last_sweep = (it == p.k_sweeps - 1);
+        // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
+        const bool last_sweep = (it == p.k_sweeps - 1) || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
         double* const Bcur = Bs + par * BPAR;
-        unsigned char* const mpar = mbox + par * mbox_par_stride;
+        unsigned char* const mpar = mbox + par * par_stride;      // (cluster exchange: only the offset part is used)
+        const unsigned cpar = (unsigned)(par * MBS * 16);
+        double2* const nb = nbuf + par * (2 * 3 * 32);
 
         // ================= phase A: segment local, this dim =================
         double2 pm[2][4];
@@ -375,10 +522,10 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
 #pragma unroll
         for (int h = 0; h < 2; ++h) {
             if (isrow[h]) Bcur[own_off[h]] = Bnd[h];
-            if (pub[h]) ll_store(mpar + pub_off[h], Bnd[h], seq);
+            if (pub[h]) { if (clus) ll_store_cluster(cm_remote[right[h] ? 1 : 0] + cpar + pub_off[h], Bnd[h], seq); else ll_store(mpar + pub_off[h], Bnd[h], seq); }
         }
         LLRaw rr;
-        if (need) ll_issue(mpar + need_off, rr);
+        if (need) { if (clus) ll_issue_smem(cm_local + cpar + need_off, rr); else ll_issue(mpar + need_off, rr); }
         {
             double Pv[2] = {0, 0}, Vv[2] = {0, 0}, Av[2] = {0, 0};
             if (has_vel) { double e0 = 0, e1 = 0; dmma884(e0, e1, cacc[0], ctab[10 * 32]); dmma884(e0, e1, cacc[1], ctab[14 * 32]); Vv[0] = e0; Vv[1] = e1; }
@@ -399,17 +546,18 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
                 for (int h = 0; h < 2; ++h) {
                     if (has_vel) yv[h] = Vv[h] * invT + w2[h].x;
                     if (has_acc) ya[h] = Av[h] * invT2 + w2[h].y;
-                    nbuf[par][h][d][lane32] = make_double2(yv[h], ya[h]);
+                    nb[(h * 3 + d) * 32] = make_double2(yv[h], ya[h]);
                 }
-                asm volatile("bar.sync %0, 96;" ::"n"(SPLIT_BALL_BAR) : "memory");
+                asm volatile("bar.sync %0, 96;" ::"r"(ball_bar) : "memory");
 #pragma unroll
                 for (int h = 0; h < 2; ++h) {
-                    const double2 s0 = nbuf[par][h][0][lane32], s1 = nbuf[par][h][1][lane32], s2 = nbuf[par][h][2][lane32];
+                    const double2 s0 = nb[(h * 3 + 0) * 32], s1 = nb[(h * 3 + 1) * 32], s2 = nb[(h * 3 + 2) * 32];
                     if (has_vel) {
                         const double y[3] = {s0.x, s1.x, s2.x};
                         const double scale = ball_scale(y, vmax);
                         const double ph = scale * yv[h];
                         w2[h].x = yv[h] - ph; gv[h] = (ph - w2[h].x) * invT;
+                        if (SOLVE) phv_[h] = ph;
                         if (last_sweep && owned) static_cast<double*>(p.phv_out)[d * stride + gt[h]] = ph;
                     }
                     if (has_acc) {
@@ -417,6 +565,7 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
                         const double scale = ball_scale(y, amax);
                         const double ph = scale * ya[h];
                         w2[h].y = ya[h] - ph; ga[h] = (ph - w2[h].y) * invT2;
+                        if (SOLVE) pha_[h] = ph;
                         if (last_sweep && owned) static_cast<double*>(p.pha_out)[d * stride + gt[h]] = ph;
                     }
                     ws[h * 3 * TS] = w2[h];
@@ -442,15 +591,21 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
                 unsigned spins = 0;
                 bool failed = false;
                 do {
-                    if (!okk) { ll_issue(mpar + need_off, rr); okk = ll_ok(rr, seq); }
+                    if (!okk) { if (clus) ll_issue_smem(cm_local + cpar + need_off, rr); else ll_issue(mpar + need_off, rr); okk = ll_ok(rr, seq); }
                     bool bail = false;
                     if ((++spins & 255u) == 0) bail = *(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS;
                     if (__any_sync(0xffffffffu, bail)) { if (!okk) { atomicExch(p.abort_flag, 1); failed = true; } break; }
                 } while (!__all_sync(0xffffffffu, okk));
-                if (failed) *abort_any = 1;
+                if (failed) { *abort_any = 1; if (SOLVE) sv.abort_sh[it & 1] = 1; }
             }
         }
-        asm volatile("bar.sync %0, 128;" ::"r"(oct - 1) : "memory");
+        if (SOLVE) {
+            __syncthreads();
+            if (sv.abort_sh[it & 1]) break;
+        } else {
+            if (use_first) asm volatile("bar.sync %0, %1;" ::"r"(bfirst), "r"(n_first) : "memory");
+            if (use_second) asm volatile("bar.sync %0, %1;" ::"r"(bsecond), "r"(n_second) : "memory");
+        }
 
         // ================= phase B: consensus, dual, residuals (this dim)
         double res_[2], own_[2], nb_[2], dz[2];
@@ -476,34 +631,80 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
             double x0 = 0, x1 = 0;
             dmma884(x0, x1, dz[0] * invTk[0], ctab[0 * 32]);
             dmma884(x0, x1, dz[1] * invTk[1], ctab[1 * 32]);
-            double2 (*rb)[3][32] = nbuf[par ^ 1];      // (free: everybody is past this sweep's ball barrier, and the launch ends here)
-            rb[0][d][lane32] = make_double2(res_[0], res_[1]);
-            rb[1][d][lane32] = make_double2(p.rho * x0, p.rho * x1);
-            asm volatile("bar.sync %0, 96;" ::"n"(SPLIT_BALL_BAR) : "memory");
-            double2 (*gb)[3][32] = nbuf[par];          // own - nb of the gap rows (the ball exchange of this sweep is over)
-            gb[0][d][lane32] = make_double2(own_[0] - nb_[0], own_[1] - nb_[1]);
-            asm volatile("bar.sync %0, 96;" ::"n"(SPLIT_BALL_BAR) : "memory");
+            double2* const rb = nbuf + (par ^ 1) * (2 * 3 * 32);      // (free: everybody is past this sweep's ball barrier, and the launch ends here)
+            rb[(0 * 3 + d) * 32] = make_double2(res_[0], res_[1]);
+            rb[(1 * 3 + d) * 32] = make_double2(rho_cur * x0, rho_cur * x1);
+            asm volatile("bar.sync %0, 96;" ::"r"(ball_bar) : "memory");
+            double2* const gb = nb;                     // own - nb of the gap rows (the ball exchange of this sweep is over)
+            gb[d * 32] = make_double2(own_[0] - nb_[0], own_[1] - nb_[1]);
+            asm volatile("bar.sync %0, 96;" ::"r"(ball_bar) : "memory");
+            double rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
             if (d == 0) {
                 const double Tp0 = static_cast<const double*>(p.Tpow)[gseg * LANES + 2 * lane], Tp1 = static_cast<const double*>(p.Tpow)[gseg * LANES + 2 * lane + 1];
-                double rp2 = 0, rd2 = 0, rdn2 = 0, gap2 = 0;
 #pragma unroll
                 for (int h = 0; h < 2; ++h)
 #pragma unroll
                     for (int dd = 0; dd < 3; ++dd) {
-                        const double2 r2 = rb[0][dd][lane32], g2 = gb[0][dd][lane32];
+                        const double2 r2 = rb[dd * 32], g2 = gb[dd * 32];
                         const double r = h ? r2.y : r2.x, g = h ? g2.y : g2.x;
                         rp2 = fma(r, r, rp2);
                         if (gaprow[h]) gap2 = fma(g, g, gap2);
                     }
 #pragma unroll
-                for (int dd = 0; dd < 3; ++dd) { const double2 x2 = rb[1][dd][lane32]; rd_accum(rd2, rdn2, x2.x, x2.y, Tp0, Tp1); }
+                for (int dd = 0; dd < 3; ++dd) { const double2 x2 = rb[(3 + dd) * 32]; rd_accum(rd2, rdn2, x2.x, x2.y, Tp0, Tp1); }
 #pragma unroll
                 for (int m = 1; m < 4; m <<= 1) { rp2 += shfl_xor(rp2, m); rd2 += shfl_xor(rd2, m); rdn2 += shfl_xor(rdn2, m); gap2 += shfl_xor(gap2, m); }
                 if (owned && lane == 0) { double* o = p.part + gseg * 4; o[0] = rp2; o[1] = rd2; o[2] = rdn2; o[3] = gap2; }
             }
+            if (SOLVE && ce > 0) {
+                // ---- octet partial (the dim-0 warp holds the per-segment sums), then the CTA-wide decision
+                if (d == 0) {
+                    double q4[4] = {rp2, rd2, rdn2, gap2};
+                    if (!(owned && lane == 0)) { q4[0] = q4[1] = q4[2] = q4[3] = 0.0; }
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { q4[k] += shfl_xor(q4[k], 4); q4[k] += shfl_xor(q4[k], 8); q4[k] += shfl_xor(q4[k], 16); }
+                    if (lane32 == 0) { for (int k = 0; k < 4; ++k) sv.wsum[oct][k] = q4[k]; }
+                }
+                double rho_new = rho_cur;
+                if (solve_decide(p, seq, noct, sv.wsum, sv.allp, sv.tot, ncheck, rho_cur, rho_new, stopped)) { sweeps_done = it + 1; break; }
+                if (rho_new != rho_cur) {      // Eq. 24 moved rho: scaled duals times rho_old / rho_new (A16), operands, operator rows
+                    const double ratio = rho_cur / rho_new;
+                    const double lo = has_box ? lohi[d * SA] : 0.0, hi = has_box ? lohi[(3 + d) * SA] : 0.0;
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        double2 zz = zus[h * 3 * TS];
+                        zz.y *= ratio;
+                        zus[h * 3 * TS] = zz;
+                        gM[h] = (zz.x - zz.y) * invTk[h];
+                        if (has_box) {
+                            double2 q = qs[h * 3 * TS];
+                            if (q.x < 0) q.x *= ratio;
+                            if (q.y < 0) q.y *= ratio;
+                            qs[h * 3 * TS] = q;
+                            A0[h] = (hi - fabs(q.x)) + (lo + fabs(q.y));
+                        }
+                        if (has_vel || has_acc) {
+                            double2 w2 = ws[h * 3 * TS];
+                            w2.x *= ratio; w2.y *= ratio;
+                            ws[h * 3 * TS] = w2;
+                            if (has_vel) gv[h] = (phv_[h] - w2.x) * invT;
+                            if (has_acc) ga[h] = (pha_[h] - w2.y) * invT2;
+                        }
+                        if (d == 0) refresh_operator_rows<N2, TS>(p, gseg, gt[h], jj[h], rho_new, Pms + h * 4 * TS, c0s + h * 3 * TS);
+                    }
+                    asm volatile("bar.sync %0, 96;" ::"r"(ball_bar) : "memory");      // the other two dims read the new operator rows
+                    rho_cur = rho_new;
+                }
+            }
         }
     }
+    if (SOLVE && ce > 0 && cta == 0 && threadIdx.x == 0) {
+        double* o = p.solve_out;
+        o[0] = (double)sweeps_done; o[1] = (double)stopped; o[2] = rho_cur;
+        o[3] = sqrt(sv.tot[0]); o[4] = sqrt(sv.tot[1]); o[5] = sqrt(sv.tot[2]); o[6] = sqrt(sv.tot[3]);
+    }
 
+    if (clus) cluster_barrier();      // nobody leaves while a neighbour may still store into its mailbox
     // ---- write iterate k + k_sweeps back (phi went out on the last sweep)
     if (owned) {
 #pragma unroll
@@ -531,22 +732,37 @@ template <typename Real, int S, int CM, int MAXT, bool SOLVE, bool POLY = false,
 // warps on a scheduler share its 16 K registers)
 __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 1) cadmm_sweeps_mma_kernel(const KParams p) {
     constexpr int N2 = 2 * S;
-    static_assert(!SPLIT || (sizeof(Real) == 8 && !SOLVE && !POLY && !WIDE), "split tail: plain fp64 sweeps only");
+    static_assert(!SPLIT || (sizeof(Real) == 8 && !POLY && !WIDE), "split octets: fp64, box / ball sets only");
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int MBS = WIDE ? 48 : 24;              // mailbox slots per CTA and parity: [2 sides][4 or 8 orders][3 dims]
     __shared__ int abort_any;
-    __shared__ double2 nbuf_sh[SPLIT ? 2 : 1][2][3][SPLIT ? 32 : 1];
-    if constexpr (SPLIT) {      // the last three warps run the last octet, one dim each
-        if ((int)threadIdx.x >= (int)blockDim.x - 96) {
-            split_tail_sweeps<S, (CM == 0 || CM == CM_RUNTIME) ? 7 : CM, MAXT>(p, smem_raw, &abort_any, reinterpret_cast<double2 (*)[2][3][32]>(&nbuf_sh[0][0][0][0]));
+    __shared__ int abort_sh[2];
+    __shared__ __align__(16) unsigned char cmbox[2 * MBS * 16];      // cluster exchange: this CTA's mailbox (see below)
+    __shared__ double wsum_sh[SOLVE ? 32 : 1][4];      // in-kernel stop rule: per-octet partial sums, per-CTA partial sums, totals
+    __shared__ double allp_sh[SOLVE ? 160 : 1][4];
+    __shared__ double tot_sh[4];
+    // ---- CTA-wide prologue (before the split octets branch off): constant MMA operands, flags, cluster mailbox cleared
+    {
+        const SmemLayoutMma L0 = smem_layout_mma(CM != 0 || POLY, MAXT / 4, POLY, (int)sizeof(Real), WIDE);
+        if (threadIdx.x < 32) fill_ctab<S, WIDE>(reinterpret_cast<double*>(smem_raw + L0.ctab) + threadIdx.x, (int)threadIdx.x);
+        if (threadIdx.x < 2) abort_sh[threadIdx.x] = 0;
+        if (threadIdx.x == 0) abort_any = 0;
+        if (p.flags & KF_CLUSTER) for (int i = threadIdx.x; i < 2 * MBS * 4; i += blockDim.x) reinterpret_cast<unsigned*>(cmbox)[i] = 0u;
+    }
+    if constexpr (SPLIT) {      // the last p.split_octets octets run on three warps each, one dim per warp
+        // (SPLIT with the in-kernel stop rule: every octet is split, this is the whole kernel)
+        if (SOLVE || (int)threadIdx.x >= (int)blockDim.x - 96 * p.split_octets) {
+            const SolveShared sv = {abort_sh, wsum_sh, allp_sh, tot_sh};
+            split_tail_sweeps<S, (CM == 0 || CM == CM_RUNTIME) ? 7 : CM, MAXT, SOLVE>(p, smem_raw, &abort_any, cmbox, sv);
             return;
         }
     }
+    if constexpr (!(SPLIT && SOLVE)) {
     // WIDE: the paper-literal consensus (reading A1): derivative orders 0..2s-2 at both boundaries.
     // Orders 0..s-1 are the first block (as always); orders s..2s-2 form a SECOND block of consensus rows with the same
     // lane <-> row map: lane t owns order s+t at the start boundary (item h = 0) and at the end boundary (h = 1), t <= s-2.
     // Rows that do not exist (t = s-1; the trajectory ends, where z_0 / z_N carry orders < s only) have 1/T^k = 0 in
     // invTk2: their operand, boundary value, residual and dual are identically 0.
-    constexpr int MBS = WIDE ? 48 : 24;              // mailbox slots per CTA and parity: [2 sides][4 or 8 orders][3 dims]
     constexpr int LPS = 4;                         // lanes per segment
     constexpr bool CONS = CM != 0 || POLY;
     static_assert(!(SOLVE && POLY), "the in-kernel stop rule is not instantiated for polytope corridors (host loop)");
@@ -556,8 +772,7 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
     // apply a2 stays fp64 (an fp32 operator loses Q against rho G): the fp64 pipe then carries the MMAs only.
     using R2 = typename Pair<Real>::type;
 
-    const int T = SPLIT ? blockDim.x - 96 : blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
-    const int grp = (tid >> 2) & 7;                // segment within the warp = row / column group of the MMA fragments
+    const int T = SPLIT ? blockDim.x - 96 * p.split_octets : blockDim.x, tid = threadIdx.x, lane = tid & (LPS - 1), sl = tid >> 2;
     // Shared-memory arrays are laid out for the LARGEST CTA of this instantiation whatever the launched size (one CTA
     // per SM: the space is there), so every stride is a compile-time constant and every shared-memory address is one
     // per-thread base register plus an immediate (with run-time strides ptxas re-derived the offsets inside the loop).
@@ -614,53 +829,6 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
         korder[h] = right[h] ? jj[h] - S : jj[h];
     }
 
-    // ---- constant operands of the two contractions (B fragments: row k = 4*kstep + lane, column n = grp)
-    // a1: k runs over the 32 items [consensus rows | E0 samples | E1 samples | E2 samples], n = coefficient row
-    // a3: k = coefficient row, n runs over the items of one block, permuted so that the accumulator columns
-    //     2*lane, 2*lane+1 are the lane's own items lane, lane+4
-    if (tid < 32) {
-        const int a = grp;
-#pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
-            const int b = kk >> 1, item = lane + 4 * (kk & 1);
-            const double tau = (double)(item + 1) / (double)(MS + 1);       // sample time (reading A10)
-            double v = 0.0;
-            if (a < N2) {
-                if (b == 0) { if (item < N2) v = beta_entry(item % S, a, item < S ? 0.0 : 1.0); }
-                else v = beta_entry(b - 1, a, tau);
-            }
-            ctab[kk * 32] = v;
-        }
-        const int item = (grp >> 1) + 4 * (grp & 1);
-        const double tau = (double)(item + 1) / (double)(MS + 1);
-#pragma unroll
-        for (int kk = 0; kk < 2; ++kk) {
-            const int ar = 4 * kk + lane;
-#pragma unroll
-            for (int nt = 0; nt < 4; ++nt) {
-                double v = 0.0;
-                if (ar < N2) {
-                    if (nt == 0) { if (item < N2) v = beta_entry(item % S, ar, item < S ? 0.0 : 1.0); }
-                    else v = beta_entry(nt - 1, ar, tau);
-                }
-                ctab[(8 + kk * 4 + nt) * 32] = v;
-            }
-        }
-        if (WIDE) {
-            // second consensus block.  a1 operand of k-step h (h = 0 start, 1 end boundary): row k = lane <-> order S + lane,
-            // column n = grp = coefficient row.  a3 operand of k-step kk: row k = coefficient row 4 kk + lane, column n = grp
-            // <-> item (grp >> 1, side grp & 1), so that accumulator columns 2t, 2t+1 are the lane's own two rows.
-#pragma unroll
-            for (int h = 0; h < 2; ++h)
-                ctab[(16 + h) * 32] = (a < N2 && lane <= S - 2) ? beta_entry(S + lane, a, h ? 1.0 : 0.0) : 0.0;
-            const int t2 = grp >> 1, h2 = grp & 1;
-#pragma unroll
-            for (int kk = 0; kk < 2; ++kk) {
-                const int ar = 4 * kk + lane;
-                ctab[(18 + kk) * 32] = (ar < N2 && t2 <= S - 2) ? beta_entry(S + t2, ar, h2 ? 1.0 : 0.0) : 0.0;
-            }
-        }
-    }
     // B operand of a k-block: entries i0 (k-step of the lane's first item) and i1 (second item) of the constant table
     auto ldb = [&](int i0, int i1) {
         BOp b;
@@ -787,7 +955,7 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
             }
             if (has_vel) { w_v = static_cast<const Real*>(p.wv)[i]; ph_v = static_cast<const Real*>(p.phv)[i]; gv[h][d] = (ph_v - w_v) * invT; }
             if (has_acc) { w_a = static_cast<const Real*>(p.wa)[i]; ph_a = static_cast<const Real*>(p.pha)[i]; ga[h][d] = (ph_a - w_a) * invT2; }
-            if (CONS) { ws[(h * 3 + d) * TS] = make2(w_v, w_a); phs[(h * 3 + d) * TS] = make2(ph_v, ph_a); }
+            if (CONS) { ws[(h * 3 + d) * TS] = make2(w_v, w_a); if (!SPLIT) phs[(h * 3 + d) * TS] = make2(ph_v, ph_a); }
         }
     if constexpr (POLY) {      // consensus rows enter the segment's rotated frame; the E0 operand is sum_k (b_k - s_k - v_k) a_k
 #pragma unroll
@@ -808,12 +976,10 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
     // cluster exchange (KF_CLUSTER: the grid is one thread-block cluster): the mailbox of a CTA lives in its own shared
     // memory, [2 parity][2 sides: 0 = from the left neighbour, 1 = from the right][MBS/2 slots]; the neighbours store into
     // it through distributed shared memory, this CTA polls it locally
-    const bool clus = !SPLIT && (flags & KF_CLUSTER) != 0;
-    __shared__ __align__(16) unsigned char cmbox[2 * MBS * 16];
+    const bool clus = (flags & KF_CLUSTER) != 0;
     const unsigned cm_local = smem_u32(cmbox);
     unsigned cm_remote[2] = {0, 0};      // the mailbox of the CTA my item h publishes to
     if (clus) {
-        for (int i = tid; i < 2 * MBS * 4; i += T) reinterpret_cast<unsigned*>(cmbox)[i] = 0u;
         cm_remote[0] = cta > 0 ? cluster_map(cm_local, (unsigned)(cta - 1)) : 0u;            // left neighbour
         cm_remote[1] = cta + 1 < nctas ? cluster_map(cm_local, (unsigned)(cta + 1)) : 0u;    // right neighbour
         cluster_barrier();      // every CTA of the cluster runs and has cleared its mailbox before anyone stores into it
@@ -831,19 +997,13 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
         }
     }
     const size_t par_stride = clus ? (size_t)MBS * 16 : mbox_par_stride;
-    __shared__ int abort_sh[2];
-    if (tid < 2) abort_sh[tid] = 0;
-    if (tid == 0) abort_any = 0;
     const int warp = tid >> 5, nwarps = T >> 5;
     const bool pairwise = SPLIT || (nb_sync && nctas > 1 && nwarps <= 17 && (flags & KF_PAIRWISE));
-    const int npair = nwarps + (SPLIT ? 1 : 0);      // octets of the CTA (SPLIT: the last one is run by the three tail warps)
+    const int npair = nwarps + (SPLIT ? p.split_octets : 0);      // octets of the CTA (SPLIT: the last ones run on three warps each)
     // in-kernel solve: stop rule and Eq. 24 evaluated on the device (all CTAs all-gather their residual partial
     // sums through LL slots and take the same decision from the same numbers)
     const int ce = SOLVE ? p.check_every : 0;
     double rho_cur = p.rho;
-    __shared__ double wsum_sh[SOLVE ? 32 : 1][4];
-    __shared__ double allp_sh[SOLVE ? 160 : 1][4];
-    __shared__ double tot_sh[4];
     int ncheck = 0, sweeps_done = p.k_sweeps, stopped = 0;
     __syncthreads();
     for (int it = 0; it < p.k_sweeps; ++it) {
@@ -1045,7 +1205,14 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
                         ws[(h * 3 + d) * TS] = w2[h][d];
                         // phi itself is only read back at the end of the launch and by the rho change of a test sweep (its
                         // effect on the next sweep is already in the operands gv, ga)
-                        if (last_sweep) phs[(h * 3 + d) * TS] = ph2[h][d];
+                        // (SPLIT: that slot of shared memory is the split octets' ball exchange; phi goes straight out)
+                        if (last_sweep) {
+                            if (!SPLIT) phs[(h * 3 + d) * TS] = ph2[h][d];
+                            else if (owned) {
+                                if (has_vel) static_cast<Real*>(p.phv_out)[d * stride + gt[h]] = ph2[h][d].x;
+                                if (has_acc) static_cast<Real*>(p.pha_out)[d * stride + gt[h]] = ph2[h][d].y;
+                            }
+                        }
                     }
             }
             if constexpr (POLY) {         // a7 + a8 per (sample, plane): q = -(a_k'p - b_k + v);  next operand sum_k (b_k - |q_k|) a_k
@@ -1106,8 +1273,8 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
         if (wait_failed) { abort_sh[it & 1] = 1; *(volatile int*)&abort_any = 1; }
         if (pairwise) {
             const int first = (warp & 1) ? warp - 1 : warp, second = (warp & 1) ? warp : warp - 1;
-            if (first >= 0 && first + 1 < npair) asm volatile("bar.sync %0, %1;" ::"r"(first), "r"(SPLIT && first == nwarps - 1 ? 128 : 64) : "memory");
-            if (second >= 0 && second + 1 < npair) asm volatile("bar.sync %0, %1;" ::"r"(second), "r"(SPLIT && second == nwarps - 1 ? 128 : 64) : "memory");
+            if (first >= 0 && first + 1 < npair) asm volatile("bar.sync %0, %1;" ::"r"(first), "r"(SPLIT ? pair_threads(first, nwarps) : 64) : "memory");
+            if (second >= 0 && second + 1 < npair) asm volatile("bar.sync %0, %1;" ::"r"(second), "r"(SPLIT ? pair_threads(second, nwarps) : 64) : "memory");
         } else if (nctas == 1) {
             __syncthreads();
         } else if (!nb_sync) {
@@ -1208,47 +1375,10 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
 #pragma unroll
                 for (int k = 0; k < 4; ++k) { q4[k] += shfl_xor(q4[k], 4); q4[k] += shfl_xor(q4[k], 8); q4[k] += shfl_xor(q4[k], 16); }
                 if ((tid & 31) == 0) { for (int k = 0; k < 4; ++k) wsum_sh[tid >> 5][k] = q4[k]; }
-                __syncthreads();
-                unsigned char* const rb = static_cast<unsigned char*>(p.resbox) + (size_t)(ncheck & 1) * p.max_ctas * 4 * 16;
-                if (tid == 0) {
-                    for (int k = 0; k < 4; ++k) {
-                        double acc = 0.0;
-                        for (int w = 0; w < (T >> 5); ++w) acc += wsum_sh[w][k];
-                        ll_store(rb + ((size_t)cta * 4 + k) * 16, acc, seq);
-                    }
-                }
-                int gather_failed = 0;
-                for (int tt = tid; tt < nctas; tt += T) {
-                    const long long t0 = global_ns();
-                    unsigned spins = 0;
-                    for (int k = 0; k < 4; ++k) {
-                        LLRaw r;
-                        ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
-                        while (!ll_ok(r, seq)) {
-                            if ((++spins & 255u) == 0 && (*(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS)) {
-                                atomicExch(p.abort_flag, 1); gather_failed = 1; break;
-                            }
-                            ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
-                        }
-                        allp_sh[tt][k] = ll_value(r);
-                    }
-                }
-                gather_failed = __syncthreads_or(gather_failed);
-                if (tid < 4) {
-                    double acc = 0.0;
-                    for (int tt = 0; tt < nctas; ++tt) acc += allp_sh[tt][tid];
-                    tot_sh[tid] = acc;
-                }
-                __syncthreads();
-                ++ncheck;
-                const double rp = sqrt(tot_sh[0]), rd = sqrt(tot_sh[p.rd_sel]);
-                const bool conv = rp < p.tol && rd < p.tol;
-                if (conv || gather_failed || !(rp == rp) || !(rd == rd)) { stopped = conv ? 1 : 0; sweeps_done = it + 1; break; }
-                if (p.adaptive) {      // Eq. 24, then reading A16 for the scaled duals
-                    double rho_new = rho_cur;
-                    if (rp > p.mu * rd) rho_new = rho_cur * p.tau_incr;
-                    else if (rd > p.mu * rp) rho_new = rho_cur / p.tau_decr;
-                    if (rho_new != rho_cur) {
+                double rho_new = rho_cur;
+                if (solve_decide(p, seq, npair, wsum_sh, allp_sh, tot_sh, ncheck, rho_cur, rho_new, stopped)) { sweeps_done = it + 1; break; }
+                {
+                    if (rho_new != rho_cur) {      // reading A16 for the scaled duals
                         const Real ratio = (Real)(rho_cur / rho_new);
                         // u, w, v = max(0,-q) are scaled duals: times rho_old/rho_new; then the operands that depend on them
 #pragma unroll
@@ -1311,12 +1441,17 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
                 if (has_box) { const R2 q = qs[(h * 3 + d) * TS]; static_cast<Real*>(p.qp_out)[i] = q.x; static_cast<Real*>(p.qn_out)[i] = q.y; }
                 if (POLY && d == 0) for (int k = 0; k < KP; ++k) static_cast<double*>(p.qpl_out)[k * stride + gt[h]] = qpls[(k * 2 + h) * TS];
                 if (has_vel || has_acc) {
-                    const R2 w2 = ws[(h * 3 + d) * TS], ph = phs[(h * 3 + d) * TS];
-                    if (has_vel) { static_cast<Real*>(p.wv_out)[i] = w2.x; static_cast<Real*>(p.phv_out)[i] = ph.x; }
-                    if (has_acc) { static_cast<Real*>(p.wa_out)[i] = w2.y; static_cast<Real*>(p.pha_out)[i] = ph.y; }
+                    const R2 w2 = ws[(h * 3 + d) * TS];
+                    R2 ph = make2((Real)0, (Real)0);
+                    const bool ph_here = !SPLIT || p.k_sweeps == 0;      // (SPLIT: phi went out on the last sweep)
+                    if (!SPLIT) ph = phs[(h * 3 + d) * TS];
+                    else if (p.k_sweeps == 0) ph = make2(has_vel ? static_cast<const Real*>(p.phv)[i] : (Real)0, has_acc ? static_cast<const Real*>(p.pha)[i] : (Real)0);
+                    if (has_vel) { static_cast<Real*>(p.wv_out)[i] = w2.x; if (ph_here) static_cast<Real*>(p.phv_out)[i] = ph.x; }
+                    if (has_acc) { static_cast<Real*>(p.wa_out)[i] = w2.y; if (ph_here) static_cast<Real*>(p.pha_out)[i] = ph.y; }
                 }
             }
     }
+    }      // if constexpr (!(SPLIT && SOLVE))
 }
 
 // one launch: a single CTA plainly; KF_CLUSTER: the whole grid as ONE thread-block cluster (<= 16 CTAs, co-scheduled by
@@ -1348,21 +1483,6 @@ cudaError_t launch_mma(const KParams& p, int ctas, int threads, size_t smem, cud
     return launch_any(kern, p, ctas, threads, smem, st);
 }
 
-// split-tail instantiations (fp64, box + velocity [+ acceleration], plain sweeps): `threads` counts the unsplit warps as planned
-// (4k+1 of them); the launch replaces the last one by three
-template <int S, int CM>
-cudaError_t launch_mma_split(const KParams& p, int ctas, int threads, size_t smem, cudaStream_t st) {
-    auto kern = cadmm_sweeps_mma_kernel<double, S, CM, MAXT_MMA, false, false, false, true>;
-    return launch_any(kern, p, ctas, threads + 64, smem, st);
-}
-template <int S, int CM>
-cudaError_t limits_mma_split(int threads, size_t smem, int* per_sm) {
-    auto kern = cadmm_sweeps_mma_kernel<double, S, CM, MAXT_MMA, false, false, false, true>;
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, kern, threads + 64, smem);
-}
-
 // can `ctas` CTAs of this size run as ONE thread-block cluster?  *nclusters = co-resident clusters (0: no)
 template <typename K>
 cudaError_t cluster_query(K kern, int ctas, int threads, size_t smem, int* nclusters) {
@@ -1379,6 +1499,26 @@ cudaError_t cluster_query(K kern, int ctas, int threads, size_t smem, int* nclus
     cfg.attrs = at; cfg.numAttrs = 1;
     return cudaOccupancyMaxActiveClusters(nclusters, (const void*)kern, &cfg);
 }
+// SPLIT instantiations (fp64, box + velocity [+ acceleration], plain sweeps): `threads` counts one warp per octet as planned; the
+// launch runs the last `nsplit` octets on three warps each
+template <int S, int CM>
+cudaError_t launch_mma_split(const KParams& p, int nsplit, int ctas, int threads, size_t smem, cudaStream_t st) {
+    auto kern = p.check_every > 0 ? cadmm_sweeps_mma_kernel<double, S, CM, MAXT_MMA, true, false, false, true>
+                                  : cadmm_sweeps_mma_kernel<double, S, CM, MAXT_MMA, false, false, false, true>;
+    KParams ps = p;
+    ps.split_octets = nsplit;
+    return launch_any(kern, ps, ctas, threads + 64 * nsplit, smem, st);
+}
+template <int S, int CM>
+cudaError_t cluster_mma_split(int ctas, int threads, size_t smem, int* nclusters) {
+    int a = 0, b = 0;
+    cudaError_t e = cluster_query(cadmm_sweeps_mma_kernel<double, S, CM, MAXT_MMA, true, false, false, true>, ctas, threads, smem, &a);
+    if (e != cudaSuccess) return e;
+    e = cluster_query(cadmm_sweeps_mma_kernel<double, S, CM, MAXT_MMA, false, false, false, true>, ctas, threads, smem, &b);
+    *nclusters = a < b ? a : b;
+    return e;
+}
+
 template <typename Real, int S, int CM, int MAXT>
 cudaError_t cluster_mma(int ctas, int threads, size_t smem, int* nclusters) {
     int a = 0, b = 0;
@@ -1463,11 +1603,21 @@ int max_threads_mma(int dtype, bool poly, bool wide) {
 // Split tail (see split_tail_sweeps): a plain fp64 launch of several CTAs with warp-pair synchronisation over the L2 mailbox whose
 // CTAs hold 4k+1 octets (5 or 9 warps) runs its last octet on three warps.  TOP_SPLIT_TAIL=0 in the environment keeps the
 // unsplit launch (A/B measurements; the results are bit-identical).
-bool split_tail_applies(uint32_t f, int check_every, int dtype, int ctas, int threads) {
-    static const bool enabled = [] { const char* e = getenv("TOP_SPLIT_TAIL"); return !(e && e[0] == '0'); }();
-    const int cm = mma_mask(f), warps = threads / 32;
-    return enabled && dtype == 0 && !(f & (KF_POLY | KF_WIDE | KF_CLUSTER)) && check_every == 0 && ctas > 1 &&
-           (f & KF_NEIGHBOUR_SYNC) && (f & KF_PAIRWISE) && (cm == 3 || cm == 7) && threads % 32 == 0 && (warps == 5 || warps == 9);
+bool split_supported(uint32_t f, int dtype) {
+    const int cm = mma_mask(f);
+    return dtype == 0 && !(f & (KF_POLY | KF_WIDE)) && (cm == 3 || cm == 7);
+}
+
+int split_octets_for(uint32_t f, int check_every, int dtype, int ctas, int threads) {
+    // TOP_SPLIT_TAIL=0: never; =1: only the tail of 4k+1 octets; unset: also every octet of CTAs of <= 4 octets
+    static const int mode = [] { const char* e = getenv("TOP_SPLIT_TAIL"); return !e ? 2 : (e[0] == '0' ? 0 : (e[0] == '1' ? 1 : 2)); }();
+    const int warps = threads / 32;
+    if (!split_supported(f, dtype) || mode == 0 || ctas < 2 || !(f & KF_NEIGHBOUR_SYNC) || threads % 32 != 0) return 0;
+    // short chains run as one cluster: every octet on three warps (measured, us per sweep, box + velocity: 1 octet per CTA
+    // 1.36 -> 1.02, 2 octets 1.35 -> 1.17, 3 octets 1.36 -> 1.28, 4 octets 1.39 -> 1.43; over the L2 mailbox it does not pay)
+    if ((f & KF_CLUSTER) && warps <= SPLIT_MAX_ALL) return mode > 1 ? warps : 0;
+    // long chains: the tail of 4k+1 octets (plain sweeps under warp-pair synchronisation)
+    return check_every == 0 && (f & KF_PAIRWISE) && !(f & KF_CLUSTER) && (warps == 5 || warps == 9) ? 1 : 0;
 }
 
 cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int threads, size_t smem, cudaStream_t st) {
@@ -1481,10 +1631,10 @@ cudaError_t launch_sweeps_mma(const KParams& p, int dtype, int s, int ctas, int 
         if (dtype != 0) return cudaErrorInvalidValue;      // fp64 only
         return s == 3 ? launch_mma_wide<3>(p, ctas, threads, smem, st) : launch_mma_wide<4>(p, ctas, threads, smem, st);
     }
-    if (split_tail_applies(p.flags, p.check_every, dtype, ctas, threads)) {
+    if (const int ns = split_octets_for(p.flags, p.check_every, dtype, ctas, threads)) {
         const int cm = mma_mask(kflags);
-        if (s == 3) return cm == 3 ? launch_mma_split<3, 3>(p, ctas, threads, smem, st) : launch_mma_split<3, 7>(p, ctas, threads, smem, st);
-        return cm == 3 ? launch_mma_split<4, 3>(p, ctas, threads, smem, st) : launch_mma_split<4, 7>(p, ctas, threads, smem, st);
+        if (s == 3) return cm == 3 ? launch_mma_split<3, 3>(p, ns, ctas, threads, smem, st) : launch_mma_split<3, 7>(p, ns, ctas, threads, smem, st);
+        return cm == 3 ? launch_mma_split<4, 3>(p, ns, ctas, threads, smem, st) : launch_mma_split<4, 7>(p, ns, ctas, threads, smem, st);
     }
 #define CALL(R_, S_, C_, M_) return launch_mma<R_, S_, C_, M_>(p, ctas, threads, smem, st);
     TOP_DISPATCH_MMA(CALL)
@@ -1521,6 +1671,15 @@ cudaError_t sweep_cluster_limits_mma(int dtype, int s, uint32_t kflags, int ctas
                    : cluster_query(cadmm_sweeps_mma_kernel<double, 4, CM_RUNTIME, MAXT_MMA_WIDE, false, false, true>, ctas, threads, smem, &b);
         *nclusters = a < b ? a : b;
         return e;
+    }
+    if (const int ns = split_octets_for(kflags | KF_CLUSTER | KF_NEIGHBOUR_SYNC | KF_PAIRWISE, 0, dtype, ctas, threads)) {
+        // plain sweeps of this plan run the SPLIT instantiation (more threads per CTA); the in-kernel solve the unsplit one: both must fit
+        const int cmm = mma_mask(kflags);
+        int a = 0;
+        cudaError_t e = s == 3 ? (cmm == 3 ? cluster_mma_split<3, 3>(ctas, threads + 64 * ns, smem, &a) : cluster_mma_split<3, 7>(ctas, threads + 64 * ns, smem, &a))
+                               : (cmm == 3 ? cluster_mma_split<4, 3>(ctas, threads + 64 * ns, smem, &a) : cluster_mma_split<4, 7>(ctas, threads + 64 * ns, smem, &a));
+        if (e != cudaSuccess) return e;
+        if (a < 1) return cudaSuccess;
     }
 #define CALL(R_, S_, C_, M_) return cluster_mma<R_, S_, C_, M_>(ctas, threads, smem, nclusters);
     TOP_DISPATCH_MMA(CALL)

@@ -100,3 +100,60 @@ def test_split_tail_default_plan_config4_and_many_launches():
     a2.iterate(9); b2.iterate(9)
     a2.solve(1e-12); b2.solve(1e-12)
     same_bits(a2, b2, W.small_constrained(N=150, s=4, acc=True), "iterate then solve")
+
+
+# ---- short chains as one cluster: EVERY octet of a CTA on three warps (<= 3 octets per CTA), sweeps and in-kernel solve
+
+@pytest.mark.parametrize("N,s,acc,threads", [
+    (100, 4, False, 96),      # config 2's shape: 13 CTAs of one octet
+    (77, 3, True, 96),
+    (200, 4, True, 192),      # two octets per CTA
+    (301, 4, True, 288),      # three; the last CTA is ragged
+    (500, 4, True, 128),      # four octets per CTA: not split
+])
+def test_all_octets_split_in_a_cluster_bit_identical(N, s, acc, threads):
+    w = W.small_constrained(N=N, s=s, acc=acc)
+    a = top.from_workload(w, dtype="f64")
+    li = a.launch_info()
+    assert 2 <= li["ctas"] <= 16 and li["threads"] == threads, li
+    b = top.from_workload(w, dtype="f64", lanes=4, segs_per_cta=li["segs_per_cta"], sync="neighbour")      # L2 mailbox, unsplit
+    assert b.launch_info()["threads"] == 32 * ((li["segs_per_cta"] + 7) // 8)
+    o = make_oracle(w, 0)
+    done = 0
+    for cp in (1, 2, 3, 10, 100, 400):
+        a.iterate(cp - done); b.iterate(cp - done); o.sweep(cp - done)
+        done = cp
+        same_bits(a, b, w, "sweep %d" % cp)
+        check(field_errors(a, [o], w, [0]), "sweep %d" % cp)
+
+
+@pytest.mark.parametrize("adaptive", [False, True])
+@pytest.mark.parametrize("N,ce", [(100, 1), (200, 4), (301, 1)])
+def test_all_octets_split_in_kernel_solve(N, ce, adaptive):
+    """The SPLIT + SOLVE instantiation: same decisions, same sweep count, same rho sequence as the oracle and as the unsplit
+    solve kernel; state bit-identical to the latter."""
+    w = W.small_constrained(N=N, s=4, acc=True)
+    kw = dict(check_every=ce, max_iter=600, adaptive_rho=adaptive, eps_n_scaled=True)
+    a = top.from_workload(w, dtype="f64", **kw)
+    li = a.launch_info()
+    assert li["threads"] == 96 * ((li["segs_per_cta"] + 7) // 8), li
+    b = top.from_workload(w, dtype="f64", lanes=4, segs_per_cta=li["segs_per_cta"], sync="neighbour", **kw)
+    o = make_oracle(w, 0)
+    eps = 0.05
+    if adaptive and ce == 1:
+        it_o = o.solve_adaptive(eps * w.N, 600)
+    else:
+        it_o = None
+    oka, ita = a.solve(eps)
+    okb, itb = b.solve(eps)
+    assert oka == okb and ita[0] == itb[0] and a.rho == b.rho, (ita, itb, a.rho, b.rho)
+    same_bits(a, b, w, "after solve")
+    if it_o is not None:
+        assert ita[0] == it_o and abs(a.rho - o.rho) <= 1e-12 * o.rho, (ita, it_o, a.rho, o.rho)
+        check(field_errors(a, [o], w, [0]), "after adaptive solve")
+    elif not adaptive:
+        o.sweep(int(ita[0]))
+        check(field_errors(a, [o], w, [0]), "after solve")
+    # and on from there with plain sweeps (split launch continues from the solve kernel's state)
+    a.iterate(5); b.iterate(5)
+    same_bits(a, b, w, "solve then iterate")
