@@ -204,12 +204,26 @@ __device__ __noinline__ void refresh_operator_rows(const KParams& p, long long g
 // adds them in the same order, so all CTAs take the same decision from the same numbers), Eq. 23, Eq. 24.
 // Returns true when the launch ends here (converged: stopped = 1; or a failed gather / non-finite residual); otherwise rho_new is
 // the penalty of the next sweep (== rho_cur unless Eq. 24 moved it).
+// KF_CLUSTER: the all-gather goes through distributed shared memory -- every CTA stores its four sums straight into the result
+// box of EVERY CTA of the cluster (cresbox: [2 parity][16 CTAs][4] LL slots in each CTA's shared memory) and polls its own copy:
+// one one-way DSMEM store instead of an L2 round trip with polling (a test sweep of config 2: 3.6 -> 2.x us).
+constexpr int CRES_BYTES = 2 * 16 * 4 * 16;
 __device__ __forceinline__ bool solve_decide(const KParams& p, unsigned seq, int noct, double (*wsum_sh)[4], double (*allp_sh)[4], double* tot_sh,
-                                             int& ncheck, double rho_cur, double& rho_new, int& stopped) {
+                                             unsigned char* cresbox, int& ncheck, double rho_cur, double& rho_new, int& stopped) {
     const int tid = threadIdx.x, T = blockDim.x, cta = blockIdx.x, nctas = gridDim.x;
+    const bool clus = (p.flags & KF_CLUSTER) != 0;
     __syncthreads();
     unsigned char* const rb = static_cast<unsigned char*>(p.resbox) + (size_t)(ncheck & 1) * p.max_ctas * 4 * 16;
-    if (tid == 0) {
+    const unsigned cres_local = smem_u32(cresbox), cpar = (unsigned)((ncheck & 1) * 16 * 4 * 16);
+    if (clus) {
+        // lanes 0..3 of every warp add the octets' sums of quantity k = lane in the same fixed order; thread t delivers quantity
+        // t & 3 to CTA t >> 2
+        double acc = 0.0;
+        if ((tid & 31) < 4) for (int w = 0; w < noct; ++w) acc += wsum_sh[w][tid & 3];
+        acc = __shfl_sync(0xffffffffu, acc, tid & 3);
+        for (int t = tid; t < nctas * 4; t += T)
+            ll_store_cluster(cluster_map(cres_local, (unsigned)(t >> 2)) + cpar + (unsigned)((cta * 4 + (t & 3)) * 16), acc, seq);
+    } else if (tid == 0) {
         for (int k = 0; k < 4; ++k) {
             double acc = 0.0;
             for (int w = 0; w < noct; ++w) acc += wsum_sh[w][k];
@@ -222,12 +236,13 @@ __device__ __forceinline__ bool solve_decide(const KParams& p, unsigned seq, int
         unsigned spins = 0;
         for (int k = 0; k < 4; ++k) {
             LLRaw r;
-            ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
+            const unsigned cslot = cres_local + cpar + (unsigned)((tt * 4 + k) * 16);
+            if (clus) ll_issue_smem(cslot, r); else ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
             while (!ll_ok(r, seq)) {
                 if ((++spins & 255u) == 0 && (*(volatile int*)p.abort_flag || global_ns() - t0 > WAIT_TIMEOUT_NS)) {
                     atomicExch(p.abort_flag, 1); gather_failed = 1; break;
                 }
-                ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
+                if (clus) ll_issue_smem(cslot, r); else ll_issue(rb + ((size_t)tt * 4 + k) * 16, r);
             }
             allp_sh[tt][k] = ll_value(r);
         }
@@ -327,7 +342,7 @@ __device__ __forceinline__ int pair_threads(int b, int W) { return (b >= W ? 96 
 
 // SOLVE (in-kernel stop rule and Eq. 24, as in cadmm_sweeps_mma_kernel): only for CTAs that are split entirely; one CTA barrier
 // per sweep instead of the pair barriers.
-struct SolveShared { int* abort_sh; double (*wsum)[4]; double (*allp)[4]; double* tot; };
+struct SolveShared { int* abort_sh; double (*wsum)[4]; double (*allp)[4]; double* tot; unsigned char* cres; };
 
 template <int S, int CM, int MAXT, bool SOLVE>
 __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned char* smem_raw, volatile int* abort_any, unsigned char* cmbox, const SolveShared sv) {
@@ -666,7 +681,7 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
                     if (lane32 == 0) { for (int k = 0; k < 4; ++k) sv.wsum[oct][k] = q4[k]; }
                 }
                 double rho_new = rho_cur;
-                if (solve_decide(p, seq, noct, sv.wsum, sv.allp, sv.tot, ncheck, rho_cur, rho_new, stopped)) { sweeps_done = it + 1; break; }
+                if (solve_decide(p, seq, noct, sv.wsum, sv.allp, sv.tot, sv.cres, ncheck, rho_cur, rho_new, stopped)) { sweeps_done = it + 1; break; }
                 if (rho_new != rho_cur) {      // Eq. 24 moved rho: scaled duals times rho_old / rho_new (A16), operands, operator rows
                     const double ratio = rho_cur / rho_new;
                     const double lo = has_box ? lohi[d * SA] : 0.0, hi = has_box ? lohi[(3 + d) * SA] : 0.0;
@@ -741,18 +756,22 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
     __shared__ double wsum_sh[SOLVE ? 32 : 1][4];      // in-kernel stop rule: per-octet partial sums, per-CTA partial sums, totals
     __shared__ double allp_sh[SOLVE ? 160 : 1][4];
     __shared__ double tot_sh[4];
+    __shared__ __align__(16) unsigned char cresbox[SOLVE ? CRES_BYTES : 16];      // cluster exchange: this CTA's copy of the per-CTA residual sums
     // ---- CTA-wide prologue (before the split octets branch off): constant MMA operands, flags, cluster mailbox cleared
     {
         const SmemLayoutMma L0 = smem_layout_mma(CM != 0 || POLY, MAXT / 4, POLY, (int)sizeof(Real), WIDE);
         if (threadIdx.x < 32) fill_ctab<S, WIDE>(reinterpret_cast<double*>(smem_raw + L0.ctab) + threadIdx.x, (int)threadIdx.x);
         if (threadIdx.x < 2) abort_sh[threadIdx.x] = 0;
         if (threadIdx.x == 0) abort_any = 0;
-        if (p.flags & KF_CLUSTER) for (int i = threadIdx.x; i < 2 * MBS * 4; i += blockDim.x) reinterpret_cast<unsigned*>(cmbox)[i] = 0u;
+        if (p.flags & KF_CLUSTER) {
+            for (int i = threadIdx.x; i < 2 * MBS * 4; i += blockDim.x) reinterpret_cast<unsigned*>(cmbox)[i] = 0u;
+            if (SOLVE) for (int i = threadIdx.x; i < CRES_BYTES / 4; i += blockDim.x) reinterpret_cast<unsigned*>(cresbox)[i] = 0u;
+        }
     }
     if constexpr (SPLIT) {      // the last p.split_octets octets run on three warps each, one dim per warp
         // (SPLIT with the in-kernel stop rule: every octet is split, this is the whole kernel)
         if (SOLVE || (int)threadIdx.x >= (int)blockDim.x - 96 * p.split_octets) {
-            const SolveShared sv = {abort_sh, wsum_sh, allp_sh, tot_sh};
+            const SolveShared sv = {abort_sh, wsum_sh, allp_sh, tot_sh, cresbox};
             split_tail_sweeps<S, (CM == 0 || CM == CM_RUNTIME) ? 7 : CM, MAXT, SOLVE>(p, smem_raw, &abort_any, cmbox, sv);
             return;
         }
@@ -1376,7 +1395,7 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
                 for (int k = 0; k < 4; ++k) { q4[k] += shfl_xor(q4[k], 4); q4[k] += shfl_xor(q4[k], 8); q4[k] += shfl_xor(q4[k], 16); }
                 if ((tid & 31) == 0) { for (int k = 0; k < 4; ++k) wsum_sh[tid >> 5][k] = q4[k]; }
                 double rho_new = rho_cur;
-                if (solve_decide(p, seq, npair, wsum_sh, allp_sh, tot_sh, ncheck, rho_cur, rho_new, stopped)) { sweeps_done = it + 1; break; }
+                if (solve_decide(p, seq, npair, wsum_sh, allp_sh, tot_sh, cresbox, ncheck, rho_cur, rho_new, stopped)) { sweeps_done = it + 1; break; }
                 {
                     if (rho_new != rho_cur) {      // reading A16 for the scaled duals
                         const Real ratio = (Real)(rho_cur / rho_new);
@@ -1615,7 +1634,9 @@ int split_octets_for(uint32_t f, int check_every, int dtype, int ctas, int threa
     if (!split_supported(f, dtype) || mode == 0 || ctas < 2 || !(f & KF_NEIGHBOUR_SYNC) || threads % 32 != 0) return 0;
     // short chains run as one cluster: every octet on three warps (measured, us per sweep, box + velocity: 1 octet per CTA
     // 1.36 -> 1.02, 2 octets 1.35 -> 1.17, 3 octets 1.36 -> 1.28, 4 octets 1.39 -> 1.43; over the L2 mailbox it does not pay)
-    if ((f & KF_CLUSTER) && warps <= SPLIT_MAX_ALL) return mode > 1 ? warps : 0;
+    // (in-kernel stop rule: a TEST sweep costs 0.7 us more when split -- three more octet barriers for the residual sums -- and a
+    // plain one 0.33 us less: it pays from a test every third sweep on)
+    if ((f & KF_CLUSTER) && warps <= SPLIT_MAX_ALL) return mode > 1 && (check_every == 0 || check_every >= 3) ? warps : 0;
     // long chains: the tail of 4k+1 octets (plain sweeps under warp-pair synchronisation)
     return check_every == 0 && (f & KF_PAIRWISE) && !(f & KF_CLUSTER) && (warps == 5 || warps == 9) ? 1 : 0;
 }
