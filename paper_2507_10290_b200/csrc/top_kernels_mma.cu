@@ -482,7 +482,7 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
     const int n_first = use_first ? pair_threads(bfirst, W) : 0, n_second = use_second ? pair_threads(bsecond, W) : 0;
     const int ce = SOLVE ? p.check_every : 0;
     double rho_cur = p.rho;
-    int ncheck = 0, sweeps_done = p.k_sweeps, stopped = 0;
+    int ncheck = 0, sweeps_done = p.k_sweeps, stopped = 0, since_test = 0;
     double phv_[2] = {0, 0}, pha_[2] = {0, 0};      // SOLVE: phi of the newest iterate (Eq. 24 rebuilds the operands gv, ga from it)
     __syncthreads();      // (the one CTA barrier of the launch: the unsplit warps arrive from cadmm_sweeps_mma_kernel)
 
@@ -490,7 +490,9 @@ __device__ __forceinline__ void split_tail_sweeps(const KParams& p, unsigned cha
         const unsigned seq = p.seq_base + (unsigned)it + 1u;
         const int par = (int)(seq & 1u);
         // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
-        const bool last_sweep = (it == p.k_sweeps - 1) || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
+        bool test_sweep = false;      // (a counter, not (it + 1) % ce: the integer division showed up in the profile of short chains)
+        if (SOLVE && ce > 0 && ++since_test == ce) { since_test = 0; test_sweep = true; }
+        const bool last_sweep = (it == p.k_sweeps - 1) || test_sweep;
         double* const Bcur = Bs + par * BPAR;
         unsigned char* const mpar = mbox + par * par_stride;      // (cluster exchange: only the offset part is used)
         const unsigned cpar = (unsigned)(par * MBS * 16);
@@ -1023,14 +1025,16 @@ __global__ void __launch_bounds__(SPLIT ? (MAXT + 64 + 127) / 128 * 128 : MAXT, 
     // sums through LL slots and take the same decision from the same numbers)
     const int ce = SOLVE ? p.check_every : 0;
     double rho_cur = p.rho;
-    int ncheck = 0, sweeps_done = p.k_sweeps, stopped = 0;
+    int ncheck = 0, sweeps_done = p.k_sweeps, stopped = 0, since_test = 0;
     __syncthreads();
     for (int it = 0; it < p.k_sweeps; ++it) {
         const unsigned seq = p.seq_base + (unsigned)it + 1u;
         const int par = (int)(seq & 1u);
         const bool final_sweep = (it == p.k_sweeps - 1);
         // sweeps on which residuals (and the coefficients) are materialised: the last one, and every test sweep
-        const bool last_sweep = final_sweep || (SOLVE && ce > 0 && (it + 1) % (SOLVE ? max(ce, 1) : 1) == 0);
+        bool test_sweep = false;
+        if (SOLVE && ce > 0 && ++since_test == ce) { since_test = 0; test_sweep = true; }
+        const bool last_sweep = final_sweep || test_sweep;
         Real* const Bcur = Bs + par * BPAR;
         Real* const Bcur2 = Bs2 + par * BPAR;
         unsigned char* const mpar = mbox + par * par_stride;     // (cluster exchange: only the offset part is used)
@@ -1634,9 +1638,8 @@ int split_octets_for(uint32_t f, int check_every, int dtype, int ctas, int threa
     if (!split_supported(f, dtype) || mode == 0 || ctas < 2 || !(f & KF_NEIGHBOUR_SYNC) || threads % 32 != 0) return 0;
     // short chains run as one cluster: every octet on three warps (measured, us per sweep, box + velocity: 1 octet per CTA
     // 1.36 -> 1.02, 2 octets 1.35 -> 1.17, 3 octets 1.36 -> 1.28, 4 octets 1.39 -> 1.43; over the L2 mailbox it does not pay)
-    // (in-kernel stop rule: a TEST sweep costs 0.7 us more when split -- three more octet barriers for the residual sums -- and a
-    // plain one 0.33 us less: it pays from a test every third sweep on)
-    if ((f & KF_CLUSTER) && warps <= SPLIT_MAX_ALL) return mode > 1 && (check_every == 0 || check_every >= 3) ? warps : 0;
+    // (with the in-kernel stop rule as well: config 2, a test every sweep 3.08 -> 2.74 us per sweep, every 8th 1.75 -> 1.34)
+    if ((f & KF_CLUSTER) && warps <= SPLIT_MAX_ALL) return mode > 1 ? warps : 0;
     // long chains: the tail of 4k+1 octets (plain sweeps under warp-pair synchronisation)
     return check_every == 0 && (f & KF_PAIRWISE) && !(f & KF_CLUSTER) && (warps == 5 || warps == 9) ? 1 : 0;
 }

@@ -128,7 +128,7 @@ def test_all_octets_split_in_a_cluster_bit_identical(N, s, acc, threads):
 
 
 @pytest.mark.parametrize("adaptive", [False, True])
-@pytest.mark.parametrize("N,ce", [(100, 1), (100, 3), (200, 4), (301, 8)])      # (a test every sweep or every other sweep keeps the unsplit solve kernel)
+@pytest.mark.parametrize("N,ce", [(100, 1), (100, 3), (200, 4), (301, 1)])
 def test_all_octets_split_in_kernel_solve(N, ce, adaptive):
     """The SPLIT + SOLVE instantiation: same decisions, same sweep count, same rho sequence as the oracle and as the unsplit
     solve kernel; state bit-identical to the latter."""
