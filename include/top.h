@@ -283,6 +283,47 @@ TOP_API top_status top_precompute_operator(int32_t s, double T, double rho, int3
                                            uint32_t flags, const double* p0, const double* p1,
                                            double* Pm_hat, double* c0_hat);
 
+/* top_operator_rows_static -- the x-update operator of Eq. 20a (first bracket) for up to
+ * TOP_STATIC_MAX_SEGMENTS segments, computed on the GPU by the same double-double kernel that top_create runs, WITHOUT
+ * ANY ALLOCATION: no cudaMalloc / cudaFree / memory-pool call, no solver handle.  It is for callers that own their device
+ * buffers but may not take new ones -- a plug-in inside a host application that reserved the whole device heap at start-up,
+ * a fixed-rate re-planning loop that cannot afford the device-wide synchronisation and the unbounded latency of the
+ * allocator, a thread that works while another thread of the process records a CUDA graph (an allocation call would break
+ * that recording), a process with a fixed memory budget.  Everything else in this header needs a solver, and top_create
+ * allocates one arena per solver.
+ *   device      CUDA device ordinal, -1 = the current device
+ *   nseg        number of segments, 1 <= nseg <= TOP_STATIC_MAX_SEGMENTS (more: TOP_E_UNSUPPORTED; split the call)
+ *   s           3 (jerk) or 4 (snap)
+ *   durations   HOST [nseg] seconds, finite and > 0 (copied inside the call)
+ *   rho         > 0, penalty of Eq. 5
+ *   box/vel/acc != 0: the penalty blocks of the box corridor / velocity ball / acceleration ball at the 8 sample times
+ *               are part of the operator (readings A10, A11)
+ *   flags       one TOP_WAYPOINT_* mode
+ *   rows_out    DEVICE buffer of the selected device, 64 * nseg doubles, caller-owned and caller-allocated:
+ *               rows_out[(b * nseg + g) * 8 + a] = rho * Pm_hat_g[a][b] (Pm_hat is symmetric), the operator of segment g in the
+ *               normalised-time basis c^_a = c_a T^a -- rho times the Pm_hat that top_precompute_operator returns on the host
+ *               for T = durations[g] -- zero for a >= 2s or b >= 2s
+ *   cuda_stream the work is enqueued on this stream (NULL = legacy default stream) and the call waits for it: on return
+ *               rows_out is complete and `durations` may be freed.
+ * Where the working memory is.  The kernel's scratch (28 KB of Gram tables, the device copy of the durations, a status word;
+ * 156.25 KB in all) is a static array inside libtop.so's device image: every GPU on which the process uses this library
+ * holds it from module load to process exit, whether or not this function is ever called.  TOP_STATIC_MAX_SEGMENTS is what
+ * that array was sized for.
+ * First call.  The first call on each device looks up the array's device address and fills the Gram tables with one
+ * synchronous copy (and, as for any kernel, the driver loads the code on first launch).  Make that first call during
+ * start-up, before any stream capture begins; later calls enqueue two small copies, a memset and two kernels.
+ * Sharing.  Every call on a device uses the same array, and the array keeps what the last call left in it (the call itself
+ * re-zeroes the status word).  Two calls that ran on the GPU at the same time would overwrite each other's durations and
+ * status: the library therefore holds a per-device lock for the whole (synchronous) call, so calls on one device are
+ * serialised, from whatever threads and streams they come.  Different processes have separate copies of the array.
+ * Errors: TOP_E_INVALID (arguments; rows_out is not device memory of that device; an operator that is not positive
+ * definite -- rows_out is then unspecified), TOP_E_UNSUPPORTED (nseg beyond the maximum), TOP_E_CUDA.  The message is in
+ * top_last_error(NULL). */
+#define TOP_STATIC_MAX_SEGMENTS 16384
+TOP_API top_status top_operator_rows_static(int32_t device, int32_t nseg, int32_t s, const double* durations, double rho,
+                                            int32_t box, int32_t vel, int32_t acc, uint32_t flags, double* rows_out,
+                                            void* cuda_stream);
+
 TOP_API top_status top_destroy(top_solver* h);
 
 /* Message of the last failing call on this handle (h == NULL: of the last failing top_create on this

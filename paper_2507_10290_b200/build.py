@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtop.so")
-SOURCES = ["top_kernels.cu", "top_kernels_mma.cu", "top_kernels_numeric.cu", "top_api.cpp"]
+SOURCES = ["top_kernels.cu", "top_kernels_mma.cu", "top_kernels_numeric.cu", "top_static_scratch.cu", "top_api.cpp"]
 DEPS = SOURCES + ["top_internal.h", "top_device.cuh", os.path.join("..", "..", "include", "top.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden"]

@@ -490,6 +490,21 @@ int max_segs_per_cta(int dtype, int s, bool constrained, int lanes, bool mma, si
 
 }  // namespace
 
+// Host helpers for top_operator_rows_static (top_static_scratch.cu), which lives in a .cu file beside its static device array.
+namespace top {
+void gram_tables_dd(int s, GramDD* out) {       // the tables of gram_tables(s), each entry split into a double-double
+    const GramTables& G = gram_tables(s);
+    const xreal* tabs[GRAM_TABLES] = {G.Q1, G.Gc[0], G.Gc[1], G.Gc[2], G.Gc[3], G.Ge[0], G.Ge[1], G.Ge[2],
+                                      G.Gw[0][0], G.Gw[0][1], G.Gw[0][2], G.Gw[1][0], G.Gw[1][1], G.Gw[1][2]};
+    for (int t = 0; t < GRAM_TABLES; ++t)
+        for (int i = 0; i < MAXN * MAXN; ++i) {
+            const double hi = (double)tabs[t][i];
+            out->hi[t][i] = hi; out->lo[t][i] = (double)(tabs[t][i] - (xreal)hi);
+        }
+}
+int report_error(int status, const char* msg) { return (int)fail(nullptr, (top_status)status, msg); }
+}  // namespace top
+
 namespace {
 // (re)build rho*Pm^ and c0^ on the device for `rho` from the spectral data
 cudaError_t refresh_operator(top_solver* h, double rho) {

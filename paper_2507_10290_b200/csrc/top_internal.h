@@ -149,6 +149,10 @@ struct PrecompParams {
     int* bad;                     // set to 1 when a segment's operator is not positive definite
 };
 cudaError_t launch_precompute_operator(const PrecompParams& p, cudaStream_t st);
+// host helpers of top_api.cpp for the entry point that lives outside it (top_static_scratch.cu): the Gram tables of
+// order s in {3, 4} split into double-double, and the message behind top_last_error(NULL) (returns `status`)
+void gram_tables_dd(int s, GramDD* out);
+int report_error(int status, const char* msg);
 // NumericSolve branch (top_kernels_numeric.cu): one sweep = x-update kernel + consensus kernel.  fp64 only.
 struct NumParams {
     const double* Pm;         // [MAXN][stride] rho * Pm^ rows of the QUADRATIC part (no ball terms)

@@ -28,6 +28,7 @@ SYNC = {"auto": 0, "grid": 16, "neighbour": 32, "pairwise": 48}
 
 EXPORTS = ["top_create", "top_reset", "top_iterate", "top_solve", "top_get_residuals", "top_get_coeffs", "top_get_state",
            "top_snapshot_bytes", "top_snapshot_save", "top_snapshot_restore", "top_iteration", "top_numeric_info", "top_set_rho", "top_get_rho", "top_launch_info", "top_memory_info", "top_capacity", "top_fma_peak", "top_precompute_operator",
+           "top_operator_rows_static",
            "top_destroy", "top_last_error"]
 
 
@@ -106,6 +107,9 @@ def lib():
     L.top_precompute_operator.restype = ctypes.c_int
     L.top_precompute_operator.argtypes = [ctypes.c_int32, ctypes.c_double, ctypes.c_double, ctypes.c_int32,
                                           ctypes.c_int32, ctypes.c_int32, ctypes.c_uint32, dp, dp, dp, dp]
+    L.top_operator_rows_static.restype = ctypes.c_int
+    L.top_operator_rows_static.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, dp, ctypes.c_double, ctypes.c_int32,
+                                           ctypes.c_int32, ctypes.c_int32, ctypes.c_uint32, vp, vp]
     L.top_destroy.restype = ctypes.c_int
     L.top_destroy.argtypes = [vp]
     L.top_last_error.restype = ctypes.c_char_p
@@ -137,6 +141,28 @@ def precompute_operator(s, T, rho, p0, p1, box=False, vel=False, acc=False, mode
     if st != TOP_OK:
         raise TopError(st, L.top_last_error(None).decode())
     return Pm, c0
+
+
+STATIC_MAX_SEGMENTS = 16384
+
+
+def operator_rows_static(durations, s, rho, rows_out_ptr: int, box=False, vel=False, acc=False, mode="hard", device=-1,
+                         stream=0):
+    """top_operator_rows_static: rho * Pm_hat of every segment, written by the GPU into a device buffer the caller already
+    owns, for callers that must not allocate device memory (a plug-in in a process that reserved the whole heap, a
+    fixed-rate re-planning loop, a thread beside a CUDA-graph capture).  The kernel's scratch is a static array inside the
+    library, so at most STATIC_MAX_SEGMENTS segments per call; calls on one device are serialised and the call waits
+    for the stream.  Make the first call on a device at start-up, outside any stream capture.
+
+    durations: host array [nseg]; rows_out_ptr: raw device pointer to 64 * nseg doubles, laid out [8 (b)][nseg][8 (a)]
+    (e.g. torch.empty((8, nseg, 8), dtype=torch.float64, device="cuda").data_ptr()).  Nothing is returned: the result is
+    in the caller's buffer."""
+    L = lib()
+    T = _f64(np.asarray(durations).reshape(-1))
+    st = L.top_operator_rows_static(int(device), int(T.size), int(s), _dptr(T), float(rho), int(box), int(vel), int(acc),
+                                    WAYPOINT[mode], ctypes.c_void_p(rows_out_ptr), ctypes.c_void_p(stream))
+    if st != TOP_OK:
+        raise TopError(st, L.top_last_error(None).decode())
 
 
 def capacity(s, dtype="f64", constrained=True, device=-1):
