@@ -1369,7 +1369,8 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
         CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
         RescaleParams r;
         r.u = h->d_u; r.qp = nullptr; r.qn = nullptr; r.wv = h->d_wv; r.wa = h->d_wa;
-        r.count = 3 * (long long)LS; r.ratio = old / rho; r.qpl = h->d_qpl; r.qpl_count = (long long)h->K * (long long)LS; r.u2 = nullptr;
+        r.count = 3 * (long long)LS; r.ratio = old / rho; r.qpl = h->d_qpl; r.qpl_count = (long long)h->K * (long long)LS;
+        r.u2 = h->d_u2;      // wide consensus: the scaled duals of the second row block as well (null otherwise)
         r.yv = r.ya = nullptr; r.y_count = 0;
         CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
         h->launches += 2;

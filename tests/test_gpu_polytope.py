@@ -146,3 +146,34 @@ def test_polytope_with_paper_literal_consensus(s, acc, K, segs, mode):
     for cp in (1, 2, 3, 10, 50, 200):
         sol.iterate(cp - done); o.sweep(cp - done); done = cp
         compare(sol, [o], w, "sweep %d" % cp)
+
+
+def test_polytope_wide_set_rho_and_adaptive_solve():
+    """top_set_rho and Eq. 24 on the paper's literal configuration (polytope corridor + n_c = 2s-1): every scaled dual is
+    rescaled by rho_old / rho_new -- also the second consensus block (orders s..2s-2) -- so the multipliers rho * u are
+    unchanged (reading A16) and the iterates stay on the oracle's (coupled operator, wide consensus)."""
+    w = W.polytope_corridor(W.small_constrained(N=33, s=4, acc=True, seed=12), K=6, seed=4)
+    sol = top.from_workload(w, segs_per_cta=8, mode="free", consensus="wide")
+    o = poly_oracle(w, mode="free", long_double=True, consensus="wide")
+    sol.iterate(12); o.sweep(12, 1)
+    u_before = sol.state("u").copy()
+    assert np.abs(u_before[0, 1:-1, 4:7]).max() > 0 and np.abs(u_before[0, 1:-1, 11:14]).max() > 0     # the second block is live
+    sol.set_rho(2.5); o.set_rho(2.5)
+    assert np.allclose(sol.state("u") * 2.5, u_before * w.rho, rtol=1e-14, atol=0)       # rho * u unchanged, every row
+    w.rho = 2.5
+    compare(sol, [o], w, "right after set_rho")
+    sol.iterate(9); o.sweep(9, 1)
+    compare(sol, [o], w, "9 sweeps after set_rho")
+    sol.close()
+    # Eq. 24 through top_solve (host loop on polytope solvers: every change of rho goes through top_set_rho)
+    w2 = W.polytope_corridor(W.small_constrained(N=33, s=4, acc=True, seed=12), K=6, seed=4)
+    o2 = poly_oracle(w2, mode="free", long_double=True, consensus="wide")
+    n_ref = o2.solve_adaptive(1e-300, 60, every=2)         # never converges: 60 sweeps with a test (and Eq. 24) every 2nd
+    assert n_ref == 60 and o2.rho != w2.rho
+    sol2 = top.from_workload(w2, segs_per_cta=8, mode="free", consensus="wide", adaptive_rho=True, check_every=2, max_iter=60)
+    ok, it = sol2.solve(1e-300)
+    assert not ok and sol2.iteration == 60
+    assert sol2.rho == pytest.approx(o2.rho, rel=1e-12)
+    w2.rho = o2.rho
+    compare(sol2, [o2], w2, "adaptive, 60 sweeps")
+    sol2.close()
