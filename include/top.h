@@ -29,6 +29,14 @@
  *  - Kernels are enqueued on top_options.cuda_stream (a cudaStream_t passed as void*;
  *    NULL = the legacy default stream).  top_iterate is asynchronous with respect to the
  *    host; every call that returns data to the host synchronises that stream first.
+ *
+ * Environment variables (read by the library; none changes a result):
+ *  - TOP_TRACE_CREATE=1     top_create / top_reset print their phase times (ms) to stderr.
+ *  - TOP_SPLIT_TAIL=0|1     A/B switch of the tensor-core kernel's "split octets" launch shape: 0 = never
+ *                           split, 1 = only the last octet of CTAs holding 4k+1 octets, unset = the planner's choice.
+ *                           Read once per process.  Bit-identical results in every setting.
+ *  - TOP_TEST_SEQ_START=n   test hook: the 64-bit counter whose low 32 bits number the inter-CTA mailbox messages starts at n
+ *                           instead of 0 in solvers created afterwards (tests/test_gpu_cluster.py runs across the 2^32 wrap).
  */
 #ifndef TOP_H
 #define TOP_H

@@ -144,7 +144,8 @@ struct top_solver {
     double h_solve[8] = {0, 0, 0, 0, 0, 0, 0, 0};
     bool have_residuals = false;
     int64_t iter = 0, launches = 0;
-    unsigned long long seq_counter = 0;   // sweeps launched so far over all waves (mailbox sequence space)
+    unsigned long long seq_counter = 0;   // sweeps launched so far over all waves (mailbox sequence space; the slots carry its low 32 bits)
+    size_t bedge_bytes = 0, resbox_bytes = 0;   // sizes of the two mailboxes (cleared when the sequence space starts a new epoch)
     std::string err;
 };
 
@@ -891,6 +892,8 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
     h->vmax = has_vel ? cons->vmax : 0; h->amax = has_acc ? cons->amax : 0;
     h->wp_mode = mode;
     h->wide = (o.flags & TOP_CONSENSUS_WIDE) != 0;
+    // test hook (include/top.h, "Environment variables"): start the mailbox sequence counter near the end of its 32-bit space
+    if (const char* e = std::getenv("TOP_TEST_SEQ_START")) h->seq_counter = std::strtoull(e, nullptr, 0);
     h->numeric = (o.flags & TOP_XUPDATE_NUMERIC) != 0;
     if (h->numeric && (dtype != TOP_F64 || h->has_poly || h->wide))
         CREATE_FAIL(fail(h, TOP_E_UNSUPPORTED, "TOP_XUPDATE_NUMERIC: TOP_F64 only, no polytope corridor, no TOP_CONSENSUS_WIDE"));
@@ -1098,6 +1101,7 @@ top_status create_impl(top_solver** out, int32_t batch, int32_t N, int32_t s, in
         void* cur[8] = {h->d_zt, h->d_u, h->d_qp, h->d_qn, h->d_phv, h->d_wv, h->d_pha, h->d_wa};
         for (int i = 0; i < 8; ++i) if (cur[i]) h->alt[i] = A + o_alt[i];
     }
+    h->bedge_bytes = (size_t)2 * h->max_ctas * (h->wide ? 48 : 24) * 16; h->resbox_bytes = (size_t)2 * h->max_ctas * 4 * 16;
     h->d_Bedge = A + o_Bedge; h->d_resbox = A + o_resbox; h->d_sync = A + o_sync; h->d_abort = (int*)(A + o_abort);
     h->stage.reset(new (std::nothrow) unsigned char[h->upload_bytes]);
     if (!h->stage) CREATE_FAIL(fail(h, TOP_E_NOMEM, "host allocation failed"));
@@ -1238,6 +1242,14 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
             p.max_ctas = h->max_ctas; p.rho = h->rho; p.vmax = h->vmax; p.amax = h->amax;
             p.rot = h->d_rot; p.planes = h->d_planes; p.qpl = h->d_qpl; p.qpl_out = h->d_qpl; p.K = h->K;
             p.invTk2 = h->d_invTk2; p.zt2 = h->d_zt2; p.u2 = h->d_u2;
+            // mailbox sequence numbers are the low 32 bits of seq_counter + 1 .. + kk.  A slot is valid when it carries the
+            // reader's number, and cleared slots carry 0: a launch must never issue 0 nor a number that a slot may still hold
+            // from 2^32 sweeps ago, so a launch that would run past 2^32 - 1 starts a new epoch on cleared mailboxes
+            if ((h->seq_counter & 0xffffffffull) + (unsigned long long)kk > 0xffffffffull) {
+                h->seq_counter = (h->seq_counter | 0xffffffffull) + 1ull;
+                CU(cudaMemsetAsync(h->d_Bedge, 0, h->bedge_bytes, h->stream), "cudaMemsetAsync");
+                CU(cudaMemsetAsync(h->d_resbox, 0, h->resbox_bytes, h->stream), "cudaMemsetAsync");
+            }
             p.seq_base = (unsigned int)(h->seq_counter & 0xffffffffull);
             h->seq_counter += (unsigned long long)kk;
             if (w.ctas > 1 && !(p.flags & KF_NEIGHBOUR_SYNC))
@@ -1258,6 +1270,9 @@ top_status run_sweeps(top_solver* h, int64_t k, const InKernelSolve* iks = nullp
             CU(cudaStreamSynchronize(h->stream), "cudaStreamSynchronize");
             const int64_t done = (int64_t)h->h_solve[0];
             h->iter += done;
+            // the sequence space advances by the sweeps that ran, not by the cap (one wave on this path): a default top_solve
+            // reserves max_iter numbers, and a re-planning loop would otherwise walk through 2^32 in a few thousand calls
+            if (done >= 0 && done < kk) h->seq_counter -= (unsigned long long)(kk - done);
             if (h->h_solve[2] != h->rho) {      // the kernel refreshed its on-chip operator only: bring the arrays along
                 h->rho = h->h_solve[2];
                 CU(refresh_operator(h, h->rho), "operator refresh launch");      // (Eq. 24 ran: the spectral form is there)
