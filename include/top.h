@@ -29,6 +29,8 @@
  *  - Kernels are enqueued on top_options.cuda_stream (a cudaStream_t passed as void*;
  *    NULL = the legacy default stream).  top_iterate is asynchronous with respect to the
  *    host; every call that returns data to the host synchronises that stream first.
+ *    The stream must outlive the handle: top_destroy synchronises it and returns the arena to the pool in
+ *    stream order (if the stream is gone or is being captured it falls back to a synchronising cudaFree).
  *
  * Environment variables (read by the library; none changes a result):
  *  - TOP_TRACE_CREATE=1     top_create / top_reset print their phase times (ms) to stderr.
@@ -185,8 +187,9 @@ TOP_API top_status top_create(top_solver** out, int32_t batch, int32_t N, int32_
  * re-planning loop calls it.  batch, N, s, dims, dtype, options and the constraint
  * SELECTION (box present or not, vmax > 0 or not, amax > 0 or not) are those of top_create; waypoints, durations, end
  * states, box bounds, vmax, amax and rho are new (same layouts as top_create; host pointers, copied).  Nothing is
- * allocated: the per-segment operator is recomputed on the host, one host-to-device copy, one init kernel; the
- * iterate is iterate 0 again and top_iteration() restarts at 0.  Asynchronous with respect to the host.
+ * allocated: one host-to-device copy of the caller's arrays, the per-segment operator recomputed by the device kernel
+ * that top_create uses (polytope corridors: on the host, as in top_create), one init kernel; the iterate is iterate 0
+ * again and top_iteration() restarts at 0.  Asynchronous with respect to the host.
  * Errors: TOP_E_INVALID (as top_create, or a different constraint selection), TOP_E_CUDA, TOP_E_NOMEM.
  */
 TOP_API top_status top_reset(top_solver* h, const double* waypoints, const double* durations,

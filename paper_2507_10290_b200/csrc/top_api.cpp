@@ -449,14 +449,6 @@ void spectral_operator(const Spectral& S, int n, bool hard, xreal rho, const xre
         }
 }
 
-template <typename Real>
-void project_ball_host(const double* y, double bound, Real* phi) {
-    const double n2 = y[0] * y[0] + y[1] * y[1] + y[2] * y[2];
-    double sc = 1;
-    if (n2 > bound * bound) sc = bound / std::sqrt(n2);
-    for (int d = 0; d < 3; ++d) phi[d] = (Real)(sc * y[d]);
-}
-
 top_status download_real(top_solver* h, const void* src, std::vector<double>& dst, size_t count) {
     dst.resize(count);
     if (h->dtype == TOP_F64) {
@@ -1303,7 +1295,8 @@ extern "C" TOP_API top_status top_iterate(top_solver* h, int64_t k) {
     return run_sweeps(h, k);
 }
 
-extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iters) {
+namespace { top_status set_rho_impl(top_solver* h, double rho); }
+static top_status solve_impl(top_solver* h, double eps, int64_t* iters) {
     if (!h) return TOP_E_INVALID;
     if (!(eps > 0)) return fail(h, TOP_E_INVALID, "eps must be > 0");
     const double tol = (h->opt_flags & TOP_EPS_N_SCALED) ? eps * h->N : eps;
@@ -1356,14 +1349,15 @@ extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iter
             double rho_new = h->rho;
             if (rp > h->adapt_mu * rd) rho_new = h->rho * h->adapt_incr;
             else if (rd > h->adapt_mu * rp) rho_new = h->rho / h->adapt_decr;
-            if (rho_new != h->rho) { st = top_set_rho(h, rho_new); if (st != TOP_OK) return st; }
+            if (rho_new != h->rho) { st = set_rho_impl(h, rho_new); if (st != TOP_OK) return st; }
         }
     }
     if (iters) for (int b = 0; b < h->batch; ++b) iters[b] = first[b] >= 0 ? first[b] : done;
     return all ? TOP_OK : TOP_NOT_CONVERGED;
 }
 
-extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
+namespace {
+top_status set_rho_impl(top_solver* h, double rho) {
     if (!h) return TOP_E_INVALID;
     if (!(rho > 0) || !std::isfinite(rho)) return fail(h, TOP_E_INVALID, "rho must be finite and > 0");
     if (rho == h->rho) return TOP_OK;
@@ -1373,21 +1367,26 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
         // polytope corridor: three operators per segment; they are rebuilt on the host for the new rho (no spectral form),
         // uploaded, c0^ follows on the device, and the scaled duals (u, w, and v = max(0,-q) of every plane) are rescaled
         const double old = h->rho;
-        h->rho = rho;
-        top_status so = stage_operators(h);
-        if (so != TOP_OK) { h->rho = old; return so; }
-        CU(cudaMemcpyAsync(h->d_upload, h->stage.get(), h->off_wp, cudaMemcpyHostToDevice, h->stream), "H2D operators");
-        InitParams ip;
-        std::memset(&ip, 0, sizeof ip);
-        fill_init_params(h, ip);
-        ip.c0_only = 1;
-        CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
-        RescaleParams r;
-        r.u = h->d_u; r.qp = nullptr; r.qn = nullptr; r.wv = h->d_wv; r.wa = h->d_wa;
-        r.count = 3 * (long long)LS; r.ratio = old / rho; r.qpl = h->d_qpl; r.qpl_count = (long long)h->K * (long long)LS;
-        r.u2 = h->d_u2;      // wide consensus: the scaled duals of the second row block as well (null otherwise)
-        r.yv = r.ya = nullptr; r.y_count = 0;
-        CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
+        h->rho = rho;            // (stage_operators builds for h->rho; put back below if anything fails)
+        auto enqueue = [&]() -> top_status {
+            top_status so = stage_operators(h);
+            if (so != TOP_OK) return so;
+            CU(cudaMemcpyAsync(h->d_upload, h->stage.get(), h->off_wp, cudaMemcpyHostToDevice, h->stream), "H2D operators");
+            InitParams ip;
+            std::memset(&ip, 0, sizeof ip);
+            fill_init_params(h, ip);
+            ip.c0_only = 1;
+            CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
+            RescaleParams r;
+            r.u = h->d_u; r.qp = nullptr; r.qn = nullptr; r.wv = h->d_wv; r.wa = h->d_wa;
+            r.count = 3 * (long long)LS; r.ratio = old / rho; r.qpl = h->d_qpl; r.qpl_count = (long long)h->K * (long long)LS;
+            r.u2 = h->d_u2;      // wide consensus: the scaled duals of the second row block as well (null otherwise)
+            r.yv = r.ya = nullptr; r.y_count = 0;
+            CU(launch_rescale_duals(r, h->dtype, h->stream), "dual rescale launch");
+            return TOP_OK;
+        };
+        const top_status st = enqueue();
+        if (st != TOP_OK) { h->rho = old; return st; }      // the handle keeps reporting the rho its device operator has
         h->launches += 2;
         return TOP_OK;
     }
@@ -1403,6 +1402,7 @@ extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
     h->rho = rho;
     return TOP_OK;
 }
+}  // namespace
 
 extern "C" TOP_API double top_get_rho(const top_solver* h) { return h ? h->rho : std::numeric_limits<double>::quiet_NaN(); }
 
@@ -1438,7 +1438,7 @@ extern "C" TOP_API top_status top_get_coeffs(top_solver* h, void* out, int32_t o
     return TOP_OK;
 }
 
-extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, double* out, size_t count) {
+static top_status get_state_impl(top_solver* h, const char* field, double* out, size_t count) {
     if (!h) return TOP_E_INVALID;
     if (!field || !out) return fail(h, TOP_E_INVALID, "field and out are required");
     const std::string f(field);
@@ -1576,7 +1576,7 @@ extern "C" TOP_API top_status top_snapshot_save(top_solver* h, void* host_buf, s
     return check_abort(h);
 }
 
-extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* host_buf, size_t bytes) {
+static top_status snapshot_restore_impl(top_solver* h, const void* host_buf, size_t bytes) {
     if (!h) return TOP_E_INVALID;
     if (h->numeric) return fail(h, TOP_E_UNSUPPORTED, "snapshots are not built for TOP_XUPDATE_NUMERIC");
     if (!host_buf || bytes != top_snapshot_bytes(h)) return fail(h, TOP_E_INVALID, "top_snapshot_restore: buffer size does not match this solver");
@@ -1596,15 +1596,21 @@ extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* ho
     o += (size_t)h->batch * 4 * 8;
     if (h->has_poly) CU(cudaMemcpyAsync(h->d_qpl, o, (size_t)h->K * (size_t)h->stride * 8, cudaMemcpyHostToDevice, h->stream), "H2D snapshot");
     if (hd.rho != h->rho && h->has_poly) {
-        h->rho = hd.rho;
-        top_status so = stage_operators(h);
-        if (so != TOP_OK) return so;
-        CU(cudaMemcpyAsync(h->d_upload, h->stage.get(), h->off_wp, cudaMemcpyHostToDevice, h->stream), "H2D operators");
-        InitParams ip;
-        std::memset(&ip, 0, sizeof ip);
-        fill_init_params(h, ip);
-        ip.c0_only = 1;
-        CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
+        const double old = h->rho;
+        h->rho = hd.rho;         // (stage_operators builds for h->rho; put back if anything fails)
+        auto enqueue = [&]() -> top_status {
+            top_status so = stage_operators(h);
+            if (so != TOP_OK) return so;
+            CU(cudaMemcpyAsync(h->d_upload, h->stage.get(), h->off_wp, cudaMemcpyHostToDevice, h->stream), "H2D operators");
+            InitParams ip;
+            std::memset(&ip, 0, sizeof ip);
+            fill_init_params(h, ip);
+            ip.c0_only = 1;
+            CU(launch_init(ip, h->dtype, h->stream), "init kernel launch");
+            return TOP_OK;
+        };
+        const top_status so = enqueue();
+        if (so != TOP_OK) { h->rho = old; return so; }
     } else if (hd.rho != h->rho) {
         top_status se = ensure_spectral(h);
         if (se != TOP_OK) return se;
@@ -1731,11 +1737,30 @@ extern "C" TOP_API top_status top_precompute_operator(int32_t s, double T, doubl
     return TOP_OK;
 }
 
+extern "C" TOP_API top_status top_solve(top_solver* h, double eps, int64_t* iters) {
+    if (!h) return TOP_E_INVALID;
+    TOP_GUARDED(h, return solve_impl(h, eps, iters);)
+}
+extern "C" TOP_API top_status top_set_rho(top_solver* h, double rho) {
+    if (!h) return TOP_E_INVALID;
+    TOP_GUARDED(h, return set_rho_impl(h, rho);)
+}
+extern "C" TOP_API top_status top_get_state(top_solver* h, const char* field, double* out, size_t count) {
+    if (!h) return TOP_E_INVALID;
+    TOP_GUARDED(h, return get_state_impl(h, field, out, count);)
+}
+extern "C" TOP_API top_status top_snapshot_restore(top_solver* h, const void* host_buf, size_t bytes) {
+    if (!h) return TOP_E_INVALID;
+    TOP_GUARDED(h, return snapshot_restore_impl(h, host_buf, bytes);)
+}
+
 extern "C" TOP_API top_status top_destroy(top_solver* h) {
     if (!h) return TOP_OK;
     cudaSetDevice(h->device);
     cudaStreamSynchronize(h->stream);
-    if (h->arena) { if (h->arena_pooled) cudaFreeAsync(h->arena, h->stream); else cudaFree(h->arena); }
+    // a pooled arena goes back to the pool in stream order; if that fails (the caller destroyed the stream first, or it is
+    // being captured) cudaFree -- legal for pool allocations, synchronises -- so that the arena is never left allocated
+    if (h->arena && (!h->arena_pooled || cudaFreeAsync(h->arena, h->stream) != cudaSuccess)) { cudaGetLastError(); cudaFree(h->arena); }
     cudaGetLastError();
     delete h;
     return TOP_OK;
