@@ -177,3 +177,64 @@ def test_polytope_wide_set_rho_and_adaptive_solve():
     w2.rho = o2.rho
     compare(sol2, [o2], w2, "adaptive, 60 sweeps")
     sol2.close()
+
+
+@pytest.mark.parametrize("Np,kw,segs", [(5920, {}, 40), (4736, {"consensus": "wide", "mode": "free"}, 32)])
+def test_polytope_full_size_on_the_plan_bench_times(Np, kw, segs):
+    """The two polytope workloads bench.py quotes (config-4 shape, K = 8 planes per segment; N = 5920, and the paper's literal
+    configuration with n_c = 2s-1 and free waypoints at N = 4736) on the planner's own launch: 148 CTAs over the L2 mailbox,
+    5 / 4 octet warps per CTA -- not the <= 16-CTA cluster plan the small cases above run on.  Every field incl. the
+    per-(sample, plane) slack and dual against the long-double oracle's coupled operator, 1e-9."""
+    w = W.polytope_corridor(W.config4(seed=1004, N=Np), K=8, seed=3)
+    sol = top.from_workload(w, **kw)
+    li = sol.launch_info()
+    assert li["waves"] == 1 and li["ctas"] > 16 and li["segs_per_cta"] == segs, li
+    o = poly_oracle(w, long_double=True, **kw)
+    compare(sol, [o], w, "iterate 0")
+    done = 0
+    for cp in (1, 2, 10, 100):
+        sol.iterate(cp - done); o.sweep(cp - done, 0); done = cp
+        compare(sol, [o], w, "N=%d sweep %d" % (Np, cp))
+    sol.close()
+
+
+@pytest.mark.parametrize("sync", ["pairwise", "neighbour", "grid"])
+@pytest.mark.parametrize("kw", [{}, {"consensus": "wide", "mode": "free"}])
+def test_polytope_explicit_sync_modes(sync, kw):
+    """POLY / POLY+WIDE over the L2 mailbox with each inter-CTA synchronisation (the explicit modes never use the cluster)."""
+    w = W.polytope_corridor(W.small_constrained(N=301, s=4, acc=True, seed=31), K=7, seed=9)
+    sol = top.from_workload(w, sync=sync, segs_per_cta=8, **kw)
+    assert sol.launch_info()["ctas"] == 38
+    o = poly_oracle(w, long_double=True, **kw)
+    done = 0
+    for cp in (1, 2, 3, 25, 120):
+        sol.iterate(cp - done); o.sweep(cp - done, 1); done = cp
+        compare(sol, [o], w, "%s sweep %d" % (sync, cp))
+    sol.close()
+
+
+def test_polytope_random_option_sweep():
+    """Seeded random sweep over the polytope options (sizes incl. ragged CTAs, s, K, acc, waypoint mode, consensus width, sync mode,
+    segments per CTA, rho, launch chunking, a change of rho in between) against the long-double oracle."""
+    rng = np.random.default_rng(11)
+    for case in range(30):
+        N = int(rng.choice([1, 2, 5, 9, 17, 33, 64, 129, 300]))
+        s = int(rng.choice([3, 4])); acc = bool(rng.integers(2)); K = int(rng.choice([1, 3, 6, 8, 13, 16]))
+        w = W.polytope_corridor(W.small_constrained(N=N, s=s, acc=acc, seed=int(rng.integers(1 << 30))), K=K, seed=int(rng.integers(1 << 30)))
+        if rng.integers(3) == 0:
+            w.vmax = 0.0
+        w.rho = float(rng.choice([0.3, 1.0, 10.0, 80.0]))
+        mode = str(rng.choice(["hard", "hard", "pinned_z", "free"]))
+        kw = {"consensus": "wide"} if rng.integers(3) == 0 else {}
+        sync = str(rng.choice(["auto", "pairwise", "neighbour", "grid"]))
+        segs = int(rng.choice([0, 4, 8, 16]))
+        sol = top.from_workload(w, mode=mode, sync=sync, segs_per_cta=segs, **kw)
+        o = poly_oracle(w, mode=mode, long_double=True, **kw)
+        ks = [int(k) for k in rng.integers(1, 40, size=3)]
+        for j, k in enumerate(ks):
+            sol.iterate(k); o.sweep(k, 1)
+            compare(sol, [o], w, (case, N, s, acc, K, w.rho, mode, kw, sync, segs, ks, j))
+            if j == 0 and case % 3 == 0:
+                w.rho = w.rho * 1.7
+                sol.set_rho(w.rho); o.set_rho(w.rho)
+        sol.close()
