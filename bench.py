@@ -402,6 +402,10 @@ def main():
                       "segments": w.N, "batch": w.batch, "s": w.s, "rho": w.rho, "sweeps_per_step": sweeps,
                       "l2": "flushed between steps (256 MiB write); state is on-chip during a step",
                       "sync": args.sync, **info, "parallelism": "replicas x%d (no collective)" % world},
+           # compact per-config record (filled below on rank 0 of the default run; kept near the front of the line so that a
+           # truncated copy still carries it): [us per sweep per wave, segment-iterations/s, fraction of the measured FMA
+           # peak, CTAs, threads per CTA, oracle segment-iterations/s on all host cores (null with --no-cpu-baseline)]
+           "per_config": None,
            "clocks": clocks, "gpu_launches": int(gpu_launches), "wall_s": t_wall,
            "us_per_sweep": 1e3 * total_ms / args.steps / sweeps,
            "residuals_after": {k: float(v[0]) for k, v in res.items()}}
@@ -499,7 +503,11 @@ def main():
                 torch.cuda.synchronize()
                 msk = e0.elapsed_time(e1) / 3
                 li = so.launch_info()
+                cpu_o = None
+                if not args.no_cpu_baseline and world == 1:      # the oracle beside every config: all host cores, ~1.5 s each
+                    cpu_o = oracle_rate(wo, 1.5, args.oracle_threads)[0]
                 others[wo.name] = {"segment_iterations_per_s": wo.batch * wo.N * k / (msk * 1e-3), "sweeps": k,
+                                   "cpu_baseline": cpu_o,
                                    "us_per_sweep_per_wave": 1e3 * msk / k / li["waves"], "dtype": wo.dtype,
                                    "ctas": li["ctas"], "threads": li["threads"], "waves": li["waves"],
                                    "roofline": roofline_entry(top, name, wo, li["waves"], msk, k, peaks, sms, sm_mhz)}
@@ -565,6 +573,16 @@ def main():
                              "note": "latency bound: the sweep waits for the segments with the longest inner iteration"}}
             sn.close()
             out["other_workloads"] = others
+            pc = {}
+            for nm, e in others.items():
+                if "us_per_sweep_per_wave" in e and e.get("roofline"):
+                    cb = e.get("cpu_baseline")
+                    pc[nm] = [round(e["us_per_sweep_per_wave"], 4), float("%.4g" % e["segment_iterations_per_s"]),
+                              round(e["roofline"]["frac"], 4), e.get("ctas"), e.get("threads"),
+                              None if not cb else float("%.4g" % cb["value"])]
+            pc[w.name] = [round(out["us_per_sweep"], 4), float("%.4g" % value), round(out.get("roofline", {}).get("frac", 0.0), 4), info["ctas"],
+                          info["threads"], None]
+            out["per_config"] = pc
             # ---- the paper's own regime (Tables I-II): tolerance ||r|| < N*0.05 on config 2, fixed rho
             # vs adaptive rho (Eq. 24, rho0 = 1, updated every sweep as in Alg. 1 line 14)
             w2 = make_workload("cfg2", rank)
@@ -617,6 +635,8 @@ def main():
                 out["time_to_eps_cfg2"] = entry
         if not args.no_cpu_baseline and world == 1:
             out["cpu_baseline"] = cpu_baseline_both(w, args.oracle_seconds, args.oracle_threads)
+            if out.get("per_config") and w.name in out["per_config"]:
+                out["per_config"][w.name][5] = float("%.4g" % out["cpu_baseline"]["value"])
         print(json.dumps(out))
     sol.close()
     if world > 1:
