@@ -148,3 +148,19 @@ def test_numeric_unsupported():
         top.from_workload(w, dtype="f64", numeric=True).snapshot()
     with pytest.raises(top.TopError):
         top.from_workload(w, dtype="f64").inner_iterations()
+
+
+def test_numeric_random_option_sweep():
+    """Seeded random draws over the NumericSolve options (N incl. 1 and sizes that span several CTAs, s, box / ball subsets, waypoint
+    mode, rho, batch) against the oracle's numeric branch, at the derived 1e-6 bar, over the first sweeps."""
+    rng = np.random.default_rng(29)
+    for case in range(12):
+        N = int(rng.choice([1, 2, 5, 17, 64, 129, 300])); s = int(rng.choice([3, 4])); acc = bool(rng.integers(2))
+        batch = int(rng.choice([1, 1, 2]))
+        w = W.small_constrained(N=N, s=s, acc=acc, batch=batch, seed=int(rng.integers(1 << 30)))
+        if rng.integers(4) == 0:
+            w.box_lo, w.box_hi = None, None
+        w.rho = float(rng.choice([1.0, 10.0, 80.0]))
+        mode = str(rng.choice(["hard", "hard", "pinned_z", "free"]))
+        cps = sorted(set(int(k) for k in rng.integers(1, 25, size=3)))
+        run(w, cps, mode=mode)[0].close()
